@@ -1,0 +1,159 @@
+"""CPU oracle for the Linac hot path -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+ctypes/numpy wrappers over `oracle/linac_oracle.c` (plain C, `%` arithmetic, the paper's
+one-column-at-a-time Gauss-Jordan loop; citations are in the C file's header).  Only
+`tests/`, `__graft_entry__.smoke()` and `bench.py`'s `cpu_baseline` / `--impl reference`
+legs may import this package; nothing under `paper_2605_25863_b200/` does, and this package
+imports nothing from there.
+
+Pins (tests/test_oracle_*.py, `-m "not gpu"`): every function here is pinned against
+something other than itself -- brute force over tiny fields, Leibniz determinants, closed
+forms (Vandermonde), Python big-int arithmetic, sympy's GF(p) RREF as a black box, LAPACK
+for fp64.  No function is "parity unpinned".
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+PIVOT_FIRST, PIVOT_LAST, PIVOT_MAX = 0, 1, 2
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(path)
+        u32p, i32p, i64p, f64p = (C.POINTER(C.c_uint32), C.POINTER(C.c_int32), C.POINTER(C.c_int64),
+                                  C.POINTER(C.c_double))
+        L.oracle_inv_modp.restype = C.c_uint32
+        L.oracle_inv_modp.argtypes = [C.c_uint32, C.c_uint32]
+        L.oracle_pow_modp.restype = C.c_uint32
+        L.oracle_pow_modp.argtypes = [C.c_uint32, C.c_uint64, C.c_uint32]
+        L.oracle_max_threads.restype = C.c_int
+        L.oracle_rref_modp.restype = C.c_int
+        L.oracle_rref_modp.argtypes = [u32p, C.c_int64, C.c_int64, C.c_int64, C.c_uint32, C.c_int, C.c_int, i64p, i32p]
+        L.oracle_det_modp.restype = C.c_int
+        L.oracle_det_modp.argtypes = [u32p, C.c_int64, C.c_int64, C.c_uint32, u32p]
+        L.oracle_nullspace_modp.restype = C.c_int
+        L.oracle_nullspace_modp.argtypes = [u32p, C.c_int64, C.c_int64, C.c_int64, C.c_uint32, C.c_int64, i32p, u32p,
+                                            C.c_int64]
+        L.oracle_matmul_modp.restype = C.c_int
+        L.oracle_matmul_modp.argtypes = [u32p, C.c_int64, u32p, C.c_int64, u32p, C.c_int64, C.c_int64, C.c_int64,
+                                         C.c_int64, C.c_uint32, C.c_int]
+        L.oracle_solve_f64.restype = C.c_int
+        L.oracle_solve_f64.argtypes = [f64p, C.c_int64, C.c_int64, f64p, C.c_int64, C.c_int64, C.c_double, C.c_int, i64p]
+        L.oracle_backward_error.restype = C.c_double
+        L.oracle_backward_error.argtypes = [f64p, C.c_int64, C.c_int64, f64p, C.c_int64, f64p, C.c_int64, C.c_int64,
+                                            C.c_int]
+        _lib = L
+    return _lib
+
+
+def _u32(a):
+    return a.ctypes.data_as(C.POINTER(C.c_uint32))
+
+
+def _f64(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def max_threads() -> int:
+    return int(lib().oracle_max_threads())
+
+
+def inv_modp(a: int, p: int) -> int:
+    return int(lib().oracle_inv_modp(a, p))
+
+
+def pow_modp(a: int, e: int, p: int) -> int:
+    return int(lib().oracle_pow_modp(a, e, p))
+
+
+def rref_modp(a: np.ndarray, p: int, pivot_rule: int = PIVOT_FIRST, nthreads: int = 1, ld: int | None = None):
+    """RREF over F_p of the 2-D uint32 array `a` (not modified).  Returns (R, rank, pivot_cols).
+
+    With `ld` > cols the matrix is embedded in a padded buffer (padding filled with a sentinel)
+    and the test that padding is untouched is left to the caller via the returned full buffer.
+    """
+    a = np.ascontiguousarray(a, dtype=np.uint32)
+    rows, cols = a.shape
+    r = a.copy()
+    rank = C.c_int64(0)
+    piv = np.zeros(max(1, min(rows, cols)), dtype=np.int32)
+    rc = lib().oracle_rref_modp(_u32(r), rows, cols, cols if ld is None else ld, p, pivot_rule, nthreads,
+                                C.byref(rank), piv.ctypes.data_as(C.POINTER(C.c_int32)))
+    if rc != 0:
+        raise ValueError(f"oracle_rref_modp failed: {rc}")
+    return r, int(rank.value), piv[: rank.value].copy()
+
+
+def det_modp(a: np.ndarray, p: int) -> int:
+    a = np.ascontiguousarray(a, dtype=np.uint32).copy()
+    n = a.shape[0]
+    assert a.shape == (n, n)
+    d = C.c_uint32(0)
+    rc = lib().oracle_det_modp(_u32(a), n, n, p, C.byref(d))
+    if rc != 0:
+        raise ValueError(f"oracle_det_modp failed: {rc}")
+    return int(d.value)
+
+
+def nullspace_modp(r: np.ndarray, p: int, rank: int, pivot_cols: np.ndarray) -> np.ndarray:
+    """Canonical kernel basis K (cols x (cols-rank)) from an RREF `r`."""
+    r = np.ascontiguousarray(r, dtype=np.uint32)
+    rows, cols = r.shape
+    d = cols - rank
+    k = np.zeros((cols, max(d, 0)), dtype=np.uint32)
+    piv = np.ascontiguousarray(pivot_cols, dtype=np.int32)
+    if piv.size == 0:
+        piv = np.zeros(1, dtype=np.int32)
+    kbuf = k if d > 0 else np.zeros((max(cols, 1), 1), dtype=np.uint32)
+    rc = lib().oracle_nullspace_modp(_u32(r), rows, cols, cols, p, rank, piv.ctypes.data_as(C.POINTER(C.c_int32)),
+                                     _u32(kbuf), max(d, 1) if d == 0 else d)
+    if rc != 0:
+        raise ValueError(f"oracle_nullspace_modp failed: {rc}")
+    return k
+
+
+def matmul_modp(a: np.ndarray, b: np.ndarray, p: int, nthreads: int = 1) -> np.ndarray:
+    a = np.ascontiguousarray(a, dtype=np.uint32)
+    b = np.ascontiguousarray(b, dtype=np.uint32)
+    m, k = a.shape
+    k2, n = b.shape
+    assert k == k2
+    c = np.zeros((m, n), dtype=np.uint32)
+    if m and n:
+        lib().oracle_matmul_modp(_u32(a), max(k, 1), _u32(b), max(n, 1), _u32(c), max(n, 1), m, k, n, p, nthreads)
+    return c
+
+
+def solve_f64(a: np.ndarray, b: np.ndarray, tol: float = -1.0, nthreads: int = 1):
+    """Row-scaled partial-pivot Gauss-Jordan solve.  Returns (status, info, X); inputs untouched."""
+    a = np.ascontiguousarray(a, dtype=np.float64).copy()
+    b2 = np.ascontiguousarray(b, dtype=np.float64)
+    x = (b2.reshape(-1, 1) if b2.ndim == 1 else b2).copy()
+    n = a.shape[0]
+    info = C.c_int64(0)
+    rc = lib().oracle_solve_f64(_f64(a), n, n, _f64(x), x.shape[1], x.shape[1], tol, nthreads, C.byref(info))
+    if rc < 0:
+        raise ValueError("oracle_solve_f64: bad arguments")
+    return rc, int(info.value), (x.reshape(b2.shape) if rc == 0 else None)
+
+
+def backward_error(a0: np.ndarray, x: np.ndarray, b0: np.ndarray, nthreads: int = 1) -> float:
+    a0 = np.ascontiguousarray(a0, dtype=np.float64)
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    b0 = np.ascontiguousarray(b0, dtype=np.float64)
+    if x.ndim == 1:
+        x = x.reshape(-1, 1)
+        b0 = b0.reshape(-1, 1)
+    n = a0.shape[0]
+    return float(lib().oracle_backward_error(_f64(a0), n, n, _f64(x), x.shape[1], _f64(b0), b0.shape[1],
+                                             x.shape[1], nthreads))
