@@ -1,0 +1,141 @@
+/*
+ * linac.h -- C ABI of the B200-native Linac hot path (arxiv/paper_2605_25863).
+ *
+ * Dense Gaussian elimination to REDUCED row-echelon form over a 32-bit prime field F_p
+ * (uint32 storage, 2 <= p < 2^31), canonical null-space basis, and an fp64 partial-pivot solve.
+ * Citations "PAPER.md:<line>" refer to the paper text this library was written from.
+ *
+ * Conventions (all entry points)
+ *   - extern "C", plain pointers and sizes; no exceptions cross the boundary.
+ *   - Every function returns a linac_status (int).  Outputs are defined only on LINAC_OK,
+ *     except where a function documents otherwise.
+ *   - "device" pointers must be device memory of the CURRENT CUDA device (compute capability
+ *     10.x; anything else -> LINAC_ERR_UNSUPPORTED_DEVICE: there is no fallback path).
+ *     "host" pointers are ordinary host memory.
+ *   - Ownership: the library never frees or keeps caller memory.  Matrices, K and the optional
+ *     workspace are caller-allocated.  `stream` is the caller's CUDA stream (cudaStream_t passed
+ *     as void*; NULL = default stream).  Calls enqueue their work on `stream` and SYNCHRONISE it
+ *     before returning (rank / pivots are host outputs).
+ *   - Matrices are row-major with a leading dimension in ELEMENTS (ld >= cols).  Columns
+ *     cols..ld-1 are never read as data and never written (the paper pads rows the same way,
+ *     PAPER.md:227).
+ *   - Workspace: if linac_set_workspace() gave the library a buffer at least as large as the
+ *     *_workspace() query, it is used; otherwise the library allocates (and caches) its own with
+ *     cudaMalloc and linac_release() frees it.  One call at a time per process (the workspace
+ *     and the internal state are global); calls are serialised by an internal mutex.
+ */
+#ifndef LINAC_H_
+#define LINAC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    LINAC_OK = 0,
+    LINAC_ERR_INVALID_ARG = 1,        /* null matrix with non-empty shape, negative size, ld < cols, cols >= 2^31 */
+    LINAC_ERR_BAD_MODULUS = 2,        /* p < 2, p >= 2^31, or p composite (deterministic Miller-Rabin on the host) */
+    LINAC_ERR_WORKSPACE = 3,          /* workspace allocation failed */
+    LINAC_ERR_CUDA = 4,               /* a CUDA call failed; linac_last_cuda_error() has the text */
+    LINAC_ERR_SINGULAR = 5,           /* fp64: pivot with |pivot| <= tol */
+    LINAC_ERR_BUFFER_TOO_SMALL = 6,   /* K buffer has fewer columns than the nullity */
+    LINAC_ERR_UNSUPPORTED_DEVICE = 7, /* current device is not sm_100 class */
+    LINAC_ERR_INTERNAL = 8            /* an internal consistency check failed (a bug; never a data property) */
+} linac_status;
+
+/* Static strings; never NULL. */
+const char *linac_status_string(int status);
+const char *linac_last_cuda_error(void);
+/* major*10000 + minor*100 + patch */
+int linac_version(void);
+
+/* ---- workspace ------------------------------------------------------------------------- */
+/* Bytes of device workspace linac_rref_u32 / linac_nullspace_u32 want for this shape (host out). */
+int linac_rref_u32_workspace(int64_t rows, int64_t cols, size_t *bytes);
+/* Bytes of device workspace linac_solve_f64 wants. */
+int linac_solve_f64_workspace(int64_t n, int64_t nrhs, size_t *bytes);
+/* Hand the library a device buffer to use as workspace (NULL, 0 to take it back).  The buffer
+ * stays the caller's; it must outlive the calls that use it. */
+int linac_set_workspace(void *dev_ptr, size_t bytes);
+/* Free library-owned workspace and cached state (idempotent). */
+int linac_release(void);
+
+/* ---- F_p: reduced row-echelon form ------------------------------------------------------- */
+/*
+ * linac_rref_u32 -- the operation of cuda_row_reduce(matrix, field_characteristic=p)
+ * (PAPER.md:147-155): in place, dA (DEVICE, rows x cols, ld) becomes THE reduced row-echelon
+ * form of A over F_p: non-zero rows first, each with leading entry 1, pivot columns strictly
+ * increasing, a pivot the only non-zero of its column, zero rows at the bottom,
+ * entries canonical in [0,p).  Row permutations only (partial pivoting); any shape
+ * (PAPER.md:73, 239).  Input entries >= p are first reduced mod p.
+ *   rank            HOST out: number of non-zero rows.
+ *   pivot_cols_out  HOST out, capacity min(rows, cols) int32, ascending; may be NULL.
+ * rows == 0 or cols == 0 is legal: rank 0, nothing touched.
+ * The schedule is NOT the paper's per-column kernel sequence: it is a blocked
+ * right-looking elimination (panel factorisation + Schur update A22 -= L21.U12 mod p) followed by
+ * back-elimination of the free columns; the result is identical because the RREF is unique.
+ */
+int linac_rref_u32(uint32_t *dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, void *stream,
+                   int64_t *rank, int32_t *pivot_cols_out);
+
+/* ---- F_p: canonical null-space basis ------------------------------------------------------- */
+/*
+ * linac_nullspace_u32 -- reduces dA in place exactly as linac_rref_u32, then writes the canonical
+ * kernel basis of PAPER.md:403-415 (eq. 8-9) to dK (DEVICE, row-major, cols x nullity, ldk):
+ * with free (non-pivot) columns f_0 < ... < f_{d-1}, d = nullity = cols - rank, column t has
+ *   K[f_t, t] = p - 1 ("fixes their coefficients to minus the identity"),
+ *   K[c_k, t] = R[k, f_t] for each pivot row k with pivot column c_k,   0 elsewhere,
+ * so that A.K = 0 mod p (eq. 9).
+ *   nullity          HOST out, always set when the reduction succeeded.
+ *   k_capacity_cols  columns available in dK.  If < nullity: returns LINAC_ERR_BUFFER_TOO_SMALL,
+ *                    nullity, rank and pivots are valid, dA holds the RREF, dK is untouched; the
+ *                    caller may then call linac_nullspace_from_rref_u32.
+ * dK may be NULL iff k_capacity_cols == 0.
+ */
+int linac_nullspace_u32(uint32_t *dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, void *stream,
+                        int64_t *rank, int32_t *pivot_cols_out, uint32_t *dK, int64_t ldk,
+                        int64_t k_capacity_cols, int64_t *nullity);
+
+/* Kernel basis from an RREF already on the device.  pivot_cols: HOST, `rank` ascending entries. */
+int linac_nullspace_from_rref_u32(const uint32_t *dR, int64_t rows, int64_t cols, int64_t ld, uint32_t p,
+                                  int64_t rank, const int32_t *pivot_cols, uint32_t *dK, int64_t ldk,
+                                  void *stream);
+
+/* ---- fp64: partial-pivot solve ------------------------------------------------------------- */
+/*
+ * linac_solve_f64 -- solves A X = B (eq. 10-12) in floating point:
+ * row equilibration s_r = max_c |A[r,c]|, A[r,:] /= s_r, B[r,:] /= s_r (CudaSetRowScales /
+ * CudaRescaleRows), then Gaussian elimination with partial pivoting on the
+ * column maximum and triangular solves for the right-hand sides.
+ *   dA  DEVICE n x n (lda), overwritten by the factors.   dB  DEVICE n x nrhs (ldb), overwritten by X.
+ *   tol threshold below which a pivot of the row-scaled matrix counts as zero;
+ *       tol < 0 selects n * 2^-52.
+ *   info HOST out: 0, or the 1-based column of the first pivot with |pivot| <= tol
+ *       (then the return value is LINAC_ERR_SINGULAR and dA/dB are undefined).
+ */
+int linac_solve_f64(double *dA, int64_t n, int64_t lda, double *dB, int64_t nrhs, int64_t ldb, double tol,
+                    void *stream, int64_t *info);
+
+/* ---- instrumentation (host-side counters of the LAST F_p call; for tests and bench.py) ------ */
+typedef struct {
+    int64_t kernel_launches;     /* kernels this library launched                                 */
+    int64_t host_syncs;          /* stream synchronisations inside the call                       */
+    int64_t panels;              /* base panels factored                                          */
+    int64_t row_swaps;           /* row exchanges performed                                       */
+    int64_t update_macs;         /* field multiply-accumulates executed by Schur/TRSM updates     */
+    int64_t residual_nonzero;    /* internal check: must be 0                                     */
+    double  ms_update;           /* device ms spent in the Schur-update (GEMM) kernels, if timed  */
+    double  ms_total;            /* device ms of the whole call, if timed                         */
+} linac_stats;
+int linac_get_last_stats(linac_stats *out);
+/* Tunables, mainly for A/B measurements: name in {"gemm_path" (0 auto, 1 CUDA-core, 2 tensor), "timing" (0/1), "tc_min_k", "tc_min_mn"}.
+ * Returns LINAC_ERR_INVALID_ARG for unknown names / out-of-range values. */
+int linac_set_option(const char *name, int64_t value);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LINAC_H_ */

@@ -1,0 +1,174 @@
+// linac_common.cu -- library state, error plumbing, workspace, host number theory.
+#include <cstring>
+#include <mutex>
+#include <string>
+
+#include "linac_internal.h"
+
+namespace linac {
+
+static std::string g_cuda_error = "";
+static Options g_options;
+static linac_stats g_stats;
+static void* g_user_ws = nullptr;
+static size_t g_user_ws_bytes = 0;
+static void* g_own_ws = nullptr;
+static size_t g_own_ws_bytes = 0;
+std::mutex g_call_mutex;
+
+void set_cuda_error(cudaError_t e, const char* what, const char* file, int line) {
+    char buf[1024];
+    snprintf(buf, sizeof buf, "%s (%s) at %s:%d: %s", cudaGetErrorName(e), cudaGetErrorString(e), file, line, what);
+    g_cuda_error = buf;
+    cudaGetLastError();   // clear the sticky-less error so the next call starts clean
+}
+
+Options& options() { return g_options; }
+linac_stats& stats() { return g_stats; }
+
+int acquire_workspace(size_t bytes, Arena* arena) {
+    if (g_user_ws && g_user_ws_bytes >= bytes) {
+        arena->base = (char*)g_user_ws;
+        arena->size = g_user_ws_bytes;
+        arena->off = 0;
+        return LINAC_OK;
+    }
+    if (g_own_ws_bytes < bytes) {
+        if (g_own_ws) cudaFree(g_own_ws);
+        g_own_ws = nullptr;
+        g_own_ws_bytes = 0;
+        cudaError_t e = cudaMalloc(&g_own_ws, bytes);
+        if (e != cudaSuccess) {
+            set_cuda_error(e, "cudaMalloc(workspace)", __FILE__, __LINE__);
+            return LINAC_ERR_WORKSPACE;
+        }
+        g_own_ws_bytes = bytes;
+    }
+    arena->base = (char*)g_own_ws;
+    arena->size = g_own_ws_bytes;
+    arena->off = 0;
+    return LINAC_OK;
+}
+
+static uint64_t mulmod_u64(uint64_t a, uint64_t b, uint64_t m) { return (unsigned __int128)a * b % m; }
+static uint64_t powmod_u64(uint64_t a, uint64_t e, uint64_t m) {
+    uint64_t r = 1 % m;
+    a %= m;
+    while (e) {
+        if (e & 1) r = mulmod_u64(r, a, m);
+        a = mulmod_u64(a, a, m);
+        e >>= 1;
+    }
+    return r;
+}
+
+// Deterministic Miller-Rabin: bases {2,3,5,7} decide every n < 3,215,031,751.
+bool is_prime_u32(uint32_t n) {
+    if (n < 2) return false;
+    for (uint32_t q : {2u, 3u, 5u, 7u, 11u, 13u}) {
+        if (n == q) return true;
+        if (n % q == 0) return false;
+    }
+    uint32_t d = n - 1;
+    int s = 0;
+    while ((d & 1) == 0) { d >>= 1; ++s; }
+    for (uint64_t a : {2ull, 3ull, 5ull, 7ull}) {
+        uint64_t x = powmod_u64(a, d, n);
+        if (x == 1 || x == n - 1) continue;
+        bool comp = true;
+        for (int i = 1; i < s; ++i) {
+            x = mulmod_u64(x, x, n);
+            if (x == n - 1) { comp = false; break; }
+        }
+        if (comp) return false;
+    }
+    return true;
+}
+
+ModP make_modp(uint32_t p) {
+    ModP f;
+    f.p = p;
+    f.c32 = (uint32_t)((1ull << 32) % p);
+    f.m64 = (uint64_t)((((unsigned __int128)1) << 64) / p);
+    for (int k = 0; k < 7; ++k) f.w[k] = (uint32_t)powmod_u64(2, 8 * k, p);
+    return f;
+}
+
+int check_device() {
+    int dev = 0;
+    LINAC_CUDA(cudaGetDevice(&dev));
+    int major = 0;
+    LINAC_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10) return LINAC_ERR_UNSUPPORTED_DEVICE;
+    return LINAC_OK;
+}
+
+}  // namespace linac
+
+using namespace linac;
+
+extern "C" {
+
+const char* linac_status_string(int status) {
+    switch (status) {
+        case LINAC_OK: return "ok";
+        case LINAC_ERR_INVALID_ARG: return "invalid argument";
+        case LINAC_ERR_BAD_MODULUS: return "modulus must be a prime with 2 <= p < 2^31";
+        case LINAC_ERR_WORKSPACE: return "workspace allocation failed";
+        case LINAC_ERR_CUDA: return "CUDA error";
+        case LINAC_ERR_SINGULAR: return "matrix is singular to the given tolerance";
+        case LINAC_ERR_BUFFER_TOO_SMALL: return "null-space buffer has too few columns";
+        case LINAC_ERR_UNSUPPORTED_DEVICE: return "current CUDA device is not compute capability 10.x";
+        case LINAC_ERR_INTERNAL: return "internal consistency check failed";
+        default: return "unknown status";
+    }
+}
+
+const char* linac_last_cuda_error(void) { return g_cuda_error.c_str(); }
+
+int linac_version(void) { return 100; }   // 0.1.0
+
+int linac_set_workspace(void* dev_ptr, size_t bytes) {
+    std::lock_guard<std::mutex> lock(g_call_mutex);
+    if ((dev_ptr == nullptr) != (bytes == 0)) return LINAC_ERR_INVALID_ARG;
+    g_user_ws = dev_ptr;
+    g_user_ws_bytes = bytes;
+    return LINAC_OK;
+}
+
+int linac_release(void) {
+    std::lock_guard<std::mutex> lock(g_call_mutex);
+    if (g_own_ws) cudaFree(g_own_ws);
+    g_own_ws = nullptr;
+    g_own_ws_bytes = 0;
+    return LINAC_OK;
+}
+
+int linac_get_last_stats(linac_stats* out) {
+    if (!out) return LINAC_ERR_INVALID_ARG;
+    *out = g_stats;
+    return LINAC_OK;
+}
+
+int linac_set_option(const char* name, int64_t value) {
+    if (!name) return LINAC_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_call_mutex);
+    if (!strcmp(name, "gemm_path")) {
+        if (value < 0 || value > 2) return LINAC_ERR_INVALID_ARG;
+        g_options.gemm_path = value;
+    } else if (!strcmp(name, "timing")) {
+        if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
+        g_options.timing = value;
+    } else if (!strcmp(name, "tc_min_k")) {
+        if (value < 32) return LINAC_ERR_INVALID_ARG;
+        g_options.tc_min_k = value;
+    } else if (!strcmp(name, "tc_min_mn")) {
+        if (value < 128) return LINAC_ERR_INVALID_ARG;
+        g_options.tc_min_mn = value;
+    } else {
+        return LINAC_ERR_INVALID_ARG;
+    }
+    return LINAC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,79 @@
+// linac_internal.h -- shared host-side declarations of the library (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <cstdio>
+
+#include "../../include/linac.h"
+#include "modp.cuh"
+
+namespace linac {
+
+constexpr int PW = 32;   // base panel width (columns factored by one panel kernel)
+constexpr int CH = 64;   // rows per chunk scanned by the pivot kernel
+
+// What the pivot kernel reports for one base panel (device -> pinned host, one small copy).
+struct PanelInfo {
+    int32_t r;               // pivots found in this panel (<= width)
+    int32_t nswaps;          // how many of swp[] are real exchanges
+    int32_t pc[PW];          // local pivot columns, ascending
+    int64_t swp[PW];         // LAPACK-style: at step a exchange rows (i0+a) and swp[a] (>= i0+a)
+    int32_t residual;        // internal check, must stay 0
+    int32_t pad;
+};
+
+// Error plumbing: first failing CUDA call wins; text kept for linac_last_cuda_error().
+void set_cuda_error(cudaError_t e, const char* what, const char* file, int line);
+#define LINAC_CUDA(call)                                                     \
+    do {                                                                     \
+        cudaError_t e__ = (call);                                            \
+        if (e__ != cudaSuccess) {                                            \
+            ::linac::set_cuda_error(e__, #call, __FILE__, __LINE__);         \
+            return LINAC_ERR_CUDA;                                           \
+        }                                                                    \
+    } while (0)
+
+// Global, mutex-protected library state (workspace, options, stats).
+struct Options {
+    int64_t gemm_path = 0;    // 0 = auto, 1 = CUDA-core (SIMT) only, 2 = tensor (tcgen05) where legal
+    int64_t timing = 0;       // 1 = bracket update kernels with events (costs syncs; for profiling runs)
+    int64_t tc_min_k = 256;   // smallest K the tensor path is used for
+    int64_t tc_min_mn = 512;  // smallest M and N the tensor path is used for
+};
+Options& options();
+linac_stats& stats();
+
+// Workspace arena: bump allocation inside either the caller's buffer or a library-owned one.
+struct Arena {
+    char* base = nullptr;
+    size_t size = 0, off = 0;
+    void* take(size_t bytes, size_t align = 256) {
+        size_t o = (off + align - 1) / align * align;
+        if (o + bytes > size) return nullptr;
+        off = o + bytes;
+        return base + o;
+    }
+};
+int acquire_workspace(size_t bytes, Arena* arena);   // returns linac_status
+
+ModP make_modp(uint32_t p);
+bool is_prime_u32(uint32_t p);
+int check_device();                                    // LINAC_OK or UNSUPPORTED_DEVICE / CUDA
+
+// ---- F_p GEMM  C -= Aop . B  (mod p) ------------------------------------------------------------
+// C: M x N (ldc).  B: K x N (ldb).  Aop: M x K gathered from `Abase` (lda): element (m,k) is
+// Abase[m*lda + kcols[k]] if kcols != nullptr (device array), else Abase[m*lda + k].
+struct GemmArgs {
+    uint32_t* C; int64_t ldc;
+    const uint32_t* Abase; int64_t lda; const int32_t* kcols;
+    const uint32_t* B; int64_t ldb;
+    int64_t M, N, K;
+};
+int gemm_modp_simt(const GemmArgs& g, const ModP& f, cudaStream_t s);
+// Tensor-core (tcgen05 int8 limb) path; returns LINAC_OK if it ran, or a negative value if the
+// shape/alignment is not supported (caller falls back to the SIMT kernel).
+int gemm_modp_tc(const GemmArgs& g, const ModP& f, cudaStream_t s, Arena* scratch);
+size_t gemm_modp_tc_scratch_bytes(int64_t M, int64_t N, int64_t K);
+
+}  // namespace linac

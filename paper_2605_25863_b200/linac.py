@@ -1,0 +1,222 @@
+"""Thin Python binding of the C ABI in include/linac.h (ctypes; argument marshalling only).
+
+PyTorch is used for device memory and streams, nothing else: every step of the path runs in the
+library's CUDA kernels.  There is NO CPU fallback -- importing this module on a box where
+`liblinac.so` cannot be loaded, or calling it without a CUDA device, raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblinac.so")
+
+OK, ERR_INVALID_ARG, ERR_BAD_MODULUS, ERR_WORKSPACE, ERR_CUDA = 0, 1, 2, 3, 4
+ERR_SINGULAR, ERR_BUFFER_TOO_SMALL, ERR_UNSUPPORTED_DEVICE, ERR_INTERNAL = 5, 6, 7, 8
+
+#: every symbol include/linac.h declares (checked by tests/test_abi.py)
+SYMBOLS = [
+    "linac_status_string", "linac_last_cuda_error", "linac_version",
+    "linac_rref_u32_workspace", "linac_solve_f64_workspace", "linac_set_workspace", "linac_release",
+    "linac_rref_u32", "linac_nullspace_u32", "linac_nullspace_from_rref_u32", "linac_solve_f64",
+    "linac_get_last_stats", "linac_set_option",
+]
+
+
+class LinacError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = _lib().linac_status_string(status).decode()
+        if status == ERR_CUDA:
+            msg += ": " + _lib().linac_last_cuda_error().decode()
+        super().__init__(f"{where}: {msg} (status {status})")
+
+
+class Stats(C.Structure):
+    _fields_ = [("kernel_launches", C.c_int64), ("host_syncs", C.c_int64), ("panels", C.c_int64),
+                ("row_swaps", C.c_int64), ("update_macs", C.c_int64), ("residual_nonzero", C.c_int64),
+                ("ms_update", C.c_double), ("ms_total", C.c_double)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+_LIB = None
+
+
+def _lib() -> C.CDLL:
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2605_25863_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i64, u32, sz = C.c_void_p, C.c_int64, C.c_uint32, C.c_size_t
+        L.linac_status_string.restype = C.c_char_p
+        L.linac_status_string.argtypes = [C.c_int]
+        L.linac_last_cuda_error.restype = C.c_char_p
+        L.linac_version.restype = C.c_int
+        L.linac_rref_u32_workspace.argtypes = [i64, i64, C.POINTER(sz)]
+        L.linac_solve_f64_workspace.argtypes = [i64, i64, C.POINTER(sz)]
+        L.linac_set_workspace.argtypes = [vp, sz]
+        L.linac_rref_u32.argtypes = [vp, i64, i64, i64, u32, vp, C.POINTER(i64), vp]
+        L.linac_nullspace_u32.argtypes = [vp, i64, i64, i64, u32, vp, C.POINTER(i64), vp, vp, i64, i64, C.POINTER(i64)]
+        L.linac_nullspace_from_rref_u32.argtypes = [vp, i64, i64, i64, u32, i64, vp, vp, i64, vp]
+        L.linac_solve_f64.argtypes = [vp, i64, i64, vp, i64, i64, C.c_double, vp, C.POINTER(i64)]
+        L.linac_get_last_stats.argtypes = [C.POINTER(Stats)]
+        L.linac_set_option.argtypes = [C.c_char_p, i64]
+        _LIB = L
+    return _LIB
+
+
+def version() -> int:
+    return int(_lib().linac_version())
+
+
+def set_option(name: str, value: int) -> None:
+    rc = _lib().linac_set_option(name.encode(), int(value))
+    if rc:
+        raise LinacError(rc, f"linac_set_option({name})")
+
+
+def last_stats() -> dict:
+    s = Stats()
+    _lib().linac_get_last_stats(C.byref(s))
+    return s.as_dict()
+
+
+_ws_tensor = None
+
+
+def _ensure_workspace(nbytes: int, device) -> None:
+    """Workspace is a torch allocation handed to the library (the caller owns device memory)."""
+    global _ws_tensor
+    if nbytes == 0:
+        return
+    if _ws_tensor is None or _ws_tensor.numel() < nbytes or _ws_tensor.device != device:
+        _lib().linac_set_workspace(None, 0)
+        _ws_tensor = None
+        _ws_tensor = torch.empty(nbytes, dtype=torch.uint8, device=device)
+        rc = _lib().linac_set_workspace(_ws_tensor.data_ptr(), _ws_tensor.numel())
+        if rc:
+            raise LinacError(rc, "linac_set_workspace")
+
+
+def release_workspace() -> None:
+    global _ws_tensor
+    _lib().linac_set_workspace(None, 0)
+    _lib().linac_release()
+    _ws_tensor = None
+
+
+def _check_matrix(t: torch.Tensor, dtypes, what: str):
+    if not t.is_cuda:
+        raise ValueError(f"{what} must be a CUDA tensor (there is no CPU path)")
+    if t.dtype not in dtypes:
+        raise TypeError(f"{what}: dtype {t.dtype} not in {dtypes}")
+    if t.dim() != 2 or (t.numel() and t.stride(1) != 1):
+        raise ValueError(f"{what} must be 2-D with unit column stride")
+    ld = t.stride(0) if t.shape[0] > 1 else max(t.shape[1], t.stride(0) if t.shape[0] else 0)
+    return t.shape[0], t.shape[1], max(ld, t.shape[1])
+
+
+def _stream_ptr(device):
+    return C.c_void_p(torch.cuda.current_stream(device).cuda_stream)
+
+
+_U32 = (torch.uint32, torch.int32)
+
+
+def rref_u32(a: torch.Tensor, p: int):
+    """In place: `a` (CUDA, uint32/int32 storage, rows x cols, row stride = ld) -> its RREF over F_p.
+
+    Returns (rank, pivot_cols) with pivot_cols a host int32 tensor.  Mirrors linac_rref_u32.
+    """
+    rows, cols, ld = _check_matrix(a, _U32, "a")
+    with torch.cuda.device(a.device):
+        need = C.c_size_t(0)
+        _lib().linac_rref_u32_workspace(rows, cols, C.byref(need))
+        _ensure_workspace(need.value, a.device)
+        rank = C.c_int64(0)
+        piv = torch.empty(max(1, min(rows, cols)), dtype=torch.int32)
+        rc = _lib().linac_rref_u32(a.data_ptr(), rows, cols, ld, p, _stream_ptr(a.device), C.byref(rank), piv.data_ptr())
+    if rc:
+        raise LinacError(rc, "linac_rref_u32")
+    return int(rank.value), piv[: rank.value].clone()
+
+
+def nullspace_u32(a: torch.Tensor, p: int, k: torch.Tensor | None = None):
+    """Reduce `a` in place and return (rank, pivot_cols, K) with K = cols x nullity on the device.
+
+    If `k` is given it is used as the output buffer (cols x capacity); too small -> LinacError with
+    status ERR_BUFFER_TOO_SMALL (a then holds the RREF).  If `k` is None the nullity is found first
+    with a capacity-0 call semantics: the RREF is computed once, K allocated, then filled by
+    linac_nullspace_from_rref_u32.
+    """
+    rows, cols, ld = _check_matrix(a, _U32, "a")
+    with torch.cuda.device(a.device):
+        need = C.c_size_t(0)
+        _lib().linac_rref_u32_workspace(rows, cols, C.byref(need))
+        _ensure_workspace(need.value, a.device)
+        rank, nullity = C.c_int64(0), C.c_int64(0)
+        piv = torch.empty(max(1, min(rows, cols)), dtype=torch.int32)
+        if k is not None:
+            krows, kcap, ldk = _check_matrix(k, _U32, "k")
+            if krows != cols:
+                raise ValueError("k must have `cols` rows")
+            rc = _lib().linac_nullspace_u32(a.data_ptr(), rows, cols, ld, p, _stream_ptr(a.device), C.byref(rank),
+                                            piv.data_ptr(), k.data_ptr(), ldk, kcap, C.byref(nullity))
+            if rc:
+                raise LinacError(rc, "linac_nullspace_u32")
+            return int(rank.value), piv[: rank.value].clone(), k[:, : nullity.value]
+        rc = _lib().linac_nullspace_u32(a.data_ptr(), rows, cols, ld, p, _stream_ptr(a.device), C.byref(rank),
+                                        piv.data_ptr(), None, 0, 0, C.byref(nullity))
+        if rc not in (OK, ERR_BUFFER_TOO_SMALL):
+            raise LinacError(rc, "linac_nullspace_u32")
+        d = int(nullity.value)
+        kk = torch.empty((cols, d), dtype=a.dtype, device=a.device)
+        if d:
+            rc = _lib().linac_nullspace_from_rref_u32(a.data_ptr(), rows, cols, ld, p, rank.value, piv.data_ptr(),
+                                                      kk.data_ptr(), d, _stream_ptr(a.device))
+            if rc:
+                raise LinacError(rc, "linac_nullspace_from_rref_u32")
+    return int(rank.value), piv[: rank.value].clone(), kk
+
+
+def nullspace_from_rref_u32(r: torch.Tensor, p: int, rank: int, pivot_cols: torch.Tensor) -> torch.Tensor:
+    rows, cols, ld = _check_matrix(r, _U32, "r")
+    piv = pivot_cols.to(dtype=torch.int32, device="cpu").contiguous()
+    d = cols - rank
+    k = torch.empty((cols, d), dtype=r.dtype, device=r.device)
+    with torch.cuda.device(r.device):
+        rc = _lib().linac_nullspace_from_rref_u32(r.data_ptr(), rows, cols, ld, p, rank, piv.data_ptr(),
+                                                  k.data_ptr() if d else None, max(d, 1), _stream_ptr(r.device))
+    if rc:
+        raise LinacError(rc, "linac_nullspace_from_rref_u32")
+    return k
+
+
+def solve_f64(a: torch.Tensor, b: torch.Tensor, tol: float = -1.0) -> int:
+    """In place: solves a x = b (a: n x n float64 CUDA, overwritten by factors; b: n x nrhs, becomes x).
+
+    Returns info (0).  A singular pivot raises LinacError(status ERR_SINGULAR) with `.info` set.
+    """
+    n, n2, lda = _check_matrix(a, (torch.float64,), "a")
+    nb, nrhs, ldb = _check_matrix(b, (torch.float64,), "b")
+    if n != n2 or nb != n:
+        raise ValueError("a must be n x n and b n x nrhs")
+    with torch.cuda.device(a.device):
+        need = C.c_size_t(0)
+        _lib().linac_solve_f64_workspace(n, nrhs, C.byref(need))
+        _ensure_workspace(need.value, a.device)
+        info = C.c_int64(0)
+        rc = _lib().linac_solve_f64(a.data_ptr(), n, lda, b.data_ptr(), nrhs, ldb, float(tol), _stream_ptr(a.device),
+                                    C.byref(info))
+    if rc:
+        err = LinacError(rc, "linac_solve_f64")
+        err.info = int(info.value)
+        raise err
+    return int(info.value)
