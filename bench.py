@@ -1,0 +1,278 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the Linac hot path on B200 (contract: see DESIGN.md "Measurement").
+
+A "step" is one pass of the whole hot path (S0 ingest .. S7 finalise) over one
+seeded synthetic matrix of the workload BASELINE.json's metric is quoted on: config c3, the
+paper's N = 10^4 point (dense uniform over F_{2^31-1}).  `--workload c2|c5|...`
+selects another config; the default finishes in well under a minute.
+
+  value      : whole-job Gmulmod/s = (2 N^3 / 3) / t, matrix already resident in HBM, t = CUDA-event
+               time of the C-ABI call (max over ranks); N > 1 runs independent replicas (weak).
+  e2e        : same metric with HOST buffers: pinned H2D of the matrix + call + D2H of the RREF.
+  roofline   : the Schur-update kernel (dominant): executed field MACs / its event-timed duration.
+  cpu_baseline: the CPU oracle timed on a bounded sample on this box's host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import linac_inputs as gen  # noqa: E402
+
+PAPER_A100_GMULMOD = {"c3": (2 * 1e4 ** 3 / 3) / 3.6 / 1e9,            # PAPER.md:59  (3.6 s at N = 10^4)
+                      "c5": (2 * 1e5 ** 3 / 3) / (45 * 60) / 1e9}       # PAPER.md:61  (45 min at N = 10^5)
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return dict(hbm_gbs=d["hbm_gbs"], bf16_burst=d["bf16_tflops"], bf16_sustained=d["bf16_tflops_sustained"],
+                    sm_max_mhz=d.get("sm_max_mhz", 1965.0), source="measured")
+    return dict(hbm_gbs=6650.0, bf16_burst=1590.0, bf16_sustained=1400.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._pump, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 7 for i in range(4) if r[3 + i] == "Active"})
+        busy = [x for x in sm if x > 0.6 * (max(mx) if mx else 1)] or sm
+        return {"sm_mhz": float(np.median(busy)) if busy else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def make_workload(name: str, rank_seed: int = 0):
+    """Returns (host uint32 matrix, p, description).  rank_seed shifts the seed for replicas."""
+    c = dict(gen.CONFIGS[name])
+    if c["kind"] == "uniform":
+        a = gen.uniform_matrix(c["rows"], c["cols"], c["p"], c["seed"] + 1000 * rank_seed)  # == replicas.replica_seed
+    elif c["kind"] == "lowrank":
+        a, _, _ = gen.lowrank_factors(c["rows"], c["inner"], c["cols"], c["p"], c["seed_b"] + 1000 * rank_seed, c["seed_c"])
+    elif c["kind"] == "sparse_dep":
+        raise SystemExit("workload c5 is generated on the device: use --workload c5 (handled separately)")
+    else:
+        raise SystemExit(f"workload {name} is not an F_p RREF config")
+    return a, c["p"], c
+
+
+def oracle_sample_gmulmod(n: int, p: int, threads: int):
+    """Times the CPU oracle (as it stands) on an n x n dense uniform matrix; returns (Gmulmod/s, seconds)."""
+    import oracle
+    a = gen.uniform_matrix(n, n, p, seed=4)
+    t0 = time.perf_counter()
+    _, rank, _ = oracle.rref_modp(a, p, nthreads=threads)
+    dt = time.perf_counter() - t0
+    assert rank == n
+    return (2 * n ** 3 / 3) / dt / 1e9, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, a bounded sample of the same workload per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    threads = oracle.max_threads()
+    n = args.ref_n
+    p = gen.CONFIGS[args.workload].get("p", 2147483647)
+    for _ in range(args.warmup):
+        oracle_sample_gmulmod(min(n, 512), p, threads)
+    times = []
+    for _ in range(args.steps):
+        _, dt = oracle_sample_gmulmod(n, p, threads)
+        times.append(dt)
+    t = float(np.mean(times))
+    val = (2 * n ** 3 / 3) / t / 1e9
+    sample = f"{n}x{n} dense uniform F_p sample of workload {args.workload}, CPU oracle Gauss-Jordan"
+    print(json.dumps({
+        "impl": "reference", "metric": "rref_gmulmod_per_s", "value": val, "unit": "Gmulmod/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": {"workload": args.workload, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": "Gmulmod/s", "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "Gmulmod/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3"])
+    ap.add_argument("--ref-n", type=int, default=1280, help="sample size for the oracle legs")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    import paper_2605_25863_b200 as L
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    from paper_2605_25863_b200 import replicas
+    a_host, p, cfg = make_workload(args.workload, rank_seed=rank)      # replicas: one matrix per rank
+    rows, cols = a_host.shape
+    n_nominal = 2.0 * rows * cols * min(rows, cols) / 3.0              # 2N^3/3 for square N
+    pinned = torch.from_numpy(a_host.view(np.int32)).pin_memory()
+    d_in = pinned.to(dev, non_blocking=False)
+    d_work = torch.empty_like(d_in)
+    out_host = torch.empty_like(pinned).pin_memory()
+    stream = torch.cuda.current_stream(dev)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize(dev)
+
+    def step_resident():
+        d_work.copy_(d_in)                        # restore the input: NOT part of the step
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        rank_, _ = L.rref_u32(d_work, p)
+        e1.record(stream)
+        e1.synchronize()
+        return e0.elapsed_time(e1), rank_
+
+    def step_e2e():
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        d_work.copy_(pinned, non_blocking=True)   # H2D of this step's input
+        rank_, piv = L.rref_u32(d_work, p)
+        out_host.copy_(d_work, non_blocking=True)  # D2H of the RREF
+        e1.record(stream)
+        e1.synchronize()
+        return e0.elapsed_time(e1), rank_
+
+    L.set_option("timing", 0)
+    for _ in range(args.warmup):
+        step_resident()
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    times, ranks = [], []
+    for _ in range(args.steps):
+        ms, rk = step_resident()
+        times.append(ms)
+        ranks.append(rk)
+    barrier()
+    clocks = sampler.stop()
+    stats = L.last_stats()
+    total_ms = float(sum(times))
+    total_ms = replicas.max_over_ranks(total_ms, dev)
+    ms_per_step = total_ms / args.steps
+    value = replicas.aggregate_throughput(n_nominal, ms_per_step * 1e-3, world) / 1e9
+
+    # end-to-end leg
+    step_e2e()
+    barrier()
+    e2e_times = [step_e2e()[0] for _ in range(max(2, min(args.steps, 3)))]
+    barrier()
+    e2e_ms = float(np.mean(e2e_times))
+    e2e_ms = replicas.max_over_ranks(e2e_ms, dev)
+    e2e_value = replicas.aggregate_throughput(n_nominal, e2e_ms * 1e-3, world) / 1e9
+
+    # roofline of the dominant kernel family (Schur update), event-timed launch by launch
+    L.set_option("timing", 1)
+    step_resident()
+    step_resident()
+    st_t = L.last_stats()
+    L.set_option("timing", 0)
+    peaks = load_peaks()
+    macs, ms_upd = st_t["update_macs"], st_t["ms_update"]
+    path = st_t.get("gemm_path_used", None)
+    achieved_tmacs = macs / (ms_upd * 1e-3) / 1e12 if ms_upd > 0 else None
+    tensor_used = bool(st_t.get("tc_launches", 0))
+    if tensor_used:
+        # 16 u8xu8 MACs per field MAC on the int8 tensor pipe; int8 dense peak = 2 x measured bf16 (nominal ratio)
+        peak = peaks["bf16_sustained"] * 2.0
+        ach = achieved_tmacs * 16 * 2 if achieved_tmacs else None
+        roof = {"bound": "tensor", "achieved": ach, "peak": peak, "unit": "TOP/s (int8, 2 ops per MAC)",
+                "frac": ach / peak if ach else None, "traffic": None,
+                "note": f"peak = 2 x {peaks['source']} sustained bf16 (guide's nominal int8:bf16 ratio)"}
+    else:
+        # CUDA-core path: one IMAD.WIDE.U32 per field MAC; nominal issue peak 148 SM x 64 lanes x f_max
+        peak = 148 * 64 * peaks["sm_max_mhz"] * 1e6 / 1e12
+        roof = {"bound": "alu", "achieved": achieved_tmacs, "peak": peak, "unit": "T field-MAC/s",
+                "frac": achieved_tmacs / peak if achieved_tmacs else None, "traffic": None,
+                "note": "peak = 148 SM x 64 IMAD lanes x max SM clock (DESIGN.md); "
+                        "achieved = executed update MACs / summed event time of the update kernels"}
+    roof["update_share_of_step"] = ms_upd / st_t["ms_total"] if st_t["ms_total"] else None
+
+    out = {
+        "metric": "rref_gmulmod_per_s", "value": value, "unit": "Gmulmod/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": (value / world / PAPER_A100_GMULMOD[args.workload]) if args.workload in PAPER_A100_GMULMOD else None,
+        "dtype": "u32", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: {rows}x{cols} uint32 dense uniform, p={p}", "rank": int(ranks[-1]),
+                   "parallelism": "replicas" if world > 1 else "single", "l2": "input (%d MB) larger than L2" %
+                   (a_host.nbytes // 2 ** 20) if a_host.nbytes > 126 * 2 ** 20 else "input fits L2; restored by a device copy each step"},
+        "e2e": {"value": e2e_value, "unit": "Gmulmod/s", "ms_per_step": e2e_ms, "h2d_bytes_per_step": int(a_host.nbytes),
+                "d2h_bytes_per_step": int(a_host.nbytes)},
+        "gpu_launches": int(stats["kernel_launches"]) * args.steps,
+        "clocks": clocks, "roofline": roof,
+        "stats": {k: stats[k] for k in ("kernel_launches", "host_syncs", "panels", "row_swaps", "update_macs")},
+        "baseline_context": "paper: A100, 3.6 s at N=1e4 (PAPER.md:59) = 185 Gmulmod/s; another machine, context only",
+    }
+    if rank == 0 and not args.no_cpu_baseline:
+        import oracle
+        threads = oracle.max_threads()
+        v, dt = oracle_sample_gmulmod(args.ref_n, p, threads)
+        out["cpu_baseline"] = {"value": v, "unit": "Gmulmod/s", "cores": threads, "kind": "oracle", "seconds": dt,
+                               "sample": f"{args.ref_n}x{args.ref_n} dense uniform F_p (same recipe as the workload), "
+                                         f"oracle Gauss-Jordan, {threads} OpenMP threads"}
+    if rank == 0:
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

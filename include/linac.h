@@ -127,6 +127,7 @@ typedef struct {
     int64_t row_swaps;           /* row exchanges performed                                       */
     int64_t update_macs;         /* field multiply-accumulates executed by Schur/TRSM updates     */
     int64_t residual_nonzero;    /* internal check: must be 0                                     */
+    int64_t tc_launches;         /* Schur updates that ran on the tensor-core (tcgen05) path      */
     double  ms_update;           /* device ms spent in the Schur-update (GEMM) kernels, if timed  */
     double  ms_total;            /* device ms of the whole call, if timed                         */
 } linac_stats;
