@@ -1,13 +1,487 @@
-// f64_solve.cu -- fp64 partial-pivot solve (placeholder: implemented in a later commit).
+// f64_solve.cu -- linac_solve_f64: row-equilibrated LU with partial pivoting + triangular solves.
+//
+// F1  row scales (CudaSetRowScales / CudaRescaleRows)
+// F2  blocked right-looking LU, partial pivoting on the column maximum:
+//       * 32-column panels factored by ONE cooperative kernel (grid of one CTA per SM, the strip
+//         resident in shared memory, one grid-wide sync per column: warp-shuffle arg-max inside
+//         each CTA, candidates exchanged through global memory)
+//       * row exchanges applied to whole rows of A and B (CudaSwitchRows)
+//       * row-block solves and trailing updates A22 -= L21.U12 as DGEMMs, organised recursively
+//     B rides along as extra trailing columns, which performs the forward substitution
+//     (the paper reduces the augmented matrix (A b)).
+// F3  back substitution with U on the right-hand sides (blocked, GEMM for the off-diagonal part).
+// A pivot with |pivot| <= tol marks the matrix singular (CudaCompareHeadToTolerance).
+#include <cooperative_groups.h>
+
+#include <algorithm>
+#include <climits>
+#include <mutex>
+
 #include "linac_internal.h"
 
-extern "C" {
-int linac_solve_f64_workspace(int64_t n, int64_t nrhs, size_t* bytes) {
-    if (!bytes || n < 0 || nrhs < 0) return LINAC_ERR_INVALID_ARG;
-    *bytes = 0;
+namespace cg = cooperative_groups;
+
+namespace linac {
+extern std::mutex g_call_mutex;
+namespace {
+
+constexpr int FW = 32;              // panel width
+constexpr int FTHREADS = 256;       // panel kernel block size
+
+// ---------------------------------------------------------------- F1
+// One block per row: s = max_c |A[r,c]| over A's columns (reading Q11), then A[r,:] /= s, B[r,:] /= s.
+__global__ void __launch_bounds__(256) row_scale_kernel(double* __restrict__ A, int64_t n, int64_t lda,
+                                                        double* __restrict__ B, int64_t nrhs, int64_t ldb,
+                                                        int* __restrict__ info) {
+    __shared__ double red[8];
+    const int64_t r = blockIdx.x;
+    double* row = A + r * lda;
+    double m = 0.0;
+    for (int64_t c = threadIdx.x; c < n; c += blockDim.x) m = fmax(m, fabs(row[c]));
+    for (int o = 16; o; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+    __syncthreads();
+    m = red[0];
+    for (int w = 1; w < 8; ++w) m = fmax(m, red[w]);
+    if (m == 0.0) {
+        if (threadIdx.x == 0) atomicMin(info, 1);      // a zero row: singular at the very first column
+        return;
+    }
+    for (int64_t c = threadIdx.x; c < n; c += blockDim.x) row[c] = row[c] / m;
+    for (int64_t c = threadIdx.x; c < nrhs; c += blockDim.x) B[r * ldb + c] = B[r * ldb + c] / m;
+}
+
+// ---------------------------------------------------------------- F2 panel
+struct Cand {                 // one CTA's arg-max candidate for a column, with the row's content
+    double absval;
+    long long row;            // absolute row index, -1 if the CTA owns no eligible row
+    double content[FW];
+};
+
+// Cooperative kernel: factors A[j0:n, j0:j0+w) in place (unit-lower L below, U on and above the
+// diagonal), records the exchanges in ipiv[j0..j0+w).  CTA b owns rows [j0 + b*R, j0 + (b+1)*R).
+__global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict__ A, int64_t n, int64_t lda, int64_t j0,
+                                                              int w, int rows_per_cta, double tol,
+                                                              Cand* __restrict__ cand /* [2][gridDim] */,
+                                                              double* __restrict__ target /* [2][FW] */,
+                                                              long long* __restrict__ ipiv, int* __restrict__ info) {
+    extern __shared__ double S[];                       // rows_per_cta x (FW+1)
+    __shared__ double s_val[FTHREADS / 32];
+    __shared__ int s_idx[FTHREADS / 32];
+    __shared__ double pv[FW];
+    __shared__ long long s_g;
+    cg::grid_group grid = cg::this_grid();
+    const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
+    const int G = gridDim.x, b = blockIdx.x;
+    const int64_t r0 = j0 + (int64_t)b * rows_per_cta;
+    const int nr = (int)max((int64_t)0, min((int64_t)rows_per_cta, n - r0));
+    constexpr int LDS = FW + 1;
+
+    for (int k = wq; k < nr; k += FTHREADS / 32) S[k * LDS + lane] = lane < w ? A[(r0 + k) * lda + j0 + lane] : 0.0;
+    __syncthreads();
+
+    // publish the candidate for column c among own rows with absolute index >= j0 + c, and row j0+c itself
+    auto publish = [&](int c) {
+        const int64_t jc = j0 + c;
+        double best = -1.0;
+        int bi = -1;
+        for (int k = tid; k < nr; k += FTHREADS) {
+            if (r0 + k < jc) continue;
+            const double v = fabs(S[k * LDS + c]);
+            if (v > best) { best = v; bi = k; }          // strict >: lowest index wins inside a thread
+        }
+        for (int o = 16; o; o >>= 1) {
+            const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+            const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (ov > best || (ov == best && oi >= 0 && (bi < 0 || oi < bi))) { best = ov; bi = oi; }
+        }
+        if (lane == 0) { s_val[wq] = best; s_idx[wq] = bi; }
+        __syncthreads();
+        if (wq == 0) {
+            best = lane < FTHREADS / 32 ? s_val[lane] : -1.0;
+            bi = lane < FTHREADS / 32 ? s_idx[lane] : -1;
+            for (int o = 4; o; o >>= 1) {
+                const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+                const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+                if (ov > best || (ov == best && oi >= 0 && (bi < 0 || oi < bi))) { best = ov; bi = oi; }
+            }
+            bi = __shfl_sync(0xffffffffu, bi, 0);
+            best = __shfl_sync(0xffffffffu, best, 0);
+            Cand* cd = cand + (size_t)(c & 1) * G + b;
+            if (lane == 0) { cd->absval = best; cd->row = bi >= 0 ? r0 + bi : -1; }
+            if (bi >= 0) cd->content[lane] = S[bi * LDS + lane];
+            if (jc >= r0 && jc < r0 + nr) target[(c & 1) * FW + lane] = S[(int)(jc - r0) * LDS + lane];
+        }
+        __syncthreads();
+    };
+
+    publish(0);
+    for (int c = 0; c < w; ++c) {
+        grid.sync();
+        const int64_t jc = j0 + c;
+        // every CTA reduces the G candidates identically: largest |value|, lowest row on ties (reading Q12)
+        if (wq == 0) {
+            double best = -1.0;
+            long long brow = -1;
+            int bcta = -1;
+            for (int q = lane; q < G; q += 32) {
+                const Cand* cd = cand + (size_t)(c & 1) * G + q;
+                const double v = __ldcg(&cd->absval);
+                const long long rr = __ldcg(&cd->row);
+                if (rr >= 0 && (v > best || (v == best && rr < brow))) { best = v; brow = rr; bcta = q; }
+            }
+            for (int o = 16; o; o >>= 1) {
+                const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+                const long long orow = __shfl_xor_sync(0xffffffffu, brow, o);
+                const int oc = __shfl_xor_sync(0xffffffffu, bcta, o);
+                if (orow >= 0 && (ov > best || (ov == best && (brow < 0 || orow < brow)))) { best = ov; brow = orow; bcta = oc; }
+            }
+            pv[lane] = __ldcg(&cand[(size_t)(c & 1) * G + bcta].content[lane]);
+            if (lane == 0) {
+                s_g = brow;
+                if (b == 0) {
+                    ipiv[jc] = brow;
+                    if (!(best > tol)) atomicMin(info, (int)min((int64_t)INT_MAX, jc + 1));
+                }
+            }
+        }
+        __syncthreads();
+        const long long g = s_g;
+        // exchange rows jc and g (content of row jc comes from `target`, pivot row from `pv`)
+        if (g != jc) {
+            if (g >= r0 && g < r0 + nr && tid < FW) S[(int)(g - r0) * LDS + tid] = __ldcg(&target[(c & 1) * FW + tid]);
+        }
+        if (jc >= r0 && jc < r0 + nr && tid < FW) S[(int)(jc - r0) * LDS + tid] = pv[tid];
+        __syncthreads();
+        double piv = pv[c];
+        if (!(fabs(piv) > tol)) piv = 1.0;              // singular: flagged above; keep the arithmetic finite
+        // multipliers and rank-1 update of own rows below jc: one warp per row, lane = column
+        for (int k = wq; k < nr; k += FTHREADS / 32) {
+            if (r0 + k <= jc) continue;
+            const double l = S[k * LDS + c] / piv;
+            if (lane == c) S[k * LDS + c] = l;
+            else if (lane > c && lane < w) S[k * LDS + lane] -= l * pv[lane];
+        }
+        __syncthreads();
+        if (c + 1 < w) publish(c + 1);
+    }
+    for (int k = wq; k < nr; k += FTHREADS / 32)
+        if (lane < w) A[(r0 + k) * lda + j0 + lane] = S[k * LDS + lane];
+}
+
+// Row exchanges of one panel applied to whole rows outside the panel columns; one thread per column.
+__global__ void f64_swap_kernel(double* __restrict__ M, int64_t ld, int64_t c_begin, int64_t c_end, int64_t skip0,
+                                int64_t skip1, const long long* __restrict__ ipiv, int64_t j0, int w) {
+    int64_t c = c_begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= c_end || (c >= skip0 && c < skip1)) return;
+    for (int a = 0; a < w; ++a) {
+        const int64_t s = ipiv[j0 + a];
+        if (s != j0 + a && s >= 0) {
+            const double x = M[(j0 + a) * ld + c], y = M[s * ld + c];
+            M[(j0 + a) * ld + c] = y;
+            M[s * ld + c] = x;
+        }
+    }
+}
+
+// X <- L11^{-1} X, L11 unit lower nb x nb at A[t0:t0+nb, t0:t0+nb]; one thread per column of X.
+constexpr int FT = 128;
+__global__ void __launch_bounds__(FT) f64_trsm_lower_kernel(double* __restrict__ X, int64_t ldx, int64_t ncols,
+                                                            const double* __restrict__ A, int64_t lda, int64_t t0, int nb) {
+    __shared__ double L[FW][FW + 1];
+    __shared__ double Xs[FW][FT];
+    const int tid = threadIdx.x;
+    for (int e = tid; e < nb * nb; e += FT) L[e / nb][e % nb] = A[(t0 + e / nb) * lda + t0 + e % nb];
+    const int64_t c = (int64_t)blockIdx.x * FT + tid;
+    const bool on = c < ncols;
+    for (int a = 0; a < nb; ++a) Xs[a][tid] = on ? X[(int64_t)a * ldx + c] : 0.0;
+    __syncthreads();
+    if (!on) return;
+    for (int a = 1; a < nb; ++a) {
+        double s = Xs[a][tid];
+        for (int q = 0; q < a; ++q) s -= L[a][q] * Xs[q][tid];
+        Xs[a][tid] = s;
+        X[(int64_t)a * ldx + c] = s;
+    }
+}
+
+// X <- U11^{-1} X, U11 upper nb x nb (non-unit) at A[t0:t0+nb, t0:t0+nb].
+__global__ void __launch_bounds__(FT) f64_trsm_upper_kernel(double* __restrict__ X, int64_t ldx, int64_t ncols,
+                                                            const double* __restrict__ A, int64_t lda, int64_t t0, int nb) {
+    __shared__ double U[FW][FW + 1];
+    __shared__ double Xs[FW][FT];
+    const int tid = threadIdx.x;
+    for (int e = tid; e < nb * nb; e += FT) U[e / nb][e % nb] = A[(t0 + e / nb) * lda + t0 + e % nb];
+    const int64_t c = (int64_t)blockIdx.x * FT + tid;
+    const bool on = c < ncols;
+    for (int a = 0; a < nb; ++a) Xs[a][tid] = on ? X[(int64_t)a * ldx + c] : 0.0;
+    __syncthreads();
+    if (!on) return;
+    for (int a = nb - 1; a >= 0; --a) {
+        double s = Xs[a][tid];
+        for (int q = a + 1; q < nb; ++q) s -= U[a][q] * Xs[q][tid];
+        s /= U[a][a];
+        Xs[a][tid] = s;
+        X[(int64_t)a * ldx + c] = s;
+    }
+}
+
+// ---------------------------------------------------------------- F2 trailing update: C -= A.B (DFMA)
+constexpr int DM = 128, DN = 128, DK = 8, DTM = 8, DTN = 8;
+constexpr int DTHREADS = (DM / DTM) * (DN / DTN);      // 256
+__global__ void __launch_bounds__(DTHREADS) dgemm_sub_kernel(double* __restrict__ C, int64_t ldc,
+                                                             const double* __restrict__ A, int64_t lda,
+                                                             const double* __restrict__ B, int64_t ldb, int64_t M,
+                                                             int64_t N, int64_t K) {
+    __shared__ __align__(16) double As[2][DK][DM + 2];
+    __shared__ __align__(16) double Bs[2][DK][DN];
+    const int tid = threadIdx.x, tx = tid % (DN / DTN), ty = tid / (DN / DTN);
+    const int64_t m0 = (int64_t)blockIdx.y * DM, n0 = (int64_t)blockIdx.x * DN;
+    double acc[DTM][DTN];
+#pragma unroll
+    for (int i = 0; i < DTM; ++i)
+#pragma unroll
+        for (int j = 0; j < DTN; ++j) acc[i][j] = 0.0;
+
+    // each thread stages 4 A elements (128x8) and 4 B elements (8x128) per k-block
+    double ra[4], rb[4];
+    auto gload = [&](int64_t k0) {
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+            const int idx = tid + t * DTHREADS;
+            const int kk = idx % DK, mm = idx / DK;
+            const int64_t m = m0 + mm, k = k0 + kk;
+            ra[t] = (m < M && k < K) ? A[m * lda + k] : 0.0;
+            const int nn = idx % DN, kb = idx / DN;
+            const int64_t n = n0 + nn, k2 = k0 + kb;
+            rb[t] = (n < N && k2 < K) ? B[k2 * ldb + n] : 0.0;
+        }
+    };
+    auto sstore = [&](int buf) {
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+            const int idx = tid + t * DTHREADS;
+            As[buf][idx % DK][idx / DK] = ra[t];
+            Bs[buf][idx / DN][idx % DN] = rb[t];
+        }
+    };
+    gload(0);
+    sstore(0);
+    __syncthreads();
+    int buf = 0;
+    for (int64_t k0 = 0; k0 < K; k0 += DK) {
+        const bool more = k0 + DK < K;
+        if (more) gload(k0 + DK);
+#pragma unroll
+        for (int kk = 0; kk < DK; ++kk) {
+            double a[DTM], bb[DTN];
+#pragma unroll
+            for (int i = 0; i < DTM; i += 2)
+                *reinterpret_cast<double2*>(&a[i]) = *reinterpret_cast<const double2*>(&As[buf][kk][ty * DTM + i]);
+#pragma unroll
+            for (int j = 0; j < DTN; j += 2)
+                *reinterpret_cast<double2*>(&bb[j]) = *reinterpret_cast<const double2*>(&Bs[buf][kk][tx * DTN + j]);
+#pragma unroll
+            for (int i = 0; i < DTM; ++i)
+#pragma unroll
+                for (int j = 0; j < DTN; ++j) acc[i][j] = fma(a[i], bb[j], acc[i][j]);
+        }
+        if (more) {
+            sstore(buf ^ 1);
+            __syncthreads();
+            buf ^= 1;
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < DTM; ++i) {
+        const int64_t m = m0 + ty * DTM + i;
+        if (m >= M) continue;
+#pragma unroll
+        for (int j = 0; j < DTN; ++j) {
+            const int64_t n = n0 + tx * DTN + j;
+            if (n < N) C[m * ldc + n] -= acc[i][j];
+        }
+    }
+}
+
+struct F64 {
+    double* A; int64_t n, lda;
+    double* B; int64_t nrhs, ldb;
+    double tol;
+    cudaStream_t s;
+    Cand* cand; double* target; long long* ipiv; int* info;
+    int grid, rows_cap;         // cooperative grid size and the smem row capacity per CTA
+    size_t smem_max;
+};
+
+int dgemm_sub(F64& c, double* C, int64_t ldc, const double* A, int64_t lda, const double* B, int64_t ldb, int64_t M,
+              int64_t N, int64_t K) {
+    if (M <= 0 || N <= 0 || K <= 0) return LINAC_OK;
+    dim3 grid((unsigned)((N + DN - 1) / DN), (unsigned)((M + DM - 1) / DM));
+    dgemm_sub_kernel<<<grid, DTHREADS, 0, c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
+    LINAC_CUDA(cudaGetLastError());
+    stats().kernel_launches++;
+    stats().update_macs += M * N * K;
     return LINAC_OK;
 }
-int linac_solve_f64(double*, int64_t, int64_t, double*, int64_t, int64_t, double, void*, int64_t*) {
-    return LINAC_ERR_INTERNAL;
+
+// X <- L^{-1} X for the unit-lower block at [t0, t0+nb) on an arbitrary row-major X (ldx, ncols).
+int trsm_lower_f64(F64& c, double* X, int64_t ldx, int64_t ncols, int64_t t0, int64_t nb) {
+    if (nb <= 0 || ncols <= 0) return LINAC_OK;
+    if (nb <= FW) {
+        f64_trsm_lower_kernel<<<(unsigned)((ncols + FT - 1) / FT), FT, 0, c.s>>>(X, ldx, ncols, c.A, c.lda, t0, (int)nb);
+        LINAC_CUDA(cudaGetLastError());
+        stats().kernel_launches++;
+        return LINAC_OK;
+    }
+    const int64_t h = std::max<int64_t>(FW, nb / 2 / FW * FW);
+    int rc = trsm_lower_f64(c, X, ldx, ncols, t0, h);
+    if (rc) return rc;
+    rc = dgemm_sub(c, X + h * ldx, ldx, c.A + (t0 + h) * c.lda + t0, c.lda, X, ldx, nb - h, ncols, h);
+    if (rc) return rc;
+    return trsm_lower_f64(c, X + h * ldx, ldx, ncols, t0 + h, nb - h);
 }
+
+int trsm_upper_f64(F64& c, double* X, int64_t ldx, int64_t ncols, int64_t t0, int64_t nb) {
+    if (nb <= 0 || ncols <= 0) return LINAC_OK;
+    if (nb <= FW) {
+        f64_trsm_upper_kernel<<<(unsigned)((ncols + FT - 1) / FT), FT, 0, c.s>>>(X, ldx, ncols, c.A, c.lda, t0, (int)nb);
+        LINAC_CUDA(cudaGetLastError());
+        stats().kernel_launches++;
+        return LINAC_OK;
+    }
+    const int64_t h = std::max<int64_t>(FW, nb / 2 / FW * FW);
+    int rc = trsm_upper_f64(c, X + h * ldx, ldx, ncols, t0 + h, nb - h);
+    if (rc) return rc;
+    rc = dgemm_sub(c, X, ldx, c.A + t0 * c.lda + t0 + h, c.lda, X + h * ldx, ldx, h, ncols, nb - h);
+    if (rc) return rc;
+    return trsm_upper_f64(c, X, ldx, ncols, t0, h);
 }
+
+int panel_f64(F64& c, int64_t j0, int w) {
+    const int64_t m = c.n - j0;
+    int rows_per_cta = (int)((m + c.grid - 1) / c.grid);
+    rows_per_cta = std::max(rows_per_cta, 1);
+    if (rows_per_cta > c.rows_cap) return LINAC_ERR_INVALID_ARG;
+    size_t smem = (size_t)rows_per_cta * (FW + 1) * sizeof(double);
+    double* A = c.A; int64_t n = c.n, lda = c.lda; double tol = c.tol;
+    Cand* cand = c.cand; double* target = c.target; long long* ipiv = c.ipiv; int* info = c.info;
+    void* args[] = {&A, &n, &lda, &j0, &w, &rows_per_cta, &tol, &cand, &target, &ipiv, &info};
+    LINAC_CUDA(cudaLaunchCooperativeKernel((void*)f64_panel_kernel, dim3(c.grid), dim3(FTHREADS), args, smem, c.s));
+    // exchanges on the rest of A (left L part and right trailing part) and on B
+    const int64_t ncol = c.n;
+    f64_swap_kernel<<<(unsigned)((ncol + 255) / 256), 256, 0, c.s>>>(c.A, c.lda, 0, ncol, j0, j0 + w, c.ipiv, j0, w);
+    LINAC_CUDA(cudaGetLastError());
+    if (c.nrhs > 0) {
+        f64_swap_kernel<<<(unsigned)((c.nrhs + 255) / 256), 256, 0, c.s>>>(c.B, c.ldb, 0, c.nrhs, -1, -1, c.ipiv, j0, w);
+        LINAC_CUDA(cudaGetLastError());
+    }
+    stats().kernel_launches += 3;
+    stats().panels++;
+    return LINAC_OK;
+}
+
+// LU of columns [j0, j1) (square part: rows >= j0), right-looking recursion inside the range.
+int factor_f64(F64& c, int64_t j0, int64_t j1) {
+    const int64_t w = j1 - j0;
+    if (w <= 0) return LINAC_OK;
+    if (w <= FW) return panel_f64(c, j0, (int)w);
+    const int64_t h = std::max<int64_t>(FW, w / 2 / FW * FW);
+    const int64_t jm = j0 + h;
+    int rc = factor_f64(c, j0, jm);
+    if (rc) return rc;
+    rc = trsm_lower_f64(c, c.A + j0 * c.lda + jm, c.lda, j1 - jm, j0, h);
+    if (rc) return rc;
+    rc = dgemm_sub(c, c.A + jm * c.lda + jm, c.lda, c.A + jm * c.lda + j0, c.lda, c.A + j0 * c.lda + jm, c.lda,
+                   c.n - jm, j1 - jm, h);
+    if (rc) return rc;
+    return factor_f64(c, jm, j1);
+}
+
+size_t f64_workspace_bytes(int64_t n) {
+    (void)n;
+    return 4096 + 2 * 1024 * sizeof(Cand) + 2 * FW * sizeof(double) + (size_t)std::max<int64_t>(n, 1) * 8 + 1024;
+}
+
+}  // namespace
+}  // namespace linac
+
+using namespace linac;
+
+extern "C" {
+
+int linac_solve_f64_workspace(int64_t n, int64_t nrhs, size_t* bytes) {
+    if (!bytes || n < 0 || nrhs < 0) return LINAC_ERR_INVALID_ARG;
+    *bytes = n == 0 ? 0 : f64_workspace_bytes(n);
+    return LINAC_OK;
+}
+
+int linac_solve_f64(double* dA, int64_t n, int64_t lda, double* dB, int64_t nrhs, int64_t ldb, double tol, void* stream,
+                    int64_t* info_out) {
+    std::lock_guard<std::mutex> lock(g_call_mutex);
+    linac_stats& st = stats();
+    st = linac_stats{};
+    if (n < 0 || nrhs < 0 || !info_out) return LINAC_ERR_INVALID_ARG;
+    *info_out = 0;
+    if (n == 0) return LINAC_OK;
+    if (!dA || lda < n || (nrhs > 0 && (!dB || ldb < nrhs))) return LINAC_ERR_INVALID_ARG;
+    int rc = check_device();
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    Arena arena;
+    rc = acquire_workspace(f64_workspace_bytes(n), &arena);
+    if (rc) return rc;
+
+    F64 c;
+    c.A = dA; c.n = n; c.lda = lda; c.B = dB; c.nrhs = nrhs; c.ldb = ldb; c.s = s;
+    c.tol = tol < 0 ? (double)n * 2.220446049250313e-16 : tol;
+    int dev = 0, sms = 0, smem_optin = 0;
+    LINAC_CUDA(cudaGetDevice(&dev));
+    LINAC_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    LINAC_CUDA(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    c.grid = std::min(sms, 1024);
+    c.smem_max = (size_t)smem_optin - 4096;
+    c.rows_cap = (int)(c.smem_max / ((FW + 1) * sizeof(double)));
+    if ((n + c.grid - 1) / c.grid > c.rows_cap) return LINAC_ERR_INVALID_ARG;   // n > ~118k: strip no longer fits on chip
+    LINAC_CUDA(cudaFuncSetAttribute(f64_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max));
+    c.cand = (Cand*)arena.take(2 * 1024 * sizeof(Cand));
+    c.target = (double*)arena.take(2 * FW * sizeof(double));
+    c.ipiv = (long long*)arena.take((size_t)n * 8);
+    c.info = (int*)arena.take(256);
+    if (!c.cand || !c.target || !c.ipiv || !c.info) return LINAC_ERR_WORKSPACE;
+    const int big = INT_MAX;
+    LINAC_CUDA(cudaMemcpyAsync(c.info, &big, sizeof(int), cudaMemcpyHostToDevice, s));
+
+    cudaEvent_t e0, e1;
+    LINAC_CUDA(cudaEventCreate(&e0));
+    LINAC_CUDA(cudaEventCreate(&e1));
+    cudaEventRecord(e0, s);
+    row_scale_kernel<<<(unsigned)n, 256, 0, s>>>(dA, n, lda, dB, nrhs, ldb, c.info);          // F1
+    LINAC_CUDA(cudaGetLastError());
+    st.kernel_launches++;
+    // F2 with B as trailing columns: factor A in outer blocks so B's forward substitution is blocked too
+    rc = factor_f64(c, 0, n);
+    if (rc == LINAC_OK && nrhs > 0) rc = trsm_lower_f64(c, dB, ldb, nrhs, 0, n);              // forward substitution (L)
+    if (rc == LINAC_OK && nrhs > 0) rc = trsm_upper_f64(c, dB, ldb, nrhs, 0, n);              // F3 back substitution (U)
+    int h_info = INT_MAX;
+    if (rc == LINAC_OK) {
+        cudaEventRecord(e1, s);
+        LINAC_CUDA(cudaMemcpyAsync(&h_info, c.info, sizeof(int), cudaMemcpyDeviceToHost, s));
+    }
+    cudaError_t e = cudaStreamSynchronize(s);
+    st.host_syncs++;
+    if (e != cudaSuccess) { set_cuda_error(e, "cudaStreamSynchronize(solve_f64)", __FILE__, __LINE__); rc = rc ? rc : LINAC_ERR_CUDA; }
+    float ms = 0;
+    if (rc == LINAC_OK) cudaEventElapsedTime(&ms, e0, e1);
+    st.ms_total = ms;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (rc) return rc;
+    if (h_info != INT_MAX) {
+        *info_out = h_info;
+        return LINAC_ERR_SINGULAR;
+    }
+    return LINAC_OK;
+}
+
+}  // extern "C"

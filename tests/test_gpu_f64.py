@@ -1,0 +1,105 @@
+"""fp64 path through the C ABI: backward error <= 1e-11 on the original data (BASELINE.json), agreement with
+the oracle's solution to rounding, singular detection, exact special cases."""
+import numpy as np
+import pytest
+import torch
+
+import linac_inputs as gen
+from gpu_util import require_cuda
+
+pytestmark = pytest.mark.gpu
+ETA_MAX = 1e-11        # north_star: ||Ax-b|| / (||A|| ||x|| + ||b||) <= 1e-11
+
+
+@pytest.fixture(autouse=True, scope="module")
+def _cuda():
+    require_cuda()
+
+
+def gpu_solve(a, b, tol=-1.0, lda=None, ldb=None):
+    import paper_2605_25863_b200 as L
+    n, nrhs = b.shape
+    lda = n if lda is None else lda
+    ldb = nrhs if ldb is None else ldb
+    da = torch.full((n, lda), float("nan"), dtype=torch.float64, device="cuda")
+    db = torch.full((n, ldb), float("nan"), dtype=torch.float64, device="cuda")
+    da[:, :n] = torch.from_numpy(a).cuda()
+    db[:, :nrhs] = torch.from_numpy(b).cuda()
+    L.solve_f64(da[:, :n], db[:, :nrhs], tol)
+    if ldb > nrhs:
+        assert torch.isnan(db[:, nrhs:]).all()
+    return db[:, :nrhs].cpu().numpy()
+
+
+@pytest.mark.parametrize("n,nrhs", [(1, 1), (2, 2), (31, 3), (32, 1), (33, 5), (64, 64), (100, 7), (257, 9), (1000, 64)])
+def test_solve_backward_error_and_oracle_agreement(oracle, n, nrhs):
+    a, b = gen.shifted_normal_system(n, nrhs, seed_a=5, seed_b=6)
+    x = gpu_solve(a, b)
+    eta = oracle.backward_error(a, x, b, nthreads=oracle.max_threads())
+    assert eta <= ETA_MAX
+    rc, info, x_ref = oracle.solve_f64(a, b, nthreads=oracle.max_threads())
+    assert rc == 0
+    assert np.allclose(x, x_ref, rtol=1e-9, atol=1e-12)          # several x are "correct": loose agreement only
+
+
+def test_unshifted_gaussian_needs_pivoting(oracle):
+    """Plain N(0,1) matrix (no diagonal shift): without partial pivoting the error would be huge."""
+    n = 500
+    a = gen.normal_matrix(n, n, seed=21)
+    b = gen.normal_matrix(n, 4, seed=22)
+    x = gpu_solve(a, b)
+    assert oracle.backward_error(a, x, b, nthreads=oracle.max_threads()) <= ETA_MAX
+
+
+def test_row_scaling_and_leading_dimensions(oracle):
+    n, nrhs = 150, 6
+    a, b = gen.shifted_normal_system(n, nrhs, seed_a=7, seed_b=8)
+    scale = 10.0 ** np.linspace(-8, 8, n)
+    a2, b2 = a * scale[:, None], b * scale[:, None]          # badly row-scaled, same solution
+    x = gpu_solve(a2, b2, lda=n + 3, ldb=nrhs + 2)
+    assert oracle.backward_error(a, x, b) <= ETA_MAX
+    assert oracle.backward_error(a2, x, b2) <= ETA_MAX
+
+
+def test_exact_cases_and_manufactured_solution():
+    n = 96
+    b = gen.normal_matrix(n, 3, seed=3)
+    assert np.array_equal(gpu_solve(np.eye(n), b), b)
+    d = 2.0 ** np.arange(-10, n - 10, dtype=np.float64)
+    assert np.array_equal(gpu_solve(np.diag(d), b), b / d[:, None])
+    perm = np.random.default_rng(1).permutation(n)
+    pm = np.eye(n)[perm]
+    assert np.array_equal(gpu_solve(pm, b), pm.T @ b)
+    a, _ = gen.shifted_normal_system(n, 1, seed_a=9, seed_b=10)
+    ones = np.ones((n, 2))
+    assert np.allclose(gpu_solve(a, a @ ones), ones, rtol=1e-12)
+
+
+def test_singular_is_reported():
+    import paper_2605_25863_b200 as L
+    n = 80
+    a, b = gen.shifted_normal_system(n, 2, seed_a=1, seed_b=2)
+    a[50] = a[20]
+    with pytest.raises(L.LinacError) as e:
+        gpu_solve(a, b)
+    assert e.value.status == L.linac.ERR_SINGULAR and 1 <= e.value.info <= n
+    z, _ = gen.shifted_normal_system(n, 2, seed_a=1, seed_b=2)
+    z[7] = 0.0
+    with pytest.raises(L.LinacError) as e:
+        gpu_solve(z, b)
+    assert e.value.status == L.linac.ERR_SINGULAR
+    # caller-controlled threshold
+    a, b = gen.shifted_normal_system(n, 2, seed_a=1, seed_b=2)
+    a[50] = a[20] * (1 + 1e-9)
+    with pytest.raises(L.LinacError):
+        gpu_solve(a, b, tol=1e-6)
+    gpu_solve(a, b, tol=0.0)
+
+
+def test_medium_size_several_panels_and_recursion_levels(oracle):
+    n, nrhs = 3000, 64
+    a, b = gen.shifted_normal_system(n, nrhs, seed_a=5, seed_b=6)
+    x = gpu_solve(a, b)
+    assert oracle.backward_error(a, x, b, nthreads=oracle.max_threads()) <= ETA_MAX
+    ref = np.linalg.solve(a, b)
+    assert np.allclose(x, ref, rtol=1e-9, atol=1e-12)
