@@ -104,6 +104,18 @@ int linac_nullspace_from_rref_u32(const uint32_t *dR, int64_t rows, int64_t cols
                                   int64_t rank, const int32_t *pivot_cols, uint32_t *dK, int64_t ldk,
                                   void *stream);
 
+/* ---- F_p: the Schur-update primitive on its own (S5; exposed for measurement and tests) ------ */
+/*
+ * linac_gemm_sub_u32 -- C <- C - A.B (mod p), the blocked form of the paper's row update
+ * "row_k -= head_k * pivot_row" for K pivots at once.  All DEVICE, row-major:
+ * C is M x N (ldc), A is M x K (lda), B is K x N (ldb); entries must already be in [0,p).
+ * path: 0 = automatic choice, 1 = CUDA-core kernel (IMAD.WIDE + delayed reduction),
+ *       2 = tensor-core kernel (tcgen05 int8 limb planes; LINAC_ERR_INVALID_ARG if the shape is
+ *       not supported by it).  Synchronises `stream` before returning.
+ */
+int linac_gemm_sub_u32(uint32_t *dC, int64_t ldc, const uint32_t *dA, int64_t lda, const uint32_t *dB, int64_t ldb,
+                       int64_t M, int64_t N, int64_t K, uint32_t p, int path, void *stream);
+
 /* ---- fp64: partial-pivot solve ------------------------------------------------------------- */
 /*
  * linac_solve_f64 -- solves A X = B (eq. 10-12) in floating point:

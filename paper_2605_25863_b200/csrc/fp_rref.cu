@@ -362,4 +362,42 @@ int linac_nullspace_from_rref_u32(const uint32_t* dR, int64_t rows, int64_t cols
     return nullspace_from_rref_impl(dR, rows, cols, ld, p, rank, pivot_cols, dK, ldk, (cudaStream_t)stream);
 }
 
+int linac_gemm_sub_u32(uint32_t* dC, int64_t ldc, const uint32_t* dA, int64_t lda, const uint32_t* dB, int64_t ldb, int64_t M,
+                       int64_t N, int64_t K, uint32_t p, int path, void* stream) {
+    std::lock_guard<std::mutex> lock(g_call_mutex);
+    if (M < 0 || N < 0 || K < 0 || path < 0 || path > 2) return LINAC_ERR_INVALID_ARG;
+    if (p < 2 || p >= (1u << 31) || !is_prime_u32(p)) return LINAC_ERR_BAD_MODULUS;
+    if (M == 0 || N == 0 || K == 0) return LINAC_OK;
+    if (!dC || !dA || !dB || ldc < N || lda < K || ldb < N) return LINAC_ERR_INVALID_ARG;
+    int rc = check_device();
+    if (rc) return rc;
+    stats() = linac_stats{};
+    const ModP f = make_modp(p);
+    cudaStream_t s = (cudaStream_t)stream;
+    GemmArgs g{dC, ldc, dA, lda, nullptr, dB, ldb, M, N, K};
+    cudaEvent_t e0, e1;
+    LINAC_CUDA(cudaEventCreate(&e0));
+    LINAC_CUDA(cudaEventCreate(&e1));
+    rc = -1;
+    cudaEventRecord(e0, s);
+    if (path == 2 || (path == 0 && K >= options().tc_min_k && M >= options().tc_min_mn && N >= options().tc_min_mn)) {
+        Arena arena;
+        rc = acquire_workspace(gemm_modp_tc_scratch_bytes(M, N, K) + 4096, &arena);
+        if (rc) return rc;
+        rc = gemm_modp_tc(g, f, s, &arena);
+        if (rc < 0 && path == 2) rc = LINAC_ERR_INVALID_ARG;
+    }
+    if (rc < 0) rc = gemm_modp_simt(g, f, s);
+    cudaEventRecord(e1, s);
+    cudaError_t e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) { set_cuda_error(e, "cudaStreamSynchronize(gemm)", __FILE__, __LINE__); rc = rc ? rc : LINAC_ERR_CUDA; }
+    float ms = 0;
+    if (e == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
+    stats().ms_update = ms;
+    stats().ms_total = ms;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    return rc;
+}
+
 }  // extern "C"

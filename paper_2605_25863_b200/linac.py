@@ -21,7 +21,7 @@ ERR_SINGULAR, ERR_BUFFER_TOO_SMALL, ERR_UNSUPPORTED_DEVICE, ERR_INTERNAL = 5, 6,
 SYMBOLS = [
     "linac_status_string", "linac_last_cuda_error", "linac_version",
     "linac_rref_u32_workspace", "linac_solve_f64_workspace", "linac_set_workspace", "linac_release",
-    "linac_rref_u32", "linac_nullspace_u32", "linac_nullspace_from_rref_u32", "linac_solve_f64",
+    "linac_rref_u32", "linac_nullspace_u32", "linac_nullspace_from_rref_u32", "linac_gemm_sub_u32", "linac_solve_f64",
     "linac_get_last_stats", "linac_set_option",
 ]
 
@@ -65,6 +65,7 @@ def _lib() -> C.CDLL:
         L.linac_rref_u32.argtypes = [vp, i64, i64, i64, u32, vp, C.POINTER(i64), vp]
         L.linac_nullspace_u32.argtypes = [vp, i64, i64, i64, u32, vp, C.POINTER(i64), vp, vp, i64, i64, C.POINTER(i64)]
         L.linac_nullspace_from_rref_u32.argtypes = [vp, i64, i64, i64, u32, i64, vp, vp, i64, vp]
+        L.linac_gemm_sub_u32.argtypes = [vp, i64, vp, i64, vp, i64, i64, i64, i64, u32, C.c_int, vp]
         L.linac_solve_f64.argtypes = [vp, i64, i64, vp, i64, i64, C.c_double, vp, C.POINTER(i64)]
         L.linac_get_last_stats.argtypes = [C.POINTER(Stats)]
         L.linac_set_option.argtypes = [C.c_char_p, i64]
@@ -197,6 +198,20 @@ def nullspace_from_rref_u32(r: torch.Tensor, p: int, rank: int, pivot_cols: torc
     if rc:
         raise LinacError(rc, "linac_nullspace_from_rref_u32")
     return k
+
+
+def gemm_sub_u32(c: torch.Tensor, a: torch.Tensor, b: torch.Tensor, p: int, path: int = 0) -> None:
+    """In place: c <- c - a.b (mod p) on the device (S5 primitive).  path 0 auto, 1 CUDA cores, 2 tensor cores."""
+    m, n, ldc = _check_matrix(c, _U32, "c")
+    m2, k, lda = _check_matrix(a, _U32, "a")
+    k2, n2, ldb = _check_matrix(b, _U32, "b")
+    if m != m2 or n != n2 or k != k2:
+        raise ValueError("shape mismatch")
+    with torch.cuda.device(c.device):
+        rc = _lib().linac_gemm_sub_u32(c.data_ptr(), ldc, a.data_ptr(), lda, b.data_ptr(), ldb, m, n, k, p, path,
+                                       _stream_ptr(c.device))
+    if rc:
+        raise LinacError(rc, "linac_gemm_sub_u32")
 
 
 def solve_f64(a: torch.Tensor, b: torch.Tensor, tol: float = -1.0) -> int:

@@ -1,0 +1,75 @@
+"""S5 primitive C <- C - A.B mod p: CUDA-core kernel and tensor-core (tcgen05 int8 limb) kernel, each
+element by element against the oracle's plain triple loop."""
+import numpy as np
+import pytest
+import torch
+
+import linac_inputs as gen
+from gpu_util import require_cuda, from_device
+
+pytestmark = pytest.mark.gpu
+P31 = 2147483647
+P29 = 2147483629
+
+
+@pytest.fixture(autouse=True, scope="module")
+def _cuda():
+    require_cuda()
+
+
+def run_gemm(c, a, b, p, path):
+    import paper_2605_25863_b200 as L
+    dc = torch.from_numpy(c.view(np.int32)).cuda()
+    da = torch.from_numpy(a.view(np.int32)).cuda()
+    db = torch.from_numpy(b.view(np.int32)).cuda()
+    L.gemm_sub_u32(dc, da, db, p, path)
+    return from_device(dc), L.last_stats()
+
+
+def expected(oracle, c, a, b, p):
+    prod = oracle.matmul_modp(a, b, p, nthreads=oracle.max_threads())
+    return ((c.astype(np.int64) - prod.astype(np.int64)) % p).astype(np.uint32)
+
+
+SHAPES = [(1, 1, 1), (5, 7, 3), (128, 64, 16), (129, 65, 17), (200, 300, 100), (257, 130, 33)]
+TC_SHAPES = [(128, 64, 128), (128, 64, 32), (256, 128, 256), (300, 200, 150), (512, 512, 512), (1000, 900, 700),
+             (640, 576, 4224), (130, 70, 1)]
+
+
+@pytest.mark.parametrize("m,n,k", SHAPES + TC_SHAPES)
+@pytest.mark.parametrize("p", [P31, P29, 7])
+def test_simt_kernel(oracle, m, n, k, p):
+    if (m, n, k) == (640, 576, 4224) and p != P31:
+        pytest.skip("one modulus is enough at the largest shape")
+    a = gen.uniform_matrix(m, k, p, seed=1)
+    b = gen.uniform_matrix(k, n, p, seed=2)
+    c = gen.uniform_matrix(m, n, p, seed=3)
+    out, _ = run_gemm(c, a, b, p, path=1)
+    assert np.array_equal(out, expected(oracle, c, a, b, p))
+
+
+@pytest.mark.parametrize("m,n,k", TC_SHAPES)
+@pytest.mark.parametrize("p", [P31, P29, 7])
+def test_tensor_core_kernel(oracle, m, n, k, p):
+    if (m, n, k) == (640, 576, 4224) and p != P31:
+        pytest.skip("one modulus is enough at the largest shape")
+    a = gen.uniform_matrix(m, k, p, seed=1)
+    b = gen.uniform_matrix(k, n, p, seed=2)
+    c = gen.uniform_matrix(m, n, p, seed=3)
+    out, st = run_gemm(c, a, b, p, path=2)
+    assert st["tc_launches"] >= 1
+    assert np.array_equal(out, expected(oracle, c, a, b, p))
+
+
+def test_tensor_core_worst_case_operands(oracle):
+    """All entries p-1: every limb product at its maximum, K = 4096 in one launch (s32 accumulator headroom)."""
+    m, n, k = 128, 64, 4096
+    a = np.full((m, k), P31 - 1, dtype=np.uint32)
+    b = np.full((k, n), P31 - 1, dtype=np.uint32)
+    c = np.zeros((m, n), dtype=np.uint32)
+    out, st = run_gemm(c, a, b, P31, path=2)
+    assert st["tc_launches"] == 1
+    want = (-(k * pow(P31 - 1, 2, P31))) % P31
+    assert (out == want).all()
+    out1, _ = run_gemm(c, a, b, P31, path=1)
+    assert (out1 == want).all()
