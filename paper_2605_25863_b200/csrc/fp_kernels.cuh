@@ -1,14 +1,19 @@
 // fp_kernels.cuh -- the small kernels of the F_p path (everything except the Schur-update GEMM).
 //
-// Storage convention of the forward phase (in place, LAPACK-like).  Pivot t (global pivot index)
-// lives in ROW t and column pivcols[t].  After a panel is factored:
-//   (row t, col pivcols[t])            holds d_t^{-1}  (d_t = the pivot value before normalisation;
-//                                      the echelon row's leading 1 is implicit)
-//   (row t, col c > pivcols[t])        holds E_t[c], the normalised echelon row
-//   (row k > t, col pivcols[t])        holds the multiplier L[k][t]  (row_k = sum_t L[k][t] E_t)
-//   (row k, non-pivot col c of a finished panel, k >= #pivots left of c) holds a true 0
-// The finalise kernel overwrites every pivot column with a unit vector, which removes the L
-// entries and the stored d^{-1} -- that is what makes the result the RREF of PAPER.md:153.
+// Storage convention of the forward phase (in place).  Base panel b covers columns [32b, 32b+w).
+// Its pivots (global pivot indices t in [pstart[b], pstart[b+1])) live in ROWS t after the panel's
+// row exchanges; pivcols[t] is the pivot column.  With P the pivot rows and Jp the pivot columns of
+// the panel, T_b = (A[P, Jp])^{-1} is kept in a side buffer; the reduced pivot rows are U = T_b A[P, :]
+// (identity on Jp).  Because U is the identity on the panel's pivot columns, the multiplier of any
+// other row k against reduced pivot row t is simply the stored entry A[k, pivcols[t]] -- the panel
+// columns of the rows below are never rewritten:
+//   (row k >= pstart[b+1], col pivcols[t])   raw value = multiplier L[k][t]
+//   (row t, col c right of the panel)        U[t][c] once the enclosing recursion node has applied T
+//   (row t of panel b, free column of b)     U[t][c]   (written by panel_finish_kernel when r < w)
+//   (row k >= pstart[b+1], free column of b) mathematically 0; storage holds garbage that the
+//                                            gather / finalise kernels replace by 0
+// The finalise kernel overwrites every pivot column with a unit vector and the garbage with zeros,
+// which makes the result the RREF of PAPER.md:153.
 #pragma once
 #include <climits>
 
@@ -27,273 +32,263 @@ __global__ void reduce_mod_p_kernel(uint32_t* __restrict__ A, int64_t rows, int6
     }
 }
 
+// d*x - h*y mod p with one reduction: d*x + (p-h)*y < 2^63.
+__device__ __forceinline__ uint32_t lincomb(uint32_t d, uint32_t x, uint32_t h, uint32_t y, const ModP& f) {
+    return reduce64((uint64_t)d * x + (uint64_t)(f.p - h) * y, f);
+}
+
 // ------------------------------------------------------------------------------------------
-// S1 + S2 (decision part): pivot search for one base panel (columns [j0, j0+w), rows >= i0).
+// S1 + S2 + S3 for one base panel (columns [j0, j0+w), rows >= i0), one CTA of 256 threads.
 //
-// One CTA.  Works on a shared-memory copy, so global memory still holds the original strip when
-// it ends.  Rows are scanned in chunks of CH; each chunk is first reduced against the echelon rows
-// found so far, then searched column by column for the FIRST row with a non-zero entry (warp
-// ballot / atomicMin; for F_p any non-zero pivot will do).  Elimination inside the
-// chunk is division-free (row_k <- d*row_k - h*row_q), so no modular inverse sits on the
-// column-to-column dependency chain; the new pivot rows are normalised together at the end of
-// the chunk, one warp per row, inverses computed in parallel.
-// Stops as soon as w pivots are known; otherwise it has looked at every row, which is what
-// proves that the remaining columns of the panel are free columns.
-__global__ void __launch_bounds__(256) panel_pivots_kernel(const uint32_t* __restrict__ A, int64_t ld, int64_t rows,
+// Phase 1 (pivot search, K3/K4/K6 of PAPER.md:241-243): rows are scanned in chunks of CH = 32 held in
+// shared memory; a chunk is first reduced against the pivot rows found so far, then searched column
+// by column for the FIRST row with a non-zero entry (warp ballot; for F_p any non-zero pivot will do,
+// PAPER.md:241).  Elimination is division-free (row_k <- d*row_k - h*row_q), so no modular inverse
+// sits on the column-to-column dependency chain.  The scan stops once w pivots are known; otherwise
+// it has looked at every row, which is what proves the remaining columns are free columns.
+// Phase 2 (K7 "rescale the head to 1", done for the whole panel at once): Gauss-Jordan
+// on [D | I], D = A[pivot rows, pivot columns] in ascending pivot-column order (no search needed:
+// pivot rows with a larger leading column vanish on the smaller columns, so D has an LU factorisation
+// without pivoting), division-free, followed by r independent extended-Euclid inverses.
+// Outputs: rec (r, local pivot columns, LAPACK-style exchange list), T (32x32, zero padded),
+// E = T A[P, panel] when r < w (the free columns' entries of the reduced pivot rows), pivcols.
+__global__ void __launch_bounds__(256) panel_factor_kernel(const uint32_t* __restrict__ A, int64_t ld, int64_t rows,
                                                            int64_t i0, int64_t j0, int w, ModP f,
-                                                           PanelInfo* __restrict__ info, uint32_t* __restrict__ Eout,
-                                                           int32_t* __restrict__ pivcols_global) {
+                                                           PanelRec* __restrict__ rec, uint32_t* __restrict__ Tout,
+                                                           uint32_t* __restrict__ Eout,
+                                                           int32_t* __restrict__ pivcols_global,
+                                                           const int* __restrict__ fail_flag, int panel_index) {
     __shared__ uint32_t X[CH][PW + 1];
-    __shared__ uint32_t E[PW][PW + 1];     // normalised echelon rows, discovery order
-    __shared__ int epc[PW];                // pivot column of E[t]
-    __shared__ long long esrc[PW];         // source row (absolute) of E[t]
-    __shared__ int urow[PW];               // chunk-local row that became pivot t (this chunk)
-    __shared__ int ord[PW];                // E rows sorted by pivot column
-    __shared__ int found[PW];
-    __shared__ int any_nz;
+    __shared__ uint32_t Ep[PW][PW + 1];        // pivot rows as selected (unnormalised), discovery order
+    __shared__ uint32_t G[PW][2 * PW + 1];     // phase 2: [D | I]
+    __shared__ int epc[PW];                    // pivot column of pivot t (discovery order)
+    __shared__ long long esrc[PW];             // source row (absolute) of pivot t
+    __shared__ int ord[PW];                    // pivots sorted by pivot column
+    __shared__ uint32_t ginv[PW];
+    __shared__ long long pos_of[PW];           // absolute position of the row that started at i0 + b
+    __shared__ int at[PW];                     // which of those rows sits at top position a
+    __shared__ int s_nsw;
+
+    if (fail_flag && *fail_flag < panel_index) return;      // an earlier panel left the optimistic schedule
 
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
-    int r = 0;
+    int r = 0;                 // uniform over the CTA
+    unsigned pcmask = 0;       // pivot columns so far (uniform)
 
     for (int64_t cs = i0; cs < rows && r < w; cs += CH) {
         const int nh = (int)min((int64_t)CH, rows - cs);
-        if (tid < PW) found[tid] = INT_MAX;
-        if (tid == 0) any_nz = 0;
-        __syncthreads();
-        // load + reduce against the current echelon rows (ascending pivot column)
         int nz = 0;
-        for (int k = wq; k < CH; k += 8) {
+#pragma unroll
+        for (int t = 0; t < CH / 8; ++t) {
+            const int k = wq * (CH / 8) + t;
             uint32_t s = 0;
-            if (k < nh && lane < w) {
-                s = A[(cs + k) * ld + j0 + lane];
-                if (s >= f.p) s %= f.p;
-            }
-            for (int a = 0; a < r; ++a) {
-                const int t = ord[a];
-                const uint32_t l = __shfl_sync(0xffffffffu, s, epc[t]);
-                if (l) s = submulmod(s, l, E[t][lane], f);
+            if (k < nh && lane < w) s = A[(cs + k) * ld + j0 + lane];
+            for (int a = 0; a < r; ++a) {          // ascending pivot column
+                const int tt = ord[a];
+                const int c = epc[tt];
+                const uint32_t l = __shfl_sync(0xffffffffu, s, c);
+                if (l) s = lane > c ? lincomb(Ep[tt][c], s, l, Ep[tt][lane], f) : (lane == c ? 0u : mulmod(Ep[tt][c], s, f));
             }
             X[k][lane] = s;
             nz |= (s != 0);
         }
-        if (__any_sync(0xffffffffu, nz) && lane == 0) any_nz = 1;
-        __syncthreads();
-        if (!any_nz) continue;          // the whole chunk lies in the span found so far
+        if (!__syncthreads_or(nz)) continue;       // the whole chunk lies in the span found so far
 
-        const int r_start = r;
-        unsigned usedmask = 0;          // bit t: my warp's row wq + 8t is already a pivot row
+        unsigned used = 0;                         // chunk rows that became pivot rows (uniform)
         for (int c = 0; c < w && r < w; ++c) {
-            // lanes 0..7 test this warp's 8 rows
-            if (lane < 8) {
-                const int k = wq + 8 * lane;
-                if (!((usedmask >> lane) & 1u) && X[k][c] != 0) atomicMin(&found[c], k);
-            }
-            __syncthreads();
-            const int q = found[c];
-            if (q == INT_MAX) continue;
+            if ((pcmask >> c) & 1u) continue;
+            const unsigned cand = __ballot_sync(0xffffffffu, X[lane][c] != 0) & ~used;
+            if (!cand) continue;
+            const int q = __ffs(cand) - 1;
             const uint32_t d = X[q][c];
             const uint32_t pv = X[q][lane];
-            for (int t = 0; t < 8; ++t) {
-                const int k = wq + 8 * t;
-                if (k == q) { usedmask |= 1u << t; continue; }
-                if ((usedmask >> t) & 1u) continue;
+#pragma unroll
+            for (int t = 0; t < CH / 8; ++t) {
+                const int k = wq * (CH / 8) + t;
+                if (k == q || ((used >> k) & 1u)) continue;
                 const uint32_t h = X[k][c];
                 if (h == 0) continue;
-                // division-free: scales row k by d != 0, which changes neither its span nor its zeros
-                X[k][lane] = submod(mulmod(d, X[k][lane], f), mulmod(h, pv, f), f);
+                if (lane > c) X[k][lane] = lincomb(d, X[k][lane], h, pv, f);   // column c itself is not rewritten
             }
-            if (tid == 0) { epc[r] = c; esrc[r] = cs + q; urow[r] = q; }
+            if (wq == 0) Ep[r][lane] = ((pcmask >> lane) & 1u) ? 0u : pv;      // stale entries at earlier pivot columns are zeros
+            if (tid == 0) { epc[r] = c; esrc[r] = cs + q; }
+            used |= 1u << q;
+            pcmask |= 1u << c;
             ++r;
-            __syncwarp();               // lanes 0..7 read what other lanes of this warp just wrote
+            __syncthreads();
         }
-        __syncthreads();
-        // normalise the new pivot rows (parallel inverses), one warp per row
-        for (int t = r_start + wq; t < r; t += 8) {
-            const int q = urow[t];
-            const uint32_t dinv = invmod(X[q][epc[t]], f);
-            E[t][lane] = mulmod(X[q][lane], dinv, f);
-        }
-        if (tid == 0) {                 // insertion sort of <= 32 pivot columns
-            for (int t = r_start; t < r; ++t) {
-                int a = t;
-                while (a > 0 && epc[ord[a - 1]] > epc[t]) { ord[a] = ord[a - 1]; --a; }
-                ord[a] = t;
-            }
+        // rank sort of the pivots by column (needed to reduce the next chunk, and at the end)
+        if (wq == 0) {
+            const int mine = lane < r ? epc[lane] : INT_MAX;
+            int pos = 0;
+            for (int s = 0; s < r; ++s) pos += (epc[s] < mine);
+            if (lane < r) ord[pos] = lane;
         }
         __syncthreads();
     }
 
-    // outputs
-    __syncthreads();
-    for (int a = wq; a < r; a += 8) Eout[a * PW + lane] = E[ord[a]][lane];
-    if (tid == 0) {
-        info->r = r;
-        info->residual = 0;
-        // Row i0+a must receive source row esrc[ord[a]]: turn that into sequential exchanges.
-        long long pos_of[PW];   // where the row that originally sat at i0+b is now (only b < r matter)
-        for (int b = 0; b < r; ++b) pos_of[b] = i0 + b;
-        int nsw = 0;
-        for (int a = 0; a < r; ++a) {
-            long long src = esrc[ord[a]];
-            // current position of the original row `src`: it moved only if it was one of the top rows
-            long long cur = src;
-            if (src < i0 + r) cur = pos_of[src - i0];
-            info->swp[a] = cur;
-            info->pc[a] = epc[ord[a]];
-            pivcols_global[i0 + a] = (int32_t)(j0 + epc[ord[a]]);
-            if (cur != i0 + a) {
-                ++nsw;
-                // the row now at i0+a goes to `cur`; find which original top row that is
-                for (int b = 0; b < r; ++b)
-                    if (pos_of[b] == i0 + a) { pos_of[b] = cur; break; }
-                if (src < i0 + r) pos_of[src - i0] = i0 + a;
+    // ---- exchange list: row i0+a must receive source row esrc[ord[a]]
+    if (wq == 0) {
+        const bool inplace = lane >= r || esrc[ord[lane]] == i0 + lane;
+        const bool all_inplace = __all_sync(0xffffffffu, inplace);
+        if (lane < r) { pos_of[lane] = i0 + lane; at[lane] = lane; }
+        __syncwarp();
+        if (lane == 0) {
+            int nsw = 0;
+            if (all_inplace) {
+                for (int a = 0; a < r; ++a) rec->swp[a] = i0 + a;
+            } else {
+                for (int a = 0; a < r; ++a) {
+                    const long long src = esrc[ord[a]];
+                    const long long cur = src < i0 + r ? pos_of[(int)(src - i0)] : src;
+                    rec->swp[a] = cur;
+                    if (cur != i0 + a) {
+                        ++nsw;
+                        const int x = at[a];                 // top-origin row now sitting at position a
+                        pos_of[x] = cur;
+                        if (cur < i0 + r) at[(int)(cur - i0)] = x;
+                    }
+                }
             }
+            s_nsw = nsw;
         }
-        info->nswaps = nsw;
+    }
+    // ---- phase 2: T = D^{-1}
+    for (int e = tid; e < PW * 2 * PW; e += 256) {
+        const int a = e / (2 * PW), b = e % (2 * PW);
+        uint32_t v = 0;
+        if (a < r) {
+            if (b < PW) { if (b < r) v = A[esrc[ord[a]] * ld + j0 + epc[ord[b]]]; }
+            else v = (b - PW == a) ? 1u : 0u;
+        }
+        G[a][b] = v;
+    }
+    __syncthreads();
+    for (int t = 0; t < r; ++t) {
+        const uint32_t d = G[t][t];
+        const uint32_t pl = lane > t ? G[t][lane] : 0u;
+        const uint32_t pr = lane <= t ? G[t][PW + lane] : 0u;
+#pragma unroll
+        for (int u = 0; u < PW / 8; ++u) {
+            const int s = wq * (PW / 8) + u;
+            if (s == t || s >= r) continue;
+            const uint32_t h = G[s][t];
+            if (h == 0) continue;
+            if (lane > t || lane == s) G[s][lane] = lincomb(d, G[s][lane], h, pl, f);
+            if (lane <= t || lane == s) G[s][PW + lane] = lincomb(d, G[s][PW + lane], h, pr, f);
+        }
+        __syncthreads();
+    }
+    if (wq == 0 && lane < r) ginv[lane] = invmod(G[lane][lane], f);
+    __syncthreads();
+    for (int e = tid; e < PW * PW; e += 256) {
+        const int a = e / PW, b = e % PW;
+        const uint32_t v = (a < r && b < r) ? mulmod(ginv[a], G[a][PW + b], f) : 0u;
+        Tout[e] = v;
+        G[a][b] = v;                  // keep T in shared memory for E below (left half is dead now)
+    }
+    if (r < w && r > 0) {
+        // E = T . A[P, panel]: reduced pivot rows restricted to the panel (identity on the pivot columns)
+        for (int e = tid; e < PW * PW; e += 256) {
+            const int a = e / PW, b = e % PW;
+            X[a][b] = (a < r && b < w) ? A[esrc[ord[a]] * ld + j0 + b] : 0u;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int u = 0; u < PW / 8; ++u) {
+            const int a = wq * (PW / 8) + u;
+            uint64_t acc = 0;
+            for (int b = 0; b < r; ++b) {
+                acc += (uint64_t)G[a][b] * X[b][lane];
+                if (b & 1) acc = fold64(acc, f);
+            }
+            Eout[a * PW + lane] = a < r ? reduce64(acc, f) : 0u;
+        }
+    }
+    if (tid < PW) {
+        rec->pc[tid] = tid < r ? epc[ord[tid]] : -1;
+        if (tid < r) pivcols_global[i0 + tid] = (int32_t)(j0 + epc[ord[tid]]);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        rec->r = r;
+        rec->w = w;
+        rec->nswaps = s_nsw;
     }
 }
 
 // ------------------------------------------------------------------------------------------
-// K5 CudaSwitchRows for a whole panel: the exchanges are applied to complete
-// rows, one thread per column (so the sequence of exchanges needs no inter-thread ordering).
-__global__ void apply_swaps_kernel(uint32_t* __restrict__ A, int64_t ld, int64_t cols, int64_t i0,
-                                   const PanelInfo* __restrict__ info) {
-    if (info->nswaps == 0) return;
+// K5 CudaSwitchRows for a whole panel: the exchanges are applied to complete rows,
+// one thread per column (so the sequence of exchanges needs no inter-thread ordering).  When the
+// panel is rank deficient the same thread then stores the reduced pivot rows' panel entries E.
+__global__ void panel_finish_kernel(uint32_t* __restrict__ A, int64_t ld, int64_t cols, int64_t i0, int64_t j0,
+                                    const PanelRec* __restrict__ rec, const uint32_t* __restrict__ E,
+                                    const int* __restrict__ fail_flag, int panel_index) {
+    if (fail_flag && *fail_flag < panel_index) return;
+    const int r = rec->r, ns = rec->nswaps, w = rec->w;
+    if (r == 0 || (ns == 0 && r == w)) return;
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= cols) return;
-    const int r = info->r;
-    for (int a = 0; a < r; ++a) {
-        const int64_t s = info->swp[a];
-        if (s != i0 + a) {
-            uint32_t x = A[(i0 + a) * ld + c], y = A[s * ld + c];
-            A[(i0 + a) * ld + c] = y;
-            A[s * ld + c] = x;
+    if (ns > 0) {
+        for (int a = 0; a < r; ++a) {
+            const int64_t s = rec->swp[a];
+            if (s != i0 + a) {
+                const uint32_t x = A[(i0 + a) * ld + c], y = A[s * ld + c];
+                A[(i0 + a) * ld + c] = y;
+                A[s * ld + c] = x;
+            }
         }
     }
+    if (r < w && c >= j0 && c < j0 + w)
+        for (int a = 0; a < r; ++a) A[(i0 + a) * ld + c] = E[a * PW + (int)(c - j0)];
 }
 
 // ------------------------------------------------------------------------------------------
-// S2 + S3: with the panel's echelon rows E known, every row k >= i0 of the strip is rewritten in
-// place from its ORIGINAL values: forward substitution against E gives the multipliers L[k][t]
-// (stored at the pivot columns); pivot rows additionally get normalised (K7) and keep
-// their echelon entries.  One warp per row, lane = panel column; rows are independent.
-__global__ void __launch_bounds__(256) panel_apply_kernel(uint32_t* __restrict__ A, int64_t ld, int64_t rows, int64_t i0,
-                                                          int64_t j0, int w, ModP f, PanelInfo* __restrict__ info,
-                                                          const uint32_t* __restrict__ Eg) {
-    __shared__ uint32_t E[PW][PW + 1];
-    __shared__ int pc[PW];
-    const int r = info->r;
-    if (r == 0) return;
-    const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
-    for (int a = wq; a < r; a += 8) E[a][lane] = Eg[a * PW + lane];
-    if (tid < r) pc[tid] = info->pc[tid];
+// S4 row-block solve, base case: X <- T X for one base panel (r <= 32 pivot rows i0..i0+r),
+// X = A[i0 : i0+r, c0 : c0+ncols].  A 32x32 tile of X per CTA; thread = (4 output rows, 1 column).
+__global__ void __launch_bounds__(256) apply_t_kernel(uint32_t* __restrict__ X, int64_t ldx, int64_t ncols,
+                                                      const uint32_t* __restrict__ T, int r, ModP f,
+                                                      const int* __restrict__ fail_flag, int epoch) {
+    if (fail_flag && *fail_flag <= epoch) return;
+    __shared__ uint32_t Ts[PW][PW + 1];
+    __shared__ uint32_t Xs[PW][PW + 1];
+    const int tid = threadIdx.x, lane = tid & 31, g = tid >> 5;
+    const int64_t c = (int64_t)blockIdx.x * PW + lane;
+    for (int e = tid; e < PW * PW; e += 256) Ts[e / PW][e % PW] = T[e];
+#pragma unroll
+    for (int u = 0; u < PW / 8; ++u) {
+        const int a = g * (PW / 8) + u;
+        Xs[a][lane] = (a < r && c < ncols) ? X[(int64_t)a * ldx + c] : 0u;
+    }
     __syncthreads();
-    unsigned pivmask = 0;                       // bit c: local column c is a pivot column
-    for (int t = 0; t < r; ++t) pivmask |= 1u << pc[t];
-
-    const int64_t k = i0 + (int64_t)blockIdx.x * 8 + wq;
-    if (k >= rows) return;
-    uint32_t s = 0;
-    if (lane < w) {
-        s = A[k * ld + j0 + lane];
-        if (s >= f.p) s %= f.p;
-    }
-    const int64_t a = k - i0;
-    const int steps = a < r ? (int)a : r;
-    for (int t = 0; t < steps; ++t) {
-        const uint32_t l = __shfl_sync(0xffffffffu, s, pc[t]);
-        if (lane == pc[t]) s = l;                            // keep the multiplier where the zero would be
-        else if (lane > pc[t] && l) s = submulmod(s, l, E[t][lane], f);
-    }
-    if (a < r) {
-        // pivot row: what is left is d_a * E_a; normalise, store d_a^{-1} on the (implicit-1) pivot
-        const int pa = pc[a];
-        const uint32_t d = __shfl_sync(0xffffffffu, s, pa);
-        const uint32_t dinv = d ? invmod(d, f) : 0;
-        if (d == 0 && lane == 0) atomicAdd(&info->residual, 1);
-        if (lane == pa) s = dinv;
-        else if (lane > pa) s = mulmod(s, dinv, f);
-        else if (!((pivmask >> lane) & 1u) && s != 0) atomicAdd(&info->residual, 1);
-    } else {
-        // a row below the pivots must have been reduced to zero on the non-pivot columns
-        if (lane < w && !((pivmask >> lane) & 1u) && s != 0) atomicAdd(&info->residual, 1);
-    }
-    if (lane < w) A[k * ld + j0 + lane] = s;
-}
-
-// ------------------------------------------------------------------------------------------
-// S4 row-block solve, base case: X <- L11^{-1} X for nb <= 32 pivots (global pivot indices
-// t0..t0+nb), X = A[t0 : t0+nb, c0 : c0+ncols].  L11[a][b] = A[t0+a][pivcols[t0+b]] (b < a), the
-// diagonal position holds d_a^{-1}.  One thread per column of X, the column kept in shared memory.
-constexpr int TRSM_THREADS = 128;
-__global__ void __launch_bounds__(TRSM_THREADS) trsm_lower_base_kernel(uint32_t* __restrict__ X, int64_t ldx,
-                                                                       int64_t ncols, const uint32_t* __restrict__ A,
-                                                                       int64_t lda, const int32_t* __restrict__ pivcols,
-                                                                       int64_t t0, int nb, ModP f) {
-    __shared__ uint32_t L[PW][PW + 1];
-    __shared__ uint32_t Xs[PW][TRSM_THREADS];
-    const int tid = threadIdx.x;
-    for (int e = tid; e < nb * nb; e += TRSM_THREADS) {
-        const int a = e / nb, b = e % nb;
-        L[a][b] = b <= a ? A[(t0 + a) * lda + pivcols[t0 + b]] : 0;
-    }
-    const int64_t c = (int64_t)blockIdx.x * TRSM_THREADS + tid;
-    const bool on = c < ncols;
-    for (int a = 0; a < nb; ++a) Xs[a][tid] = on ? X[(int64_t)a * ldx + c] : 0;
-    __syncthreads();
-    if (!on) return;
-    for (int a = 0; a < nb; ++a) {
+    if (c >= ncols) return;
+#pragma unroll
+    for (int u = 0; u < PW / 8; ++u) {
+        const int a = g * (PW / 8) + u;
+        if (a >= r) continue;
         uint64_t acc = 0;
-        for (int b = 0; b < a; ++b) {
-            acc += (uint64_t)L[a][b] * Xs[b][tid];
-            if (b & 1) acc = fold64(acc, f);
+#pragma unroll 8
+        for (int b = 0; b < PW; b += 2) {
+            acc += (uint64_t)Ts[a][b] * Xs[b][lane];
+            acc += (uint64_t)Ts[a][b + 1] * Xs[b + 1][lane];
+            acc = fold64(acc, f);
         }
-        const uint32_t v = submod(Xs[a][tid], reduce64(acc, f), f);
-        const uint32_t y = mulmod(v, L[a][a], f);
-        Xs[a][tid] = y;
-        X[(int64_t)a * ldx + c] = y;
-    }
-}
-
-// S6 back-elimination, base case: X <- T^{-1} X, T unit upper triangular nb x nb with
-// T[a][b] = A[t0+a][pivcols[t0+b]] for b > a (the echelon rows' entries above later pivots).
-__global__ void __launch_bounds__(TRSM_THREADS) trsm_upper_base_kernel(uint32_t* __restrict__ X, int64_t ldx,
-                                                                       int64_t ncols, const uint32_t* __restrict__ A,
-                                                                       int64_t lda, const int32_t* __restrict__ pivcols,
-                                                                       int64_t t0, int nb, ModP f) {
-    __shared__ uint32_t T[PW][PW + 1];
-    __shared__ uint32_t Xs[PW][TRSM_THREADS];
-    const int tid = threadIdx.x;
-    for (int e = tid; e < nb * nb; e += TRSM_THREADS) {
-        const int a = e / nb, b = e % nb;
-        T[a][b] = b > a ? A[(t0 + a) * lda + pivcols[t0 + b]] : 0;
-    }
-    const int64_t c = (int64_t)blockIdx.x * TRSM_THREADS + tid;
-    const bool on = c < ncols;
-    for (int a = 0; a < nb; ++a) Xs[a][tid] = on ? X[(int64_t)a * ldx + c] : 0;
-    __syncthreads();
-    if (!on) return;
-    for (int a = nb - 2; a >= 0; --a) {
-        uint64_t acc = 0;
-        for (int b = a + 1; b < nb; ++b) {
-            acc += (uint64_t)T[a][b] * Xs[b][tid];
-            if ((b - a) % 2 == 0) acc = fold64(acc, f);
-        }
-        const uint32_t y = submod(Xs[a][tid], reduce64(acc, f), f);
-        Xs[a][tid] = y;
-        X[(int64_t)a * ldx + c] = y;
+        X[(int64_t)a * ldx + c] = reduce64(acc, f);
     }
 }
 
 // ------------------------------------------------------------------------------------------
-// Free-column gather / scatter for the back-elimination workspace: F[k][t] = A[k][freecols[t]].
+// Free-column gather / scatter for the back-elimination workspace: F[k][t] = A[k][freecols[t]] for
+// k below the column's threshold row (the number of pivots found up to and including the column's
+// panel); rows at or beyond it are mathematically zero there (storage may hold garbage).
 __global__ void gather_cols_kernel(const uint32_t* __restrict__ A, int64_t ld, int64_t nrows,
-                                   const int32_t* __restrict__ colidx, int64_t ncols, uint32_t* __restrict__ F,
-                                   int64_t ldf) {
+                                   const int32_t* __restrict__ colidx, const int32_t* __restrict__ thresh, int64_t ncols,
+                                   uint32_t* __restrict__ F, int64_t ldf) {
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= ncols) return;
     const int64_t c = colidx[t];
-    for (int64_t k = blockIdx.y; k < nrows; k += gridDim.y) F[k * ldf + t] = A[k * ld + c];
+    const int64_t th = thresh[t];
+    for (int64_t k = blockIdx.y; k < nrows; k += gridDim.y) F[k * ldf + t] = k < th ? A[k * ld + c] : 0u;
 }
 __global__ void scatter_cols_kernel(uint32_t* __restrict__ A, int64_t ld, int64_t nrows,
                                     const int32_t* __restrict__ colidx, int64_t ncols, const uint32_t* __restrict__ F,
@@ -304,24 +299,20 @@ __global__ void scatter_cols_kernel(uint32_t* __restrict__ A, int64_t ld, int64_
     for (int64_t k = blockIdx.y; k < nrows; k += gridDim.y) A[k * ld + c] = F[k * ldf + t];
 }
 
-// S7 finalise: every pivot column becomes a unit vector over ALL rows (removes the multipliers
-// and the stored inverses); rows >= rank are zero rows.
-__global__ void finalize_pivot_cols_kernel(uint32_t* __restrict__ A, int64_t ld, int64_t rows,
-                                           const int32_t* __restrict__ pivcols, int64_t rank) {
-    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= rank) return;
-    const int64_t c = pivcols[t];
-    for (int64_t k = blockIdx.y; k < rows; k += gridDim.y) A[k * ld + c] = (k == t) ? 1u : 0u;
-}
-
-// Internal check used by tests: counts non-zeros in rows >= rank (must be 0).
-__global__ void count_nonzero_tail_kernel(const uint32_t* __restrict__ A, int64_t ld, int64_t rows, int64_t cols,
-                                          int64_t rank, unsigned long long* __restrict__ count) {
+// S7 finalise.  colinfo[c] >= 0: column c is the pivot column of pivot t = colinfo[c]; it becomes the
+// unit vector e_t over ALL rows (removes multipliers and raw pivot blocks).  colinfo[c] < 0: free
+// column whose entries in rows >= -(colinfo[c]+1) become 0.  Rows >= rank end up zero.
+__global__ void finalize_kernel(uint32_t* __restrict__ A, int64_t ld, int64_t rows, int64_t cols,
+                                const int32_t* __restrict__ colinfo) {
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= cols) return;
-    unsigned long long n = 0;
-    for (int64_t k = rank + blockIdx.y; k < rows; k += gridDim.y) n += A[k * ld + c] != 0;
-    if (n) atomicAdd(count, n);
+    const int32_t ci = colinfo[c];
+    if (ci >= 0) {
+        for (int64_t k = blockIdx.y; k < rows; k += gridDim.y) A[k * ld + c] = (k == ci) ? 1u : 0u;
+    } else {
+        const int64_t th = -((int64_t)ci + 1);
+        for (int64_t k = th + blockIdx.y; k < rows; k += gridDim.y) A[k * ld + c] = 0u;
+    }
 }
 
 // ------------------------------------------------------------------------------------------

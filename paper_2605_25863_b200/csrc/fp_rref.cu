@@ -1,12 +1,12 @@
 // fp_rref.cu -- host orchestration of the F_p path: linac_rref_u32 / linac_nullspace_u32.
 //
-// Schedule: S0 ingest -> recursive right-looking elimination
-// (base panels of PW columns: pivot kernel + row exchanges + in-place multipliers; above them
-// row-block solves and Schur updates C -= L21.U12 mod p as GEMMs) -> back-elimination of the free
-// columns (blocked unit-upper-triangular solve, again GEMMs) -> finalise (pivot columns become
-// unit vectors).  One small device->host copy per base panel tells the host how many pivots the
-// panel produced; that is the only host involvement (the paper's loop has none, at
-// the price of 8 launches per COLUMN).
+// Schedule: S0 ingest -> recursive right-looking elimination over
+// base panels of PW columns (panel kernel: pivot rows, pivot columns and T = (pivot block)^-1; row
+// exchanges; the multipliers are the stored entries themselves) with row-block solves U12 = T.A12 and
+// Schur updates C -= L21.U12 mod p as GEMMs -> back-elimination of the free columns (blocked
+// unit-upper-triangular solve, again GEMMs) -> finalise.  One small device->host copy per base panel
+// tells the host how many pivots the panel produced; that is the only host involvement (the paper's
+// loop has none, at the price of 8 launches per COLUMN).
 #include <algorithm>
 #include <mutex>
 #include <vector>
@@ -23,19 +23,21 @@ struct Fp {
     int64_t rows, cols, ld;
     ModP f;
     cudaStream_t s;
+    int64_t nb;               // number of base panels = ceil(cols / PW)
     // device metadata
     int32_t* d_pivcols;
-    PanelInfo* d_info;
-    uint32_t* d_E;
+    PanelRec* d_rec;          // [nb]
+    uint32_t* d_T;            // [nb][PW*PW]
+    uint32_t* d_E;            // [nb][PW*PW]
     Arena* arena;
     // host
-    PanelInfo* h_info;        // pinned
+    PanelRec* h_rec;          // pinned, one record
+    std::vector<int64_t> pstart;     // [nb+1] pivots found left of panel b
     std::vector<int32_t> pivcols;
-    int status = LINAC_OK;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
 };
 
-int64_t round_down(int64_t x, int64_t m) { return x / m * m; }
+int64_t panel_col0(int64_t b) { return b * PW; }
 
 int run_gemm(Fp& c, const GemmArgs& g) {
     Options& o = options();
@@ -58,62 +60,75 @@ int run_gemm(Fp& c, const GemmArgs& g) {
     return rc;
 }
 
-// X <- L11^{-1} X for pivots [t0, t0+nb) on columns [c0, c1) of rows t0.. (S4).
-int trsm_lower(Fp& c, int64_t t0, int64_t nb, int64_t c0, int64_t c1) {
-    if (nb <= 0 || c1 <= c0) return LINAC_OK;
-    if (nb <= PW) {
+// X <- L^{-1} X (S4) for the pivots of panels [b0, b1) on columns [c0, c1) of their rows: per base
+// panel X_b <- T_b X_b; between blocks X_bottom -= L[bottom rows, top pivot columns] . X_top.
+int trsm_lower(Fp& c, int64_t b0, int64_t b1, int64_t c0, int64_t c1) {
+    const int64_t t0 = c.pstart[b0], t1 = c.pstart[b1];
+    if (t1 <= t0 || c1 <= c0) return LINAC_OK;
+    if (b1 - b0 == 1) {
         const int64_t ncols = c1 - c0;
-        trsm_lower_base_kernel<<<(unsigned)((ncols + TRSM_THREADS - 1) / TRSM_THREADS), TRSM_THREADS, 0, c.s>>>(
-            c.A + t0 * c.ld + c0, c.ld, ncols, c.A, c.ld, c.d_pivcols, t0, (int)nb, c.f);
+        apply_t_kernel<<<(unsigned)((ncols + PW - 1) / PW), 256, 0, c.s>>>(c.A + t0 * c.ld + c0, c.ld, ncols,
+                                                                           c.d_T + b0 * PW * PW, (int)(t1 - t0), c.f,
+                                                                           nullptr, 0);
         LINAC_CUDA(cudaGetLastError());
         stats().kernel_launches++;
-        stats().update_macs += nb * nb / 2 * ncols;
+        stats().update_macs += (t1 - t0) * (t1 - t0) * ncols;
         return LINAC_OK;
     }
-    const int64_t h = std::max<int64_t>(PW, round_down(nb / 2, PW));
-    int rc = trsm_lower(c, t0, h, c0, c1);
+    const int64_t bh = b0 + (b1 - b0) / 2, th = c.pstart[bh];
+    int rc = trsm_lower(c, b0, bh, c0, c1);
     if (rc) return rc;
-    GemmArgs g{c.A + (t0 + h) * c.ld + c0, c.ld, c.A + (t0 + h) * c.ld, c.ld, c.d_pivcols + t0,
-               c.A + t0 * c.ld + c0,       c.ld, nb - h,                c1 - c0, h};
-    rc = run_gemm(c, g);
-    if (rc) return rc;
-    return trsm_lower(c, t0 + h, nb - h, c0, c1);
+    if (th > t0 && t1 > th) {
+        GemmArgs g{c.A + th * c.ld + c0, c.ld, c.A + th * c.ld, c.ld, c.d_pivcols + t0,
+                   c.A + t0 * c.ld + c0, c.ld, t1 - th,         c1 - c0, th - t0};
+        rc = run_gemm(c, g);
+        if (rc) return rc;
+    }
+    return trsm_lower(c, bh, b1, c0, c1);
 }
 
-// One base panel: columns [j0, j0+w), rows >= i0.  Returns the number of pivots through *r.
-int base_panel(Fp& c, int64_t j0, int w, int64_t i0, int64_t* r) {
-    panel_pivots_kernel<<<1, 256, 0, c.s>>>(c.A, c.ld, c.rows, i0, j0, w, c.f, c.d_info, c.d_E, c.d_pivcols);
+// One base panel b with active rows >= i0.  Returns the number of pivots through *r.
+int base_panel(Fp& c, int64_t b, int64_t i0, int64_t* r) {
+    const int64_t j0 = panel_col0(b);
+    const int w = (int)std::min<int64_t>(PW, c.cols - j0);
+    panel_factor_kernel<<<1, 256, 0, c.s>>>(c.A, c.ld, c.rows, i0, j0, w, c.f, c.d_rec + b, c.d_T + b * PW * PW,
+                                            c.d_E + b * PW * PW, c.d_pivcols, nullptr, (int)b);
     LINAC_CUDA(cudaGetLastError());
-    apply_swaps_kernel<<<(unsigned)((c.cols + 255) / 256), 256, 0, c.s>>>(c.A, c.ld, c.cols, i0, c.d_info);
+    panel_finish_kernel<<<(unsigned)((c.cols + 255) / 256), 256, 0, c.s>>>(c.A, c.ld, c.cols, i0, j0, c.d_rec + b,
+                                                                          c.d_E + b * PW * PW, nullptr, (int)b);
     LINAC_CUDA(cudaGetLastError());
-    const int64_t nrows = c.rows - i0;
-    panel_apply_kernel<<<(unsigned)((nrows + 7) / 8), 256, 0, c.s>>>(c.A, c.ld, c.rows, i0, j0, w, c.f, c.d_info, c.d_E);
-    LINAC_CUDA(cudaGetLastError());
-    LINAC_CUDA(cudaMemcpyAsync(c.h_info, c.d_info, sizeof(PanelInfo), cudaMemcpyDeviceToHost, c.s));
+    LINAC_CUDA(cudaMemcpyAsync(c.h_rec, c.d_rec + b, sizeof(PanelRec), cudaMemcpyDeviceToHost, c.s));
     LINAC_CUDA(cudaStreamSynchronize(c.s));
     linac_stats& st = stats();
-    st.kernel_launches += 3;
+    st.kernel_launches += 2;
     st.host_syncs++;
     st.panels++;
-    st.row_swaps += c.h_info->nswaps;
-    st.residual_nonzero += c.h_info->residual;
-    *r = c.h_info->r;
-    for (int a = 0; a < c.h_info->r; ++a) c.pivcols[i0 + a] = (int32_t)(j0 + c.h_info->pc[a]);
+    st.row_swaps += c.h_rec->nswaps;
+    *r = c.h_rec->r;
+    for (int a = 0; a < c.h_rec->r; ++a) c.pivcols[i0 + a] = (int32_t)(j0 + c.h_rec->pc[a]);
     return LINAC_OK;
 }
 
-// Recursive factorisation of columns [j0, j1) with active rows [i0, rows).
-int factor(Fp& c, int64_t j0, int64_t j1, int64_t i0, int64_t* r_out) {
-    const int64_t w = j1 - j0;
+// Recursive factorisation of panels [b0, b1) with active rows [i0, rows).  Fills pstart[b0+1 .. b1].
+int factor(Fp& c, int64_t b0, int64_t b1, int64_t i0, int64_t* r_out) {
     *r_out = 0;
-    if (w <= 0 || i0 >= c.rows) return LINAC_OK;
-    if (w <= PW) return base_panel(c, j0, (int)w, i0, r_out);
-    const int64_t jm = j0 + std::max<int64_t>(PW, round_down(w / 2, PW));
+    if (b1 <= b0) return LINAC_OK;
+    if (i0 >= c.rows) {                              // no rows left: every remaining column is free
+        for (int64_t b = b0; b < b1; ++b) c.pstart[b + 1] = i0;
+        return LINAC_OK;
+    }
+    if (b1 - b0 == 1) {
+        int rc = base_panel(c, b0, i0, r_out);
+        c.pstart[b0 + 1] = i0 + *r_out;
+        return rc;
+    }
+    const int64_t bm = b0 + (b1 - b0) / 2;
+    const int64_t jm = panel_col0(bm), j1 = std::min(c.cols, panel_col0(b1));
     int64_t r1 = 0, r2 = 0;
-    int rc = factor(c, j0, jm, i0, &r1);
+    int rc = factor(c, b0, bm, i0, &r1);
     if (rc) return rc;
     if (r1 > 0) {
-        rc = trsm_lower(c, i0, r1, jm, j1);
+        rc = trsm_lower(c, b0, bm, jm, j1);
         if (rc) return rc;
         const int64_t m2 = c.rows - (i0 + r1);
         if (m2 > 0) {
@@ -123,35 +138,34 @@ int factor(Fp& c, int64_t j0, int64_t j1, int64_t i0, int64_t* r_out) {
             if (rc) return rc;
         }
     }
-    rc = factor(c, jm, j1, i0 + r1, &r2);
+    rc = factor(c, bm, b1, i0 + r1, &r2);
     *r_out = r1 + r2;
     return rc;
 }
 
-// X <- T^{-1} X on the gathered free columns F (rank x nf, ldf), pivots [t0, t0+nb) (S6).
-int trsm_upper(Fp& c, uint32_t* F, int64_t ldf, int64_t nf, int64_t t0, int64_t nb) {
-    if (nb <= 0 || nf <= 0) return LINAC_OK;
-    if (nb <= PW) {
-        trsm_upper_base_kernel<<<(unsigned)((nf + TRSM_THREADS - 1) / TRSM_THREADS), TRSM_THREADS, 0, c.s>>>(
-            F + t0 * ldf, ldf, nf, c.A, c.ld, c.d_pivcols, t0, (int)nb, c.f);
-        LINAC_CUDA(cudaGetLastError());
-        stats().kernel_launches++;
-        stats().update_macs += nb * nb / 2 * nf;
-        return LINAC_OK;
+// X <- T^{-1} X on the gathered free columns F (rank x nf, ldf) for the pivots of panels [b0, b1) (S6).
+// T = U[pivot rows, pivot columns] is unit upper triangular and the identity inside one base panel.
+int trsm_upper(Fp& c, uint32_t* F, int64_t ldf, int64_t nf, int64_t b0, int64_t b1) {
+    const int64_t t0 = c.pstart[b0], t1 = c.pstart[b1];
+    if (t1 <= t0 || nf <= 0 || b1 - b0 <= 1) return LINAC_OK;
+    const int64_t bh = b0 + (b1 - b0) / 2, th = c.pstart[bh];
+    int rc = trsm_upper(c, F, ldf, nf, bh, b1);
+    if (rc) return rc;
+    if (th > t0 && t1 > th) {
+        // X_top -= U[top rows, bottom pivot columns] . X_bottom
+        GemmArgs g{F + t0 * ldf, ldf, c.A + t0 * c.ld, c.ld, c.d_pivcols + th, F + th * ldf, ldf, th - t0, nf, t1 - th};
+        rc = run_gemm(c, g);
+        if (rc) return rc;
     }
-    const int64_t h = std::max<int64_t>(PW, round_down(nb / 2, PW));   // top block [t0, t0+h), bottom the rest
-    int rc = trsm_upper(c, F, ldf, nf, t0 + h, nb - h);
-    if (rc) return rc;
-    // X_top -= T[top, bottom pivots] . X_bottom
-    GemmArgs g{F + t0 * ldf, ldf, c.A + t0 * c.ld, c.ld, c.d_pivcols + t0 + h, F + (t0 + h) * ldf, ldf, h, nf, nb - h};
-    rc = run_gemm(c, g);
-    if (rc) return rc;
-    return trsm_upper(c, F, ldf, nf, t0, h);
+    return trsm_upper(c, F, ldf, nf, b0, bh);
 }
+
+int64_t num_panels(int64_t cols) { return (cols + PW - 1) / PW; }
 
 size_t meta_bytes(int64_t rows, int64_t cols) {
     const int64_t mn = std::max<int64_t>(1, std::min(rows, cols));
-    return 4096 + sizeof(PanelInfo) + PW * PW * 4 + (size_t)mn * 4 + (size_t)cols * 8 + 8 * 256;
+    const int64_t nb = num_panels(cols);
+    return 8192 + (size_t)nb * (sizeof(PanelRec) + 256 + 2 * PW * PW * 4) + (size_t)mn * 4 + (size_t)cols * 4 + 8 * 256;
 }
 
 // Free-column slab width for the back-elimination workspace.
@@ -163,27 +177,26 @@ int64_t backelim_slab(int64_t rows, int64_t cols) {
 size_t workspace_bytes(int64_t rows, int64_t cols) {
     const int64_t mn = std::max<int64_t>(1, std::min(rows, cols));
     size_t b = meta_bytes(rows, cols);
-    b += (size_t)mn * (size_t)backelim_slab(rows, cols) * 4 + 256;          // gathered free columns
+    b += (size_t)mn * (size_t)backelim_slab(rows, cols) * 4 + 2 * (size_t)backelim_slab(rows, cols) * 4 + 1024;   // gathered free columns
     b += gemm_modp_tc_scratch_bytes(rows, cols, std::min<int64_t>(mn, 4096)) + 256;
     return b;
 }
 
-struct PinnedInfo {
-    PanelInfo* p = nullptr;
-    ~PinnedInfo() { if (p) cudaFreeHost(p); }
+struct PinnedRec {
+    PanelRec* p = nullptr;
+    ~PinnedRec() { if (p) cudaFreeHost(p); }
 };
 
 int validate(const uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p) {
-    if (rows < 0 || cols < 0 || cols >= (1ll << 31) || rows >= (1ll << 40)) return LINAC_ERR_INVALID_ARG;
+    if (rows < 0 || cols < 0 || cols >= (1ll << 31) || rows >= (1ll << 31)) return LINAC_ERR_INVALID_ARG;
     if (rows > 0 && cols > 0 && (dA == nullptr || ld < cols)) return LINAC_ERR_INVALID_ARG;
     if (p < 2 || p >= (1u << 31) || !is_prime_u32(p)) return LINAC_ERR_BAD_MODULUS;
     return LINAC_OK;
 }
 
-// The whole reduction.  On success the device arrays d_pivcols (in the arena) stay valid until the
-// arena is reused, which linac_nullspace_u32 relies on.
+// The whole reduction.
 int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, cudaStream_t s, int64_t* rank,
-              int32_t* pivot_cols_out, Arena* arena, int32_t** d_pivcols_out) {
+              int32_t* pivot_cols_out, Arena* arena) {
     linac_stats& st = stats();
     st = linac_stats{};
     int rc = validate(dA, rows, cols, ld, p);
@@ -196,18 +209,22 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     rc = acquire_workspace(workspace_bytes(rows, cols), arena);
     if (rc) return rc;
 
-    static PinnedInfo pinned;
-    if (!pinned.p) LINAC_CUDA(cudaMallocHost(&pinned.p, sizeof(PanelInfo)));
+    static PinnedRec pinned;
+    if (!pinned.p) LINAC_CUDA(cudaMallocHost(&pinned.p, sizeof(PanelRec)));
 
     Fp c;
     c.A = dA; c.rows = rows; c.cols = cols; c.ld = ld; c.f = make_modp(p); c.s = s; c.arena = arena;
+    c.nb = num_panels(cols);
     const int64_t mn = std::min(rows, cols);
-    c.d_info = (PanelInfo*)arena->take(sizeof(PanelInfo));
-    c.d_E = (uint32_t*)arena->take(PW * PW * 4);
+    c.d_rec = (PanelRec*)arena->take((size_t)c.nb * sizeof(PanelRec));
+    c.d_T = (uint32_t*)arena->take((size_t)c.nb * PW * PW * 4);
+    c.d_E = (uint32_t*)arena->take((size_t)c.nb * PW * PW * 4);
     c.d_pivcols = (int32_t*)arena->take((size_t)mn * 4);
-    if (!c.d_info || !c.d_E || !c.d_pivcols) return LINAC_ERR_WORKSPACE;
-    c.h_info = pinned.p;
+    int32_t* d_colinfo = (int32_t*)arena->take((size_t)cols * 4);
+    if (!c.d_rec || !c.d_T || !c.d_E || !c.d_pivcols || !d_colinfo) return LINAC_ERR_WORKSPACE;
+    c.h_rec = pinned.p;
     c.pivcols.assign(mn, -1);
+    c.pstart.assign(c.nb + 1, 0);
     LINAC_CUDA(cudaEventCreate(&c.ev0));
     LINAC_CUDA(cudaEventCreate(&c.ev1));
     cudaEvent_t t0, t1;
@@ -224,40 +241,47 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     }
     // forward elimination
     int64_t r = 0;
-    rc = factor(c, 0, cols, 0, &r);
-    if (rc == LINAC_OK && st.residual_nonzero != 0) rc = LINAC_ERR_INTERNAL;
+    rc = factor(c, 0, c.nb, 0, &r);
+    // column classification: pivot index, or the threshold row of a free column
+    std::vector<int32_t> colinfo(cols);
+    std::vector<int32_t> freec, freeth;
+    if (rc == LINAC_OK) {
+        for (int64_t b = 0; b < c.nb; ++b) {
+            const int64_t j0 = panel_col0(b), j1 = std::min(cols, j0 + PW);
+            for (int64_t cc = j0; cc < j1; ++cc) colinfo[cc] = -(int32_t)c.pstart[b + 1] - 1;
+        }
+        for (int64_t t = 0; t < r; ++t) colinfo[c.pivcols[t]] = (int32_t)t;
+        for (int64_t cc = r > 0 ? c.pivcols[0] : cols; cc < cols; ++cc)   // free columns left of the first pivot are all zero
+            if (colinfo[cc] < 0) { freec.push_back((int32_t)cc); freeth.push_back(-(colinfo[cc] + 1)); }
+    }
     // S6 back-elimination of the free columns, a slab at a time
-    if (rc == LINAC_OK && r > 0 && r < cols) {
-        std::vector<char> is_piv(cols, 0);
-        for (int64_t t = 0; t < r; ++t) is_piv[c.pivcols[t]] = 1;
-        std::vector<int32_t> freec;
-        for (int64_t cc = c.pivcols[0]; cc < cols; ++cc)   // free columns left of the first pivot are all zero
-            if (!is_piv[cc]) freec.push_back((int32_t)cc);
+    if (rc == LINAC_OK && r > 0 && !freec.empty()) {
         const int64_t slab = backelim_slab(rows, cols);
         int32_t* d_free = (int32_t*)arena->take((size_t)std::max<int64_t>(1, slab) * 4);
+        int32_t* d_th = (int32_t*)arena->take((size_t)std::max<int64_t>(1, slab) * 4);
         uint32_t* F = (uint32_t*)arena->take((size_t)r * (size_t)slab * 4);
-        if (!d_free || !F) rc = LINAC_ERR_WORKSPACE;
+        if (!d_free || !d_th || !F) rc = LINAC_ERR_WORKSPACE;
         for (size_t f0 = 0; rc == LINAC_OK && f0 < freec.size(); f0 += (size_t)slab) {
             const int64_t nf = (int64_t)std::min<size_t>((size_t)slab, freec.size() - f0);
-            // only pivots whose column lies left of the slab's last free column can be affected
             LINAC_CUDA(cudaMemcpyAsync(d_free, freec.data() + f0, (size_t)nf * 4, cudaMemcpyHostToDevice, s));
+            LINAC_CUDA(cudaMemcpyAsync(d_th, freeth.data() + f0, (size_t)nf * 4, cudaMemcpyHostToDevice, s));
             dim3 grid((unsigned)((nf + 255) / 256), (unsigned)std::min<int64_t>(r, 1024));
-            gather_cols_kernel<<<grid, 256, 0, s>>>(dA, ld, r, d_free, nf, F, nf);
+            gather_cols_kernel<<<grid, 256, 0, s>>>(dA, ld, r, d_free, d_th, nf, F, nf);
             LINAC_CUDA(cudaGetLastError());
-            rc = trsm_upper(c, F, nf, nf, 0, r);
+            rc = trsm_upper(c, F, nf, nf, 0, c.nb);
             if (rc) break;
             scatter_cols_kernel<<<grid, 256, 0, s>>>(dA, ld, r, d_free, nf, F, nf);
             LINAC_CUDA(cudaGetLastError());
-            LINAC_CUDA(cudaStreamSynchronize(s));   // freec slab (pageable host memory) is reused next round
+            LINAC_CUDA(cudaStreamSynchronize(s));   // the host staging vectors are pageable memory
             st.kernel_launches += 2;
             st.host_syncs++;
         }
     }
     // S7 finalise
-    if (rc == LINAC_OK && r > 0) {
-        LINAC_CUDA(cudaMemcpyAsync(c.d_pivcols, c.pivcols.data(), (size_t)r * 4, cudaMemcpyHostToDevice, s));
-        dim3 grid((unsigned)((r + 255) / 256), (unsigned)std::min<int64_t>(rows, 1024));
-        finalize_pivot_cols_kernel<<<grid, 256, 0, s>>>(dA, ld, rows, c.d_pivcols, r);
+    if (rc == LINAC_OK) {
+        LINAC_CUDA(cudaMemcpyAsync(d_colinfo, colinfo.data(), (size_t)cols * 4, cudaMemcpyHostToDevice, s));
+        dim3 grid((unsigned)((cols + 255) / 256), (unsigned)std::min<int64_t>(rows, 1024));
+        finalize_kernel<<<grid, 256, 0, s>>>(dA, ld, rows, cols, d_colinfo);
         LINAC_CUDA(cudaGetLastError());
         st.kernel_launches++;
     }
@@ -273,7 +297,6 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     if (rc) return rc;
     *rank = r;
     if (pivot_cols_out) std::copy(c.pivcols.begin(), c.pivcols.begin() + r, pivot_cols_out);
-    if (d_pivcols_out) *d_pivcols_out = c.d_pivcols;
     return LINAC_OK;
 }
 
@@ -325,7 +348,7 @@ int linac_rref_u32(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_
                    int32_t* pivot_cols_out) {
     std::lock_guard<std::mutex> lock(g_call_mutex);
     Arena arena;
-    return rref_impl(dA, rows, cols, ld, p, (cudaStream_t)stream, rank, pivot_cols_out, &arena, nullptr);
+    return rref_impl(dA, rows, cols, ld, p, (cudaStream_t)stream, rank, pivot_cols_out, &arena);
 }
 
 int linac_nullspace_u32(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, void* stream, int64_t* rank,
@@ -336,7 +359,7 @@ int linac_nullspace_u32(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, ui
     Arena arena;
     std::vector<int32_t> piv((size_t)std::max<int64_t>(1, std::min(rows, cols)));
     int64_t r = 0;
-    int rc = rref_impl(dA, rows, cols, ld, p, (cudaStream_t)stream, &r, piv.data(), &arena, nullptr);
+    int rc = rref_impl(dA, rows, cols, ld, p, (cudaStream_t)stream, &r, piv.data(), &arena);
     if (rc) return rc;
     if (rank) *rank = r;
     *nullity = cols - r;

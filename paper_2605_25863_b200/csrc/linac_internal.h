@@ -11,16 +11,17 @@
 namespace linac {
 
 constexpr int PW = 32;   // base panel width (columns factored by one panel kernel)
-constexpr int CH = 64;   // rows per chunk scanned by the pivot kernel
+constexpr int CH = 32;   // rows per chunk scanned by the panel kernel
 
-// What the pivot kernel reports for one base panel (device -> pinned host, one small copy).
-struct PanelInfo {
-    int32_t r;               // pivots found in this panel (<= width)
+// What the panel kernel reports for one base panel (kept on the device per panel; the host reads it
+// with one small copy when it needs the pivot count).
+struct PanelRec {
+    int32_t r;               // pivots found in this panel (<= w)
     int32_t nswaps;          // how many of swp[] are real exchanges
-    int32_t pc[PW];          // local pivot columns, ascending
-    int64_t swp[PW];         // LAPACK-style: at step a exchange rows (i0+a) and swp[a] (>= i0+a)
-    int32_t residual;        // internal check, must stay 0
+    int32_t w;               // panel width
     int32_t pad;
+    int32_t pc[PW];          // local pivot columns, ascending (-1 beyond r)
+    int64_t swp[PW];         // LAPACK-style: at step a exchange rows (i0+a) and swp[a] (>= i0+a)
 };
 
 // Error plumbing: first failing CUDA call wins; text kept for linac_last_cuda_error().
