@@ -144,7 +144,8 @@ typedef struct {
     double  ms_total;            /* device ms of the whole call, if timed                         */
 } linac_stats;
 int linac_get_last_stats(linac_stats *out);
-/* Tunables, mainly for A/B measurements: name in {"gemm_path" (0 auto, 1 CUDA-core, 2 tensor), "timing" (0/1), "tc_min_k", "tc_min_mn"}.
+/* Tunables, mainly for A/B measurements: name in {"gemm_path" (0 auto, 1 CUDA-core, 2 tensor), "timing" (0/1), "tc_min_k", "tc_min_mn",
+ * "strip_width" (columns per cooperative strip kernel: 32..256, multiple of 32)}.
  * Returns LINAC_ERR_INVALID_ARG for unknown names / out-of-range values. */
 int linac_set_option(const char *name, int64_t value);
 

@@ -1,17 +1,20 @@
 // fp_rref.cu -- host orchestration of the F_p path: linac_rref_u32 / linac_nullspace_u32.
 //
 // Schedule: S0 ingest -> recursive right-looking elimination over
-// base panels of PW columns (panel kernel: pivot rows, pivot columns and T = (pivot block)^-1; row
-// exchanges; the multipliers are the stored entries themselves) with row-block solves U12 = T.A12 and
-// Schur updates C -= L21.U12 mod p as GEMMs -> back-elimination of the free columns (blocked
-// unit-upper-triangular solve, again GEMMs) -> finalise.  One small device->host copy per base panel
-// tells the host how many pivots the panel produced; that is the only host involvement (the paper's
-// loop has none, at the price of 8 launches per COLUMN).
+// STRIPS of `strip_width` columns.  One cooperative kernel factors a strip (fp_strip.cuh: pivot rows,
+// pivot columns and T = (pivot block)^-1 per 32-column base panel, row exchanges, the in-strip updates;
+// the multipliers are the stored entries themselves); between strips the row-block solves U12 = L11^-1 A12
+// (column-parallel leaf kernel per strip, GEMMs between strips) and the Schur updates C -= L21.U12 mod p
+// (tensor-core GEMMs) -> back-elimination of the free columns (blocked unit-upper-triangular solve with
+// the same leaf kernel and GEMMs) -> finalise.  One small device->host copy per STRIP tells the host how
+// many pivots it produced; that is the only host involvement (the paper's loop has none, at
+// the price of 8 launches per COLUMN).
 #include <algorithm>
 #include <mutex>
 #include <vector>
 
 #include "fp_kernels.cuh"
+#include "fp_strip.cuh"
 
 namespace linac {
 extern std::mutex g_call_mutex;
@@ -24,17 +27,24 @@ struct Fp {
     ModP f;
     cudaStream_t s;
     int64_t nb;               // number of base panels = ceil(cols / PW)
+    int64_t bps;              // base panels per strip
+    int64_t ns;               // number of strips
+    int coop_grid;            // CTAs of the cooperative strip kernel
     // device metadata
     int32_t* d_pivcols;
+    int32_t* d_pstart;        // [nb+1]
     PanelRec* d_rec;          // [nb]
     uint32_t* d_T;            // [nb][PW*PW]
     uint32_t* d_E;            // [nb][PW*PW]
     Arena* arena;
     // host
-    PanelRec* h_rec;          // pinned, one record
-    std::vector<int64_t> pstart;     // [nb+1] pivots found left of panel b
+    PanelRec* h_rec;          // pinned, MAXBP records
+    std::vector<int64_t> pstart;     // [nb+1] pivots found left of base panel b
     std::vector<int32_t> pivcols;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+
+    int64_t sb0(int64_t s) const { return std::min(nb, s * bps); }          // first base panel of strip s
+    int64_t sp(int64_t s) const { return pstart[sb0(s)]; }                  // pivots found left of strip s
 };
 
 int64_t panel_col0(int64_t b) { return b * PW; }
@@ -60,23 +70,30 @@ int run_gemm(Fp& c, const GemmArgs& g) {
     return rc;
 }
 
-// X <- L^{-1} X (S4) for the pivots of panels [b0, b1) on columns [c0, c1) of their rows: per base
-// panel X_b <- T_b X_b; between blocks X_bottom -= L[bottom rows, top pivot columns] . X_top.
-int trsm_lower(Fp& c, int64_t b0, int64_t b1, int64_t c0, int64_t c1) {
-    const int64_t t0 = c.pstart[b0], t1 = c.pstart[b1];
+size_t trsm_smem_bytes(int64_t K) { return (size_t)K * PW * 4 + (size_t)PW * (PW + 1) * 4; }
+
+// Leaf of both triangular solves: the pivots of ONE strip against columns [0, ncols) of X.
+template <bool LOWER>
+int trsm_leaf(Fp& c, int64_t s, uint32_t* X, int64_t ldx, int64_t ncols) {
+    const int64_t K = c.sp(s + 1) - c.sp(s);
+    if (K <= 0 || ncols <= 0) return LINAC_OK;
+    if (!LOWER && c.sb0(s + 1) - c.sb0(s) <= 1) return LINAC_OK;     // U is the identity inside one base panel
+    trsm_strip_kernel<LOWER><<<(unsigned)((ncols + PW - 1) / PW), TNT, trsm_smem_bytes(K), c.s>>>(
+        c.A, c.ld, X, ldx, ncols, c.d_pstart, (int)c.sb0(s), (int)c.sb0(s + 1), c.d_T, c.d_pivcols, c.f);
+    LINAC_CUDA(cudaGetLastError());
+    stats().kernel_launches++;
+    stats().update_macs += K * K / 2 * ncols;
+    return LINAC_OK;
+}
+
+// X <- L^{-1} X (S4) for the pivots of strips [s0, s1) on columns [c0, c1) of their rows: leaf kernel per
+// strip; between blocks X_bottom -= L[bottom rows, top pivot columns] . X_top.
+int trsm_lower(Fp& c, int64_t s0, int64_t s1, int64_t c0, int64_t c1) {
+    const int64_t t0 = c.sp(s0), t1 = c.sp(s1);
     if (t1 <= t0 || c1 <= c0) return LINAC_OK;
-    if (b1 - b0 == 1) {
-        const int64_t ncols = c1 - c0;
-        apply_t_kernel<<<(unsigned)((ncols + PW - 1) / PW), 256, 0, c.s>>>(c.A + t0 * c.ld + c0, c.ld, ncols,
-                                                                           c.d_T + b0 * PW * PW, (int)(t1 - t0), c.f,
-                                                                           nullptr, 0);
-        LINAC_CUDA(cudaGetLastError());
-        stats().kernel_launches++;
-        stats().update_macs += (t1 - t0) * (t1 - t0) * ncols;
-        return LINAC_OK;
-    }
-    const int64_t bh = b0 + (b1 - b0) / 2, th = c.pstart[bh];
-    int rc = trsm_lower(c, b0, bh, c0, c1);
+    if (s1 - s0 == 1) return trsm_leaf<true>(c, s0, c.A + t0 * c.ld + c0, c.ld, c1 - c0);
+    const int64_t sh = s0 + (s1 - s0) / 2, th = c.sp(sh);
+    int rc = trsm_lower(c, s0, sh, c0, c1);
     if (rc) return rc;
     if (th > t0 && t1 > th) {
         GemmArgs g{c.A + th * c.ld + c0, c.ld, c.A + th * c.ld, c.ld, c.d_pivcols + t0,
@@ -84,51 +101,57 @@ int trsm_lower(Fp& c, int64_t b0, int64_t b1, int64_t c0, int64_t c1) {
         rc = run_gemm(c, g);
         if (rc) return rc;
     }
-    return trsm_lower(c, bh, b1, c0, c1);
+    return trsm_lower(c, sh, s1, c0, c1);
 }
 
-// One base panel b with active rows >= i0.  Returns the number of pivots through *r.
-int base_panel(Fp& c, int64_t b, int64_t i0, int64_t* r) {
-    const int64_t j0 = panel_col0(b);
-    const int w = (int)std::min<int64_t>(PW, c.cols - j0);
-    panel_factor_kernel<<<1, 256, 0, c.s>>>(c.A, c.ld, c.rows, i0, j0, w, c.f, c.d_rec + b, c.d_T + b * PW * PW,
-                                            c.d_E + b * PW * PW, c.d_pivcols, nullptr, (int)b);
-    LINAC_CUDA(cudaGetLastError());
-    panel_finish_kernel<<<(unsigned)((c.cols + 255) / 256), 256, 0, c.s>>>(c.A, c.ld, c.cols, i0, j0, c.d_rec + b,
-                                                                          c.d_E + b * PW * PW, nullptr, (int)b);
-    LINAC_CUDA(cudaGetLastError());
-    LINAC_CUDA(cudaMemcpyAsync(c.h_rec, c.d_rec + b, sizeof(PanelRec), cudaMemcpyDeviceToHost, c.s));
+// One strip s with active rows >= i0 (one cooperative launch).  Returns the number of pivots through *r.
+int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r) {
+    const int64_t b0 = c.sb0(s), b1 = c.sb0(s + 1);
+    const int64_t j0 = panel_col0(b0), j1 = std::min(c.cols, panel_col0(b1));
+    StripArgs a;
+    a.A = c.A; a.ld = c.ld; a.rows = c.rows; a.cols = c.cols; a.i0 = i0; a.j0 = j0; a.ws = (int)(j1 - j0); a.f = c.f;
+    a.rec = c.d_rec; a.T = c.d_T; a.E = c.d_E; a.pivcols = c.d_pivcols; a.pstart = c.d_pstart;
+    void* args[] = {&a};
+    LINAC_CUDA(cudaLaunchCooperativeKernel((void*)strip_factor_kernel, dim3((unsigned)c.coop_grid), dim3(SNT), args,
+                                           sizeof(StripSmem), c.s));
+    LINAC_CUDA(cudaMemcpyAsync(c.h_rec, c.d_rec + b0, (size_t)(b1 - b0) * sizeof(PanelRec), cudaMemcpyDeviceToHost, c.s));
     LINAC_CUDA(cudaStreamSynchronize(c.s));
     linac_stats& st = stats();
-    st.kernel_launches += 2;
+    st.kernel_launches++;
     st.host_syncs++;
-    st.panels++;
-    st.row_swaps += c.h_rec->nswaps;
-    *r = c.h_rec->r;
-    for (int a = 0; a < c.h_rec->r; ++a) c.pivcols[i0 + a] = (int32_t)(j0 + c.h_rec->pc[a]);
+    int64_t cur = i0;
+    for (int64_t b = b0; b < b1; ++b) {
+        const PanelRec& h = c.h_rec[b - b0];
+        if (h.r < 0 || h.r > PW || cur + h.r > c.rows) return LINAC_ERR_INTERNAL;
+        st.panels++;
+        st.row_swaps += h.r > 0 ? h.nswaps : 0;
+        for (int q = 0; q < h.r; ++q) c.pivcols[cur + q] = (int32_t)(panel_col0(b) + h.pc[q]);
+        cur += h.r;
+        c.pstart[b + 1] = cur;
+    }
+    *r = cur - i0;
     return LINAC_OK;
 }
 
-// Recursive factorisation of panels [b0, b1) with active rows [i0, rows).  Fills pstart[b0+1 .. b1].
-int factor(Fp& c, int64_t b0, int64_t b1, int64_t i0, int64_t* r_out) {
+// Recursive factorisation of strips [s0, s1) with active rows [i0, rows).  Fills pstart for their panels.
+int factor(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t* r_out) {
     *r_out = 0;
-    if (b1 <= b0) return LINAC_OK;
+    if (s1 <= s0) return LINAC_OK;
     if (i0 >= c.rows) {                              // no rows left: every remaining column is free
-        for (int64_t b = b0; b < b1; ++b) c.pstart[b + 1] = i0;
+        for (int64_t b = c.sb0(s0); b < c.sb0(s1); ++b) c.pstart[b + 1] = i0;
+        std::vector<int32_t> fill((size_t)(c.sb0(s1) - c.sb0(s0)), (int32_t)i0);
+        LINAC_CUDA(cudaMemcpyAsync(c.d_pstart + c.sb0(s0) + 1, fill.data(), fill.size() * 4, cudaMemcpyHostToDevice, c.s));
+        LINAC_CUDA(cudaStreamSynchronize(c.s));      // `fill` is pageable and dies here
         return LINAC_OK;
     }
-    if (b1 - b0 == 1) {
-        int rc = base_panel(c, b0, i0, r_out);
-        c.pstart[b0 + 1] = i0 + *r_out;
-        return rc;
-    }
-    const int64_t bm = b0 + (b1 - b0) / 2;
-    const int64_t jm = panel_col0(bm), j1 = std::min(c.cols, panel_col0(b1));
+    if (s1 - s0 == 1) return factor_strip(c, s0, i0, r_out);
+    const int64_t sm = s0 + (s1 - s0) / 2;
+    const int64_t jm = panel_col0(c.sb0(sm)), j1 = std::min(c.cols, panel_col0(c.sb0(s1)));
     int64_t r1 = 0, r2 = 0;
-    int rc = factor(c, b0, bm, i0, &r1);
+    int rc = factor(c, s0, sm, i0, &r1);
     if (rc) return rc;
     if (r1 > 0) {
-        rc = trsm_lower(c, b0, bm, jm, j1);
+        rc = trsm_lower(c, s0, sm, jm, j1);
         if (rc) return rc;
         const int64_t m2 = c.rows - (i0 + r1);
         if (m2 > 0) {
@@ -138,18 +161,19 @@ int factor(Fp& c, int64_t b0, int64_t b1, int64_t i0, int64_t* r_out) {
             if (rc) return rc;
         }
     }
-    rc = factor(c, bm, b1, i0 + r1, &r2);
+    rc = factor(c, sm, s1, i0 + r1, &r2);
     *r_out = r1 + r2;
     return rc;
 }
 
-// X <- T^{-1} X on the gathered free columns F (rank x nf, ldf) for the pivots of panels [b0, b1) (S6).
-// T = U[pivot rows, pivot columns] is unit upper triangular and the identity inside one base panel.
-int trsm_upper(Fp& c, uint32_t* F, int64_t ldf, int64_t nf, int64_t b0, int64_t b1) {
-    const int64_t t0 = c.pstart[b0], t1 = c.pstart[b1];
-    if (t1 <= t0 || nf <= 0 || b1 - b0 <= 1) return LINAC_OK;
-    const int64_t bh = b0 + (b1 - b0) / 2, th = c.pstart[bh];
-    int rc = trsm_upper(c, F, ldf, nf, bh, b1);
+// X <- T^{-1} X on the gathered free columns F (rank x nf, ldf) for the pivots of strips [s0, s1) (S6).
+// T = U[pivot rows, pivot columns] is unit upper triangular.
+int trsm_upper(Fp& c, uint32_t* F, int64_t ldf, int64_t nf, int64_t s0, int64_t s1) {
+    const int64_t t0 = c.sp(s0), t1 = c.sp(s1);
+    if (t1 <= t0 || nf <= 0) return LINAC_OK;
+    if (s1 - s0 == 1) return trsm_leaf<false>(c, s0, F + t0 * ldf, ldf, nf);
+    const int64_t sh = s0 + (s1 - s0) / 2, th = c.sp(sh);
+    int rc = trsm_upper(c, F, ldf, nf, sh, s1);
     if (rc) return rc;
     if (th > t0 && t1 > th) {
         // X_top -= U[top rows, bottom pivot columns] . X_bottom
@@ -157,7 +181,23 @@ int trsm_upper(Fp& c, uint32_t* F, int64_t ldf, int64_t nf, int64_t b0, int64_t 
         rc = run_gemm(c, g);
         if (rc) return rc;
     }
-    return trsm_upper(c, F, ldf, nf, b0, bh);
+    return trsm_upper(c, F, ldf, nf, s0, sh);
+}
+
+// Grid of the cooperative strip kernel: every CTA must be resident (one per SM with 1024 threads).
+int strip_grid(int* grid) {
+    static int cached = 0;
+    if (!cached) {
+        LINAC_CUDA(cudaFuncSetAttribute(strip_factor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(StripSmem)));
+        int dev = 0, sms = 0, per_sm = 0;
+        LINAC_CUDA(cudaGetDevice(&dev));
+        LINAC_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        LINAC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, strip_factor_kernel, SNT, sizeof(StripSmem)));
+        if (per_sm < 1 || sms < 1) return LINAC_ERR_INTERNAL;
+        cached = sms;                                 // one CTA per SM: more would only lengthen the grid barrier
+    }
+    *grid = cached;
+    return LINAC_OK;
 }
 
 int64_t num_panels(int64_t cols) { return (cols + PW - 1) / PW; }
@@ -165,7 +205,7 @@ int64_t num_panels(int64_t cols) { return (cols + PW - 1) / PW; }
 size_t meta_bytes(int64_t rows, int64_t cols) {
     const int64_t mn = std::max<int64_t>(1, std::min(rows, cols));
     const int64_t nb = num_panels(cols);
-    return 8192 + (size_t)nb * (sizeof(PanelRec) + 256 + 2 * PW * PW * 4) + (size_t)mn * 4 + (size_t)cols * 4 + 8 * 256;
+    return 8192 + (size_t)nb * (sizeof(PanelRec) + 256 + 2 * PW * PW * 4 + 4) + (size_t)mn * 4 + (size_t)cols * 4 + 10 * 256;
 }
 
 // Free-column slab width for the back-elimination workspace.
@@ -210,18 +250,24 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     if (rc) return rc;
 
     static PinnedRec pinned;
-    if (!pinned.p) LINAC_CUDA(cudaMallocHost(&pinned.p, sizeof(PanelRec)));
+    if (!pinned.p) LINAC_CUDA(cudaMallocHost(&pinned.p, MAXBP * sizeof(PanelRec)));
 
     Fp c;
     c.A = dA; c.rows = rows; c.cols = cols; c.ld = ld; c.f = make_modp(p); c.s = s; c.arena = arena;
     c.nb = num_panels(cols);
+    c.bps = std::max<int64_t>(1, std::min<int64_t>(MAXBP, options().strip_width / PW));
+    c.ns = (c.nb + c.bps - 1) / c.bps;
+    rc = strip_grid(&c.coop_grid);
+    if (rc) return rc;
     const int64_t mn = std::min(rows, cols);
     c.d_rec = (PanelRec*)arena->take((size_t)c.nb * sizeof(PanelRec));
     c.d_T = (uint32_t*)arena->take((size_t)c.nb * PW * PW * 4);
     c.d_E = (uint32_t*)arena->take((size_t)c.nb * PW * PW * 4);
     c.d_pivcols = (int32_t*)arena->take((size_t)mn * 4);
     int32_t* d_colinfo = (int32_t*)arena->take((size_t)cols * 4);
-    if (!c.d_rec || !c.d_T || !c.d_E || !c.d_pivcols || !d_colinfo) return LINAC_ERR_WORKSPACE;
+    c.d_pstart = (int32_t*)arena->take((size_t)(c.nb + 1) * 4);
+    if (!c.d_rec || !c.d_T || !c.d_E || !c.d_pivcols || !d_colinfo || !c.d_pstart) return LINAC_ERR_WORKSPACE;
+    LINAC_CUDA(cudaMemsetAsync(c.d_pstart, 0, (size_t)(c.nb + 1) * 4, s));
     c.h_rec = pinned.p;
     c.pivcols.assign(mn, -1);
     c.pstart.assign(c.nb + 1, 0);
@@ -241,7 +287,7 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     }
     // forward elimination
     int64_t r = 0;
-    rc = factor(c, 0, c.nb, 0, &r);
+    rc = factor(c, 0, c.ns, 0, &r);
     // column classification: pivot index, or the threshold row of a free column
     std::vector<int32_t> colinfo(cols);
     std::vector<int32_t> freec, freeth;
@@ -268,7 +314,7 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
             dim3 grid((unsigned)((nf + 255) / 256), (unsigned)std::min<int64_t>(r, 1024));
             gather_cols_kernel<<<grid, 256, 0, s>>>(dA, ld, r, d_free, d_th, nf, F, nf);
             LINAC_CUDA(cudaGetLastError());
-            rc = trsm_upper(c, F, nf, nf, 0, c.nb);
+            rc = trsm_upper(c, F, nf, nf, 0, c.ns);
             if (rc) break;
             scatter_cols_kernel<<<grid, 256, 0, s>>>(dA, ld, r, d_free, nf, F, nf);
             LINAC_CUDA(cudaGetLastError());

@@ -1,0 +1,526 @@
+// fp_strip.cuh -- S1-S4 of the F_p path for one STRIP of up to 8 base panels: a cooperative kernel.
+//
+// One launch factors columns [j0, j0+ws) (ws <= SW_MAX) over the active rows >= i0, base panel by
+// base panel (PW = 32 columns each), with the whole grid resident (one CTA of 1024 threads per SM):
+//
+//   P1  (CTA 0)      pivot search + T = (pivot block)^-1 for the panel         (S1, S2)
+//       grid.sync
+//   P1b (all CTAs)   row exchanges on complete rows, only if the panel needs any (K5)
+//       grid.sync
+//   P2  (all CTAs)   U12 = T.A12 on the pivot rows and A22 -= L21.U12 on the rows below, restricted
+//                    to the strip's columns right of the panel                  (S3/S4 inside the strip)
+//       grid.sync
+//
+// so the ~10 dependent launches and the host round trip per base panel of the earlier schedule
+// become two or three grid barriers.  Everything right of the strip is updated afterwards by the
+// row-block solve (trsm_strip_kernel) and the tensor-core Schur update.
+//
+// Storage convention: see fp_kernels.cuh (multipliers are the raw entries at the pivot columns).
+#pragma once
+#include <climits>
+#include <cooperative_groups.h>
+
+#include "linac_internal.h"
+
+namespace linac {
+namespace cg = cooperative_groups;
+
+constexpr int SW_MAX = 256;                 // widest strip (columns)
+constexpr int SNT = 1024;                   // threads per CTA of the strip kernel (32 warps)
+constexpr int SRB = 256;                    // rows of one P2 tile
+constexpr int MAXBP = SW_MAX / PW;          // base panels per strip
+
+// d*x - h*y mod p with one reduction: d*x + (p-h)*y < 2^63.
+__device__ __forceinline__ uint32_t lincomb(uint32_t d, uint32_t x, uint32_t h, uint32_t y, const ModP& f) {
+    return reduce64((uint64_t)d * x + (uint64_t)(f.p - h) * y, f);
+}
+
+struct StripSmem {
+    // ---- P1
+    uint32_t W[2][PW][PW + 1];       // fast path: double-buffered block; general path: W[0] = chunk X, W[1] = Ep
+    uint32_t G[PW][2 * PW + 1];      // general path phase 2: [D | I]
+    uint32_t gs[2][PW];              // fast path: per-row scale / pivot value
+    int epc[PW];                     // pivot column of pivot t (discovery order)
+    long long esrc[PW];              // source row (absolute) of pivot t
+    int ord[PW];                     // pivots sorted by pivot column
+    uint32_t ginv[PW];
+    long long pos_of[PW];
+    int at[PW];
+    int nsw;
+    int fast_ok;
+    // ---- P2
+    uint32_t Ts[PW][PW + 1];
+    uint32_t Ar[PW][PW + 1];
+    __align__(16) uint32_t Us[PW][PW];       // this CTA's slice of U12 (kept until the deferred write-back)
+    uint32_t Ls[SRB][PW + 1];
+    int rank_of[PW];                 // panel column -> pivot index within the panel, or -1
+    // deferred write-back of Us
+    long long u_row0;                // first pivot row (absolute), or -1 if nothing is pending
+    long long u_col0;
+    int u_r, u_nc;
+};
+
+// ------------------------------------------------------------------------------------------------
+// P1, fast path: the 32 candidate rows i0..i0+31 and the 32 panel columns as one block, inverted IN
+// PLACE by division-free Gauss-Jordan with row pivoting (first non-zero among the unused rows; for
+// F_p any non-zero pivot will do).  Warp = block row (kept in registers), lane = column.
+// Step c: every row k != q becomes d*row_k - h_k*row_q with d the pivot; the slot of column c then
+// holds the column of the accumulated transform that belongs to source row q, and g_k tracks the
+// scalar each row has been multiplied by (for q: the pivot value).  At the end
+//   T[a][b] = g_{q_a}^-1 * W[q_a][b],   q_a = the row that pivoted column a,
+// is the inverse of D = A[pivot rows in column order, panel].  Fails (returns false, nothing
+// written) as soon as a column has no pivot among the unused rows: the caller then runs the general
+// path, which handles rank-deficient and multi-chunk panels.
+__device__ bool panel_fast(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t i0, int64_t j0, const ModP& f) {
+    const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
+    uint32_t x = A[(i0 + wq) * ld + j0 + lane];
+    uint32_t g = 1u;
+    unsigned used = 0;
+    sm.W[0][wq][lane] = x;
+    if (lane == 0) sm.gs[0][wq] = 1u;
+    __syncthreads();
+    bool ok = true;
+#pragma unroll 1
+    for (int c = 0; c < PW; ++c) {
+        const int buf = c & 1;
+        const unsigned cand = __ballot_sync(0xffffffffu, sm.W[buf][lane][c] != 0) & ~used;
+        if (!cand) { ok = false; break; }                     // uniform over the CTA
+        const int q = __ffs(cand) - 1;
+        const uint32_t d = sm.W[buf][q][c];
+        const uint32_t gq = sm.gs[buf][q];
+        const uint32_t pv = sm.W[buf][q][lane];
+        const uint32_t h = __shfl_sync(0xffffffffu, x, c);
+        if (wq != q) {
+            x = lincomb(d, lane == c ? 0u : x, h, lane == c ? gq : pv, f);
+            g = mulmod(d, g, f);
+        } else {
+            if (lane == c) x = g;
+            g = d;
+        }
+        if (tid == 0) { sm.epc[c] = c; sm.esrc[c] = i0 + q; sm.ord[c] = c; }
+        used |= 1u << q;
+        sm.W[buf ^ 1][wq][lane] = x;
+        if (lane == 0) sm.gs[buf ^ 1][wq] = g;
+        __syncthreads();
+    }
+    return ok;          // on success the final block is in W[0] (32 steps), scales in gs[0]
+}
+
+// ------------------------------------------------------------------------------------------------
+// P1, general path (any width w <= 32, any number of rows): rows are scanned in chunks of 32 held in
+// shared memory (warp = chunk row, lane = column); a chunk is first reduced against the pivot rows
+// found so far, then searched column by column for the FIRST row with a non-zero entry (warp ballot).
+// Elimination is division-free (row_k <- d*row_k - h*row_q), so no modular inverse sits on the
+// column-to-column dependency chain.  The scan stops once w pivots are known; otherwise it has looked
+// at every row, which is what proves the remaining columns are free columns.  Returns r.
+__device__ int panel_scan(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t rows, int64_t i0, int64_t j0, int w,
+                          const ModP& f) {
+    const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
+    uint32_t (*X)[PW + 1] = sm.W[0];
+    uint32_t (*Ep)[PW + 1] = sm.W[1];          // pivot rows as selected (unnormalised), discovery order
+    int r = 0;
+    unsigned pcmask = 0;
+    for (int64_t cs = i0; cs < rows && r < w; cs += PW) {
+        const int nh = (int)min((int64_t)PW, rows - cs);
+        uint32_t s = 0;
+        if (wq < nh && lane < w) s = A[(cs + wq) * ld + j0 + lane];
+        for (int a = 0; a < r; ++a) {              // ascending pivot column
+            const int tt = sm.ord[a];
+            const int c = sm.epc[tt];
+            const uint32_t l = __shfl_sync(0xffffffffu, s, c);
+            if (l) s = lane > c ? lincomb(Ep[tt][c], s, l, Ep[tt][lane], f) : (lane == c ? 0u : mulmod(Ep[tt][c], s, f));
+        }
+        X[wq][lane] = s;
+        if (!__syncthreads_or(s != 0)) continue;   // the whole chunk lies in the span found so far
+
+        unsigned used = 0;
+        for (int c = 0; c < w && r < w; ++c) {
+            if ((pcmask >> c) & 1u) continue;
+            const unsigned cand = __ballot_sync(0xffffffffu, X[lane][c] != 0) & ~used;
+            if (!cand) continue;
+            const int q = __ffs(cand) - 1;
+            const uint32_t d = X[q][c];
+            const uint32_t pv = X[q][lane];
+            if (wq != q && !((used >> wq) & 1u)) {
+                const uint32_t h = X[wq][c];
+                if (h != 0 && lane > c) X[wq][lane] = lincomb(d, X[wq][lane], h, pv, f);   // column c itself is not rewritten
+            }
+            if (wq == 0) Ep[r][lane] = ((pcmask >> lane) & 1u) ? 0u : pv;   // entries at earlier pivot columns are zeros
+            if (tid == 0) { sm.epc[r] = c; sm.esrc[r] = cs + q; }
+            used |= 1u << q;
+            pcmask |= 1u << c;
+            ++r;
+            __syncthreads();
+        }
+        if (wq == 0) {                             // rank sort of the pivots by column
+            const int mine = lane < r ? sm.epc[lane] : INT_MAX;
+            int pos = 0;
+            for (int t = 0; t < r; ++t) pos += (sm.epc[t] < mine);
+            if (lane < r) sm.ord[pos] = lane;
+        }
+        __syncthreads();
+    }
+    return r;
+}
+
+// T = D^-1 for the general path: Gauss-Jordan on [D | I], D = A[pivot rows, pivot columns] in ascending
+// pivot-column order (no search needed: pivot rows with a larger leading column vanish on the smaller
+// columns, so D has an LU factorisation without pivoting), division-free; leaves g (diagonal) and the
+// transform in G.  Also E = T.A[P, panel] when r < w.
+__device__ void panel_invert_general(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t j0, int w, int r, const ModP& f,
+                                     uint32_t* Tout, uint32_t* Eout) {
+    const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
+    for (int e = tid; e < PW * 2 * PW; e += SNT) {
+        const int a = e / (2 * PW), b = e % (2 * PW);
+        uint32_t v = 0;
+        if (a < r) {
+            if (b < PW) { if (b < r) v = A[sm.esrc[sm.ord[a]] * ld + j0 + sm.epc[sm.ord[b]]]; }
+            else v = (b - PW == a) ? 1u : 0u;
+        }
+        sm.G[a][b] = v;
+    }
+    __syncthreads();
+    for (int t = 0; t < r; ++t) {
+        const uint32_t d = sm.G[t][t];
+        const uint32_t pl = lane > t ? sm.G[t][lane] : 0u;
+        const uint32_t pr = lane <= t ? sm.G[t][PW + lane] : 0u;
+        if (wq != t && wq < r) {
+            const uint32_t h = sm.G[wq][t];
+            if (h != 0) {
+                if (lane > t || lane == wq) sm.G[wq][lane] = lincomb(d, sm.G[wq][lane], h, pl, f);
+                if (lane <= t || lane == wq) sm.G[wq][PW + lane] = lincomb(d, sm.G[wq][PW + lane], h, pr, f);
+            }
+        }
+        __syncthreads();
+    }
+    if (wq == 0 && lane < r) sm.ginv[lane] = invmod(sm.G[lane][lane], f);
+    __syncthreads();
+    {
+        const int a = wq, b = lane;
+        const uint32_t v = (a < r && b < r) ? mulmod(sm.ginv[a], sm.G[a][PW + b], f) : 0u;
+        Tout[a * PW + b] = v;
+        sm.Ts[a][b] = v;
+    }
+    if (r < w && r > 0) {
+        // E = T . A[P, panel]: reduced pivot rows restricted to the panel (identity on the pivot columns)
+        sm.Ar[wq][lane] = (wq < r && lane < w) ? A[sm.esrc[sm.ord[wq]] * ld + j0 + lane] : 0u;
+        __syncthreads();
+        uint64_t acc = 0;
+        for (int b = 0; b < r; ++b) {
+            acc += (uint64_t)sm.Ts[wq][b] * sm.Ar[b][lane];
+            if (b & 1) acc = fold64(acc, f);
+        }
+        Eout[wq * PW + lane] = wq < r ? reduce64(acc, f) : 0u;
+    }
+}
+
+// Exchange list (LAPACK style): row i0+a must receive source row esrc[ord[a]].  Warp 0 only.
+__device__ void panel_exchange_list(StripSmem& sm, int64_t i0, int r, PanelRec* rec) {
+    const int lane = threadIdx.x & 31;
+    const bool inplace = lane >= r || sm.esrc[sm.ord[lane]] == i0 + lane;
+    const bool all_inplace = __all_sync(0xffffffffu, inplace);
+    if (lane < r) { sm.pos_of[lane] = i0 + lane; sm.at[lane] = lane; }
+    __syncwarp();
+    if (all_inplace) {
+        if (lane < r) rec->swp[lane] = i0 + lane;
+        if (lane == 0) sm.nsw = 0;
+    } else if (lane == 0) {
+        int nsw = 0;
+        for (int a = 0; a < r; ++a) {
+            const long long src = sm.esrc[sm.ord[a]];
+            const long long cur = src < i0 + r ? sm.pos_of[(int)(src - i0)] : src;
+            rec->swp[a] = cur;
+            if (cur != i0 + a) {
+                ++nsw;
+                const int x = sm.at[a];                 // top-origin row now sitting at position a
+                sm.pos_of[x] = cur;
+                if (cur < i0 + r) sm.at[(int)(cur - i0)] = x;
+            }
+        }
+        sm.nsw = nsw;
+    }
+}
+
+// P1 for one base panel (columns [j0, j0+w), rows >= i0), executed by ONE CTA of SNT threads.
+// Outputs: rec (r, local pivot columns, exchange list), T (32x32, zero padded), E = T A[P, panel] when
+// r < w (the free columns' entries of the reduced pivot rows), pivcols.
+__device__ void panel_factor(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t rows, int64_t i0, int64_t j0, int w,
+                             const ModP& f, PanelRec* rec, uint32_t* Tout, uint32_t* Eout, int32_t* pivcols_global) {
+    const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
+    int r = 0;
+    bool fast = false;
+    if (w == PW && rows - i0 >= PW) fast = panel_fast(sm, A, ld, i0, j0, f);
+    if (fast) {
+        r = PW;
+        if (wq == 0) {
+            sm.ginv[lane] = invmod(sm.gs[0][(int)(sm.esrc[lane] - i0)], f);
+            panel_exchange_list(sm, i0, r, rec);
+        }
+        __syncthreads();
+        const int qa = (int)(sm.esrc[wq] - i0);
+        Tout[wq * PW + lane] = mulmod(sm.ginv[wq], sm.W[0][qa][lane], f);
+    } else {
+        __syncthreads();
+        r = panel_scan(sm, A, ld, rows, i0, j0, w, f);
+        if (wq == 0) panel_exchange_list(sm, i0, r, rec);
+        __syncthreads();
+        panel_invert_general(sm, A, ld, j0, w, r, f, Tout, Eout);
+    }
+    if (tid < PW) {
+        rec->pc[tid] = tid < r ? sm.epc[sm.ord[tid]] : -1;
+        if (tid < r) pivcols_global[i0 + tid] = (int32_t)(j0 + sm.epc[sm.ord[tid]]);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        rec->r = r;
+        rec->w = w;
+        rec->nswaps = sm.nsw;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// The strip kernel.  Panel metadata arrays are indexed by the GLOBAL base panel number b = j0/PW + i.
+// pstart[b+1] (device) receives the number of pivots found left of panel b+1.
+struct StripArgs {
+    uint32_t* A;
+    int64_t ld, rows, cols;
+    int64_t i0;              // first active row
+    int64_t j0;              // first column of the strip (multiple of PW)
+    int ws;                  // strip width in columns
+    ModP f;
+    PanelRec* rec;           // [nb]
+    uint32_t* T;             // [nb][PW*PW]
+    uint32_t* E;             // [nb][PW*PW]
+    int32_t* pivcols;        // [min(rows, cols)]
+    int32_t* pstart;         // [nb+1]
+};
+
+__device__ __forceinline__ void strip_flush_u(StripSmem& sm, uint32_t* A, int64_t ld) {
+    if (sm.u_row0 < 0) return;
+    const int lane = threadIdx.x & 31, wq = threadIdx.x >> 5;
+    if (wq < sm.u_r && lane < sm.u_nc) A[(sm.u_row0 + wq) * ld + sm.u_col0 + lane] = sm.Us[wq][lane];
+}
+
+__global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a) {
+    extern __shared__ __align__(16) unsigned char strip_smem_raw[];
+    StripSmem& sm = *reinterpret_cast<StripSmem*>(strip_smem_raw);
+    cg::grid_group grid = cg::this_grid();
+    const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
+    const int G = gridDim.x, cta = blockIdx.x;
+    uint32_t* A = a.A;
+    const int64_t ld = a.ld;
+    const ModP f = a.f;
+    const int nbp = (a.ws + PW - 1) / PW;
+    const int64_t b0 = a.j0 / PW;
+    int64_t cur = a.i0;
+
+    if (tid == 0) sm.u_row0 = -1;
+    __syncthreads();
+
+    for (int i = 0; i < nbp; ++i) {
+        const int64_t b = b0 + i;
+        const int64_t jp = a.j0 + (int64_t)i * PW;
+        const int w = (int)min((int64_t)PW, a.j0 + a.ws - jp);
+        if (cur >= a.rows) {                       // no rows left: every remaining column is free (uniform over the grid)
+            if (cta == 0 && tid == 0)
+                for (int t = i; t < nbp; ++t) {
+                    a.rec[b0 + t].r = 0; a.rec[b0 + t].nswaps = 0; a.rec[b0 + t].w = 0;
+                    a.pstart[b0 + t + 1] = (int32_t)cur;
+                }
+            break;
+        }
+        // pending U12 slice of the previous panel: its readers all passed the last grid barrier
+        strip_flush_u(sm, A, ld);
+        __syncthreads();
+        if (tid == 0) sm.u_row0 = -1;
+        // ---- P1
+        if (cta == 0) {
+            panel_factor(sm, A, ld, a.rows, cur, jp, w, f, a.rec + b, a.T + b * PW * PW, a.E + b * PW * PW, a.pivcols);
+            if (tid == 0) a.pstart[b + 1] = (int32_t)(cur + a.rec[b].r);
+        }
+        grid.sync();
+        const PanelRec* rec = a.rec + b;
+        const int r = rec->r, nsw = rec->nswaps;
+        if (r == 0) continue;
+        // ---- P1b: row exchanges on complete rows, one thread per column (so the sequence of
+        // exchanges needs no inter-thread ordering)
+        if (nsw > 0) {
+            for (int64_t c = (int64_t)cta * SNT + tid; c < a.cols; c += (int64_t)G * SNT) {
+                for (int t = 0; t < r; ++t) {
+                    const int64_t s = rec->swp[t];
+                    if (s != cur + t) {
+                        const uint32_t x = A[(cur + t) * ld + c], y = A[s * ld + c];
+                        A[(cur + t) * ld + c] = y;
+                        A[s * ld + c] = x;
+                    }
+                }
+            }
+            grid.sync();
+        }
+        const int64_t mb0 = cur + r;                 // first row below the pivot rows
+        const int64_t cu0 = jp + w, cu1 = a.j0 + a.ws;
+        const int ncu = (int)(cu1 - cu0);
+        // reduced pivot rows' entries inside a rank-deficient panel (nobody reads these during P2)
+        if (r < w && cta == G - 1)
+            if (wq < r && lane < w) A[(cur + wq) * ld + jp + lane] = a.E[b * PW * PW + wq * PW + lane];
+        if (ncu > 0) {
+            // ---- P2
+            const int ncb = (ncu + PW - 1) / PW;
+            const int nrw = max(1, G / ncb);                   // row workers per column block
+            const int cb = cta % ncb, rw = cta / ncb;
+            if (rw < nrw) {
+                const int64_t cc0 = cu0 + (int64_t)cb * PW;
+                const int nc = (int)min((int64_t)PW, cu1 - cc0);
+                sm.Ts[wq][lane] = a.T[b * PW * PW + wq * PW + lane];
+                sm.Ar[wq][lane] = (wq < r && lane < nc) ? A[(cur + wq) * ld + cc0 + lane] : 0u;
+                if (tid < PW) sm.rank_of[tid] = -1;
+                __syncthreads();
+                if (tid < r) sm.rank_of[rec->pc[tid]] = tid;
+                {
+                    uint64_t acc = 0;
+#pragma unroll 8
+                    for (int k = 0; k < PW; k += 2) {
+                        acc += (uint64_t)sm.Ts[wq][k] * sm.Ar[k][lane];
+                        acc += (uint64_t)sm.Ts[wq][k + 1] * sm.Ar[k + 1][lane];
+                        acc = fold64(acc, f);
+                    }
+                    sm.Us[wq][lane] = wq < r ? reduce64(acc, f) : 0u;
+                }
+                if (rw == 0 && tid == 0) { sm.u_row0 = cur; sm.u_col0 = cc0; sm.u_r = r; sm.u_nc = nc; }
+                __syncthreads();
+                // rows below the pivots, split evenly over this column block's row workers
+                const int64_t mrem = a.rows - mb0;
+                int64_t rpw = (mrem + nrw - 1) / nrw;
+                rpw = (rpw + 31) / 32 * 32;
+                const int64_t my0 = mb0 + (int64_t)rw * rpw, my1 = min(a.rows, my0 + rpw);
+                const int rg = wq >> 2, cgp = wq & 3;                 // 8 row groups x 4 column groups of 8
+                const int kcol = sm.rank_of[lane];
+                for (int64_t m0 = my0; m0 < my1; m0 += SRB) {
+                    // L tile: SRB rows x 32 panel columns, stored at its pivot index
+#pragma unroll
+                    for (int t = 0; t < SRB / 32; ++t) {
+                        const int rl = wq + 32 * t;
+                        const int64_t m = m0 + rl;
+                        if (kcol >= 0) sm.Ls[rl][kcol] = m < my1 ? A[m * ld + jp + lane] : 0u;
+                    }
+                    const int64_t m = m0 + rg * 32 + lane;
+                    uint32_t* crow = A + m * ld + cc0 + cgp * 8;
+                    uint32_t cv[8];
+                    const int nvalid = m < my1 ? max(0, min(8, nc - cgp * 8)) : 0;
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) cv[e] = e < nvalid ? crow[e] : 0u;
+                    __syncthreads();
+                    if (nvalid > 0) {
+                        uint64_t acc[8];
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) acc[e] = 0;
+                        const uint32_t* lrow = sm.Ls[rg * 32 + lane];
+                        for (int k = 0; k + 1 < r; k += 2) {
+                            const uint32_t l0 = lrow[k], l1 = lrow[k + 1];
+                            const uint4 u0a = *reinterpret_cast<const uint4*>(&sm.Us[k][cgp * 8]);
+                            const uint4 u0b = *reinterpret_cast<const uint4*>(&sm.Us[k][cgp * 8 + 4]);
+                            const uint4 u1a = *reinterpret_cast<const uint4*>(&sm.Us[k + 1][cgp * 8]);
+                            const uint4 u1b = *reinterpret_cast<const uint4*>(&sm.Us[k + 1][cgp * 8 + 4]);
+                            const uint32_t u0[8] = {u0a.x, u0a.y, u0a.z, u0a.w, u0b.x, u0b.y, u0b.z, u0b.w};
+                            const uint32_t u1[8] = {u1a.x, u1a.y, u1a.z, u1a.w, u1b.x, u1b.y, u1b.z, u1b.w};
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) {
+                                uint64_t x = acc[e];
+                                x += (uint64_t)l0 * u0[e];
+                                x += (uint64_t)l1 * u1[e];
+                                acc[e] = fold64(x, f);
+                            }
+                        }
+                        if (r & 1) {
+                            const uint32_t l0 = lrow[r - 1];
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) acc[e] = fold64(acc[e] + (uint64_t)l0 * sm.Us[r - 1][cgp * 8 + e], f);
+                        }
+#pragma unroll
+                        for (int e = 0; e < 8; ++e)
+                            if (e < nvalid) crow[e] = submod(cv[e], reduce64(acc[e], f), f);
+                    }
+                    __syncthreads();
+                }
+            }
+            if (i + 1 < nbp) grid.sync();
+        }
+        cur = mb0;
+    }
+    strip_flush_u(sm, A, ld);
+}
+
+// ------------------------------------------------------------------------------------------------
+// S4 / S6 leaf: triangular solve against ONE strip's pivots, column-parallel (a CTA owns 32 columns
+// of X and keeps them in shared memory, so the sequential dependence between base panels never
+// leaves the CTA).  X has K = pstart[bs1] - pstart[bs0] rows (the strip's pivot rows, in order).
+//   LOWER (row-block solve, U12 = L11^-1 A12):  for each base panel b, ascending:
+//           X_b <- T_b X_b ;  X_t -= sum_k L[t][k] X_b[k]  for the strip's pivot rows t after b
+//   UPPER (back-elimination of the free columns): for each base panel b, descending:
+//           X_t -= sum_k U[t][k] X_b[k]  for the strip's pivot rows t before b
+// with L[t][k] = U[t][k] = A[row t][pivcols[first pivot of b + k]] (fp_kernels.cuh storage convention).
+constexpr int TNT = 512;       // threads per CTA (16 warps)
+
+template <bool LOWER>
+__global__ void __launch_bounds__(TNT) trsm_strip_kernel(const uint32_t* __restrict__ A, int64_t ld,
+                                                         uint32_t* __restrict__ X, int64_t ldx, int64_t ncols,
+                                                         const int32_t* __restrict__ pstart, int bs0, int bs1,
+                                                         const uint32_t* __restrict__ T,
+                                                         const int32_t* __restrict__ pivcols, ModP f) {
+    extern __shared__ __align__(16) unsigned char trsm_smem_raw[];
+    uint32_t (*Xs)[PW] = reinterpret_cast<uint32_t (*)[PW]>(trsm_smem_raw);                 // [K][32]
+    const int t0 = pstart[bs0], K = pstart[bs1] - t0;
+    uint32_t (*Ts)[PW + 1] = reinterpret_cast<uint32_t (*)[PW + 1]>(trsm_smem_raw + (size_t)K * PW * 4);   // [32][33]
+    const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
+    constexpr int NW = TNT / 32;
+    const int64_t c = (int64_t)blockIdx.x * PW + lane;
+    const bool cok = c < ncols;
+    for (int t = wq; t < K; t += NW) Xs[t][lane] = cok ? X[(int64_t)t * ldx + c] : 0u;
+    __syncthreads();
+    const int nbp = bs1 - bs0;
+    for (int ii = 0; ii < nbp; ++ii) {
+        const int b = LOWER ? bs0 + ii : bs1 - 1 - ii;
+        const int s = pstart[b] - t0, e = pstart[b + 1] - t0, r = e - s;
+        if (r == 0) continue;
+        if (LOWER) {
+            for (int x = tid; x < PW * PW; x += TNT) Ts[x / PW][x % PW] = T[(int64_t)b * PW * PW + x];
+            __syncthreads();
+            uint32_t y[PW / NW];
+#pragma unroll
+            for (int u = 0; u < PW / NW; ++u) {
+                const int a = wq + NW * u;
+                uint64_t acc = 0;
+                for (int k = 0; k + 1 < r; k += 2) {
+                    acc += (uint64_t)Ts[a][k] * Xs[s + k][lane];
+                    acc += (uint64_t)Ts[a][k + 1] * Xs[s + k + 1][lane];
+                    acc = fold64(acc, f);
+                }
+                if (r & 1) acc = fold64(acc + (uint64_t)Ts[a][r - 1] * Xs[s + r - 1][lane], f);
+                y[u] = reduce64(acc, f);
+            }
+            __syncthreads();
+#pragma unroll
+            for (int u = 0; u < PW / NW; ++u)
+                if (wq + NW * u < r) Xs[s + wq + NW * u][lane] = y[u];
+            __syncthreads();
+        }
+        const int lo = LOWER ? e : 0, hi = LOWER ? K : s;
+        const int32_t pc = lane < r ? pivcols[t0 + s + lane] : 0;
+        for (int t = lo + wq; t < hi; t += NW) {
+            const uint32_t lv = lane < r ? A[(int64_t)(t0 + t) * ld + pc] : 0u;
+            uint64_t acc = 0;
+            for (int k = 0; k + 1 < r; k += 2) {
+                acc += (uint64_t)__shfl_sync(0xffffffffu, lv, k) * Xs[s + k][lane];
+                acc += (uint64_t)__shfl_sync(0xffffffffu, lv, k + 1) * Xs[s + k + 1][lane];
+                acc = fold64(acc, f);
+            }
+            if (r & 1) acc = fold64(acc + (uint64_t)__shfl_sync(0xffffffffu, lv, r - 1) * Xs[s + r - 1][lane], f);
+            Xs[t][lane] = submod(Xs[t][lane], reduce64(acc, f), f);
+        }
+        __syncthreads();
+    }
+    if (cok)
+        for (int t = wq; t < K; t += NW) X[(int64_t)t * ldx + c] = Xs[t][lane];
+}
+
+}  // namespace linac

@@ -11,7 +11,6 @@
 namespace linac {
 
 constexpr int PW = 32;   // base panel width (columns factored by one panel kernel)
-constexpr int CH = 32;   // rows per chunk scanned by the panel kernel
 
 // What the panel kernel reports for one base panel (kept on the device per panel; the host reads it
 // with one small copy when it needs the pivot count).
@@ -41,6 +40,7 @@ struct Options {
     int64_t timing = 0;       // 1 = bracket update kernels with events (costs syncs; for profiling runs)
     int64_t tc_min_k = 256;   // smallest K the tensor path is used for
     int64_t tc_min_mn = 512;  // smallest M and N the tensor path is used for
+    int64_t strip_width = 128; // columns factored by one cooperative strip kernel (multiple of 32, <= 256)
 };
 Options& options();
 linac_stats& stats();
