@@ -138,6 +138,8 @@ def main():
     ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3"])
     ap.add_argument("--ref-n", type=int, default=1280, help="sample size for the oracle legs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
+                    help="library tunable for A/B runs (linac_set_option), e.g. --opt strip_width=256")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -192,6 +194,9 @@ def main():
         return e0.elapsed_time(e1), rank_
 
     L.set_option("timing", 0)
+    for kv in args.opt:
+        name, val = kv.split("=")
+        L.set_option(name, int(val))
     for _ in range(args.warmup):
         step_resident()
     sampler = ClockSampler(local)

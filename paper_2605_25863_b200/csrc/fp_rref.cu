@@ -145,6 +145,33 @@ int factor(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t* r_out) {
         return LINAC_OK;
     }
     if (s1 - s0 == 1) return factor_strip(c, s0, i0, r_out);
+    if ((s1 - s0) * c.bps * PW <= options().flat_cols) {
+        // flat right-looking sweep over the node's strips: factor, row-block solve on the columns to the
+        // right (inside the node), Schur update of everything below with K = the strip's pivots
+        const int64_t jend = std::min(c.cols, panel_col0(c.sb0(s1)));
+        int64_t cur = i0;
+        for (int64_t s = s0; s < s1; ++s) {
+            int64_t r = 0;
+            if (cur >= c.rows) return factor(c, s, s1, cur, &r);      // marks the remaining columns free
+            int rc = factor_strip(c, s, cur, &r);
+            if (rc) return rc;
+            const int64_t jc = std::min(c.cols, panel_col0(c.sb0(s + 1)));
+            if (r > 0 && jend > jc) {
+                rc = trsm_leaf<true>(c, s, c.A + cur * c.ld + jc, c.ld, jend - jc);
+                if (rc) return rc;
+                const int64_t m2 = c.rows - (cur + r);
+                if (m2 > 0) {
+                    GemmArgs g{c.A + (cur + r) * c.ld + jc, c.ld, c.A + (cur + r) * c.ld, c.ld, c.d_pivcols + cur,
+                               c.A + cur * c.ld + jc,       c.ld, m2,                      jend - jc, r};
+                    rc = run_gemm(c, g);
+                    if (rc) return rc;
+                }
+            }
+            cur += r;
+            *r_out = cur - i0;
+        }
+        return LINAC_OK;
+    }
     const int64_t sm = s0 + (s1 - s0) / 2;
     const int64_t jm = panel_col0(c.sb0(sm)), j1 = std::min(c.cols, panel_col0(c.sb0(s1)));
     int64_t r1 = 0, r2 = 0;

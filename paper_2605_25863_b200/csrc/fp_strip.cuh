@@ -48,12 +48,12 @@ struct StripSmem {
     int at[PW];
     int nsw;
     int fast_ok;
+    int r_out;
     // ---- P2
     uint32_t Ts[PW][PW + 1];
     uint32_t Ar[PW][PW + 1];
     __align__(16) uint32_t Us[PW][PW];       // this CTA's slice of U12 (kept until the deferred write-back)
-    uint32_t Ls[SRB][PW + 1];
-    int rank_of[PW];                 // panel column -> pivot index within the panel, or -1
+    __align__(16) uint32_t Lk[PW][SRB + 4];  // L tile, k-major (pivot index, row)
     // deferred write-back of Us
     long long u_row0;                // first pivot row (absolute), or -1 if nothing is pending
     long long u_col0;
@@ -73,37 +73,45 @@ struct StripSmem {
 // path, which handles rank-deficient and multi-chunk panels.
 __device__ bool panel_fast(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t i0, int64_t j0, const ModP& f) {
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
-    uint32_t x = A[(i0 + wq) * ld + j0 + lane];
-    uint32_t g = 1u;
-    unsigned used = 0;
-    sm.W[0][wq][lane] = x;
-    if (lane == 0) sm.gs[0][wq] = 1u;
-    __syncthreads();
-    bool ok = true;
-#pragma unroll 1
-    for (int c = 0; c < PW; ++c) {
-        const int buf = c & 1;
-        const unsigned cand = __ballot_sync(0xffffffffu, sm.W[buf][lane][c] != 0) & ~used;
-        if (!cand) { ok = false; break; }                     // uniform over the CTA
-        const int q = __ffs(cand) - 1;
-        const uint32_t d = sm.W[buf][q][c];
-        const uint32_t gq = sm.gs[buf][q];
-        const uint32_t pv = sm.W[buf][q][lane];
-        const uint32_t h = __shfl_sync(0xffffffffu, x, c);
-        if (wq != q) {
-            x = lincomb(d, lane == c ? 0u : x, h, lane == c ? gq : pv, f);
-            g = mulmod(d, g, f);
-        } else {
-            if (lane == c) x = g;
-            g = d;
-        }
-        if (tid == 0) { sm.epc[c] = c; sm.esrc[c] = i0 + q; sm.ord[c] = c; }
-        used |= 1u << q;
-        sm.W[buf ^ 1][wq][lane] = x;
-        if (lane == 0) sm.gs[buf ^ 1][wq] = g;
-        __syncthreads();
+    constexpr int FW = 8, RPW = PW / FW;          // 8 working warps, 4 block rows each (registers)
+    uint32_t x[RPW];
+    if (wq < FW) {
+#pragma unroll
+        for (int i = 0; i < RPW; ++i) x[i] = A[(i0 + wq * RPW + i) * ld + j0 + lane];
+#pragma unroll
+        for (int i = 0; i < RPW; ++i) sm.W[0][wq * RPW + i][lane] = x[i];
     }
-    return ok;          // on success the final block is in W[0] (32 steps), scales in gs[0]
+    __syncthreads();
+    if (wq < FW) {
+        unsigned used = 0;
+        uint32_t dtot = 1u;                       // product of the pivots so far (the scale of every unused row)
+        bool ok = true;
+#pragma unroll 2
+        for (int c = 0; c < PW; ++c) {
+            const int buf = c & 1;
+            const unsigned cand = __ballot_sync(0xffffffffu, sm.W[buf][lane][c] != 0) & ~used;
+            if (!cand) { ok = false; break; }                 // uniform over the working warps
+            const int q = __ffs(cand) - 1;
+            const uint32_t pv = sm.W[buf][q][lane];
+            const uint32_t d = __shfl_sync(0xffffffffu, pv, c);
+            const uint32_t y = lane == c ? dtot : pv;         // slot c of the pivot row holds its scale
+#pragma unroll
+            for (int i = 0; i < RPW; ++i) {
+                const int row = wq * RPW + i;
+                const uint32_t h = __shfl_sync(0xffffffffu, x[i], c);
+                if (row != q) x[i] = lincomb(d, lane == c ? 0u : x[i], h, y, f);
+                else if (lane == c) x[i] = dtot;
+                sm.W[buf ^ 1][row][lane] = x[i];
+            }
+            if (tid == 0) { sm.esrc[c] = i0 + q; sm.gs[0][c] = dtot; }    // gs[0][c] = prefix product BEFORE step c
+            dtot = mulmod(dtot, d, f);
+            used |= 1u << q;
+            asm volatile("bar.sync 1, %0;" ::"n"(FW * 32) : "memory");
+        }
+        if (tid == 0) { sm.fast_ok = ok ? 1 : 0; sm.gs[1][0] = dtot; }
+    }
+    __syncthreads();
+    return sm.fast_ok != 0;     // on success the final block is in W[0] (32 steps); gs[1][0] = product of all pivots
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -251,12 +259,14 @@ __device__ void panel_factor(StripSmem& sm, const uint32_t* A, int64_t ld, int64
     bool fast = false;
     if (w == PW && rows - i0 >= PW) fast = panel_fast(sm, A, ld, i0, j0, f);
     if (fast) {
+        // row q_a that pivoted column a has been scaled by g = (all pivots) / (pivots before step a), so
+        // 1/g = prefix[a] / (all pivots): ONE modular inverse for the panel (K7)
         r = PW;
-        if (wq == 0) {
-            sm.ginv[lane] = invmod(sm.gs[0][(int)(sm.esrc[lane] - i0)], f);
-            panel_exchange_list(sm, i0, r, rec);
-        }
+        if (tid < PW) { sm.epc[tid] = tid; sm.ord[tid] = tid; }
+        const uint32_t inv_all = invmod(sm.gs[1][0], f);
+        if (wq == 0) sm.ginv[lane] = mulmod(sm.gs[0][lane], inv_all, f);
         __syncthreads();
+        if (wq == 0) panel_exchange_list(sm, i0, r, rec);
         const int qa = (int)(sm.esrc[wq] - i0);
         Tout[wq * PW + lane] = mulmod(sm.ginv[wq], sm.W[0][qa][lane], f);
     } else {
@@ -275,6 +285,7 @@ __device__ void panel_factor(StripSmem& sm, const uint32_t* A, int64_t ld, int64
         rec->r = r;
         rec->w = w;
         rec->nswaps = sm.nsw;
+        sm.r_out = r;
     }
 }
 
@@ -316,7 +327,6 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
 
     if (tid == 0) sm.u_row0 = -1;
     __syncthreads();
-
     for (int i = 0; i < nbp; ++i) {
         const int64_t b = b0 + i;
         const int64_t jp = a.j0 + (int64_t)i * PW;
@@ -333,10 +343,54 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
         strip_flush_u(sm, A, ld);
         __syncthreads();
         if (tid == 0) sm.u_row0 = -1;
+        // geometry of P2 (independent of what P1 finds, except through r)
+        const int64_t cu0 = jp + w, cu1 = a.j0 + a.ws;
+        const int ncu = (int)(cu1 - cu0);
+        const int ncb = max(1, (ncu + PW - 1) / PW);
+        const int nrw = max(1, G / ncb);                   // row workers per column block
+        const int cb = cta % ncb, rw = cta / ncb;
+        const bool worker = ncu > 0 && rw < nrw;
+        const int64_t cc0 = cu0 + (int64_t)cb * PW;
+        const int nc = (int)min((int64_t)PW, cu1 - cc0);
+        int64_t my0 = 0, my1 = 0;
+        auto my_rows = [&](int64_t mb0_) {                 // rows below the pivots, split evenly over the row workers
+            const int64_t mrem = a.rows - mb0_;
+            int64_t rpw = (mrem + nrw - 1) / nrw;
+            rpw = (rpw + 31) / 32 * 32;
+            my0 = mb0_ + (int64_t)rw * rpw;
+            my1 = min(a.rows, my0 + rpw);
+        };
+        uint32_t cv[SRB / 32];
+        int kcol = lane;
+        auto load_tile = [&](int64_t m0) {                 // L tile -> shared memory (k-major), C tile -> registers
+            uint32_t lreg[SRB / 32];
+#pragma unroll
+            for (int t = 0; t < SRB / 32; ++t) {
+                const int64_t m = m0 + wq + 32 * t;
+                lreg[t] = (kcol >= 0 && m < my1) ? A[m * ld + jp + lane] : 0u;
+            }
+#pragma unroll
+            for (int t = 0; t < SRB / 32; ++t) {
+                const int64_t m = m0 + wq * (SRB / 32) + t;
+                cv[t] = (lane < nc && m < my1) ? A[m * ld + cc0 + lane] : 0u;
+            }
+            if (kcol >= 0) {
+#pragma unroll
+                for (int t = 0; t < SRB / 32; ++t) sm.Lk[kcol][wq + 32 * t] = lreg[t];
+            }
+        };
+        // Prefetch of the first tile while CTA 0 factors the panel, assuming the common outcome (32
+        // pivots from the first 32 rows, no exchanges); checked after the barrier.
+        bool pre = false;
+        if (worker && cta != 0 && w == PW && cur + PW < a.rows) {
+            my_rows(cur + PW);
+            load_tile(my0);
+            pre = true;
+        }
         // ---- P1
         if (cta == 0) {
             panel_factor(sm, A, ld, a.rows, cur, jp, w, f, a.rec + b, a.T + b * PW * PW, a.E + b * PW * PW, a.pivcols);
-            if (tid == 0) a.pstart[b + 1] = (int32_t)(cur + a.rec[b].r);
+            if (tid == 0) a.pstart[b + 1] = (int32_t)(cur + sm.r_out);
         }
         grid.sync();
         const PanelRec* rec = a.rec + b;
@@ -358,24 +412,25 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
             grid.sync();
         }
         const int64_t mb0 = cur + r;                 // first row below the pivot rows
-        const int64_t cu0 = jp + w, cu1 = a.j0 + a.ws;
-        const int ncu = (int)(cu1 - cu0);
         // reduced pivot rows' entries inside a rank-deficient panel (nobody reads these during P2)
         if (r < w && cta == G - 1)
             if (wq < r && lane < w) A[(cur + wq) * ld + jp + lane] = a.E[b * PW * PW + wq * PW + lane];
         if (ncu > 0) {
             // ---- P2
-            const int ncb = (ncu + PW - 1) / PW;
-            const int nrw = max(1, G / ncb);                   // row workers per column block
-            const int cb = cta % ncb, rw = cta / ncb;
-            if (rw < nrw) {
-                const int64_t cc0 = cu0 + (int64_t)cb * PW;
-                const int nc = (int)min((int64_t)PW, cu1 - cc0);
-                sm.Ts[wq][lane] = a.T[b * PW * PW + wq * PW + lane];
-                sm.Ar[wq][lane] = (wq < r && lane < nc) ? A[(cur + wq) * ld + cc0 + lane] : 0u;
-                if (tid < PW) sm.rank_of[tid] = -1;
+            if (worker) {
+                const uint32_t tval = a.T[b * PW * PW + wq * PW + lane];
+                const uint32_t aval = (wq < r && lane < nc) ? A[(cur + wq) * ld + cc0 + lane] : 0u;
+                if (!(pre && r == PW && nsw == 0)) {
+                    // pivot index of panel column `lane` (pc[] is ascending), or -1
+                    const unsigned pcm = __reduce_or_sync(0xffffffffu, lane < r ? 1u << rec->pc[lane] : 0u);
+                    kcol = ((pcm >> lane) & 1u) ? __popc(pcm & ((1u << lane) - 1u)) : -1;
+                    my_rows(mb0);
+                    __syncthreads();                 // a rejected prefetch may still be landing in Lk
+                    load_tile(my0);
+                }
+                sm.Ts[wq][lane] = tval;
+                sm.Ar[wq][lane] = aval;
                 __syncthreads();
-                if (tid < r) sm.rank_of[rec->pc[tid]] = tid;
                 {
                     uint64_t acc = 0;
 #pragma unroll 8
@@ -387,60 +442,40 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
                     sm.Us[wq][lane] = wq < r ? reduce64(acc, f) : 0u;
                 }
                 if (rw == 0 && tid == 0) { sm.u_row0 = cur; sm.u_col0 = cc0; sm.u_r = r; sm.u_nc = nc; }
-                __syncthreads();
-                // rows below the pivots, split evenly over this column block's row workers
-                const int64_t mrem = a.rows - mb0;
-                int64_t rpw = (mrem + nrw - 1) / nrw;
-                rpw = (rpw + 31) / 32 * 32;
-                const int64_t my0 = mb0 + (int64_t)rw * rpw, my1 = min(a.rows, my0 + rpw);
-                const int rg = wq >> 2, cgp = wq & 3;                 // 8 row groups x 4 column groups of 8
-                const int kcol = sm.rank_of[lane];
                 for (int64_t m0 = my0; m0 < my1; m0 += SRB) {
-                    // L tile: SRB rows x 32 panel columns, stored at its pivot index
-#pragma unroll
-                    for (int t = 0; t < SRB / 32; ++t) {
-                        const int rl = wq + 32 * t;
-                        const int64_t m = m0 + rl;
-                        if (kcol >= 0) sm.Ls[rl][kcol] = m < my1 ? A[m * ld + jp + lane] : 0u;
-                    }
-                    const int64_t m = m0 + rg * 32 + lane;
-                    uint32_t* crow = A + m * ld + cc0 + cgp * 8;
-                    uint32_t cv[8];
-                    const int nvalid = m < my1 ? max(0, min(8, nc - cgp * 8)) : 0;
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) cv[e] = e < nvalid ? crow[e] : 0u;
-                    __syncthreads();
-                    if (nvalid > 0) {
-                        uint64_t acc[8];
-#pragma unroll
-                        for (int e = 0; e < 8; ++e) acc[e] = 0;
-                        const uint32_t* lrow = sm.Ls[rg * 32 + lane];
-                        for (int k = 0; k + 1 < r; k += 2) {
-                            const uint32_t l0 = lrow[k], l1 = lrow[k + 1];
-                            const uint4 u0a = *reinterpret_cast<const uint4*>(&sm.Us[k][cgp * 8]);
-                            const uint4 u0b = *reinterpret_cast<const uint4*>(&sm.Us[k][cgp * 8 + 4]);
-                            const uint4 u1a = *reinterpret_cast<const uint4*>(&sm.Us[k + 1][cgp * 8]);
-                            const uint4 u1b = *reinterpret_cast<const uint4*>(&sm.Us[k + 1][cgp * 8 + 4]);
-                            const uint32_t u0[8] = {u0a.x, u0a.y, u0a.z, u0a.w, u0b.x, u0b.y, u0b.z, u0b.w};
-                            const uint32_t u1[8] = {u1a.x, u1a.y, u1a.z, u1a.w, u1b.x, u1b.y, u1b.z, u1b.w};
-#pragma unroll
-                            for (int e = 0; e < 8; ++e) {
-                                uint64_t x = acc[e];
-                                x += (uint64_t)l0 * u0[e];
-                                x += (uint64_t)l1 * u1[e];
-                                acc[e] = fold64(x, f);
-                            }
-                        }
-                        if (r & 1) {
-                            const uint32_t l0 = lrow[r - 1];
-#pragma unroll
-                            for (int e = 0; e < 8; ++e) acc[e] = fold64(acc[e] + (uint64_t)l0 * sm.Us[r - 1][cgp * 8 + e], f);
-                        }
-#pragma unroll
-                        for (int e = 0; e < 8; ++e)
-                            if (e < nvalid) crow[e] = submod(cv[e], reduce64(acc[e], f), f);
+                    if (m0 != my0) {
+                        __syncthreads();             // previous tile's readers of Lk are done
+                        load_tile(m0);
                     }
                     __syncthreads();
+                    // thread = 8 consecutive rows x 1 column: L by broadcast LDS.128, U by one LDS per k
+                    uint64_t acc[SRB / 32];
+#pragma unroll
+                    for (int t = 0; t < SRB / 32; ++t) acc[t] = 0;
+#pragma unroll 1
+                    for (int k = 0; k + 1 < r; k += 2) {
+#pragma unroll
+                        for (int kk = 0; kk < 2; ++kk) {
+                            const uint4 la = *reinterpret_cast<const uint4*>(&sm.Lk[k + kk][wq * 8]);
+                            const uint4 lb = *reinterpret_cast<const uint4*>(&sm.Lk[k + kk][wq * 8 + 4]);
+                            const uint32_t u = sm.Us[k + kk][lane];
+                            const uint32_t l[8] = {la.x, la.y, la.z, la.w, lb.x, lb.y, lb.z, lb.w};
+#pragma unroll
+                            for (int t = 0; t < 8; ++t) acc[t] += (uint64_t)l[t] * u;
+                        }
+#pragma unroll
+                        for (int t = 0; t < 8; ++t) acc[t] = fold64(acc[t], f);
+                    }
+                    if (r & 1) {
+                        const uint32_t u0 = sm.Us[r - 1][lane];
+#pragma unroll
+                        for (int t = 0; t < 8; ++t) acc[t] = fold64(acc[t] + (uint64_t)sm.Lk[r - 1][wq * 8 + t] * u0, f);
+                    }
+#pragma unroll
+                    for (int t = 0; t < 8; ++t) {
+                        const int64_t m = m0 + wq * 8 + t;
+                        if (lane < nc && m < my1) A[m * ld + cc0 + lane] = submod(cv[t], reduce64(acc[t], f), f);
+                    }
                 }
             }
             if (i + 1 < nbp) grid.sync();

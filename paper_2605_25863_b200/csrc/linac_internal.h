@@ -38,8 +38,9 @@ void set_cuda_error(cudaError_t e, const char* what, const char* file, int line)
 struct Options {
     int64_t gemm_path = 0;    // 0 = auto, 1 = CUDA-core (SIMT) only, 2 = tensor (tcgen05) where legal
     int64_t timing = 0;       // 1 = bracket update kernels with events (costs syncs; for profiling runs)
-    int64_t tc_min_k = 256;   // smallest K the tensor path is used for
-    int64_t tc_min_mn = 512;  // smallest M and N the tensor path is used for
+    int64_t tc_min_k = 128;   // smallest K the tensor path is used for
+    int64_t tc_min_mn = 128;  // smallest M and N the tensor path is used for
+    int64_t flat_cols = 16384; // nodes of at most this many columns are swept flat (right-looking), wider ones recurse
     int64_t strip_width = 128; // columns factored by one cooperative strip kernel (multiple of 32, <= 256)
 };
 Options& options();
