@@ -25,8 +25,10 @@
 #include <mutex>
 
 #include "linac_internal.h"
+#include "tc_ptx.cuh"
 
 namespace linac {
+using namespace tc;
 namespace {
 
 constexpr int TM = 128;          // output tile rows  (UMMA M)
@@ -39,83 +41,6 @@ constexpr int SMEM_BYTES = STAGES * (A_STAGE + B_STAGE) + 1024 /*align*/ + 256 /
 constexpr int TMEM_COLS = 512;
 constexpr int NTHREADS = 192;    // warp 0: TMA, warp 1: MMA + TMEM alloc, warps 2..5: epilogue
 constexpr int64_t KC_MAX = 4096;
-
-// ----------------------------------------------------------------------------- PTX helpers
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred P1;\n\t"
-        "WAIT_LOOP:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
-        "@P1 bra DONE;\n\t"
-        "bra WAIT_LOOP;\n\t"
-        "DONE:\n\t"
-        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-
-__device__ __forceinline__ void tma_load_3d(void* smem_dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2) {
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
-        ::"r"(smem_u32(smem_dst)), "l"(tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
-}
-__device__ __forceinline__ void prefetch_tmap(const CUtensorMap* tm) {
-    asm volatile("prefetch.tensormap [%0];" ::"l"(tm) : "memory");
-}
-
-__device__ __forceinline__ void tmem_alloc(uint32_t* holder_smem, uint32_t ncols) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(holder_smem)), "r"(ncols) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
-}
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-
-// D[tmem] (+)= A[smem desc] . B[smem desc]^T, unsigned 8-bit operands, s32 accumulate.
-__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc, uint32_t accumulate) {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "setp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t"
-        "}" ::"r"(tmem_d), "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate) : "memory");
-}
-// mbarrier arrives when all previously issued tcgen05.mma of this thread have completed.
-__device__ __forceinline__ void umma_commit(uint64_t* bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&r)[8]) {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
-                 : "r"(taddr));
-}
-__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-
-// K-major operand tile, 128-byte swizzle: rows of 128 bytes, 8-row groups 1024 bytes apart.
-__device__ __forceinline__ uint64_t make_desc_sw128(uint32_t saddr) {
-    uint64_t d = 0;
-    d |= (uint64_t)((saddr >> 4) & 0x3FFF);          // start address
-    d |= (uint64_t)1 << 16;                          // leading byte offset (unused for swizzled K-major)
-    d |= (uint64_t)(1024 >> 4) << 32;                // stride byte offset between 8-row groups
-    d |= (uint64_t)1 << 46;                          // descriptor version (Blackwell)
-    d |= (uint64_t)2 << 61;                          // SWIZZLE_128B
-    return d;
-}
-// kind::i8 instruction descriptor: D = s32, A/B unsigned 8-bit, both K-major, M = 128.
-__host__ __device__ constexpr uint32_t make_idesc_i8(int n) {
-    return (2u << 4) | (0u << 7) | (0u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(TM >> 4) << 24);
-}
 
 // ----------------------------------------------------------------------------- the GEMM kernel
 __global__ void __launch_bounds__(NTHREADS, 1)
@@ -248,6 +173,221 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     }
 }
 
+// ----------------------------------------------------------------------------- the small-K (panel) kernel
+// K <= 256 is the Schur update behind ONE strip: every output element is read and written once per
+// 128..256 field products, so the epilogue and the C traffic weigh as much as the MMAs.  This kernel is
+// persistent (one CTA per SM), A-stationary (the 128-row limb planes of L21 stay in shared memory while
+// the CTA sweeps a run of 32-column output tiles), and overlaps the three stages of a tile:
+//   warp 0      TMA producer: A k-stages (ring of 2 x 64 KB) and B k-stages (ring of 4 x 16 KB)
+//   warp 1      MMA issuer: 128x128x32 kind::i8 MMAs (four B limb planes stacked along N), two TMEM
+//               accumulator buffers of 7 x 32 columns
+//   warps 2-9   epilogue: tcgen05.ld, limb recombination sum_w S_w (2^(8w) mod p), one Barrett reduction,
+//               C tile staged through shared memory by TMA in both directions (128-byte swizzle), so no
+//               thread-per-row global access ever reaches the LSU.
+constexpr int PN = 32;                       // output tile columns
+constexpr int P_A_STAGE = 4 * TM * KB;       // 65536
+constexpr int P_B_STAGE = 4 * PN * KB;       // 16384
+constexpr int P_C_TILE = TM * PN * 4;        // 16384
+constexpr int P_NAS = 2, P_NBS = 4;
+constexpr int P_SMEM = P_NAS * P_A_STAGE + P_NBS * P_B_STAGE + 2 * P_C_TILE + 1024 + 256;
+constexpr int P_THREADS = 320;
+constexpr int P_ACC_COLS = 256;              // TMEM columns reserved per accumulator buffer (224 used)
+
+struct PanelSched {
+    int mtiles, ntiles, nchunks, tiles_per_chunk, nitems;
+};
+
+struct TileIter {
+    int item, mt, nt, nt_end;
+    bool valid;
+    __device__ __forceinline__ void load_item(const PanelSched& sc) {
+        valid = item < sc.nitems;
+        if (!valid) return;
+        mt = item / sc.nchunks;
+        const int ch = item % sc.nchunks;
+        nt = ch * sc.tiles_per_chunk;
+        nt_end = min(sc.ntiles, nt + sc.tiles_per_chunk);
+    }
+    __device__ __forceinline__ void init(const PanelSched& sc) { item = blockIdx.x; load_item(sc); }
+    __device__ __forceinline__ bool last_of_item() const { return nt + 1 >= nt_end; }
+    __device__ __forceinline__ void next(const PanelSched& sc) {
+        if (++nt >= nt_end) { item += gridDim.x; load_item(sc); }
+    }
+};
+
+__global__ void __launch_bounds__(P_THREADS, 1)
+gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+                     const __grid_constant__ CUtensorMap tmC, int nks /* k-stages: kp / 128 */, PanelSched sc, ModP f) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    uint8_t* sA = smem;
+    uint8_t* sB = sA + P_NAS * P_A_STAGE;
+    uint8_t* sC = sB + P_NBS * P_B_STAGE;
+    uint64_t* bars = (uint64_t*)(sC + 2 * P_C_TILE);
+    uint64_t* a_full = bars;                 // [2]
+    uint64_t* a_empty = bars + 2;            // [2]
+    uint64_t* b_full = bars + 4;             // [4]
+    uint64_t* b_empty = bars + 8;            // [4]
+    uint64_t* acc_full = bars + 12;          // [2]
+    uint64_t* acc_empty = bars + 14;         // [2]
+    uint64_t* c_full = bars + 16;            // [2]
+    uint32_t* tmem_holder = (uint32_t*)(bars + 18);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (warp == 0 && lane == 0) {
+        prefetch_tmap(&tmA);
+        prefetch_tmap(&tmB);
+        prefetch_tmap(&tmC);
+        for (int i = 0; i < 2; ++i) { mbar_init(&a_full[i], 1); mbar_init(&a_empty[i], 1); mbar_init(&acc_full[i], 1);
+                                      mbar_init(&acc_empty[i], 8); mbar_init(&c_full[i], 1); }
+        for (int i = 0; i < P_NBS; ++i) { mbar_init(&b_full[i], 1); mbar_init(&b_empty[i], 1); }
+        fence_barrier_init();
+    }
+    if (warp == 1) tmem_alloc(tmem_holder, TMEM_COLS);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_holder;
+
+    if (warp == 0) {
+        if (lane == 0) {
+            uint32_t a_cnt = 0, b_cnt = 0;
+            TileIter it;
+            it.init(sc);
+            while (it.valid) {
+                for (int ks = 0; ks < nks; ++ks, ++a_cnt) {
+                    const int s = a_cnt % P_NAS;
+                    mbar_wait(&a_empty[s], ((a_cnt / P_NAS) & 1) ^ 1);
+                    mbar_expect_tx(&a_full[s], P_A_STAGE);
+                    tma_load_3d(sA + s * P_A_STAGE, &tmA, &a_full[s], ks * KB, it.mt * TM, 0);
+                }
+                const int item = it.item;
+                while (it.valid && it.item == item) {
+                    for (int ks = 0; ks < nks; ++ks, ++b_cnt) {
+                        const int s = b_cnt % P_NBS;
+                        mbar_wait(&b_empty[s], ((b_cnt / P_NBS) & 1) ^ 1);
+                        mbar_expect_tx(&b_full[s], P_B_STAGE);
+                        tma_load_3d(sB + s * P_B_STAGE, &tmB, &b_full[s], ks * KB, it.nt * PN, 0);
+                    }
+                    it.next(sc);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        if (lane == 0) {
+            constexpr uint32_t id128 = make_idesc_i8(4 * PN), id96 = make_idesc_i8(3 * PN), id32 = make_idesc_i8(PN);
+            uint32_t a_cnt = 0, b_cnt = 0, t_cnt = 0;
+            TileIter it;
+            it.init(sc);
+            while (it.valid) {
+                const int item = it.item;
+                bool first_tile = true;
+                while (it.valid && it.item == item) {
+                    const uint32_t buf = t_cnt & 1;
+                    mbar_wait(&acc_empty[buf], ((t_cnt >> 1) & 1) ^ 1);
+                    tc_fence_after();
+                    const uint32_t d0 = tmem_base + buf * P_ACC_COLS;
+                    const bool last = it.last_of_item();
+                    for (int ks = 0; ks < nks; ++ks, ++b_cnt) {
+                        const uint32_t ac = a_cnt + ks;
+                        const int sa = ac % P_NAS;
+                        if (first_tile) mbar_wait(&a_full[sa], (ac / P_NAS) & 1);
+                        const int sb = b_cnt % P_NBS;
+                        mbar_wait(&b_full[sb], (b_cnt / P_NBS) & 1);
+                        tc_fence_after();
+                        const uint32_t a0 = smem_u32(sA + sa * P_A_STAGE), b0 = smem_u32(sB + sb * P_B_STAGE);
+#pragma unroll
+                        for (int kk = 0; kk < KB / 32; ++kk) {
+                            const uint32_t ko = kk * 32;
+                            if (ks == 0 && kk == 0) {
+                                // first k step of the tile: slots 0-3 and 4-6 are overwritten, the rest accumulate
+                                umma_i8(d0, make_desc_sw128(a0), make_desc_sw128(b0), id128, 0u);
+                                umma_i8(d0 + 4 * PN, make_desc_sw128(a0 + 3 * (TM * KB)), make_desc_sw128(b0 + PN * KB), id96, 0u);
+                                umma_i8(d0 + 1 * PN, make_desc_sw128(a0 + 1 * (TM * KB)), make_desc_sw128(b0), id128, 1u);
+                                umma_i8(d0 + 2 * PN, make_desc_sw128(a0 + 2 * (TM * KB)), make_desc_sw128(b0), id128, 1u);
+                                umma_i8(d0 + 3 * PN, make_desc_sw128(a0 + 3 * (TM * KB)), make_desc_sw128(b0), id32, 1u);
+                            } else {
+#pragma unroll
+                                for (int i = 0; i < 4; ++i)
+                                    umma_i8(d0 + i * PN, make_desc_sw128(a0 + i * (TM * KB) + ko), make_desc_sw128(b0 + ko), id128, 1u);
+                            }
+                        }
+                        umma_commit(&b_empty[sb]);
+                        if (last) umma_commit(&a_empty[sa]);
+                    }
+                    umma_commit(&acc_full[buf]);
+                    ++t_cnt;
+                    first_tile = false;
+                    it.next(sc);
+                }
+                a_cnt += nks;
+            }
+        }
+    } else {
+        const int e = warp - 2, q = warp & 3, h = e >> 2;
+        const int row = q * 32 + lane;
+        const bool elected = threadIdx.x == 64;
+        const uint64_t w4 = f.w[4], w5 = f.w[5], w6 = f.w[6];
+        uint32_t t_cnt = 0;
+        TileIter it;
+        it.init(sc);
+        if (elected && it.valid) {
+            mbar_expect_tx(&c_full[0], P_C_TILE);
+            tma_load_2d(sC, &tmC, &c_full[0], it.nt * PN, it.mt * TM);
+        }
+        while (it.valid) {
+            const uint32_t buf = t_cnt & 1, ph = (t_cnt >> 1) & 1;
+            const int mt = it.mt, nt = it.nt;
+            it.next(sc);
+            if (elected && it.valid) {
+                tma_store_wait_read0();          // the store that last read the other C buffer is done with it
+                mbar_expect_tx(&c_full[buf ^ 1], P_C_TILE);
+                tma_load_2d(sC + (buf ^ 1) * P_C_TILE, &tmC, &c_full[buf ^ 1], it.nt * PN, it.mt * TM);
+            }
+            mbar_wait(&acc_full[buf], ph);
+            tc_fence_after();
+            uint32_t S[7][16];
+            const uint32_t t0 = tmem_base + ((uint32_t)(q * 32) << 16) + buf * P_ACC_COLS + h * 16;
+#pragma unroll
+            for (int w = 0; w < 7; ++w) tmem_ld16(t0 + w * PN, S[w]);
+            tmem_ld_wait();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&acc_empty[buf]);
+            mbar_wait(&c_full[buf], ph);
+            uint8_t* crow = sC + buf * P_C_TILE + row * 128;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                uint4* pc = reinterpret_cast<uint4*>(crow + (((4 * h + j) ^ (row & 7)) << 4));
+                uint4 c4 = *pc;
+                uint32_t cv[4] = {c4.x, c4.y, c4.z, c4.w};
+#pragma unroll
+                for (int x = 0; x < 4; ++x) {
+                    const int el = 4 * j + x;
+                    uint64_t v = (uint64_t)S[0][el] + ((uint64_t)S[1][el] << 8) + ((uint64_t)S[2][el] << 16) + ((uint64_t)S[3][el] << 24);
+                    v += (uint64_t)S[4][el] * w4 + (uint64_t)S[5][el] * w5 + (uint64_t)S[6][el] * w6;
+                    cv[x] = submod(cv[x], reduce64(v, f), f);
+                }
+                *pc = make_uint4(cv[0], cv[1], cv[2], cv[3]);
+            }
+            fence_proxy_async();
+            asm volatile("bar.sync 1, 256;" ::: "memory");
+            if (elected) {
+                tma_store_2d(&tmC, sC + buf * P_C_TILE, nt * PN, mt * TM);
+                tma_store_commit();
+            }
+            ++t_cnt;
+        }
+        if (elected) tma_store_wait_all();
+        tc_fence_before();
+    }
+    __syncthreads();
+    if (warp == 1) {
+        tc_fence_after();
+        tmem_dealloc(tmem_base, TMEM_COLS);
+    }
+}
+
 // ----------------------------------------------------------------------------- limb-split pre-passes
 // Aq[limb][m][kp]: row m, k-major, zero padded to kp.  One thread packs 4 consecutive k.
 __global__ void split_a_kernel(const uint32_t* __restrict__ Ab, int64_t lda, const int32_t* __restrict__ kcols, int64_t k0,
@@ -328,6 +468,45 @@ bool make_limb_map(CUtensorMap* tm, uint8_t* base, int64_t rows, int64_t kp, int
     return r == CUDA_SUCCESS;
 }
 
+// 2-D map over C (uint32, row-major): box = 32 columns x 128 rows, 128-byte swizzle.
+bool make_c_map(CUtensorMap* tm, uint32_t* C, int64_t ldc, int64_t M, int64_t N) {
+    EncodeTiledFn enc = get_encode_fn();
+    if (!enc) return false;
+    cuuint64_t dims[2] = {(cuuint64_t)N, (cuuint64_t)M};
+    cuuint64_t strides[1] = {(cuuint64_t)ldc * 4};
+    cuuint32_t box[2] = {(cuuint32_t)PN, (cuuint32_t)TM};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, C, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+int sm_count() {
+    static int sms = 0;
+    if (!sms) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    }
+    return sms;
+}
+
+// Work items of the panel kernel: (128-row tile, run of 32-column tiles); run length chosen so that the
+// items fill a whole number of waves over the persistent grid with runs of about 24 tiles.
+PanelSched make_sched(int64_t M, int64_t N, int grid) {
+    PanelSched sc;
+    sc.mtiles = (int)((M + TM - 1) / TM);
+    sc.ntiles = (int)((N + PN - 1) / PN);
+    const int64_t total = (int64_t)sc.mtiles * sc.ntiles;
+    const int64_t waves = std::max<int64_t>(1, (total + (int64_t)grid * 24 - 1) / ((int64_t)grid * 24));
+    int64_t nchunks = (waves * grid + sc.mtiles - 1) / sc.mtiles;
+    nchunks = std::max<int64_t>(1, std::min<int64_t>(nchunks, sc.ntiles));
+    sc.tiles_per_chunk = (int)((sc.ntiles + nchunks - 1) / nchunks);
+    sc.nchunks = (sc.ntiles + sc.tiles_per_chunk - 1) / sc.tiles_per_chunk;
+    sc.nitems = sc.mtiles * sc.nchunks;
+    return sc;
+}
+
 int64_t chunk_k(int64_t K) {
     // equal chunks of at most KC_MAX, each a multiple of KB
     const int64_t nchunks = (K + KC_MAX - 1) / KC_MAX;
@@ -352,6 +531,42 @@ int gemm_modp_tc(const GemmArgs& g, const ModP& f, cudaStream_t s, Arena* scratc
             return -1;
         }
         attr_set = true;
+    }
+    const bool panel_ok = g.K <= 2 * KB && options().tc_panel != 0 && ((((uintptr_t)g.C) | ((uintptr_t)g.ldc * 4)) & 15) == 0;
+    if (panel_ok) {
+        static bool pattr = false;
+        if (!pattr) {
+            if (cudaFuncSetAttribute(gemm_tc_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM) != cudaSuccess) {
+                cudaGetLastError();
+                return -1;
+            }
+            pattr = true;
+        }
+        const int64_t kp = (g.K + KB - 1) / KB * KB;
+        uint8_t* Aq = (uint8_t*)scratch->take((size_t)4 * g.M * kp, 1024);
+        uint8_t* Bq = (uint8_t*)scratch->take((size_t)4 * g.N * kp, 1024);
+        if (!Aq || !Bq) return -1;
+        {
+            dim3 grid((unsigned)((kp / 4 + 127) / 128), (unsigned)std::min<int64_t>(g.M, 16384));
+            split_a_kernel<<<grid, 128, 0, s>>>(g.Abase, g.lda, g.kcols, 0, g.M, g.K, kp, Aq);
+            LINAC_CUDA(cudaGetLastError());
+        }
+        {
+            dim3 grid((unsigned)(kp / 128), (unsigned)((g.N + 31) / 32));
+            split_b_kernel<<<grid, 256, 0, s>>>(g.B, g.ldb, g.K, g.N, kp, Bq);
+            LINAC_CUDA(cudaGetLastError());
+        }
+        CUtensorMap tmA, tmB, tmC;
+        if (!make_limb_map(&tmA, Aq, g.M, kp, TM) || !make_limb_map(&tmB, Bq, g.N, kp, PN) || !make_c_map(&tmC, g.C, g.ldc, g.M, g.N))
+            return -1;
+        const int grid = sm_count();
+        const PanelSched sc = make_sched(g.M, g.N, grid);
+        gemm_tc_panel_kernel<<<(unsigned)std::min(grid, sc.nitems), P_THREADS, P_SMEM, s>>>(tmA, tmB, tmC, (int)(kp / KB), sc, f);
+        LINAC_CUDA(cudaGetLastError());
+        stats().kernel_launches += 3;
+        stats().tc_launches++;
+        stats().update_macs += g.M * g.N * g.K;
+        return LINAC_OK;
     }
     const int64_t kc = chunk_k(g.K);
     uint8_t* Aq = (uint8_t*)scratch->take((size_t)4 * g.M * kc, 1024);

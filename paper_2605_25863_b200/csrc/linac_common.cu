@@ -165,6 +165,9 @@ int linac_set_option(const char* name, int64_t value) {
     } else if (!strcmp(name, "tc_min_mn")) {
         if (value < 128) return LINAC_ERR_INVALID_ARG;
         g_options.tc_min_mn = value;
+    } else if (!strcmp(name, "tc_panel")) {
+        if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
+        g_options.tc_panel = value;
     } else if (!strcmp(name, "flat_cols")) {
         if (value < 0) return LINAC_ERR_INVALID_ARG;
         g_options.flat_cols = value;

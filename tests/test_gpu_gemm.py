@@ -33,7 +33,9 @@ def expected(oracle, c, a, b, p):
 
 SHAPES = [(1, 1, 1), (5, 7, 3), (128, 64, 16), (129, 65, 17), (200, 300, 100), (257, 130, 33)]
 TC_SHAPES = [(128, 64, 128), (128, 64, 32), (256, 128, 256), (300, 200, 150), (512, 512, 512), (1000, 900, 700),
-             (640, 576, 4224), (130, 70, 1)]
+             (640, 576, 4224), (130, 70, 1),
+             # K <= 256: the persistent A-stationary panel kernel (several items per CTA, ragged M and N tiles)
+             (1000, 2100, 256), (3000, 1500, 128), (5000, 40, 200), (20000, 100, 256)]
 
 
 @pytest.mark.parametrize("m,n,k", SHAPES + TC_SHAPES)
@@ -73,3 +75,15 @@ def test_tensor_core_worst_case_operands(oracle):
     assert (out == want).all()
     out1, _ = run_gemm(c, a, b, P31, path=1)
     assert (out1 == want).all()
+
+
+@pytest.mark.parametrize("k", [128, 256])
+def test_panel_kernel_worst_case_operands(k):
+    """All entries p-1 at the panel kernel's largest K: every limb product at its maximum."""
+    m, n = 300, 100
+    a = np.full((m, k), P31 - 1, dtype=np.uint32)
+    b = np.full((k, n), P31 - 1, dtype=np.uint32)
+    c = np.zeros((m, n), dtype=np.uint32)
+    out, st = run_gemm(c, a, b, P31, path=2)
+    assert st["tc_launches"] == 1
+    assert (out == (-(k * pow(P31 - 1, 2, P31))) % P31).all()
