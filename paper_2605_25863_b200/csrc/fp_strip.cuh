@@ -73,7 +73,7 @@ struct StripSmem {
 // path, which handles rank-deficient and multi-chunk panels.
 __device__ bool panel_fast(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t i0, int64_t j0, const ModP& f) {
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
-    constexpr int FW = 8, RPW = PW / FW;          // 8 working warps, 4 block rows each (registers)
+    constexpr int FW = 16, RPW = PW / FW;         // 16 working warps, 2 block rows each (registers)
     uint32_t x[RPW];
     if (wq < FW) {
 #pragma unroll

@@ -188,8 +188,8 @@ constexpr int PN = 32;                       // output tile columns
 constexpr int P_A_STAGE = 4 * TM * KB;       // 65536
 constexpr int P_B_STAGE = 4 * PN * KB;       // 16384
 constexpr int P_C_TILE = TM * PN * 4;        // 16384
-constexpr int P_NAS = 2, P_NBS = 4;
-constexpr int P_SMEM = P_NAS * P_A_STAGE + P_NBS * P_B_STAGE + 2 * P_C_TILE + 1024 + 256;
+constexpr int P_NAS = 2, P_NBS = 3, P_NCS = 3;
+constexpr int P_SMEM = P_NAS * P_A_STAGE + P_NBS * P_B_STAGE + P_NCS * P_C_TILE + 1024 + 256;
 constexpr int P_THREADS = 320;
 constexpr int P_ACC_COLS = 256;              // TMEM columns reserved per accumulator buffer (224 used)
 
@@ -223,15 +223,15 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
     uint8_t* sA = smem;
     uint8_t* sB = sA + P_NAS * P_A_STAGE;
     uint8_t* sC = sB + P_NBS * P_B_STAGE;
-    uint64_t* bars = (uint64_t*)(sC + 2 * P_C_TILE);
+    uint64_t* bars = (uint64_t*)(sC + P_NCS * P_C_TILE);
     uint64_t* a_full = bars;                 // [2]
     uint64_t* a_empty = bars + 2;            // [2]
     uint64_t* b_full = bars + 4;             // [4]
     uint64_t* b_empty = bars + 8;            // [4]
     uint64_t* acc_full = bars + 12;          // [2]
     uint64_t* acc_empty = bars + 14;         // [2]
-    uint64_t* c_full = bars + 16;            // [2]
-    uint32_t* tmem_holder = (uint32_t*)(bars + 18);
+    uint64_t* c_full = bars + 16;            // [3]
+    uint32_t* tmem_holder = (uint32_t*)(bars + 20);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (warp == 0 && lane == 0) {
@@ -239,7 +239,8 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
         prefetch_tmap(&tmB);
         prefetch_tmap(&tmC);
         for (int i = 0; i < 2; ++i) { mbar_init(&a_full[i], 1); mbar_init(&a_empty[i], 1); mbar_init(&acc_full[i], 1);
-                                      mbar_init(&acc_empty[i], 8); mbar_init(&c_full[i], 1); }
+                                      mbar_init(&acc_empty[i], 8); }
+        for (int i = 0; i < P_NCS; ++i) mbar_init(&c_full[i], 1);
         for (int i = 0; i < P_NBS; ++i) { mbar_init(&b_full[i], 1); mbar_init(&b_empty[i], 1); }
         fence_barrier_init();
     }
@@ -337,12 +338,13 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
         }
         while (it.valid) {
             const uint32_t buf = t_cnt & 1, ph = (t_cnt >> 1) & 1;
+            const uint32_t cb = t_cnt % P_NCS, cph = (t_cnt / P_NCS) & 1, cbn = (t_cnt + 1) % P_NCS;
             const int mt = it.mt, nt = it.nt;
             it.next(sc);
             if (elected && it.valid) {
-                tma_store_wait_read0();          // the store that last read the other C buffer is done with it
-                mbar_expect_tx(&c_full[buf ^ 1], P_C_TILE);
-                tma_load_2d(sC + (buf ^ 1) * P_C_TILE, &tmC, &c_full[buf ^ 1], it.nt * PN, it.mt * TM);
+                tma_store_wait_read1();          // the store that last read C buffer cbn (two tiles ago) is done with it
+                mbar_expect_tx(&c_full[cbn], P_C_TILE);
+                tma_load_2d(sC + cbn * P_C_TILE, &tmC, &c_full[cbn], it.nt * PN, it.mt * TM);
             }
             mbar_wait(&acc_full[buf], ph);
             tc_fence_after();
@@ -354,8 +356,8 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(&acc_empty[buf]);
-            mbar_wait(&c_full[buf], ph);
-            uint8_t* crow = sC + buf * P_C_TILE + row * 128;
+            mbar_wait(&c_full[cb], cph);
+            uint8_t* crow = sC + cb * P_C_TILE + row * 128;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 uint4* pc = reinterpret_cast<uint4*>(crow + (((4 * h + j) ^ (row & 7)) << 4));
@@ -373,7 +375,7 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             fence_proxy_async();
             asm volatile("bar.sync 1, 256;" ::: "memory");
             if (elected) {
-                tma_store_2d(&tmC, sC + buf * P_C_TILE, nt * PN, mt * TM);
+                tma_store_2d(&tmC, sC + cb * P_C_TILE, nt * PN, mt * TM);
                 tma_store_commit();
             }
             ++t_cnt;
