@@ -250,6 +250,8 @@ def main():
                 "note": "peak = 148 SM x 64 IMAD lanes x max SM clock (DESIGN.md); "
                         "achieved = executed update MACs / summed event time of the update kernels"}
     roof["update_share_of_step"] = ms_upd / st_t["ms_total"] if st_t["ms_total"] else None
+    roof["timed_split_ms"] = {"update": ms_upd, "strip": st_t.get("ms_strip"), "trsm": st_t.get("ms_trsm"),
+                              "total_with_timing_syncs": st_t["ms_total"]}
 
     out = {
         "metric": "rref_gmulmod_per_s", "value": value, "unit": "Gmulmod/s", "n_gpus": world, "steps": args.steps,

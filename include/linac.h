@@ -142,6 +142,8 @@ typedef struct {
     int64_t tc_launches;         /* Schur updates that ran on the tensor-core (tcgen05) path      */
     double  ms_update;           /* device ms spent in the Schur-update (GEMM) kernels, if timed  */
     double  ms_total;            /* device ms of the whole call, if timed                         */
+    double  ms_strip;            /* device ms in the cooperative strip kernels (S1-S4), if timed   */
+    double  ms_trsm;             /* device ms in the triangular-solve leaf kernels, if timed       */
 } linac_stats;
 int linac_get_last_stats(linac_stats *out);
 /* Tunables, mainly for A/B measurements: name in {"gemm_path" (0 auto, 1 CUDA-core, 2 tensor), "timing" (0/1), "tc_min_k", "tc_min_mn",

@@ -70,6 +70,19 @@ int run_gemm(Fp& c, const GemmArgs& g) {
     return rc;
 }
 
+// Brackets one kernel class with events when the "timing" option is on (costs a host sync per launch).
+struct Timed {
+    Fp& c; double& acc; bool on;
+    Timed(Fp& c_, double& acc_) : c(c_), acc(acc_), on(options().timing != 0) { if (on) cudaEventRecord(c.ev0, c.s); }
+    ~Timed() {
+        if (!on) return;
+        cudaEventRecord(c.ev1, c.s);
+        cudaEventSynchronize(c.ev1);
+        float ms = 0;
+        if (cudaEventElapsedTime(&ms, c.ev0, c.ev1) == cudaSuccess) acc += ms;
+    }
+};
+
 size_t trsm_smem_bytes(int64_t K) { return (size_t)K * PW * 4 + (size_t)PW * (PW + 1) * 4; }
 
 // Leaf of both triangular solves: the pivots of ONE strip against columns [0, ncols) of X.
@@ -78,6 +91,7 @@ int trsm_leaf(Fp& c, int64_t s, uint32_t* X, int64_t ldx, int64_t ncols) {
     const int64_t K = c.sp(s + 1) - c.sp(s);
     if (K <= 0 || ncols <= 0) return LINAC_OK;
     if (!LOWER && c.sb0(s + 1) - c.sb0(s) <= 1) return LINAC_OK;     // U is the identity inside one base panel
+    Timed tm(c, stats().ms_trsm);
     trsm_strip_kernel<LOWER><<<(unsigned)((ncols + PW - 1) / PW), TNT, trsm_smem_bytes(K), c.s>>>(
         c.A, c.ld, X, ldx, ncols, c.d_pstart, (int)c.sb0(s), (int)c.sb0(s + 1), c.d_T, c.d_pivcols, c.f);
     LINAC_CUDA(cudaGetLastError());
@@ -109,16 +123,31 @@ int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r) {
     const int64_t b0 = c.sb0(s), b1 = c.sb0(s + 1);
     const int64_t j0 = panel_col0(b0), j1 = std::min(c.cols, panel_col0(b1));
     StripArgs a;
-    a.A = c.A; a.ld = c.ld; a.rows = c.rows; a.cols = c.cols; a.i0 = i0; a.j0 = j0; a.ws = (int)(j1 - j0); a.f = c.f;
+    a.A = c.A; a.ld = c.ld; a.rows = c.rows; a.cols = c.cols; a.i0 = i0; a.j0 = j0; a.ws = (int)(j1 - j0);
     a.rec = c.d_rec; a.T = c.d_T; a.E = c.d_E; a.pivcols = c.d_pivcols; a.pstart = c.d_pstart;
     void* args[] = {&a};
-    LINAC_CUDA(cudaLaunchCooperativeKernel((void*)strip_factor_kernel, dim3((unsigned)c.coop_grid), dim3(SNT), args,
-                                           sizeof(StripSmem), c.s));
+    {
+        Timed tm(c, stats().ms_strip);
+        LINAC_CUDA(cudaLaunchCooperativeKernel((void*)strip_factor_kernel, dim3((unsigned)c.coop_grid), dim3(SNT), args,
+                                               sizeof(StripSmem), c.s));
+    }
     LINAC_CUDA(cudaMemcpyAsync(c.h_rec, c.d_rec + b0, (size_t)(b1 - b0) * sizeof(PanelRec), cudaMemcpyDeviceToHost, c.s));
     LINAC_CUDA(cudaStreamSynchronize(c.s));
     linac_stats& st = stats();
     st.kernel_launches++;
     st.host_syncs++;
+#ifdef LINAC_TRACE
+    if (s == 0 || s == c.ns / 2) {
+        unsigned long long h[64];
+        cudaMemcpyFromSymbol(h, g_strip_trace, sizeof h);
+        for (int ct = 0; ct < 2; ++ct) {
+            printf("strip %ld cta %d panel 1 (ns since phase A start):", (long)s, ct);
+            for (int k = 1; k < 10; ++k) printf(" [%d]%lld", k, h[ct * 32 + k] ? (long long)(h[ct * 32 + k] - h[ct * 32]) : -1ll);
+            printf("\n");
+        }
+        printf("  P1 loop cycles: search %llu  pivot-row %llu  update %llu  barrier %llu\n", h[40], h[41], h[42], h[43]);
+    }
+#endif
     int64_t cur = i0;
     for (int64_t b = b0; b < b1; ++b) {
         const PanelRec& h = c.h_rec[b - b0];
@@ -305,6 +334,7 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     LINAC_CUDA(cudaEventCreate(&t1));
     LINAC_CUDA(cudaEventRecord(t0, s));
 
+    LINAC_CUDA(cudaMemcpyToSymbolAsync(c_f, &c.f, sizeof(ModP), 0, cudaMemcpyHostToDevice, s));
     // S0 ingest
     {
         dim3 grid((unsigned)((cols + 255) / 256), (unsigned)std::min<int64_t>(rows, 2048));

@@ -25,6 +25,21 @@
 namespace linac {
 namespace cg = cooperative_groups;
 
+// Debug build only (-DLINAC_TRACE, see build.py): %globaltimer stamps of CTA 0 / CTA 1 for the first
+// panel of a strip, printed by the host after the launch.
+#ifdef LINAC_TRACE
+__device__ unsigned long long g_strip_trace[64];
+#define STRIP_STAMP(slot) do { if (threadIdx.x == 0 && blockIdx.x < 2 && g_trace_on) { unsigned long long t_; \
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_)); g_strip_trace[blockIdx.x * 32 + (slot)] = t_; } } while (0)
+__device__ int g_trace_on = 0;
+#else
+#define STRIP_STAMP(slot) do { } while (0)
+#endif
+
+// The field of the running call (set once per call by the host, cudaMemcpyToSymbolAsync on the call's
+// stream): read through the constant bank, so no device function carries it in registers or on the stack.
+__constant__ ModP c_f;
+
 constexpr int SW_MAX = 256;                 // widest strip (columns)
 constexpr int SNT = 1024;                   // threads per CTA of the strip kernel (32 warps)
 constexpr int SRB = 256;                    // rows of one P2 tile
@@ -34,6 +49,12 @@ constexpr int MAXBP = SW_MAX / PW;          // base panels per strip
 __device__ __forceinline__ uint32_t lincomb(uint32_t d, uint32_t x, uint32_t h, uint32_t y, const ModP& f) {
     return reduce64((uint64_t)d * x + (uint64_t)(f.p - h) * y, f);
 }
+
+struct UPending {
+    long long row0;                  // first pivot row (absolute), or -1 if nothing is pending
+    long long col0;
+    int r, nc;
+};
 
 struct StripSmem {
     // ---- P1
@@ -52,12 +73,9 @@ struct StripSmem {
     // ---- P2
     uint32_t Ts[PW][PW + 1];
     uint32_t Ar[PW][PW + 1];
-    __align__(16) uint32_t Us[PW][PW];       // this CTA's slice of U12 (kept until the deferred write-back)
+    __align__(16) uint32_t Us[2][PW][PW];    // this CTA's U12 slices (slot 0: next panel's columns, slot 1: the rest)
     __align__(16) uint32_t Lk[PW][SRB + 4];  // L tile, k-major (pivot index, row)
-    // deferred write-back of Us
-    long long u_row0;                // first pivot row (absolute), or -1 if nothing is pending
-    long long u_col0;
-    int u_r, u_nc;
+    UPending pend[2];                // deferred write-back of Us[slot]
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -68,25 +86,35 @@ struct StripSmem {
 // holds the column of the accumulated transform that belongs to source row q, and g_k tracks the
 // scalar each row has been multiplied by (for q: the pivot value).  At the end
 //   T[a][b] = g_{q_a}^-1 * W[q_a][b],   q_a = the row that pivoted column a,
-// is the inverse of D = A[pivot rows in column order, panel].  Fails (returns false, nothing
+// is the inverse of D = A[pivot rows in column order, panel].  Every product here is a Montgomery product
+// (a*b*2^-32 mod p, four instructions instead of Barrett's fourteen): the extra factor 2^-32 only rescales
+// rows, which a division-free elimination does not care about, and the tracked scales absorb it.  Fails (returns false, nothing
 // written) as soon as a column has no pivot among the unused rows: the caller then runs the general
 // path, which handles rank-deficient and multi-chunk panels.
-__device__ bool panel_fast(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t i0, int64_t j0, const ModP& f) {
+__device__ __forceinline__ bool panel_fast(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t i0, int64_t j0) {
+    const ModP& f = c_f;
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
-    constexpr int FW = 16, RPW = PW / FW;         // 16 working warps, 2 block rows each (registers)
-    uint32_t x[RPW];
+    constexpr int FW = 8, RPW = PW / FW;          // 8 working warps, 4 block rows each (registers)
+    static_assert(RPW == 4, "the row macros below are written for four rows per warp");
+    uint32_t x0 = 0, x1 = 0, x2 = 0, x3 = 0;
+    const int row0 = wq * RPW;
     if (wq < FW) {
-#pragma unroll
-        for (int i = 0; i < RPW; ++i) x[i] = A[(i0 + wq * RPW + i) * ld + j0 + lane];
-#pragma unroll
-        for (int i = 0; i < RPW; ++i) sm.W[0][wq * RPW + i][lane] = x[i];
+        x0 = A[(i0 + row0 + 0) * ld + j0 + lane];
+        x1 = A[(i0 + row0 + 1) * ld + j0 + lane];
+        x2 = A[(i0 + row0 + 2) * ld + j0 + lane];
+        x3 = A[(i0 + row0 + 3) * ld + j0 + lane];
+        sm.W[0][row0 + 0][lane] = x0;
+        sm.W[0][row0 + 1][lane] = x1;
+        sm.W[0][row0 + 2][lane] = x2;
+        sm.W[0][row0 + 3][lane] = x3;
     }
     __syncthreads();
+    STRIP_STAMP(1);
     if (wq < FW) {
         unsigned used = 0;
         uint32_t dtot = 1u;                       // product of the pivots so far (the scale of every unused row)
         bool ok = true;
-#pragma unroll 2
+#pragma unroll 1
         for (int c = 0; c < PW; ++c) {
             const int buf = c & 1;
             const unsigned cand = __ballot_sync(0xffffffffu, sm.W[buf][lane][c] != 0) & ~used;
@@ -94,23 +122,28 @@ __device__ bool panel_fast(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t
             const int q = __ffs(cand) - 1;
             const uint32_t pv = sm.W[buf][q][lane];
             const uint32_t d = __shfl_sync(0xffffffffu, pv, c);
-            const uint32_t y = lane == c ? dtot : pv;         // slot c of the pivot row holds its scale
-#pragma unroll
-            for (int i = 0; i < RPW; ++i) {
-                const int row = wq * RPW + i;
-                const uint32_t h = __shfl_sync(0xffffffffu, x[i], c);
-                if (row != q) x[i] = lincomb(d, lane == c ? 0u : x[i], h, y, f);
-                else if (lane == c) x[i] = dtot;
-                sm.W[buf ^ 1][row][lane] = x[i];
+            const bool atc = lane == c;
+            const uint32_t y = atc ? dtot : pv;               // slot c of the pivot row holds its scale
+            // row <- d (x) row - h (x) pivot row for the rows that are not the pivot row; the pivot row keeps its
+            // entries and receives its scale in slot c
+#define FAST_ROW(X, I)                                                                                   \
+            {                                                                                            \
+                const uint32_t h = __shfl_sync(0xffffffffu, X, c);                                       \
+                const uint32_t upd = redc((uint64_t)d * (atc ? 0u : X) + (uint64_t)(f.p - h) * y, f);    \
+                X = (row0 + I) != q ? upd : (atc ? dtot : X);                                            \
+                sm.W[buf ^ 1][row0 + I][lane] = X;                                                       \
             }
+            FAST_ROW(x0, 0) FAST_ROW(x1, 1) FAST_ROW(x2, 2) FAST_ROW(x3, 3)
+#undef FAST_ROW
             if (tid == 0) { sm.esrc[c] = i0 + q; sm.gs[0][c] = dtot; }    // gs[0][c] = prefix product BEFORE step c
-            dtot = mulmod(dtot, d, f);
+            dtot = mulredc(dtot, d, f);
             used |= 1u << q;
             asm volatile("bar.sync 1, %0;" ::"n"(FW * 32) : "memory");
         }
         if (tid == 0) { sm.fast_ok = ok ? 1 : 0; sm.gs[1][0] = dtot; }
     }
     __syncthreads();
+    STRIP_STAMP(2);
     return sm.fast_ok != 0;     // on success the final block is in W[0] (32 steps); gs[1][0] = product of all pivots
 }
 
@@ -121,8 +154,8 @@ __device__ bool panel_fast(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t
 // Elimination is division-free (row_k <- d*row_k - h*row_q), so no modular inverse sits on the
 // column-to-column dependency chain.  The scan stops once w pivots are known; otherwise it has looked
 // at every row, which is what proves the remaining columns are free columns.  Returns r.
-__device__ int panel_scan(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t rows, int64_t i0, int64_t j0, int w,
-                          const ModP& f) {
+__device__ __noinline__ int panel_scan(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t rows, int64_t i0, int64_t j0, int w) {
+    const ModP& f = c_f;
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
     uint32_t (*X)[PW + 1] = sm.W[0];
     uint32_t (*Ep)[PW + 1] = sm.W[1];          // pivot rows as selected (unnormalised), discovery order
@@ -175,8 +208,9 @@ __device__ int panel_scan(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t 
 // pivot-column order (no search needed: pivot rows with a larger leading column vanish on the smaller
 // columns, so D has an LU factorisation without pivoting), division-free; leaves g (diagonal) and the
 // transform in G.  Also E = T.A[P, panel] when r < w.
-__device__ void panel_invert_general(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t j0, int w, int r, const ModP& f,
-                                     uint32_t* Tout, uint32_t* Eout) {
+__device__ __noinline__ void panel_invert_general(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t j0, int w, int r,
+                                                  uint32_t* Tout, uint32_t* Eout) {
+    const ModP& f = c_f;
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
     for (int e = tid; e < PW * 2 * PW; e += SNT) {
         const int a = e / (2 * PW), b = e % (2 * PW);
@@ -253,28 +287,30 @@ __device__ void panel_exchange_list(StripSmem& sm, int64_t i0, int r, PanelRec* 
 // Outputs: rec (r, local pivot columns, exchange list), T (32x32, zero padded), E = T A[P, panel] when
 // r < w (the free columns' entries of the reduced pivot rows), pivcols.
 __device__ void panel_factor(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t rows, int64_t i0, int64_t j0, int w,
-                             const ModP& f, PanelRec* rec, uint32_t* Tout, uint32_t* Eout, int32_t* pivcols_global) {
+                             PanelRec* rec, uint32_t* Tout, uint32_t* Eout, int32_t* pivcols_global) {
+    const ModP& f = c_f;
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
     int r = 0;
     bool fast = false;
-    if (w == PW && rows - i0 >= PW) fast = panel_fast(sm, A, ld, i0, j0, f);
+    if (w == PW && rows - i0 >= PW && f.ninv != 0) fast = panel_fast(sm, A, ld, i0, j0);
     if (fast) {
         // row q_a that pivoted column a has been scaled by g = (all pivots) / (pivots before step a), so
         // 1/g = prefix[a] / (all pivots): ONE modular inverse for the panel (K7)
         r = PW;
         if (tid < PW) { sm.epc[tid] = tid; sm.ord[tid] = tid; }
-        const uint32_t inv_all = invmod(sm.gs[1][0], f);
-        if (wq == 0) sm.ginv[lane] = mulmod(sm.gs[0][lane], inv_all, f);
+        // (with Montgomery products the identity reads 1/g_a = prefix[a] (x) 1/(all pivots))
+        if (wq == 0) sm.ginv[lane] = mulredc(sm.gs[0][lane], invmod_fermat(sm.gs[1][0], f), f);
         __syncthreads();
         if (wq == 0) panel_exchange_list(sm, i0, r, rec);
+        STRIP_STAMP(3);
         const int qa = (int)(sm.esrc[wq] - i0);
         Tout[wq * PW + lane] = mulmod(sm.ginv[wq], sm.W[0][qa][lane], f);
     } else {
         __syncthreads();
-        r = panel_scan(sm, A, ld, rows, i0, j0, w, f);
+        r = panel_scan(sm, A, ld, rows, i0, j0, w);
         if (wq == 0) panel_exchange_list(sm, i0, r, rec);
         __syncthreads();
-        panel_invert_general(sm, A, ld, j0, w, r, f, Tout, Eout);
+        panel_invert_general(sm, A, ld, j0, w, r, Tout, Eout);
     }
     if (tid < PW) {
         rec->pc[tid] = tid < r ? sm.epc[sm.ord[tid]] : -1;
@@ -287,6 +323,7 @@ __device__ void panel_factor(StripSmem& sm, const uint32_t* A, int64_t ld, int64
         rec->nswaps = sm.nsw;
         sm.r_out = r;
     }
+    STRIP_STAMP(4);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -298,7 +335,6 @@ struct StripArgs {
     int64_t i0;              // first active row
     int64_t j0;              // first column of the strip (multiple of PW)
     int ws;                  // strip width in columns
-    ModP f;
     PanelRec* rec;           // [nb]
     uint32_t* T;             // [nb][PW*PW]
     uint32_t* E;             // [nb][PW*PW]
@@ -306,12 +342,112 @@ struct StripArgs {
     int32_t* pstart;         // [nb+1]
 };
 
-__device__ __forceinline__ void strip_flush_u(StripSmem& sm, uint32_t* A, int64_t ld) {
-    if (sm.u_row0 < 0) return;
+// Deferred write-back of a U12 slice: the raw entries it replaces are read by every row worker of
+// the column block, so the owner (row worker 0) keeps the slice in shared memory until the next
+// grid barrier has passed.
+__device__ __forceinline__ void strip_flush_u(StripSmem& sm, int slot, uint32_t* A, int64_t ld) {
+    const UPending& u = sm.pend[slot];
+    if (u.row0 < 0) return;
     const int lane = threadIdx.x & 31, wq = threadIdx.x >> 5;
-    if (wq < sm.u_r && lane < sm.u_nc) A[(sm.u_row0 + wq) * ld + sm.u_col0 + lane] = sm.Us[wq][lane];
+    if (wq < u.r && lane < u.nc) A[(u.row0 + wq) * ld + u.col0 + lane] = sm.Us[slot][wq][lane];
 }
 
+// One CTA's share of the in-strip update behind a factored base panel (pivot rows pr0..pr0+r, panel
+// columns jp.., T at Tb, pivot columns in rec):
+//   U = T . A[pr0 : pr0+r, cc0 : cc0+nc]                                   (kept in Us[slot])
+//   A[m, cc0 : cc0+nc] -= sum_k A[m, pivot column k] * U[k, :]   for this worker's rows m >= pr0 + r
+// Row worker rw of nrw.  Tiles of SRB rows: the L tile goes to shared memory k-major, the C tile stays
+// in registers (thread = 8 consecutive rows x 1 column: L by broadcast LDS.128, U by one LDS per k).
+__device__ __noinline__ void strip_update(StripSmem& sm, int slot, uint32_t* A, int64_t ld, int64_t rows,
+                             const uint32_t* Tb, const PanelRec* rec, int64_t jp, int64_t pr0, int r, int64_t cc0, int nc,
+                             int rw, int nrw) {
+    const ModP& f = c_f;
+    const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
+    const int64_t mb0 = pr0 + r;
+    const int64_t mrem = rows - mb0;
+    int64_t rpw = (mrem + nrw - 1) / nrw;
+    rpw = (rpw + 7) / 8 * 8;
+    const int64_t my0 = mb0 + (int64_t)rw * rpw, my1 = min(rows, my0 + rpw);
+    // pivot index of panel column `lane` (pc[] is ascending), or -1
+    const unsigned pcm = __reduce_or_sync(0xffffffffu, lane < r ? 1u << rec->pc[lane] : 0u);
+    const int kcol = ((pcm >> lane) & 1u) ? __popc(pcm & ((1u << lane) - 1u)) : -1;
+    uint32_t cv[SRB / 32];
+    auto load_tile = [&](int64_t m0) {
+        uint32_t lreg[SRB / 32];
+#pragma unroll
+        for (int t = 0; t < SRB / 32; ++t) {
+            const int64_t m = m0 + wq + 32 * t;
+            lreg[t] = (kcol >= 0 && m < my1) ? A[m * ld + jp + lane] : 0u;
+        }
+#pragma unroll
+        for (int t = 0; t < SRB / 32; ++t) {
+            const int64_t m = m0 + wq * (SRB / 32) + t;
+            cv[t] = (lane < nc && m < my1) ? A[m * ld + cc0 + lane] : 0u;
+        }
+        if (kcol >= 0) {
+#pragma unroll
+            for (int t = 0; t < SRB / 32; ++t) sm.Lk[kcol][wq + 32 * t] = lreg[t];
+        }
+    };
+    const uint32_t tval = Tb[wq * PW + lane];
+    const uint32_t aval = (wq < r && lane < nc) ? A[(pr0 + wq) * ld + cc0 + lane] : 0u;
+    if (my0 < my1) load_tile(my0);
+    sm.Ts[wq][lane] = tval;
+    sm.Ar[wq][lane] = aval;
+    __syncthreads();
+    {
+        uint64_t acc = 0;
+#pragma unroll 8
+        for (int k = 0; k < PW; k += 2) {
+            acc += (uint64_t)sm.Ts[wq][k] * sm.Ar[k][lane];
+            acc += (uint64_t)sm.Ts[wq][k + 1] * sm.Ar[k + 1][lane];
+            acc = fold64(acc, f);
+        }
+        sm.Us[slot][wq][lane] = wq < r ? reduce64(acc, f) : 0u;
+    }
+    if (rw == 0 && tid == 0) { UPending& u = sm.pend[slot]; u.row0 = pr0; u.col0 = cc0; u.r = r; u.nc = nc; }
+    for (int64_t m0 = my0; m0 < my1; m0 += SRB) {
+        if (m0 != my0) {
+            __syncthreads();             // previous tile's readers of Lk are done
+            load_tile(m0);
+        }
+        __syncthreads();
+        if (m0 + wq * 8 < my1) {
+            uint64_t acc[SRB / 32];
+#pragma unroll
+            for (int t = 0; t < SRB / 32; ++t) acc[t] = 0;
+#pragma unroll 1
+            for (int k = 0; k + 1 < r; k += 2) {
+#pragma unroll
+                for (int kk = 0; kk < 2; ++kk) {
+                    const uint4 la = *reinterpret_cast<const uint4*>(&sm.Lk[k + kk][wq * 8]);
+                    const uint4 lb = *reinterpret_cast<const uint4*>(&sm.Lk[k + kk][wq * 8 + 4]);
+                    const uint32_t u = sm.Us[slot][k + kk][lane];
+                    const uint32_t l[8] = {la.x, la.y, la.z, la.w, lb.x, lb.y, lb.z, lb.w};
+#pragma unroll
+                    for (int t = 0; t < 8; ++t) acc[t] += (uint64_t)l[t] * u;
+                }
+#pragma unroll
+                for (int t = 0; t < 8; ++t) acc[t] = fold64(acc[t], f);
+            }
+            if (r & 1) {
+                const uint32_t u0 = sm.Us[slot][r - 1][lane];
+#pragma unroll
+                for (int t = 0; t < 8; ++t) acc[t] = fold64(acc[t] + (uint64_t)sm.Lk[r - 1][wq * 8 + t] * u0, f);
+            }
+#pragma unroll
+            for (int t = 0; t < 8; ++t) {
+                const int64_t m = m0 + wq * 8 + t;
+                if (lane < nc && m < my1) A[m * ld + cc0 + lane] = submod(cv[t], reduce64(acc[t], f), f);
+            }
+        }
+    }
+    __syncthreads();                     // Ts / Ar / Lk may be reused by the caller's next phase
+}
+
+// The strip kernel, with one panel of look-ahead: while CTA 0 factors panel i (phase A), the other
+// CTAs finish panel i-1's update on the columns right of panel i; only the update of panel i's OWN
+// columns (phase B of the previous iteration) sits on the panel-to-panel dependency chain.
 __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a) {
     extern __shared__ __align__(16) unsigned char strip_smem_raw[];
     StripSmem& sm = *reinterpret_cast<StripSmem*>(strip_smem_raw);
@@ -320,84 +456,75 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
     const int G = gridDim.x, cta = blockIdx.x;
     uint32_t* A = a.A;
     const int64_t ld = a.ld;
-    const ModP f = a.f;
     const int nbp = (a.ws + PW - 1) / PW;
     const int64_t b0 = a.j0 / PW;
+    const int64_t cu1 = a.j0 + a.ws;               // end of the strip
     int64_t cur = a.i0;
+    // panel i-1, if it still owes the update of the columns right of panel i
+    bool owe = false;
+    int64_t pb = 0, pjp = 0, ppr0 = 0, pcu0 = 0;
+    int pr = 0;
 
-    if (tid == 0) sm.u_row0 = -1;
+    if (tid == 0) { sm.pend[0].row0 = -1; sm.pend[1].row0 = -1; }
     __syncthreads();
     for (int i = 0; i < nbp; ++i) {
         const int64_t b = b0 + i;
         const int64_t jp = a.j0 + (int64_t)i * PW;
-        const int w = (int)min((int64_t)PW, a.j0 + a.ws - jp);
-        if (cur >= a.rows) {                       // no rows left: every remaining column is free (uniform over the grid)
-            if (cta == 0 && tid == 0)
-                for (int t = i; t < nbp; ++t) {
-                    a.rec[b0 + t].r = 0; a.rec[b0 + t].nswaps = 0; a.rec[b0 + t].w = 0;
-                    a.pstart[b0 + t + 1] = (int32_t)cur;
-                }
-            break;
-        }
-        // pending U12 slice of the previous panel: its readers all passed the last grid barrier
-        strip_flush_u(sm, A, ld);
+        const int w = (int)min((int64_t)PW, cu1 - jp);
+        // ---- phase A
+#ifdef LINAC_TRACE
+        if (threadIdx.x == 0 && blockIdx.x < 2) g_trace_on = (i == 1);
+#endif
+        STRIP_STAMP(0);
+        strip_flush_u(sm, 0, A, ld);               // its readers all passed the last grid barrier
         __syncthreads();
-        if (tid == 0) sm.u_row0 = -1;
-        // geometry of P2 (independent of what P1 finds, except through r)
-        const int64_t cu0 = jp + w, cu1 = a.j0 + a.ws;
-        const int ncu = (int)(cu1 - cu0);
-        const int ncb = max(1, (ncu + PW - 1) / PW);
-        const int nrw = max(1, G / ncb);                   // row workers per column block
-        const int cb = cta % ncb, rw = cta / ncb;
-        const bool worker = ncu > 0 && rw < nrw;
-        const int64_t cc0 = cu0 + (int64_t)cb * PW;
-        const int nc = (int)min((int64_t)PW, cu1 - cc0);
-        int64_t my0 = 0, my1 = 0;
-        auto my_rows = [&](int64_t mb0_) {                 // rows below the pivots, split evenly over the row workers
-            const int64_t mrem = a.rows - mb0_;
-            int64_t rpw = (mrem + nrw - 1) / nrw;
-            rpw = (rpw + 31) / 32 * 32;
-            my0 = mb0_ + (int64_t)rw * rpw;
-            my1 = min(a.rows, my0 + rpw);
-        };
-        uint32_t cv[SRB / 32];
-        int kcol = lane;
-        auto load_tile = [&](int64_t m0) {                 // L tile -> shared memory (k-major), C tile -> registers
-            uint32_t lreg[SRB / 32];
-#pragma unroll
-            for (int t = 0; t < SRB / 32; ++t) {
-                const int64_t m = m0 + wq + 32 * t;
-                lreg[t] = (kcol >= 0 && m < my1) ? A[m * ld + jp + lane] : 0u;
-            }
-#pragma unroll
-            for (int t = 0; t < SRB / 32; ++t) {
-                const int64_t m = m0 + wq * (SRB / 32) + t;
-                cv[t] = (lane < nc && m < my1) ? A[m * ld + cc0 + lane] : 0u;
-            }
-            if (kcol >= 0) {
-#pragma unroll
-                for (int t = 0; t < SRB / 32; ++t) sm.Lk[kcol][wq + 32 * t] = lreg[t];
-            }
-        };
-        // Prefetch of the first tile while CTA 0 factors the panel, assuming the common outcome (32
-        // pivots from the first 32 rows, no exchanges); checked after the barrier.
-        bool pre = false;
-        if (worker && cta != 0 && w == PW && cur + PW < a.rows) {
-            my_rows(cur + PW);
-            load_tile(my0);
-            pre = true;
-        }
-        // ---- P1
+        if (tid == 0) sm.pend[0].row0 = -1;
         if (cta == 0) {
-            panel_factor(sm, A, ld, a.rows, cur, jp, w, f, a.rec + b, a.T + b * PW * PW, a.E + b * PW * PW, a.pivcols);
-            if (tid == 0) a.pstart[b + 1] = (int32_t)(cur + sm.r_out);
+            if (cur < a.rows) {
+                panel_factor(sm, A, ld, a.rows, cur, jp, w, a.rec + b, a.T + b * PW * PW, a.E + b * PW * PW, a.pivcols);
+                if (tid == 0) a.pstart[b + 1] = (int32_t)(cur + sm.r_out);
+            } else if (tid == 0) {                 // no rows left: the panel's columns are free
+                a.rec[b].r = 0; a.rec[b].nswaps = 0; a.rec[b].w = w;
+                a.pstart[b + 1] = (int32_t)cur;
+            }
         }
+        if (owe && (cta > 0 || G == 1)) {
+            const int ncu = (int)(cu1 - pcu0);
+            const int nrest = (ncu + PW - 1) / PW - 1;             // column blocks 1.. (block 0 = panel i, done)
+            const int workers = G == 1 ? 1 : G - 1, job = G == 1 ? 0 : cta - 1;
+            if (nrest > 0) {
+                if (workers >= nrest) {
+                    const int nrw = workers / nrest, cb = 1 + job % nrest, rw = job / nrest;
+                    const int64_t cc0 = pcu0 + (int64_t)cb * PW;
+                    if (rw < nrw)
+                        strip_update(sm, 1, A, ld, a.rows, a.T + pb * PW * PW, a.rec + pb, pjp, ppr0, pr, cc0,
+                                     (int)min((int64_t)PW, cu1 - cc0), rw, nrw);
+                } else {                                            // tiny grid: blocks in turn (flush between them)
+                    for (int cb = 1 + job; cb <= nrest; cb += workers) {
+                        const int64_t cc0 = pcu0 + (int64_t)cb * PW;
+                        strip_update(sm, 1, A, ld, a.rows, a.T + pb * PW * PW, a.rec + pb, pjp, ppr0, pr, cc0,
+                                     (int)min((int64_t)PW, cu1 - cc0), 0, 1);
+                        // sole reader and writer of this block: the slice can go back at once
+                        strip_flush_u(sm, 1, A, ld);
+                        __syncthreads();
+                        if (tid == 0) sm.pend[1].row0 = -1;
+                        __syncthreads();
+                    }
+                }
+            }
+        }
+        owe = false;
+        STRIP_STAMP(6);
         grid.sync();
+        STRIP_STAMP(7);
+        strip_flush_u(sm, 1, A, ld);
+        __syncthreads();
+        if (tid == 0) sm.pend[1].row0 = -1;
         const PanelRec* rec = a.rec + b;
         const int r = rec->r, nsw = rec->nswaps;
         if (r == 0) continue;
-        // ---- P1b: row exchanges on complete rows, one thread per column (so the sequence of
-        // exchanges needs no inter-thread ordering)
+        // ---- row exchanges on complete rows, one thread per column (so the sequence of exchanges
+        // needs no inter-thread ordering)
         if (nsw > 0) {
             for (int64_t c = (int64_t)cta * SNT + tid; c < a.cols; c += (int64_t)G * SNT) {
                 for (int t = 0; t < r; ++t) {
@@ -411,78 +538,25 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
             }
             grid.sync();
         }
-        const int64_t mb0 = cur + r;                 // first row below the pivot rows
-        // reduced pivot rows' entries inside a rank-deficient panel (nobody reads these during P2)
+        // reduced pivot rows' entries inside a rank-deficient panel (nobody reads these during the updates)
         if (r < w && cta == G - 1)
             if (wq < r && lane < w) A[(cur + wq) * ld + jp + lane] = a.E[b * PW * PW + wq * PW + lane];
-        if (ncu > 0) {
-            // ---- P2
-            if (worker) {
-                const uint32_t tval = a.T[b * PW * PW + wq * PW + lane];
-                const uint32_t aval = (wq < r && lane < nc) ? A[(cur + wq) * ld + cc0 + lane] : 0u;
-                if (!(pre && r == PW && nsw == 0)) {
-                    // pivot index of panel column `lane` (pc[] is ascending), or -1
-                    const unsigned pcm = __reduce_or_sync(0xffffffffu, lane < r ? 1u << rec->pc[lane] : 0u);
-                    kcol = ((pcm >> lane) & 1u) ? __popc(pcm & ((1u << lane) - 1u)) : -1;
-                    my_rows(mb0);
-                    __syncthreads();                 // a rejected prefetch may still be landing in Lk
-                    load_tile(my0);
-                }
-                sm.Ts[wq][lane] = tval;
-                sm.Ar[wq][lane] = aval;
-                __syncthreads();
-                {
-                    uint64_t acc = 0;
-#pragma unroll 8
-                    for (int k = 0; k < PW; k += 2) {
-                        acc += (uint64_t)sm.Ts[wq][k] * sm.Ar[k][lane];
-                        acc += (uint64_t)sm.Ts[wq][k + 1] * sm.Ar[k + 1][lane];
-                        acc = fold64(acc, f);
-                    }
-                    sm.Us[wq][lane] = wq < r ? reduce64(acc, f) : 0u;
-                }
-                if (rw == 0 && tid == 0) { sm.u_row0 = cur; sm.u_col0 = cc0; sm.u_r = r; sm.u_nc = nc; }
-                for (int64_t m0 = my0; m0 < my1; m0 += SRB) {
-                    if (m0 != my0) {
-                        __syncthreads();             // previous tile's readers of Lk are done
-                        load_tile(m0);
-                    }
-                    __syncthreads();
-                    // thread = 8 consecutive rows x 1 column: L by broadcast LDS.128, U by one LDS per k
-                    uint64_t acc[SRB / 32];
-#pragma unroll
-                    for (int t = 0; t < SRB / 32; ++t) acc[t] = 0;
-#pragma unroll 1
-                    for (int k = 0; k + 1 < r; k += 2) {
-#pragma unroll
-                        for (int kk = 0; kk < 2; ++kk) {
-                            const uint4 la = *reinterpret_cast<const uint4*>(&sm.Lk[k + kk][wq * 8]);
-                            const uint4 lb = *reinterpret_cast<const uint4*>(&sm.Lk[k + kk][wq * 8 + 4]);
-                            const uint32_t u = sm.Us[k + kk][lane];
-                            const uint32_t l[8] = {la.x, la.y, la.z, la.w, lb.x, lb.y, lb.z, lb.w};
-#pragma unroll
-                            for (int t = 0; t < 8; ++t) acc[t] += (uint64_t)l[t] * u;
-                        }
-#pragma unroll
-                        for (int t = 0; t < 8; ++t) acc[t] = fold64(acc[t], f);
-                    }
-                    if (r & 1) {
-                        const uint32_t u0 = sm.Us[r - 1][lane];
-#pragma unroll
-                        for (int t = 0; t < 8; ++t) acc[t] = fold64(acc[t] + (uint64_t)sm.Lk[r - 1][wq * 8 + t] * u0, f);
-                    }
-#pragma unroll
-                    for (int t = 0; t < 8; ++t) {
-                        const int64_t m = m0 + wq * 8 + t;
-                        if (lane < nc && m < my1) A[m * ld + cc0 + lane] = submod(cv[t], reduce64(acc[t], f), f);
-                    }
-                }
-            }
-            if (i + 1 < nbp) grid.sync();
+        const int64_t cu0 = jp + w;
+        if (cu0 < cu1) {
+            // ---- phase B: the next panel's columns, all CTAs as row workers
+            strip_update(sm, 0, A, ld, a.rows, a.T + b * PW * PW, rec, jp, cur, r, cu0, (int)min((int64_t)PW, cu1 - cu0),
+                         cta, G);
+            owe = cu1 - cu0 > PW;
+            pb = b; pjp = jp; ppr0 = cur; pcu0 = cu0; pr = r;
+            STRIP_STAMP(8);
+            grid.sync();
+            STRIP_STAMP(9);
         }
-        cur = mb0;
+        cur += r;
     }
-    strip_flush_u(sm, A, ld);
+    // Panel nbp-1 is the strip's last: it has no columns to its right, so nothing is owed here.
+    strip_flush_u(sm, 0, A, ld);
+    strip_flush_u(sm, 1, A, ld);
 }
 
 // ------------------------------------------------------------------------------------------------

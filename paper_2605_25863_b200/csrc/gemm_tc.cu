@@ -215,6 +215,7 @@ struct TileIter {
     }
 };
 
+template <bool MONT>
 __global__ void __launch_bounds__(P_THREADS, 1)
 gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                      const __grid_constant__ CUtensorMap tmC, int nks /* k-stages: kp / 128 */, PanelSched sc, ModP f) {
@@ -328,7 +329,6 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
         const int e = warp - 2, q = warp & 3, h = e >> 2;
         const int row = q * 32 + lane;
         const bool elected = threadIdx.x == 64;
-        const uint64_t w4 = f.w[4], w5 = f.w[5], w6 = f.w[6];
         uint32_t t_cnt = 0;
         TileIter it;
         it.init(sc);
@@ -366,9 +366,17 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
 #pragma unroll
                 for (int x = 0; x < 4; ++x) {
                     const int el = 4 * j + x;
-                    uint64_t v = (uint64_t)S[0][el] + ((uint64_t)S[1][el] << 8) + ((uint64_t)S[2][el] << 16) + ((uint64_t)S[3][el] << 24);
-                    v += (uint64_t)S[4][el] * w4 + (uint64_t)S[5][el] * w5 + (uint64_t)S[6][el] * w6;
-                    cv[x] = submod(cv[x], reduce64(v, f), f);
+                    if (MONT) {
+                        // sum_w S_w (2^(8w) 2^32 mod p) < 7 * 2^26 * p < 2^32 p, so one Montgomery reduction finishes
+                        uint64_t v = (uint64_t)S[0][el] * f.wm[0];
+#pragma unroll
+                        for (int w = 1; w < 7; ++w) v += (uint64_t)S[w][el] * f.wm[w];
+                        cv[x] = submod(cv[x], redc(v, f), f);
+                    } else {
+                        uint64_t v = (uint64_t)S[0][el] + ((uint64_t)S[1][el] << 8) + ((uint64_t)S[2][el] << 16) + ((uint64_t)S[3][el] << 24);
+                        v += (uint64_t)S[4][el] * f.w[4] + (uint64_t)S[5][el] * f.w[5] + (uint64_t)S[6][el] * f.w[6];
+                        cv[x] = submod(cv[x], reduce64(v, f), f);
+                    }
                 }
                 *pc = make_uint4(cv[0], cv[1], cv[2], cv[3]);
             }
@@ -538,7 +546,8 @@ int gemm_modp_tc(const GemmArgs& g, const ModP& f, cudaStream_t s, Arena* scratc
     if (panel_ok) {
         static bool pattr = false;
         if (!pattr) {
-            if (cudaFuncSetAttribute(gemm_tc_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM) != cudaSuccess) {
+            if (cudaFuncSetAttribute(gemm_tc_panel_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM) != cudaSuccess ||
+                cudaFuncSetAttribute(gemm_tc_panel_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM) != cudaSuccess) {
                 cudaGetLastError();
                 return -1;
             }
@@ -563,7 +572,10 @@ int gemm_modp_tc(const GemmArgs& g, const ModP& f, cudaStream_t s, Arena* scratc
             return -1;
         const int grid = sm_count();
         const PanelSched sc = make_sched(g.M, g.N, grid);
-        gemm_tc_panel_kernel<<<(unsigned)std::min(grid, sc.nitems), P_THREADS, P_SMEM, s>>>(tmA, tmB, tmC, (int)(kp / KB), sc, f);
+        if (f.ninv)
+            gemm_tc_panel_kernel<true><<<(unsigned)std::min(grid, sc.nitems), P_THREADS, P_SMEM, s>>>(tmA, tmB, tmC, (int)(kp / KB), sc, f);
+        else
+            gemm_tc_panel_kernel<false><<<(unsigned)std::min(grid, sc.nitems), P_THREADS, P_SMEM, s>>>(tmA, tmB, tmC, (int)(kp / KB), sc, f);
         LINAC_CUDA(cudaGetLastError());
         stats().kernel_launches += 3;
         stats().tc_launches++;

@@ -91,6 +91,13 @@ ModP make_modp(uint32_t p) {
     f.c32 = (uint32_t)((1ull << 32) % p);
     f.m64 = (uint64_t)((((unsigned __int128)1) << 64) / p);
     for (int k = 0; k < 7; ++k) f.w[k] = (uint32_t)powmod_u64(2, 8 * k, p);
+    for (int k = 0; k < 7; ++k) f.wm[k] = (uint32_t)powmod_u64(2, 8 * k + 32, p);
+    f.ninv = 0;
+    if (p & 1) {                                   // Newton iteration for p^-1 mod 2^32, then negate
+        uint32_t inv = p;                          // correct to 3 bits
+        for (int i = 0; i < 5; ++i) inv *= 2u - p * inv;
+        f.ninv = 0u - inv;
+    }
     return f;
 }
 

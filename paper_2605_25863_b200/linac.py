@@ -38,7 +38,8 @@ class LinacError(RuntimeError):
 class Stats(C.Structure):
     _fields_ = [("kernel_launches", C.c_int64), ("host_syncs", C.c_int64), ("panels", C.c_int64),
                 ("row_swaps", C.c_int64), ("update_macs", C.c_int64), ("residual_nonzero", C.c_int64), ("tc_launches", C.c_int64),
-                ("ms_update", C.c_double), ("ms_total", C.c_double)]
+                ("ms_update", C.c_double), ("ms_total", C.c_double),
+                ("ms_strip", C.c_double), ("ms_trsm", C.c_double)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
