@@ -181,7 +181,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 //   warp 0      TMA producer: A k-stages (ring of 2 x 64 KB) and B k-stages (ring of 4 x 16 KB)
 //   warp 1      MMA issuer: 128x128x32 kind::i8 MMAs (four B limb planes stacked along N), two TMEM
 //               accumulator buffers of 7 x 32 columns
-//   warps 2-9   epilogue: tcgen05.ld, limb recombination sum_w S_w (2^(8w) mod p), one Barrett reduction,
+//   warp 2      C mover (TMA loads / L2 prefetch / TMA stores of the C tiles)
+//   warps 3-18  epilogue: tcgen05.ld, limb recombination sum_w S_w (2^(8w) mod p), one Barrett reduction,
 //               C tile staged through shared memory by TMA in both directions (128-byte swizzle), so no
 //               thread-per-row global access ever reaches the LSU.
 constexpr int PN = 32;                       // output tile columns
@@ -190,7 +191,9 @@ constexpr int P_B_STAGE = 4 * PN * KB;       // 16384
 constexpr int P_C_TILE = TM * PN * 4;        // 16384
 constexpr int P_NAS = 2, P_NBS = 3, P_NCS = 3;
 constexpr int P_SMEM = P_NAS * P_A_STAGE + P_NBS * P_B_STAGE + P_NCS * P_C_TILE + 1024 + 256;
-constexpr int P_THREADS = 320;
+constexpr int P_EPI_WARPS = 16;              // epilogue warps: 4 TMEM lane quarters x 4 groups of 8 columns
+constexpr int P_THREADS = 96 + 32 * P_EPI_WARPS;
+constexpr int P_PF = 6;                      // L2 prefetch distance for C tiles
 constexpr int P_ACC_COLS = 256;              // TMEM columns reserved per accumulator buffer (224 used)
 
 struct PanelSched {
@@ -215,6 +218,12 @@ struct TileIter {
     }
 };
 
+__device__ __forceinline__ TileIter sc_init(const PanelSched& sc) {
+    TileIter it;
+    it.init(sc);
+    return it;
+}
+
 template <bool MONT>
 __global__ void __launch_bounds__(P_THREADS, 1)
 gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
@@ -232,7 +241,8 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
     uint64_t* acc_full = bars + 12;          // [2]
     uint64_t* acc_empty = bars + 14;         // [2]
     uint64_t* c_full = bars + 16;            // [3]
-    uint32_t* tmem_holder = (uint32_t*)(bars + 20);
+    uint64_t* c_done = bars + 19;            // [3]
+    uint32_t* tmem_holder = (uint32_t*)(bars + 22);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (warp == 0 && lane == 0) {
@@ -240,8 +250,8 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
         prefetch_tmap(&tmB);
         prefetch_tmap(&tmC);
         for (int i = 0; i < 2; ++i) { mbar_init(&a_full[i], 1); mbar_init(&a_empty[i], 1); mbar_init(&acc_full[i], 1);
-                                      mbar_init(&acc_empty[i], 8); }
-        for (int i = 0; i < P_NCS; ++i) mbar_init(&c_full[i], 1);
+                                      mbar_init(&acc_empty[i], P_EPI_WARPS); }
+        for (int i = 0; i < P_NCS; ++i) { mbar_init(&c_full[i], 1); mbar_init(&c_done[i], P_EPI_WARPS); }
         for (int i = 0; i < P_NBS; ++i) { mbar_init(&b_full[i], 1); mbar_init(&b_empty[i], 1); }
         fence_barrier_init();
     }
@@ -276,93 +286,119 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             }
         }
     } else if (warp == 1) {
-        if (lane == 0) {
-            constexpr uint32_t id128 = make_idesc_i8(4 * PN), id96 = make_idesc_i8(3 * PN), id32 = make_idesc_i8(PN);
-            uint32_t a_cnt = 0, b_cnt = 0, t_cnt = 0;
-            TileIter it;
-            it.init(sc);
-            while (it.valid) {
-                const int item = it.item;
-                bool first_tile = true;
-                while (it.valid && it.item == item) {
-                    const uint32_t buf = t_cnt & 1;
-                    mbar_wait(&acc_empty[buf], ((t_cnt >> 1) & 1) ^ 1);
+        // The whole warp runs this loop with uniform control flow (so descriptors and counters live in uniform
+        // registers and cost one add per MMA); one elected lane issues the tcgen05 instructions.
+        constexpr uint32_t id128 = make_idesc_i8(4 * PN), id96 = make_idesc_i8(3 * PN), id32 = make_idesc_i8(PN);
+        constexpr uint64_t LIMB = (uint64_t)((TM * KB) >> 4);          // descriptor step between A limb planes
+        constexpr uint64_t KSTEP = 32 >> 4;                            // descriptor step of one 32-byte k slice
+        uint64_t adesc[P_NAS], bdesc[P_NBS];
+#pragma unroll
+        for (int i = 0; i < P_NAS; ++i) adesc[i] = make_desc_sw128(smem_u32(sA + i * P_A_STAGE));
+#pragma unroll
+        for (int i = 0; i < P_NBS; ++i) bdesc[i] = make_desc_sw128(smem_u32(sB + i * P_B_STAGE));
+        uint32_t a_cnt = 0, b_cnt = 0, t_cnt = 0;
+        TileIter it = sc_init(sc);
+        while (it.valid) {
+            const int item = it.item;
+            bool first_tile = true;
+            while (it.valid && it.item == item) {
+                const uint32_t buf = t_cnt & 1;
+                mbar_wait(&acc_empty[buf], ((t_cnt >> 1) & 1) ^ 1);
+                tc_fence_after();
+                const uint32_t d0 = tmem_base + buf * P_ACC_COLS;
+                const bool last = it.last_of_item();
+                for (int ks = 0; ks < nks; ++ks, ++b_cnt) {
+                    const uint32_t ac = a_cnt + ks;
+                    const int sa = ac % P_NAS;
+                    if (first_tile) mbar_wait(&a_full[sa], (ac / P_NAS) & 1);
+                    const int sb = b_cnt % P_NBS;
+                    mbar_wait(&b_full[sb], (b_cnt / P_NBS) & 1);
                     tc_fence_after();
-                    const uint32_t d0 = tmem_base + buf * P_ACC_COLS;
-                    const bool last = it.last_of_item();
-                    for (int ks = 0; ks < nks; ++ks, ++b_cnt) {
-                        const uint32_t ac = a_cnt + ks;
-                        const int sa = ac % P_NAS;
-                        if (first_tile) mbar_wait(&a_full[sa], (ac / P_NAS) & 1);
-                        const int sb = b_cnt % P_NBS;
-                        mbar_wait(&b_full[sb], (b_cnt / P_NBS) & 1);
-                        tc_fence_after();
-                        const uint32_t a0 = smem_u32(sA + sa * P_A_STAGE), b0 = smem_u32(sB + sb * P_B_STAGE);
-#pragma unroll
-                        for (int kk = 0; kk < KB / 32; ++kk) {
-                            const uint32_t ko = kk * 32;
-                            if (ks == 0 && kk == 0) {
-                                // first k step of the tile: slots 0-3 and 4-6 are overwritten, the rest accumulate
-                                umma_i8(d0, make_desc_sw128(a0), make_desc_sw128(b0), id128, 0u);
-                                umma_i8(d0 + 4 * PN, make_desc_sw128(a0 + 3 * (TM * KB)), make_desc_sw128(b0 + PN * KB), id96, 0u);
-                                umma_i8(d0 + 1 * PN, make_desc_sw128(a0 + 1 * (TM * KB)), make_desc_sw128(b0), id128, 1u);
-                                umma_i8(d0 + 2 * PN, make_desc_sw128(a0 + 2 * (TM * KB)), make_desc_sw128(b0), id128, 1u);
-                                umma_i8(d0 + 3 * PN, make_desc_sw128(a0 + 3 * (TM * KB)), make_desc_sw128(b0), id32, 1u);
-                            } else {
-#pragma unroll
-                                for (int i = 0; i < 4; ++i)
-                                    umma_i8(d0 + i * PN, make_desc_sw128(a0 + i * (TM * KB) + ko), make_desc_sw128(b0 + ko), id128, 1u);
-                            }
+                    const uint64_t da = sa == 0 ? adesc[0] : adesc[1];
+                    const uint64_t db = sb == 0 ? bdesc[0] : (sb == 1 ? bdesc[1] : bdesc[2]);
+                    if (elect_one()) {
+                        if (ks == 0) {
+                            // first k step of the tile: slots 0-3 and 4-6 are overwritten, the rest accumulate
+                            umma_i8(d0, da, db, id128, 0u);
+                            umma_i8(d0 + 4 * PN, da + 3 * LIMB, db + ((PN * KB) >> 4), id96, 0u);
+                            umma_i8(d0 + 1 * PN, da + 1 * LIMB, db, id128, 1u);
+                            umma_i8(d0 + 2 * PN, da + 2 * LIMB, db, id128, 1u);
+                            umma_i8(d0 + 3 * PN, da + 3 * LIMB, db, id32, 1u);
+                        } else {
+                            umma_i8_x4(d0, da, db, id128, PN, LIMB);
                         }
+#pragma unroll
+                        for (int kk = 1; kk < KB / 32; ++kk) umma_i8_x4(d0, da + kk * KSTEP, db + kk * KSTEP, id128, PN, LIMB);
                         umma_commit(&b_empty[sb]);
                         if (last) umma_commit(&a_empty[sa]);
+                        if (ks == nks - 1) umma_commit(&acc_full[buf]);
                     }
-                    umma_commit(&acc_full[buf]);
-                    ++t_cnt;
-                    first_tile = false;
-                    it.next(sc);
+                    __syncwarp();
                 }
-                a_cnt += nks;
+                ++t_cnt;
+                first_tile = false;
+                it.next(sc);
             }
+            a_cnt += nks;
+        }
+    } else if (warp == 2) {
+        // C mover: TMA loads of the C tiles two tiles ahead (three buffers), L2 prefetch P_PF tiles ahead
+        // (the trailing matrix is far larger than L2), TMA stores once the epilogue warps are done with a tile.
+        if (lane == 0) {
+            TileIter ld = sc_init(sc), pf = ld, st = ld;
+            uint32_t l_cnt = 0, t_cnt = 0;
+            for (int i = 0; i < P_PF && pf.valid; ++i) pf.next(sc);
+            for (int i = 0; i < 2 && ld.valid; ++i, ++l_cnt) {
+                mbar_expect_tx(&c_full[l_cnt % P_NCS], P_C_TILE);
+                tma_load_2d(sC + (l_cnt % P_NCS) * P_C_TILE, &tmC, &c_full[l_cnt % P_NCS], ld.nt * PN, ld.mt * TM);
+                ld.next(sc);
+            }
+            while (st.valid) {
+                const uint32_t cb = t_cnt % P_NCS;
+                if (pf.valid) { tma_prefetch_l2_2d(&tmC, pf.nt * PN, pf.mt * TM); pf.next(sc); }
+                mbar_wait(&c_done[cb], (t_cnt / P_NCS) & 1);
+                tma_store_2d(&tmC, sC + cb * P_C_TILE, st.nt * PN, st.mt * TM);
+                tma_store_commit();
+                st.next(sc);
+                ++t_cnt;
+                if (ld.valid) {
+                    // buffer of tile t+2 == buffer of tile t-1, whose store was committed one iteration ago
+                    tma_store_wait_read1();
+                    const uint32_t lb = l_cnt % P_NCS;
+                    mbar_expect_tx(&c_full[lb], P_C_TILE);
+                    tma_load_2d(sC + lb * P_C_TILE, &tmC, &c_full[lb], ld.nt * PN, ld.mt * TM);
+                    ld.next(sc);
+                    ++l_cnt;
+                }
+            }
+            tma_store_wait_all();
         }
     } else {
-        const int e = warp - 2, q = warp & 3, h = e >> 2;
+        const int e = warp - 3, q = warp & 3, g = e >> 2;      // TMEM lane quarter, column group of 8
         const int row = q * 32 + lane;
-        const bool elected = threadIdx.x == 64;
         uint32_t t_cnt = 0;
-        TileIter it;
-        it.init(sc);
-        if (elected && it.valid) {
-            mbar_expect_tx(&c_full[0], P_C_TILE);
-            tma_load_2d(sC, &tmC, &c_full[0], it.nt * PN, it.mt * TM);
-        }
+        TileIter it = sc_init(sc);
         while (it.valid) {
             const uint32_t buf = t_cnt & 1, ph = (t_cnt >> 1) & 1;
-            const uint32_t cb = t_cnt % P_NCS, cph = (t_cnt / P_NCS) & 1, cbn = (t_cnt + 1) % P_NCS;
-            const int mt = it.mt, nt = it.nt;
+            const uint32_t cb = t_cnt % P_NCS, cph = (t_cnt / P_NCS) & 1;
             it.next(sc);
-            if (elected && it.valid) {
-                tma_store_wait_read1();          // the store that last read C buffer cbn (two tiles ago) is done with it
-                mbar_expect_tx(&c_full[cbn], P_C_TILE);
-                tma_load_2d(sC + cbn * P_C_TILE, &tmC, &c_full[cbn], it.nt * PN, it.mt * TM);
-            }
             mbar_wait(&acc_full[buf], ph);
             tc_fence_after();
-            uint32_t S[7][16];
-            const uint32_t t0 = tmem_base + ((uint32_t)(q * 32) << 16) + buf * P_ACC_COLS + h * 16;
+            uint32_t S[7][8];
+            const uint32_t t0 = tmem_base + ((uint32_t)(q * 32) << 16) + buf * P_ACC_COLS + g * 8;
 #pragma unroll
-            for (int w = 0; w < 7; ++w) tmem_ld16(t0 + w * PN, S[w]);
+            for (int w = 0; w < 7; ++w) tmem_ld8(t0 + w * PN, S[w]);
             tmem_ld_wait();
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(&acc_empty[buf]);
             mbar_wait(&c_full[cb], cph);
-            uint8_t* crow = sC + cb * P_C_TILE + row * 128;
+            const uint32_t crow = smem_u32(sC + cb * P_C_TILE + row * 128);
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                uint4* pc = reinterpret_cast<uint4*>(crow + (((4 * h + j) ^ (row & 7)) << 4));
-                uint4 c4 = *pc;
-                uint32_t cv[4] = {c4.x, c4.y, c4.z, c4.w};
+            for (int j = 0; j < 2; ++j) {
+                const uint32_t pc = crow + (((2 * g + j) ^ (row & 7)) << 4);
+                uint32_t cv[4];
+                asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(cv[0]), "=r"(cv[1]), "=r"(cv[2]), "=r"(cv[3]) : "r"(pc));
 #pragma unroll
                 for (int x = 0; x < 4; ++x) {
                     const int el = 4 * j + x;
@@ -378,17 +414,13 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                         cv[x] = submod(cv[x], reduce64(v, f), f);
                     }
                 }
-                *pc = make_uint4(cv[0], cv[1], cv[2], cv[3]);
+                asm volatile("st.shared.v4.u32 [%4], {%0, %1, %2, %3};" ::"r"(cv[0]), "r"(cv[1]), "r"(cv[2]), "r"(cv[3]), "r"(pc) : "memory");
             }
-            fence_proxy_async();
-            asm volatile("bar.sync 1, 256;" ::: "memory");
-            if (elected) {
-                tma_store_2d(&tmC, sC + cb * P_C_TILE, nt * PN, mt * TM);
-                tma_store_commit();
-            }
+            fence_proxy_async();                 // the tile in shared memory is read next by the TMA store
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&c_done[cb]);
             ++t_cnt;
         }
-        if (elected) tma_store_wait_all();
         tc_fence_before();
     }
     __syncthreads();

@@ -58,6 +58,32 @@ __device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t desc_a, uint64
         "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t"
         "}" ::"r"(tmem_d), "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate) : "memory");
 }
+// Four accumulating MMAs of one k slice: A limb plane i (descriptor a + i*limb_step) against the stacked B
+// planes into accumulator columns d + i*dstep.
+__device__ __forceinline__ void umma_i8_x4(uint32_t d, uint64_t a, uint64_t b, uint32_t idesc, uint32_t dstep, uint64_t limb_step) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        ".reg .b64 a1, a2, a3;\n\t"
+        ".reg .b32 d1, d2, d3;\n\t"
+        "setp.eq.b32 p, 0, 0;\n\t"
+        "add.u64 a1, %1, %5;\n\t"
+        "add.u64 a2, a1, %5;\n\t"
+        "add.u64 a3, a2, %5;\n\t"
+        "add.u32 d1, %0, %4;\n\t"
+        "add.u32 d2, d1, %4;\n\t"
+        "add.u32 d3, d2, %4;\n\t"
+        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t"
+        "tcgen05.mma.cta_group::1.kind::i8 [d1], a1, %2, %3, p;\n\t"
+        "tcgen05.mma.cta_group::1.kind::i8 [d2], a2, %2, %3, p;\n\t"
+        "tcgen05.mma.cta_group::1.kind::i8 [d3], a3, %2, %3, p;\n\t"
+        "}" ::"r"(d), "l"(a), "l"(b), "r"(idesc), "r"(dstep), "l"(limb_step) : "memory");
+}
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
 // mbarrier arrives when all previously issued tcgen05.mma of this thread have completed.
 __device__ __forceinline__ void umma_commit(uint64_t* bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
@@ -77,6 +103,9 @@ __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* t
 __device__ __forceinline__ void tma_store_2d(const CUtensorMap* tm, const void* smem_src, int c0, int c1) {
     asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
                  ::"l"(tm), "r"(smem_u32(smem_src)), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_l2_2d(const CUtensorMap* tm, int c0, int c1) {
+    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"(tm), "r"(c0), "r"(c1) : "memory");
 }
 __device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void tma_store_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
