@@ -83,7 +83,6 @@ struct Timed {
     }
 };
 
-size_t trsm_smem_bytes(int64_t K) { return (size_t)K * PW * 4 + (size_t)PW * (PW + 1) * 4; }
 
 // Leaf of both triangular solves: the pivots of ONE strip against columns [0, ncols) of X.
 template <bool LOWER>
@@ -249,6 +248,8 @@ int strip_grid(int* grid) {
         LINAC_CUDA(cudaGetDevice(&dev));
         LINAC_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
         LINAC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, strip_factor_kernel, SNT, sizeof(StripSmem)));
+        LINAC_CUDA(cudaFuncSetAttribute(trsm_strip_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)trsm_smem_bytes(SW_MAX)));
+        LINAC_CUDA(cudaFuncSetAttribute(trsm_strip_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)trsm_smem_bytes(SW_MAX)));
         if (per_sm < 1 || sms < 1) return LINAC_ERR_INTERNAL;
         cached = sms;                                 // one CTA per SM: more would only lengthen the grid barrier
     }

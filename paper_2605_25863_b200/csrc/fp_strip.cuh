@@ -569,6 +569,13 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
 //           X_t -= sum_k U[t][k] X_b[k]  for the strip's pivot rows t before b
 // with L[t][k] = U[t][k] = A[row t][pivcols[first pivot of b + k]] (fp_kernels.cuh storage convention).
 constexpr int TNT = 512;       // threads per CTA (16 warps)
+constexpr int TLS = PW + 4;    // row stride of the staged L block (16-byte aligned rows, conflict-free stores)
+constexpr int TLR = SW_MAX - PW;                       // most rows an L block can have
+constexpr int TNL = (TLR * PW + TNT - 1) / TNT;        // prefetch registers per thread for one L block
+
+__host__ __device__ inline size_t trsm_smem_bytes(int64_t K) {
+    return (size_t)K * PW * 4 + (size_t)PW * (PW + 1) * 4 + (size_t)TLR * TLS * 4;
+}
 
 template <bool LOWER>
 __global__ void __launch_bounds__(TNT) trsm_strip_kernel(const uint32_t* __restrict__ A, int64_t ld,
@@ -577,23 +584,60 @@ __global__ void __launch_bounds__(TNT) trsm_strip_kernel(const uint32_t* __restr
                                                          const uint32_t* __restrict__ T,
                                                          const int32_t* __restrict__ pivcols, ModP f) {
     extern __shared__ __align__(16) unsigned char trsm_smem_raw[];
-    uint32_t (*Xs)[PW] = reinterpret_cast<uint32_t (*)[PW]>(trsm_smem_raw);                 // [K][32]
     const int t0 = pstart[bs0], K = pstart[bs1] - t0;
-    uint32_t (*Ts)[PW + 1] = reinterpret_cast<uint32_t (*)[PW + 1]>(trsm_smem_raw + (size_t)K * PW * 4);   // [32][33]
+    uint32_t (*Xs)[PW] = reinterpret_cast<uint32_t (*)[PW]>(trsm_smem_raw);                                 // [K][32]
+    uint32_t (*Ts)[PW + 1] = reinterpret_cast<uint32_t (*)[PW + 1]>(trsm_smem_raw + (size_t)K * PW * 4);     // [32][33]
+    uint32_t (*Lp)[TLS] = reinterpret_cast<uint32_t (*)[TLS]>(trsm_smem_raw + (size_t)K * PW * 4 + PW * (PW + 1) * 4);
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
     constexpr int NW = TNT / 32;
     const int64_t c = (int64_t)blockIdx.x * PW + lane;
     const bool cok = c < ncols;
-    for (int t = wq; t < K; t += NW) Xs[t][lane] = cok ? X[(int64_t)t * ldx + c] : 0u;
-    __syncthreads();
     const int nbp = bs1 - bs0;
+
+    // The L (or U) block and T of a base panel are fetched into registers one panel ahead, so their global
+    // latency hides under the previous panel's arithmetic instead of sitting on the panel-to-panel chain.
+    uint32_t lpre[TNL], tpre[2];
+    int nxt = 0;                                       // next panel (in processing order) to prefetch
+    auto panel_of = [&](int ii) { return LOWER ? bs0 + ii : bs1 - 1 - ii; };
+    auto prefetch = [&]() {
+        while (nxt < nbp && pstart[panel_of(nxt) + 1] == pstart[panel_of(nxt)]) ++nxt;     // skip empty panels
+        if (nxt >= nbp) return;
+        const int b = panel_of(nxt);
+        const int s = pstart[b] - t0, e = pstart[b + 1] - t0, r = e - s;
+        const int lo = LOWER ? e : 0, nrow = LOWER ? K - e : s;
+        if (LOWER) {
+            tpre[0] = T[(int64_t)b * PW * PW + tid];
+            tpre[1] = T[(int64_t)b * PW * PW + TNT + tid];
+        }
+        const int32_t pc = lane < r ? pivcols[t0 + s + lane] : -1;
+#pragma unroll
+        for (int j = 0; j < TNL; ++j) {
+            const int row = wq + NW * j;
+            lpre[j] = (row < nrow && pc >= 0) ? A[(int64_t)(t0 + lo + row) * ld + pc] : 0u;
+        }
+    };
+    prefetch();
+    for (int t = wq; t < K; t += NW) Xs[t][lane] = cok ? X[(int64_t)t * ldx + c] : 0u;
+
     for (int ii = 0; ii < nbp; ++ii) {
-        const int b = LOWER ? bs0 + ii : bs1 - 1 - ii;
+        const int b = panel_of(ii);
         const int s = pstart[b] - t0, e = pstart[b + 1] - t0, r = e - s;
         if (r == 0) continue;
+        const int lo = LOWER ? e : 0, nrow = LOWER ? K - e : s;
+        // registers -> shared memory (the previous panel's readers passed the barrier that ended its update)
         if (LOWER) {
-            for (int x = tid; x < PW * PW; x += TNT) Ts[x / PW][x % PW] = T[(int64_t)b * PW * PW + x];
-            __syncthreads();
+            Ts[tid / PW][tid % PW] = tpre[0];
+            Ts[(TNT + tid) / PW][tid % PW] = tpre[1];
+        }
+#pragma unroll
+        for (int j = 0; j < TNL; ++j) {
+            const int row = wq + NW * j;
+            if (row < nrow) Lp[row][lane] = lpre[j];
+        }
+        __syncthreads();
+        nxt = ii + 1;
+        prefetch();
+        if (LOWER) {
             uint32_t y[PW / NW];
 #pragma unroll
             for (int u = 0; u < PW / NW; ++u) {
@@ -613,18 +657,20 @@ __global__ void __launch_bounds__(TNT) trsm_strip_kernel(const uint32_t* __restr
                 if (wq + NW * u < r) Xs[s + wq + NW * u][lane] = y[u];
             __syncthreads();
         }
-        const int lo = LOWER ? e : 0, hi = LOWER ? K : s;
-        const int32_t pc = lane < r ? pivcols[t0 + s + lane] : 0;
-        for (int t = lo + wq; t < hi; t += NW) {
-            const uint32_t lv = lane < r ? A[(int64_t)(t0 + t) * ld + pc] : 0u;
+        for (int row = wq; row < nrow; row += NW) {
             uint64_t acc = 0;
-            for (int k = 0; k + 1 < r; k += 2) {
-                acc += (uint64_t)__shfl_sync(0xffffffffu, lv, k) * Xs[s + k][lane];
-                acc += (uint64_t)__shfl_sync(0xffffffffu, lv, k + 1) * Xs[s + k + 1][lane];
+            int k = 0;
+            for (; k + 3 < r; k += 4) {
+                const uint4 l4 = *reinterpret_cast<const uint4*>(&Lp[row][k]);
+                acc += (uint64_t)l4.x * Xs[s + k][lane];
+                acc += (uint64_t)l4.y * Xs[s + k + 1][lane];
+                acc = fold64(acc, f);
+                acc += (uint64_t)l4.z * Xs[s + k + 2][lane];
+                acc += (uint64_t)l4.w * Xs[s + k + 3][lane];
                 acc = fold64(acc, f);
             }
-            if (r & 1) acc = fold64(acc + (uint64_t)__shfl_sync(0xffffffffu, lv, r - 1) * Xs[s + r - 1][lane], f);
-            Xs[t][lane] = submod(Xs[t][lane], reduce64(acc, f), f);
+            for (; k < r; ++k) acc = fold64(acc + (uint64_t)Lp[row][k] * Xs[s + k][lane], f);
+            Xs[lo + row][lane] = submod(Xs[lo + row][lane], reduce64(acc, f), f);
         }
         __syncthreads();
     }
