@@ -12,8 +12,9 @@ matrices in F_{2^31-1}", PAPER.md:308 -- not a public data set, so these stand i
     idx = r * cols + c  as a 64-bit counter
 
 so any element / row of any config can be re-created without the rest (needed to certify
-the N = 10^5 config without holding a second 40 GB copy).  `linac_inputs/device_gen.cu`
-implements the same counter-based generator on the device, bit-identically.
+the N = 10^5 config without holding a second 40 GB copy).  `linac_inputs/gen_torch.py`
+implements the same counter-based generator with torch integer ops (so it can run on the device),
+bit-identically.
 """
 from .gen import (  # noqa: F401
     splitmix64,

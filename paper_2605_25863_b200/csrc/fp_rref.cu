@@ -141,10 +141,9 @@ int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r) {
         cudaMemcpyFromSymbol(h, g_strip_trace, sizeof h);
         for (int ct = 0; ct < 2; ++ct) {
             printf("strip %ld cta %d panel 1 (ns since phase A start):", (long)s, ct);
-            for (int k = 1; k < 10; ++k) printf(" [%d]%lld", k, h[ct * 32 + k] ? (long long)(h[ct * 32 + k] - h[ct * 32]) : -1ll);
+            for (int k = 1; k < 14; ++k) printf(" [%d]%lld", k, h[ct * 32 + k] ? (long long)(h[ct * 32 + k] - h[ct * 32]) : -1ll);
             printf("\n");
         }
-        printf("  P1 loop cycles: search %llu  pivot-row %llu  update %llu  barrier %llu\n", h[40], h[41], h[42], h[43]);
     }
 #endif
     int64_t cur = i0;

@@ -355,46 +355,46 @@ __device__ __forceinline__ void strip_flush_u(StripSmem& sm, int slot, uint32_t*
 // One CTA's share of the in-strip update behind a factored base panel (pivot rows pr0..pr0+r, panel
 // columns jp.., T at Tb, pivot columns in rec):
 //   U = T . A[pr0 : pr0+r, cc0 : cc0+nc]                                   (kept in Us[slot])
-//   A[m, cc0 : cc0+nc] -= sum_k A[m, pivot column k] * U[k, :]   for this worker's rows m >= pr0 + r
-// Row worker rw of nrw.  Tiles of SRB rows: the L tile goes to shared memory k-major, the C tile stays
-// in registers (thread = 8 consecutive rows x 1 column: L by broadcast LDS.128, U by one LDS per k).
-__device__ __noinline__ void strip_update(StripSmem& sm, int slot, uint32_t* A, int64_t ld, int64_t rows,
-                             const uint32_t* Tb, const PanelRec* rec, int64_t jp, int64_t pr0, int r, int64_t cc0, int nc,
-                             int rw, int nrw) {
+//   A[m, cc0 : cc0+nc] -= sum_k A[m, pivot column k] * U[k, :]   for this worker's rows m in [my0, my1)
+// Tiles of 32*RPT rows: the L tile goes to shared memory k-major, the C tile stays in registers (thread =
+// RPT consecutive rows x 1 column: L by one broadcast vector LDS per k, U by one LDS per k).  RPT is chosen
+// from the number of rows the worker owns, so that a short share still spreads over all 32 warps.
+template <int RPT>
+__device__ __noinline__ void strip_update_t(StripSmem& sm, int slot, uint32_t* A, int64_t ld, const uint32_t* Tb,
+                                            const PanelRec* rec, int64_t jp, int64_t pr0, int r, int64_t cc0, int nc,
+                                            int64_t my0, int64_t my1, bool owner) {
     const ModP& f = c_f;
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
-    const int64_t mb0 = pr0 + r;
-    const int64_t mrem = rows - mb0;
-    int64_t rpw = (mrem + nrw - 1) / nrw;
-    rpw = (rpw + 7) / 8 * 8;
-    const int64_t my0 = mb0 + (int64_t)rw * rpw, my1 = min(rows, my0 + rpw);
+    constexpr int TR = 32 * RPT;
     // pivot index of panel column `lane` (pc[] is ascending), or -1
     const unsigned pcm = __reduce_or_sync(0xffffffffu, lane < r ? 1u << rec->pc[lane] : 0u);
     const int kcol = ((pcm >> lane) & 1u) ? __popc(pcm & ((1u << lane) - 1u)) : -1;
-    uint32_t cv[SRB / 32];
+    uint32_t cv[RPT];
     auto load_tile = [&](int64_t m0) {
-        uint32_t lreg[SRB / 32];
+        uint32_t lreg[RPT];
 #pragma unroll
-        for (int t = 0; t < SRB / 32; ++t) {
+        for (int t = 0; t < RPT; ++t) {
             const int64_t m = m0 + wq + 32 * t;
             lreg[t] = (kcol >= 0 && m < my1) ? A[m * ld + jp + lane] : 0u;
         }
 #pragma unroll
-        for (int t = 0; t < SRB / 32; ++t) {
-            const int64_t m = m0 + wq * (SRB / 32) + t;
+        for (int t = 0; t < RPT; ++t) {
+            const int64_t m = m0 + wq * RPT + t;
             cv[t] = (lane < nc && m < my1) ? A[m * ld + cc0 + lane] : 0u;
         }
         if (kcol >= 0) {
 #pragma unroll
-            for (int t = 0; t < SRB / 32; ++t) sm.Lk[kcol][wq + 32 * t] = lreg[t];
+            for (int t = 0; t < RPT; ++t) sm.Lk[kcol][wq + 32 * t] = lreg[t];
         }
     };
+    if (slot == 0) STRIP_STAMP(10);
     const uint32_t tval = Tb[wq * PW + lane];
     const uint32_t aval = (wq < r && lane < nc) ? A[(pr0 + wq) * ld + cc0 + lane] : 0u;
     if (my0 < my1) load_tile(my0);
     sm.Ts[wq][lane] = tval;
     sm.Ar[wq][lane] = aval;
     __syncthreads();
+    if (slot == 0) STRIP_STAMP(11);
     {
         uint64_t acc = 0;
 #pragma unroll 8
@@ -405,44 +405,73 @@ __device__ __noinline__ void strip_update(StripSmem& sm, int slot, uint32_t* A, 
         }
         sm.Us[slot][wq][lane] = wq < r ? reduce64(acc, f) : 0u;
     }
-    if (rw == 0 && tid == 0) { UPending& u = sm.pend[slot]; u.row0 = pr0; u.col0 = cc0; u.r = r; u.nc = nc; }
-    for (int64_t m0 = my0; m0 < my1; m0 += SRB) {
+    if (owner && tid == 0) { UPending& u = sm.pend[slot]; u.row0 = pr0; u.col0 = cc0; u.r = r; u.nc = nc; }
+    for (int64_t m0 = my0; m0 < my1; m0 += TR) {
         if (m0 != my0) {
             __syncthreads();             // previous tile's readers of Lk are done
             load_tile(m0);
         }
         __syncthreads();
-        if (m0 + wq * 8 < my1) {
-            uint64_t acc[SRB / 32];
+        if (slot == 0) STRIP_STAMP(12);
+        if (m0 + wq * RPT < my1) {
+            uint64_t acc[RPT];
 #pragma unroll
-            for (int t = 0; t < SRB / 32; ++t) acc[t] = 0;
-#pragma unroll 1
-            for (int k = 0; k + 1 < r; k += 2) {
+            for (int t = 0; t < RPT; ++t) acc[t] = 0;
+            auto mac = [&](int k) {
+                const uint32_t u = sm.Us[slot][k][lane];
+                uint32_t l[RPT];
+                if constexpr (RPT == 1) {
+                    l[0] = sm.Lk[k][wq];
+                } else if constexpr (RPT == 2) {
+                    const uint2 v = *reinterpret_cast<const uint2*>(&sm.Lk[k][wq * 2]);
+                    l[0] = v.x; l[1] = v.y;
+                } else {
 #pragma unroll
-                for (int kk = 0; kk < 2; ++kk) {
-                    const uint4 la = *reinterpret_cast<const uint4*>(&sm.Lk[k + kk][wq * 8]);
-                    const uint4 lb = *reinterpret_cast<const uint4*>(&sm.Lk[k + kk][wq * 8 + 4]);
-                    const uint32_t u = sm.Us[slot][k + kk][lane];
-                    const uint32_t l[8] = {la.x, la.y, la.z, la.w, lb.x, lb.y, lb.z, lb.w};
-#pragma unroll
-                    for (int t = 0; t < 8; ++t) acc[t] += (uint64_t)l[t] * u;
+                    for (int h = 0; h < RPT / 4; ++h) {
+                        const uint4 v = *reinterpret_cast<const uint4*>(&sm.Lk[k][wq * RPT + 4 * h]);
+                        l[4 * h] = v.x; l[4 * h + 1] = v.y; l[4 * h + 2] = v.z; l[4 * h + 3] = v.w;
+                    }
                 }
 #pragma unroll
-                for (int t = 0; t < 8; ++t) acc[t] = fold64(acc[t], f);
+                for (int t = 0; t < RPT; ++t) acc[t] += (uint64_t)l[t] * u;
+            };
+#pragma unroll 1
+            for (int k = 0; k + 1 < r; k += 2) {
+                mac(k);
+                mac(k + 1);
+#pragma unroll
+                for (int t = 0; t < RPT; ++t) acc[t] = fold64(acc[t], f);
             }
             if (r & 1) {
-                const uint32_t u0 = sm.Us[slot][r - 1][lane];
+                mac(r - 1);
 #pragma unroll
-                for (int t = 0; t < 8; ++t) acc[t] = fold64(acc[t] + (uint64_t)sm.Lk[r - 1][wq * 8 + t] * u0, f);
+                for (int t = 0; t < RPT; ++t) acc[t] = fold64(acc[t], f);
             }
 #pragma unroll
-            for (int t = 0; t < 8; ++t) {
-                const int64_t m = m0 + wq * 8 + t;
+            for (int t = 0; t < RPT; ++t) {
+                const int64_t m = m0 + wq * RPT + t;
                 if (lane < nc && m < my1) A[m * ld + cc0 + lane] = submod(cv[t], reduce64(acc[t], f), f);
             }
         }
     }
     __syncthreads();                     // Ts / Ar / Lk may be reused by the caller's next phase
+    if (slot == 0) STRIP_STAMP(13);
+}
+
+// Row worker rw of nrw: its rows, then the variant whose tile matches them.
+__device__ __forceinline__ void strip_update(StripSmem& sm, int slot, uint32_t* A, int64_t ld, int64_t rows,
+                                             const uint32_t* Tb, const PanelRec* rec, int64_t jp, int64_t pr0, int r,
+                                             int64_t cc0, int nc, int rw, int nrw) {
+    const int64_t mb0 = pr0 + r;
+    const int64_t mrem = rows - mb0;
+    int64_t rpw = (mrem + nrw - 1) / nrw;
+    rpw = (rpw + 7) / 8 * 8;
+    const int64_t my0 = min(rows, mb0 + (int64_t)rw * rpw), my1 = min(rows, my0 + rpw);
+    const int64_t n = my1 - my0;
+    if (n <= 32) strip_update_t<1>(sm, slot, A, ld, Tb, rec, jp, pr0, r, cc0, nc, my0, my1, rw == 0);
+    else if (n <= 64) strip_update_t<2>(sm, slot, A, ld, Tb, rec, jp, pr0, r, cc0, nc, my0, my1, rw == 0);
+    else if (n <= 128) strip_update_t<4>(sm, slot, A, ld, Tb, rec, jp, pr0, r, cc0, nc, my0, my1, rw == 0);
+    else strip_update_t<8>(sm, slot, A, ld, Tb, rec, jp, pr0, r, cc0, nc, my0, my1, rw == 0);
 }
 
 // The strip kernel, with one panel of look-ahead: while CTA 0 factors panel i (phase A), the other

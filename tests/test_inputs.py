@@ -53,3 +53,22 @@ def test_normal_system():
     assert np.allclose(np.diag(a).mean(), 4 * np.sqrt(300), atol=0.3)
     a2, _ = gen.shifted_normal_system(300, 8, 5, 6)
     assert np.array_equal(a, a2)
+
+
+def test_torch_generators_match_numpy_bit_for_bit():
+    """gen_torch (used to build config c5 on the device) against gen, on the CPU."""
+    import torch
+    from linac_inputs import gen_torch
+    p = 2147483647
+    u = gen_torch.uniform_rows(5, 7, 33, p, seed=4, device="cpu").numpy().view(np.uint32)
+    assert np.array_equal(u, gen.uniform_rows(5, 7, 33, p, seed=4))
+    rows = cols = 230
+    want = gen.sparse_dependent_rows(0, rows, rows, cols, p, seed=7, seed_dep=8)
+    got = gen_torch.sparse_dependent_rows(0, rows, rows, cols, p, seed=7, seed_dep=8).numpy().view(np.uint32)
+    assert np.array_equal(got, want)
+    part = gen_torch.sparse_dependent_rows(90, 70, rows, cols, p, seed=7, seed_dep=8).numpy().view(np.uint32)
+    assert np.array_equal(part, want[90:160])
+    dst = torch.zeros((rows, cols), dtype=torch.int32)
+    gen_torch.fill_c5(dst, dict(p=p, seed=7, seed_dep=8, period=50, terms=3), block_rows=64)
+    assert np.array_equal(dst.numpy().view(np.uint32), want)
+    assert 0.05 < (want != 0).mean() < 0.2 and (want[49] != 0).mean() > 0.2      # sparse rows, denser combinations
