@@ -29,6 +29,9 @@ sys.path.insert(0, ROOT)
 
 import linac_inputs as gen  # noqa: E402
 
+WORKLOAD_KIND = {"uniform": "dense uniform", "lowrank": "product of uniform factors (exact rank)",
+                 "sparse_dep": "90% zeros, every 50th row dependent"}
+
 PAPER_A100_GMULMOD = {"c3": (2 * 1e4 ** 3 / 3) / 3.6 / 1e9,            # PAPER.md:59  (3.6 s at N = 10^4)
                       "c5": (2 * 1e5 ** 3 / 3) / (45 * 60) / 1e9}       # PAPER.md:61  (45 min at N = 10^5)
 
@@ -135,7 +138,7 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3"])
+    ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c5"])
     ap.add_argument("--ref-n", type=int, default=1280, help="sample size for the oracle legs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
@@ -159,13 +162,24 @@ def main():
     dev = torch.device("cuda", local)
 
     from paper_2605_25863_b200 import replicas
-    a_host, p, cfg = make_workload(args.workload, rank_seed=rank)      # replicas: one matrix per rank
-    rows, cols = a_host.shape
+    on_device = gen.CONFIGS[args.workload]["kind"] == "sparse_dep"     # c5: 40 GB, generated straight into HBM
+    if on_device:
+        from linac_inputs import gen_torch
+        cfg = dict(gen.CONFIGS[args.workload])
+        cfg["seed"] += 1000 * rank
+        p, rows, cols = cfg["p"], cfg["rows"], cfg["cols"]
+        a_host = pinned = out_host = d_in = None
+        d_work = torch.empty((rows, cols), dtype=torch.int32, device=dev)
+        nbytes = rows * cols * 4
+    else:
+        a_host, p, cfg = make_workload(args.workload, rank_seed=rank)      # replicas: one matrix per rank
+        rows, cols = a_host.shape
+        nbytes = a_host.nbytes
+        pinned = torch.from_numpy(a_host.view(np.int32)).pin_memory()
+        d_in = pinned.to(dev, non_blocking=False)
+        d_work = torch.empty_like(d_in)
+        out_host = torch.empty_like(pinned).pin_memory()
     n_nominal = 2.0 * rows * cols * min(rows, cols) / 3.0              # 2N^3/3 for square N
-    pinned = torch.from_numpy(a_host.view(np.int32)).pin_memory()
-    d_in = pinned.to(dev, non_blocking=False)
-    d_work = torch.empty_like(d_in)
-    out_host = torch.empty_like(pinned).pin_memory()
     stream = torch.cuda.current_stream(dev)
 
     def barrier():
@@ -175,7 +189,10 @@ def main():
             torch.cuda.synchronize(dev)
 
     def step_resident():
-        d_work.copy_(d_in)                        # restore the input: NOT part of the step
+        if on_device:
+            gen_torch.fill_c5(d_work, cfg)        # regenerate the input: NOT part of the step
+        else:
+            d_work.copy_(d_in)                    # restore the input: NOT part of the step
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         rank_, _ = L.rref_u32(d_work, p)
@@ -215,14 +232,16 @@ def main():
     ms_per_step = total_ms / args.steps
     value = replicas.aggregate_throughput(n_nominal, ms_per_step * 1e-3, world) / 1e9
 
-    # end-to-end leg
-    step_e2e()
-    barrier()
-    e2e_times = [step_e2e()[0] for _ in range(max(2, min(args.steps, 3)))]
-    barrier()
-    e2e_ms = float(np.mean(e2e_times))
-    e2e_ms = replicas.max_over_ranks(e2e_ms, dev)
-    e2e_value = replicas.aggregate_throughput(n_nominal, e2e_ms * 1e-3, world) / 1e9
+    # end-to-end leg (host buffers; not run for the device-generated 40 GB config)
+    e2e_ms = e2e_value = None
+    if not on_device:
+        step_e2e()
+        barrier()
+        e2e_times = [step_e2e()[0] for _ in range(max(2, min(args.steps, 3)))]
+        barrier()
+        e2e_ms = float(np.mean(e2e_times))
+        e2e_ms = replicas.max_over_ranks(e2e_ms, dev)
+        e2e_value = replicas.aggregate_throughput(n_nominal, e2e_ms * 1e-3, world) / 1e9
 
     # roofline of the dominant kernel family (Schur update), event-timed launch by launch
     L.set_option("timing", 1)
@@ -241,7 +260,11 @@ def main():
         ach = achieved_tmacs * 16 * 2 if achieved_tmacs else None
         roof = {"bound": "tensor", "achieved": ach, "peak": peak, "unit": "TOP/s (int8, 2 ops per MAC)",
                 "frac": ach / peak if ach else None, "traffic": None,
-                "note": f"peak = 2 x {peaks['source']} sustained bf16 (guide's nominal int8:bf16 ratio)"}
+                "kernel": "Schur-update GEMMs on tcgen05 kind::i8 (gemm_tc_panel_kernel for K <= 256, gemm_tc_kernel above), "
+                          "limb-split pre-passes included in the time",
+                "note": f"achieved = executed update field-MACs x 16 u8 MACs x 2 ops / summed CUDA-event time of those "
+                        f"launches on the call's stream; peak = 2 x {peaks['source']} sustained bf16 (guide's nominal "
+                        f"int8:bf16 ratio); traffic: see profiles/ (ncu --set full capture of the top launch)"}
     else:
         # CUDA-core path: one IMAD.WIDE.U32 per field MAC; nominal issue peak 148 SM x 64 lanes x f_max
         peak = 148 * 64 * peaks["sm_max_mhz"] * 1e6 / 1e12
@@ -258,15 +281,18 @@ def main():
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": (value / world / PAPER_A100_GMULMOD[args.workload]) if args.workload in PAPER_A100_GMULMOD else None,
         "dtype": "u32", "data": "synthetic",
-        "config": {"workload": f"{args.workload}: {rows}x{cols} uint32 dense uniform, p={p}", "rank": int(ranks[-1]),
+        "config": {"workload": f"{args.workload}: {rows}x{cols} uint32 {WORKLOAD_KIND[cfg['kind']]}, p={p}", "rank": int(ranks[-1]),
                    "parallelism": "replicas" if world > 1 else "single", "l2": "input (%d MB) larger than L2" %
-                   (a_host.nbytes // 2 ** 20) if a_host.nbytes > 126 * 2 ** 20 else "input fits L2; restored by a device copy each step"},
-        "e2e": {"value": e2e_value, "unit": "Gmulmod/s", "ms_per_step": e2e_ms, "h2d_bytes_per_step": int(a_host.nbytes),
-                "d2h_bytes_per_step": int(a_host.nbytes)},
+                   (nbytes // 2 ** 20) if nbytes > 126 * 2 ** 20 else "input fits L2; restored by a device copy each step",
+                   "options": args.opt},
+        "e2e": {"value": e2e_value, "unit": "Gmulmod/s", "ms_per_step": e2e_ms,
+                "h2d_bytes_per_step": 0 if on_device else int(nbytes), "d2h_bytes_per_step": 0 if on_device else int(nbytes),
+                **({"note": "not measured: this config is generated on the device (40 GB)"} if on_device else {})},
         "gpu_launches": int(stats["kernel_launches"]) * args.steps,
         "clocks": clocks, "roofline": roof,
         "stats": {k: stats[k] for k in ("kernel_launches", "host_syncs", "panels", "row_swaps", "update_macs")},
-        "baseline_context": "paper: A100, 3.6 s at N=1e4 (PAPER.md:59) = 185 Gmulmod/s; another machine, context only",
+        "baseline_context": "paper, A100: 3.6 s at N=1e4 (PAPER.md:59) = 185 Gmulmod/s, 45 min at N=1e5 (PAPER.md:61) = 247 "
+                            "Gmulmod/s; another machine, context only",
     }
     if rank == 0 and not args.no_cpu_baseline:
         import oracle
