@@ -41,11 +41,14 @@ struct Fp {
     PanelRec* h_rec;          // pinned, MAXBP records
     std::vector<int64_t> pstart;     // [nb+1] pivots found left of base panel b
     std::vector<int32_t> pivcols;
-    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev_strip = nullptr;
+    cudaStream_t copy_s = nullptr;   // second stream: device->host reads of the pivot counts
 
     int64_t sb0(int64_t s) const { return std::min(nb, s * bps); }          // first base panel of strip s
     int64_t sp(int64_t s) const { return pstart[sb0(s)]; }                  // pivots found left of strip s
 };
+
+constexpr int LINAC_EARLY_SOLVE_DONE = -1000;      // internal: factor_strip already enqueued the row-block solve
 
 int64_t panel_col0(int64_t b) { return b * PW; }
 
@@ -118,7 +121,10 @@ int trsm_lower(Fp& c, int64_t s0, int64_t s1, int64_t c0, int64_t c1) {
 }
 
 // One strip s with active rows >= i0 (one cooperative launch).  Returns the number of pivots through *r.
-int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r) {
+// If early_ncols > 0 the strip's row-block solve on columns [early_c0, early_c0 + early_ncols) is enqueued right
+// behind the strip kernel (it takes the pivot counts from device memory), and the host reads the pivot counts
+// through a second stream meanwhile: the round trip then hides under the solve instead of idling the GPU.
+int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r, int64_t early_c0 = 0, int64_t early_ncols = 0) {
     const int64_t b0 = c.sb0(s), b1 = c.sb0(s + 1);
     const int64_t j0 = panel_col0(b0), j1 = std::min(c.cols, panel_col0(b1));
     StripArgs a;
@@ -130,9 +136,21 @@ int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r) {
         LINAC_CUDA(cudaLaunchCooperativeKernel((void*)strip_factor_kernel, dim3((unsigned)c.coop_grid), dim3(SNT), args,
                                                sizeof(StripSmem), c.s));
     }
-    LINAC_CUDA(cudaMemcpyAsync(c.h_rec, c.d_rec + b0, (size_t)(b1 - b0) * sizeof(PanelRec), cudaMemcpyDeviceToHost, c.s));
-    LINAC_CUDA(cudaStreamSynchronize(c.s));
     linac_stats& st = stats();
+    if (early_ncols > 0 && options().timing == 0) {
+        LINAC_CUDA(cudaEventRecord(c.ev_strip, c.s));
+        trsm_strip_kernel<true><<<(unsigned)((early_ncols + PW - 1) / PW), TNT, trsm_smem_bytes(j1 - j0), c.s>>>(
+            c.A, c.ld, c.A + i0 * c.ld + early_c0, c.ld, early_ncols, c.d_pstart, (int)b0, (int)b1, c.d_T, c.d_pivcols, c.f);
+        LINAC_CUDA(cudaGetLastError());
+        st.kernel_launches++;
+        LINAC_CUDA(cudaStreamWaitEvent(c.copy_s, c.ev_strip, 0));
+        LINAC_CUDA(cudaMemcpyAsync(c.h_rec, c.d_rec + b0, (size_t)(b1 - b0) * sizeof(PanelRec), cudaMemcpyDeviceToHost, c.copy_s));
+        LINAC_CUDA(cudaStreamSynchronize(c.copy_s));
+    } else {
+        early_ncols = 0;
+        LINAC_CUDA(cudaMemcpyAsync(c.h_rec, c.d_rec + b0, (size_t)(b1 - b0) * sizeof(PanelRec), cudaMemcpyDeviceToHost, c.s));
+        LINAC_CUDA(cudaStreamSynchronize(c.s));
+    }
     st.kernel_launches++;
     st.host_syncs++;
 #ifdef LINAC_TRACE
@@ -157,11 +175,12 @@ int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r) {
         c.pstart[b + 1] = cur;
     }
     *r = cur - i0;
-    return LINAC_OK;
+    if (early_ncols > 0) st.update_macs += (*r) * (*r) / 2 * early_ncols;
+    return early_ncols > 0 ? LINAC_EARLY_SOLVE_DONE : LINAC_OK;
 }
 
 // Recursive factorisation of strips [s0, s1) with active rows [i0, rows).  Fills pstart for their panels.
-int factor(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t* r_out) {
+int factor(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t* r_out, bool allow_flat = true) {
     *r_out = 0;
     if (s1 <= s0) return LINAC_OK;
     if (i0 >= c.rows) {                              // no rows left: every remaining column is free
@@ -172,19 +191,30 @@ int factor(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t* r_out) {
         return LINAC_OK;
     }
     if (s1 - s0 == 1) return factor_strip(c, s0, i0, r_out);
-    if ((s1 - s0) * c.bps * PW <= options().flat_cols) {
-        // flat right-looking sweep over the node's strips: factor, row-block solve on the columns to the
-        // right (inside the node), Schur update of everything below with K = the strip's pivots
+    if (allow_flat && (s1 - s0) * c.bps * PW <= options().flat_cols) {
+        // Flat right-looking sweep over the node, a GROUP of flat_group strips at a time: the group is factored
+        // by binary recursion confined to its own columns, then one row-block solve on the node's columns to
+        // the right and ONE Schur update of everything below with K = the group's pivots (256 for two strips:
+        // half as many read-modify-write passes over the trailing matrix as a per-strip update).
         const int64_t jend = std::min(c.cols, panel_col0(c.sb0(s1)));
+        const int64_t grp = std::max<int64_t>(1, options().flat_group);
         int64_t cur = i0;
-        for (int64_t s = s0; s < s1; ++s) {
+        for (int64_t s = s0; s < s1; s += grp) {
+            const int64_t se = std::min(s1, s + grp);
             int64_t r = 0;
-            if (cur >= c.rows) return factor(c, s, s1, cur, &r);      // marks the remaining columns free
-            int rc = factor_strip(c, s, cur, &r);
+            const int64_t jc = std::min(c.cols, panel_col0(c.sb0(se)));
+            int rc;
+            bool solved = false;
+            if (se - s == 1 && cur < c.rows) {
+                rc = factor_strip(c, s, cur, &r, jc, jend - jc);
+                solved = rc == LINAC_EARLY_SOLVE_DONE;
+                if (solved) rc = LINAC_OK;
+            } else {
+                rc = factor(c, s, se, cur, &r, false);                    // also marks columns free once rows run out
+            }
             if (rc) return rc;
-            const int64_t jc = std::min(c.cols, panel_col0(c.sb0(s + 1)));
             if (r > 0 && jend > jc) {
-                rc = trsm_leaf<true>(c, s, c.A + cur * c.ld + jc, c.ld, jend - jc);
+                if (!solved) rc = trsm_lower(c, s, se, jc, jend);
                 if (rc) return rc;
                 const int64_t m2 = c.rows - (cur + r);
                 if (m2 > 0) {
@@ -202,7 +232,7 @@ int factor(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t* r_out) {
     const int64_t sm = s0 + (s1 - s0) / 2;
     const int64_t jm = panel_col0(c.sb0(sm)), j1 = std::min(c.cols, panel_col0(c.sb0(s1)));
     int64_t r1 = 0, r2 = 0;
-    int rc = factor(c, s0, sm, i0, &r1);
+    int rc = factor(c, s0, sm, i0, &r1, allow_flat);
     if (rc) return rc;
     if (r1 > 0) {
         rc = trsm_lower(c, s0, sm, jm, j1);
@@ -215,7 +245,7 @@ int factor(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t* r_out) {
             if (rc) return rc;
         }
     }
-    rc = factor(c, sm, s1, i0 + r1, &r2);
+    rc = factor(c, sm, s1, i0 + r1, &r2, allow_flat);
     *r_out = r1 + r2;
     return rc;
 }
@@ -329,6 +359,10 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     c.pstart.assign(c.nb + 1, 0);
     LINAC_CUDA(cudaEventCreate(&c.ev0));
     LINAC_CUDA(cudaEventCreate(&c.ev1));
+    LINAC_CUDA(cudaEventCreateWithFlags(&c.ev_strip, cudaEventDisableTiming));
+    static cudaStream_t copy_stream = nullptr;
+    if (!copy_stream) LINAC_CUDA(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
+    c.copy_s = copy_stream;
     cudaEvent_t t0, t1;
     LINAC_CUDA(cudaEventCreate(&t0));
     LINAC_CUDA(cudaEventCreate(&t1));
@@ -396,7 +430,7 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     if (e == cudaSuccess) cudaEventElapsedTime(&ms, t0, t1);
     st.ms_total = ms;
     cudaEventDestroy(t0); cudaEventDestroy(t1);
-    cudaEventDestroy(c.ev0); cudaEventDestroy(c.ev1);
+    cudaEventDestroy(c.ev0); cudaEventDestroy(c.ev1); cudaEventDestroy(c.ev_strip);
     if (rc) return rc;
     *rank = r;
     if (pivot_cols_out) std::copy(c.pivcols.begin(), c.pivcols.begin() + r, pivot_cols_out);

@@ -91,22 +91,29 @@ struct StripSmem {
 // rows, which a division-free elimination does not care about, and the tracked scales absorb it.  Fails (returns false, nothing
 // written) as soon as a column has no pivot among the unused rows: the caller then runs the general
 // path, which handles rank-deficient and multi-chunk panels.
+// Block rows per working warp of the fast panel: 8 (4 warps, one per scheduler) or 4 (8 warps).
+#ifndef FAST_RPW
+#define FAST_RPW 4
+#endif
+#if FAST_RPW == 8
+#define FAST_IF8(...) __VA_ARGS__
+#else
+#define FAST_IF8(...)
+#endif
 __device__ __forceinline__ bool panel_fast(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t i0, int64_t j0) {
     const ModP& f = c_f;
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
-    constexpr int FW = 8, RPW = PW / FW;          // 8 working warps, 4 block rows each (registers)
-    static_assert(RPW == 4, "the row macros below are written for four rows per warp");
-    uint32_t x0 = 0, x1 = 0, x2 = 0, x3 = 0;
+    constexpr int FW = PW / FAST_RPW, RPW = FAST_RPW;          // working warps, block rows per warp (registers)
+    uint32_t x0 = 0, x1 = 0, x2 = 0, x3 = 0, x4 = 0, x5 = 0, x6 = 0, x7 = 0;
     const int row0 = wq * RPW;
+#define FAST_EACH_ROW(M) M(x0, 0) M(x1, 1) M(x2, 2) M(x3, 3) FAST_IF8(M(x4, 4) M(x5, 5) M(x6, 6) M(x7, 7))
     if (wq < FW) {
-        x0 = A[(i0 + row0 + 0) * ld + j0 + lane];
-        x1 = A[(i0 + row0 + 1) * ld + j0 + lane];
-        x2 = A[(i0 + row0 + 2) * ld + j0 + lane];
-        x3 = A[(i0 + row0 + 3) * ld + j0 + lane];
-        sm.W[0][row0 + 0][lane] = x0;
-        sm.W[0][row0 + 1][lane] = x1;
-        sm.W[0][row0 + 2][lane] = x2;
-        sm.W[0][row0 + 3][lane] = x3;
+#define FAST_LOAD(X, I) X = A[(i0 + row0 + I) * ld + j0 + lane];
+        FAST_EACH_ROW(FAST_LOAD)
+#undef FAST_LOAD
+#define FAST_PUT(X, I) sm.W[0][row0 + I][lane] = X;
+        FAST_EACH_ROW(FAST_PUT)
+#undef FAST_PUT
     }
     __syncthreads();
     STRIP_STAMP(1);
@@ -133,7 +140,7 @@ __device__ __forceinline__ bool panel_fast(StripSmem& sm, const uint32_t* A, int
                 X = (row0 + I) != q ? upd : (atc ? dtot : X);                                            \
                 sm.W[buf ^ 1][row0 + I][lane] = X;                                                       \
             }
-            FAST_ROW(x0, 0) FAST_ROW(x1, 1) FAST_ROW(x2, 2) FAST_ROW(x3, 3)
+            FAST_EACH_ROW(FAST_ROW)
 #undef FAST_ROW
             if (tid == 0) { sm.esrc[c] = i0 + q; sm.gs[0][c] = dtot; }    // gs[0][c] = prefix product BEFORE step c
             dtot = mulredc(dtot, d, f);
@@ -361,13 +368,12 @@ __device__ __forceinline__ void strip_flush_u(StripSmem& sm, int slot, uint32_t*
 // from the number of rows the worker owns, so that a short share still spreads over all 32 warps.
 template <int RPT>
 __device__ __noinline__ void strip_update_t(StripSmem& sm, int slot, uint32_t* A, int64_t ld, const uint32_t* Tb,
-                                            const PanelRec* rec, int64_t jp, int64_t pr0, int r, int64_t cc0, int nc,
+                                            unsigned pcm, int64_t jp, int64_t pr0, int r, int64_t cc0, int nc,
                                             int64_t my0, int64_t my1, bool owner) {
     const ModP& f = c_f;
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
     constexpr int TR = 32 * RPT;
-    // pivot index of panel column `lane` (pc[] is ascending), or -1
-    const unsigned pcm = __reduce_or_sync(0xffffffffu, lane < r ? 1u << rec->pc[lane] : 0u);
+    // pivot index of panel column `lane` (pcm = mask of the panel's pivot columns, ascending), or -1
     const int kcol = ((pcm >> lane) & 1u) ? __popc(pcm & ((1u << lane) - 1u)) : -1;
     uint32_t cv[RPT];
     auto load_tile = [&](int64_t m0) {
@@ -460,7 +466,7 @@ __device__ __noinline__ void strip_update_t(StripSmem& sm, int slot, uint32_t* A
 
 // Row worker rw of nrw: its rows, then the variant whose tile matches them.
 __device__ __forceinline__ void strip_update(StripSmem& sm, int slot, uint32_t* A, int64_t ld, int64_t rows,
-                                             const uint32_t* Tb, const PanelRec* rec, int64_t jp, int64_t pr0, int r,
+                                             const uint32_t* Tb, unsigned pcm, int64_t jp, int64_t pr0, int r,
                                              int64_t cc0, int nc, int rw, int nrw) {
     const int64_t mb0 = pr0 + r;
     const int64_t mrem = rows - mb0;
@@ -468,10 +474,10 @@ __device__ __forceinline__ void strip_update(StripSmem& sm, int slot, uint32_t* 
     rpw = (rpw + 7) / 8 * 8;
     const int64_t my0 = min(rows, mb0 + (int64_t)rw * rpw), my1 = min(rows, my0 + rpw);
     const int64_t n = my1 - my0;
-    if (n <= 32) strip_update_t<1>(sm, slot, A, ld, Tb, rec, jp, pr0, r, cc0, nc, my0, my1, rw == 0);
-    else if (n <= 64) strip_update_t<2>(sm, slot, A, ld, Tb, rec, jp, pr0, r, cc0, nc, my0, my1, rw == 0);
-    else if (n <= 128) strip_update_t<4>(sm, slot, A, ld, Tb, rec, jp, pr0, r, cc0, nc, my0, my1, rw == 0);
-    else strip_update_t<8>(sm, slot, A, ld, Tb, rec, jp, pr0, r, cc0, nc, my0, my1, rw == 0);
+    if (n <= 32) strip_update_t<1>(sm, slot, A, ld, Tb, pcm, jp, pr0, r, cc0, nc, my0, my1, rw == 0);
+    else if (n <= 64) strip_update_t<2>(sm, slot, A, ld, Tb, pcm, jp, pr0, r, cc0, nc, my0, my1, rw == 0);
+    else if (n <= 128) strip_update_t<4>(sm, slot, A, ld, Tb, pcm, jp, pr0, r, cc0, nc, my0, my1, rw == 0);
+    else strip_update_t<8>(sm, slot, A, ld, Tb, pcm, jp, pr0, r, cc0, nc, my0, my1, rw == 0);
 }
 
 // The strip kernel, with one panel of look-ahead: while CTA 0 factors panel i (phase A), the other
@@ -493,6 +499,7 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
     bool owe = false;
     int64_t pb = 0, pjp = 0, ppr0 = 0, pcu0 = 0;
     int pr = 0;
+    unsigned ppcm = 0;
 
     if (tid == 0) { sm.pend[0].row0 = -1; sm.pend[1].row0 = -1; }
     __syncthreads();
@@ -526,12 +533,12 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
                     const int nrw = workers / nrest, cb = 1 + job % nrest, rw = job / nrest;
                     const int64_t cc0 = pcu0 + (int64_t)cb * PW;
                     if (rw < nrw)
-                        strip_update(sm, 1, A, ld, a.rows, a.T + pb * PW * PW, a.rec + pb, pjp, ppr0, pr, cc0,
+                        strip_update(sm, 1, A, ld, a.rows, a.T + pb * PW * PW, ppcm, pjp, ppr0, pr, cc0,
                                      (int)min((int64_t)PW, cu1 - cc0), rw, nrw);
                 } else {                                            // tiny grid: blocks in turn (flush between them)
                     for (int cb = 1 + job; cb <= nrest; cb += workers) {
                         const int64_t cc0 = pcu0 + (int64_t)cb * PW;
-                        strip_update(sm, 1, A, ld, a.rows, a.T + pb * PW * PW, a.rec + pb, pjp, ppr0, pr, cc0,
+                        strip_update(sm, 1, A, ld, a.rows, a.T + pb * PW * PW, ppcm, pjp, ppr0, pr, cc0,
                                      (int)min((int64_t)PW, cu1 - cc0), 0, 1);
                         // sole reader and writer of this block: the slice can go back at once
                         strip_flush_u(sm, 1, A, ld);
@@ -549,8 +556,10 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
         strip_flush_u(sm, 1, A, ld);
         __syncthreads();
         if (tid == 0) sm.pend[1].row0 = -1;
+        // everything the updates need from the panel record, in ONE round trip to L2
         const PanelRec* rec = a.rec + b;
-        const int r = rec->r, nsw = rec->nswaps;
+        const int r = rec->r, nsw = rec->nswaps, pcl = rec->pc[lane];
+        const unsigned pcm = __reduce_or_sync(0xffffffffu, pcl >= 0 ? 1u << pcl : 0u);
         if (r == 0) continue;
         // ---- row exchanges on complete rows, one thread per column (so the sequence of exchanges
         // needs no inter-thread ordering)
@@ -573,10 +582,10 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
         const int64_t cu0 = jp + w;
         if (cu0 < cu1) {
             // ---- phase B: the next panel's columns, all CTAs as row workers
-            strip_update(sm, 0, A, ld, a.rows, a.T + b * PW * PW, rec, jp, cur, r, cu0, (int)min((int64_t)PW, cu1 - cu0),
+            strip_update(sm, 0, A, ld, a.rows, a.T + b * PW * PW, pcm, jp, cur, r, cu0, (int)min((int64_t)PW, cu1 - cu0),
                          cta, G);
             owe = cu1 - cu0 > PW;
-            pb = b; pjp = jp; ppr0 = cur; pcu0 = cu0; pr = r;
+            pb = b; pjp = jp; ppr0 = cur; pcu0 = cu0; pr = r; ppcm = pcm;
             STRIP_STAMP(8);
             grid.sync();
             STRIP_STAMP(9);

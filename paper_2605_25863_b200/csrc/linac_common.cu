@@ -175,6 +175,9 @@ int linac_set_option(const char* name, int64_t value) {
     } else if (!strcmp(name, "tc_panel")) {
         if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
         g_options.tc_panel = value;
+    } else if (!strcmp(name, "flat_group")) {
+        if (value < 1 || value > 64) return LINAC_ERR_INVALID_ARG;
+        g_options.flat_group = value;
     } else if (!strcmp(name, "flat_cols")) {
         if (value < 0) return LINAC_ERR_INVALID_ARG;
         g_options.flat_cols = value;

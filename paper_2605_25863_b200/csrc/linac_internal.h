@@ -42,6 +42,7 @@ struct Options {
     int64_t tc_min_mn = 128;  // smallest M and N the tensor path is used for
     int64_t tc_panel = 1;     // 1 = K <= 256 updates use the persistent A-stationary tensor kernel
     int64_t flat_cols = 16384; // nodes of at most this many columns are swept flat (right-looking), wider ones recurse
+    int64_t flat_group = 1;   // strips per Schur update of the flat sweep (K = flat_group * strip_width)
     int64_t strip_width = 128; // columns factored by one cooperative strip kernel (multiple of 32, <= 256)
 };
 Options& options();
