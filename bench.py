@@ -32,6 +32,9 @@ import linac_inputs as gen  # noqa: E402
 WORKLOAD_KIND = {"uniform": "dense uniform", "lowrank": "product of uniform factors (exact rank)",
                  "sparse_dep": "90% zeros, every 50th row dependent"}
 
+#: ncu --set full, gemm_tc_panel_kernel, second launch of a c3 call (profiles/r01_v6_launches_c3.md)
+NCU_TOP_LAUNCH_DRAM_BYTES_C3 = 395558144 + 324742912
+
 PAPER_A100_GMULMOD = {"c3": (2 * 1e4 ** 3 / 3) / 3.6 / 1e9,            # PAPER.md:59  (3.6 s at N = 10^4)
                       "c5": (2 * 1e5 ** 3 / 3) / (45 * 60) / 1e9}       # PAPER.md:61  (45 min at N = 10^5)
 
@@ -272,6 +275,20 @@ def main():
                 "frac": achieved_tmacs / peak if achieved_tmacs else None, "traffic": None,
                 "note": "peak = 148 SM x 64 IMAD lanes x max SM clock (DESIGN.md); "
                         "achieved = executed update MACs / summed event time of the update kernels"}
+    # the largest single launch, per launch: algorithmic bytes (C read + C written + both limb-plane sets read) and,
+    # for the default workload, the DRAM traffic ncu measured for the same launch (profiles/r01_v6_launches_c3.md)
+    tm_, tn_, tk_ = st_t.get("top_m", 0), st_t.get("top_n", 0), st_t.get("top_k", 0)
+    if tensor_used and st_t.get("ms_update_top", 0) > 0:
+        kp_ = -(-tk_ // 128) * 128
+        roof["top_launch"] = {
+            "M": tm_, "N": tn_, "K": tk_, "ms": st_t["ms_update_top"],
+            "achieved": 32.0 * tm_ * tn_ * tk_ / (st_t["ms_update_top"] * 1e-3) / 1e12,
+            "algorithmic_bytes": 8 * tm_ * tn_ + 4 * kp_ * (tm_ + tn_),
+            "note": "event-timed, limb split included"}
+        if args.workload == "c3" and not args.opt:
+            roof["traffic"] = NCU_TOP_LAUNCH_DRAM_BYTES_C3
+            roof["top_launch"]["traffic_note"] = ("roofline.traffic = dram__bytes_read.sum + dram__bytes_write.sum of the "
+                                                  "M = N = 9744, K = 128 launch in the ncu --set full capture")
     roof["update_share_of_step"] = ms_upd / st_t["ms_total"] if st_t["ms_total"] else None
     roof["timed_split_ms"] = {"update": ms_upd, "strip": st_t.get("ms_strip"), "trsm": st_t.get("ms_trsm"),
                               "total_with_timing_syncs": st_t["ms_total"]}

@@ -144,6 +144,8 @@ typedef struct {
     double  ms_total;            /* device ms of the whole call, if timed                         */
     double  ms_strip;            /* device ms in the cooperative strip kernels (S1-S4), if timed   */
     double  ms_trsm;             /* device ms in the triangular-solve leaf kernels, if timed       */
+    double  ms_update_top;       /* device ms of the largest single Schur update (incl. its limb split), if timed */
+    int64_t top_m, top_n, top_k; /* its shape                                                      */
 } linac_stats;
 int linac_get_last_stats(linac_stats *out);
 /* Tunables, mainly for A/B measurements: name in {"gemm_path" (0 auto, 1 CUDA-core, 2 tensor), "timing" (0/1), "tc_min_k", "tc_min_mn",

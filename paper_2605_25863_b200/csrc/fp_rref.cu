@@ -69,6 +69,10 @@ int run_gemm(Fp& c, const GemmArgs& g) {
         float ms = 0;
         cudaEventElapsedTime(&ms, c.ev0, c.ev1);
         stats().ms_update += ms;
+        if ((double)g.M * g.N * g.K > (double)stats().top_m * stats().top_n * stats().top_k) {
+            stats().top_m = g.M; stats().top_n = g.N; stats().top_k = g.K;
+            stats().ms_update_top = ms;
+        }
     }
     return rc;
 }
