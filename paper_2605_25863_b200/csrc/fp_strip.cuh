@@ -293,8 +293,11 @@ __device__ void panel_exchange_list(StripSmem& sm, int64_t i0, int r, PanelRec* 
 // P1 for one base panel (columns [j0, j0+w), rows >= i0), executed by ONE CTA of SNT threads.
 // Outputs: rec (r, local pivot columns, exchange list), T (32x32, zero padded), E = T A[P, panel] when
 // r < w (the free columns' entries of the reduced pivot rows), pivcols.
-__device__ void panel_factor(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t rows, int64_t i0, int64_t j0, int w,
-                             PanelRec* rec, uint32_t* Tout, uint32_t* Eout, int32_t* pivcols_global) {
+// With allow_general = false only the fast path is tried (the caller has not finished updating the rows beyond
+// the 32 candidates); returns whether the panel was factored.
+__device__ bool panel_factor(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t rows, int64_t i0, int64_t j0, int w,
+                             PanelRec* rec, uint32_t* Tout, uint32_t* Eout, int32_t* pivcols_global,
+                             bool allow_general = true) {
     const ModP& f = c_f;
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
     int r = 0;
@@ -313,6 +316,7 @@ __device__ void panel_factor(StripSmem& sm, const uint32_t* A, int64_t ld, int64
         const int qa = (int)(sm.esrc[wq] - i0);
         Tout[wq * PW + lane] = mulmod(sm.ginv[wq], sm.W[0][qa][lane], f);
     } else {
+        if (!allow_general) return false;
         __syncthreads();
         r = panel_scan(sm, A, ld, rows, i0, j0, w);
         if (wq == 0) panel_exchange_list(sm, i0, r, rec);
@@ -331,6 +335,7 @@ __device__ void panel_factor(StripSmem& sm, const uint32_t* A, int64_t ld, int64
         sm.r_out = r;
     }
     STRIP_STAMP(4);
+    return true;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -467,22 +472,30 @@ __device__ __noinline__ void strip_update_t(StripSmem& sm, int slot, uint32_t* A
 // Row worker rw of nrw: its rows, then the variant whose tile matches them.
 __device__ __forceinline__ void strip_update(StripSmem& sm, int slot, uint32_t* A, int64_t ld, int64_t rows,
                                              const uint32_t* Tb, unsigned pcm, int64_t jp, int64_t pr0, int r,
-                                             int64_t cc0, int nc, int rw, int nrw) {
-    const int64_t mb0 = pr0 + r;
+                                             int64_t cc0, int nc, int rw, int nrw, int skip, bool owner) {
+    const int64_t mb0 = min(rows, pr0 + r + skip);       // `skip` rows right below the pivots belong to someone else
     const int64_t mrem = rows - mb0;
     int64_t rpw = (mrem + nrw - 1) / nrw;
     rpw = (rpw + 7) / 8 * 8;
     const int64_t my0 = min(rows, mb0 + (int64_t)rw * rpw), my1 = min(rows, my0 + rpw);
     const int64_t n = my1 - my0;
-    if (n <= 32) strip_update_t<1>(sm, slot, A, ld, Tb, pcm, jp, pr0, r, cc0, nc, my0, my1, rw == 0);
-    else if (n <= 64) strip_update_t<2>(sm, slot, A, ld, Tb, pcm, jp, pr0, r, cc0, nc, my0, my1, rw == 0);
-    else if (n <= 128) strip_update_t<4>(sm, slot, A, ld, Tb, pcm, jp, pr0, r, cc0, nc, my0, my1, rw == 0);
-    else strip_update_t<8>(sm, slot, A, ld, Tb, pcm, jp, pr0, r, cc0, nc, my0, my1, rw == 0);
+    if (n <= 32) strip_update_t<1>(sm, slot, A, ld, Tb, pcm, jp, pr0, r, cc0, nc, my0, my1, owner);
+    else if (n <= 64) strip_update_t<2>(sm, slot, A, ld, Tb, pcm, jp, pr0, r, cc0, nc, my0, my1, owner);
+    else if (n <= 128) strip_update_t<4>(sm, slot, A, ld, Tb, pcm, jp, pr0, r, cc0, nc, my0, my1, owner);
+    else strip_update_t<8>(sm, slot, A, ld, Tb, pcm, jp, pr0, r, cc0, nc, my0, my1, owner);
 }
 
-// The strip kernel, with one panel of look-ahead: while CTA 0 factors panel i (phase A), the other
-// CTAs finish panel i-1's update on the columns right of panel i; only the update of panel i's OWN
-// columns (phase B of the previous iteration) sits on the panel-to-panel dependency chain.
+// The strip kernel, software-pipelined so that ONE grid barrier per base panel sits on the pivot-to-pivot
+// dependency chain.  Loop invariant at the top of iteration i: panel i is factored (record, T, pivot columns
+// published and a barrier passed) and every update of the panels before i has been applied everywhere.  Then,
+// between two barriers,
+//   CTA 0        updates the 32 candidate rows of panel i+1 (its own U slice, a 32-row tile) and factors panel
+//                i+1 from them by the fast path;
+//   CTAs 1..G-1  apply panel i's update to all the other rows below and all strip columns to the right
+//                (2-D split: column block x row worker; U = T.A12 recomputed per CTA, written back by the
+//                owners after the barrier because every row worker reads the raw entries).
+// If the fast path does not apply or fails (rank-deficient candidates), CTA 0 factors panel i+1 by the general
+// path after the barrier, when all rows are up to date, and one more barrier follows.
 __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a) {
     extern __shared__ __align__(16) unsigned char strip_smem_raw[];
     StripSmem& sm = *reinterpret_cast<StripSmem*>(strip_smem_raw);
@@ -495,72 +508,51 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
     const int64_t b0 = a.j0 / PW;
     const int64_t cu1 = a.j0 + a.ws;               // end of the strip
     int64_t cur = a.i0;
-    // panel i-1, if it still owes the update of the columns right of panel i
-    bool owe = false;
-    int64_t pb = 0, pjp = 0, ppr0 = 0, pcu0 = 0;
-    int pr = 0;
-    unsigned ppcm = 0;
+
+    // CTA 0: factor panel bb (columns jpp.., width ww) from row `row` on, fast path first, general path otherwise.
+    auto factor_full = [&](int64_t bb, int64_t jpp, int ww, int64_t row) {
+        if (cta != 0) return;
+        if (row < a.rows) {
+            panel_factor(sm, A, ld, a.rows, row, jpp, ww, a.rec + bb, a.T + bb * PW * PW, a.E + bb * PW * PW, a.pivcols);
+            if (tid == 0) a.pstart[bb + 1] = (int32_t)(row + sm.r_out);
+        } else if (tid == 0) {                     // no rows left: the panel's columns are free
+            a.rec[bb].r = 0; a.rec[bb].nswaps = 0; a.rec[bb].w = ww;
+            a.pstart[bb + 1] = (int32_t)row;
+        }
+    };
+    auto flush_all = [&]() {                       // U slices whose readers all passed the last grid barrier
+        strip_flush_u(sm, 0, A, ld);
+        strip_flush_u(sm, 1, A, ld);
+        __syncthreads();
+        if (tid == 0) { sm.pend[0].row0 = -1; sm.pend[1].row0 = -1; }
+    };
 
     if (tid == 0) { sm.pend[0].row0 = -1; sm.pend[1].row0 = -1; }
     __syncthreads();
+    factor_full(b0, a.j0, (int)min((int64_t)PW, cu1 - a.j0), cur);
+    grid.sync();
     for (int i = 0; i < nbp; ++i) {
         const int64_t b = b0 + i;
         const int64_t jp = a.j0 + (int64_t)i * PW;
         const int w = (int)min((int64_t)PW, cu1 - jp);
-        // ---- phase A
+        const int64_t cu0 = jp + w;                // first strip column right of panel i
+        const int wn = (int)min((int64_t)PW, cu1 - cu0);      // width of panel i+1 (<= 0: panel i is the last)
 #ifdef LINAC_TRACE
         if (threadIdx.x == 0 && blockIdx.x < 2) g_trace_on = (i == 1);
 #endif
         STRIP_STAMP(0);
-        strip_flush_u(sm, 0, A, ld);               // its readers all passed the last grid barrier
-        __syncthreads();
-        if (tid == 0) sm.pend[0].row0 = -1;
-        if (cta == 0) {
-            if (cur < a.rows) {
-                panel_factor(sm, A, ld, a.rows, cur, jp, w, a.rec + b, a.T + b * PW * PW, a.E + b * PW * PW, a.pivcols);
-                if (tid == 0) a.pstart[b + 1] = (int32_t)(cur + sm.r_out);
-            } else if (tid == 0) {                 // no rows left: the panel's columns are free
-                a.rec[b].r = 0; a.rec[b].nswaps = 0; a.rec[b].w = w;
-                a.pstart[b + 1] = (int32_t)cur;
-            }
-        }
-        if (owe && (cta > 0 || G == 1)) {
-            const int ncu = (int)(cu1 - pcu0);
-            const int nrest = (ncu + PW - 1) / PW - 1;             // column blocks 1.. (block 0 = panel i, done)
-            const int workers = G == 1 ? 1 : G - 1, job = G == 1 ? 0 : cta - 1;
-            if (nrest > 0) {
-                if (workers >= nrest) {
-                    const int nrw = workers / nrest, cb = 1 + job % nrest, rw = job / nrest;
-                    const int64_t cc0 = pcu0 + (int64_t)cb * PW;
-                    if (rw < nrw)
-                        strip_update(sm, 1, A, ld, a.rows, a.T + pb * PW * PW, ppcm, pjp, ppr0, pr, cc0,
-                                     (int)min((int64_t)PW, cu1 - cc0), rw, nrw);
-                } else {                                            // tiny grid: blocks in turn (flush between them)
-                    for (int cb = 1 + job; cb <= nrest; cb += workers) {
-                        const int64_t cc0 = pcu0 + (int64_t)cb * PW;
-                        strip_update(sm, 1, A, ld, a.rows, a.T + pb * PW * PW, ppcm, pjp, ppr0, pr, cc0,
-                                     (int)min((int64_t)PW, cu1 - cc0), 0, 1);
-                        // sole reader and writer of this block: the slice can go back at once
-                        strip_flush_u(sm, 1, A, ld);
-                        __syncthreads();
-                        if (tid == 0) sm.pend[1].row0 = -1;
-                        __syncthreads();
-                    }
-                }
-            }
-        }
-        owe = false;
-        STRIP_STAMP(6);
-        grid.sync();
-        STRIP_STAMP(7);
-        strip_flush_u(sm, 1, A, ld);
-        __syncthreads();
-        if (tid == 0) sm.pend[1].row0 = -1;
+        flush_all();
         // everything the updates need from the panel record, in ONE round trip to L2
         const PanelRec* rec = a.rec + b;
         const int r = rec->r, nsw = rec->nswaps, pcl = rec->pc[lane];
         const unsigned pcm = __reduce_or_sync(0xffffffffu, pcl >= 0 ? 1u << pcl : 0u);
-        if (r == 0) continue;
+        if (r == 0) {                              // free panel: nothing to apply, the next panel is factored as is
+            if (wn > 0) {
+                factor_full(b + 1, cu0, wn, cur);
+                grid.sync();
+            }
+            continue;
+        }
         // ---- row exchanges on complete rows, one thread per column (so the sequence of exchanges
         // needs no inter-thread ordering)
         if (nsw > 0) {
@@ -579,20 +571,57 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
         // reduced pivot rows' entries inside a rank-deficient panel (nobody reads these during the updates)
         if (r < w && cta == G - 1)
             if (wq < r && lane < w) A[(cur + wq) * ld + jp + lane] = a.E[b * PW * PW + wq * PW + lane];
-        const int64_t cu0 = jp + w;
-        if (cu0 < cu1) {
-            // ---- phase B: the next panel's columns, all CTAs as row workers
-            strip_update(sm, 0, A, ld, a.rows, a.T + b * PW * PW, pcm, jp, cur, r, cu0, (int)min((int64_t)PW, cu1 - cu0),
-                         cta, G);
-            owe = cu1 - cu0 > PW;
-            pb = b; pjp = jp; ppr0 = cur; pcu0 = cu0; pr = r; ppcm = pcm;
-            STRIP_STAMP(8);
-            grid.sync();
-            STRIP_STAMP(9);
+        if (wn <= 0) { cur += r; continue; }       // last panel of the strip: nothing to its right
+        const int ncu = (int)(cu1 - cu0);
+        const int ncb = (ncu + PW - 1) / PW;
+        const uint32_t* Tb = a.T + b * PW * PW;
+        // CTA 0 runs ahead on the next panel if its 32 candidate rows exist and the fast path can take them
+        const bool ahead = G >= 2 && G - 1 >= ncb && wn == PW && cur + r + PW <= a.rows && c_f.ninv != 0;
+        STRIP_STAMP(5);
+        if (G == 1 || G - 1 < ncb) {
+            // degenerate grids: the column blocks in turn (sole reader and writer: the slice goes back at once)
+            for (int cb = (G == 1 ? 0 : cta - 1); cb >= 0 && cb < ncb; cb += (G == 1 ? 1 : G - 1)) {
+                const int64_t cc0 = cu0 + (int64_t)cb * PW;
+                strip_update(sm, 1, A, ld, a.rows, Tb, pcm, jp, cur, r, cc0, (int)min((int64_t)PW, cu1 - cc0), 0, 1, 0, true);
+                strip_flush_u(sm, 1, A, ld);
+                __syncthreads();
+                if (tid == 0) sm.pend[1].row0 = -1;
+                __syncthreads();
+            }
+            if (cta == 0 && tid == 0) a.rec[b + 1].pad = 0;
+        } else if (cta == 0) {
+            if (ahead) {
+                strip_update_t<1>(sm, 0, A, ld, Tb, pcm, jp, cur, r, cu0, wn, cur + r, cur + r + PW, true);
+                STRIP_STAMP(1);
+                const bool got = panel_factor(sm, A, ld, a.rows, cur + r, cu0, wn, a.rec + b + 1, a.T + (b + 1) * PW * PW,
+                                              a.E + (b + 1) * PW * PW, a.pivcols, false);
+                if (tid == 0) {
+                    if (got) a.pstart[b + 2] = (int32_t)(cur + r + sm.r_out);
+                    a.rec[b + 1].pad = got ? 1 : 0;
+                }
+            } else if (tid == 0) {
+                a.rec[b + 1].pad = 0;
+            }
+        } else {
+            const int nrw = (G - 1) / ncb, job = cta - 1, cb = job % ncb, rw = job / ncb;
+            if (rw < nrw) {
+                const int64_t cc0 = cu0 + (int64_t)cb * PW;
+                const bool shared0 = cb == 0 && ahead;           // CTA 0 owns the candidate rows of block 0 and its U slice
+                strip_update(sm, 1, A, ld, a.rows, Tb, pcm, jp, cur, r, cc0, (int)min((int64_t)PW, cu1 - cc0), rw, nrw,
+                             shared0 ? PW : 0, rw == 0 && !shared0);
+            }
         }
+        STRIP_STAMP(6);
+        grid.sync();
+        STRIP_STAMP(7);
         cur += r;
+        // rec.pad is written ONLY between the barriers above (by CTA 0), never by the factorisation that may follow,
+        // so every CTA reads the same value however late it gets here
+        if (a.rec[b + 1].pad != 1) {
+            factor_full(b + 1, cu0, wn, cur);      // every row is up to date now (pending U slices are rows < cur)
+            grid.sync();
+        }
     }
-    // Panel nbp-1 is the strip's last: it has no columns to its right, so nothing is owed here.
     strip_flush_u(sm, 0, A, ld);
     strip_flush_u(sm, 1, A, ld);
 }
