@@ -70,12 +70,17 @@ struct StripSmem {
     int nsw;
     int fast_ok;
     int r_out;
+    int last_r, last_nsw;            // CTA 0's own copy of the record it wrote last (saves it a round trip to L2)
+    unsigned last_pcm;
     // ---- P2
     uint32_t Ts[PW][PW + 1];
     uint32_t Ar[PW][PW + 1];
     __align__(16) uint32_t Us[2][PW][PW];    // this CTA's U12 slices (slot 0: next panel's columns, slot 1: the rest)
     __align__(16) uint32_t Lk[PW][SRB + 4];  // L tile, k-major (pivot index, row)
     UPending pend[2];                // deferred write-back of Us[slot]
+    // ---- CTA 0 running ahead: T and the candidate rows' multipliers with 16-byte aligned rows
+    __align__(16) uint32_t Bt[PW][PW + 4];
+    __align__(16) uint32_t Bl[PW][PW + 4];
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -324,8 +329,11 @@ __device__ bool panel_factor(StripSmem& sm, const uint32_t* A, int64_t ld, int64
         panel_invert_general(sm, A, ld, j0, w, r, Tout, Eout);
     }
     if (tid < PW) {
-        rec->pc[tid] = tid < r ? sm.epc[sm.ord[tid]] : -1;
-        if (tid < r) pivcols_global[i0 + tid] = (int32_t)(j0 + sm.epc[sm.ord[tid]]);
+        const int pc = tid < r ? sm.epc[sm.ord[tid]] : -1;
+        rec->pc[tid] = pc;
+        if (tid < r) pivcols_global[i0 + tid] = (int32_t)(j0 + pc);
+        const unsigned pcm = __reduce_or_sync(0xffffffffu, pc >= 0 ? 1u << pc : 0u);
+        if (tid == 0) sm.last_pcm = pcm;
     }
     __syncthreads();
     if (tid == 0) {
@@ -333,6 +341,8 @@ __device__ bool panel_factor(StripSmem& sm, const uint32_t* A, int64_t ld, int64
         rec->w = w;
         rec->nswaps = sm.nsw;
         sm.r_out = r;
+        sm.last_r = r;
+        sm.last_nsw = sm.nsw;
     }
     STRIP_STAMP(4);
     return true;
@@ -469,6 +479,49 @@ __device__ __noinline__ void strip_update_t(StripSmem& sm, int slot, uint32_t* A
     if (slot == 0) STRIP_STAMP(13);
 }
 
+// CTA 0 running ahead of the others: U = T . A[pr0 : pr0+r, cc0 : cc0+32] (kept in Us[0], written back after the
+// next barrier) and the update of the 32 candidate rows c0row.. of the next panel, one output per thread
+// (warp = row, lane = column), the row operand read by LDS.128.  Latency matters here, not throughput: this
+// sits between two panel factorisations on the pivot-to-pivot chain.
+__device__ __noinline__ void strip_ahead_update(StripSmem& sm, uint32_t* A, int64_t ld, const uint32_t* Tb, unsigned pcm,
+                                                int64_t jp, int64_t pr0, int r, int64_t cc0, int64_t c0row) {
+    const ModP& f = c_f;
+    const int tid = threadIdx.x, lane = tid & 31, a = tid >> 5;
+    const int kcol = ((pcm >> lane) & 1u) ? __popc(pcm & ((1u << lane) - 1u)) : -1;
+    const uint32_t t = Tb[a * PW + lane];
+    const uint32_t ar = a < r ? A[(pr0 + a) * ld + cc0 + lane] : 0u;
+    const uint32_t l = A[(c0row + a) * ld + jp + lane];
+    uint32_t c = A[(c0row + a) * ld + cc0 + lane];
+    sm.Bt[a][lane] = t;                                   // zero beyond r (T is stored zero padded)
+    sm.Ar[a][lane] = ar;
+    if (kcol >= 0) sm.Bl[a][kcol] = l;
+    if (lane >= r) sm.Bl[a][lane] = 0u;                   // the r pivot indices fill 0..r-1
+    __syncthreads();
+    auto dot = [&](const uint32_t* row, const uint32_t (*col)[PW + 1]) {
+        uint64_t acc = 0;
+#pragma unroll
+        for (int k = 0; k < PW; k += 4) {
+            const uint4 v = *reinterpret_cast<const uint4*>(row + k);
+            acc += (uint64_t)v.x * col[k][lane];
+            acc += (uint64_t)v.y * col[k + 1][lane];
+            acc = fold64(acc, f);
+            acc += (uint64_t)v.z * col[k + 2][lane];
+            acc += (uint64_t)v.w * col[k + 3][lane];
+            acc = fold64(acc, f);
+        }
+        return reduce64(acc, f);
+    };
+    const uint32_t u = dot(sm.Bt[a], sm.Ar);
+    __syncthreads();                                      // every reader of Ar is done: Ar now carries U
+    sm.Ar[a][lane] = a < r ? u : 0u;
+    sm.Us[0][a][lane] = a < r ? u : 0u;
+    if (tid == 0) { UPending& p = sm.pend[0]; p.row0 = pr0; p.col0 = cc0; p.r = r; p.nc = PW; }
+    __syncthreads();
+    c = submod(c, dot(sm.Bl[a], sm.Ar), f);
+    A[(c0row + a) * ld + cc0 + lane] = c;
+    __syncthreads();                                      // the panel factorisation that follows reads these rows
+}
+
 // Row worker rw of nrw: its rows, then the variant whose tile matches them.
 __device__ __forceinline__ void strip_update(StripSmem& sm, int slot, uint32_t* A, int64_t ld, int64_t rows,
                                              const uint32_t* Tb, unsigned pcm, int64_t jp, int64_t pr0, int r,
@@ -517,6 +570,7 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
             if (tid == 0) a.pstart[bb + 1] = (int32_t)(row + sm.r_out);
         } else if (tid == 0) {                     // no rows left: the panel's columns are free
             a.rec[bb].r = 0; a.rec[bb].nswaps = 0; a.rec[bb].w = ww;
+            sm.last_r = 0; sm.last_nsw = 0; sm.last_pcm = 0;
             a.pstart[bb + 1] = (int32_t)row;
         }
     };
@@ -544,8 +598,15 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
         flush_all();
         // everything the updates need from the panel record, in ONE round trip to L2
         const PanelRec* rec = a.rec + b;
-        const int r = rec->r, nsw = rec->nswaps, pcl = rec->pc[lane];
-        const unsigned pcm = __reduce_or_sync(0xffffffffu, pcl >= 0 ? 1u << pcl : 0u);
+        int r, nsw;
+        unsigned pcm;
+        if (cta == 0) {                            // CTA 0 wrote the record itself
+            r = sm.last_r; nsw = sm.last_nsw; pcm = sm.last_pcm;
+        } else {
+            const int pcl = rec->pc[lane];
+            r = rec->r; nsw = rec->nswaps;
+            pcm = __reduce_or_sync(0xffffffffu, pcl >= 0 ? 1u << pcl : 0u);
+        }
         if (r == 0) {                              // free panel: nothing to apply, the next panel is factored as is
             if (wn > 0) {
                 factor_full(b + 1, cu0, wn, cur);
@@ -591,7 +652,7 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
             if (cta == 0 && tid == 0) a.rec[b + 1].pad = 0;
         } else if (cta == 0) {
             if (ahead) {
-                strip_update_t<1>(sm, 0, A, ld, Tb, pcm, jp, cur, r, cu0, wn, cur + r, cur + r + PW, true);
+                strip_ahead_update(sm, A, ld, Tb, pcm, jp, cur, r, cu0, cur + r);
                 STRIP_STAMP(1);
                 const bool got = panel_factor(sm, A, ld, a.rows, cur + r, cu0, wn, a.rec + b + 1, a.T + (b + 1) * PW * PW,
                                               a.E + (b + 1) * PW * PW, a.pivcols, false);
