@@ -150,3 +150,27 @@ def test_nullspace_matches_oracle(oracle, m, r, n):
             L.nullspace_u32(buf3, P29, small)
         assert e.value.status == L.linac.ERR_BUFFER_TOO_SMALL
         assert np.array_equal(from_device(buf3), r_ref)      # documented: dA already holds the RREF
+
+
+# ------------------------------------------------------------------ schedule variants
+@pytest.mark.parametrize("opts", [
+    {"strip_width": 32}, {"strip_width": 64}, {"strip_width": 256}, {"strip_width": 96, "flat_group": 2},
+    {"flat_cols": 0}, {"flat_cols": 256, "flat_group": 4}, {"tc_panel": 0}, {"gemm_path": 1},
+    {"tc_min_k": 32, "tc_min_mn": 128, "strip_width": 32},
+])
+def test_schedule_options_do_not_change_the_result(oracle, opts):
+    """Every tunable only changes the schedule (strip width, flat sweep vs recursion, which GEMM kernel): the RREF
+    is unique, so the bytes must not move.  One rank-deficient and one full-rank wide matrix."""
+    import paper_2605_25863_b200 as L
+    defaults = {"strip_width": 128, "flat_group": 1, "flat_cols": 16384, "tc_panel": 1, "gemm_path": 0,
+                "tc_min_k": 128, "tc_min_mn": 128}
+    a1, _, _ = gen.lowrank_factors(700, 333, 900, P29, seed_b=21, seed_c=22)
+    a2 = gen.uniform_matrix(600, 1100, P31, seed=23)
+    try:
+        for k, v in opts.items():
+            L.set_option(k, v)
+        check_against_oracle(oracle, a1, P29)
+        check_against_oracle(oracle, a2, P31)
+    finally:
+        for k, v in defaults.items():
+            L.set_option(k, v)
