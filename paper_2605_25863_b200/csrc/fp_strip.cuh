@@ -1,19 +1,19 @@
-// fp_strip.cuh -- S1-S4 of the F_p path for one STRIP of up to 8 base panels: a cooperative kernel.
+// fp_strip.cuh -- S1-S4 of the F_p path for one STRIP of up to 8 base panels: a cooperative kernel, and the
+// column-parallel triangular-solve leaf that follows it.
 //
-// One launch factors columns [j0, j0+ws) (ws <= SW_MAX) over the active rows >= i0, base panel by
-// base panel (PW = 32 columns each), with the whole grid resident (one CTA of 1024 threads per SM):
+// One launch factors columns [j0, j0+ws) (ws <= SW_MAX) over the active rows >= i0, base panel by base panel
+// (PW = 32 columns each), with the whole grid resident (one CTA of 1024 threads per SM).  Per base panel, between
+// two grid barriers (strip_factor_kernel below has the details):
 //
-//   P1  (CTA 0)      pivot search + T = (pivot block)^-1 for the panel         (S1, S2)
-//       grid.sync
-//   P1b (all CTAs)   row exchanges on complete rows, only if the panel needs any (K5)
-//       grid.sync
-//   P2  (all CTAs)   U12 = T.A12 on the pivot rows and A22 -= L21.U12 on the rows below, restricted
-//                    to the strip's columns right of the panel                  (S3/S4 inside the strip)
-//       grid.sync
+//   CTA 0        ahead update of the next panel's 32 candidate rows, then pivot search + T = (pivot block)^-1
+//                of the NEXT panel from them                                       (S1, S2)
+//   CTAs 1..     U12 = T.A12 on the pivot rows and A22 -= L21.U12 on the rows below, restricted to the
+//                strip's columns right of the panel                               (S3/S4 inside the strip)
+//   (if needed)  row exchanges on complete rows (K5); general-path factorisation by CTA 0
 //
-// so the ~10 dependent launches and the host round trip per base panel of the earlier schedule
-// become two or three grid barriers.  Everything right of the strip is updated afterwards by the
-// row-block solve (trsm_strip_kernel) and the tensor-core Schur update.
+// so the ~10 dependent launches and the host round trip per base panel of a launch-per-step schedule become one
+// grid barrier.  Everything right of the strip is updated afterwards by the row-block solve (trsm_strip_kernel)
+// and the tensor-core Schur update.
 //
 // Storage convention: see fp_kernels.cuh (multipliers are the raw entries at the pivot columns).
 #pragma once
