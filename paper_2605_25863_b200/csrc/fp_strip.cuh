@@ -766,18 +766,25 @@ __global__ void __launch_bounds__(TNT) trsm_strip_kernel(const uint32_t* __restr
         nxt = ii + 1;
         prefetch();
         if (LOWER) {
-            uint32_t y[PW / NW];
-#pragma unroll
-            for (int u = 0; u < PW / NW; ++u) {
-                const int a = wq + NW * u;
-                uint64_t acc = 0;
+            // two outputs per thread (rows wq and wq + 16 of T) share the X loads
+            static_assert(PW / NW == 2, "the T product below is written for two rows per warp");
+            uint32_t y[2];
+            {
+                uint64_t a0 = 0, a1 = 0;
+                const uint32_t* t0r = Ts[wq];
+                const uint32_t* t1r = Ts[wq + NW];
                 for (int k = 0; k + 1 < r; k += 2) {
-                    acc += (uint64_t)Ts[a][k] * Xs[s + k][lane];
-                    acc += (uint64_t)Ts[a][k + 1] * Xs[s + k + 1][lane];
-                    acc = fold64(acc, f);
+                    const uint32_t x0 = Xs[s + k][lane], x1 = Xs[s + k + 1][lane];
+                    a0 = fold64(a0 + (uint64_t)t0r[k] * x0 + (uint64_t)t0r[k + 1] * x1, f);
+                    a1 = fold64(a1 + (uint64_t)t1r[k] * x0 + (uint64_t)t1r[k + 1] * x1, f);
                 }
-                if (r & 1) acc = fold64(acc + (uint64_t)Ts[a][r - 1] * Xs[s + r - 1][lane], f);
-                y[u] = reduce64(acc, f);
+                if (r & 1) {
+                    const uint32_t x0 = Xs[s + r - 1][lane];
+                    a0 = fold64(a0 + (uint64_t)t0r[r - 1] * x0, f);
+                    a1 = fold64(a1 + (uint64_t)t1r[r - 1] * x0, f);
+                }
+                y[0] = reduce64(a0, f);
+                y[1] = reduce64(a1, f);
             }
             __syncthreads();
 #pragma unroll
@@ -785,20 +792,29 @@ __global__ void __launch_bounds__(TNT) trsm_strip_kernel(const uint32_t* __restr
                 if (wq + NW * u < r) Xs[s + wq + NW * u][lane] = y[u];
             __syncthreads();
         }
-        for (int row = wq; row < nrow; row += NW) {
-            uint64_t acc = 0;
+        // rows in pairs (row, row + 16) sharing the X loads; L by LDS.128 along k
+        for (int row = wq; row < nrow; row += 2 * NW) {
+            const bool two = row + NW < nrow;
+            const uint32_t* l0 = Lp[row];
+            const uint32_t* l1 = Lp[two ? row + NW : row];
+            uint64_t a0 = 0, a1 = 0;
             int k = 0;
             for (; k + 3 < r; k += 4) {
-                const uint4 l4 = *reinterpret_cast<const uint4*>(&Lp[row][k]);
-                acc += (uint64_t)l4.x * Xs[s + k][lane];
-                acc += (uint64_t)l4.y * Xs[s + k + 1][lane];
-                acc = fold64(acc, f);
-                acc += (uint64_t)l4.z * Xs[s + k + 2][lane];
-                acc += (uint64_t)l4.w * Xs[s + k + 3][lane];
-                acc = fold64(acc, f);
+                const uint4 p = *reinterpret_cast<const uint4*>(l0 + k);
+                const uint4 q = *reinterpret_cast<const uint4*>(l1 + k);
+                const uint32_t x0 = Xs[s + k][lane], x1 = Xs[s + k + 1][lane], x2 = Xs[s + k + 2][lane], x3 = Xs[s + k + 3][lane];
+                a0 = fold64(a0 + (uint64_t)p.x * x0 + (uint64_t)p.y * x1, f);
+                a1 = fold64(a1 + (uint64_t)q.x * x0 + (uint64_t)q.y * x1, f);
+                a0 = fold64(a0 + (uint64_t)p.z * x2 + (uint64_t)p.w * x3, f);
+                a1 = fold64(a1 + (uint64_t)q.z * x2 + (uint64_t)q.w * x3, f);
             }
-            for (; k < r; ++k) acc = fold64(acc + (uint64_t)Lp[row][k] * Xs[s + k][lane], f);
-            Xs[lo + row][lane] = submod(Xs[lo + row][lane], reduce64(acc, f), f);
+            for (; k < r; ++k) {
+                const uint32_t x0 = Xs[s + k][lane];
+                a0 = fold64(a0 + (uint64_t)l0[k] * x0, f);
+                a1 = fold64(a1 + (uint64_t)l1[k] * x0, f);
+            }
+            Xs[lo + row][lane] = submod(Xs[lo + row][lane], reduce64(a0, f), f);
+            if (two) Xs[lo + row + NW][lane] = submod(Xs[lo + row + NW][lane], reduce64(a1, f), f);
         }
         __syncthreads();
     }
