@@ -99,7 +99,7 @@ int trsm_leaf(Fp& c, int64_t s, uint32_t* X, int64_t ldx, int64_t ncols) {
     if (!LOWER && c.sb0(s + 1) - c.sb0(s) <= 1) return LINAC_OK;     // U is the identity inside one base panel
     Timed tm(c, stats().ms_trsm);
     trsm_strip_kernel<LOWER><<<(unsigned)((ncols + PW - 1) / PW), TNT, trsm_smem_bytes(K), c.s>>>(
-        c.A, c.ld, X, ldx, ncols, c.d_pstart, (int)c.sb0(s), (int)c.sb0(s + 1), c.d_T, c.d_pivcols, c.f);
+        c.A, c.ld, X, ldx, ncols, c.d_pstart, (int)c.sb0(s), (int)c.sb0(s + 1), c.d_T, c.d_pivcols, c.f, nullptr, 0);
     LINAC_CUDA(cudaGetLastError());
     stats().kernel_launches++;
     stats().update_macs += K * K / 2 * ncols;
@@ -128,7 +128,8 @@ int trsm_lower(Fp& c, int64_t s0, int64_t s1, int64_t c0, int64_t c1) {
 // If early_ncols > 0 the strip's row-block solve on columns [early_c0, early_c0 + early_ncols) is enqueued right
 // behind the strip kernel (it takes the pivot counts from device memory), and the host reads the pivot counts
 // through a second stream meanwhile: the round trip then hides under the solve instead of idling the GPU.
-int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r, int64_t early_c0 = 0, int64_t early_ncols = 0) {
+int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r, int64_t early_c0 = 0, int64_t early_ncols = 0,
+                 uint8_t* early_Bq = nullptr, int early_kp = 0) {
     const int64_t b0 = c.sb0(s), b1 = c.sb0(s + 1);
     const int64_t j0 = panel_col0(b0), j1 = std::min(c.cols, panel_col0(b1));
     StripArgs a;
@@ -144,7 +145,8 @@ int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r, int64_t early_c0 = 0,
     if (early_ncols > 0 && options().timing == 0) {
         LINAC_CUDA(cudaEventRecord(c.ev_strip, c.s));
         trsm_strip_kernel<true><<<(unsigned)((early_ncols + PW - 1) / PW), TNT, trsm_smem_bytes(j1 - j0), c.s>>>(
-            c.A, c.ld, c.A + i0 * c.ld + early_c0, c.ld, early_ncols, c.d_pstart, (int)b0, (int)b1, c.d_T, c.d_pivcols, c.f);
+            c.A, c.ld, c.A + i0 * c.ld + early_c0, c.ld, early_ncols, c.d_pstart, (int)b0, (int)b1, c.d_T, c.d_pivcols, c.f,
+            early_Bq, early_kp);
         LINAC_CUDA(cudaGetLastError());
         st.kernel_launches++;
         LINAC_CUDA(cudaStreamWaitEvent(c.copy_s, c.ev_strip, 0));
@@ -209,8 +211,18 @@ int factor(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t* r_out, bool allow
             const int64_t jc = std::min(c.cols, panel_col0(c.sb0(se)));
             int rc;
             bool solved = false;
+            // the row-block solve can hand U12 to the Schur update as u8 limb planes (saves the update's own split)
+            const size_t mark = c.arena->off;
+            uint8_t* Bq = nullptr;
+            int kp_b = 0;
             if (se - s == 1 && cur < c.rows) {
-                rc = factor_strip(c, s, cur, &r, jc, jend - jc);
+                const int64_t ws = jc - panel_col0(c.sb0(s));
+                const Options& o = options();
+                if (o.gemm_path != 1 && o.tc_panel != 0 && ws <= 256 && jend - jc >= o.tc_min_mn && ws >= o.tc_min_k) {
+                    kp_b = (int)((ws + 127) / 128 * 128);
+                    Bq = (uint8_t*)c.arena->take((size_t)4 * (jend - jc) * kp_b, 1024);
+                }
+                rc = factor_strip(c, s, cur, &r, jc, jend - jc, Bq, kp_b);
                 solved = rc == LINAC_EARLY_SOLVE_DONE;
                 if (solved) rc = LINAC_OK;
             } else {
@@ -224,10 +236,12 @@ int factor(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t* r_out, bool allow
                 if (m2 > 0) {
                     GemmArgs g{c.A + (cur + r) * c.ld + jc, c.ld, c.A + (cur + r) * c.ld, c.ld, c.d_pivcols + cur,
                                c.A + cur * c.ld + jc,       c.ld, m2,                      jend - jc, r};
+                    if (solved && Bq) { g.Bq_ready = Bq; g.kp_ready = kp_b; }
                     rc = run_gemm(c, g);
                     if (rc) return rc;
                 }
             }
+            c.arena->off = mark;
             cur += r;
             *r_out = cur - i0;
         }

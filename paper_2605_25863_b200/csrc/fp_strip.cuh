@@ -710,7 +710,8 @@ __global__ void __launch_bounds__(TNT) trsm_strip_kernel(const uint32_t* __restr
                                                          uint32_t* __restrict__ X, int64_t ldx, int64_t ncols,
                                                          const int32_t* __restrict__ pstart, int bs0, int bs1,
                                                          const uint32_t* __restrict__ T,
-                                                         const int32_t* __restrict__ pivcols, ModP f) {
+                                                         const int32_t* __restrict__ pivcols, ModP f,
+                                                         uint8_t* __restrict__ Bq, int kp) {
     extern __shared__ __align__(16) unsigned char trsm_smem_raw[];
     const int t0 = pstart[bs0], K = pstart[bs1] - t0;
     uint32_t (*Xs)[PW] = reinterpret_cast<uint32_t (*)[PW]>(trsm_smem_raw);                                 // [K][32]
@@ -820,6 +821,27 @@ __global__ void __launch_bounds__(TNT) trsm_strip_kernel(const uint32_t* __restr
     }
     if (cok)
         for (int t = wq; t < K; t += NW) X[(int64_t)t * ldx + c] = Xs[t][lane];
+    // Optionally hand the result to the Schur update already split into its four u8 limb planes
+    // (Bq[limb][column][kp], k-major, zero padded to kp): saves the update its own pass over U12.
+    if (Bq != nullptr && cok) {
+        const int64_t plane = ncols * (int64_t)kp;
+        for (int job = wq; job < 4 * (kp / 16); job += NW) {          // (limb, 16 consecutive k) per warp, lane = column
+            const int l = job / (kp / 16), k0 = (job % (kp / 16)) * 16;
+            uint32_t w[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                uint32_t packed = 0;
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int k = k0 + 4 * q + e;
+                    const uint32_t v = k < K ? Xs[k][lane] : 0u;
+                    packed |= ((v >> (8 * l)) & 0xFFu) << (8 * e);
+                }
+                w[q] = packed;
+            }
+            *reinterpret_cast<uint4*>(Bq + (int64_t)l * plane + c * kp + k0) = make_uint4(w[0], w[1], w[2], w[3]);
+        }
+    }
 }
 
 }  // namespace linac

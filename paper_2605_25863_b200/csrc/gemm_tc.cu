@@ -585,19 +585,21 @@ int gemm_modp_tc(const GemmArgs& g, const ModP& f, cudaStream_t s, Arena* scratc
             }
             pattr = true;
         }
-        const int64_t kp = (g.K + KB - 1) / KB * KB;
+        const bool b_ready = g.Bq_ready != nullptr && g.kp_ready >= g.K && g.kp_ready <= 2 * KB && g.kp_ready % KB == 0;
+        const int64_t kp = b_ready ? g.kp_ready : (g.K + KB - 1) / KB * KB;
         uint8_t* Aq = (uint8_t*)scratch->take((size_t)4 * g.M * kp, 1024);
-        uint8_t* Bq = (uint8_t*)scratch->take((size_t)4 * g.N * kp, 1024);
+        uint8_t* Bq = b_ready ? g.Bq_ready : (uint8_t*)scratch->take((size_t)4 * g.N * kp, 1024);
         if (!Aq || !Bq) return -1;
         {
             dim3 grid((unsigned)((kp / 4 + 127) / 128), (unsigned)std::min<int64_t>(g.M, 16384));
             split_a_kernel<<<grid, 128, 0, s>>>(g.Abase, g.lda, g.kcols, 0, g.M, g.K, kp, Aq);
             LINAC_CUDA(cudaGetLastError());
         }
-        {
+        if (!b_ready) {
             dim3 grid((unsigned)(kp / 128), (unsigned)((g.N + 31) / 32));
             split_b_kernel<<<grid, 256, 0, s>>>(g.B, g.ldb, g.K, g.N, kp, Bq);
             LINAC_CUDA(cudaGetLastError());
+            stats().kernel_launches++;
         }
         CUtensorMap tmA, tmB, tmC;
         if (!make_limb_map(&tmA, Aq, g.M, kp, TM) || !make_limb_map(&tmB, Bq, g.N, kp, PN) || !make_c_map(&tmC, g.C, g.ldc, g.M, g.N))
@@ -609,7 +611,7 @@ int gemm_modp_tc(const GemmArgs& g, const ModP& f, cudaStream_t s, Arena* scratc
         else
             gemm_tc_panel_kernel<false><<<(unsigned)std::min(grid, sc.nitems), P_THREADS, P_SMEM, s>>>(tmA, tmB, tmC, (int)(kp / KB), sc, f);
         LINAC_CUDA(cudaGetLastError());
-        stats().kernel_launches += 3;
+        stats().kernel_launches += 2;
         stats().tc_launches++;
         stats().update_macs += g.M * g.N * g.K;
         return LINAC_OK;

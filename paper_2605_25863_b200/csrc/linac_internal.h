@@ -73,6 +73,11 @@ struct GemmArgs {
     const uint32_t* Abase; int64_t lda; const int32_t* kcols;
     const uint32_t* B; int64_t ldb;
     int64_t M, N, K;
+    // Optional: the u8 limb planes of B already written by the producer of B (Bq[limb][n][kp_ready], k-major, zero
+    // padded to kp_ready, a multiple of 128): the tensor path then skips its own split of B.  Only honoured by the
+    // K <= 256 panel kernel; anything else ignores it and splits B itself.
+    uint8_t* Bq_ready = nullptr;
+    int64_t kp_ready = 0;
 };
 int gemm_modp_simt(const GemmArgs& g, const ModP& f, cudaStream_t s);
 // Tensor-core (tcgen05 int8 limb) path; returns LINAC_OK if it ran, or a negative value if the
