@@ -6,7 +6,7 @@
 //         resident in shared memory, one grid-wide sync per column: warp-shuffle arg-max inside
 //         each CTA, candidates exchanged through global memory)
 //       * row exchanges applied to whole rows of A and B (CudaSwitchRows)
-//       * row-block solves and trailing updates A22 -= L21.U12 as DGEMMs, organised recursively
+//       * row-block solves and trailing updates A22 -= L21.U12 as DGEMMs (DMMA m8n8k4), organised recursively
 //     B rides along as extra trailing columns, which performs the forward substitution
 //     (the paper reduces the augmented matrix (A b)).
 // F3  back substitution with U on the right-hand sides (blocked, GEMM for the off-diagonal part).
@@ -304,6 +304,99 @@ __global__ void __launch_bounds__(DTHREADS) dgemm_sub_kernel(double* __restrict_
     }
 }
 
+// The same update on the FP64 tensor pipe (DMMA m8n8k4, the only FP64 MMA shape sm_100 has): 128 x 128 tile, 8 warps
+// as 2 x 4, a 64 x 32 warp tile = 8 x 4 MMA tiles.  Operands come from shared memory one double per thread and
+// per fragment, so a k-step costs 12 LDS.64 per 32 MMAs: five times less shared-memory traffic per flop than the
+// 8 x 8 register tile of the DFMA kernel above, which was co-bound by the shared-memory pipe.
+constexpr int QK = 8;                     // k per shared-memory stage
+constexpr int QLD = DM + 4;               // row stride in doubles: = 4 mod 16, conflict-free fragment loads
+__device__ __forceinline__ void dmma_8x8x4(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+__global__ void __launch_bounds__(256) dgemm_sub_mma_kernel(double* __restrict__ C, int64_t ldc,
+                                                            const double* __restrict__ A, int64_t lda,
+                                                            const double* __restrict__ B, int64_t ldb, int64_t M,
+                                                            int64_t N, int64_t K) {
+    __shared__ __align__(16) double As[2][QK][QLD];       // k-major
+    __shared__ __align__(16) double Bs[2][QK][QLD];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wm0 = (warp >> 2) * 64, wn0 = (warp & 3) * 32;
+    const int g = lane >> 2, q = lane & 3;                // fragment coordinates (PTX ISA, m8n8k4 .f64)
+    const int64_t m0 = (int64_t)blockIdx.y * DM, n0 = (int64_t)blockIdx.x * DN;
+    double acc[8][4][2];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    double ra[4], rb[4];
+    auto gload = [&](int64_t k0) {
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+            const int idx = tid + t * 256;
+            const int kk = idx % QK, mm = idx / QK;
+            const int64_t m = m0 + mm, k = k0 + kk;
+            ra[t] = (m < M && k < K) ? A[m * lda + k] : 0.0;
+            const int nn = idx % DN, kb = idx / DN;
+            const int64_t n = n0 + nn, k2 = k0 + kb;
+            rb[t] = (n < N && k2 < K) ? B[k2 * ldb + n] : 0.0;
+        }
+    };
+    auto sstore = [&](int buf) {
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+            const int idx = tid + t * 256;
+            As[buf][idx % QK][idx / QK] = ra[t];
+            Bs[buf][idx / DN][idx % DN] = rb[t];
+        }
+    };
+    gload(0);
+    sstore(0);
+    __syncthreads();
+    int buf = 0;
+    for (int64_t k0 = 0; k0 < K; k0 += QK) {
+        const bool more = k0 + QK < K;
+        if (more) gload(k0 + QK);
+#pragma unroll
+        for (int ks = 0; ks < QK; ks += 4) {
+            double a[8], b[4];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) a[i] = As[buf][ks + q][wm0 + i * 8 + g];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) b[j] = Bs[buf][ks + q][wn0 + j * 8 + g];
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) dmma_8x8x4(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
+        if (more) {
+            sstore(buf ^ 1);
+            __syncthreads();
+            buf ^= 1;
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const int64_t m = m0 + wm0 + i * 8 + g;
+        if (m >= M) continue;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int64_t n = n0 + wn0 + j * 8 + q * 2;
+            double* pc = C + m * ldc + n;
+            if (n + 1 < N && ((reinterpret_cast<uintptr_t>(pc) & 15) == 0)) {
+                double2 v = *reinterpret_cast<double2*>(pc);
+                v.x -= acc[i][j][0];
+                v.y -= acc[i][j][1];
+                *reinterpret_cast<double2*>(pc) = v;
+            } else {
+                if (n < N) pc[0] -= acc[i][j][0];
+                if (n + 1 < N) pc[1] -= acc[i][j][1];
+            }
+        }
+    }
+}
+
 struct F64 {
     double* A; int64_t n, lda;
     double* B; int64_t nrhs, ldb;
@@ -318,7 +411,10 @@ int dgemm_sub(F64& c, double* C, int64_t ldc, const double* A, int64_t lda, cons
               int64_t N, int64_t K) {
     if (M <= 0 || N <= 0 || K <= 0) return LINAC_OK;
     dim3 grid((unsigned)((N + DN - 1) / DN), (unsigned)((M + DM - 1) / DM));
-    dgemm_sub_kernel<<<grid, DTHREADS, 0, c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
+    if (options().f64_mma != 0)
+        dgemm_sub_mma_kernel<<<grid, 256, 0, c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
+    else
+        dgemm_sub_kernel<<<grid, DTHREADS, 0, c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
     LINAC_CUDA(cudaGetLastError());
     stats().kernel_launches++;
     stats().update_macs += M * N * K;

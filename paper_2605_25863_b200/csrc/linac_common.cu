@@ -172,6 +172,9 @@ int linac_set_option(const char* name, int64_t value) {
     } else if (!strcmp(name, "tc_min_mn")) {
         if (value < 128) return LINAC_ERR_INVALID_ARG;
         g_options.tc_min_mn = value;
+    } else if (!strcmp(name, "f64_mma")) {
+        if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
+        g_options.f64_mma = value;
     } else if (!strcmp(name, "tc_panel")) {
         if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
         g_options.tc_panel = value;
