@@ -10,6 +10,8 @@
 // many pivots it produced; that is the only host involvement (the paper's loop has none, at
 // the price of 8 launches per COLUMN).
 #include <algorithm>
+#include <atomic>
+#include <cstring>
 #include <mutex>
 #include <vector>
 
@@ -38,7 +40,7 @@ struct Fp {
     uint32_t* d_E;            // [nb][PW*PW]
     Arena* arena;
     // host
-    PanelRec* h_rec;          // pinned, MAXBP records
+    unsigned long long* h_mail;      // mapped pinned, MAXBP * MAIL_WORDS tagged words written by the strip kernel itself
     std::vector<int64_t> pstart;     // [nb+1] pivots found left of base panel b
     std::vector<int32_t> pivcols;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev_strip = nullptr;
@@ -135,6 +137,9 @@ int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r, int64_t early_c0 = 0,
     StripArgs a;
     a.A = c.A; a.ld = c.ld; a.rows = c.rows; a.cols = c.cols; a.i0 = i0; a.j0 = j0; a.ws = (int)(j1 - j0);
     a.rec = c.d_rec; a.T = c.d_T; a.E = c.d_E; a.pivcols = c.d_pivcols; a.pstart = c.d_pstart;
+    static unsigned long long seq_counter = 0;
+    a.host_mail = c.h_mail; a.seq = (++seq_counter) & 0xFFFFFFFFull;
+    if (a.seq == 0) a.seq = ++seq_counter & 0xFFFFFFFFull;      // 0 is the mailbox's initial content
     void* args[] = {&a};
     {
         Timed tm(c, stats().ms_strip);
@@ -149,13 +154,26 @@ int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r, int64_t early_c0 = 0,
             early_Bq, early_kp);
         LINAC_CUDA(cudaGetLastError());
         st.kernel_launches++;
-        LINAC_CUDA(cudaStreamWaitEvent(c.copy_s, c.ev_strip, 0));
-        LINAC_CUDA(cudaMemcpyAsync(c.h_rec, c.d_rec + b0, (size_t)(b1 - b0) * sizeof(PanelRec), cudaMemcpyDeviceToHost, c.copy_s));
-        LINAC_CUDA(cudaStreamSynchronize(c.copy_s));
     } else {
         early_ncols = 0;
-        LINAC_CUDA(cudaMemcpyAsync(c.h_rec, c.d_rec + b0, (size_t)(b1 - b0) * sizeof(PanelRec), cudaMemcpyDeviceToHost, c.s));
-        LINAC_CUDA(cudaStreamSynchronize(c.s));
+    }
+    // Wait for the strip kernel's mail (it may arrive before the kernel, let alone the solve behind it, has ended).
+    {
+        volatile unsigned long long* mailbox = c.h_mail;
+        const int nw = (int)(b1 - b0) * MAIL_WORDS;
+        int seen = 0;                                     // words [0, seen) already carry this launch's tag
+        for (uint64_t spins = 0; seen < nw; ++spins) {
+            while (seen < nw && (mailbox[seen] >> 32) == a.seq) ++seen;
+            if (seen < nw && (spins & 0x3FFF) == 0x3FFF) {
+                const cudaError_t q = cudaStreamQuery(c.s);
+                if (q != cudaSuccess && q != cudaErrorNotReady) { set_cuda_error(q, "strip kernel", __FILE__, __LINE__); return LINAC_ERR_CUDA; }
+                if (q == cudaSuccess) {                   // stream drained: the mail must be complete by now
+                    while (seen < nw && (mailbox[seen] >> 32) == a.seq) ++seen;
+                    if (seen < nw) return LINAC_ERR_INTERNAL;
+                }
+            }
+        }
+        std::atomic_thread_fence(std::memory_order_acquire);
     }
     st.kernel_launches++;
     st.host_syncs++;
@@ -172,12 +190,13 @@ int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r, int64_t early_c0 = 0,
 #endif
     int64_t cur = i0;
     for (int64_t b = b0; b < b1; ++b) {
-        const PanelRec& h = c.h_rec[b - b0];
-        if (h.r < 0 || h.r > PW || cur + h.r > c.rows) return LINAC_ERR_INTERNAL;
+        const unsigned long long* m = c.h_mail + (b - b0) * MAIL_WORDS;
+        const int32_t hr = (int32_t)(uint32_t)m[0], hns = (int32_t)(uint32_t)m[1];
+        if (hr < 0 || hr > PW || cur + hr > c.rows) return LINAC_ERR_INTERNAL;
         st.panels++;
-        st.row_swaps += h.r > 0 ? h.nswaps : 0;
-        for (int q = 0; q < h.r; ++q) c.pivcols[cur + q] = (int32_t)(panel_col0(b) + h.pc[q]);
-        cur += h.r;
+        st.row_swaps += hr > 0 ? hns : 0;
+        for (int q = 0; q < hr; ++q) c.pivcols[cur + q] = (int32_t)(panel_col0(b) + (int32_t)(uint32_t)m[2 + q]);
+        cur += hr;
         c.pstart[b + 1] = cur;
     }
     *r = cur - i0;
@@ -327,7 +346,7 @@ size_t workspace_bytes(int64_t rows, int64_t cols) {
 }
 
 struct PinnedRec {
-    PanelRec* p = nullptr;
+    unsigned long long* p = nullptr;
     ~PinnedRec() { if (p) cudaFreeHost(p); }
 };
 
@@ -354,7 +373,10 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     if (rc) return rc;
 
     static PinnedRec pinned;
-    if (!pinned.p) LINAC_CUDA(cudaMallocHost(&pinned.p, MAXBP * sizeof(PanelRec)));
+    if (!pinned.p) {
+        LINAC_CUDA(cudaHostAlloc(&pinned.p, MAXBP * MAIL_WORDS * sizeof(unsigned long long), cudaHostAllocMapped));
+        memset(pinned.p, 0, MAXBP * MAIL_WORDS * sizeof(unsigned long long));
+    }
 
     Fp c;
     c.A = dA; c.rows = rows; c.cols = cols; c.ld = ld; c.f = make_modp(p); c.s = s; c.arena = arena;
@@ -372,7 +394,7 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     c.d_pstart = (int32_t*)arena->take((size_t)(c.nb + 1) * 4);
     if (!c.d_rec || !c.d_T || !c.d_E || !c.d_pivcols || !d_colinfo || !c.d_pstart) return LINAC_ERR_WORKSPACE;
     LINAC_CUDA(cudaMemsetAsync(c.d_pstart, 0, (size_t)(c.nb + 1) * 4, s));
-    c.h_rec = pinned.p;
+    c.h_mail = pinned.p;
     c.pivcols.assign(mn, -1);
     c.pstart.assign(c.nb + 1, 0);
     LINAC_CUDA(cudaEventCreate(&c.ev0));

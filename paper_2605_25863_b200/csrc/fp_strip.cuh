@@ -44,6 +44,7 @@ constexpr int SW_MAX = 256;                 // widest strip (columns)
 constexpr int SNT = 1024;                   // threads per CTA of the strip kernel (32 warps)
 constexpr int SRB = 256;                    // rows of one P2 tile
 constexpr int MAXBP = SW_MAX / PW;          // base panels per strip
+constexpr int MAIL_WORDS = 2 + PW;          // per panel: r, nswaps, pc[32]
 
 // d*x - h*y mod p with one reduction: d*x + (p-h)*y < 2^63.
 __device__ __forceinline__ uint32_t lincomb(uint32_t d, uint32_t x, uint32_t h, uint32_t y, const ModP& f) {
@@ -362,6 +363,8 @@ struct StripArgs {
     uint32_t* E;             // [nb][PW*PW]
     int32_t* pivcols;        // [min(rows, cols)]
     int32_t* pstart;         // [nb+1]
+    unsigned long long* host_mail;  // mapped pinned host memory: MAXBP * MAIL_WORDS tagged words, written by CTA 0
+    unsigned long long seq;         // tag of this launch (32 significant bits)
 };
 
 // Deferred write-back of a U12 slice: the raw entries it replaces are read by every row worker of
@@ -562,6 +565,24 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
     const int64_t cu1 = a.j0 + a.ws;               // end of the strip
     int64_t cur = a.i0;
 
+    // CTA 0, once it has written the record of the strip's LAST panel: mail what the host needs of all records
+    // (r, nswaps, pc[32] per panel) through mapped memory -- posted PCIe writes, no copy engine, so a large
+    // transfer the caller has in flight cannot delay the host's next launches.  Every 64-bit word carries the
+    // launch's sequence number in its upper half, so no system-wide fence (a PCIe round trip) is needed: the host
+    // waits until every word shows the tag.  Sent as early as possible: the host only needs it to enqueue what follows.
+    auto mail = [&]() {
+        if (a.host_mail == nullptr) return;
+        __syncthreads();
+        volatile unsigned long long* dst = a.host_mail;
+        for (int e = tid; e < nbp * MAIL_WORDS; e += SNT) {
+            const PanelRec* rc = a.rec + b0 + e / MAIL_WORDS;
+            const int k = e % MAIL_WORDS;
+            const uint32_t v = k == 0 ? (uint32_t)rc->r : (k == 1 ? (uint32_t)rc->nswaps : (uint32_t)rc->pc[k - 2]);
+            dst[e] = (a.seq << 32) | v;
+        }
+    };
+    const int64_t blast = b0 + nbp - 1;
+
     // CTA 0: factor panel bb (columns jpp.., width ww) from row `row` on, fast path first, general path otherwise.
     auto factor_full = [&](int64_t bb, int64_t jpp, int ww, int64_t row) {
         if (cta != 0) return;
@@ -573,6 +594,7 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
             sm.last_r = 0; sm.last_nsw = 0; sm.last_pcm = 0;
             a.pstart[bb + 1] = (int32_t)row;
         }
+        if (bb == blast) mail();
     };
     auto flush_all = [&]() {                       // U slices whose readers all passed the last grid barrier
         strip_flush_u(sm, 0, A, ld);
@@ -660,6 +682,7 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
                     if (got) a.pstart[b + 2] = (int32_t)(cur + r + sm.r_out);
                     a.rec[b + 1].pad = got ? 1 : 0;
                 }
+                if (got && b + 1 == blast) mail();
             } else if (tid == 0) {
                 a.rec[b + 1].pad = 0;
             }
