@@ -101,7 +101,7 @@ int trsm_leaf(Fp& c, int64_t s, uint32_t* X, int64_t ldx, int64_t ncols) {
     if (!LOWER && c.sb0(s + 1) - c.sb0(s) <= 1) return LINAC_OK;     // U is the identity inside one base panel
     Timed tm(c, stats().ms_trsm);
     trsm_strip_kernel<LOWER><<<(unsigned)((ncols + PW - 1) / PW), TNT, trsm_smem_bytes(K), c.s>>>(
-        c.A, c.ld, X, ldx, ncols, c.d_pstart, (int)c.sb0(s), (int)c.sb0(s + 1), c.d_T, c.d_pivcols, c.f, nullptr, 0);
+        c.A, c.ld, X, ldx, ncols, c.d_pstart, (int)c.sb0(s), (int)c.sb0(s + 1), c.d_T, c.d_pivcols, c.f, nullptr, 0, nullptr, 0, nullptr);
     LINAC_CUDA(cudaGetLastError());
     stats().kernel_launches++;
     stats().update_macs += K * K / 2 * ncols;
@@ -138,8 +138,10 @@ int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r, int64_t early_c0 = 0,
     a.A = c.A; a.ld = c.ld; a.rows = c.rows; a.cols = c.cols; a.i0 = i0; a.j0 = j0; a.ws = (int)(j1 - j0);
     a.rec = c.d_rec; a.T = c.d_T; a.E = c.d_E; a.pivcols = c.d_pivcols; a.pstart = c.d_pstart;
     static unsigned long long seq_counter = 0;
-    a.host_mail = c.h_mail; a.seq = (++seq_counter) & 0xFFFFFFFFull;
+    a.seq = (++seq_counter) & 0xFFFFFFFFull;
     if (a.seq == 0) a.seq = ++seq_counter & 0xFFFFFFFFull;      // 0 is the mailbox's initial content
+    const bool early = early_ncols > 0 && options().timing == 0;
+    a.host_mail = early ? nullptr : c.h_mail;                    // with an early solve, the solve kernel mails
     void* args[] = {&a};
     {
         Timed tm(c, stats().ms_strip);
@@ -147,11 +149,10 @@ int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r, int64_t early_c0 = 0,
                                                sizeof(StripSmem), c.s));
     }
     linac_stats& st = stats();
-    if (early_ncols > 0 && options().timing == 0) {
-        LINAC_CUDA(cudaEventRecord(c.ev_strip, c.s));
+    if (early) {
         trsm_strip_kernel<true><<<(unsigned)((early_ncols + PW - 1) / PW), TNT, trsm_smem_bytes(j1 - j0), c.s>>>(
             c.A, c.ld, c.A + i0 * c.ld + early_c0, c.ld, early_ncols, c.d_pstart, (int)b0, (int)b1, c.d_T, c.d_pivcols, c.f,
-            early_Bq, early_kp);
+            early_Bq, early_kp, c.h_mail, a.seq, c.d_rec);
         LINAC_CUDA(cudaGetLastError());
         st.kernel_launches++;
     } else {

@@ -44,7 +44,6 @@ constexpr int SW_MAX = 256;                 // widest strip (columns)
 constexpr int SNT = 1024;                   // threads per CTA of the strip kernel (32 warps)
 constexpr int SRB = 256;                    // rows of one P2 tile
 constexpr int MAXBP = SW_MAX / PW;          // base panels per strip
-constexpr int MAIL_WORDS = 2 + PW;          // per panel: r, nswaps, pc[32]
 
 // d*x - h*y mod p with one reduction: d*x + (p-h)*y < 2^63.
 __device__ __forceinline__ uint32_t lincomb(uint32_t d, uint32_t x, uint32_t h, uint32_t y, const ModP& f) {
@@ -349,6 +348,21 @@ __device__ bool panel_factor(StripSmem& sm, const uint32_t* A, int64_t ld, int64
     return true;
 }
 
+// What the host needs of a strip's records (r, nswaps, pc[32] per panel), posted to mapped pinned host memory --
+// PCIe writes, no copy engine, so a large transfer the caller has in flight cannot delay the host's next launches.
+// Every 64-bit word carries the launch's sequence number in its upper half, so no system-wide fence is needed: the
+// host waits until every word shows the tag.  Called by all threads of ONE CTA.
+constexpr int MAIL_WORDS = 2 + PW;          // per panel: r, nswaps, pc[32]
+__device__ __forceinline__ void mail_records(volatile unsigned long long* dst, unsigned long long seq, const PanelRec* rec,
+                                             int nbp) {
+    for (int e = threadIdx.x; e < nbp * MAIL_WORDS; e += blockDim.x) {
+        const PanelRec* rc = rec + e / MAIL_WORDS;
+        const int k = e % MAIL_WORDS;
+        const uint32_t v = k == 0 ? (uint32_t)rc->r : (k == 1 ? (uint32_t)rc->nswaps : (uint32_t)rc->pc[k - 2]);
+        dst[e] = (seq << 32) | v;
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // The strip kernel.  Panel metadata arrays are indexed by the GLOBAL base panel number b = j0/PW + i.
 // pstart[b+1] (device) receives the number of pivots found left of panel b+1.
@@ -565,21 +579,13 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
     const int64_t cu1 = a.j0 + a.ws;               // end of the strip
     int64_t cur = a.i0;
 
-    // CTA 0, once it has written the record of the strip's LAST panel: mail what the host needs of all records
-    // (r, nswaps, pc[32] per panel) through mapped memory -- posted PCIe writes, no copy engine, so a large
-    // transfer the caller has in flight cannot delay the host's next launches.  Every 64-bit word carries the
-    // launch's sequence number in its upper half, so no system-wide fence (a PCIe round trip) is needed: the host
-    // waits until every word shows the tag.  Sent as early as possible: the host only needs it to enqueue what follows.
+    // CTA 0, once it has written the record of the strip's LAST panel, mails the records to the host -- unless the
+    // row-block solve launched right behind this kernel does it (host_mail == nullptr): there the PCIe drain hides
+    // under 40 us of work instead of sitting in front of this kernel's last grid barrier.
     auto mail = [&]() {
         if (a.host_mail == nullptr) return;
         __syncthreads();
-        volatile unsigned long long* dst = a.host_mail;
-        for (int e = tid; e < nbp * MAIL_WORDS; e += SNT) {
-            const PanelRec* rc = a.rec + b0 + e / MAIL_WORDS;
-            const int k = e % MAIL_WORDS;
-            const uint32_t v = k == 0 ? (uint32_t)rc->r : (k == 1 ? (uint32_t)rc->nswaps : (uint32_t)rc->pc[k - 2]);
-            dst[e] = (a.seq << 32) | v;
-        }
+        mail_records(a.host_mail, a.seq, a.rec + b0, nbp);
     };
     const int64_t blast = b0 + nbp - 1;
 
@@ -734,8 +740,11 @@ __global__ void __launch_bounds__(TNT) trsm_strip_kernel(const uint32_t* __restr
                                                          const int32_t* __restrict__ pstart, int bs0, int bs1,
                                                          const uint32_t* __restrict__ T,
                                                          const int32_t* __restrict__ pivcols, ModP f,
-                                                         uint8_t* __restrict__ Bq, int kp) {
+                                                         uint8_t* __restrict__ Bq, int kp,
+                                                         unsigned long long* host_mail, unsigned long long seq,
+                                                         const PanelRec* rec) {
     extern __shared__ __align__(16) unsigned char trsm_smem_raw[];
+    if (host_mail != nullptr && blockIdx.x == 0) mail_records(host_mail, seq, rec + bs0, bs1 - bs0);
     const int t0 = pstart[bs0], K = pstart[bs1] - t0;
     uint32_t (*Xs)[PW] = reinterpret_cast<uint32_t (*)[PW]>(trsm_smem_raw);                                 // [K][32]
     uint32_t (*Ts)[PW + 1] = reinterpret_cast<uint32_t (*)[PW + 1]>(trsm_smem_raw + (size_t)K * PW * 4);     // [32][33]
