@@ -131,13 +131,14 @@ int trsm_lower(Fp& c, int64_t s0, int64_t s1, int64_t c0, int64_t c1) {
 // behind the strip kernel (it takes the pivot counts from device memory), and the host reads the pivot counts
 // through a second stream meanwhile: the round trip then hides under the solve instead of idling the GPU.
 int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r, int64_t early_c0 = 0, int64_t early_ncols = 0,
-                 uint8_t* early_Bq = nullptr, int early_kp = 0) {
+                 uint8_t* early_Bq = nullptr, int early_kp = 0, uint8_t* tail_Aq = nullptr) {
     const int64_t b0 = c.sb0(s), b1 = c.sb0(s + 1);
     const int64_t j0 = panel_col0(b0), j1 = std::min(c.cols, panel_col0(b1));
     StripArgs a;
     a.A = c.A; a.ld = c.ld; a.rows = c.rows; a.cols = c.cols; a.i0 = i0; a.j0 = j0; a.ws = (int)(j1 - j0);
     a.rec = c.d_rec; a.T = c.d_T; a.E = c.d_E; a.pivcols = c.d_pivcols; a.pstart = c.d_pstart;
     static unsigned long long seq_counter = 0;
+    a.Aq = tail_Aq; a.kp = early_kp;
     a.seq = (++seq_counter) & 0xFFFFFFFFull;
     if (a.seq == 0) a.seq = ++seq_counter & 0xFFFFFFFFull;      // 0 is the mailbox's initial content
     const bool early = early_ncols > 0 && options().timing == 0;
@@ -234,6 +235,7 @@ int factor(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t* r_out, bool allow
             // the row-block solve can hand U12 to the Schur update as u8 limb planes (saves the update's own split)
             const size_t mark = c.arena->off;
             uint8_t* Bq = nullptr;
+            uint8_t* Aq = nullptr;
             int kp_b = 0;
             if (se - s == 1 && cur < c.rows) {
                 const int64_t ws = jc - panel_col0(c.sb0(s));
@@ -241,8 +243,9 @@ int factor(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t* r_out, bool allow
                 if (o.gemm_path != 1 && o.tc_panel != 0 && ws <= 256 && jend - jc >= o.tc_min_mn && ws >= o.tc_min_k) {
                     kp_b = (int)((ws + 127) / 128 * 128);
                     Bq = (uint8_t*)c.arena->take((size_t)4 * (jend - jc) * kp_b, 1024);
+                    if (Bq) Aq = (uint8_t*)c.arena->take((size_t)4 * (c.rows - cur) * kp_b, 1024);
                 }
-                rc = factor_strip(c, s, cur, &r, jc, jend - jc, Bq, kp_b);
+                rc = factor_strip(c, s, cur, &r, jc, jend - jc, Bq, kp_b, Aq);
                 solved = rc == LINAC_EARLY_SOLVE_DONE;
                 if (solved) rc = LINAC_OK;
             } else {
@@ -256,7 +259,7 @@ int factor(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t* r_out, bool allow
                 if (m2 > 0) {
                     GemmArgs g{c.A + (cur + r) * c.ld + jc, c.ld, c.A + (cur + r) * c.ld, c.ld, c.d_pivcols + cur,
                                c.A + cur * c.ld + jc,       c.ld, m2,                      jend - jc, r};
-                    if (solved && Bq) { g.Bq_ready = Bq; g.kp_ready = kp_b; }
+                    if (solved && Bq) { g.Bq_ready = Bq; g.kp_ready = kp_b; g.Aq_ready = Aq; }
                     rc = run_gemm(c, g);
                     if (rc) return rc;
                 }

@@ -377,6 +377,8 @@ struct StripArgs {
     uint32_t* E;             // [nb][PW*PW]
     int32_t* pivcols;        // [min(rows, cols)]
     int32_t* pstart;         // [nb+1]
+    uint8_t* Aq;             // optional: receives the u8 limb planes of L21 (rows below the strip x its pivot columns)
+    int kp;                  //   Aq[limb][m][kp], k-major, zero padded to kp (what the Schur update's TMA loads expect)
     unsigned long long* host_mail;  // mapped pinned host memory: MAXBP * MAIL_WORDS tagged words, written by CTA 0
     unsigned long long seq;         // tag of this launch (32 significant bits)
 };
@@ -714,6 +716,31 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
     }
     strip_flush_u(sm, 0, A, ld);
     strip_flush_u(sm, 1, A, ld);
+    // Tail: every pivot column of the strip is known and the rows below are final in those columns, so the whole
+    // grid writes the limb planes of L21 for the Schur update that follows (saves that update its own split pass).
+    if (a.Aq != nullptr) {
+        const int K = (int)(cur - a.i0);
+        const int64_t M = a.rows - cur;
+        const int64_t plane = M * a.kp;
+        const int nword = a.kp / 4;                       // 4 k per 32-bit word
+        for (int wd = lane; wd < nword; wd += 32) {
+            int32_t pc[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) pc[e] = wd * 4 + e < K ? a.pivcols[a.i0 + wd * 4 + e] : -1;
+            for (int64_t m = (int64_t)cta * (SNT / 32) + wq; m < M; m += (int64_t)G * (SNT / 32)) {
+                const uint32_t* row = A + (cur + m) * ld;
+                uint32_t v[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) v[e] = pc[e] >= 0 ? row[pc[e]] : 0u;
+#pragma unroll
+                for (int l = 0; l < 4; ++l) {
+                    const uint32_t packed = ((v[0] >> (8 * l)) & 0xFF) | (((v[1] >> (8 * l)) & 0xFF) << 8) |
+                                            (((v[2] >> (8 * l)) & 0xFF) << 16) | (((v[3] >> (8 * l)) & 0xFF) << 24);
+                    *reinterpret_cast<uint32_t*>(a.Aq + l * plane + m * a.kp + wd * 4) = packed;
+                }
+            }
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -587,13 +587,15 @@ int gemm_modp_tc(const GemmArgs& g, const ModP& f, cudaStream_t s, Arena* scratc
         }
         const bool b_ready = g.Bq_ready != nullptr && g.kp_ready >= g.K && g.kp_ready <= 2 * KB && g.kp_ready % KB == 0;
         const int64_t kp = b_ready ? g.kp_ready : (g.K + KB - 1) / KB * KB;
-        uint8_t* Aq = (uint8_t*)scratch->take((size_t)4 * g.M * kp, 1024);
+        const bool a_ready = b_ready && g.Aq_ready != nullptr;
+        uint8_t* Aq = a_ready ? g.Aq_ready : (uint8_t*)scratch->take((size_t)4 * g.M * kp, 1024);
         uint8_t* Bq = b_ready ? g.Bq_ready : (uint8_t*)scratch->take((size_t)4 * g.N * kp, 1024);
         if (!Aq || !Bq) return -1;
-        {
+        if (!a_ready) {
             dim3 grid((unsigned)((kp / 4 + 127) / 128), (unsigned)std::min<int64_t>(g.M, 16384));
             split_a_kernel<<<grid, 128, 0, s>>>(g.Abase, g.lda, g.kcols, 0, g.M, g.K, kp, Aq);
             LINAC_CUDA(cudaGetLastError());
+            stats().kernel_launches++;
         }
         if (!b_ready) {
             dim3 grid((unsigned)(kp / 128), (unsigned)((g.N + 31) / 32));
@@ -611,7 +613,7 @@ int gemm_modp_tc(const GemmArgs& g, const ModP& f, cudaStream_t s, Arena* scratc
         else
             gemm_tc_panel_kernel<false><<<(unsigned)std::min(grid, sc.nitems), P_THREADS, P_SMEM, s>>>(tmA, tmB, tmC, (int)(kp / KB), sc, f);
         LINAC_CUDA(cudaGetLastError());
-        stats().kernel_launches += 2;
+        stats().kernel_launches += 1;
         stats().tc_launches++;
         stats().update_macs += g.M * g.N * g.K;
         return LINAC_OK;

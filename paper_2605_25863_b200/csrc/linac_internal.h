@@ -79,6 +79,7 @@ struct GemmArgs {
     // K <= 256 panel kernel; anything else ignores it and splits B itself.
     uint8_t* Bq_ready = nullptr;
     int64_t kp_ready = 0;
+    uint8_t* Aq_ready = nullptr;      // same for A: Aq[limb][m][kp_ready], written by the strip kernel's tail
 };
 int gemm_modp_simt(const GemmArgs& g, const ModP& f, cudaStream_t s);
 // Tensor-core (tcgen05 int8 limb) path; returns LINAC_OK if it ran, or a negative value if the
