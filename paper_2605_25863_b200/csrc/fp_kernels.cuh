@@ -32,6 +32,21 @@ __global__ void reduce_mod_p_kernel(uint32_t* __restrict__ A, int64_t rows, int6
     }
 }
 
+// The same for 16-byte aligned rows (base and ld): four columns per thread, 128-bit loads, a store only where a
+// residue changed.  cols4 = cols / 4; the caller runs the scalar kernel on the remaining cols % 4 columns.
+__global__ void reduce_mod_p_vec4_kernel(uint32_t* __restrict__ A, int64_t rows, int64_t cols4, int64_t ld, uint32_t p) {
+    const int64_t c4 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c4 >= cols4) return;
+    for (int64_t r = blockIdx.y; r < rows; r += gridDim.y) {
+        uint4* q = reinterpret_cast<uint4*>(A + r * ld) + c4;
+        uint4 v = *q;
+        if (v.x >= p || v.y >= p || v.z >= p || v.w >= p) {
+            v.x %= p; v.y %= p; v.z %= p; v.w %= p;
+            *q = v;
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // Free-column gather / scatter for the back-elimination workspace: F[k][t] = A[k][freecols[t]] for
 // k below the column's threshold row (the number of pivots found up to and including the column's

@@ -415,10 +415,21 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     LINAC_CUDA(cudaMemcpyToSymbolAsync(c_f, &c.f, sizeof(ModP), 0, cudaMemcpyHostToDevice, s));
     // S0 ingest
     {
-        dim3 grid((unsigned)((cols + 255) / 256), (unsigned)std::min<int64_t>(rows, 2048));
-        reduce_mod_p_kernel<<<grid, 256, 0, s>>>(dA, rows, cols, ld, p);
-        LINAC_CUDA(cudaGetLastError());
-        st.kernel_launches++;
+        const bool vec = ((((uintptr_t)dA) | ((uintptr_t)ld * 4)) & 15) == 0 && cols >= 4;
+        const int64_t cols4 = vec ? cols / 4 : 0;
+        if (vec) {
+            dim3 grid((unsigned)((cols4 + 255) / 256), (unsigned)std::min<int64_t>(rows, 4096));
+            reduce_mod_p_vec4_kernel<<<grid, 256, 0, s>>>(dA, rows, cols4, ld, p);
+            LINAC_CUDA(cudaGetLastError());
+            st.kernel_launches++;
+        }
+        if (cols - 4 * cols4 > 0) {
+            const int64_t rest = cols - 4 * cols4;
+            dim3 grid((unsigned)((rest + 255) / 256), (unsigned)std::min<int64_t>(rows, 2048));
+            reduce_mod_p_kernel<<<grid, 256, 0, s>>>(dA + 4 * cols4, rows, rest, ld, p);
+            LINAC_CUDA(cudaGetLastError());
+            st.kernel_launches++;
+        }
     }
     // forward elimination
     int64_t r = 0;

@@ -99,10 +99,15 @@ def test_wide_and_tall(oracle, shape):
     check_against_oracle(oracle, a, P31)
 
 
-def test_entries_ge_p_are_reduced(oracle):
+@pytest.mark.parametrize("shape", [(90, 110), (96, 112), (70, 259)])
+def test_entries_ge_p_are_reduced(oracle, shape):
+    """Scalar ingest (rows not 16-byte aligned), the 128-bit ingest, and both on one matrix (cols % 4 != 0 with
+    an aligned leading dimension is exercised through the padded variant below)."""
     rng = np.random.default_rng(4)
-    a = rng.integers(0, 2**32, size=(90, 110), dtype=np.uint64).astype(np.uint32)
+    a = rng.integers(0, 2**32, size=shape, dtype=np.uint64).astype(np.uint32)
     check_against_oracle(oracle, a, P29)
+    if shape[1] % 4:
+        check_against_oracle(oracle, a, P29, ld=(shape[1] + 7) // 4 * 4)
 
 
 def test_augmented_solve_nontrivial_output(oracle):
