@@ -34,8 +34,8 @@ import linac_inputs as gen  # noqa: E402
 WORKLOAD_KIND = {"uniform": "dense uniform", "lowrank": "product of uniform factors (exact rank)",
                  "sparse_dep": "90% zeros, every 50th row dependent"}
 
-#: ncu --set full, gemm_tc_panel_kernel, second launch of a c3 call (profiles/r01_v8_launches_c3.md)
-NCU_TOP_LAUNCH_DRAM_BYTES_C3 = 396569088 + 326528768
+#: ncu --set full, gemm_tc_panel_kernel, second launch of a c3 call (profiles/r01_v9_launches_c3.md)
+NCU_TOP_LAUNCH_DRAM_BYTES_C3 = 396063488 + 324826368
 
 PAPER_A100_GMULMOD = {"c3": (2 * 1e4 ** 3 / 3) / 3.6 / 1e9,            # PAPER.md:59  (3.6 s at N = 10^4)
                       "c5": (2 * 1e5 ** 3 / 3) / (45 * 60) / 1e9}       # PAPER.md:61  (45 min at N = 10^5)
@@ -322,7 +322,7 @@ def main():
                 "note": "peak = 148 SM x 64 IMAD lanes x max SM clock (DESIGN.md); "
                         "achieved = executed update MACs / summed event time of the update kernels"}
     # the largest single launch, per launch: algorithmic bytes (C read + C written + both limb-plane sets read) and,
-    # for the default workload, the DRAM traffic ncu measured for the same launch (profiles/r01_v8_launches_c3.md)
+    # for the default workload, the DRAM traffic ncu measured for the same launch (profiles/r01_v9_launches_c3.md)
     tm_, tn_, tk_ = st_t.get("top_m", 0), st_t.get("top_n", 0), st_t.get("top_k", 0)
     if tensor_used and st_t.get("ms_update_top", 0) > 0:
         kp_ = -(-tk_ // 128) * 128
