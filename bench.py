@@ -13,6 +13,7 @@ selects another config; the default finishes in well under a minute.
                beside it as e2e.serial_ms_per_step.
   roofline   : the Schur-update kernel (dominant): executed field MACs / its event-timed duration.
   cpu_baseline: the CPU oracle timed on a bounded sample on this box's host cores.
+  fp64       : (default workload only) linac_solve_f64 on config c4: ms per solve, GFLOP/s, backward error.
 """
 from __future__ import annotations
 
@@ -109,6 +110,39 @@ def oracle_sample_gmulmod(n: int, p: int, threads: int):
     return (2 * n ** 3 / 3) / dt / 1e9, dt
 
 
+def f64_leg(torch, L, dev, n=16384, nrhs=64, reps=3):
+    """The metric's second half ("fp64 GFLOP/s"): linac_solve_f64 on config c4's shape and distribution
+    (A = G + 4 sqrt(N) I with G i.i.d. N(0,1), 64 N(0,1) right-hand sides), drawn on the device from a seeded torch
+    generator (the numpy recipe of linac_inputs takes half a minute on the host); the solve works in place, so every
+    repetition restores A and B by a device copy outside the timed region.  Backward error in the infinity norm on
+    the ORIGINAL data, computed with torch fp64 on the device."""
+    g = torch.Generator(device=dev)
+    g.manual_seed(5)
+    a0 = torch.randn((n, n), dtype=torch.float64, device=dev, generator=g)
+    a0.diagonal().add_(4.0 * n ** 0.5)
+    b0 = torch.randn((n, nrhs), dtype=torch.float64, device=dev, generator=g)
+    a, b = torch.empty_like(a0), torch.empty_like(b0)
+    stream = torch.cuda.current_stream(dev)
+    times = []
+    for i in range(reps + 1):
+        a.copy_(a0)
+        b.copy_(b0)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        L.solve_f64(a, b)
+        e1.record(stream)
+        e1.synchronize()
+        if i:
+            times.append(e0.elapsed_time(e1))
+    resid = (a0 @ b - b0).abs().amax(dim=0)
+    eta = float((resid / (a0.abs().sum(dim=1).max() * b.abs().amax(dim=0) + b0.abs().amax(dim=0))).max())
+    ms = float(np.mean(times))
+    flop = 2.0 * n ** 3 / 3.0 + 2.0 * n * n * nrhs
+    return {"workload": f"c4: {n}x{n} float64 N(0,1) + 4 sqrt(N) I, {nrhs} right-hand sides (torch generator, seed 5)",
+            "ms_per_solve": ms, "gflops": flop / ms / 1e6, "backward_error": eta, "backward_error_bound": 1e-11,
+            "note": "flop = 2N^3/3 + 2N^2 nrhs; trailing update on the FP64 tensor pipe (DMMA m8n8k4)"}
+
+
 def run_reference(args):
     """--impl reference: the oracle on the host cores, a bounded sample of the same workload per step."""
     rank = int(os.environ.get("RANK", "0"))
@@ -146,6 +180,7 @@ def main():
     ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c5"])
     ap.add_argument("--ref-n", type=int, default=1280, help="sample size for the oracle legs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-f64", action="store_true", help="skip the fp64 leg (config c4) of the default run")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
                     help="library tunable for A/B runs (linac_set_option), e.g. --opt strip_width=256")
     args = ap.parse_args()
@@ -361,6 +396,8 @@ def main():
         "baseline_context": "paper, A100: 3.6 s at N=1e4 (PAPER.md:59) = 185 Gmulmod/s, 45 min at N=1e5 (PAPER.md:61) = 247 "
                             "Gmulmod/s; another machine, context only",
     }
+    if rank == 0 and world == 1 and args.workload == "c3" and not args.no_f64:
+        out["fp64"] = f64_leg(torch, L, dev)
     if rank == 0 and not args.no_cpu_baseline:
         import oracle
         threads = oracle.max_threads()
