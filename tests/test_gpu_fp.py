@@ -179,3 +179,29 @@ def test_schedule_options_do_not_change_the_result(oracle, opts):
     finally:
         for k, v in defaults.items():
             L.set_option(k, v)
+
+
+# ------------------------------------------------------------------ mid-size stress (several strips, all paths)
+@pytest.mark.parametrize("case", ["tall", "wide", "p3", "zero_blocks", "sparse2000", "lowrank_swaps"])
+def test_mid_size_stress(oracle, case):
+    """Shapes spanning many strips where the general panel path, row exchanges, free columns and rank exhaustion
+    all occur, still small enough for the oracle."""
+    if case == "tall":
+        a, p = gen.uniform_matrix(3000, 700, P31, seed=31), P31
+    elif case == "wide":
+        a, p = gen.uniform_matrix(700, 3000, P29, seed=32), P29
+    elif case == "p3":
+        a, p = gen.uniform_matrix(1200, 1200, 3, seed=33), 3              # a third of all entries are zero
+    elif case == "zero_blocks":
+        a, p = gen.uniform_matrix(1500, 1500, 65521, seed=34), 65521
+        a[:, 100:230] = 0
+        a[:, 700:701] = 0
+        a[300:420, :] = 0
+        a[:, 1000:1100] = a[:, 0:100]                                     # dependent columns
+    elif case == "sparse2000":
+        a, p = gen.sparse_dependent_rows(0, 2000, 2000, 2000, P31, seed=7, seed_dep=8), P31
+    else:
+        a, _, _ = gen.lowrank_factors(1800, 900, 1600, P31, seed_b=35, seed_c=36)
+        a, p = a[::-1].copy(), P31                                        # reversed rows: same row space
+        a[:64, :] = 0                                                     # pivots must come from further down
+    check_against_oracle(oracle, a, p)
