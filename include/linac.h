@@ -104,6 +104,22 @@ int linac_nullspace_from_rref_u32(const uint32_t *dR, int64_t rows, int64_t cols
                                   int64_t rank, const int32_t *pivot_cols, uint32_t *dK, int64_t ldk,
                                   void *stream);
 
+/* ---- F_p: linear systems (eq. 10-14) ------------------ */
+/*
+ * linac_solve_u32 -- solves A X = B over F_p by row reducing the augmented matrix M = (A | B) (eq. 11).
+ *   dM   DEVICE rows x (cols + nrhs) row-major (ld >= cols + nrhs): (A | B) on entry, the RREF of M on return.
+ *   dX   DEVICE cols x nrhs (ldx >= nrhs), out: for every CONSISTENT right-hand side the particular solution with
+ *        the free variables set to zero; the columns of inconsistent right-hand sides are zero.
+ *   rank_a          HOST out: rank of A (number of pivot columns < cols).
+ *   pivot_cols_out  HOST out, capacity min(rows, cols + nrhs) int32: pivot columns of the RREF of M; may be NULL.
+ *   consistent      HOST out, nrhs bytes: 1 iff rank(A) = rank(A | b_j) (eq. 13).  The right-hand sides are reduced
+ *        together, so b_j counts as consistent iff its column is not a pivot column AND vanishes on the rows whose
+ *        pivots lie in the augmented block (such a row is the (0 ... 0 | 1) of eq. 14 for an earlier right-hand side).
+ * rows, cols or nrhs equal to 0 are legal.  Same conventions and errors as linac_rref_u32.
+ */
+int linac_solve_u32(uint32_t *dM, int64_t rows, int64_t cols, int64_t nrhs, int64_t ld, uint32_t p, void *stream,
+                    int64_t *rank_a, int32_t *pivot_cols_out, uint8_t *consistent, uint32_t *dX, int64_t ldx);
+
 /* ---- F_p: the Schur-update primitive on its own (S5; exposed for measurement and tests) ------ */
 /*
  * linac_gemm_sub_u32 -- C <- C - A.B (mod p), the blocked form of the paper's row update

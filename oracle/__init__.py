@@ -122,6 +122,30 @@ def nullspace_modp(r: np.ndarray, p: int, rank: int, pivot_cols: np.ndarray) -> 
     return k
 
 
+def solve_modp(a: np.ndarray, b: np.ndarray, p: int, nthreads: int = 1):
+    """A X = B over F_p, ONE right-hand side at a time, exactly as the paper states it:
+    reduce M = (A | b) (eq. 11); the system is consistent iff the augmented column is not a pivot column (eq. 13-14);
+    then the pivot columns of A are the solved variables, the free variables are set to zero.
+    Returns (consistent bool[nrhs], X uint32[cols, nrhs]) with zero columns for inconsistent right-hand sides.
+    Pinned in tests/test_oracle_modp.py: A.x = b by a plain product, and consistency against brute-force
+    enumeration of all p^cols vectors over tiny fields."""
+    a = np.ascontiguousarray(a, dtype=np.uint32)
+    b = np.ascontiguousarray(b, dtype=np.uint32)
+    rows, cols = a.shape
+    nrhs = b.shape[1]
+    cons = np.zeros(nrhs, dtype=bool)
+    x = np.zeros((cols, nrhs), dtype=np.uint32)
+    for j in range(nrhs):
+        m = np.ascontiguousarray(np.hstack([a, b[:, j:j + 1]]))
+        r, rank, piv = rref_modp(m, p, nthreads=nthreads)
+        if rank > 0 and piv[rank - 1] == cols:          # the augmented column became a pivot column: (0 ... 0 | 1)
+            continue
+        cons[j] = True
+        for k in range(rank):
+            x[piv[k], j] = r[k, cols]
+    return cons, x
+
+
 def matmul_modp(a: np.ndarray, b: np.ndarray, p: int, nthreads: int = 1) -> np.ndarray:
     a = np.ascontiguousarray(a, dtype=np.uint32)
     b = np.ascontiguousarray(b, dtype=np.uint32)

@@ -104,4 +104,23 @@ __global__ void nullspace_kernel(const uint32_t* __restrict__ R, int64_t ld, int
     }
 }
 
+// ------------------------------------------------------------------------------------------
+// Solutions of A X = B from the RREF R of (A | B).  Rows [0, rank_a) have their pivots in
+// A's columns (colrow[c] = that row, or -1 for a free column c), rows [rank_a, rank_m) in the augmented block.
+// One thread per right-hand side j: consistent iff column cols+j vanishes on rows [rank_a, rank_m) (this
+// includes "is not a pivot column"); then X[c][j] = R[colrow[c]][cols+j] for pivot columns, 0 for free ones.
+__global__ void solve_extract_kernel(const uint32_t* __restrict__ R, int64_t ld, int64_t cols, int64_t nrhs,
+                                     int64_t rank_a, int64_t rank_m, const int32_t* __restrict__ colrow,
+                                     uint32_t* __restrict__ X, int64_t ldx, uint8_t* __restrict__ consistent) {
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= nrhs) return;
+    bool ok = true;
+    for (int64_t k = rank_a; k < rank_m; ++k) ok = ok && R[k * ld + cols + j] == 0u;
+    if (blockIdx.y == 0) consistent[j] = ok ? 1 : 0;
+    for (int64_t c = blockIdx.y; c < cols; c += gridDim.y) {
+        const int32_t k = colrow[c];
+        X[c * ldx + j] = (ok && k >= 0) ? R[(int64_t)k * ld + cols + j] : 0u;
+    }
+}
+
 }  // namespace linac

@@ -564,6 +564,49 @@ int linac_nullspace_u32(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, ui
     return rc;
 }
 
+int linac_solve_u32(uint32_t* dM, int64_t rows, int64_t cols, int64_t nrhs, int64_t ld, uint32_t p, void* stream,
+                    int64_t* rank_a, int32_t* pivot_cols_out, uint8_t* consistent, uint32_t* dX, int64_t ldx) {
+    std::lock_guard<std::mutex> lock(g_call_mutex);
+    if (cols < 0 || nrhs < 0 || !rank_a || (nrhs > 0 && !consistent)) return LINAC_ERR_INVALID_ARG;
+    if (cols > 0 && nrhs > 0 && (!dX || ldx < nrhs)) return LINAC_ERR_INVALID_ARG;
+    const int64_t wide = cols + nrhs;
+    Arena arena;
+    std::vector<int32_t> piv((size_t)std::max<int64_t>(1, std::min(rows, wide)));
+    int64_t r = 0;
+    int rc = rref_impl(dM, rows, wide, ld, p, (cudaStream_t)stream, &r, piv.data(), &arena);
+    if (rc) return rc;
+    int64_t ra = 0;
+    while (ra < r && piv[ra] < cols) ++ra;                     // pivot columns are ascending
+    *rank_a = ra;
+    if (pivot_cols_out) std::copy(piv.begin(), piv.begin() + r, pivot_cols_out);
+    if (nrhs == 0) return LINAC_OK;
+    if (rows == 0) {                                            // no equations: every right-hand side is empty, x = 0
+        std::fill(consistent, consistent + nrhs, (uint8_t)1);
+        if (cols > 0) LINAC_CUDA(cudaMemset2DAsync(dX, (size_t)ldx * 4, 0, (size_t)nrhs * 4, (size_t)cols, (cudaStream_t)stream));
+        LINAC_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+        return LINAC_OK;
+    }
+    cudaStream_t s = (cudaStream_t)stream;
+    std::vector<int32_t> colrow((size_t)std::max<int64_t>(1, cols), -1);
+    for (int64_t k = 0; k < ra; ++k) colrow[piv[k]] = (int32_t)k;
+    int32_t* d_colrow = nullptr;
+    uint8_t* d_cons = nullptr;
+    LINAC_CUDA(cudaMalloc(&d_colrow, colrow.size() * 4 + (size_t)nrhs + 16));
+    d_cons = reinterpret_cast<uint8_t*>(d_colrow + colrow.size());
+    cudaError_t e = cudaMemcpyAsync(d_colrow, colrow.data(), colrow.size() * 4, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) {
+        dim3 grid((unsigned)((nrhs + 127) / 128), (unsigned)std::max<int64_t>(1, std::min<int64_t>(cols, 2048)));
+        solve_extract_kernel<<<grid, 128, 0, s>>>(dM, ld, cols, nrhs, ra, r, d_colrow, dX, ldx, d_cons);
+        e = cudaGetLastError();
+        stats().kernel_launches++;
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(consistent, d_cons, (size_t)nrhs, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    cudaFree(d_colrow);
+    if (e != cudaSuccess) { set_cuda_error(e, "linac_solve_u32", __FILE__, __LINE__); return LINAC_ERR_CUDA; }
+    return LINAC_OK;
+}
+
 int linac_nullspace_from_rref_u32(const uint32_t* dR, int64_t rows, int64_t cols, int64_t ld, uint32_t p, int64_t rank,
                                   const int32_t* pivot_cols, uint32_t* dK, int64_t ldk, void* stream) {
     std::lock_guard<std::mutex> lock(g_call_mutex);

@@ -21,7 +21,8 @@ ERR_SINGULAR, ERR_BUFFER_TOO_SMALL, ERR_UNSUPPORTED_DEVICE, ERR_INTERNAL = 5, 6,
 SYMBOLS = [
     "linac_status_string", "linac_last_cuda_error", "linac_version",
     "linac_rref_u32_workspace", "linac_solve_f64_workspace", "linac_set_workspace", "linac_release",
-    "linac_rref_u32", "linac_nullspace_u32", "linac_nullspace_from_rref_u32", "linac_gemm_sub_u32", "linac_solve_f64",
+    "linac_rref_u32", "linac_nullspace_u32", "linac_nullspace_from_rref_u32", "linac_solve_u32", "linac_gemm_sub_u32",
+    "linac_solve_f64",
     "linac_get_last_stats", "linac_set_option",
 ]
 
@@ -67,6 +68,7 @@ def _lib() -> C.CDLL:
         L.linac_rref_u32.argtypes = [vp, i64, i64, i64, u32, vp, C.POINTER(i64), vp]
         L.linac_nullspace_u32.argtypes = [vp, i64, i64, i64, u32, vp, C.POINTER(i64), vp, vp, i64, i64, C.POINTER(i64)]
         L.linac_nullspace_from_rref_u32.argtypes = [vp, i64, i64, i64, u32, i64, vp, vp, i64, vp]
+        L.linac_solve_u32.argtypes = [vp, i64, i64, i64, i64, u32, vp, C.POINTER(i64), vp, vp, vp, i64]
         L.linac_gemm_sub_u32.argtypes = [vp, i64, vp, i64, vp, i64, i64, i64, i64, u32, C.c_int, vp]
         L.linac_solve_f64.argtypes = [vp, i64, i64, vp, i64, i64, C.c_double, vp, C.POINTER(i64)]
         L.linac_get_last_stats.argtypes = [C.POINTER(Stats)]
@@ -187,6 +189,31 @@ def nullspace_u32(a: torch.Tensor, p: int, k: torch.Tensor | None = None):
             if rc:
                 raise LinacError(rc, "linac_nullspace_from_rref_u32")
     return int(rank.value), piv[: rank.value].clone(), kk
+
+
+def solve_u32(m: torch.Tensor, cols: int, p: int):
+    """In place: `m` = (A | B) (CUDA, uint32/int32 storage, rows x (cols + nrhs)) -> its RREF over F_p.
+
+    Returns (rank_a, pivot_cols, consistent, X): X is cols x nrhs on the device (particular solutions, free variables
+    zero; zero columns for inconsistent right-hand sides), `consistent` a host bool tensor.  Mirrors linac_solve_u32.
+    """
+    rows, wide, ld = _check_matrix(m, _U32, "m")
+    nrhs = wide - cols
+    if cols < 0 or nrhs < 0:
+        raise ValueError("cols must lie in [0, m.shape[1]]")
+    with torch.cuda.device(m.device):
+        need = C.c_size_t(0)
+        _lib().linac_rref_u32_workspace(rows, wide, C.byref(need))
+        _ensure_workspace(need.value, m.device)
+        rank_a = C.c_int64(0)
+        piv = torch.empty(max(1, min(rows, wide)), dtype=torch.int32)
+        cons = torch.zeros(max(1, nrhs), dtype=torch.uint8)
+        x = torch.zeros((cols, nrhs), dtype=m.dtype, device=m.device)
+        rc = _lib().linac_solve_u32(m.data_ptr(), rows, cols, nrhs, ld, p, _stream_ptr(m.device), C.byref(rank_a),
+                                    piv.data_ptr(), cons.data_ptr(), x.data_ptr() if x.numel() else None, max(1, nrhs))
+        if rc:
+            raise LinacError(rc, "linac_solve_u32")
+    return int(rank_a.value), piv, cons[:nrhs].bool(), x
 
 
 def nullspace_from_rref_u32(r: torch.Tensor, p: int, rank: int, pivot_cols: torch.Tensor) -> torch.Tensor:

@@ -281,3 +281,44 @@ def test_sparse_dependent_generator_rank(oracle):
     _, rank, piv = oracle.rref_modp(a, P31)
     assert rank == rows - rows // 50
     assert 0.85 < (a[np.arange(rows) % 50 != 49] == 0).mean() < 0.95
+
+
+# ------------------------------------------------------------------ solve_modp
+def test_solve_modp_against_brute_force_and_plain_products(oracle):
+    import itertools
+    rng = np.random.default_rng(11)
+    # (1) tiny fields: consistency must equal "some x in F_p^cols solves it" by enumeration; a returned x must solve it
+    for p, rows, cols in [(2, 4, 4), (3, 3, 4), (3, 5, 3), (5, 3, 3), (2, 6, 5)]:
+        for trial in range(12):
+            a = rng.integers(0, p, size=(rows, cols)).astype(np.uint32)
+            if trial % 3 == 0:
+                a[:, -1] = a[:, 0]                                   # force rank deficiency
+            b = rng.integers(0, p, size=(rows, 3)).astype(np.uint32)
+            cons, x = oracle.solve_modp(a, b, p)
+            allx = np.array(list(itertools.product(range(p), repeat=cols)), dtype=np.int64).T      # cols x p^cols
+            prod = (a.astype(np.int64) @ allx) % p
+            for j in range(3):
+                solvable = bool((prod == b[:, j:j + 1].astype(np.int64)).all(axis=0).any())
+                assert bool(cons[j]) == solvable
+                if solvable:
+                    assert np.array_equal((a.astype(np.int64) @ x[:, j].astype(np.int64)) % p, b[:, j].astype(np.int64))
+                else:
+                    assert not x[:, j].any()
+    # (2) a big prime: manufactured solutions b = A.y are consistent and A.x = b (x need not equal y when A is singular);
+    #     full-rank square A gives x = y exactly (eq. 12)
+    p = 2147483629
+    a = gen.uniform_matrix(40, 40, p, seed=5)
+    y = gen.uniform_matrix(40, 4, p, seed=6)
+    b = oracle.matmul_modp(a, y, p)
+    cons, x = oracle.solve_modp(a, b, p)
+    assert cons.all() and np.array_equal(x, y)
+    a2, _, _ = gen.lowrank_factors(30, 12, 45, p, seed_b=7, seed_c=8)
+    y2 = gen.uniform_matrix(45, 2, p, seed=9)
+    b2 = np.hstack([oracle.matmul_modp(a2, y2, p), gen.uniform_matrix(30, 1, p, seed=10)])       # last one: random -> inconsistent w.h.p.
+    cons2, x2 = oracle.solve_modp(a2, b2, p)
+    assert list(cons2) == [True, True, False]
+    assert np.array_equal(oracle.matmul_modp(a2, x2[:, :2], p), b2[:, :2])
+    # free variables are zero: x is supported on the pivot columns of A
+    _, rank, piv = oracle.rref_modp(a2, p)
+    free = np.setdiff1d(np.arange(45), piv[:rank])
+    assert not x2[free].any()
