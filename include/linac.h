@@ -120,6 +120,22 @@ int linac_nullspace_from_rref_u32(const uint32_t *dR, int64_t rows, int64_t cols
 int linac_solve_u32(uint32_t *dM, int64_t rows, int64_t cols, int64_t nrhs, int64_t ld, uint32_t p, void *stream,
                     int64_t *rank_a, int32_t *pivot_cols_out, uint8_t *consistent, uint32_t *dX, int64_t ldx);
 
+/* ---- F_p: building the matrix on the device -- */
+/*
+ * linac_load_matrix_u32 -- the operation of cuda_load_matrix: every column is a monomial in the "basis
+ * variables", evaluated at one sampling point per row,
+ *     A[r][c] = prod_{t < d} bases[r][ lindices[c][t] ]   (mod p).
+ *   dA        DEVICE out, n_rows x n_cols row-major (ld >= n_cols): exactly what linac_rref_u32 consumes, so the
+ *             host -> device copy of A that the paper keeps disappears.
+ *   dBases    DEVICE n_rows x n_basis uint32 (ldb >= n_basis); entries >= p are reduced mod p.
+ *   dLindices DEVICE n_cols x d int32, row-major, contiguous.  Reading (the paper's footnote on monomials of lower
+ *             degree is lost in the extraction): an index outside [0, n_basis) stands for "no factor" (1), so -1 pads
+ *             monomials with fewer than d factors; d = 0 gives the all-ones matrix.
+ * Pure streaming kernel (4 B written per element); synchronises `stream` before returning.
+ */
+int linac_load_matrix_u32(uint32_t *dA, int64_t n_rows, int64_t n_cols, int64_t ld, const uint32_t *dBases,
+                          int64_t n_basis, int64_t ldb, const int32_t *dLindices, int64_t d, uint32_t p, void *stream);
+
 /* ---- F_p: the Schur-update primitive on its own (S5; exposed for measurement and tests) ------ */
 /*
  * linac_gemm_sub_u32 -- C <- C - A.B (mod p), the blocked form of the paper's row update

@@ -146,6 +146,26 @@ def solve_modp(a: np.ndarray, b: np.ndarray, p: int, nthreads: int = 1):
     return cons, x
 
 
+def load_matrix_modp(bases: np.ndarray, lindices: np.ndarray, p: int) -> np.ndarray:
+    """A[r][c] = prod_t bases[r][lindices[c][t]] mod p, the definition written out with plain
+    numpy integer arithmetic, one factor at a time.  An index outside [0, n_basis) means "no factor" (the reading
+    stated in include/linac.h).  Pinned in tests/test_oracle_modp.py against Python big-int products and the closed
+    form of a Vandermonde matrix."""
+    bases = np.asarray(bases, dtype=np.uint64) % np.uint64(p)
+    lind = np.asarray(lindices, dtype=np.int64)
+    n_rows, n_basis = bases.shape
+    n_cols, d = lind.shape
+    a = np.full((n_rows, n_cols), 1 % p, dtype=np.uint64)
+    for t in range(d):
+        idx = lind[:, t]
+        ok = (idx >= 0) & (idx < n_basis)
+        factor = np.ones((n_rows, n_cols), dtype=np.uint64)
+        if ok.any():
+            factor[:, ok] = bases[:, idx[ok]]
+        a = a * factor % np.uint64(p)
+    return a.astype(np.uint32)
+
+
 def matmul_modp(a: np.ndarray, b: np.ndarray, p: int, nthreads: int = 1) -> np.ndarray:
     a = np.ascontiguousarray(a, dtype=np.uint32)
     b = np.ascontiguousarray(b, dtype=np.uint32)

@@ -123,4 +123,63 @@ __global__ void solve_extract_kernel(const uint32_t* __restrict__ R, int64_t ld,
     }
 }
 
+// ------------------------------------------------------------------------------------------
+// cuda_load_matrix: A[r][c] = prod_t bases[r][lind[c][t]] mod p.  A CTA owns 256 columns
+// (their index lists staged once in shared memory) and walks over its share of the rows; the row of basis values is
+// staged per row, the 256 products are written as one coalesced row segment.  Bound: the 4 B written per element.
+constexpr int LM_COLS = 256;
+constexpr int LM_ROWS = 8;           // rows per pass: the index tile is read once per factor for all of them
+// MONT: the staged basis values are put in Montgomery form (one Barrett product each, shared by 256 columns), every
+// factor then costs a 4-instruction Montgomery product instead of a 14-instruction Barrett one (p odd).
+template <bool MONT>
+__global__ void __launch_bounds__(LM_COLS) load_matrix_kernel(uint32_t* __restrict__ A, int64_t n_rows, int64_t n_cols,
+                                                              int64_t ld, const uint32_t* __restrict__ bases, int64_t n_basis,
+                                                              int64_t ldb, const int32_t* __restrict__ lind, int d,
+                                                              int basis_cap, ModP f) {
+    extern __shared__ __align__(16) unsigned char lm_smem[];
+    int32_t* L = reinterpret_cast<int32_t*>(lm_smem);                          // index tile, stored [t][col]
+    uint32_t* Bv = reinterpret_cast<uint32_t*>(lm_smem + (size_t)LM_COLS * d * 4);   // [LM_ROWS][basis_cap]
+    const int tid = threadIdx.x;
+    const int64_t c0 = (int64_t)blockIdx.x * LM_COLS, c = c0 + tid;
+    for (int e = tid; e < LM_COLS * d; e += LM_COLS) {                        // coalesced read of the index tile
+        const int cl = e / d, t = e - cl * d;
+        const int32_t v = c0 + cl < n_cols ? lind[(c0 + cl) * d + t] : -1;
+        L[t * LM_COLS + cl] = (v >= 0 && v < n_basis) ? v : -1;
+    }
+    const bool staged = n_basis <= basis_cap;
+    auto prep = [&](uint32_t v) {                                              // canonical residue, Montgomery form if MONT
+        v = v >= f.p ? v % f.p : v;
+        return MONT ? reduce64((uint64_t)v * f.c32, f) : v;
+    };
+    for (int64_t r0 = (int64_t)blockIdx.y * LM_ROWS; r0 < n_rows; r0 += (int64_t)gridDim.y * LM_ROWS) {
+        const int nr = (int)min((int64_t)LM_ROWS, n_rows - r0);
+        __syncthreads();
+        if (staged)
+            for (int rr = 0; rr < nr; ++rr)
+                for (int bb = tid; bb < (int)n_basis; bb += LM_COLS)
+                    Bv[(size_t)rr * basis_cap + bb] = prep(bases[(r0 + rr) * ldb + bb]);
+        __syncthreads();
+        if (c < n_cols) {
+            uint32_t acc[LM_ROWS];
+            const uint32_t one = MONT ? f.c32 % f.p : 1u % f.p;
+#pragma unroll
+            for (int rr = 0; rr < LM_ROWS; ++rr) acc[rr] = one;
+            for (int t = 0; t < d; ++t) {
+                const int32_t i = L[t * LM_COLS + tid];
+                if (i < 0) continue;
+#pragma unroll
+                for (int rr = 0; rr < LM_ROWS; ++rr) {
+                    if (rr < nr) {
+                        const uint32_t v = staged ? Bv[(size_t)rr * basis_cap + i] : prep(bases[(r0 + rr) * ldb + i]);
+                        acc[rr] = MONT ? mulredc(acc[rr], v, f) : mulmod(acc[rr], v, f);
+                    }
+                }
+            }
+#pragma unroll
+            for (int rr = 0; rr < LM_ROWS; ++rr)
+                if (rr < nr) A[(r0 + rr) * ld + c] = MONT ? redc(acc[rr], f) : acc[rr];
+        }
+    }
+}
+
 }  // namespace linac

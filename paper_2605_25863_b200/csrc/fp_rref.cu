@@ -607,6 +607,39 @@ int linac_solve_u32(uint32_t* dM, int64_t rows, int64_t cols, int64_t nrhs, int6
     return LINAC_OK;
 }
 
+int linac_load_matrix_u32(uint32_t* dA, int64_t n_rows, int64_t n_cols, int64_t ld, const uint32_t* dBases, int64_t n_basis,
+                          int64_t ldb, const int32_t* dLindices, int64_t d, uint32_t p, void* stream) {
+    std::lock_guard<std::mutex> lock(g_call_mutex);
+    if (n_rows < 0 || n_cols < 0 || n_basis < 0 || d < 0 || d > 4096) return LINAC_ERR_INVALID_ARG;
+    if (p < 2 || p >= (1u << 31) || !is_prime_u32(p)) return LINAC_ERR_BAD_MODULUS;
+    if (n_rows == 0 || n_cols == 0) return LINAC_OK;
+    if (!dA || ld < n_cols || (d > 0 && !dLindices) || (n_basis > 0 && (!dBases || ldb < n_basis))) return LINAC_ERR_INVALID_ARG;
+    int rc = check_device();
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t idx_bytes = (size_t)LM_COLS * (size_t)d * 4;
+    if (idx_bytes > 160 * 1024) return LINAC_ERR_INVALID_ARG;           // d <= 160 with the tile in shared memory
+    const int basis_cap = (int)std::min<int64_t>(std::max<int64_t>(n_basis, 1), (int64_t)((96 * 1024 - std::min<size_t>(idx_bytes, 64 * 1024)) / (4 * LM_ROWS)));
+    const size_t smem = idx_bytes + (size_t)basis_cap * 4 * LM_ROWS;
+    const ModP f = make_modp(p);
+    // about eight CTAs per SM in total, each walking over many 8-row passes: the index tile is staged once per CTA
+    const int64_t gx = (n_cols + LM_COLS - 1) / LM_COLS;
+    const int64_t gy = std::max<int64_t>(1, std::min<int64_t>((n_rows + LM_ROWS - 1) / LM_ROWS, (148 * 8 + gx - 1) / gx));
+    dim3 grid((unsigned)gx, (unsigned)gy);
+    if (f.ninv) {
+        LINAC_CUDA(cudaFuncSetAttribute(load_matrix_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(216 * 1024)));
+        load_matrix_kernel<true><<<grid, LM_COLS, smem, s>>>(dA, n_rows, n_cols, ld, dBases, n_basis, ldb, dLindices, (int)d, basis_cap, f);
+    } else {
+        LINAC_CUDA(cudaFuncSetAttribute(load_matrix_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(216 * 1024)));
+        load_matrix_kernel<false><<<grid, LM_COLS, smem, s>>>(dA, n_rows, n_cols, ld, dBases, n_basis, ldb, dLindices, (int)d, basis_cap, f);
+    }
+    LINAC_CUDA(cudaGetLastError());
+    stats() = linac_stats{};
+    stats().kernel_launches = 1;
+    LINAC_CUDA(cudaStreamSynchronize(s));
+    return LINAC_OK;
+}
+
 int linac_nullspace_from_rref_u32(const uint32_t* dR, int64_t rows, int64_t cols, int64_t ld, uint32_t p, int64_t rank,
                                   const int32_t* pivot_cols, uint32_t* dK, int64_t ldk, void* stream) {
     std::lock_guard<std::mutex> lock(g_call_mutex);

@@ -21,7 +21,7 @@ ERR_SINGULAR, ERR_BUFFER_TOO_SMALL, ERR_UNSUPPORTED_DEVICE, ERR_INTERNAL = 5, 6,
 SYMBOLS = [
     "linac_status_string", "linac_last_cuda_error", "linac_version",
     "linac_rref_u32_workspace", "linac_solve_f64_workspace", "linac_set_workspace", "linac_release",
-    "linac_rref_u32", "linac_nullspace_u32", "linac_nullspace_from_rref_u32", "linac_solve_u32", "linac_gemm_sub_u32",
+    "linac_rref_u32", "linac_nullspace_u32", "linac_nullspace_from_rref_u32", "linac_solve_u32", "linac_load_matrix_u32", "linac_gemm_sub_u32",
     "linac_solve_f64",
     "linac_get_last_stats", "linac_set_option",
 ]
@@ -69,6 +69,7 @@ def _lib() -> C.CDLL:
         L.linac_nullspace_u32.argtypes = [vp, i64, i64, i64, u32, vp, C.POINTER(i64), vp, vp, i64, i64, C.POINTER(i64)]
         L.linac_nullspace_from_rref_u32.argtypes = [vp, i64, i64, i64, u32, i64, vp, vp, i64, vp]
         L.linac_solve_u32.argtypes = [vp, i64, i64, i64, i64, u32, vp, C.POINTER(i64), vp, vp, vp, i64]
+        L.linac_load_matrix_u32.argtypes = [vp, i64, i64, i64, vp, i64, i64, vp, i64, u32, vp]
         L.linac_gemm_sub_u32.argtypes = [vp, i64, vp, i64, vp, i64, i64, i64, i64, u32, C.c_int, vp]
         L.linac_solve_f64.argtypes = [vp, i64, i64, vp, i64, i64, C.c_double, vp, C.POINTER(i64)]
         L.linac_get_last_stats.argtypes = [C.POINTER(Stats)]
@@ -214,6 +215,28 @@ def solve_u32(m: torch.Tensor, cols: int, p: int):
         if rc:
             raise LinacError(rc, "linac_solve_u32")
     return int(rank_a.value), piv, cons[:nrhs].bool(), x
+
+
+def load_matrix_u32(bases: torch.Tensor, lindices: torch.Tensor, p: int, out: torch.Tensor | None = None) -> torch.Tensor:
+    """A[r][c] = prod_t bases[r][lindices[c][t]] mod p on the device (mirrors linac_load_matrix_u32).
+
+    bases: CUDA n_rows x n_basis (uint32/int32 storage); lindices: CUDA n_cols x d int32, contiguous; an index outside
+    [0, n_basis) means "no factor".  Returns the n_rows x n_cols matrix (uint32 bits in an int32 tensor unless `out`)."""
+    n_rows, n_basis, ldb = _check_matrix(bases, _U32, "bases")
+    if lindices.dtype != torch.int32 or lindices.dim() != 2 or not lindices.is_cuda or not lindices.is_contiguous():
+        raise ValueError("lindices must be a contiguous CUDA int32 tensor of shape (n_cols, d)")
+    n_cols, d = lindices.shape
+    if out is None:
+        out = torch.empty((n_rows, n_cols), dtype=torch.int32, device=bases.device)
+    orow, ocol, ld = _check_matrix(out, _U32, "out")
+    if (orow, ocol) != (n_rows, n_cols):
+        raise ValueError("out has the wrong shape")
+    with torch.cuda.device(bases.device):
+        rc = _lib().linac_load_matrix_u32(out.data_ptr(), n_rows, n_cols, ld, bases.data_ptr(), n_basis, ldb,
+                                          lindices.data_ptr() if lindices.numel() else None, d, p, _stream_ptr(bases.device))
+    if rc:
+        raise LinacError(rc, "linac_load_matrix_u32")
+    return out
 
 
 def nullspace_from_rref_u32(r: torch.Tensor, p: int, rank: int, pivot_cols: torch.Tensor) -> torch.Tensor:

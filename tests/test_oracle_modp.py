@@ -322,3 +322,32 @@ def test_solve_modp_against_brute_force_and_plain_products(oracle):
     _, rank, piv = oracle.rref_modp(a2, p)
     free = np.setdiff1d(np.arange(45), piv[:rank])
     assert not x2[free].any()
+
+
+# ------------------------------------------------------------------ load_matrix_modp
+def test_load_matrix_modp_pins(oracle):
+    rng = np.random.default_rng(12)
+    p = 2147483629
+    bases = gen.uniform_matrix(9, 6, p, seed=13)
+    lind = rng.integers(-1, 6, size=(11, 5)).astype(np.int32)              # -1 = no factor
+    a = oracle.load_matrix_modp(bases, lind, p)
+    for r in range(9):                                                      # Python big integers, no modular shortcuts
+        for c in range(11):
+            prod = 1
+            for t in range(5):
+                if lind[c, t] >= 0:
+                    prod *= int(bases[r, lind[c, t]])
+            assert int(a[r, c]) == prod % p
+    # closed form: columns x^0 .. x^7 of a Vandermonde matrix (index 0 repeated c times, padded with -1)
+    x = gen.uniform_matrix(20, 1, p, seed=14)
+    lv = np.full((8, 7), -1, dtype=np.int32)
+    for c in range(8):
+        lv[c, :c] = 0
+    v = oracle.load_matrix_modp(x, lv, p)
+    assert np.array_equal(v, np.array([[pow(int(xi), c, p) for c in range(8)] for xi in x[:, 0]], dtype=np.uint32))
+    # d = 1 is a gather of columns; d = 0 the all-ones matrix; entries >= p are reduced
+    g = oracle.load_matrix_modp(bases, np.array([[3], [0], [5]], dtype=np.int32), p)
+    assert np.array_equal(g, bases[:, [3, 0, 5]])
+    assert (oracle.load_matrix_modp(bases, np.zeros((4, 0), dtype=np.int32), p) == 1).all()
+    big = np.array([[p + 5, 7]], dtype=np.uint32)
+    assert oracle.load_matrix_modp(big, np.array([[0, 1]], dtype=np.int32), p)[0, 0] == 35
