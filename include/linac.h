@@ -120,6 +120,22 @@ int linac_nullspace_from_rref_u32(const uint32_t *dR, int64_t rows, int64_t cols
 int linac_solve_u32(uint32_t *dM, int64_t rows, int64_t cols, int64_t nrhs, int64_t ld, uint32_t p, void *stream,
                     int64_t *rank_a, int32_t *pivot_cols_out, uint8_t *consistent, uint32_t *dX, int64_t ldx);
 
+/* ---- F_p: rank factorisation (eq. 7) ----------------- */
+/*
+ * linac_rank_factor_u32 -- A = C.R over F_p with R the non-zero rows of the RREF of A ("drop_bottom_zero_rows")
+ * and C = A[:, J], J the pivot columns (a basis of the column space taken from A itself).
+ *   dA   DEVICE rows x cols (lda >= cols), const: A is left untouched.
+ *   dR   DEVICE rows x cols (ldr >= cols), out: the whole RREF of A (it is also the work buffer); R is its
+ *        first `rank` rows, the rest are zero rows.
+ *   dC   DEVICE rows x min(rows, cols) (ldc >= min(rows, cols)), out: columns [0, rank) are written, canonical
+ *        in [0,p); the remaining columns are not touched.
+ *   rank, pivot_cols_out  as in linac_rref_u32 (rank is required).
+ * rows == 0 or cols == 0 is legal (rank 0).  Same errors as linac_rref_u32.  dA, dR, dC must not overlap.
+ */
+int linac_rank_factor_u32(const uint32_t *dA, int64_t rows, int64_t cols, int64_t lda, uint32_t p, void *stream,
+                          uint32_t *dR, int64_t ldr, uint32_t *dC, int64_t ldc, int64_t *rank,
+                          int32_t *pivot_cols_out);
+
 /* ---- F_p: building the matrix on the device -- */
 /*
  * linac_load_matrix_u32 -- the operation of cuda_load_matrix: every column is a monomial in the "basis

@@ -146,6 +146,17 @@ def solve_modp(a: np.ndarray, b: np.ndarray, p: int, nthreads: int = 1):
     return cons, x
 
 
+def rank_factor_modp(a: np.ndarray, p: int, nthreads: int = 1):
+    """Rank factorisation A = C.R exactly as the paper states it (eq. 7): R = the RREF of A with its
+    bottom zero rows dropped, J = its pivot columns, C = A[:, J] (entries reduced to [0,p)).  Returns (C, R, J).
+    Pinned in tests/test_oracle_modp.py: C.R = A by a plain product, C has full column rank (brute force over a tiny
+    field), and the textbook 3x3 example worked by hand."""
+    a = np.ascontiguousarray(a, dtype=np.uint32)
+    r, rank, piv = rref_modp(a, p, nthreads=nthreads)
+    c = (a[:, piv].astype(np.uint64) % np.uint64(p)).astype(np.uint32)
+    return np.ascontiguousarray(c), np.ascontiguousarray(r[:rank]), piv
+
+
 def load_matrix_modp(bases: np.ndarray, lindices: np.ndarray, p: int) -> np.ndarray:
     """A[r][c] = prod_t bases[r][lindices[c][t]] mod p, the definition written out with plain
     numpy integer arithmetic, one factor at a time.  An index outside [0, n_basis) means "no factor" (the reading

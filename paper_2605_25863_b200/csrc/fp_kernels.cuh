@@ -124,6 +124,20 @@ __global__ void solve_extract_kernel(const uint32_t* __restrict__ R, int64_t ld,
 }
 
 // ------------------------------------------------------------------------------------------
+// Column basis of a rank factorisation A = C.R (eq. 7): C = A[:, J] with J the pivot columns,
+// entries reduced to [0,p).  Thread per pivot (J ascending, so a warp's reads fall in few sectors), grid.y over rows.
+__global__ void gather_columns_kernel(const uint32_t* __restrict__ A, int64_t lda, int64_t rows, int64_t rank,
+                                      const int32_t* __restrict__ piv, uint32_t* __restrict__ Cm, int64_t ldc, uint32_t p) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= rank) return;
+    const int64_t c = piv[k];
+    for (int64_t r = blockIdx.y; r < rows; r += gridDim.y) {
+        const uint32_t v = A[r * lda + c];
+        Cm[r * ldc + k] = v >= p ? v % p : v;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // cuda_load_matrix: A[r][c] = prod_t bases[r][lind[c][t]] mod p.  A CTA owns 256 columns
 // (their index lists staged once in shared memory) and walks over its share of the rows; the row of basis values is
 // staged per row, the 256 products are written as one coalesced row segment.  Bound: the 4 B written per element.

@@ -607,6 +607,42 @@ int linac_solve_u32(uint32_t* dM, int64_t rows, int64_t cols, int64_t nrhs, int6
     return LINAC_OK;
 }
 
+int linac_rank_factor_u32(const uint32_t* dA, int64_t rows, int64_t cols, int64_t lda, uint32_t p, void* stream,
+                          uint32_t* dR, int64_t ldr, uint32_t* dC, int64_t ldc, int64_t* rank, int32_t* pivot_cols_out) {
+    std::lock_guard<std::mutex> lock(g_call_mutex);
+    if (rows < 0 || cols < 0 || !rank) return LINAC_ERR_INVALID_ARG;
+    const int64_t cap = std::min(rows, cols);
+    if (rows > 0 && cols > 0 && (!dA || !dR || !dC || lda < cols || ldr < cols || ldc < cap)) return LINAC_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (rows > 0 && cols > 0) {
+        int rc = check_device();
+        if (rc) return rc;
+        LINAC_CUDA(cudaMemcpy2DAsync(dR, (size_t)ldr * 4, dA, (size_t)lda * 4, (size_t)cols * 4, (size_t)rows,
+                                     cudaMemcpyDeviceToDevice, s));
+    }
+    Arena arena;
+    std::vector<int32_t> piv((size_t)std::max<int64_t>(1, cap));
+    int64_t r = 0;
+    int rc = rref_impl(dR, rows, cols, ldr, p, s, &r, piv.data(), &arena);
+    if (rc) return rc;
+    *rank = r;
+    if (pivot_cols_out) std::copy(piv.begin(), piv.begin() + r, pivot_cols_out);
+    if (r == 0) return LINAC_OK;
+    int32_t* d_piv = nullptr;
+    LINAC_CUDA(cudaMalloc(&d_piv, (size_t)r * 4));
+    cudaError_t e = cudaMemcpyAsync(d_piv, piv.data(), (size_t)r * 4, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) {
+        dim3 grid((unsigned)((r + 255) / 256), (unsigned)std::min<int64_t>(rows, 148 * 8));
+        gather_columns_kernel<<<grid, 256, 0, s>>>(dA, lda, rows, r, d_piv, dC, ldc, p);
+        e = cudaGetLastError();
+        stats().kernel_launches++;
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    cudaFree(d_piv);
+    if (e != cudaSuccess) { set_cuda_error(e, "linac_rank_factor_u32", __FILE__, __LINE__); return LINAC_ERR_CUDA; }
+    return LINAC_OK;
+}
+
 int linac_load_matrix_u32(uint32_t* dA, int64_t n_rows, int64_t n_cols, int64_t ld, const uint32_t* dBases, int64_t n_basis,
                           int64_t ldb, const int32_t* dLindices, int64_t d, uint32_t p, void* stream) {
     std::lock_guard<std::mutex> lock(g_call_mutex);

@@ -21,7 +21,7 @@ ERR_SINGULAR, ERR_BUFFER_TOO_SMALL, ERR_UNSUPPORTED_DEVICE, ERR_INTERNAL = 5, 6,
 SYMBOLS = [
     "linac_status_string", "linac_last_cuda_error", "linac_version",
     "linac_rref_u32_workspace", "linac_solve_f64_workspace", "linac_set_workspace", "linac_release",
-    "linac_rref_u32", "linac_nullspace_u32", "linac_nullspace_from_rref_u32", "linac_solve_u32", "linac_load_matrix_u32", "linac_gemm_sub_u32",
+    "linac_rref_u32", "linac_nullspace_u32", "linac_nullspace_from_rref_u32", "linac_solve_u32", "linac_rank_factor_u32", "linac_load_matrix_u32", "linac_gemm_sub_u32",
     "linac_solve_f64",
     "linac_get_last_stats", "linac_set_option",
 ]
@@ -69,6 +69,7 @@ def _lib() -> C.CDLL:
         L.linac_nullspace_u32.argtypes = [vp, i64, i64, i64, u32, vp, C.POINTER(i64), vp, vp, i64, i64, C.POINTER(i64)]
         L.linac_nullspace_from_rref_u32.argtypes = [vp, i64, i64, i64, u32, i64, vp, vp, i64, vp]
         L.linac_solve_u32.argtypes = [vp, i64, i64, i64, i64, u32, vp, C.POINTER(i64), vp, vp, vp, i64]
+        L.linac_rank_factor_u32.argtypes = [vp, i64, i64, i64, u32, vp, vp, i64, vp, i64, C.POINTER(i64), vp]
         L.linac_load_matrix_u32.argtypes = [vp, i64, i64, i64, vp, i64, i64, vp, i64, u32, vp]
         L.linac_gemm_sub_u32.argtypes = [vp, i64, vp, i64, vp, i64, i64, i64, i64, u32, C.c_int, vp]
         L.linac_solve_f64.argtypes = [vp, i64, i64, vp, i64, i64, C.c_double, vp, C.POINTER(i64)]
@@ -215,6 +216,29 @@ def solve_u32(m: torch.Tensor, cols: int, p: int):
         if rc:
             raise LinacError(rc, "linac_solve_u32")
     return int(rank_a.value), piv, cons[:nrhs].bool(), x
+
+
+def rank_factor_u32(a: torch.Tensor, p: int):
+    """Rank factorisation A = C.R over F_p (eq. 7): `a` is left untouched.  Returns (rank, pivot_cols, C, R) with
+    C = a[:, pivot_cols] mod p (rows x rank) and R the non-zero rows of the RREF (rank x cols), both on the device
+    (views of freshly allocated buffers).  Mirrors linac_rank_factor_u32."""
+    rows, cols, ld = _check_matrix(a, _U32, "a")
+    cap = min(rows, cols)
+    with torch.cuda.device(a.device):
+        need = C.c_size_t(0)
+        _lib().linac_rref_u32_workspace(rows, cols, C.byref(need))
+        _ensure_workspace(need.value, a.device)
+        rank = C.c_int64(0)
+        piv = torch.empty(max(1, cap), dtype=torch.int32)
+        r = torch.empty((rows, cols), dtype=a.dtype, device=a.device)
+        c = torch.empty((rows, cap), dtype=a.dtype, device=a.device)
+        rc = _lib().linac_rank_factor_u32(a.data_ptr() if a.numel() else None, rows, cols, ld, p, _stream_ptr(a.device),
+                                          r.data_ptr() if r.numel() else None, max(cols, 1),
+                                          c.data_ptr() if c.numel() else None, max(cap, 1), C.byref(rank), piv.data_ptr())
+    if rc:
+        raise LinacError(rc, "linac_rank_factor_u32")
+    k = int(rank.value)
+    return k, piv[:k].clone(), c[:, :k], r[:k]
 
 
 def load_matrix_u32(bases: torch.Tensor, lindices: torch.Tensor, p: int, out: torch.Tensor | None = None) -> torch.Tensor:

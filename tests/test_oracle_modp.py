@@ -324,6 +324,43 @@ def test_solve_modp_against_brute_force_and_plain_products(oracle):
     assert not x2[free].any()
 
 
+# ------------------------------------------------------------------ rank_factor_modp (eq. 7)
+def test_rank_factor_modp_pins(oracle):
+    import itertools
+    # (1) worked by hand over F_7: row 2 = 2 x row 1; (1,0,1) - (1,2,3) = (0,5,5) -> x 3 = (0,1,1); (1,2,3) - 2(0,1,1) = (1,0,1)
+    a = np.array([[1, 2, 3], [2, 4, 6], [1, 0, 1]], dtype=np.uint32)
+    c, r, j = oracle.rank_factor_modp(a, 7)
+    assert list(j) == [0, 1]
+    assert np.array_equal(r, np.array([[1, 0, 1], [0, 1, 1]], dtype=np.uint32))
+    assert np.array_equal(c, np.array([[1, 2], [2, 4], [1, 0]], dtype=np.uint32))
+    # (2) tiny fields: C.R = A with plain integers, and C has full column rank by enumeration of all non-zero x
+    rng = np.random.default_rng(13)
+    for p, rows, cols in [(2, 5, 6), (3, 4, 5), (5, 4, 3), (2, 6, 4), (3, 5, 5)]:
+        for trial in range(10):
+            a = rng.integers(0, p, size=(rows, cols)).astype(np.uint32)
+            if trial % 2 == 0:
+                a[:, 1] = a[:, 0]
+                a[-1] = (a[0] + a[1]) % p
+            c, r, j = oracle.rank_factor_modp(a, p)
+            k = len(j)
+            assert c.shape == (rows, k) and r.shape == (k, cols)
+            assert np.array_equal((c.astype(np.int64) @ r.astype(np.int64)) % p, a.astype(np.int64))
+            if k:
+                allx = np.array(list(itertools.product(range(p), repeat=k)), dtype=np.int64).T[:, 1:]   # non-zero x
+                assert ((c.astype(np.int64) @ allx) % p != 0).any(axis=0).all()
+    # (3) a big prime, entries >= p on input, rank-deficient by construction: C.R = A mod p by the (big-int pinned) product
+    p = 2147483629
+    a, _, _ = gen.lowrank_factors(37, 9, 52, p, seed_b=21, seed_c=22)
+    a = a.copy()
+    a[3, 5] += p                                                    # still < 2^32; the same residue
+    c, r, j = oracle.rank_factor_modp(a, p)
+    assert len(j) == 9 and c.max() < p
+    assert np.array_equal(oracle.matmul_modp(c, r, p), a % np.uint32(p))
+    # zero matrix and empty shapes: rank 0, empty factors
+    c, r, j = oracle.rank_factor_modp(np.zeros((3, 4), dtype=np.uint32), 7)
+    assert c.shape == (3, 0) and r.shape == (0, 4) and len(j) == 0
+
+
 # ------------------------------------------------------------------ load_matrix_modp
 def test_load_matrix_modp_pins(oracle):
     rng = np.random.default_rng(12)
