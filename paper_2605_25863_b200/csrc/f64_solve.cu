@@ -314,23 +314,29 @@ __device__ __forceinline__ void dmma_8x8x4(double& c0, double& c1, double a, dou
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
                  : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
-__global__ void __launch_bounds__(256) dgemm_sub_mma_kernel(double* __restrict__ C, int64_t ldc,
+// TN = 128 (8 warps as 2 x 4, 64 x 32 warp tiles) or 64 (64 x 16 warp tiles: the skinny right-hand-side updates).
+// ASSIGN: C = A.B instead of C -= A.B; a CTA reads every B element of its column range before its epilogue, so
+// C may alias B when one CTA covers all M rows (the diagonal-block step of the blocked substitution).
+template <int TN, bool ASSIGN>
+__global__ void __launch_bounds__(256) dgemm_sub_mma_kernel(double* C, int64_t ldc,
                                                             const double* __restrict__ A, int64_t lda,
-                                                            const double* __restrict__ B, int64_t ldb, int64_t M,
+                                                            const double* B, int64_t ldb, int64_t M,
                                                             int64_t N, int64_t K) {
+    constexpr int NJ = TN / 32;                            // MMA tiles per warp along n
+    constexpr int BL = QK * TN / 256;                      // B elements per thread and stage
     __shared__ __align__(16) double As[2][QK][QLD];       // k-major
-    __shared__ __align__(16) double Bs[2][QK][QLD];
+    __shared__ __align__(16) double Bs[2][QK][TN + 4];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int wm0 = (warp >> 2) * 64, wn0 = (warp & 3) * 32;
+    const int wm0 = (warp >> 2) * 64, wn0 = (warp & 3) * (TN / 4);
     const int g = lane >> 2, q = lane & 3;                // fragment coordinates (PTX ISA, m8n8k4 .f64)
-    const int64_t m0 = (int64_t)blockIdx.y * DM, n0 = (int64_t)blockIdx.x * DN;
-    double acc[8][4][2];
+    const int64_t m0 = (int64_t)blockIdx.y * DM, n0 = (int64_t)blockIdx.x * TN;
+    double acc[8][NJ][2];
 #pragma unroll
     for (int i = 0; i < 8; ++i)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+        for (int j = 0; j < NJ; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-    double ra[4], rb[4];
+    double ra[4], rb[BL];
     auto gload = [&](int64_t k0) {
 #pragma unroll
         for (int t = 0; t < 4; ++t) {
@@ -338,7 +344,11 @@ __global__ void __launch_bounds__(256) dgemm_sub_mma_kernel(double* __restrict__
             const int kk = idx % QK, mm = idx / QK;
             const int64_t m = m0 + mm, k = k0 + kk;
             ra[t] = (m < M && k < K) ? A[m * lda + k] : 0.0;
-            const int nn = idx % DN, kb = idx / DN;
+        }
+#pragma unroll
+        for (int t = 0; t < BL; ++t) {
+            const int idx = tid + t * 256;
+            const int nn = idx % TN, kb = idx / TN;
             const int64_t n = n0 + nn, k2 = k0 + kb;
             rb[t] = (n < N && k2 < K) ? B[k2 * ldb + n] : 0.0;
         }
@@ -348,7 +358,11 @@ __global__ void __launch_bounds__(256) dgemm_sub_mma_kernel(double* __restrict__
         for (int t = 0; t < 4; ++t) {
             const int idx = tid + t * 256;
             As[buf][idx % QK][idx / QK] = ra[t];
-            Bs[buf][idx / DN][idx % DN] = rb[t];
+        }
+#pragma unroll
+        for (int t = 0; t < BL; ++t) {
+            const int idx = tid + t * 256;
+            Bs[buf][idx / TN][idx % TN] = rb[t];
         }
     };
     gload(0);
@@ -360,15 +374,15 @@ __global__ void __launch_bounds__(256) dgemm_sub_mma_kernel(double* __restrict__
         if (more) gload(k0 + QK);
 #pragma unroll
         for (int ks = 0; ks < QK; ks += 4) {
-            double a[8], b[4];
+            double a[8], b[NJ];
 #pragma unroll
             for (int i = 0; i < 8; ++i) a[i] = As[buf][ks + q][wm0 + i * 8 + g];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) b[j] = Bs[buf][ks + q][wn0 + j * 8 + g];
+            for (int j = 0; j < NJ; ++j) b[j] = Bs[buf][ks + q][wn0 + j * 8 + g];
 #pragma unroll
             for (int i = 0; i < 8; ++i)
 #pragma unroll
-                for (int j = 0; j < 4; ++j) dmma_8x8x4(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                for (int j = 0; j < NJ; ++j) dmma_8x8x4(acc[i][j][0], acc[i][j][1], a[i], b[j]);
         }
         if (more) {
             sstore(buf ^ 1);
@@ -376,15 +390,19 @@ __global__ void __launch_bounds__(256) dgemm_sub_mma_kernel(double* __restrict__
             buf ^= 1;
         }
     }
+    if (ASSIGN) __syncthreads();                           // every read of B (possibly = C) is done
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
         const int64_t m = m0 + wm0 + i * 8 + g;
         if (m >= M) continue;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
+        for (int j = 0; j < NJ; ++j) {
             const int64_t n = n0 + wn0 + j * 8 + q * 2;
             double* pc = C + m * ldc + n;
-            if (n + 1 < N && ((reinterpret_cast<uintptr_t>(pc) & 15) == 0)) {
+            if (ASSIGN) {
+                if (n < N) pc[0] = acc[i][j][0];
+                if (n + 1 < N) pc[1] = acc[i][j][1];
+            } else if (n + 1 < N && ((reinterpret_cast<uintptr_t>(pc) & 15) == 0)) {
                 double2 v = *reinterpret_cast<double2*>(pc);
                 v.x -= acc[i][j][0];
                 v.y -= acc[i][j][1];
@@ -397,27 +415,118 @@ __global__ void __launch_bounds__(256) dgemm_sub_mma_kernel(double* __restrict__
     }
 }
 
+// ---------------------------------------------------------------- F3: inverses of the diagonal blocks
+// Blocked substitution on the right-hand sides (F3) with explicit inverses of the TB x TB diagonal blocks of L and
+// U: X_t = inv(D_t).B_t is then a tensor-pipe product instead of a chain of dependent leaf solves.  One CTA per
+// block, thread j owns column j of the inverse (kept in shared memory), L/U entries are warp-uniform loads.
+constexpr int TB = 128;
+template <bool LOWER>
+__global__ void __launch_bounds__(TB) f64_tri_inv_kernel(const double* __restrict__ A, int64_t n, int64_t lda,
+                                                         double* __restrict__ inv /* [blocks][TB][TB] */) {
+    extern __shared__ double XS[];                        // [TB][TB + 1]
+    constexpr int LX = TB + 1;
+    const int j = threadIdx.x;
+    const int64_t t0 = (int64_t)blockIdx.x * TB;
+    const int nb = (int)min((int64_t)TB, n - t0);
+    const double* D = A + t0 * lda + t0;
+    double* out = inv + (size_t)blockIdx.x * TB * TB;
+    if (LOWER) {
+        if (j < nb) {
+            XS[j * LX + j] = 1.0;
+            for (int i = j + 1; i < nb; ++i) {
+                double s0 = 0.0, s1 = 0.0;
+                int qq = j;
+                for (; qq + 1 < i; qq += 2) {
+                    s0 += D[(int64_t)i * lda + qq] * XS[qq * LX + j];
+                    s1 += D[(int64_t)i * lda + qq + 1] * XS[(qq + 1) * LX + j];
+                }
+                if (qq < i) s0 += D[(int64_t)i * lda + qq] * XS[qq * LX + j];
+                XS[i * LX + j] = -(s0 + s1);
+            }
+        }
+    } else {
+        if (j < nb) {
+            XS[j * LX + j] = 1.0 / D[(int64_t)j * lda + j];
+            for (int i = j - 1; i >= 0; --i) {
+                double s0 = 0.0, s1 = 0.0;
+                int qq = i + 1;
+                for (; qq + 1 <= j; qq += 2) {
+                    s0 += D[(int64_t)i * lda + qq] * XS[qq * LX + j];
+                    s1 += D[(int64_t)i * lda + qq + 1] * XS[(qq + 1) * LX + j];
+                }
+                if (qq <= j) s0 += D[(int64_t)i * lda + qq] * XS[qq * LX + j];
+                XS[i * LX + j] = -(s0 + s1) / D[(int64_t)i * lda + i];
+            }
+        }
+    }
+    __syncthreads();
+    for (int e = j; e < TB * TB; e += TB) {
+        const int r = e / TB, c = e % TB;
+        const bool tri = LOWER ? (c <= r) : (c >= r);
+        out[e] = (r < nb && c < nb && tri) ? XS[r * LX + c] : 0.0;
+    }
+}
+
 struct F64 {
     double* A; int64_t n, lda;
     double* B; int64_t nrhs, ldb;
     double tol;
     cudaStream_t s;
     Cand* cand; double* target; long long* ipiv; int* info;
+    double* inv;                // inverted diagonal blocks of L and U (F3)
     int grid, rows_cap;         // cooperative grid size and the smem row capacity per CTA
     size_t smem_max;
 };
 
 int dgemm_sub(F64& c, double* C, int64_t ldc, const double* A, int64_t lda, const double* B, int64_t ldb, int64_t M,
-              int64_t N, int64_t K) {
+              int64_t N, int64_t K, bool assign = false) {
     if (M <= 0 || N <= 0 || K <= 0) return LINAC_OK;
-    dim3 grid((unsigned)((N + DN - 1) / DN), (unsigned)((M + DM - 1) / DM));
-    if (options().f64_mma != 0)
-        dgemm_sub_mma_kernel<<<grid, 256, 0, c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
-    else
+    const bool skinny = N <= 64 || assign;
+    const int tn = skinny ? 64 : DN;
+    dim3 grid((unsigned)((N + tn - 1) / tn), (unsigned)((M + DM - 1) / DM));
+    if (assign)
+        dgemm_sub_mma_kernel<64, true><<<grid, 256, 0, c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
+    else if (options().f64_mma == 0)
         dgemm_sub_kernel<<<grid, DTHREADS, 0, c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
+    else if (skinny)
+        dgemm_sub_mma_kernel<64, false><<<grid, 256, 0, c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
+    else
+        dgemm_sub_mma_kernel<128, false><<<grid, 256, 0, c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
     LINAC_CUDA(cudaGetLastError());
     stats().kernel_launches++;
     stats().update_macs += M * N * K;
+    return LINAC_OK;
+}
+
+// F3: B <- U^{-1} L^{-1} B by blocks of TB rows with the inverted diagonal blocks: X_t = inv(D_t).B_t (one CTA per 64
+// right-hand sides, in place), then B_rest -= A[rest, t].X_t on the tensor pipe.
+int solve_rhs_f64(F64& c) {
+    const int64_t nblk = (c.n + TB - 1) / TB;
+    const size_t smem = (size_t)TB * (TB + 1) * sizeof(double);
+    LINAC_CUDA(cudaFuncSetAttribute(f64_tri_inv_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    LINAC_CUDA(cudaFuncSetAttribute(f64_tri_inv_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    double* invL = c.inv;
+    double* invU = c.inv + (size_t)nblk * TB * TB;
+    f64_tri_inv_kernel<true><<<(unsigned)nblk, TB, smem, c.s>>>(c.A, c.n, c.lda, invL);
+    f64_tri_inv_kernel<false><<<(unsigned)nblk, TB, smem, c.s>>>(c.A, c.n, c.lda, invU);
+    LINAC_CUDA(cudaGetLastError());
+    stats().kernel_launches += 2;
+    for (int64_t t = 0; t < nblk; ++t) {                                  // forward: L
+        const int64_t t0 = t * TB, nb = std::min<int64_t>(TB, c.n - t0);
+        double* Bt = c.B + t0 * c.ldb;
+        int rc = dgemm_sub(c, Bt, c.ldb, invL + (size_t)t * TB * TB, TB, Bt, c.ldb, nb, c.nrhs, nb, true);
+        if (rc) return rc;
+        rc = dgemm_sub(c, Bt + nb * c.ldb, c.ldb, c.A + (t0 + nb) * c.lda + t0, c.lda, Bt, c.ldb, c.n - t0 - nb, c.nrhs, nb);
+        if (rc) return rc;
+    }
+    for (int64_t t = nblk - 1; t >= 0; --t) {                             // backward: U
+        const int64_t t0 = t * TB, nb = std::min<int64_t>(TB, c.n - t0);
+        double* Bt = c.B + t0 * c.ldb;
+        int rc = dgemm_sub(c, Bt, c.ldb, invU + (size_t)t * TB * TB, TB, Bt, c.ldb, nb, c.nrhs, nb, true);
+        if (rc) return rc;
+        rc = dgemm_sub(c, c.B, c.ldb, c.A + t0, c.lda, Bt, c.ldb, t0, c.nrhs, nb);
+        if (rc) return rc;
+    }
     return LINAC_OK;
 }
 
@@ -496,7 +605,8 @@ int factor_f64(F64& c, int64_t j0, int64_t j1) {
 
 size_t f64_workspace_bytes(int64_t n) {
     (void)n;
-    return 4096 + 2 * 1024 * sizeof(Cand) + 2 * FW * sizeof(double) + (size_t)std::max<int64_t>(n, 1) * 8 + 1024;
+    const size_t inv = 2 * (size_t)((n + TB - 1) / TB) * TB * TB * sizeof(double);
+    return 8192 + 2 * 1024 * sizeof(Cand) + 2 * FW * sizeof(double) + (size_t)std::max<int64_t>(n, 1) * 8 + 1024 + inv;
 }
 
 }  // namespace
@@ -544,7 +654,8 @@ int linac_solve_f64(double* dA, int64_t n, int64_t lda, double* dB, int64_t nrhs
     c.target = (double*)arena.take(2 * FW * sizeof(double));
     c.ipiv = (long long*)arena.take((size_t)n * 8);
     c.info = (int*)arena.take(256);
-    if (!c.cand || !c.target || !c.ipiv || !c.info) return LINAC_ERR_WORKSPACE;
+    c.inv = nrhs > 0 ? (double*)arena.take(2 * (size_t)((n + TB - 1) / TB) * TB * TB * sizeof(double)) : nullptr;
+    if (!c.cand || !c.target || !c.ipiv || !c.info || (nrhs > 0 && !c.inv)) return LINAC_ERR_WORKSPACE;
     const int big = INT_MAX;
     LINAC_CUDA(cudaMemcpyAsync(c.info, &big, sizeof(int), cudaMemcpyHostToDevice, s));
 
@@ -557,8 +668,13 @@ int linac_solve_f64(double* dA, int64_t n, int64_t lda, double* dB, int64_t nrhs
     st.kernel_launches++;
     // F2 with B as trailing columns: factor A in outer blocks so B's forward substitution is blocked too
     rc = factor_f64(c, 0, n);
-    if (rc == LINAC_OK && nrhs > 0) rc = trsm_lower_f64(c, dB, ldb, nrhs, 0, n);              // forward substitution (L)
-    if (rc == LINAC_OK && nrhs > 0) rc = trsm_upper_f64(c, dB, ldb, nrhs, 0, n);              // F3 back substitution (U)
+    if (rc == LINAC_OK && nrhs > 0) {
+        if (options().f64_rhs_inv != 0) rc = solve_rhs_f64(c);                                // F3, blocked with inverses
+        else {
+            rc = trsm_lower_f64(c, dB, ldb, nrhs, 0, n);                                      // forward substitution (L)
+            if (rc == LINAC_OK) rc = trsm_upper_f64(c, dB, ldb, nrhs, 0, n);                  // back substitution (U)
+        }
+    }
     int h_info = INT_MAX;
     if (rc == LINAC_OK) {
         cudaEventRecord(e1, s);
