@@ -70,6 +70,9 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
     __shared__ int s_idx[FTHREADS / 32];
     __shared__ double pv[FW];
     __shared__ long long s_g;
+    __shared__ double c_val[FTHREADS / 32];
+    __shared__ long long c_row[FTHREADS / 32];
+    __shared__ int c_cta[FTHREADS / 32];
     cg::grid_group grid = cg::this_grid();
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
     const int G = gridDim.x, b = blockIdx.x;
@@ -79,6 +82,27 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
 
     for (int k = wq; k < nr; k += FTHREADS / 32) S[k * LDS + lane] = lane < w ? A[(r0 + k) * lda + j0 + lane] : 0.0;
     __syncthreads();
+
+    // second half of publishing column c: the warps' arg-max values are in s_val/s_idx (after a __syncthreads)
+    auto publish_tail = [&](int c) {
+        const int64_t jc = j0 + c;
+        if (wq == 0) {
+            double best = lane < FTHREADS / 32 ? s_val[lane] : -1.0;
+            int bi = lane < FTHREADS / 32 ? s_idx[lane] : -1;
+            for (int o = 4; o; o >>= 1) {
+                const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+                const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+                if (ov > best || (ov == best && oi >= 0 && (bi < 0 || oi < bi))) { best = ov; bi = oi; }
+            }
+            bi = __shfl_sync(0xffffffffu, bi, 0);
+            best = __shfl_sync(0xffffffffu, best, 0);
+            Cand* cd = cand + (size_t)(c & 1) * G + b;
+            if (lane == 0) { cd->absval = best; cd->row = bi >= 0 ? r0 + bi : -1; }
+            if (bi >= 0) cd->content[lane] = S[bi * LDS + lane];
+            if (jc >= r0 && jc < r0 + nr) target[(c & 1) * FW + lane] = S[(int)(jc - r0) * LDS + lane];
+        }
+        __syncthreads();
+    };
 
     // publish the candidate for column c among own rows with absolute index >= j0 + c, and row j0+c itself
     auto publish = [&](int c) {
@@ -97,34 +121,20 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
         }
         if (lane == 0) { s_val[wq] = best; s_idx[wq] = bi; }
         __syncthreads();
-        if (wq == 0) {
-            best = lane < FTHREADS / 32 ? s_val[lane] : -1.0;
-            bi = lane < FTHREADS / 32 ? s_idx[lane] : -1;
-            for (int o = 4; o; o >>= 1) {
-                const double ov = __shfl_xor_sync(0xffffffffu, best, o);
-                const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-                if (ov > best || (ov == best && oi >= 0 && (bi < 0 || oi < bi))) { best = ov; bi = oi; }
-            }
-            bi = __shfl_sync(0xffffffffu, bi, 0);
-            best = __shfl_sync(0xffffffffu, best, 0);
-            Cand* cd = cand + (size_t)(c & 1) * G + b;
-            if (lane == 0) { cd->absval = best; cd->row = bi >= 0 ? r0 + bi : -1; }
-            if (bi >= 0) cd->content[lane] = S[bi * LDS + lane];
-            if (jc >= r0 && jc < r0 + nr) target[(c & 1) * FW + lane] = S[(int)(jc - r0) * LDS + lane];
-        }
-        __syncthreads();
+        publish_tail(c);
     };
 
     publish(0);
     for (int c = 0; c < w; ++c) {
         grid.sync();
         const int64_t jc = j0 + c;
-        // every CTA reduces the G candidates identically: largest |value|, lowest row on ties (reading Q12)
-        if (wq == 0) {
+        // every CTA reduces the G candidates identically: largest |value|, lowest row on ties (reading Q12).
+        // One candidate per thread (a single round trip to L2), then warp and block reduction.
+        {
             double best = -1.0;
             long long brow = -1;
             int bcta = -1;
-            for (int q = lane; q < G; q += 32) {
+            for (int q = tid; q < G; q += FTHREADS) {
                 const Cand* cd = cand + (size_t)(c & 1) * G + q;
                 const double v = __ldcg(&cd->absval);
                 const long long rr = __ldcg(&cd->row);
@@ -136,6 +146,22 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
                 const int oc = __shfl_xor_sync(0xffffffffu, bcta, o);
                 if (orow >= 0 && (ov > best || (ov == best && (brow < 0 || orow < brow)))) { best = ov; brow = orow; bcta = oc; }
             }
+            if (lane == 0) { c_val[wq] = best; c_row[wq] = brow; c_cta[wq] = bcta; }
+        }
+        __syncthreads();
+        if (wq == 0) {
+            double best = lane < FTHREADS / 32 ? c_val[lane] : -1.0;
+            long long brow = lane < FTHREADS / 32 ? c_row[lane] : -1;
+            int bcta = lane < FTHREADS / 32 ? c_cta[lane] : -1;
+            for (int o = 4; o; o >>= 1) {
+                const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+                const long long orow = __shfl_xor_sync(0xffffffffu, brow, o);
+                const int oc = __shfl_xor_sync(0xffffffffu, bcta, o);
+                if (orow >= 0 && (ov > best || (ov == best && (brow < 0 || orow < brow)))) { best = ov; brow = orow; bcta = oc; }
+            }
+            best = __shfl_sync(0xffffffffu, best, 0);
+            brow = __shfl_sync(0xffffffffu, brow, 0);
+            bcta = __shfl_sync(0xffffffffu, bcta, 0);
             pv[lane] = __ldcg(&cand[(size_t)(c & 1) * G + bcta].content[lane]);
             if (lane == 0) {
                 s_g = brow;
@@ -155,15 +181,26 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
         __syncthreads();
         double piv = pv[c];
         if (!(fabs(piv) > tol)) piv = 1.0;              // singular: flagged above; keep the arithmetic finite
-        // multipliers and rank-1 update of own rows below jc: one warp per row, lane = column
+        const double rp = 1.0 / piv;
+        // multipliers and rank-1 update of own rows below jc: one warp per row, lane = column.  Lane c+1 sees the
+        // new entries of the next column as they are made and keeps their arg-max (lowest row on ties).
+        double best = -1.0;
+        int bi = -1;
         for (int k = wq; k < nr; k += FTHREADS / 32) {
             if (r0 + k <= jc) continue;
-            const double l = S[k * LDS + c] / piv;
+            const double l = S[k * LDS + c] * rp;
             if (lane == c) S[k * LDS + c] = l;
-            else if (lane > c && lane < w) S[k * LDS + lane] -= l * pv[lane];
+            else if (lane > c && lane < w) {
+                const double v = S[k * LDS + lane] - l * pv[lane];
+                S[k * LDS + lane] = v;
+                if (lane == c + 1 && fabs(v) > best) { best = fabs(v); bi = k; }
+            }
         }
-        __syncthreads();
-        if (c + 1 < w) publish(c + 1);
+        if (c + 1 < w) {
+            if (lane == c + 1) { s_val[wq] = best; s_idx[wq] = bi; }
+            __syncthreads();
+            publish_tail(c + 1);
+        }
     }
     for (int k = wq; k < nr; k += FTHREADS / 32)
         if (lane < w) A[(r0 + k) * lda + j0 + lane] = S[k * LDS + lane];
