@@ -242,6 +242,29 @@ __global__ void __launch_bounds__(FT) f64_trsm_lower_kernel(double* __restrict__
     }
 }
 
+// The full-width leaf (nb = 32) with the column of X in registers: right-looking order, so the 31 - q updates that
+// follow x[q] are independent (the dot-product order above is one dependent chain per entry), L read as broadcasts.
+constexpr int FT2 = 64;
+__global__ void __launch_bounds__(FT2) f64_trsm_lower32_kernel(double* __restrict__ X, int64_t ldx, int64_t ncols,
+                                                               const double* __restrict__ A, int64_t lda, int64_t t0) {
+    __shared__ __align__(16) double Lt[FW][FW + 2];        // Lt[q][a] = L[a][q]
+    const int tid = threadIdx.x;
+    for (int e = tid; e < FW * FW; e += FT2) Lt[e & 31][e >> 5] = A[(t0 + (e >> 5)) * lda + t0 + (e & 31)];
+    __syncthreads();
+    const int64_t c = (int64_t)blockIdx.x * FT2 + tid;
+    if (c >= ncols) return;
+    double x[FW];
+#pragma unroll
+    for (int a = 0; a < FW; ++a) x[a] = X[(int64_t)a * ldx + c];
+#pragma unroll
+    for (int q = 0; q < FW - 1; ++q) {
+#pragma unroll
+        for (int a = q + 1; a < FW; ++a) x[a] -= Lt[q][a] * x[q];
+    }
+#pragma unroll
+    for (int a = 1; a < FW; ++a) X[(int64_t)a * ldx + c] = x[a];
+}
+
 // X <- U11^{-1} X, U11 upper nb x nb (non-unit) at A[t0:t0+nb, t0:t0+nb].
 __global__ void __launch_bounds__(FT) f64_trsm_upper_kernel(double* __restrict__ X, int64_t ldx, int64_t ncols,
                                                             const double* __restrict__ A, int64_t lda, int64_t t0, int nb) {
@@ -571,7 +594,10 @@ int solve_rhs_f64(F64& c) {
 int trsm_lower_f64(F64& c, double* X, int64_t ldx, int64_t ncols, int64_t t0, int64_t nb) {
     if (nb <= 0 || ncols <= 0) return LINAC_OK;
     if (nb <= FW) {
-        f64_trsm_lower_kernel<<<(unsigned)((ncols + FT - 1) / FT), FT, 0, c.s>>>(X, ldx, ncols, c.A, c.lda, t0, (int)nb);
+        if (nb == FW)
+            f64_trsm_lower32_kernel<<<(unsigned)((ncols + FT2 - 1) / FT2), FT2, 0, c.s>>>(X, ldx, ncols, c.A, c.lda, t0);
+        else
+            f64_trsm_lower_kernel<<<(unsigned)((ncols + FT - 1) / FT), FT, 0, c.s>>>(X, ldx, ncols, c.A, c.lda, t0, (int)nb);
         LINAC_CUDA(cudaGetLastError());
         stats().kernel_launches++;
         return LINAC_OK;
@@ -640,6 +666,26 @@ int factor_f64(F64& c, int64_t j0, int64_t j1) {
     return factor_f64(c, jm, j1);
 }
 
+// Top level: a flat right-looking sweep over strips of `f64_strip` columns (each factored by the recursion above, then
+// one U12 solve and ONE full-size trailing update with K = strip width), so that the bulk of the flops runs in
+// square, many-tile DMMA launches instead of the recursion's skinny mid-level products.
+int factor_flat_f64(F64& c) {
+    const int64_t W = options().f64_strip;
+    if (W <= 0 || c.n <= W) return factor_f64(c, 0, c.n);
+    for (int64_t s0 = 0; s0 < c.n; s0 += W) {
+        const int64_t s1 = std::min(c.n, s0 + W);
+        int rc = factor_f64(c, s0, s1);
+        if (rc) return rc;
+        if (s1 >= c.n) break;
+        rc = trsm_lower_f64(c, c.A + s0 * c.lda + s1, c.lda, c.n - s1, s0, s1 - s0);
+        if (rc) return rc;
+        rc = dgemm_sub(c, c.A + s1 * c.lda + s1, c.lda, c.A + s1 * c.lda + s0, c.lda, c.A + s0 * c.lda + s1, c.lda,
+                       c.n - s1, c.n - s1, s1 - s0);
+        if (rc) return rc;
+    }
+    return LINAC_OK;
+}
+
 size_t f64_workspace_bytes(int64_t n) {
     (void)n;
     const size_t inv = 2 * (size_t)((n + TB - 1) / TB) * TB * TB * sizeof(double);
@@ -704,7 +750,7 @@ int linac_solve_f64(double* dA, int64_t n, int64_t lda, double* dB, int64_t nrhs
     LINAC_CUDA(cudaGetLastError());
     st.kernel_launches++;
     // F2 with B as trailing columns: factor A in outer blocks so B's forward substitution is blocked too
-    rc = factor_f64(c, 0, n);
+    rc = factor_flat_f64(c);
     if (rc == LINAC_OK && nrhs > 0) {
         if (options().f64_rhs_inv != 0) rc = solve_rhs_f64(c);                                // F3, blocked with inverses
         else {
