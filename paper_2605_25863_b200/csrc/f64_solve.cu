@@ -368,7 +368,7 @@ __global__ void __launch_bounds__(DTHREADS) dgemm_sub_kernel(double* __restrict_
 // as 2 x 4, a 64 x 32 warp tile = 8 x 4 MMA tiles.  Operands come from shared memory one double per thread and
 // per fragment, so a k-step costs 12 LDS.64 per 32 MMAs: five times less shared-memory traffic per flop than the
 // 8 x 8 register tile of the DFMA kernel above, which was co-bound by the shared-memory pipe.
-constexpr int QK = 8;                     // k per shared-memory stage
+constexpr int QK = 16;                    // k per shared-memory stage
 constexpr int QLD = DM + 4;               // row stride in doubles: = 4 mod 16, conflict-free fragment loads
 __device__ __forceinline__ void dmma_8x8x4(double& c0, double& c1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
@@ -384,8 +384,10 @@ __global__ void __launch_bounds__(256) dgemm_sub_mma_kernel(double* C, int64_t l
                                                             int64_t N, int64_t K) {
     constexpr int NJ = TN / 32;                            // MMA tiles per warp along n
     constexpr int BL = QK * TN / 256;                      // B elements per thread and stage
-    __shared__ __align__(16) double As[2][QK][QLD];       // k-major
-    __shared__ __align__(16) double Bs[2][QK][TN + 4];
+    extern __shared__ __align__(16) double dq_smem[];
+    double (*As)[QK][QLD] = reinterpret_cast<double (*)[QK][QLD]>(dq_smem);                       // [2], k-major
+    double (*Bs)[QK][TN + 4] = reinterpret_cast<double (*)[QK][TN + 4]>(dq_smem + 2 * QK * QLD);  // [2]
+    constexpr int AL = QK * DM / 256;                      // A elements per thread and stage
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wm0 = (warp >> 2) * 64, wn0 = (warp & 3) * (TN / 4);
     const int g = lane >> 2, q = lane & 3;                // fragment coordinates (PTX ISA, m8n8k4 .f64)
@@ -396,10 +398,10 @@ __global__ void __launch_bounds__(256) dgemm_sub_mma_kernel(double* C, int64_t l
 #pragma unroll
         for (int j = 0; j < NJ; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-    double ra[4], rb[BL];
+    double ra[AL], rb[BL];
     auto gload = [&](int64_t k0) {
 #pragma unroll
-        for (int t = 0; t < 4; ++t) {
+        for (int t = 0; t < AL; ++t) {
             const int idx = tid + t * 256;
             const int kk = idx % QK, mm = idx / QK;
             const int64_t m = m0 + mm, k = k0 + kk;
@@ -415,7 +417,7 @@ __global__ void __launch_bounds__(256) dgemm_sub_mma_kernel(double* C, int64_t l
     };
     auto sstore = [&](int buf) {
 #pragma unroll
-        for (int t = 0; t < 4; ++t) {
+        for (int t = 0; t < AL; ++t) {
             const int idx = tid + t * 256;
             As[buf][idx % QK][idx / QK] = ra[t];
         }
@@ -527,6 +529,8 @@ __global__ void __launch_bounds__(TB) f64_tri_inv_kernel(const double* __restric
     }
 }
 
+constexpr size_t dmma_smem_bytes(int tn) { return (size_t)(2 * QK * QLD + 2 * QK * (tn + 4)) * sizeof(double); }
+
 struct F64 {
     double* A; int64_t n, lda;
     double* B; int64_t nrhs, ldb;
@@ -545,13 +549,13 @@ int dgemm_sub(F64& c, double* C, int64_t ldc, const double* A, int64_t lda, cons
     const int tn = skinny ? 64 : DN;
     dim3 grid((unsigned)((N + tn - 1) / tn), (unsigned)((M + DM - 1) / DM));
     if (assign)
-        dgemm_sub_mma_kernel<64, true><<<grid, 256, 0, c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
+        dgemm_sub_mma_kernel<64, true><<<grid, 256, dmma_smem_bytes(64), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
     else if (options().f64_mma == 0)
         dgemm_sub_kernel<<<grid, DTHREADS, 0, c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
     else if (skinny)
-        dgemm_sub_mma_kernel<64, false><<<grid, 256, 0, c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
+        dgemm_sub_mma_kernel<64, false><<<grid, 256, dmma_smem_bytes(64), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
     else
-        dgemm_sub_mma_kernel<128, false><<<grid, 256, 0, c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
+        dgemm_sub_mma_kernel<128, false><<<grid, 256, dmma_smem_bytes(128), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
     LINAC_CUDA(cudaGetLastError());
     stats().kernel_launches++;
     stats().update_macs += M * N * K;
@@ -733,6 +737,9 @@ int linac_solve_f64(double* dA, int64_t n, int64_t lda, double* dB, int64_t nrhs
     c.rows_cap = (int)(c.smem_max / ((FW + 1) * sizeof(double)));
     if ((n + c.grid - 1) / c.grid > c.rows_cap) return LINAC_ERR_INVALID_ARG;   // n > ~118k: strip no longer fits on chip
     LINAC_CUDA(cudaFuncSetAttribute(f64_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max));
+    LINAC_CUDA(cudaFuncSetAttribute(dgemm_sub_mma_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dmma_smem_bytes(128)));
+    LINAC_CUDA(cudaFuncSetAttribute(dgemm_sub_mma_kernel<64, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dmma_smem_bytes(64)));
+    LINAC_CUDA(cudaFuncSetAttribute(dgemm_sub_mma_kernel<64, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dmma_smem_bytes(64)));
     c.cand = (Cand*)arena.take(2 * 1024 * sizeof(Cand));
     c.target = (double*)arena.take(2 * FW * sizeof(double));
     c.ipiv = (long long*)arena.take((size_t)n * 8);
