@@ -370,6 +370,12 @@ __global__ void __launch_bounds__(DTHREADS) dgemm_sub_kernel(double* __restrict_
 // 8 x 8 register tile of the DFMA kernel above, which was co-bound by the shared-memory pipe.
 constexpr int QK = 16;                    // k per shared-memory stage
 constexpr int QLD = DM + 4;               // row stride in doubles: = 4 mod 16, conflict-free fragment loads
+constexpr int QNS = 3;                    // cp.async stages
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc, bool valid) {
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    const int bytes = valid ? 8 : 0;                   // src-size 0: the 8 bytes are zero-filled, nothing is read
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(d), "l"(gsrc), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void dmma_8x8x4(double& c0, double& c1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
                  : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
@@ -377,84 +383,77 @@ __device__ __forceinline__ void dmma_8x8x4(double& c0, double& c1, double a, dou
 // TN = 128 (8 warps as 2 x 4, 64 x 32 warp tiles) or 64 (64 x 16 warp tiles: the skinny right-hand-side updates).
 // ASSIGN: C = A.B instead of C -= A.B; a CTA reads every B element of its column range before its epilogue, so
 // C may alias B when one CTA covers all M rows (the diagonal-block step of the blocked substitution).
-template <int TN, bool ASSIGN>
-__global__ void __launch_bounds__(256) dgemm_sub_mma_kernel(double* C, int64_t ldc,
+template <int TN, bool ASSIGN, int NW>
+__global__ void __launch_bounds__(NW * 32, 1) dgemm_sub_mma_kernel(double* C, int64_t ldc,
                                                             const double* __restrict__ A, int64_t lda,
                                                             const double* B, int64_t ldb, int64_t M,
                                                             int64_t N, int64_t K) {
     constexpr int NJ = TN / 32;                            // MMA tiles per warp along n
-    constexpr int BL = QK * TN / 256;                      // B elements per thread and stage
+    constexpr int NT = NW * 32;                            // threads: 8 warps as 2 x 4 (16 as 4 x 4 measured no faster)
+    constexpr int MI = 64 / NW;                            // MMA tiles per warp along m (warp tile 64 or 32 rows)
+    constexpr int BL = QK * TN / NT;                       // B elements per thread and stage
     extern __shared__ __align__(16) double dq_smem[];
-    double (*As)[QK][QLD] = reinterpret_cast<double (*)[QK][QLD]>(dq_smem);                       // [2], k-major
-    double (*Bs)[QK][TN + 4] = reinterpret_cast<double (*)[QK][TN + 4]>(dq_smem + 2 * QK * QLD);  // [2]
-    constexpr int AL = QK * DM / 256;                      // A elements per thread and stage
+    double (*As)[QK][QLD] = reinterpret_cast<double (*)[QK][QLD]>(dq_smem);                       // [QNS], k-major
+    double (*Bs)[QK][TN + 4] = reinterpret_cast<double (*)[QK][TN + 4]>(dq_smem + QNS * QK * QLD);  // [QNS]
+    constexpr int AL = QK * DM / NT;                      // A elements per thread and stage
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int wm0 = (warp >> 2) * 64, wn0 = (warp & 3) * (TN / 4);
+    const int wm0 = (warp >> 2) * (MI * 8), wn0 = (warp & 3) * (TN / 4);
     const int g = lane >> 2, q = lane & 3;                // fragment coordinates (PTX ISA, m8n8k4 .f64)
     const int64_t m0 = (int64_t)blockIdx.y * DM, n0 = (int64_t)blockIdx.x * TN;
-    double acc[8][NJ][2];
+    double acc[MI][NJ][2];
 #pragma unroll
-    for (int i = 0; i < 8; ++i)
+    for (int i = 0; i < MI; ++i)
 #pragma unroll
         for (int j = 0; j < NJ; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-    double ra[AL], rb[BL];
-    auto gload = [&](int64_t k0) {
+    // QNS-stage cp.async ring: 8-byte copies scatter A into the k-major tile, zero-fill outside the matrix
+    auto issue = [&](int64_t k0, int buf) {
 #pragma unroll
         for (int t = 0; t < AL; ++t) {
-            const int idx = tid + t * 256;
+            const int idx = tid + t * NT;
             const int kk = idx % QK, mm = idx / QK;
             const int64_t m = m0 + mm, k = k0 + kk;
-            ra[t] = (m < M && k < K) ? A[m * lda + k] : 0.0;
+            const bool ok = m < M && k < K;
+            cp_async8(&As[buf][kk][mm], ok ? A + m * lda + k : A, ok);
         }
 #pragma unroll
         for (int t = 0; t < BL; ++t) {
-            const int idx = tid + t * 256;
+            const int idx = tid + t * NT;
             const int nn = idx % TN, kb = idx / TN;
             const int64_t n = n0 + nn, k2 = k0 + kb;
-            rb[t] = (n < N && k2 < K) ? B[k2 * ldb + n] : 0.0;
+            const bool ok = n < N && k2 < K;
+            cp_async8(&Bs[buf][kb][nn], ok ? B + k2 * ldb + n : B, ok);
         }
     };
-    auto sstore = [&](int buf) {
+    const int64_t nk = (K + QK - 1) / QK;
 #pragma unroll
-        for (int t = 0; t < AL; ++t) {
-            const int idx = tid + t * 256;
-            As[buf][idx % QK][idx / QK] = ra[t];
-        }
-#pragma unroll
-        for (int t = 0; t < BL; ++t) {
-            const int idx = tid + t * 256;
-            Bs[buf][idx / TN][idx % TN] = rb[t];
-        }
-    };
-    gload(0);
-    sstore(0);
-    __syncthreads();
-    int buf = 0;
-    for (int64_t k0 = 0; k0 < K; k0 += QK) {
-        const bool more = k0 + QK < K;
-        if (more) gload(k0 + QK);
+    for (int st = 0; st < QNS - 1; ++st) {
+        if (st < nk) issue((int64_t)st * QK, st);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
+    for (int64_t kt = 0; kt < nk; ++kt) {
+        asm volatile("cp.async.wait_group %0;" ::"n"(QNS - 2) : "memory");
+        __syncthreads();                                   // stage kt has landed; stage kt-1's buffer is free
+        if (kt + QNS - 1 < nk) issue((kt + QNS - 1) * QK, (int)((kt + QNS - 1) % QNS));
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        const int buf = (int)(kt % QNS);
 #pragma unroll
         for (int ks = 0; ks < QK; ks += 4) {
-            double a[8], b[NJ];
+            double a[MI], b[NJ];
 #pragma unroll
-            for (int i = 0; i < 8; ++i) a[i] = As[buf][ks + q][wm0 + i * 8 + g];
+            for (int i = 0; i < MI; ++i) a[i] = As[buf][ks + q][wm0 + i * 8 + g];
 #pragma unroll
             for (int j = 0; j < NJ; ++j) b[j] = Bs[buf][ks + q][wn0 + j * 8 + g];
 #pragma unroll
-            for (int i = 0; i < 8; ++i)
+            for (int i = 0; i < MI; ++i)
 #pragma unroll
                 for (int j = 0; j < NJ; ++j) dmma_8x8x4(acc[i][j][0], acc[i][j][1], a[i], b[j]);
         }
-        if (more) {
-            sstore(buf ^ 1);
-            __syncthreads();
-            buf ^= 1;
-        }
     }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
     if (ASSIGN) __syncthreads();                           // every read of B (possibly = C) is done
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
+    for (int i = 0; i < MI; ++i) {
         const int64_t m = m0 + wm0 + i * 8 + g;
         if (m >= M) continue;
 #pragma unroll
@@ -529,7 +528,7 @@ __global__ void __launch_bounds__(TB) f64_tri_inv_kernel(const double* __restric
     }
 }
 
-constexpr size_t dmma_smem_bytes(int tn) { return (size_t)(2 * QK * QLD + 2 * QK * (tn + 4)) * sizeof(double); }
+constexpr size_t dmma_smem_bytes(int tn) { return (size_t)(QNS * QK * QLD + QNS * QK * (tn + 4)) * sizeof(double); }
 
 struct F64 {
     double* A; int64_t n, lda;
@@ -549,13 +548,13 @@ int dgemm_sub(F64& c, double* C, int64_t ldc, const double* A, int64_t lda, cons
     const int tn = skinny ? 64 : DN;
     dim3 grid((unsigned)((N + tn - 1) / tn), (unsigned)((M + DM - 1) / DM));
     if (assign)
-        dgemm_sub_mma_kernel<64, true><<<grid, 256, dmma_smem_bytes(64), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
+        dgemm_sub_mma_kernel<64, true, 8><<<grid, 256, dmma_smem_bytes(64), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
     else if (options().f64_mma == 0)
         dgemm_sub_kernel<<<grid, DTHREADS, 0, c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
     else if (skinny)
-        dgemm_sub_mma_kernel<64, false><<<grid, 256, dmma_smem_bytes(64), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
+        dgemm_sub_mma_kernel<64, false, 8><<<grid, 256, dmma_smem_bytes(64), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
     else
-        dgemm_sub_mma_kernel<128, false><<<grid, 256, dmma_smem_bytes(128), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
+        dgemm_sub_mma_kernel<128, false, 8><<<grid, 256, dmma_smem_bytes(128), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
     LINAC_CUDA(cudaGetLastError());
     stats().kernel_launches++;
     stats().update_macs += M * N * K;
@@ -737,9 +736,9 @@ int linac_solve_f64(double* dA, int64_t n, int64_t lda, double* dB, int64_t nrhs
     c.rows_cap = (int)(c.smem_max / ((FW + 1) * sizeof(double)));
     if ((n + c.grid - 1) / c.grid > c.rows_cap) return LINAC_ERR_INVALID_ARG;   // n > ~118k: strip no longer fits on chip
     LINAC_CUDA(cudaFuncSetAttribute(f64_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max));
-    LINAC_CUDA(cudaFuncSetAttribute(dgemm_sub_mma_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dmma_smem_bytes(128)));
-    LINAC_CUDA(cudaFuncSetAttribute(dgemm_sub_mma_kernel<64, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dmma_smem_bytes(64)));
-    LINAC_CUDA(cudaFuncSetAttribute(dgemm_sub_mma_kernel<64, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dmma_smem_bytes(64)));
+    LINAC_CUDA(cudaFuncSetAttribute(dgemm_sub_mma_kernel<128, false, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dmma_smem_bytes(128)));
+    LINAC_CUDA(cudaFuncSetAttribute(dgemm_sub_mma_kernel<64, false, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dmma_smem_bytes(64)));
+    LINAC_CUDA(cudaFuncSetAttribute(dgemm_sub_mma_kernel<64, true, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dmma_smem_bytes(64)));
     c.cand = (Cand*)arena.take(2 * 1024 * sizeof(Cand));
     c.target = (double*)arena.take(2 * FW * sizeof(double));
     c.ipiv = (long long*)arena.take((size_t)n * 8);
