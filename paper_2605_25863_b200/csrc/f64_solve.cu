@@ -26,7 +26,6 @@ extern std::mutex g_call_mutex;
 namespace {
 
 constexpr int FW = 32;              // panel width
-constexpr int FTHREADS = 256;       // panel kernel block size
 
 // ---------------------------------------------------------------- F1
 // One block per row: s = max_c |A[r,c]| over A's columns (reading Q11), then A[r,:] /= s, B[r,:] /= s.
@@ -58,8 +57,13 @@ struct Cand {                 // one CTA's arg-max candidate for a column, with 
     double content[FW];
 };
 
-// Cooperative kernel: factors A[j0:n, j0:j0+w) in place (unit-lower L below, U on and above the
+// CLUSTER = false: cooperative kernel, one CTA per SM, grid barrier and candidate records in global memory (L2).
+// CLUSTER = true: ONE thread-block cluster of up to 16 CTAs holds the strip; the per-column barrier is the hardware
+// cluster barrier and the candidate records are read from the peers' shared memory (DSMEM), which cuts the
+// per-column latency from two L2 round trips and a grid barrier to about a microsecond.
+// Factors A[j0:n, j0:j0+w) in place (unit-lower L below, U on and above the
 // diagonal), records the exchanges in ipiv[j0..j0+w).  CTA b owns rows [j0 + b*R, j0 + (b+1)*R).
+template <int FTHREADS, bool CLUSTER>
 __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict__ A, int64_t n, int64_t lda, int64_t j0,
                                                               int w, int rows_per_cta, double tol,
                                                               Cand* __restrict__ cand /* [2][gridDim] */,
@@ -73,9 +77,20 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
     __shared__ double c_val[FTHREADS / 32];
     __shared__ long long c_row[FTHREADS / 32];
     __shared__ int c_cta[FTHREADS / 32];
-    cg::grid_group grid = cg::this_grid();
+    __shared__ Cand l_cand[2];                          // CLUSTER: this CTA's records, read by the peers
+    __shared__ double l_target[2][FW];
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
-    const int G = gridDim.x, b = blockIdx.x;
+    int G = gridDim.x, b = blockIdx.x;
+    if constexpr (CLUSTER) { G = (int)cg::this_cluster().num_blocks(); b = (int)cg::this_cluster().block_rank(); }
+    auto group_sync = [&]() {
+        if constexpr (CLUSTER) cg::this_cluster().sync(); else cg::this_grid().sync();
+    };
+    auto cand_of = [&](int c, int q) -> const Cand* {   // CTA q's record for column c
+        if constexpr (CLUSTER) return cg::this_cluster().map_shared_rank(&l_cand[c & 1], q);
+        else return cand + (size_t)(c & 1) * G + q;
+    };
+    auto ld_f = [&](const double* p) { if constexpr (CLUSTER) return *p; else return __ldcg(p); };
+    auto ld_i = [&](const long long* p) { if constexpr (CLUSTER) return *p; else return __ldcg(p); };
     const int64_t r0 = j0 + (int64_t)b * rows_per_cta;
     const int nr = (int)max((int64_t)0, min((int64_t)rows_per_cta, n - r0));
     constexpr int LDS = FW + 1;
@@ -89,17 +104,17 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
         if (wq == 0) {
             double best = lane < FTHREADS / 32 ? s_val[lane] : -1.0;
             int bi = lane < FTHREADS / 32 ? s_idx[lane] : -1;
-            for (int o = 4; o; o >>= 1) {
+            for (int o = 16; o; o >>= 1) {
                 const double ov = __shfl_xor_sync(0xffffffffu, best, o);
                 const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
                 if (ov > best || (ov == best && oi >= 0 && (bi < 0 || oi < bi))) { best = ov; bi = oi; }
             }
             bi = __shfl_sync(0xffffffffu, bi, 0);
             best = __shfl_sync(0xffffffffu, best, 0);
-            Cand* cd = cand + (size_t)(c & 1) * G + b;
+            Cand* cd = CLUSTER ? &l_cand[c & 1] : cand + (size_t)(c & 1) * G + b;
             if (lane == 0) { cd->absval = best; cd->row = bi >= 0 ? r0 + bi : -1; }
             if (bi >= 0) cd->content[lane] = S[bi * LDS + lane];
-            if (jc >= r0 && jc < r0 + nr) target[(c & 1) * FW + lane] = S[(int)(jc - r0) * LDS + lane];
+            if (jc >= r0 && jc < r0 + nr) (CLUSTER ? l_target[c & 1] : target + (c & 1) * FW)[lane] = S[(int)(jc - r0) * LDS + lane];
         }
         __syncthreads();
     };
@@ -126,7 +141,7 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
 
     publish(0);
     for (int c = 0; c < w; ++c) {
-        grid.sync();
+        group_sync();
         const int64_t jc = j0 + c;
         // every CTA reduces the G candidates identically: largest |value|, lowest row on ties (reading Q12).
         // One candidate per thread (a single round trip to L2), then warp and block reduction.
@@ -135,9 +150,9 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
             long long brow = -1;
             int bcta = -1;
             for (int q = tid; q < G; q += FTHREADS) {
-                const Cand* cd = cand + (size_t)(c & 1) * G + q;
-                const double v = __ldcg(&cd->absval);
-                const long long rr = __ldcg(&cd->row);
+                const Cand* cd = cand_of(c, q);
+                const double v = ld_f(&cd->absval);
+                const long long rr = ld_i(&cd->row);
                 if (rr >= 0 && (v > best || (v == best && rr < brow))) { best = v; brow = rr; bcta = q; }
             }
             for (int o = 16; o; o >>= 1) {
@@ -153,7 +168,7 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
             double best = lane < FTHREADS / 32 ? c_val[lane] : -1.0;
             long long brow = lane < FTHREADS / 32 ? c_row[lane] : -1;
             int bcta = lane < FTHREADS / 32 ? c_cta[lane] : -1;
-            for (int o = 4; o; o >>= 1) {
+            for (int o = 16; o; o >>= 1) {
                 const double ov = __shfl_xor_sync(0xffffffffu, best, o);
                 const long long orow = __shfl_xor_sync(0xffffffffu, brow, o);
                 const int oc = __shfl_xor_sync(0xffffffffu, bcta, o);
@@ -162,7 +177,7 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
             best = __shfl_sync(0xffffffffu, best, 0);
             brow = __shfl_sync(0xffffffffu, brow, 0);
             bcta = __shfl_sync(0xffffffffu, bcta, 0);
-            pv[lane] = __ldcg(&cand[(size_t)(c & 1) * G + bcta].content[lane]);
+            pv[lane] = ld_f(&cand_of(c, bcta)->content[lane]);
             if (lane == 0) {
                 s_g = brow;
                 if (b == 0) {
@@ -175,7 +190,11 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
         const long long g = s_g;
         // exchange rows jc and g (content of row jc comes from `target`, pivot row from `pv`)
         if (g != jc) {
-            if (g >= r0 && g < r0 + nr && tid < FW) S[(int)(g - r0) * LDS + tid] = __ldcg(&target[(c & 1) * FW + tid]);
+            if (g >= r0 && g < r0 + nr && tid < FW) {
+                const double* tg = target + (c & 1) * FW;
+                if constexpr (CLUSTER) tg = cg::this_cluster().map_shared_rank(&l_target[c & 1][0], (int)((jc - j0) / rows_per_cta));
+                S[(int)(g - r0) * LDS + tid] = ld_f(tg + tid);
+            }
         }
         if (jc >= r0 && jc < r0 + nr && tid < FW) S[(int)(jc - r0) * LDS + tid] = pv[tid];
         __syncthreads();
@@ -204,6 +223,7 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
     }
     for (int k = wq; k < nr; k += FTHREADS / 32)
         if (lane < w) A[(r0 + k) * lda + j0 + lane] = S[k * LDS + lane];
+    if constexpr (CLUSTER) cg::this_cluster().sync();   // no CTA may leave while a peer can still read its records
 }
 
 // Row exchanges of one panel applied to whole rows outside the panel columns; one thread per column.
@@ -538,6 +558,8 @@ struct F64 {
     Cand* cand; double* target; long long* ipiv; int* info;
     double* inv;                // inverted diagonal blocks of L and U (F3)
     int grid, rows_cap;         // cooperative grid size and the smem row capacity per CTA
+    int panel_threads;
+    int cluster_ctas;           // CTAs of the panel cluster (0: cluster launch not available)
     size_t smem_max;
 };
 
@@ -638,7 +660,28 @@ int panel_f64(F64& c, int64_t j0, int w) {
     double* A = c.A; int64_t n = c.n, lda = c.lda; double tol = c.tol;
     Cand* cand = c.cand; double* target = c.target; long long* ipiv = c.ipiv; int* info = c.info;
     void* args[] = {&A, &n, &lda, &j0, &w, &rows_per_cta, &tol, &cand, &target, &ipiv, &info};
-    LINAC_CUDA(cudaLaunchCooperativeKernel((void*)f64_panel_kernel, dim3(c.grid), dim3(FTHREADS), args, smem, c.s));
+    if (c.cluster_ctas > 0 && m <= (int64_t)c.cluster_ctas * std::min<int64_t>(c.rows_cap, options().f64_cluster_rows)) {
+        rows_per_cta = std::max(1, (int)((m + c.cluster_ctas - 1) / c.cluster_ctas));
+        smem = (size_t)rows_per_cta * (FW + 1) * sizeof(double);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(c.cluster_ctas);
+        cfg.blockDim = dim3(512);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = c.s;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)c.cluster_ctas;
+        at[0].val.clusterDim.y = 1;
+        at[0].val.clusterDim.z = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
+        LINAC_CUDA(cudaLaunchKernelEx(&cfg, f64_panel_kernel<512, true>, A, n, lda, j0, w, rows_per_cta, tol, cand, target, ipiv, info));
+    } else if (c.panel_threads == 1024)
+        LINAC_CUDA(cudaLaunchCooperativeKernel((void*)f64_panel_kernel<1024, false>, dim3(c.grid), dim3(1024), args, smem, c.s));
+    else if (c.panel_threads == 512)
+        LINAC_CUDA(cudaLaunchCooperativeKernel((void*)f64_panel_kernel<512, false>, dim3(c.grid), dim3(512), args, smem, c.s));
+    else
+        LINAC_CUDA(cudaLaunchCooperativeKernel((void*)f64_panel_kernel<256, false>, dim3(c.grid), dim3(256), args, smem, c.s));
     // exchanges on the rest of A (left L part and right trailing part) and on B
     const int64_t ncol = c.n;
     f64_swap_kernel<<<(unsigned)((ncol + 255) / 256), 256, 0, c.s>>>(c.A, c.lda, 0, ncol, j0, j0 + w, c.ipiv, j0, w);
@@ -732,10 +775,38 @@ int linac_solve_f64(double* dA, int64_t n, int64_t lda, double* dB, int64_t nrhs
     LINAC_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     LINAC_CUDA(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
     c.grid = std::min(sms, 1024);
+    c.panel_threads = (int)options().f64_panel_threads;
+    if (options().f64_panel_grid > 0) c.grid = (int)std::min<int64_t>(sms, options().f64_panel_grid);
     c.smem_max = (size_t)smem_optin - 4096;
     c.rows_cap = (int)(c.smem_max / ((FW + 1) * sizeof(double)));
     if ((n + c.grid - 1) / c.grid > c.rows_cap) return LINAC_ERR_INVALID_ARG;   // n > ~118k: strip no longer fits on chip
-    LINAC_CUDA(cudaFuncSetAttribute(f64_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max));
+    LINAC_CUDA(cudaFuncSetAttribute(f64_panel_kernel<256, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max));
+    LINAC_CUDA(cudaFuncSetAttribute(f64_panel_kernel<512, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max));
+    LINAC_CUDA(cudaFuncSetAttribute(f64_panel_kernel<1024, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max));
+    c.cluster_ctas = 0;
+    if (options().f64_panel_cluster > 0) {                 // one cluster of up to 16 CTAs (non-portable size), if the device places it
+        const int want = (int)options().f64_panel_cluster;
+        cudaError_t ce = cudaFuncSetAttribute(f64_panel_kernel<512, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max);
+        if (ce == cudaSuccess && want > 8)
+            ce = cudaFuncSetAttribute(f64_panel_kernel<512, true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        if (ce == cudaSuccess) {
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3(want);
+            cfg.blockDim = dim3(512);
+            cfg.dynamicSmemBytes = c.smem_max;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension;
+            at[0].val.clusterDim.x = (unsigned)want;
+            at[0].val.clusterDim.y = 1;
+            at[0].val.clusterDim.z = 1;
+            cfg.attrs = at;
+            cfg.numAttrs = 1;
+            int nclusters = 0;
+            ce = cudaOccupancyMaxActiveClusters(&nclusters, f64_panel_kernel<512, true>, &cfg);
+            if (ce == cudaSuccess && nclusters >= 1) c.cluster_ctas = want;
+        }
+        if (ce != cudaSuccess) (void)cudaGetLastError();    // not available: the cooperative kernel does every panel
+    }
     LINAC_CUDA(cudaFuncSetAttribute(dgemm_sub_mma_kernel<128, false, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dmma_smem_bytes(128)));
     LINAC_CUDA(cudaFuncSetAttribute(dgemm_sub_mma_kernel<64, false, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dmma_smem_bytes(64)));
     LINAC_CUDA(cudaFuncSetAttribute(dgemm_sub_mma_kernel<64, true, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dmma_smem_bytes(64)));

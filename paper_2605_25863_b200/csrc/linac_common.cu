@@ -178,6 +178,18 @@ int linac_set_option(const char* name, int64_t value) {
     } else if (!strcmp(name, "f64_strip")) {
         if (value < 0 || (value > 0 && value % 32 != 0)) return LINAC_ERR_INVALID_ARG;
         g_options.f64_strip = value;
+    } else if (!strcmp(name, "f64_panel_threads")) {
+        if (value != 256 && value != 512 && value != 1024) return LINAC_ERR_INVALID_ARG;
+        g_options.f64_panel_threads = value;
+    } else if (!strcmp(name, "f64_panel_grid")) {
+        if (value < 0 || value > 1024) return LINAC_ERR_INVALID_ARG;
+        g_options.f64_panel_grid = value;
+    } else if (!strcmp(name, "f64_panel_cluster")) {
+        if (value < 0 || value > 16 || (value & (value - 1))) return LINAC_ERR_INVALID_ARG;
+        g_options.f64_panel_cluster = value;
+    } else if (!strcmp(name, "f64_cluster_rows")) {
+        if (value < 1) return LINAC_ERR_INVALID_ARG;
+        g_options.f64_cluster_rows = value;
     } else if (!strcmp(name, "f64_rhs_inv")) {
         if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
         g_options.f64_rhs_inv = value;

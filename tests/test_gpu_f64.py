@@ -103,3 +103,28 @@ def test_medium_size_several_panels_and_recursion_levels(oracle):
     assert oracle.backward_error(a, x, b, nthreads=oracle.max_threads()) <= ETA_MAX
     ref = np.linalg.solve(a, b)
     assert np.allclose(x, ref, rtol=1e-9, atol=1e-12)
+
+
+@pytest.mark.parametrize("opts", [
+    {"f64_strip": 0}, {"f64_strip": 256}, {"f64_rhs_inv": 0}, {"f64_mma": 0},
+    {"f64_panel_threads": 256}, {"f64_panel_threads": 1024},
+    {"f64_panel_cluster": 16, "f64_cluster_rows": 4096}, {"f64_panel_cluster": 8, "f64_cluster_rows": 100},
+])
+def test_schedule_options_solve_the_same_system(oracle, opts):
+    """Every schedule (pure recursion / flat strips, recursive / inverse-block substitution, DFMA / DMMA update, the
+    panel kernel's block sizes, the cluster + DSMEM panel kernel) on a matrix that needs row exchanges, with a
+    ragged size and more than 64 right-hand sides."""
+    import paper_2605_25863_b200 as L
+    defaults = {"f64_strip": 1024, "f64_rhs_inv": 1, "f64_mma": 1, "f64_panel_threads": 512, "f64_panel_cluster": 0,
+                "f64_cluster_rows": 128}
+    n, nrhs = 1337, 70
+    a, b = gen.normal_matrix(n, n, seed=21), gen.normal_matrix(n, nrhs, seed=22)
+    try:
+        for k, v in opts.items():
+            L.set_option(k, v)
+        x = gpu_solve(a, b)
+    finally:
+        for k, v in defaults.items():
+            L.set_option(k, v)
+    assert oracle.backward_error(a, x, b, nthreads=oracle.max_threads()) <= ETA_MAX
+    assert np.allclose(x, np.linalg.solve(a, b), rtol=1e-7, atol=1e-10)
