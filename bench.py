@@ -140,7 +140,8 @@ def f64_leg(torch, L, dev, n=16384, nrhs=64, reps=3):
     flop = 2.0 * n ** 3 / 3.0 + 2.0 * n * n * nrhs
     return {"workload": f"c4: {n}x{n} float64 N(0,1) + 4 sqrt(N) I, {nrhs} right-hand sides (torch generator, seed 5)",
             "ms_per_solve": ms, "gflops": flop / ms / 1e6, "backward_error": eta, "backward_error_bound": 1e-11,
-            "note": "flop = 2N^3/3 + 2N^2 nrhs; trailing update on the FP64 tensor pipe (DMMA m8n8k4)"}
+            "note": "flop = 2N^3/3 + 2N^2 nrhs; trailing update on the FP64 tensor pipe (DMMA m8n8k4), substitution with "
+                    "inverted 128 x 128 diagonal blocks"}
 
 
 def run_reference(args):
@@ -181,6 +182,8 @@ def main():
     ap.add_argument("--ref-n", type=int, default=1280, help="sample size for the oracle legs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-f64", action="store_true", help="skip the fp64 leg (config c4) of the default run")
+    ap.add_argument("--fp64-only", action="store_true",
+                    help="run only the fp64 leg (config c4) and print {\"fp64\": ...}; the command of the fp64 launch list")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
                     help="library tunable for A/B runs (linac_set_option), e.g. --opt strip_width=256")
     args = ap.parse_args()
@@ -200,6 +203,13 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
+    if args.fp64_only:
+        for kv in args.opt:
+            name, _, val = kv.partition("=")
+            L.set_option(name, int(val))
+        if rank == 0:
+            print(json.dumps({"fp64": f64_leg(torch, L, dev, reps=max(1, min(args.steps, 5)))}))
+        return
 
     from paper_2605_25863_b200 import replicas
     on_device = gen.CONFIGS[args.workload]["kind"] == "sparse_dep"     # c5: 40 GB, generated straight into HBM
