@@ -57,6 +57,26 @@ struct Cand {                 // one CTA's arg-max candidate for a column, with 
     double content[FW];
 };
 
+// Warp arg-max of non-negative doubles with the lowest index winning ties, on the redux.sync unit: the bit pattern of
+// a non-negative double orders like the number, so the maximum is two 32-bit max-reductions (high word, then low word
+// among the lanes that hold the maximal high word) and the tie-break one min-reduction -- about ten instructions
+// instead of five shuffle rounds on three 64-bit values.  A lane takes part iff idx >= 0 (then v >= 0); every lane
+// returns the winner's (v, idx, aux), idx = -1 if no lane took part.
+__device__ __forceinline__ void warp_argmax(double& v, int& idx, int& aux) {
+    const bool has = idx >= 0;
+    const unsigned hi = has ? (unsigned)__double2hiint(v) : 0u;
+    const unsigned lo = has ? (unsigned)__double2loint(v) : 0u;
+    const unsigned mh = __reduce_max_sync(0xffffffffu, hi);
+    const unsigned ml = __reduce_max_sync(0xffffffffu, hi == mh ? lo : 0u);
+    const unsigned key = (has && hi == mh && lo == ml) ? (unsigned)idx : 0xffffffffu;
+    const unsigned mk = __reduce_min_sync(0xffffffffu, key);
+    if (mk == 0xffffffffu) { v = -1.0; idx = -1; aux = -1; return; }
+    const int who = __ffs(__ballot_sync(0xffffffffu, key == mk)) - 1;
+    v = __hiloint2double((int)mh, (int)ml);
+    idx = (int)mk;
+    aux = __shfl_sync(0xffffffffu, aux, who);
+}
+
 // CLUSTER = false: cooperative kernel, one CTA per SM, grid barrier and candidate records in global memory (L2).
 // CLUSTER = true: ONE thread-block cluster of up to 16 CTAs holds the strip; the per-column barrier is the hardware
 // cluster barrier and the candidate records are read from the peers' shared memory (DSMEM), which cuts the
@@ -103,14 +123,8 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
         const int64_t jc = j0 + c;
         if (wq == 0) {
             double best = lane < FTHREADS / 32 ? s_val[lane] : -1.0;
-            int bi = lane < FTHREADS / 32 ? s_idx[lane] : -1;
-            for (int o = 16; o; o >>= 1) {
-                const double ov = __shfl_xor_sync(0xffffffffu, best, o);
-                const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-                if (ov > best || (ov == best && oi >= 0 && (bi < 0 || oi < bi))) { best = ov; bi = oi; }
-            }
-            bi = __shfl_sync(0xffffffffu, bi, 0);
-            best = __shfl_sync(0xffffffffu, best, 0);
+            int bi = lane < FTHREADS / 32 ? s_idx[lane] : -1, none = 0;
+            warp_argmax(best, bi, none);
             Cand* cd = CLUSTER ? &l_cand[c & 1] : cand + (size_t)(c & 1) * G + b;
             if (lane == 0) { cd->absval = best; cd->row = bi >= 0 ? r0 + bi : -1; }
             if (bi >= 0) cd->content[lane] = S[bi * LDS + lane];
@@ -129,11 +143,8 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
             const double v = fabs(S[k * LDS + c]);
             if (v > best) { best = v; bi = k; }          // strict >: lowest index wins inside a thread
         }
-        for (int o = 16; o; o >>= 1) {
-            const double ov = __shfl_xor_sync(0xffffffffu, best, o);
-            const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-            if (ov > best || (ov == best && oi >= 0 && (bi < 0 || oi < bi))) { best = ov; bi = oi; }
-        }
+        int none = 0;
+        warp_argmax(best, bi, none);
         if (lane == 0) { s_val[wq] = best; s_idx[wq] = bi; }
         __syncthreads();
         publish_tail(c);
@@ -147,37 +158,24 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
         // One candidate per thread (a single round trip to L2), then warp and block reduction.
         {
             double best = -1.0;
-            long long brow = -1;
-            int bcta = -1;
+            int brow = -1, bcta = -1;
             for (int q = tid; q < G; q += FTHREADS) {
                 const Cand* cd = cand_of(c, q);
                 const double v = ld_f(&cd->absval);
-                const long long rr = ld_i(&cd->row);
-                if (rr >= 0 && (v > best || (v == best && rr < brow))) { best = v; brow = rr; bcta = q; }
+                const int rr = (int)ld_i(&cd->row);
+                if (rr >= 0 && (brow < 0 || v > best || (v == best && rr < brow))) { best = v; brow = rr; bcta = q; }
             }
-            for (int o = 16; o; o >>= 1) {
-                const double ov = __shfl_xor_sync(0xffffffffu, best, o);
-                const long long orow = __shfl_xor_sync(0xffffffffu, brow, o);
-                const int oc = __shfl_xor_sync(0xffffffffu, bcta, o);
-                if (orow >= 0 && (ov > best || (ov == best && (brow < 0 || orow < brow)))) { best = ov; brow = orow; bcta = oc; }
-            }
+            warp_argmax(best, brow, bcta);
             if (lane == 0) { c_val[wq] = best; c_row[wq] = brow; c_cta[wq] = bcta; }
         }
         __syncthreads();
         if (wq == 0) {
             double best = lane < FTHREADS / 32 ? c_val[lane] : -1.0;
-            long long brow = lane < FTHREADS / 32 ? c_row[lane] : -1;
+            int brow = lane < FTHREADS / 32 ? (int)c_row[lane] : -1;
             int bcta = lane < FTHREADS / 32 ? c_cta[lane] : -1;
-            for (int o = 16; o; o >>= 1) {
-                const double ov = __shfl_xor_sync(0xffffffffu, best, o);
-                const long long orow = __shfl_xor_sync(0xffffffffu, brow, o);
-                const int oc = __shfl_xor_sync(0xffffffffu, bcta, o);
-                if (orow >= 0 && (ov > best || (ov == best && (brow < 0 || orow < brow)))) { best = ov; brow = orow; bcta = oc; }
-            }
-            best = __shfl_sync(0xffffffffu, best, 0);
-            brow = __shfl_sync(0xffffffffu, brow, 0);
-            bcta = __shfl_sync(0xffffffffu, bcta, 0);
-            pv[lane] = ld_f(&cand_of(c, bcta)->content[lane]);
+            warp_argmax(best, brow, bcta);
+            pv[lane] = bcta >= 0 ? ld_f(&cand_of(c, bcta)->content[lane]) : 0.0;   // no candidate (a column of NaNs): flagged below
+            if (brow < 0) brow = (int)jc;
             if (lane == 0) {
                 s_g = brow;
                 if (b == 0) {
