@@ -94,9 +94,6 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
     __shared__ int s_idx[FTHREADS / 32];
     __shared__ double pv[FW];
     __shared__ long long s_g;
-    __shared__ double c_val[FTHREADS / 32];
-    __shared__ long long c_row[FTHREADS / 32];
-    __shared__ int c_cta[FTHREADS / 32];
     __shared__ Cand l_cand[2];                          // CLUSTER: this CTA's records, read by the peers
     __shared__ double l_target[2][FW];
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
@@ -155,24 +152,32 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
         group_sync();
         const int64_t jc = j0 + c;
         // every CTA reduces the G candidates identically: largest |value|, lowest row on ties (reading Q12).
-        // One candidate per thread (a single round trip to L2), then warp and block reduction.
-        {
+        // Warp 0 alone: up to CPL candidates per lane, their loads all in flight together (one round trip), one
+        // warp arg-max, then the winner's row content (the second round trip).
+        if (wq == 0) {
+            constexpr int CPL = 5;                         // 160 candidates per pass (148 CTAs on a B200)
             double best = -1.0;
             int brow = -1, bcta = -1;
-            for (int q = tid; q < G; q += FTHREADS) {
-                const Cand* cd = cand_of(c, q);
-                const double v = ld_f(&cd->absval);
-                const int rr = (int)ld_i(&cd->row);
-                if (rr >= 0 && (brow < 0 || v > best || (v == best && rr < brow))) { best = v; brow = rr; bcta = q; }
+            for (int q0 = 0; q0 < G; q0 += 32 * CPL) {
+                double v[CPL];
+                int rr[CPL];
+#pragma unroll
+                for (int u = 0; u < CPL; ++u) {
+                    const int q = q0 + u * 32 + lane;
+                    v[u] = -1.0;
+                    rr[u] = -1;
+                    if (q < G) {
+                        const Cand* cd = cand_of(c, q);
+                        v[u] = ld_f(&cd->absval);
+                        rr[u] = (int)ld_i(&cd->row);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < CPL; ++u)
+                    if (rr[u] >= 0 && (brow < 0 || v[u] > best || (v[u] == best && rr[u] < brow))) {
+                        best = v[u]; brow = rr[u]; bcta = q0 + u * 32 + lane;
+                    }
             }
-            warp_argmax(best, brow, bcta);
-            if (lane == 0) { c_val[wq] = best; c_row[wq] = brow; c_cta[wq] = bcta; }
-        }
-        __syncthreads();
-        if (wq == 0) {
-            double best = lane < FTHREADS / 32 ? c_val[lane] : -1.0;
-            int brow = lane < FTHREADS / 32 ? (int)c_row[lane] : -1;
-            int bcta = lane < FTHREADS / 32 ? c_cta[lane] : -1;
             warp_argmax(best, brow, bcta);
             pv[lane] = bcta >= 0 ? ld_f(&cand_of(c, bcta)->content[lane]) : 0.0;   // no candidate (a column of NaNs): flagged below
             if (brow < 0) brow = (int)jc;
@@ -198,7 +203,7 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
         __syncthreads();
         double piv = pv[c];
         if (!(fabs(piv) > tol)) piv = 1.0;              // singular: flagged above; keep the arithmetic finite
-        const double rp = 1.0 / piv;
+        const double rp = __drcp_rn(piv);
         // multipliers and rank-1 update of own rows below jc: one warp per row, lane = column.  Lane c+1 sees the
         // new entries of the next column as they are made and keeps their arg-max (lowest row on ties).
         double best = -1.0;
