@@ -93,7 +93,6 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
     __shared__ double s_val[FTHREADS / 32];
     __shared__ int s_idx[FTHREADS / 32];
     __shared__ double pv[FW];
-    __shared__ long long s_g;
     __shared__ Cand l_cand[2];                          // CLUSTER: this CTA's records, read by the peers
     __shared__ double l_target[2][FW];
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
@@ -127,8 +126,7 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
             if (bi >= 0) cd->content[lane] = S[bi * LDS + lane];
             if (jc >= r0 && jc < r0 + nr) (CLUSTER ? l_target[c & 1] : target + (c & 1) * FW)[lane] = S[(int)(jc - r0) * LDS + lane];
         }
-        __syncthreads();
-    };
+    };                                                      // always followed by group_sync(), which is a block barrier too
 
     // publish the candidate for column c among own rows with absolute index >= j0 + c, and row j0+c itself
     auto publish = [&](int c) {
@@ -181,25 +179,20 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
             warp_argmax(best, brow, bcta);
             pv[lane] = bcta >= 0 ? ld_f(&cand_of(c, bcta)->content[lane]) : 0.0;   // no candidate (a column of NaNs): flagged below
             if (brow < 0) brow = (int)jc;
-            if (lane == 0) {
-                s_g = brow;
-                if (b == 0) {
-                    ipiv[jc] = brow;
-                    if (!(best > tol)) atomicMin(info, (int)min((int64_t)INT_MAX, jc + 1));
-                }
+            if (lane == 0 && b == 0) {
+                ipiv[jc] = brow;
+                if (!(best > tol)) atomicMin(info, (int)min((int64_t)INT_MAX, jc + 1));
             }
-        }
-        __syncthreads();
-        const long long g = s_g;
-        // exchange rows jc and g (content of row jc comes from `target`, pivot row from `pv`)
-        if (g != jc) {
-            if (g >= r0 && g < r0 + nr && tid < FW) {
+            __syncwarp();
+            // exchange rows jc and g = brow (content of row jc comes from `target`, the pivot row from `pv`)
+            const long long g = brow;
+            if (g != jc && g >= r0 && g < r0 + nr) {
                 const double* tg = target + (c & 1) * FW;
                 if constexpr (CLUSTER) tg = cg::this_cluster().map_shared_rank(&l_target[c & 1][0], (int)((jc - j0) / rows_per_cta));
-                S[(int)(g - r0) * LDS + tid] = ld_f(tg + tid);
+                S[(int)(g - r0) * LDS + lane] = ld_f(tg + lane);
             }
+            if (jc >= r0 && jc < r0 + nr) S[(int)(jc - r0) * LDS + lane] = pv[lane];
         }
-        if (jc >= r0 && jc < r0 + nr && tid < FW) S[(int)(jc - r0) * LDS + tid] = pv[tid];
         __syncthreads();
         double piv = pv[c];
         if (!(fabs(piv) > tol)) piv = 1.0;              // singular: flagged above; keep the arithmetic finite
@@ -208,8 +201,9 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
         // new entries of the next column as they are made and keeps their arg-max (lowest row on ties).
         double best = -1.0;
         int bi = -1;
-        for (int k = wq; k < nr; k += FTHREADS / 32) {
-            if (r0 + k <= jc) continue;
+        const int kmin = (int)max((int64_t)0, min((int64_t)nr, jc + 1 - r0));   // own rows below the pivot row
+#pragma unroll 2
+        for (int k = kmin + wq; k < nr; k += FTHREADS / 32) {
             const double l = S[k * LDS + c] * rp;
             if (lane == c) S[k * LDS + c] = l;
             else if (lane > c && lane < w) {
@@ -224,6 +218,7 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
             publish_tail(c + 1);
         }
     }
+    __syncthreads();                                        // the last column's updates (rows change warps per column)
     for (int k = wq; k < nr; k += FTHREADS / 32)
         if (lane < w) A[(r0 + k) * lda + j0 + lane] = S[k * LDS + lane];
     if constexpr (CLUSTER) cg::this_cluster().sync();   // no CTA may leave while a peer can still read its records
