@@ -54,8 +54,19 @@ __global__ void __launch_bounds__(256) row_scale_kernel(double* __restrict__ A, 
 struct Cand {                 // one CTA's arg-max candidate for a column, with the row's content
     double absval;
     long long row;            // absolute row index, -1 if the CTA owns no eligible row
-    double content[FW];
+    double2 content[FW];      // .x = the row's panel entries; .y = the column's tag (tagged mode: every 16-byte word validates itself)
 };
+
+__device__ __forceinline__ void st_tagged(double2* p, double v, unsigned tag) {
+    asm volatile("st.volatile.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(__double_as_longlong(v)), "l"((unsigned long long)tag) : "memory");
+}
+__device__ __forceinline__ double ld_tagged(const double2* p, unsigned tag) {      // spins until the word carries `tag`
+    unsigned long long w0, w1;
+    do {
+        asm volatile("ld.volatile.global.v2.u64 {%0, %1}, [%2];" : "=l"(w0), "=l"(w1) : "l"(p) : "memory");
+    } while ((unsigned)w1 != tag);
+    return __longlong_as_double((long long)w0);
+}
 
 // Warp arg-max of non-negative doubles with the lowest index winning ties, on the redux.sync unit: the bit pattern of
 // a non-negative double orders like the number, so the maximum is two 32-bit max-reductions (high word, then low word
@@ -87,14 +98,15 @@ template <int FTHREADS, bool CLUSTER>
 __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict__ A, int64_t n, int64_t lda, int64_t j0,
                                                               int w, int rows_per_cta, double tol,
                                                               Cand* __restrict__ cand /* [2][gridDim] */,
-                                                              double* __restrict__ target /* [2][FW] */,
-                                                              long long* __restrict__ ipiv, int* __restrict__ info) {
+                                                              double2* __restrict__ target /* [2][FW] */,
+                                                              long long* __restrict__ ipiv, int* __restrict__ info,
+                                                              unsigned tag0) {
     extern __shared__ double S[];                       // rows_per_cta x (FW+1)
     __shared__ double s_val[FTHREADS / 32];
     __shared__ int s_idx[FTHREADS / 32];
     __shared__ double pv[FW];
     __shared__ Cand l_cand[2];                          // CLUSTER: this CTA's records, read by the peers
-    __shared__ double l_target[2][FW];
+    __shared__ double2 l_target[2][FW];
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
     int G = gridDim.x, b = blockIdx.x;
     if constexpr (CLUSTER) { G = (int)cg::this_cluster().num_blocks(); b = (int)cg::this_cluster().block_rank(); }
@@ -122,9 +134,24 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
             int bi = lane < FTHREADS / 32 ? s_idx[lane] : -1, none = 0;
             warp_argmax(best, bi, none);
             Cand* cd = CLUSTER ? &l_cand[c & 1] : cand + (size_t)(c & 1) * G + b;
-            if (lane == 0) { cd->absval = best; cd->row = bi >= 0 ? r0 + bi : -1; }
-            if (bi >= 0) cd->content[lane] = S[bi * LDS + lane];
-            if (jc >= r0 && jc < r0 + nr) (CLUSTER ? l_target[c & 1] : target + (c & 1) * FW)[lane] = S[(int)(jc - r0) * LDS + lane];
+            const bool tagged = !CLUSTER && tag0 != 0;
+            const unsigned tag = tag0 + (unsigned)c;
+            double2* tgt = CLUSTER ? l_target[c & 1] : target + (c & 1) * FW;
+            if (tagged) {
+                // tagged records instead of a grid barrier and fences: every 16-byte word {value, tag} validates itself,
+                // so the stores need no order among themselves; the head word is {|value|, tag : row}
+                if (bi >= 0) st_tagged(&cd->content[lane], S[bi * LDS + lane], tag);
+                if (jc >= r0 && jc < r0 + nr) st_tagged(&tgt[lane], S[(int)(jc - r0) * LDS + lane], tag);
+                if (lane == 0) {
+                    const unsigned long long w0 = (unsigned long long)__double_as_longlong(best);
+                    const unsigned long long w1 = ((unsigned long long)tag << 32) | (unsigned)(bi >= 0 ? (int)(r0 + bi) : -1);
+                    asm volatile("st.volatile.global.v2.u64 [%0], {%1, %2};" ::"l"(&cd->absval), "l"(w0), "l"(w1) : "memory");
+                }
+            } else {
+                if (bi >= 0) cd->content[lane] = make_double2(S[bi * LDS + lane], 0.0);
+                if (jc >= r0 && jc < r0 + nr) tgt[lane] = make_double2(S[(int)(jc - r0) * LDS + lane], 0.0);
+                if (lane == 0) { cd->absval = best; cd->row = bi >= 0 ? r0 + bi : -1; }
+            }
         }
     };                                                      // always followed by group_sync(), which is a block barrier too
 
@@ -147,7 +174,8 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
 
     publish(0);
     for (int c = 0; c < w; ++c) {
-        group_sync();
+        const bool tagged = !CLUSTER && tag0 != 0;
+        if (!tagged) group_sync();
         const int64_t jc = j0 + c;
         // every CTA reduces the G candidates identically: largest |value|, lowest row on ties (reading Q12).
         // Warp 0 alone: up to CPL candidates per lane, their loads all in flight together (one round trip), one
@@ -159,15 +187,36 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
             for (int q0 = 0; q0 < G; q0 += 32 * CPL) {
                 double v[CPL];
                 int rr[CPL];
+                if (tagged) {                              // poll until every record of this pass carries the column's tag
+                    const unsigned tag = tag0 + (unsigned)c;
+                    bool ok;
+                    do {
+                        ok = true;
 #pragma unroll
-                for (int u = 0; u < CPL; ++u) {
-                    const int q = q0 + u * 32 + lane;
-                    v[u] = -1.0;
-                    rr[u] = -1;
-                    if (q < G) {
-                        const Cand* cd = cand_of(c, q);
-                        v[u] = ld_f(&cd->absval);
-                        rr[u] = (int)ld_i(&cd->row);
+                        for (int u = 0; u < CPL; ++u) {
+                            const int q = q0 + u * 32 + lane;
+                            v[u] = -1.0;
+                            rr[u] = -1;
+                            if (q < G) {
+                                unsigned long long w0, w1;
+                                asm volatile("ld.volatile.global.v2.u64 {%0, %1}, [%2];" : "=l"(w0), "=l"(w1) : "l"(&cand_of(c, q)->absval) : "memory");
+                                ok = ok && (unsigned)(w1 >> 32) == tag;
+                                v[u] = __longlong_as_double((long long)w0);
+                                rr[u] = (int)(unsigned)w1;
+                            }
+                        }
+                    } while (!__all_sync(0xffffffffu, ok));
+                } else {
+#pragma unroll
+                    for (int u = 0; u < CPL; ++u) {
+                        const int q = q0 + u * 32 + lane;
+                        v[u] = -1.0;
+                        rr[u] = -1;
+                        if (q < G) {
+                            const Cand* cd = cand_of(c, q);
+                            v[u] = ld_f(&cd->absval);
+                            rr[u] = (int)ld_i(&cd->row);
+                        }
                     }
                 }
 #pragma unroll
@@ -177,7 +226,8 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
                     }
             }
             warp_argmax(best, brow, bcta);
-            pv[lane] = bcta >= 0 ? ld_f(&cand_of(c, bcta)->content[lane]) : 0.0;   // no candidate (a column of NaNs): flagged below
+            // the winner's row content; no candidate (a column of NaNs): flagged below
+            pv[lane] = bcta < 0 ? 0.0 : tagged ? ld_tagged(&cand_of(c, bcta)->content[lane], tag0 + (unsigned)c) : ld_f(&cand_of(c, bcta)->content[lane].x);
             if (brow < 0) brow = (int)jc;
             if (lane == 0 && b == 0) {
                 ipiv[jc] = brow;
@@ -187,9 +237,9 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
             // exchange rows jc and g = brow (content of row jc comes from `target`, the pivot row from `pv`)
             const long long g = brow;
             if (g != jc && g >= r0 && g < r0 + nr) {
-                const double* tg = target + (c & 1) * FW;
+                const double2* tg = target + (c & 1) * FW;
                 if constexpr (CLUSTER) tg = cg::this_cluster().map_shared_rank(&l_target[c & 1][0], (int)((jc - j0) / rows_per_cta));
-                S[(int)(g - r0) * LDS + lane] = ld_f(tg + lane);
+                S[(int)(g - r0) * LDS + lane] = tagged ? ld_tagged(tg + lane, tag0 + (unsigned)c) : ld_f(&tg[lane].x);
             }
             if (jc >= r0 && jc < r0 + nr) S[(int)(jc - r0) * LDS + lane] = pv[lane];
         }
@@ -553,7 +603,7 @@ struct F64 {
     double* B; int64_t nrhs, ldb;
     double tol;
     cudaStream_t s;
-    Cand* cand; double* target; long long* ipiv; int* info;
+    Cand* cand; double2* target; long long* ipiv; int* info;
     double* inv;                // inverted diagonal blocks of L and U (F3)
     int grid, rows_cap;         // cooperative grid size and the smem row capacity per CTA
     int panel_threads;
@@ -656,8 +706,9 @@ int panel_f64(F64& c, int64_t j0, int w) {
     if (rows_per_cta > c.rows_cap) return LINAC_ERR_INVALID_ARG;
     size_t smem = (size_t)rows_per_cta * (FW + 1) * sizeof(double);
     double* A = c.A; int64_t n = c.n, lda = c.lda; double tol = c.tol;
-    Cand* cand = c.cand; double* target = c.target; long long* ipiv = c.ipiv; int* info = c.info;
-    void* args[] = {&A, &n, &lda, &j0, &w, &rows_per_cta, &tol, &cand, &target, &ipiv, &info};
+    Cand* cand = c.cand; double2* target = c.target; long long* ipiv = c.ipiv; int* info = c.info;
+    unsigned tag0 = options().f64_panel_tags != 0 ? (unsigned)(j0 + 1) : 0u;   // column j carries tag j + 1 within a solve
+    void* args[] = {&A, &n, &lda, &j0, &w, &rows_per_cta, &tol, &cand, &target, &ipiv, &info, &tag0};
     if (c.cluster_ctas > 0 && m <= (int64_t)c.cluster_ctas * std::min<int64_t>(c.rows_cap, options().f64_cluster_rows)) {
         rows_per_cta = std::max(1, (int)((m + c.cluster_ctas - 1) / c.cluster_ctas));
         smem = (size_t)rows_per_cta * (FW + 1) * sizeof(double);
@@ -673,7 +724,7 @@ int panel_f64(F64& c, int64_t j0, int w) {
         at[0].val.clusterDim.z = 1;
         cfg.attrs = at;
         cfg.numAttrs = 1;
-        LINAC_CUDA(cudaLaunchKernelEx(&cfg, f64_panel_kernel<512, true>, A, n, lda, j0, w, rows_per_cta, tol, cand, target, ipiv, info));
+        LINAC_CUDA(cudaLaunchKernelEx(&cfg, f64_panel_kernel<512, true>, A, n, lda, j0, w, rows_per_cta, tol, cand, target, ipiv, info, 0u));
     } else if (c.panel_threads == 1024)
         LINAC_CUDA(cudaLaunchCooperativeKernel((void*)f64_panel_kernel<1024, false>, dim3(c.grid), dim3(1024), args, smem, c.s));
     else if (c.panel_threads == 512)
@@ -733,7 +784,7 @@ int factor_flat_f64(F64& c) {
 size_t f64_workspace_bytes(int64_t n) {
     (void)n;
     const size_t inv = 2 * (size_t)((n + TB - 1) / TB) * TB * TB * sizeof(double);
-    return 8192 + 2 * 1024 * sizeof(Cand) + 2 * FW * sizeof(double) + (size_t)std::max<int64_t>(n, 1) * 8 + 1024 + inv;
+    return 8192 + 2 * 1024 * sizeof(Cand) + 2 * FW * sizeof(double2) + (size_t)std::max<int64_t>(n, 1) * 8 + 1024 + inv;
 }
 
 }  // namespace
@@ -809,13 +860,15 @@ int linac_solve_f64(double* dA, int64_t n, int64_t lda, double* dB, int64_t nrhs
     LINAC_CUDA(cudaFuncSetAttribute(dgemm_sub_mma_kernel<64, false, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dmma_smem_bytes(64)));
     LINAC_CUDA(cudaFuncSetAttribute(dgemm_sub_mma_kernel<64, true, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dmma_smem_bytes(64)));
     c.cand = (Cand*)arena.take(2 * 1024 * sizeof(Cand));
-    c.target = (double*)arena.take(2 * FW * sizeof(double));
+    c.target = (double2*)arena.take(2 * FW * sizeof(double2));
     c.ipiv = (long long*)arena.take((size_t)n * 8);
     c.info = (int*)arena.take(256);
     c.inv = nrhs > 0 ? (double*)arena.take(2 * (size_t)((n + TB - 1) / TB) * TB * TB * sizeof(double)) : nullptr;
     if (!c.cand || !c.target || !c.ipiv || !c.info || (nrhs > 0 && !c.inv)) return LINAC_ERR_WORKSPACE;
     const int big = INT_MAX;
     LINAC_CUDA(cudaMemcpyAsync(c.info, &big, sizeof(int), cudaMemcpyHostToDevice, s));
+    LINAC_CUDA(cudaMemsetAsync(c.cand, 0, 2 * 1024 * sizeof(Cand), s));        // tags of an earlier solve must not match
+    LINAC_CUDA(cudaMemsetAsync(c.target, 0, 2 * FW * sizeof(double2), s));
 
     cudaEvent_t e0, e1;
     LINAC_CUDA(cudaEventCreate(&e0));

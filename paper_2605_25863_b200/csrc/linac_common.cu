@@ -190,6 +190,9 @@ int linac_set_option(const char* name, int64_t value) {
     } else if (!strcmp(name, "f64_cluster_rows")) {
         if (value < 1) return LINAC_ERR_INVALID_ARG;
         g_options.f64_cluster_rows = value;
+    } else if (!strcmp(name, "f64_panel_tags")) {
+        if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
+        g_options.f64_panel_tags = value;
     } else if (!strcmp(name, "f64_rhs_inv")) {
         if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
         g_options.f64_rhs_inv = value;

@@ -107,7 +107,7 @@ def test_medium_size_several_panels_and_recursion_levels(oracle):
 
 @pytest.mark.parametrize("opts", [
     {"f64_strip": 0}, {"f64_strip": 256}, {"f64_rhs_inv": 0}, {"f64_mma": 0},
-    {"f64_panel_threads": 256}, {"f64_panel_threads": 1024},
+    {"f64_panel_threads": 256}, {"f64_panel_threads": 1024}, {"f64_panel_tags": 0},
     {"f64_panel_cluster": 16, "f64_cluster_rows": 4096}, {"f64_panel_cluster": 8, "f64_cluster_rows": 100},
 ])
 def test_schedule_options_solve_the_same_system(oracle, opts):
@@ -116,7 +116,7 @@ def test_schedule_options_solve_the_same_system(oracle, opts):
     ragged size and more than 64 right-hand sides."""
     import paper_2605_25863_b200 as L
     defaults = {"f64_strip": 1024, "f64_rhs_inv": 1, "f64_mma": 1, "f64_panel_threads": 512, "f64_panel_cluster": 0,
-                "f64_cluster_rows": 128}
+                "f64_cluster_rows": 128, "f64_panel_tags": 1}
     n, nrhs = 1337, 70
     a, b = gen.normal_matrix(n, n, seed=21), gen.normal_matrix(n, nrhs, seed=22)
     try:
