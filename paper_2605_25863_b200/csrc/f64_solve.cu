@@ -101,10 +101,11 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
                                                               double2* __restrict__ target /* [2][FW] */,
                                                               long long* __restrict__ ipiv, int* __restrict__ info,
                                                               unsigned tag0) {
-    extern __shared__ double S[];                       // rows_per_cta x (FW+1)
-    __shared__ double s_val[FTHREADS / 32];
-    __shared__ int s_idx[FTHREADS / 32];
-    __shared__ double pv[FW];
+    extern __shared__ __align__(16) double S[];         // rows_per_cta x LDS
+    constexpr int NE = FTHREADS / 32 * 4;               // arg-max entries per column: 4 row groups per warp
+    __shared__ double s_val[NE];
+    __shared__ int s_idx[NE];
+    __shared__ __align__(16) double pv_al[FW];
     __shared__ Cand l_cand[2];                          // CLUSTER: this CTA's records, read by the peers
     __shared__ double2 l_target[2][FW];
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
@@ -121,7 +122,8 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
     auto ld_i = [&](const long long* p) { if constexpr (CLUSTER) return *p; else return __ldcg(p); };
     const int64_t r0 = j0 + (int64_t)b * rows_per_cta;
     const int nr = (int)max((int64_t)0, min((int64_t)rows_per_cta, n - r0));
-    constexpr int LDS = FW + 1;
+    constexpr int LDS = FW + 2;                         // even: the update reads rows as 16-byte pairs
+    double* pv = pv_al;
 
     for (int k = wq; k < nr; k += FTHREADS / 32) S[k * LDS + lane] = lane < w ? A[(r0 + k) * lda + j0 + lane] : 0.0;
     __syncthreads();
@@ -130,8 +132,13 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
     auto publish_tail = [&](int c) {
         const int64_t jc = j0 + c;
         if (wq == 0) {
-            double best = lane < FTHREADS / 32 ? s_val[lane] : -1.0;
-            int bi = lane < FTHREADS / 32 ? s_idx[lane] : -1, none = 0;
+            double best = -1.0;
+            int bi = -1, none = 0;
+            for (int e = lane; e < NE; e += 32) {
+                const double v = s_val[e];
+                const int i = s_idx[e];
+                if (i >= 0 && (bi < 0 || v > best || (v == best && i < bi))) { best = v; bi = i; }
+            }
             warp_argmax(best, bi, none);
             Cand* cd = CLUSTER ? &l_cand[c & 1] : cand + (size_t)(c & 1) * G + b;
             const bool tagged = !CLUSTER && tag0 != 0;
@@ -167,7 +174,7 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
         }
         int none = 0;
         warp_argmax(best, bi, none);
-        if (lane == 0) { s_val[wq] = best; s_idx[wq] = bi; }
+        if (lane < 4) { s_val[wq * 4 + lane] = best; s_idx[wq * 4 + lane] = lane == 0 ? bi : -1; }
         __syncthreads();
         publish_tail(c);
     };
@@ -247,23 +254,35 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
         double piv = pv[c];
         if (!(fabs(piv) > tol)) piv = 1.0;              // singular: flagged above; keep the arithmetic finite
         const double rp = __drcp_rn(piv);
-        // multipliers and rank-1 update of own rows below jc: one warp per row, lane = column.  Lane c+1 sees the
-        // new entries of the next column as they are made and keeps their arg-max (lowest row on ties).
+        // multipliers and rank-1 update of own rows below jc: a warp takes four rows per pass, eight lanes per row,
+        // four columns per lane (two 16-byte accesses each way).  The lane that holds column c+1 sees the new
+        // entries of the next column as they are made and keeps their arg-max (lowest row on ties).
+        const int seg = lane & 7, rg = lane >> 3, jb = seg * 4;
+        const int cs = c >> 2, ns = (c + 1) >> 2, ne = (c + 1) & 3;
+        const double2 pa = *reinterpret_cast<const double2*>(pv + jb), pb = *reinterpret_cast<const double2*>(pv + jb + 2);
         double best = -1.0;
         int bi = -1;
         const int kmin = (int)max((int64_t)0, min((int64_t)nr, jc + 1 - r0));   // own rows below the pivot row
 #pragma unroll 2
-        for (int k = kmin + wq; k < nr; k += FTHREADS / 32) {
-            const double l = S[k * LDS + c] * rp;
-            if (lane == c) S[k * LDS + c] = l;
-            else if (lane > c && lane < w) {
-                const double v = S[k * LDS + lane] - l * pv[lane];
-                S[k * LDS + lane] = v;
-                if (lane == c + 1 && fabs(v) > best) { best = fabs(v); bi = k; }
+        for (int k = kmin + wq * 4 + rg; k < nr; k += FTHREADS / 32 * 4) {
+            double* row = S + k * LDS;
+            const double l = row[c] * rp;
+            if (seg >= cs) {                               // columns >= w hold zeros in S and in pv: no bound needed
+                double2 xa = *reinterpret_cast<double2*>(row + jb), xb = *reinterpret_cast<double2*>(row + jb + 2);
+                xa.x = jb + 0 > c ? xa.x - l * pa.x : (jb + 0 == c ? l : xa.x);
+                xa.y = jb + 1 > c ? xa.y - l * pa.y : (jb + 1 == c ? l : xa.y);
+                xb.x = jb + 2 > c ? xb.x - l * pb.x : (jb + 2 == c ? l : xb.x);
+                xb.y = jb + 3 > c ? xb.y - l * pb.y : (jb + 3 == c ? l : xb.y);
+                *reinterpret_cast<double2*>(row + jb) = xa;
+                *reinterpret_cast<double2*>(row + jb + 2) = xb;
+                if (seg == ns) {
+                    const double v = fabs(ne == 0 ? xa.x : ne == 1 ? xa.y : ne == 2 ? xb.x : xb.y);
+                    if (v > best) { best = v; bi = k; }
+                }
             }
         }
         if (c + 1 < w) {
-            if (lane == c + 1) { s_val[wq] = best; s_idx[wq] = bi; }
+            if (seg == ns) { s_val[wq * 4 + rg] = best; s_idx[wq * 4 + rg] = bi; }
             __syncthreads();
             publish_tail(c + 1);
         }
@@ -704,14 +723,14 @@ int panel_f64(F64& c, int64_t j0, int w) {
     int rows_per_cta = (int)((m + c.grid - 1) / c.grid);
     rows_per_cta = std::max(rows_per_cta, 1);
     if (rows_per_cta > c.rows_cap) return LINAC_ERR_INVALID_ARG;
-    size_t smem = (size_t)rows_per_cta * (FW + 1) * sizeof(double);
+    size_t smem = (size_t)rows_per_cta * (FW + 2) * sizeof(double);
     double* A = c.A; int64_t n = c.n, lda = c.lda; double tol = c.tol;
     Cand* cand = c.cand; double2* target = c.target; long long* ipiv = c.ipiv; int* info = c.info;
     unsigned tag0 = options().f64_panel_tags != 0 ? (unsigned)(j0 + 1) : 0u;   // column j carries tag j + 1 within a solve
     void* args[] = {&A, &n, &lda, &j0, &w, &rows_per_cta, &tol, &cand, &target, &ipiv, &info, &tag0};
     if (c.cluster_ctas > 0 && m <= (int64_t)c.cluster_ctas * std::min<int64_t>(c.rows_cap, options().f64_cluster_rows)) {
         rows_per_cta = std::max(1, (int)((m + c.cluster_ctas - 1) / c.cluster_ctas));
-        smem = (size_t)rows_per_cta * (FW + 1) * sizeof(double);
+        smem = (size_t)rows_per_cta * (FW + 2) * sizeof(double);
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3(c.cluster_ctas);
         cfg.blockDim = dim3(512);
@@ -827,7 +846,7 @@ int linac_solve_f64(double* dA, int64_t n, int64_t lda, double* dB, int64_t nrhs
     c.panel_threads = (int)options().f64_panel_threads;
     if (options().f64_panel_grid > 0) c.grid = (int)std::min<int64_t>(sms, options().f64_panel_grid);
     c.smem_max = (size_t)smem_optin - 4096;
-    c.rows_cap = (int)(c.smem_max / ((FW + 1) * sizeof(double)));
+    c.rows_cap = (int)(c.smem_max / ((FW + 2) * sizeof(double)));
     if ((n + c.grid - 1) / c.grid > c.rows_cap) return LINAC_ERR_INVALID_ARG;   // n > ~118k: strip no longer fits on chip
     LINAC_CUDA(cudaFuncSetAttribute(f64_panel_kernel<256, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max));
     LINAC_CUDA(cudaFuncSetAttribute(f64_panel_kernel<512, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max));
