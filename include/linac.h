@@ -200,6 +200,9 @@ int linac_get_last_stats(linac_stats *out);
  * "strip_width" (columns per cooperative strip kernel: 32..256, multiple of 32), "flat_cols" (nodes up to this many
  * columns are swept flat, wider ones recurse), "flat_group" (strips per Schur update of the flat sweep), "tc_panel" (0/1), "f64_mma" (fp64 trailing update: 1 = DMMA tensor pipe, 0 = DFMA),
  * "f64_strip" (fp64 factorisation: columns per strip of the flat top-level sweep, multiple of 32, 0 = pure recursion),
+ * "f64_panel_threads" (256/512/1024) and "f64_panel_grid" (0 = one CTA per SM) of the fp64 panel kernel, "f64_panel_tags" (1 = tagged
+ * candidate records instead of a grid barrier per column), "f64_panel_cluster" (CTAs of the cluster + DSMEM panel variant, 0 = off) with
+ * "f64_cluster_rows" (rows per CTA up to which it is used),
  * "f64_rhs_inv" (fp64 substitution on the right-hand sides: 1 = blocked, with inverted 128 x 128 diagonal blocks, 0 = recursive leaf solves)}.
  * Returns LINAC_ERR_INVALID_ARG for unknown names / out-of-range values. */
 int linac_set_option(const char *name, int64_t value);
