@@ -486,7 +486,20 @@ __global__ void __launch_bounds__(NW * 32, 1) dgemm_sub_mma_kernel(double* C, in
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wm0 = (warp >> 2) * (MI * 8), wn0 = (warp & 3) * (TN / 4);
     const int g = lane >> 2, q = lane & 3;                // fragment coordinates (PTX ISA, m8n8k4 .f64)
-    const int64_t m0 = (int64_t)blockIdx.y * DM, n0 = (int64_t)blockIdx.x * TN;
+    // Tile order: bands of RB column tiles, row tiles fastest inside a band, so that the CTAs in flight together share
+    // few B panels (a plain row-major order re-read all of B from DRAM on every wave: 4x the algorithmic traffic)
+    int tx = blockIdx.x, ty = blockIdx.y;
+    {
+        constexpr int RB = 16;
+        const int gx = gridDim.x, gy = gridDim.y;
+        const int lin = blockIdx.y * gx + blockIdx.x;
+        const int band = lin / (RB * gy);
+        const int bw = min(RB, gx - band * RB);            // the last band may be narrower
+        const int within = lin - band * RB * gy;
+        ty = within / bw;
+        tx = band * RB + within - ty * bw;
+    }
+    const int64_t m0 = (int64_t)ty * DM, n0 = (int64_t)tx * TN;
     double acc[MI][NJ][2];
 #pragma unroll
     for (int i = 0; i < MI; ++i)
