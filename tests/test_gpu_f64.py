@@ -128,3 +128,27 @@ def test_schedule_options_solve_the_same_system(oracle, opts):
             L.set_option(k, v)
     assert oracle.backward_error(a, x, b, nthreads=oracle.max_threads()) <= ETA_MAX
     assert np.allclose(x, np.linalg.solve(a, b), rtol=1e-7, atol=1e-10)
+
+
+def test_tagged_records_match_the_grid_barrier_bitwise_and_repeat():
+    """The panel kernel's per-column exchange through self-validating {value, tag} 16-byte words (option
+    f64_panel_tags, default) must pick the same pivots and produce the same bits as the grid-barrier version, run
+    after run: a torn or stale read would show up as a different pivot row somewhere in 2500 columns."""
+    import paper_2605_25863_b200 as L
+    n, nrhs = 2500, 9
+    a0 = torch.from_numpy(gen.normal_matrix(n, n, seed=31)).cuda()
+    b0 = torch.from_numpy(gen.normal_matrix(n, nrhs, seed=32)).cuda()
+
+    def solve():
+        a, b = a0.clone(), b0.clone()
+        L.solve_f64(a, b)
+        return a, b
+
+    try:
+        L.set_option("f64_panel_tags", 0)
+        lu_ref, x_ref = solve()
+    finally:
+        L.set_option("f64_panel_tags", 1)
+    for _ in range(12):
+        lu, x = solve()
+        assert torch.equal(lu, lu_ref) and torch.equal(x, x_ref)
