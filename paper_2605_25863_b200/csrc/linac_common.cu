@@ -173,7 +173,7 @@ int linac_set_option(const char* name, int64_t value) {
         if (value < 128) return LINAC_ERR_INVALID_ARG;
         g_options.tc_min_mn = value;
     } else if (!strcmp(name, "f64_mma")) {
-        if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
+        if (value < 0 || value > 2) return LINAC_ERR_INVALID_ARG;
         g_options.f64_mma = value;
     } else if (!strcmp(name, "f64_strip")) {
         if (value < 0 || (value > 0 && value % 32 != 0)) return LINAC_ERR_INVALID_ARG;

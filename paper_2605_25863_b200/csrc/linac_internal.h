@@ -41,7 +41,7 @@ struct Options {
     int64_t tc_min_k = 128;   // smallest K the tensor path is used for
     int64_t tc_min_mn = 128;  // smallest M and N the tensor path is used for
     int64_t f64_mma = 1;      // fp64 trailing update: 1 = DMMA (FP64 tensor pipe), 0 = DFMA register tile
-    int64_t f64_strip = 1024;  // fp64 factorisation: flat sweep over strips of this many columns (0 = pure recursion)
+    int64_t f64_strip = 512;   // fp64 factorisation: flat sweep over strips of this many columns (0 = pure recursion)
     int64_t f64_panel_threads = 512, f64_panel_grid = 0;   // fp64 panel kernel: block size (256/512/1024), grid (0 = one CTA per SM)
     int64_t f64_panel_cluster = 0;    // fp64 panel: CTAs of the thread-block cluster that factors strips which fit its shared memory (0 = off)
     int64_t f64_cluster_rows = 128;   // ... up to this many rows per CTA (beyond it the per-column shared-memory traffic of one SM costs more than the grid barrier)

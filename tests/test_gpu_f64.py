@@ -115,7 +115,7 @@ def test_schedule_options_solve_the_same_system(oracle, opts):
     panel kernel's block sizes, the cluster + DSMEM panel kernel) on a matrix that needs row exchanges, with a
     ragged size and more than 64 right-hand sides."""
     import paper_2605_25863_b200 as L
-    defaults = {"f64_strip": 1024, "f64_rhs_inv": 1, "f64_mma": 1, "f64_panel_threads": 512, "f64_panel_cluster": 0,
+    defaults = {"f64_strip": 512, "f64_rhs_inv": 1, "f64_mma": 1, "f64_panel_threads": 512, "f64_panel_cluster": 0,
                 "f64_cluster_rows": 128, "f64_panel_tags": 1}
     n, nrhs = 1337, 70
     a, b = gen.normal_matrix(n, n, seed=21), gen.normal_matrix(n, nrhs, seed=22)
