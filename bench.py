@@ -140,6 +140,12 @@ def f64_leg(torch, L, dev, n=16384, nrhs=64, reps=3):
     flop = 2.0 * n ** 3 / 3.0 + 2.0 * n * n * nrhs
     return {"workload": f"c4: {n}x{n} float64 N(0,1) + 4 sqrt(N) I, {nrhs} right-hand sides (torch generator, seed 5)",
             "ms_per_solve": ms, "gflops": flop / ms / 1e6, "backward_error": eta, "backward_error_bound": 1e-11,
+            "roofline": {"bound": "tensor", "achieved": flop / ms / 1e9, "peak": 36.9, "unit": "TFLOP/s (fp64 DMMA)",
+                         "frac": flop / ms / 1e9 / 36.9,
+                         "note": "whole solve (panel chain and solves included) against the FP64 tensor pipe: 148 SMs x 64 "
+                                 "FMA/clk x 2 x 1.95 GHz, consistent with ncu (68 % sub-pipe utilisation at 25.2 TFLOP/s on "
+                                 "the largest update, profiles/r01_v12_dmma_top_ncu.md) and with cuBLAS DGEMM measured at "
+                                 "36.0 TFLOP/s on this pool"},
             "note": "flop = 2N^3/3 + 2N^2 nrhs; trailing update on the FP64 tensor pipe (DMMA m8n8k4), substitution with "
                     "inverted 128 x 128 diagonal blocks"}
 
