@@ -455,7 +455,7 @@ __global__ void __launch_bounds__(DTHREADS) dgemm_sub_kernel(double* __restrict_
 // as 2 x 4, a 64 x 32 warp tile = 8 x 4 MMA tiles.  Operands come from shared memory one double per thread and
 // per fragment, so a k-step costs 12 LDS.64 per 32 MMAs: five times less shared-memory traffic per flop than the
 // 8 x 8 register tile of the DFMA kernel above, which was co-bound by the shared-memory pipe.
-constexpr int QK = 16;                    // k per shared-memory stage
+constexpr int QK = 16;                    // k per shared-memory stage (the A copy mapping below assumes 16)
 constexpr int QLD = DM + 4;               // row stride in doubles: = 4 mod 16, conflict-free fragment loads
 constexpr int QNS = 3;                    // cp.async stages
 __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc, bool valid) {
@@ -510,8 +510,10 @@ __global__ void __launch_bounds__(NW * 32, TN == 64 ? 2 : 1) dgemm_sub_mma_kerne
     auto issue = [&](int64_t k0, int buf) {
 #pragma unroll
         for (int t = 0; t < AL; ++t) {
+            // a warp copies 8 rows x 4 consecutive k (one 32-byte sector per row): its 32 scattered 8-byte writes
+            // into the k-major tile then fall on every bank pair exactly twice (QLD = 4 mod 16), the minimum
             const int idx = tid + t * NT;
-            const int kk = idx % QK, mm = idx / QK;
+            const int kk = 4 * ((idx >> 5) & 3) + (idx & 3), mm = 8 * (idx >> 7) + ((idx >> 2) & 7);
             const int64_t m = m0 + mm, k = k0 + kk;
             const bool ok = m < M && k < K;
             cp_async8(&As[buf][kk][mm], ok ? A + m * lda + k : A, ok);
