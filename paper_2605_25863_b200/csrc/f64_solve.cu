@@ -527,6 +527,15 @@ __global__ void __launch_bounds__(NW * 32, TN == 64 ? 2 : 1) dgemm_sub_mma_kerne
             cp_async8(&Bs[buf][kb][nn], ok ? B + k2 * ldb + n : B, ok);
         }
     };
+    if constexpr (!ASSIGN) {                               // the C tile is wanted at the end: start moving it into L2 now
+#pragma unroll
+        for (int i = 0; i < MI; ++i)
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) {
+                const int64_t m = m0 + wm0 + i * 8 + g, n = n0 + wn0 + j * 8 + q * 2;
+                if (m < M && n < N) asm volatile("prefetch.global.L2 [%0];" ::"l"(C + m * ldc + n));
+            }
+    }
     const int64_t nk = (K + QK - 1) / QK;
 #pragma unroll
     for (int st = 0; st < QNS - 1; ++st) {
