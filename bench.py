@@ -143,8 +143,8 @@ def f64_leg(torch, L, dev, n=16384, nrhs=64, reps=3):
             "roofline": {"bound": "tensor", "achieved": flop / ms / 1e9, "peak": 36.9, "unit": "TFLOP/s (fp64 DMMA)",
                          "frac": flop / ms / 1e9 / 36.9,
                          "note": "whole solve (panel chain and solves included) against the FP64 tensor pipe: 148 SMs x 64 "
-                                 "FMA/clk x 2 x 1.95 GHz, consistent with ncu (68 % sub-pipe utilisation at 25.2 TFLOP/s on "
-                                 "the largest update, profiles/r01_v12_dmma_top_ncu.md) and with cuBLAS DGEMM measured at "
+                                 "FMA/clk x 2 x 1.95 GHz, consistent with ncu (78 % sub-pipe utilisation at 28.8 TFLOP/s on "
+                                 "the largest update, profiles/r01_v13_dmma_top_ncu.md) and with cuBLAS DGEMM measured at "
                                  "36.0 TFLOP/s on this pool"},
             "note": "flop = 2N^3/3 + 2N^2 nrhs; trailing update on the FP64 tensor pipe (DMMA m8n8k4), substitution with "
                     "inverted 128 x 128 diagonal blocks"}
