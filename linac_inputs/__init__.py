@@ -21,6 +21,8 @@ from .gen import (  # noqa: F401
     uniform_mod_p,
     uniform_matrix,
     uniform_rows,
+    uniform_mod_p64,
+    uniform_matrix_u64,
     lowrank_factors,
     sparse_dependent_rows,
     sparse_dependent_plan,

@@ -52,6 +52,22 @@ def uniform_mod_p(h: np.ndarray, p: int) -> np.ndarray:
     return (t >> np.uint64(32)).astype(np.uint32)
 
 
+def uniform_mod_p64(h: np.ndarray, p: int) -> np.ndarray:
+    """mulhi64(h, p) for any p < 2^64 (the 64-bit backend's inputs): 128-bit product by 32-bit halves.  uint64."""
+    assert 0 < p < (1 << 64)
+    p1, p0 = np.uint64(p >> 32), np.uint64(p & 0xFFFFFFFF)
+    h1, h0 = h >> np.uint64(32), h & _MASK32
+    with np.errstate(over="ignore"):
+        mid = h1 * p0 + ((h0 * p0) >> np.uint64(32))          # < 2^64
+        mid2 = (mid & _MASK32) + h0 * p1                      # < 2^64
+        return h1 * p1 + (mid >> np.uint64(32)) + (mid2 >> np.uint64(32))
+
+
+def uniform_matrix_u64(rows: int, cols: int, p: int, seed: int) -> np.ndarray:
+    """rows x cols uint64, i.i.d. uniform in [0, p), p < 2^64; same counters as uniform_matrix."""
+    return uniform_mod_p64(splitmix64(seed, _row_counters(0, rows, cols)), p)
+
+
 def _row_counters(row0: int, nrows: int, cols: int) -> np.ndarray:
     r = np.arange(row0, row0 + nrows, dtype=np.uint64)[:, None]
     c = np.arange(cols, dtype=np.uint64)[None, :]

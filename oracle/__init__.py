@@ -9,7 +9,7 @@ imports nothing from there.
 Pins (tests/test_oracle_*.py, `-m "not gpu"`): every function here is pinned against
 something other than itself -- brute force over tiny fields, Leibniz determinants, closed
 forms (Vandermonde), Python big-int arithmetic, sympy's GF(p) RREF as a black box, LAPACK
-for fp64.  No function is "parity unpinned".
+for fp64, exact rational RREF and SVD rank for the floating-point RREF.  No function is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -49,6 +49,16 @@ def lib() -> C.CDLL:
                                          C.c_int64, C.c_uint32, C.c_int]
         L.oracle_solve_f64.restype = C.c_int
         L.oracle_solve_f64.argtypes = [f64p, C.c_int64, C.c_int64, f64p, C.c_int64, C.c_int64, C.c_double, C.c_int, i64p]
+        u64p = C.POINTER(C.c_uint64)
+        L.oracle_inv_modp64.restype = C.c_uint64
+        L.oracle_inv_modp64.argtypes = [C.c_uint64, C.c_uint64]
+        L.oracle_rref_modp64.restype = C.c_int
+        L.oracle_rref_modp64.argtypes = [u64p, C.c_int64, C.c_int64, C.c_int64, C.c_uint64, C.c_int, C.c_int, i64p, i32p]
+        L.oracle_matmul_modp64.restype = C.c_int
+        L.oracle_matmul_modp64.argtypes = [u64p, C.c_int64, u64p, C.c_int64, u64p, C.c_int64, C.c_int64, C.c_int64,
+                                           C.c_int64, C.c_uint64, C.c_int]
+        L.oracle_rref_f64.restype = C.c_int
+        L.oracle_rref_f64.argtypes = [f64p, C.c_int64, C.c_int64, C.c_int64, C.c_double, C.c_int, i64p, i32p]
         L.oracle_backward_error.restype = C.c_double
         L.oracle_backward_error.argtypes = [f64p, C.c_int64, C.c_int64, f64p, C.c_int64, f64p, C.c_int64, C.c_int64,
                                             C.c_int]
@@ -212,3 +222,60 @@ def backward_error(a0: np.ndarray, x: np.ndarray, b0: np.ndarray, nthreads: int 
     n = a0.shape[0]
     return float(lib().oracle_backward_error(_f64(a0), n, n, _f64(x), x.shape[1], _f64(b0), b0.shape[1],
                                              x.shape[1], nthreads))
+
+
+# ---- 64-bit backend ---------------------------------------------------
+
+def _u64(a):
+    return a.ctypes.data_as(C.POINTER(C.c_uint64))
+
+
+def inv_modp64(a: int, p: int) -> int:
+    return int(lib().oracle_inv_modp64(a, p))
+
+
+def rref_modp64(a: np.ndarray, p: int, pivot_rule: int = PIVOT_FIRST, nthreads: int = 1):
+    """RREF over F_p of a 2-D uint64 array, p < 2^64: the loop of rref_modp with uint64 storage and `%` on
+    unsigned __int128.  Returns (R, rank, pivot_cols).  Pinned in tests/test_oracle_wide.py (Python big-int
+    arithmetic, sympy GF(p), agreement with rref_modp for p < 2^32, brute force over tiny fields)."""
+    a = np.ascontiguousarray(a, dtype=np.uint64)
+    rows, cols = a.shape
+    r = a.copy()
+    rank = C.c_int64(0)
+    piv = np.zeros(max(1, min(rows, cols)), dtype=np.int32)
+    rc = lib().oracle_rref_modp64(_u64(r), rows, cols, cols, p, pivot_rule, nthreads, C.byref(rank),
+                                  piv.ctypes.data_as(C.POINTER(C.c_int32)))
+    if rc != 0:
+        raise ValueError(f"oracle_rref_modp64 failed: {rc}")
+    return r, int(rank.value), piv[: rank.value].copy()
+
+
+def matmul_modp64(a: np.ndarray, b: np.ndarray, p: int, nthreads: int = 1) -> np.ndarray:
+    a = np.ascontiguousarray(a, dtype=np.uint64)
+    b = np.ascontiguousarray(b, dtype=np.uint64)
+    m, k = a.shape
+    k2, n = b.shape
+    assert k == k2
+    c = np.zeros((m, n), dtype=np.uint64)
+    if m and n:
+        lib().oracle_matmul_modp64(_u64(a), max(k, 1), _u64(b), max(n, 1), _u64(c), max(n, 1), m, k, n, p, nthreads)
+    return c
+
+
+# ---- SURVEY.md 8(f) rank 3: floating-point RREF with a threshold (PAPER.md:65, 231-251) ------------------------
+
+def rref_f64(a: np.ndarray, tol: float = -1.0, nthreads: int = 1):
+    """Row-rescaled, partially pivoted Gauss-Jordan reduction of a rectangular float64 matrix with the head compared
+    to `tol` (citations in linac_oracle.c).  Returns (R, rank, pivot_cols); the input is untouched.
+    Pinned in tests/test_oracle_f64.py: exact rational RREF (sympy) of small integer matrices, numpy SVD rank of
+    low-rank products, (A | I) -> (I | A^-1) against LAPACK, the threshold semantics on a planted tiny pivot."""
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    rows, cols = a.shape
+    r = a.copy()
+    rank = C.c_int64(0)
+    piv = np.zeros(max(1, min(rows, cols)), dtype=np.int32)
+    rc = lib().oracle_rref_f64(_f64(r), rows, cols, max(cols, 1), tol, nthreads, C.byref(rank),
+                               piv.ctypes.data_as(C.POINTER(C.c_int32)))
+    if rc != 0:
+        raise ValueError(f"oracle_rref_f64 failed: {rc}")
+    return r, int(rank.value), piv[: rank.value].copy()

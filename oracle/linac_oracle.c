@@ -316,3 +316,156 @@ double oracle_backward_error(const double *A0, int64_t n, int64_t lda, const dou
     free(norm_r); free(norm_x); free(norm_b);
     return eta;
 }
+
+/* =====================================================================================================
+ * the 64-bit backend ("uint32 is used for p <= 2^32 - 1 and uint64 for
+ * 2^32 - 1 < p <= ..."; the upper bound is lost in the extraction -- DESIGN.md reading Q18
+ * takes p < 2^63).  The SAME one-column-at-a-time loop as rref_core above (same passages: PAPER.md:153,
+ * 225, 239-251), with uint64_t storage and every reduction the C `%` operator on unsigned __int128.
+ * oracle_rref_modp (32-bit storage) is already valid for every p <= 2^32 - 1: its temporaries are
+ * uint64_t and (a + P - x) < 2^33.
+ * ===================================================================================================== */
+typedef unsigned __int128 u128;
+
+/* a^{-1} mod p by the extended Euclidean algorithm on signed 128-bit; a in [1, p), p < 2^64. */
+uint64_t oracle_inv_modp64(uint64_t a, uint64_t p) {
+    __int128 r0 = (__int128)p, r1 = (__int128)(a % p);
+    __int128 t0 = 0, t1 = 1;
+    while (r1 != 0) {
+        __int128 q = r0 / r1;
+        __int128 r2 = r0 - q * r1;
+        __int128 t2 = t0 - q * t1;
+        r0 = r1; r1 = r2;
+        t0 = t1; t1 = t2;
+    }
+    t0 %= (__int128)p;
+    if (t0 < 0) t0 += (__int128)p;
+    return (uint64_t)t0;
+}
+
+int oracle_rref_modp64(uint64_t *A, int64_t rows, int64_t cols, int64_t ld, uint64_t p, int pivot_rule,
+                       int nthreads, int64_t *rank, int32_t *pivot_cols) {
+    if (rows < 0 || cols < 0 || ld < cols || p < 2 || (rows > 0 && cols > 0 && !A)) return -1;
+    const u128 P = p;
+    for (int64_t r = 0; r < rows; ++r)
+        for (int64_t c = 0; c < cols; ++c) A[r * ld + c] %= p;
+    int64_t i = 0;
+    (void)nthreads;
+    for (int64_t j = 0; j < cols && i < rows; ++j) {
+        int64_t k = -1;
+        if (pivot_rule == ORACLE_PIVOT_FIRST) {
+            for (int64_t r = i; r < rows; ++r) if (A[r * ld + j] != 0) { k = r; break; }
+        } else if (pivot_rule == ORACLE_PIVOT_LAST) {
+            for (int64_t r = rows - 1; r >= i; --r) if (A[r * ld + j] != 0) { k = r; break; }
+        } else {
+            uint64_t best = 0;
+            for (int64_t r = i; r < rows; ++r) if (A[r * ld + j] > best) { best = A[r * ld + j]; k = r; }
+        }
+        if (k < 0) continue;
+        if (k != i) {
+            uint64_t *x = A + k * ld, *y = A + i * ld;
+            for (int64_t c = 0; c < cols; ++c) { uint64_t t = x[c]; x[c] = y[c]; y[c] = t; }
+        }
+        uint64_t *pi = A + i * ld;
+        const u128 inv = oracle_inv_modp64(pi[j], p);
+        for (int64_t c = j; c < cols; ++c) pi[c] = (uint64_t)((u128)pi[c] * inv % P);
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) num_threads(nthreads) if (nthreads > 1)
+#endif
+        for (int64_t r = 0; r < rows; ++r) {
+            if (r == i) continue;
+            uint64_t *pr = A + r * ld;
+            const u128 h = pr[j];
+            if (h == 0) continue;
+            for (int64_t c = j; c < cols; ++c)
+                pr[c] = (uint64_t)(((u128)pr[c] + P - (h * (u128)pi[c] % P)) % P);
+        }
+        if (pivot_cols) pivot_cols[i] = (int32_t)j;
+        ++i;
+    }
+    if (rank) *rank = i;
+    return 0;
+}
+
+/* C = A.B mod p with 64-bit storage, plain triple loop (checks of the 64-bit results). */
+int oracle_matmul_modp64(const uint64_t *A, int64_t lda, const uint64_t *B, int64_t ldb, uint64_t *C, int64_t ldc,
+                         int64_t m, int64_t k, int64_t n, uint64_t p, int nthreads) {
+    const u128 P = p;
+    (void)nthreads;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) num_threads(nthreads) if (nthreads > 1)
+#endif
+    for (int64_t r = 0; r < m; ++r)
+        for (int64_t c = 0; c < n; ++c) {
+            u128 acc = 0;
+            for (int64_t t = 0; t < k; ++t)
+                acc = (acc + (u128)(A[r * lda + t] % p) * (u128)(B[t * ldb + c] % p) % P) % P;
+            C[r * ldc + c] = (uint64_t)acc;
+        }
+    return 0;
+}
+
+/* =====================================================================================================
+ * the paper's ORIGINAL floating-point mode: row reduction of a rectangular,
+ * possibly rank-deficient matrix to reduced echelon form with an explicit threshold deciding "which small
+ * quantities are treated as zero".  Steps, in the paper's order:
+ *   1. CudaSetRowScales / CudaRescaleRows: s_r = max_c |A[r,c]|, A[r,:] /= s_r
+ *      (a zero row stays zero).
+ *   2. for every column j, while rows are left (reading Q2):
+ *        k = arg max_{r >= i} |A[r,j]|, lowest index on ties (reading Q12); swap rows k and i
+ *        ("At this point, the maximum may still be a zero", :241);
+ *        head = A[i,j]; if |head| <= tol: nothing else happens, j advances (CudaCompareHeadToTolerance, :243, :251);
+ *        else row i /= head (:243); every other row r: row_r -= head_r * row_i on the columns from j on, and the
+ *        head of row r is SET to zero (:245-249); i advances (:251).
+ *   3. Reading Q19: what the thresholds declared zero is written as zero, so that the result is an
+ *      exact reduced echelon STRUCTURE ("zero rows possibly appearing at the bottom"): rows >= rank
+ *      become 0, and so do the entries of a pivot row left of its pivot (free-column residue below tol).
+ * tol < 0 selects max(rows, cols) * 2^-52 (reading Q10; the rescaled rows have max-norm 1).
+ * Returns 0, or -1 on bad arguments.
+ * ===================================================================================================== */
+int oracle_rref_f64(double *A, int64_t rows, int64_t cols, int64_t ld, double tol, int nthreads, int64_t *rank,
+                    int32_t *pivot_cols) {
+    if (rows < 0 || cols < 0 || ld < cols || (rows > 0 && cols > 0 && !A)) return -1;
+    if (tol < 0) tol = (double)(rows > cols ? rows : cols) * ldexp(1.0, -52);
+    (void)nthreads;
+    for (int64_t r = 0; r < rows; ++r) {
+        double s = 0.0;
+        for (int64_t c = 0; c < cols; ++c) { double v = fabs(A[r * ld + c]); if (v > s) s = v; }
+        if (s == 0.0) continue;
+        for (int64_t c = 0; c < cols; ++c) A[r * ld + c] /= s;
+    }
+    int64_t i = 0;
+    for (int64_t j = 0; j < cols && i < rows; ++j) {
+        int64_t k = i;
+        double best = fabs(A[i * ld + j]);
+        for (int64_t r = i + 1; r < rows; ++r) { double v = fabs(A[r * ld + j]); if (v > best) { best = v; k = r; } }
+        if (k != i)
+            for (int64_t c = 0; c < cols; ++c) { double t = A[i * ld + c]; A[i * ld + c] = A[k * ld + c]; A[k * ld + c] = t; }
+        const double head = A[i * ld + j];
+        if (!(fabs(head) > tol)) continue;
+        double *pi = A + i * ld;
+        for (int64_t c = j; c < cols; ++c) pi[c] /= head;
+        pi[j] = 1.0;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) num_threads(nthreads) if (nthreads > 1)
+#endif
+        for (int64_t r = 0; r < rows; ++r) {
+            if (r == i) continue;
+            double *pr = A + r * ld;
+            const double h = pr[j];
+            if (h == 0.0) continue;
+            for (int64_t c = j + 1; c < cols; ++c) pr[c] -= h * pi[c];
+            pr[j] = 0.0;
+        }
+        if (pivot_cols) pivot_cols[i] = (int32_t)j;
+        ++i;
+    }
+    if (rank) *rank = i;
+    /* step 3: flush what the thresholds declared zero */
+    for (int64_t r = i; r < rows; ++r)
+        for (int64_t c = 0; c < cols; ++c) A[r * ld + c] = 0.0;
+    if (pivot_cols)
+        for (int64_t r = 0; r < i; ++r)
+            for (int64_t c = 0; c < pivot_cols[r]; ++c) A[r * ld + c] = 0.0;
+    return 0;
+}

@@ -79,3 +79,64 @@ def test_backward_error_definition(oracle):
     expect = 1.0 / (np.abs(a).sum(axis=1).max() * np.abs(x[:, 1]).max() + np.abs(b2[:, 1]).max())
     assert abs(oracle.backward_error(a, x, b2) - expect) < 1e-12
     assert abs(oracle.backward_error(a, x, b2, nthreads=4) - expect) < 1e-12
+
+
+# ---------------------------------------------------------------- floating-point RREF with a threshold (8(f) rank 3)
+def _rref_exact(a_int):
+    """Exact rational RREF with sympy (independent black box); returns (float matrix, pivots)."""
+    import sympy
+    m, piv = sympy.Matrix(a_int.tolist()).rref()
+    return np.array(m.tolist(), dtype=np.float64), list(piv)
+
+
+def test_rref_f64_vs_exact_rational(oracle):
+    pytest.importorskip("sympy")
+    rng = np.random.default_rng(41)
+    for rows, cols, r in [(5, 7, 3), (7, 5, 4), (6, 6, 6), (6, 6, 2), (4, 9, 4), (8, 3, 2)]:
+        b = rng.integers(-4, 5, size=(rows, r))
+        c = rng.integers(-4, 5, size=(r, cols))
+        a = (b @ c).astype(np.int64)
+        want, piv = _rref_exact(a)
+        got, rank, gp = oracle.rref_f64(a.astype(np.float64), tol=1e-9)
+        assert rank == len(piv) and list(gp) == piv
+        assert np.allclose(got, want, rtol=0, atol=1e-11)
+        assert not got[rank:].any()                                 # flushed zero rows (reading Q19)
+        for k, c0 in enumerate(gp):                                 # exact structure: unit pivot columns, zeros on the left
+            assert got[k, c0] == 1.0 and np.count_nonzero(got[:, c0]) == 1 and not got[k, :c0].any()
+        got4, rank4, gp4 = oracle.rref_f64(a.astype(np.float64), tol=1e-9, nthreads=4)
+        assert rank4 == rank and np.array_equal(got4, got)
+
+
+def test_rref_f64_rank_vs_svd_and_rowspace(oracle):
+    for rows, cols, r, seed in [(40, 60, 17, 1), (60, 40, 25, 2), (50, 50, 50, 3)]:
+        a = gen.normal_matrix(rows, r, seed) @ gen.normal_matrix(r, cols, seed + 100)
+        a *= (10.0 ** gen.normal_matrix(rows, 1, seed + 200))       # badly scaled rows: the rescaling step matters
+        got, rank, piv = oracle.rref_f64(a, tol=1e-9)
+        s = np.linalg.svd(a / np.abs(a).max(axis=1, keepdims=True), compute_uv=False)
+        assert rank == int((s > 1e-9 * s[0]).sum()) == r
+        # every row of A lies in the row space of R: a = a[pivots] . R (R is the identity on the pivot columns)
+        recon = a[:, piv] @ got[:rank]
+        assert np.abs(recon - a).max() <= 1e-9 * np.abs(a).max()
+        # idempotence: reducing the result changes nothing beyond rounding
+        again, rank2, piv2 = oracle.rref_f64(got, tol=1e-9)
+        assert rank2 == rank and np.array_equal(piv2, piv) and np.allclose(again, got, rtol=0, atol=1e-10)
+
+
+def test_rref_f64_inverse_and_threshold(oracle):
+    n = 30
+    a, _ = gen.shifted_normal_system(n, 1, seed_a=7, seed_b=8)
+    got, rank, piv = oracle.rref_f64(np.hstack([a, np.eye(n)]))
+    assert rank == n and list(piv) == list(range(n))
+    # the row rescaling multiplies row r of (A | I) by 1/s_r; row operations never mix columns, so the
+    # right block is A^-1 regardless
+    assert np.allclose(got[:, n:], np.linalg.inv(a), rtol=1e-11, atol=1e-13)
+    # threshold semantics (PAPER.md:65, 243): a planted pivot of 1e-12 is a pivot for tol = 1e-15, zero for tol = 1e-9
+    m = np.array([[1.0, 2.0, 3.0], [0.0, 1e-12, 1.0], [0.0, 0.0, 1.0]])
+    _, rank_lo, piv_lo = oracle.rref_f64(m, tol=1e-15)
+    _, rank_hi, piv_hi = oracle.rref_f64(m, tol=1e-9)
+    assert (rank_lo, list(piv_lo)) == (3, [0, 1, 2]) and (rank_hi, list(piv_hi)) == (2, [0, 2])
+    # degenerate shapes
+    z, rank0, _ = oracle.rref_f64(np.zeros((3, 4)))
+    assert rank0 == 0 and not z.any()
+    e, ranke, _ = oracle.rref_f64(np.zeros((0, 4)))
+    assert ranke == 0 and e.shape == (0, 4)
