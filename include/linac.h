@@ -2,7 +2,9 @@
  * linac.h -- C ABI of the B200-native Linac hot path (arxiv/paper_2605_25863).
  *
  * Dense Gaussian elimination to REDUCED row-echelon form over a 32-bit prime field F_p
- * (uint32 storage, 2 <= p < 2^31), canonical null-space basis, and an fp64 partial-pivot solve.
+ * (uint32 storage, 2 <= p < 2^32; the tensor-core schedule for p < 2^31, a CUDA-core Montgomery schedule for
+ * 2^31 <= p < 2^32; uint64 storage for odd p < 2^63), canonical null-space basis, an fp64
+ * partial-pivot solve and the floating-point row reduction with a threshold.
  * Citations "PAPER.md:<line>" refer to the paper text this library was written from.
  *
  * Conventions (all entry points)
@@ -37,7 +39,7 @@ extern "C" {
 typedef enum {
     LINAC_OK = 0,
     LINAC_ERR_INVALID_ARG = 1,        /* null matrix with non-empty shape, negative size, ld < cols, cols >= 2^31 */
-    LINAC_ERR_BAD_MODULUS = 2,        /* p < 2, p >= 2^31, or p composite (deterministic Miller-Rabin on the host) */
+    LINAC_ERR_BAD_MODULUS = 2,        /* p outside the entry point's range, or p composite (deterministic Miller-Rabin on the host) */
     LINAC_ERR_WORKSPACE = 3,          /* workspace allocation failed */
     LINAC_ERR_CUDA = 4,               /* a CUDA call failed; linac_last_cuda_error() has the text */
     LINAC_ERR_SINGULAR = 5,           /* fp64: pivot with |pivot| <= tol */
@@ -80,6 +82,21 @@ int linac_release(void);
  */
 int linac_rref_u32(uint32_t *dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, void *stream,
                    int64_t *rank, int32_t *pivot_cols_out);
+
+/*
+ * Moduli: linac_rref_u32 (and linac_nullspace_u32 / linac_solve_u32 / linac_rank_factor_u32, which call it) accepts
+ * every prime 2 <= p <= 2^32 - 5 ("uint32 is used for p <= 2^32 - 1").  For p < 2^31 the blocked
+ * tensor-core schedule above runs; for 2^31 <= p < 2^32 the residues no longer fit four 8-bit limbs with a spare
+ * sign bit, and the call runs the CUDA-core Montgomery schedule of fp_wide.cu (blocked Gauss-Jordan, 32-column
+ * panels, no host synchronisation inside the loop) -- same result, same conventions.
+ *
+ * linac_rref_u64 -- the 64-bit backend of PAPER.md:163 ("uint64 for [larger p]"; the upper bound is lost in the
+ * extraction: this library takes odd primes 3 <= p < 2^63, reading Q18).  dA is DEVICE uint64, row-major;
+ * everything else as linac_rref_u32.  LINAC_ERR_BAD_MODULUS for p = 2, p >= 2^63 or composite p.
+ */
+int linac_rref_u64_workspace(int64_t rows, int64_t cols, size_t *bytes);
+int linac_rref_u64(uint64_t *dA, int64_t rows, int64_t cols, int64_t ld, uint64_t p, void *stream, int64_t *rank,
+                   int32_t *pivot_cols_out);
 
 /* ---- F_p: canonical null-space basis ------------------------------------------------------- */
 /*

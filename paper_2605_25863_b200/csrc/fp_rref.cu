@@ -357,7 +357,7 @@ struct PinnedRec {
 int validate(const uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p) {
     if (rows < 0 || cols < 0 || cols >= (1ll << 31) || rows >= (1ll << 31)) return LINAC_ERR_INVALID_ARG;
     if (rows > 0 && cols > 0 && (dA == nullptr || ld < cols)) return LINAC_ERR_INVALID_ARG;
-    if (p < 2 || p >= (1u << 31) || !is_prime_u32(p)) return LINAC_ERR_BAD_MODULUS;
+    if (p < 2 || !is_prime_u64(p)) return LINAC_ERR_BAD_MODULUS;
     return LINAC_OK;
 }
 
@@ -371,6 +371,9 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     if (!rank) return LINAC_ERR_INVALID_ARG;
     *rank = 0;
     if (rows == 0 || cols == 0) return LINAC_OK;
+    // 2^31 <= p < 2^32: the CUDA-core Montgomery path of fp_wide.cu; the limb-plane tensor path and the
+    // 64-bit accumulators of the strip kernels are built for p < 2^31
+    if (p >= (1u << 31)) return rref_u32_wide(dA, rows, cols, ld, p, s, rank, pivot_cols_out);
     rc = check_device();
     if (rc) return rc;
     rc = acquire_workspace(workspace_bytes(rows, cols), arena);
@@ -532,7 +535,7 @@ extern "C" {
 
 int linac_rref_u32_workspace(int64_t rows, int64_t cols, size_t* bytes) {
     if (!bytes || rows < 0 || cols < 0) return LINAC_ERR_INVALID_ARG;
-    *bytes = (rows == 0 || cols == 0) ? 0 : workspace_bytes(rows, cols);
+    *bytes = (rows == 0 || cols == 0) ? 0 : std::max(workspace_bytes(rows, cols), wide_workspace_u32(rows, cols));
     return LINAC_OK;
 }
 
@@ -683,7 +686,7 @@ int linac_nullspace_from_rref_u32(const uint32_t* dR, int64_t rows, int64_t cols
         return LINAC_ERR_INVALID_ARG;
     if (cols - rank > 0 && (!dK || ldk < cols - rank)) return LINAC_ERR_INVALID_ARG;
     if (rows > 0 && cols > 0 && (!dR || ld < cols)) return LINAC_ERR_INVALID_ARG;
-    if (p < 2 || p >= (1u << 31) || !is_prime_u32(p)) return LINAC_ERR_BAD_MODULUS;
+    if (p < 2 || !is_prime_u64(p)) return LINAC_ERR_BAD_MODULUS;
     int rc = check_device();
     if (rc) return rc;
     return nullspace_from_rref_impl(dR, rows, cols, ld, p, rank, pivot_cols, dK, ldk, (cudaStream_t)stream);

@@ -85,6 +85,30 @@ bool is_prime_u32(uint32_t n) {
     return true;
 }
 
+// Deterministic Miller-Rabin for every n < 2^64 (the first twelve primes as bases decide n < 3.3e24).
+bool is_prime_u64(uint64_t n) {
+    if (n < 2) return false;
+    const uint64_t bases[] = {2, 3, 5, 7, 11, 13, 17, 19, 23, 29, 31, 37};
+    for (uint64_t q : bases) {
+        if (n == q) return true;
+        if (n % q == 0) return false;
+    }
+    uint64_t d = n - 1;
+    int s = 0;
+    while ((d & 1) == 0) { d >>= 1; ++s; }
+    for (uint64_t a : bases) {
+        uint64_t x = powmod_u64(a, d, n);
+        if (x == 1 || x == n - 1) continue;
+        bool comp = true;
+        for (int i = 1; i < s; ++i) {
+            x = mulmod_u64(x, x, n);
+            if (x == n - 1) { comp = false; break; }
+        }
+        if (comp) return false;
+    }
+    return true;
+}
+
 ModP make_modp(uint32_t p) {
     ModP f;
     f.p = p;
@@ -120,7 +144,7 @@ const char* linac_status_string(int status) {
     switch (status) {
         case LINAC_OK: return "ok";
         case LINAC_ERR_INVALID_ARG: return "invalid argument";
-        case LINAC_ERR_BAD_MODULUS: return "modulus must be a prime with 2 <= p < 2^31";
+        case LINAC_ERR_BAD_MODULUS: return "modulus must be a prime in the range the entry point documents";
         case LINAC_ERR_WORKSPACE: return "workspace allocation failed";
         case LINAC_ERR_CUDA: return "CUDA error";
         case LINAC_ERR_SINGULAR: return "matrix is singular to the given tolerance";

@@ -70,6 +70,11 @@ int acquire_workspace(size_t bytes, Arena* arena);   // returns linac_status
 
 ModP make_modp(uint32_t p);
 bool is_prime_u32(uint32_t p);
+bool is_prime_u64(uint64_t p);                         // deterministic Miller-Rabin for every p < 2^64
+size_t wide_workspace_u32(int64_t rows, int64_t cols);
+// linac_rref_u32 for 2^31 <= p < 2^32 (fp_wide.cu); the caller holds the library mutex
+int rref_u32_wide(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, cudaStream_t s, int64_t* rank,
+                  int32_t* pivot_cols_out);
 int check_device();                                    // LINAC_OK or UNSUPPORTED_DEVICE / CUDA
 
 // ---- F_p GEMM  C -= Aop . B  (mod p) ------------------------------------------------------------

@@ -21,6 +21,7 @@ ERR_SINGULAR, ERR_BUFFER_TOO_SMALL, ERR_UNSUPPORTED_DEVICE, ERR_INTERNAL = 5, 6,
 SYMBOLS = [
     "linac_status_string", "linac_last_cuda_error", "linac_version",
     "linac_rref_u32_workspace", "linac_solve_f64_workspace", "linac_set_workspace", "linac_release",
+    "linac_rref_u64_workspace", "linac_rref_u64",
     "linac_rref_u32", "linac_nullspace_u32", "linac_nullspace_from_rref_u32", "linac_solve_u32", "linac_rank_factor_u32", "linac_load_matrix_u32", "linac_gemm_sub_u32",
     "linac_solve_f64",
     "linac_get_last_stats", "linac_set_option",
@@ -66,6 +67,8 @@ def _lib() -> C.CDLL:
         L.linac_solve_f64_workspace.argtypes = [i64, i64, C.POINTER(sz)]
         L.linac_set_workspace.argtypes = [vp, sz]
         L.linac_rref_u32.argtypes = [vp, i64, i64, i64, u32, vp, C.POINTER(i64), vp]
+        L.linac_rref_u64_workspace.argtypes = [i64, i64, C.POINTER(sz)]
+        L.linac_rref_u64.argtypes = [vp, i64, i64, i64, C.c_uint64, vp, C.POINTER(i64), vp]
         L.linac_nullspace_u32.argtypes = [vp, i64, i64, i64, u32, vp, C.POINTER(i64), vp, vp, i64, i64, C.POINTER(i64)]
         L.linac_nullspace_from_rref_u32.argtypes = [vp, i64, i64, i64, u32, i64, vp, vp, i64, vp]
         L.linac_solve_u32.argtypes = [vp, i64, i64, i64, i64, u32, vp, C.POINTER(i64), vp, vp, vp, i64]
@@ -152,6 +155,22 @@ def rref_u32(a: torch.Tensor, p: int):
         rc = _lib().linac_rref_u32(a.data_ptr(), rows, cols, ld, p, _stream_ptr(a.device), C.byref(rank), piv.data_ptr())
     if rc:
         raise LinacError(rc, "linac_rref_u32")
+    return int(rank.value), piv[: rank.value].clone()
+
+
+def rref_u64(a: torch.Tensor, p: int):
+    """In place: `a` (CUDA, int64/uint64 storage holding uint64 residues) -> its RREF over F_p, odd prime p < 2^63
+    (the 64-bit backend of PAPER.md:163).  Returns (rank, pivot_cols).  Mirrors linac_rref_u64."""
+    rows, cols, ld = _check_matrix(a, (torch.int64, torch.uint64), "a")
+    with torch.cuda.device(a.device):
+        need = C.c_size_t(0)
+        _lib().linac_rref_u64_workspace(rows, cols, C.byref(need))
+        _ensure_workspace(need.value, a.device)
+        rank = C.c_int64(0)
+        piv = torch.empty(max(1, min(rows, cols)), dtype=torch.int32)
+        rc = _lib().linac_rref_u64(a.data_ptr(), rows, cols, ld, p, _stream_ptr(a.device), C.byref(rank), piv.data_ptr())
+    if rc:
+        raise LinacError(rc, "linac_rref_u64")
     return int(rank.value), piv[: rank.value].clone()
 
 
