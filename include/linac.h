@@ -196,6 +196,24 @@ int linac_gemm_sub_u32(uint32_t *dC, int64_t ldc, const uint32_t *dA, int64_t ld
 int linac_solve_f64(double *dA, int64_t n, int64_t lda, double *dB, int64_t nrhs, int64_t ldb, double tol,
                     void *stream, int64_t *info);
 
+/* ---- floating point: row reduction with a threshold -------- */
+/*
+ * linac_rref_f64 -- the operation of cuda_row_reduce(matrix, field_characteristic=0) on a real matrix:
+ * in place, dA (DEVICE float64, rows x cols, ld) becomes its reduced row-echelon form, computed as the paper does:
+ * every row is first divided by its largest |entry| (CudaSetRowScales / CudaRescaleRows); then column
+ * by column the pivot is the largest |entry| among the rows left (partial pivoting), and a column
+ * whose pivot has |pivot| <= tol yields no pivot (CudaCompareHeadToTolerance, "explicitly control
+ * numerical thresholds").  Any shape; rank-deficient input is the point of the function.
+ *   tol   threshold on the row-scaled matrix; tol < 0 selects max(rows, cols) * 2^-52.
+ *   rank, pivot_cols_out   HOST out, as in linac_rref_u32.
+ * On return the pivots are exactly 1, pivot columns are exact unit vectors, and what the thresholds declared zero
+ * is written as zero: rows >= rank, and the entries of a pivot row left of its pivot (reading Q19).
+ * The schedule is a blocked Gauss-Jordan over 32-column panels (pivot search kernel + DMMA update of all other rows).
+ */
+int linac_rref_f64_workspace(int64_t rows, int64_t cols, size_t *bytes);
+int linac_rref_f64(double *dA, int64_t rows, int64_t cols, int64_t ld, double tol, void *stream, int64_t *rank,
+                   int32_t *pivot_cols_out);
+
 /* ---- instrumentation (host-side counters of the LAST F_p call; for tests and bench.py) ------ */
 typedef struct {
     int64_t kernel_launches;     /* kernels this library launched                                 */

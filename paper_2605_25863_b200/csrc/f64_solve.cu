@@ -16,6 +16,7 @@
 #include <algorithm>
 #include <climits>
 #include <mutex>
+#include <vector>
 
 #include "linac_internal.h"
 
@@ -57,13 +58,23 @@ struct Cand {                 // one CTA's arg-max candidate for a column, with 
     double2 content[FW];      // .x = the row's panel entries; .y = the column's tag (tagged mode: every 16-byte word validates itself)
 };
 
+// Tagged records: {payload, tag} travel as ONE 128-bit scalar memory operation (.b128, PTX ISA 8.3; SASS
+// STG/LDG.E.128.STRONG.GPU), relaxed at gpu scope.  A scalar access is a single operation of the memory model (a
+// .v2 vector access is modelled as two), so a reader sees either the old or the new 16 bytes, never a mix: the tag
+// validates the payload without a fence.
+__device__ __forceinline__ void st_b128(void* p, unsigned long long w0, unsigned long long w1) {
+    asm volatile("{ .reg .b128 t; mov.b128 t, {%0, %1}; st.relaxed.gpu.global.b128 [%2], t; }" ::"l"(w0), "l"(w1), "l"(p) : "memory");
+}
+__device__ __forceinline__ void ld_b128(const void* p, unsigned long long& w0, unsigned long long& w1) {
+    asm volatile("{ .reg .b128 t; ld.relaxed.gpu.global.b128 t, [%2]; mov.b128 {%0, %1}, t; }" : "=l"(w0), "=l"(w1) : "l"(p) : "memory");
+}
 __device__ __forceinline__ void st_tagged(double2* p, double v, unsigned tag) {
-    asm volatile("st.volatile.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(__double_as_longlong(v)), "l"((unsigned long long)tag) : "memory");
+    st_b128(p, (unsigned long long)__double_as_longlong(v), (unsigned long long)tag);
 }
 __device__ __forceinline__ double ld_tagged(const double2* p, unsigned tag) {      // spins until the word carries `tag`
     unsigned long long w0, w1;
     do {
-        asm volatile("ld.volatile.global.v2.u64 {%0, %1}, [%2];" : "=l"(w0), "=l"(w1) : "l"(p) : "memory");
+        ld_b128(p, w0, w1);
     } while ((unsigned)w1 != tag);
     return __longlong_as_double((long long)w0);
 }
@@ -88,19 +99,32 @@ __device__ __forceinline__ void warp_argmax(double& v, int& idx, int& aux) {
     aux = __shfl_sync(0xffffffffu, aux, who);
 }
 
+// What the panel kernel reports in RREF mode (device-resident: the host never reads it inside the loop).
+struct F64Rec {
+    long long i0;             // first pivot row of the panel
+    int r;                    // pivots found (<= FW)
+    int pad;
+    int pc[FW];               // local pivot columns, ascending (-1 beyond r)
+};
+
 // CLUSTER = false: cooperative kernel, one CTA per SM, grid barrier and candidate records in global memory (L2).
 // CLUSTER = true: ONE thread-block cluster of up to 16 CTAs holds the strip; the per-column barrier is the hardware
 // cluster barrier and the candidate records are read from the peers' shared memory (DSMEM), which cuts the
 // per-column latency from two L2 round trips and a grid barrier to about a microsecond.
-// Factors A[j0:n, j0:j0+w) in place (unit-lower L below, U on and above the
+// RREF = false (linac_solve_f64): factors A[j0:n, j0:j0+w) in place (unit-lower L below, U on and above the
 // diagonal), records the exchanges in ipiv[j0..j0+w).  CTA b owns rows [j0 + b*R, j0 + (b+1)*R).
-template <int FTHREADS, bool CLUSTER>
+// RREF = true (linac_rref_f64): the same elimination on the rows from i0 = *state on, as a pivot SEARCH only -- the
+// strip is not written back.  A column whose largest remaining entry is <= tol yields no pivot (CudaCompareHeadTo-
+// Tolerance) and the row counter does not advance; the pivot of ordinal t goes to row
+// i0 + t.  Outputs: ipiv[i0 + t] (exchanges), rec (i0, r, pivot columns), *state += r.
+template <int FTHREADS, bool CLUSTER, bool RREF>
 __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict__ A, int64_t n, int64_t lda, int64_t j0,
                                                               int w, int rows_per_cta, double tol,
                                                               Cand* __restrict__ cand /* [2][gridDim] */,
                                                               double2* __restrict__ target /* [2][FW] */,
                                                               long long* __restrict__ ipiv, int* __restrict__ info,
-                                                              unsigned tag0) {
+                                                              unsigned tag0, long long* __restrict__ state,
+                                                              F64Rec* __restrict__ rec, int32_t* __restrict__ pivcols) {
     extern __shared__ __align__(16) double S[];         // rows_per_cta x LDS
     constexpr int NE = FTHREADS / 32 * 4;               // arg-max entries per column: 4 row groups per warp
     __shared__ double s_val[NE];
@@ -108,6 +132,8 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
     __shared__ __align__(16) double pv_al[FW];
     __shared__ Cand l_cand[2];                          // CLUSTER: this CTA's records, read by the peers
     __shared__ double2 l_target[2][FW];
+    __shared__ int s_pc[FW];                            // RREF: pivot columns in discovery (= ascending) order
+    __shared__ int s_flag;                              // RREF: 1 iff the current column yields a pivot
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
     int G = gridDim.x, b = blockIdx.x;
     if constexpr (CLUSTER) { G = (int)cg::this_cluster().num_blocks(); b = (int)cg::this_cluster().block_rank(); }
@@ -120,7 +146,15 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
     };
     auto ld_f = [&](const double* p) { if constexpr (CLUSTER) return *p; else return __ldcg(p); };
     auto ld_i = [&](const long long* p) { if constexpr (CLUSTER) return *p; else return __ldcg(p); };
-    const int64_t r0 = j0 + (int64_t)b * rows_per_cta;
+    const int64_t i0 = RREF ? (int64_t)*state : j0;     // first row of the strip
+    if constexpr (RREF) {
+        if (i0 >= n) {                                  // no rows left: every remaining column is free (uniform exit)
+            if (b == 0 && tid == 0) { rec->i0 = i0; rec->r = 0; }
+            if (b == 0 && tid < FW) rec->pc[tid] = -1;
+            return;
+        }
+    }
+    const int64_t r0 = i0 + (int64_t)b * rows_per_cta;
     const int nr = (int)max((int64_t)0, min((int64_t)rows_per_cta, n - r0));
     constexpr int LDS = FW + 2;                         // even: the update reads rows as 16-byte pairs
     double* pv = pv_al;
@@ -128,9 +162,9 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
     for (int k = wq; k < nr; k += FTHREADS / 32) S[k * LDS + lane] = lane < w ? A[(r0 + k) * lda + j0 + lane] : 0.0;
     __syncthreads();
 
-    // second half of publishing column c: the warps' arg-max values are in s_val/s_idx (after a __syncthreads)
-    auto publish_tail = [&](int c) {
-        const int64_t jc = j0 + c;
+    // second half of publishing column c: the warps' arg-max values are in s_val/s_idx (after a __syncthreads);
+    // jc = the row the column's pivot will go to (its present content travels to the winner's owner)
+    auto publish_tail = [&](int c, int64_t jc) {
         if (wq == 0) {
             double best = -1.0;
             int bi = -1, none = 0;
@@ -152,7 +186,7 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
                 if (lane == 0) {
                     const unsigned long long w0 = (unsigned long long)__double_as_longlong(best);
                     const unsigned long long w1 = ((unsigned long long)tag << 32) | (unsigned)(bi >= 0 ? (int)(r0 + bi) : -1);
-                    asm volatile("st.volatile.global.v2.u64 [%0], {%1, %2};" ::"l"(&cd->absval), "l"(w0), "l"(w1) : "memory");
+                    st_b128(&cd->absval, w0, w1);
                 }
             } else {
                 if (bi >= 0) cd->content[lane] = make_double2(S[bi * LDS + lane], 0.0);
@@ -162,9 +196,8 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
         }
     };                                                      // always followed by group_sync(), which is a block barrier too
 
-    // publish the candidate for column c among own rows with absolute index >= j0 + c, and row j0+c itself
-    auto publish = [&](int c) {
-        const int64_t jc = j0 + c;
+    // publish the candidate for column c among own rows with absolute index >= jc, and row jc itself
+    auto publish = [&](int c, int64_t jc) {
         double best = -1.0;
         int bi = -1;
         for (int k = tid; k < nr; k += FTHREADS) {
@@ -176,14 +209,18 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
         warp_argmax(best, bi, none);
         if (lane < 4) { s_val[wq * 4 + lane] = best; s_idx[wq * 4 + lane] = lane == 0 ? bi : -1; }
         __syncthreads();
-        publish_tail(c);
+        publish_tail(c, jc);
     };
 
-    publish(0);
+    int npiv = 0;                                           // RREF: pivots found so far (uniform over the grid)
+    publish(0, i0);
     for (int c = 0; c < w; ++c) {
         const bool tagged = !CLUSTER && tag0 != 0;
         if (!tagged) group_sync();
-        const int64_t jc = j0 + c;
+        const int64_t jc = RREF ? i0 + npiv : j0 + c;       // the row this column's pivot goes to
+        if constexpr (RREF) {
+            if (jc >= n) break;                             // every row holds a pivot: the remaining columns are free
+        }
         // every CTA reduces the G candidates identically: largest |value|, lowest row on ties (reading Q12).
         // Warp 0 alone: up to CPL candidates per lane, their loads all in flight together (one round trip), one
         // warp arg-max, then the winner's row content (the second round trip).
@@ -206,7 +243,7 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
                             rr[u] = -1;
                             if (q < G) {
                                 unsigned long long w0, w1;
-                                asm volatile("ld.volatile.global.v2.u64 {%0, %1}, [%2];" : "=l"(w0), "=l"(w1) : "l"(&cand_of(c, q)->absval) : "memory");
+                                ld_b128(&cand_of(c, q)->absval, w0, w1);
                                 ok = ok && (unsigned)(w1 >> 32) == tag;
                                 v[u] = __longlong_as_double((long long)w0);
                                 rr[u] = (int)(unsigned)w1;
@@ -233,26 +270,38 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
                     }
             }
             warp_argmax(best, brow, bcta);
-            // the winner's row content; no candidate (a column of NaNs): flagged below
-            pv[lane] = bcta < 0 ? 0.0 : tagged ? ld_tagged(&cand_of(c, bcta)->content[lane], tag0 + (unsigned)c) : ld_f(&cand_of(c, bcta)->content[lane].x);
-            if (brow < 0) brow = (int)jc;
-            if (lane == 0 && b == 0) {
-                ipiv[jc] = brow;
-                if (!(best > tol)) atomicMin(info, (int)min((int64_t)INT_MAX, jc + 1));
+            const bool is_pivot = best > tol;
+            if (RREF && lane == 0) s_flag = is_pivot ? 1 : 0;   // next written after the block barriers of publish / update
+            if (!RREF || is_pivot) {
+                // the winner's row content; no candidate (a column of NaNs): flagged below
+                const double x = bcta < 0 ? 0.0 : tagged ? ld_tagged(&cand_of(c, bcta)->content[lane], tag0 + (unsigned)c) : ld_f(&cand_of(c, bcta)->content[lane].x);
+                if (brow < 0) brow = (int)jc;
+                if (lane == 0 && b == 0) {
+                    ipiv[jc] = brow;
+                    if (!RREF && !is_pivot) atomicMin(info, (int)min((int64_t)INT_MAX, jc + 1));
+                }
+                // exchange rows jc and g = brow (content of row jc comes from `target`, the pivot row from `pv`)
+                const long long g = brow;
+                if (g != jc && g >= r0 && g < r0 + nr) {
+                    const double2* tg = target + (c & 1) * FW;
+                    if constexpr (CLUSTER) tg = cg::this_cluster().map_shared_rank(&l_target[c & 1][0], (int)((jc - i0) / rows_per_cta));
+                    S[(int)(g - r0) * LDS + lane] = tagged ? ld_tagged(tg + lane, tag0 + (unsigned)c) : ld_f(&tg[lane].x);
+                }
+                if (jc >= r0 && jc < r0 + nr) S[(int)(jc - r0) * LDS + lane] = x;
+                pv[lane] = x;
             }
-            __syncwarp();
-            // exchange rows jc and g = brow (content of row jc comes from `target`, the pivot row from `pv`)
-            const long long g = brow;
-            if (g != jc && g >= r0 && g < r0 + nr) {
-                const double2* tg = target + (c & 1) * FW;
-                if constexpr (CLUSTER) tg = cg::this_cluster().map_shared_rank(&l_target[c & 1][0], (int)((jc - j0) / rows_per_cta));
-                S[(int)(g - r0) * LDS + lane] = tagged ? ld_tagged(tg + lane, tag0 + (unsigned)c) : ld_f(&tg[lane].x);
-            }
-            if (jc >= r0 && jc < r0 + nr) S[(int)(jc - r0) * LDS + lane] = pv[lane];
         }
         __syncthreads();
+        if constexpr (RREF) {
+            if (s_flag == 0) {                              // no pivot in this column: the row counter stays
+                if (c + 1 < w) publish(c + 1, jc);
+                continue;
+            }
+            if (tid == 0) s_pc[npiv] = c;
+            ++npiv;
+        }
         double piv = pv[c];
-        if (!(fabs(piv) > tol)) piv = 1.0;              // singular: flagged above; keep the arithmetic finite
+        if (!RREF && !(fabs(piv) > tol)) piv = 1.0;     // singular: flagged above; keep the arithmetic finite
         const double rp = __drcp_rn(piv);
         // multipliers and rank-1 update of own rows below jc: a warp takes four rows per pass, eight lanes per row,
         // four columns per lane (two 16-byte accesses each way).  The lane that holds column c+1 sees the new
@@ -284,12 +333,23 @@ __global__ void __launch_bounds__(FTHREADS) f64_panel_kernel(double* __restrict_
         if (c + 1 < w) {
             if (seg == ns) { s_val[wq * 4 + rg] = best; s_idx[wq * 4 + rg] = bi; }
             __syncthreads();
-            publish_tail(c + 1);
+            publish_tail(c + 1, jc + 1);
         }
     }
     __syncthreads();                                        // the last column's updates (rows change warps per column)
-    for (int k = wq; k < nr; k += FTHREADS / 32)
-        if (lane < w) A[(r0 + k) * lda + j0 + lane] = S[k * LDS + lane];
+    if constexpr (RREF) {
+        if (b == 0) {
+            if (tid < FW) {
+                const int pc = tid < npiv ? s_pc[tid] : -1;
+                rec->pc[tid] = pc;
+                if (tid < npiv) pivcols[i0 + tid] = (int32_t)(j0 + pc);
+            }
+            if (tid == 0) { rec->i0 = i0; rec->r = npiv; *state = i0 + npiv; }
+        }
+    } else {
+        for (int k = wq; k < nr; k += FTHREADS / 32)
+            if (lane < w) A[(r0 + k) * lda + j0 + lane] = S[k * LDS + lane];
+    }
     if constexpr (CLUSTER) cg::this_cluster().sync();   // no CTA may leave while a peer can still read its records
 }
 
@@ -474,7 +534,11 @@ template <int TN, bool ASSIGN, int NW>
 __global__ void __launch_bounds__(NW * 32, TN == 64 ? 2 : 1) dgemm_sub_mma_kernel(double* C, int64_t ldc,
                                                             const double* __restrict__ A, int64_t lda,
                                                             const double* B, int64_t ldb, int64_t M,
-                                                            int64_t N, int64_t K) {
+                                                            int64_t N, int64_t K, const int* __restrict__ kact) {
+    if (kact != nullptr) {                                 // K read from device memory (linac_rref_f64: the panel's pivot count)
+        K = min(K, (int64_t)*kact);
+        if (K <= 0) return;
+    }
     constexpr int NJ = TN / 32;                            // MMA tiles per warp along n
     constexpr int NT = NW * 32;                            // threads: 8 warps as 2 x 4 (16 as 4 x 4 measured no faster)
     constexpr int MI = 64 / NW;                            // MMA tiles per warp along m (warp tile 64 or 32 rows)
@@ -682,7 +746,7 @@ struct F64 {
 };
 
 int dgemm_sub(F64& c, double* C, int64_t ldc, const double* A, int64_t lda, const double* B, int64_t ldb, int64_t M,
-              int64_t N, int64_t K, bool assign = false) {
+              int64_t N, int64_t K, bool assign = false, const int* kact = nullptr) {
     if (M <= 0 || N <= 0 || K <= 0) return LINAC_OK;
     // 128 x 64 tiles with two CTAs per SM (16 warps in flight) beat one 128 x 128 CTA per SM on every shape measured
     // (c4: 225 -> 217 ms); option f64_mma = 2 keeps the 128 x 128 tile for A/B runs
@@ -690,13 +754,13 @@ int dgemm_sub(F64& c, double* C, int64_t ldc, const double* A, int64_t lda, cons
     const int tn = skinny ? 64 : DN;
     dim3 grid((unsigned)((N + tn - 1) / tn), (unsigned)((M + DM - 1) / DM));
     if (assign)
-        dgemm_sub_mma_kernel<64, true, 8><<<grid, 256, dmma_smem_bytes(64), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
-    else if (options().f64_mma == 0)
+        dgemm_sub_mma_kernel<64, true, 8><<<grid, 256, dmma_smem_bytes(64), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K, kact);
+    else if (options().f64_mma == 0 && kact == nullptr)
         dgemm_sub_kernel<<<grid, DTHREADS, 0, c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
     else if (skinny)
-        dgemm_sub_mma_kernel<64, false, 8><<<grid, 256, dmma_smem_bytes(64), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
+        dgemm_sub_mma_kernel<64, false, 8><<<grid, 256, dmma_smem_bytes(64), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K, kact);
     else
-        dgemm_sub_mma_kernel<128, false, 8><<<grid, 256, dmma_smem_bytes(128), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
+        dgemm_sub_mma_kernel<128, false, 8><<<grid, 256, dmma_smem_bytes(128), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K, kact);
     LINAC_CUDA(cudaGetLastError());
     stats().kernel_launches++;
     stats().update_macs += M * N * K;
@@ -780,7 +844,8 @@ int panel_f64(F64& c, int64_t j0, int w) {
     double* A = c.A; int64_t n = c.n, lda = c.lda; double tol = c.tol;
     Cand* cand = c.cand; double2* target = c.target; long long* ipiv = c.ipiv; int* info = c.info;
     unsigned tag0 = options().f64_panel_tags != 0 ? (unsigned)(j0 + 1) : 0u;   // column j carries tag j + 1 within a solve
-    void* args[] = {&A, &n, &lda, &j0, &w, &rows_per_cta, &tol, &cand, &target, &ipiv, &info, &tag0};
+    long long* state = nullptr; F64Rec* rec = nullptr; int32_t* pivcols = nullptr;      // RREF mode only
+    void* args[] = {&A, &n, &lda, &j0, &w, &rows_per_cta, &tol, &cand, &target, &ipiv, &info, &tag0, &state, &rec, &pivcols};
     if (c.cluster_ctas > 0 && m <= (int64_t)c.cluster_ctas * std::min<int64_t>(c.rows_cap, options().f64_cluster_rows)) {
         rows_per_cta = std::max(1, (int)((m + c.cluster_ctas - 1) / c.cluster_ctas));
         smem = (size_t)rows_per_cta * (FW + 2) * sizeof(double);
@@ -796,13 +861,13 @@ int panel_f64(F64& c, int64_t j0, int w) {
         at[0].val.clusterDim.z = 1;
         cfg.attrs = at;
         cfg.numAttrs = 1;
-        LINAC_CUDA(cudaLaunchKernelEx(&cfg, f64_panel_kernel<512, true>, A, n, lda, j0, w, rows_per_cta, tol, cand, target, ipiv, info, 0u));
+        LINAC_CUDA(cudaLaunchKernelEx(&cfg, f64_panel_kernel<512, true, false>, A, n, lda, j0, w, rows_per_cta, tol, cand, target, ipiv, info, 0u, state, rec, pivcols));
     } else if (c.panel_threads == 1024)
-        LINAC_CUDA(cudaLaunchCooperativeKernel((void*)f64_panel_kernel<1024, false>, dim3(c.grid), dim3(1024), args, smem, c.s));
+        LINAC_CUDA(cudaLaunchCooperativeKernel((void*)f64_panel_kernel<1024, false, false>, dim3(c.grid), dim3(1024), args, smem, c.s));
     else if (c.panel_threads == 512)
-        LINAC_CUDA(cudaLaunchCooperativeKernel((void*)f64_panel_kernel<512, false>, dim3(c.grid), dim3(512), args, smem, c.s));
+        LINAC_CUDA(cudaLaunchCooperativeKernel((void*)f64_panel_kernel<512, false, false>, dim3(c.grid), dim3(512), args, smem, c.s));
     else
-        LINAC_CUDA(cudaLaunchCooperativeKernel((void*)f64_panel_kernel<256, false>, dim3(c.grid), dim3(256), args, smem, c.s));
+        LINAC_CUDA(cudaLaunchCooperativeKernel((void*)f64_panel_kernel<256, false, false>, dim3(c.grid), dim3(256), args, smem, c.s));
     // exchanges on the rest of A (left L part and right trailing part) and on B
     const int64_t ncol = c.n;
     f64_swap_kernel<<<(unsigned)((ncol + 255) / 256), 256, 0, c.s>>>(c.A, c.lda, 0, ncol, j0, j0 + w, c.ipiv, j0, w);
@@ -853,6 +918,136 @@ int factor_flat_f64(F64& c) {
     return LINAC_OK;
 }
 
+// ---------------------------------------------------------------- floating-point RREF
+// linac_rref_f64: the paper's original mode -- a rectangular, possibly rank-deficient
+// matrix reduced to echelon form with a threshold.  Blocked Gauss-Jordan over 32-column panels, no host
+// synchronisation inside the loop (row counter and panel records live on the device):
+//   f64_panel_kernel<RREF>     pivot search with partial pivoting and the threshold test on the updated column
+//   f64_rref_swap_kernel       row exchanges (K5)
+//   f64_rref_pivot_rows_kernel U = D^-1 . A[pivot rows, j0:], D = the panel's pivot block (Gauss-Jordan without
+//                              further pivoting: the rows are in the order partial pivoting chose them), exactly the
+//                              identity on the pivot columns
+//   f64_rref_lcopy_kernel      L[k][t] = A[k][pivot column t], zero for the pivot rows themselves
+//   dgemm_sub_mma_kernel       A[:, j0:] -= L . U for ALL rows (above too, as in the paper's RowReduce), on DMMA
+// so the matrix ends as the RREF without a back-elimination pass.
+__global__ void f64_rref_swap_kernel(double* __restrict__ M, int64_t ld, int64_t c0, int64_t cols,
+                                     const F64Rec* __restrict__ rec, const long long* __restrict__ ipiv) {
+    const int r = rec->r;
+    if (r == 0) return;
+    const int64_t c = c0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= cols) return;
+    const int64_t i0 = rec->i0;
+    for (int a = 0; a < r; ++a) {
+        const int64_t s = ipiv[i0 + a];
+        if (s != i0 + a) {
+            const double x = M[(i0 + a) * ld + c], y = M[s * ld + c];
+            M[(i0 + a) * ld + c] = y;
+            M[s * ld + c] = x;
+        }
+    }
+}
+
+// T = D^-1, D = A[i0 : i0+r, pivot columns] after the exchanges (one CTA; its own launch, so that the kernel below can
+// overwrite the pivot rows while every CTA of it reads the same T).
+__global__ void __launch_bounds__(128) f64_rref_tinv_kernel(const double* __restrict__ A, int64_t ld, int64_t j0,
+                                                           const F64Rec* __restrict__ rec, double* __restrict__ Tout) {
+    __shared__ double G[FW][2 * FW + 1];
+    __shared__ int s_pc[FW];
+    const int r = rec->r;
+    const int tid = threadIdx.x;
+    if (r == 0) return;
+    const int64_t i0 = rec->i0;
+    if (tid < FW) s_pc[tid] = rec->pc[tid];
+    __syncthreads();
+    for (int e = tid; e < FW * 2 * FW; e += 128) {
+        const int a = e / (2 * FW), b = e % (2 * FW);
+        double v = 0.0;
+        if (a < r) {
+            if (b < FW) { if (b < r) v = A[(i0 + a) * ld + j0 + s_pc[b]]; }
+            else v = (b - FW == a) ? 1.0 : 0.0;
+        }
+        G[a][b] = v;
+    }
+    __syncthreads();
+    // Gauss-Jordan on [D | I]: thread = (row a, 16 columns); two phases per step so nobody reads a half-updated row t
+    const int a = tid >> 2, cg0 = (tid & 3) * 16;
+    for (int t = 0; t < r; ++t) {
+        const double d = G[t][t], h = G[a][t];
+        double pt[16];
+#pragma unroll
+        for (int q = 0; q < 16; ++q) pt[q] = G[t][cg0 + q] / d;
+        __syncthreads();
+        if (a < r) {
+#pragma unroll
+            for (int q = 0; q < 16; ++q) G[a][cg0 + q] = a == t ? pt[q] : G[a][cg0 + q] - h * pt[q];
+        }
+        __syncthreads();
+    }
+    for (int e = tid; e < FW * FW; e += 128) Tout[e] = G[e / FW][FW + e % FW];
+}
+
+// U = T . A[i0 : i0+r, c] for the columns c >= j0 (thread per column); written to the pivot rows and to the U buffer.
+__global__ void __launch_bounds__(128) f64_rref_pivot_rows_kernel(double* __restrict__ A, int64_t ld, int64_t j0, int64_t cols,
+                                                                 const F64Rec* __restrict__ rec, const double* __restrict__ Tin,
+                                                                 double* __restrict__ U, int64_t ldu) {
+    __shared__ double Ts[FW][FW + 1];
+    __shared__ int s_pc[FW];
+    const int r = rec->r;
+    const int tid = threadIdx.x;
+    if (r == 0) return;
+    const int64_t i0 = rec->i0;
+    if (tid < FW) s_pc[tid] = rec->pc[tid];
+    for (int e = tid; e < FW * FW; e += 128) Ts[e / FW][e % FW] = Tin[e];
+    __syncthreads();
+    const int64_t c = j0 + (int64_t)blockIdx.x * 128 + tid;
+    if (c >= cols) return;
+    int piv_ord = -1;                                       // is c one of the panel's pivot columns?
+    if (c - j0 < FW)
+        for (int t = 0; t < r; ++t) if (s_pc[t] == (int)(c - j0)) piv_ord = t;
+    double x[FW];
+#pragma unroll
+    for (int b = 0; b < FW; ++b) x[b] = b < r ? A[(i0 + b) * ld + c] : 0.0;
+    for (int q = 0; q < FW; ++q) {
+        double acc = 0.0;
+        if (q < r) {
+#pragma unroll
+            for (int b = 0; b < FW; ++b) acc += Ts[q][b] * x[b];
+            if (piv_ord >= 0) acc = piv_ord == q ? 1.0 : 0.0;      // exactly the identity on the pivot columns
+            A[(i0 + q) * ld + c] = acc;
+        }
+        U[(int64_t)q * ldu + c] = acc;
+    }
+}
+
+__global__ void f64_rref_lcopy_kernel(const double* __restrict__ A, int64_t ld, int64_t rows, int64_t j0,
+                                      const F64Rec* __restrict__ rec, double* __restrict__ L) {
+    const int r = rec->r;
+    if (r == 0) return;
+    const int t = threadIdx.x & 31;
+    const int64_t i0 = rec->i0;
+    const int pc = rec->pc[t];
+    for (int64_t k = (int64_t)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); k < rows; k += (int64_t)gridDim.x * (blockDim.x / 32)) {
+        const bool pivot_row = k >= i0 && k < i0 + r;
+        L[k * FW + t] = (pc >= 0 && !pivot_row) ? A[k * ld + j0 + pc] : 0.0;
+    }
+}
+
+// Reading Q19: what the thresholds declared zero is written as zero -- rows >= rank, and the entries of a pivot row
+// left of its pivot (sub-threshold residue in free columns).  One CTA per row.
+__global__ void f64_rref_finalize_kernel(double* __restrict__ A, int64_t ld, int64_t rows, int64_t cols,
+                                         const long long* __restrict__ state, const int32_t* __restrict__ pivcols) {
+    const int64_t k = blockIdx.x;
+    const int64_t rank = *state;
+    const int64_t end = k < rank ? pivcols[k] : cols;
+    for (int64_t c = threadIdx.x; c < end; c += blockDim.x) A[k * ld + c] = 0.0;
+}
+
+size_t f64_rref_workspace_bytes(int64_t rows, int64_t cols) {
+    const int64_t ldu = (cols + 63) / 64 * 64;
+    return 16384 + 2 * 1024 * sizeof(Cand) + 2 * FW * sizeof(double2) + (size_t)std::max<int64_t>(rows, 1) * 8 +
+           (size_t)FW * ldu * 8 + (size_t)rows * FW * 8 + (size_t)std::max<int64_t>(1, std::min(rows, cols)) * 4;
+}
+
 size_t f64_workspace_bytes(int64_t n) {
     (void)n;
     const size_t inv = 2 * (size_t)((n + TB - 1) / TB) * TB * TB * sizeof(double);
@@ -901,15 +1096,15 @@ int linac_solve_f64(double* dA, int64_t n, int64_t lda, double* dB, int64_t nrhs
     c.smem_max = (size_t)smem_optin - 4096;
     c.rows_cap = (int)(c.smem_max / ((FW + 2) * sizeof(double)));
     if ((n + c.grid - 1) / c.grid > c.rows_cap) return LINAC_ERR_INVALID_ARG;   // n > ~118k: strip no longer fits on chip
-    LINAC_CUDA(cudaFuncSetAttribute(f64_panel_kernel<256, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max));
-    LINAC_CUDA(cudaFuncSetAttribute(f64_panel_kernel<512, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max));
-    LINAC_CUDA(cudaFuncSetAttribute(f64_panel_kernel<1024, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max));
+    LINAC_CUDA(cudaFuncSetAttribute(f64_panel_kernel<256, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max));
+    LINAC_CUDA(cudaFuncSetAttribute(f64_panel_kernel<512, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max));
+    LINAC_CUDA(cudaFuncSetAttribute(f64_panel_kernel<1024, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max));
     c.cluster_ctas = 0;
     if (options().f64_panel_cluster > 0) {                 // one cluster of up to 16 CTAs (non-portable size), if the device places it
         const int want = (int)options().f64_panel_cluster;
-        cudaError_t ce = cudaFuncSetAttribute(f64_panel_kernel<512, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max);
+        cudaError_t ce = cudaFuncSetAttribute(f64_panel_kernel<512, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max);
         if (ce == cudaSuccess && want > 8)
-            ce = cudaFuncSetAttribute(f64_panel_kernel<512, true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+            ce = cudaFuncSetAttribute(f64_panel_kernel<512, true, false>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
         if (ce == cudaSuccess) {
             cudaLaunchConfig_t cfg = {};
             cfg.gridDim = dim3(want);
@@ -923,7 +1118,7 @@ int linac_solve_f64(double* dA, int64_t n, int64_t lda, double* dB, int64_t nrhs
             cfg.attrs = at;
             cfg.numAttrs = 1;
             int nclusters = 0;
-            ce = cudaOccupancyMaxActiveClusters(&nclusters, f64_panel_kernel<512, true>, &cfg);
+            ce = cudaOccupancyMaxActiveClusters(&nclusters, f64_panel_kernel<512, true, false>, &cfg);
             if (ce == cudaSuccess && nclusters >= 1) c.cluster_ctas = want;
         }
         if (ce != cudaSuccess) (void)cudaGetLastError();    // not available: the cooperative kernel does every panel
@@ -976,6 +1171,95 @@ int linac_solve_f64(double* dA, int64_t n, int64_t lda, double* dB, int64_t nrhs
         *info_out = h_info;
         return LINAC_ERR_SINGULAR;
     }
+    return LINAC_OK;
+}
+
+int linac_rref_f64_workspace(int64_t rows, int64_t cols, size_t* bytes) {
+    if (!bytes || rows < 0 || cols < 0) return LINAC_ERR_INVALID_ARG;
+    *bytes = (rows == 0 || cols == 0) ? 0 : f64_rref_workspace_bytes(rows, cols);
+    return LINAC_OK;
+}
+
+int linac_rref_f64(double* dA, int64_t rows, int64_t cols, int64_t ld, double tol, void* stream, int64_t* rank_out,
+                   int32_t* pivot_cols_out) {
+    std::lock_guard<std::mutex> lock(g_call_mutex);
+    linac_stats& st = stats();
+    st = linac_stats{};
+    if (rows < 0 || cols < 0 || rows >= (1ll << 31) || cols >= (1ll << 31) || !rank_out) return LINAC_ERR_INVALID_ARG;
+    *rank_out = 0;
+    if (rows == 0 || cols == 0) return LINAC_OK;
+    if (!dA || ld < cols) return LINAC_ERR_INVALID_ARG;
+    int rc = check_device();
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    Arena arena;
+    rc = acquire_workspace(f64_rref_workspace_bytes(rows, cols), &arena);
+    if (rc) return rc;
+    F64 c{};
+    c.A = dA; c.n = rows; c.lda = ld; c.B = nullptr; c.nrhs = 0; c.ldb = 0; c.s = s;
+    c.tol = tol < 0 ? (double)std::max(rows, cols) * 2.220446049250313e-16 : tol;
+    int dev = 0, sms = 0, smem_optin = 0;
+    LINAC_CUDA(cudaGetDevice(&dev));
+    LINAC_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    LINAC_CUDA(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    c.grid = std::min(sms, 1024);
+    c.smem_max = (size_t)smem_optin - 4096;
+    c.rows_cap = (int)(c.smem_max / ((FW + 2) * sizeof(double)));
+    int rows_per_cta = (int)((rows + c.grid - 1) / c.grid);
+    if (rows_per_cta > c.rows_cap) return LINAC_ERR_INVALID_ARG;          // rows > ~118k: the strip no longer fits on chip
+    LINAC_CUDA(cudaFuncSetAttribute(f64_panel_kernel<512, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem_max));
+    LINAC_CUDA(cudaFuncSetAttribute(dgemm_sub_mma_kernel<128, false, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dmma_smem_bytes(128)));
+    LINAC_CUDA(cudaFuncSetAttribute(dgemm_sub_mma_kernel<64, false, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dmma_smem_bytes(64)));
+    const int64_t mn = std::min(rows, cols), ldu = (cols + 63) / 64 * 64;
+    Cand* cand = (Cand*)arena.take(2 * 1024 * sizeof(Cand));
+    double2* target = (double2*)arena.take(2 * FW * sizeof(double2));
+    long long* ipiv = (long long*)arena.take((size_t)rows * 8);
+    long long* state = (long long*)arena.take(256);
+    int* dummy_info = (int*)(state + 8);
+    F64Rec* rec = (F64Rec*)arena.take(sizeof(F64Rec));
+    double* U = (double*)arena.take((size_t)FW * ldu * 8);
+    double* L = (double*)arena.take((size_t)rows * FW * 8);
+    int32_t* d_piv = (int32_t*)arena.take((size_t)mn * 4);
+    double* Tb = (double*)arena.take(FW * FW * 8);
+    if (!cand || !target || !ipiv || !state || !rec || !U || !L || !d_piv || !Tb) return LINAC_ERR_WORKSPACE;
+    LINAC_CUDA(cudaMemsetAsync(state, 0, 256, s));
+    LINAC_CUDA(cudaMemsetAsync(cand, 0, 2 * 1024 * sizeof(Cand), s));
+    LINAC_CUDA(cudaMemsetAsync(target, 0, 2 * FW * sizeof(double2), s));
+    row_scale_kernel<<<(unsigned)rows, 256, 0, s>>>(dA, cols, ld, nullptr, 0, 0, dummy_info);        // K1/K2; zero rows stay zero
+    LINAC_CUDA(cudaGetLastError());
+    st.kernel_launches++;
+    const size_t smem = (size_t)rows_per_cta * (FW + 2) * sizeof(double);
+    double tolv = c.tol;
+    int* info = dummy_info;
+    for (int64_t j0 = 0; j0 < cols; j0 += FW) {
+        int w = (int)std::min<int64_t>(FW, cols - j0);
+        int64_t j0v = j0, nv = rows, ldv = ld;
+        const int64_t nc = cols - j0;
+        unsigned tag0 = options().f64_panel_tags != 0 ? (unsigned)(j0 + 1) : 0u;
+        void* args[] = {&dA, &nv, &ldv, &j0v, &w, &rows_per_cta, &tolv, &cand, &target, &ipiv, &info, &tag0, &state, &rec, &d_piv};
+        LINAC_CUDA(cudaLaunchCooperativeKernel((void*)f64_panel_kernel<512, false, true>, dim3(c.grid), dim3(512), args, smem, s));
+        f64_rref_swap_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, s>>>(dA, ld, j0, cols, rec, ipiv);
+        f64_rref_tinv_kernel<<<1, 128, 0, s>>>(dA, ld, j0, rec, Tb);
+        f64_rref_pivot_rows_kernel<<<(unsigned)((nc + 127) / 128), 128, 0, s>>>(dA, ld, j0, cols, rec, Tb, U, ldu);
+        f64_rref_lcopy_kernel<<<(unsigned)std::min<int64_t>((rows + 7) / 8, 148 * 8), 256, 0, s>>>(dA, ld, rows, j0, rec, L);
+        LINAC_CUDA(cudaGetLastError());
+        st.kernel_launches += 5;
+        st.panels++;
+        rc = dgemm_sub(c, dA + j0, ld, L, FW, U + j0, ldu, rows, nc, FW, false, &rec->r);
+        if (rc) return rc;
+    }
+    f64_rref_finalize_kernel<<<(unsigned)rows, 256, 0, s>>>(dA, ld, rows, cols, state, d_piv);
+    LINAC_CUDA(cudaGetLastError());
+    st.kernel_launches++;
+    long long h_rank = 0;
+    std::vector<int32_t> piv((size_t)mn);
+    LINAC_CUDA(cudaMemcpyAsync(&h_rank, state, 8, cudaMemcpyDeviceToHost, s));
+    LINAC_CUDA(cudaMemcpyAsync(piv.data(), d_piv, (size_t)mn * 4, cudaMemcpyDeviceToHost, s));
+    LINAC_CUDA(cudaStreamSynchronize(s));
+    st.host_syncs++;
+    if (h_rank < 0 || h_rank > mn) return LINAC_ERR_INTERNAL;
+    *rank_out = h_rank;
+    if (pivot_cols_out) std::copy(piv.begin(), piv.begin() + h_rank, pivot_cols_out);
     return LINAC_OK;
 }
 
