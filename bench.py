@@ -1,19 +1,27 @@
 #!/usr/bin/env python
 """bench.py -- one JSON line for the Linac hot path on B200 (contract: see DESIGN.md "Measurement").
 
-A "step" is one pass of the whole hot path (S0 ingest .. S7 finalise) over one
-seeded synthetic matrix of the workload BASELINE.json's metric is quoted on: config c3, the
-paper's N = 10^4 point (dense uniform over F_{2^31-1}).  `--workload c2|c5|...`
-selects another config; the default finishes in well under a minute.
+A "step" is one pass of the whole hot path (S0 ingest .. S7 finalise) over one seeded synthetic
+matrix.  The HEADLINE workload is config c3, the paper's N = 10^4 point (dense uniform over F_{2^31-1}, PAPER.md:59,
+308): `value`, `ms_per_step`, `e2e`, `roofline`, `clocks` describe it.  The default run (1 GPU, no --workload) also
+carries one leg per remaining config and per widened row, each with its own timing, clocks and roofline:
 
-  value      : whole-job Gmulmod/s = (2 N^3 / 3) / t, matrix already resident in HBM, t = CUDA-event
-               time of the C-ABI call (max over ranks); N > 1 runs independent replicas (weak).
+  legs.c1, legs.c2   the small F_p configs (c2 with the null space), latency chains: us per pivot
+  legs.c5            N = 10^5 (40 GB, generated on the device): 1 warm-up + 2 timed calls
+  legs.fp64_solve    config c4 through linac_solve_f64: ms per solve, GFLOP/s, backward error
+  legs.rref_f64      SURVEY.md 8(f)#3: linac_rref_f64 on a rank-deficient float64 matrix
+  legs.wide_u32/u64  SURVEY.md 8(f)#4: linac_rref_u32 with p = 2^32 - 5 and linac_rref_u64 with p = 2^61 - 1
+
+  value      : whole-job Gmulmod/s = (2 N^3 / 3) / t, matrix already resident in HBM, t = CUDA-event time of the C-ABI
+               call (max over ranks); N > 1 runs independent replicas (weak scaling, no collective on the data path).
   e2e        : same metric with HOST buffers: pinned H2D of the matrix + call + D2H of the RREF every step, double
-               buffered (the copies of neighbouring steps overlap the call); the strictly serial figure is kept
-               beside it as e2e.serial_ms_per_step.
-  roofline   : the Schur-update kernel (dominant): executed field MACs / its event-timed duration.
-  cpu_baseline: the CPU oracle timed on a bounded sample on this box's host cores.
-  fp64       : (default workload only) linac_solve_f64 on config c4: ms per solve, GFLOP/s, backward error.
+               buffered; the strictly serial figure is kept beside it as e2e.serial_ms_per_step.
+  roofline   : the Schur-update kernels (dominant class): executed u8 multiply-accumulates / their CUDA-event time in
+               the PRODUCTION schedule (option timing = 2: an event pair around every launch, no host syncs), against
+               the int8 tensor peak linac_measure_peak measures live in this run (tcgen05.mma kind::i8 from on-chip
+               operands): the 2 ms burst figure when the step held the maximum clock, the 400 ms power-capped one
+               otherwise.  roofline.whole_step_frac puts the whole step against the same peak.
+  cpu_baseline: the CPU oracle timed on this box's host cores on bounded samples, with labelled cubic extrapolations.
 """
 from __future__ import annotations
 
@@ -34,12 +42,9 @@ import linac_inputs as gen  # noqa: E402
 
 WORKLOAD_KIND = {"uniform": "dense uniform", "lowrank": "product of uniform factors (exact rank)",
                  "sparse_dep": "90% zeros, every 50th row dependent"}
-
-#: ncu --set full, gemm_tc_panel_kernel, second launch of a c3 call (profiles/r01_v9_launches_c3.md)
-NCU_TOP_LAUNCH_DRAM_BYTES_C3 = 396063488 + 324826368
-
-PAPER_A100_GMULMOD = {"c3": (2 * 1e4 ** 3 / 3) / 3.6 / 1e9,            # PAPER.md:59  (3.6 s at N = 10^4)
-                      "c5": (2 * 1e5 ** 3 / 3) / (45 * 60) / 1e9}       # PAPER.md:61  (45 min at N = 10^5)
+BASELINE_CONTEXT = ("paper, A100: 3.6 s at N=1e4 (PAPER.md:59) = 185 Gmulmod/s, 45 min at N=1e5 (PAPER.md:61) = 247 "
+                    "Gmulmod/s; another machine, context only (BASELINE.json publishes no number for this metric)")
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r02_traffic.json")      # written from an ncu --set full capture of HEAD
 
 
 def load_peaks():
@@ -47,7 +52,7 @@ def load_peaks():
     if os.path.exists(path):
         d = json.load(open(path))
         return dict(hbm_gbs=d["hbm_gbs"], bf16_burst=d["bf16_tflops"], bf16_sustained=d["bf16_tflops_sustained"],
-                    sm_max_mhz=d.get("sm_max_mhz", 1965.0), source="measured")
+                    sm_max_mhz=d.get("sm_max_mhz", 1965.0), source="MEASURED_PEAKS.json")
     return dict(hbm_gbs=6650.0, bf16_burst=1590.0, bf16_sustained=1400.0, sm_max_mhz=1965.0, source="fallback")
 
 
@@ -68,6 +73,7 @@ class ClockSampler:
             threading.Thread(target=self._pump, daemon=True).start()
         except OSError:
             self.proc = None
+        return self
 
     def _pump(self):
         for line in self.proc.stdout:
@@ -78,76 +84,101 @@ class ClockSampler:
             self.proc.terminate()
         sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
         mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        pw = [float(r[2]) for r in self.rows if len(r) >= 7 and r[2].replace(".", "").isdigit()]
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         reasons = sorted({names[i] for r in self.rows if len(r) >= 7 for i in range(4) if r[3 + i] == "Active"})
         busy = [x for x in sm if x > 0.6 * (max(mx) if mx else 1)] or sm
         return {"sm_mhz": float(np.median(busy)) if busy else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": reasons, "samples": len(sm)}
+                "reasons": reasons, "samples": len(sm), "power_w_max": max(pw) if pw else None}
 
 
 def make_workload(name: str, rank_seed: int = 0):
-    """Returns (host uint32 matrix, p, description).  rank_seed shifts the seed for replicas."""
+    """Returns (host uint32 matrix, p, config).  rank_seed shifts the seed for replicas."""
     c = dict(gen.CONFIGS[name])
     if c["kind"] == "uniform":
         a = gen.uniform_matrix(c["rows"], c["cols"], c["p"], c["seed"] + 1000 * rank_seed)  # == replicas.replica_seed
     elif c["kind"] == "lowrank":
         a, _, _ = gen.lowrank_factors(c["rows"], c["inner"], c["cols"], c["p"], c["seed_b"] + 1000 * rank_seed, c["seed_c"])
-    elif c["kind"] == "sparse_dep":
-        raise SystemExit("workload c5 is generated on the device: use --workload c5 (handled separately)")
     else:
-        raise SystemExit(f"workload {name} is not an F_p RREF config")
+        raise SystemExit(f"workload {name} has no host generator here")
     return a, c["p"], c
 
 
-def oracle_sample_gmulmod(n: int, p: int, threads: int):
-    """Times the CPU oracle (as it stands) on an n x n dense uniform matrix; returns (Gmulmod/s, seconds)."""
+# ------------------------------------------------------------------------------------------------ CPU oracle legs
+def oracle_time_fp(n: int, p: int, threads: int):
+    """Seconds the CPU oracle (as it stands) takes on an n x n dense uniform matrix over F_p."""
     import oracle
     a = gen.uniform_matrix(n, n, p, seed=4)
     t0 = time.perf_counter()
     _, rank, _ = oracle.rref_modp(a, p, nthreads=threads)
     dt = time.perf_counter() - t0
     assert rank == n
-    return (2 * n ** 3 / 3) / dt / 1e9, dt
+    return dt
 
 
-def f64_leg(torch, L, dev, n=16384, nrhs=64, reps=3):
-    """The metric's second half ("fp64 GFLOP/s"): linac_solve_f64 on config c4's shape and distribution
-    (A = G + 4 sqrt(N) I with G i.i.d. N(0,1), 64 N(0,1) right-hand sides), drawn on the device from a seeded torch
-    generator (the numpy recipe of linac_inputs takes half a minute on the host); the solve works in place, so every
-    repetition restores A and B by a device copy outside the timed region.  Backward error in the infinity norm on
-    the ORIGINAL data, computed with torch fp64 on the device."""
-    g = torch.Generator(device=dev)
-    g.manual_seed(5)
-    a0 = torch.randn((n, n), dtype=torch.float64, device=dev, generator=g)
-    a0.diagonal().add_(4.0 * n ** 0.5)
-    b0 = torch.randn((n, nrhs), dtype=torch.float64, device=dev, generator=g)
-    a, b = torch.empty_like(a0), torch.empty_like(b0)
-    stream = torch.cuda.current_stream(dev)
-    times = []
-    for i in range(reps + 1):
-        a.copy_(a0)
-        b.copy_(b0)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        L.solve_f64(a, b)
-        e1.record(stream)
-        e1.synchronize()
-        if i:
-            times.append(e0.elapsed_time(e1))
-    resid = (a0 @ b - b0).abs().amax(dim=0)
-    eta = float((resid / (a0.abs().sum(dim=1).max() * b.abs().amax(dim=0) + b0.abs().amax(dim=0))).max())
-    ms = float(np.mean(times))
-    flop = 2.0 * n ** 3 / 3.0 + 2.0 * n * n * nrhs
-    return {"workload": f"c4: {n}x{n} float64 N(0,1) + 4 sqrt(N) I, {nrhs} right-hand sides (torch generator, seed 5)",
-            "ms_per_solve": ms, "gflops": flop / ms / 1e6, "backward_error": eta, "backward_error_bound": 1e-11,
-            "roofline": {"bound": "tensor", "achieved": flop / ms / 1e9, "peak": 36.9, "unit": "TFLOP/s (fp64 DMMA)",
-                         "frac": flop / ms / 1e9 / 36.9,
-                         "note": "whole solve (panel chain and solves included) against the FP64 tensor pipe: 148 SMs x 64 "
-                                 "FMA/clk x 2 x 1.95 GHz, consistent with ncu (78 % sub-pipe utilisation at 28.8 TFLOP/s on "
-                                 "the largest update, profiles/r01_v13_dmma_top_ncu.md) and with cuBLAS DGEMM measured at "
-                                 "36.0 TFLOP/s on this pool"},
-            "note": "flop = 2N^3/3 + 2N^2 nrhs; trailing update on the FP64 tensor pipe (DMMA m8n8k4), substitution with "
-                    "inverted 128 x 128 diagonal blocks"}
+def oracle_time_f64(n: int, nrhs: int, threads: int):
+    import oracle
+    a, b = gen.shifted_normal_system(n, nrhs, seed_a=5, seed_b=6)
+    t0 = time.perf_counter()
+    rc, _, _ = oracle.solve_f64(a, b, nthreads=threads)
+    dt = time.perf_counter() - t0
+    assert rc == 0
+    return dt
+
+
+def cpu_baseline_plan(p: int, full: bool):
+    """SURVEY.md 8(d) "Oracle timed beside it", bounded to ~20-30 s of CPU work by default: the oracle single-threaded at
+    c1 and at a 1024^2 sample, the OpenMP build of the same loop on all host cores at c1 and at 1536^2 / 2048^2 samples,
+    cubic extrapolations (labelled) to c2, c3 and c5, and the fp64 oracle at 1024 / 2048 extrapolated to c4.  The
+    oracle's Gauss-Jordan loop executes N^3/2 multiply-subtracts on an N x N full-rank matrix; the rate below is in
+    the metric's unit (2N^3/3 per solve).  --cpu-baseline full runs c2 and c3 themselves (minutes)."""
+    import oracle
+    threads = oracle.max_threads()
+    gm = lambda n, t: (2 * n ** 3 / 3) / t / 1e9          # noqa: E731
+    out = {"cores": threads, "kind": "oracle", "unit": "Gmulmod/s"}
+    t_c1_1 = oracle_time_fp(512, p, 1)
+    t_c1_n = oracle_time_fp(512, p, threads)
+    t_1024_1 = oracle_time_fp(1024, p, 1)
+    t_1536_n = oracle_time_fp(1536, p, threads)
+    t_2048_n = oracle_time_fp(2048, p, threads)
+    out["measured"] = {
+        "c1_single_thread": {"n": 512, "threads": 1, "seconds": t_c1_1, "value": gm(512, t_c1_1)},
+        "c1_openmp": {"n": 512, "threads": threads, "seconds": t_c1_n, "value": gm(512, t_c1_n)},
+        "sample_1024_single_thread": {"n": 1024, "threads": 1, "seconds": t_1024_1, "value": gm(1024, t_1024_1)},
+        "sample_1536_openmp": {"n": 1536, "threads": threads, "seconds": t_1536_n, "value": gm(1536, t_1536_n)},
+        "sample_2048_openmp": {"n": 2048, "threads": threads, "seconds": t_2048_n, "value": gm(2048, t_2048_n)},
+    }
+    # cubic extrapolation t(N) = t(N0) (N/N0)^3 from the largest measured sample; c2's loop runs rows*cols*rank
+    # multiply-subtracts (4096*4096*3000), c5's about rows*cols*rank too (dense after fill-in)
+    k1, kn = t_1024_1 / 1024 ** 3, t_2048_n / 2048 ** 3
+    out["extrapolated"] = {
+        "c2_single_thread_s": k1 * 4096 * 4096 * 3000, "c2_openmp_s": kn * 4096 * 4096 * 3000,
+        "c3_single_thread_s": k1 * 1e12, "c3_openmp_s": kn * 1e12,
+        "c5_single_thread_s": k1 * 1e5 * 1e5 * 98000, "c5_openmp_s": kn * 1e5 * 1e5 * 98000,
+        "label": "EXTRAPOLATED: t = t(N0) * work / N0^3 with work = rows * cols * rank, N0 = 1024 (1 thread) / 2048 "
+                 f"({threads} threads); not measured"}
+    tf1, tf2 = oracle_time_f64(1024, 64, threads), oracle_time_f64(2048, 64, threads)
+    flop = lambda n: 2.0 * n ** 3 / 3.0 + 2.0 * n * n * 64          # noqa: E731
+    out["fp64"] = {"measured": {"n1024_openmp_s": tf1, "n2048_openmp_s": tf2, "n2048_gflops": flop(2048) / tf2 / 1e9},
+                   "extrapolated": {"c4_openmp_s": tf2 * (16384 / 2048) ** 3,
+                                    "label": "EXTRAPOLATED cubically from N = 2048 (the oracle is Gauss-Jordan on (A B): "
+                                             "about N^3 multiply-adds)"},
+                   "unit": "GFLOP/s in the metric's count (2N^3/3 + 2N^2 nrhs)"}
+    if full:
+        a2, p2, _ = make_workload("c2")
+        t0 = time.perf_counter(); oracle.rref_modp(a2, p2, nthreads=1); t_c2_1 = time.perf_counter() - t0
+        t0 = time.perf_counter(); oracle.rref_modp(a2, p2, nthreads=threads); t_c2_n = time.perf_counter() - t0
+        a3, p3, _ = make_workload("c3")
+        t0 = time.perf_counter(); oracle.rref_modp(a3, p3, nthreads=threads); t_c3_n = time.perf_counter() - t0
+        out["measured"].update({"c2_single_thread": {"seconds": t_c2_1, "threads": 1},
+                                "c2_openmp": {"seconds": t_c2_n, "threads": threads},
+                                "c3_openmp": {"seconds": t_c3_n, "threads": threads, "value": gm(10000, t_c3_n)}})
+    # the contract's top-level fields: the OpenMP sample closest to the headline workload
+    out["value"] = gm(2048, t_2048_n)
+    out["seconds"] = t_2048_n
+    out["sample"] = (f"2048x2048 dense uniform F_p (same recipe as c3), oracle Gauss-Jordan, {threads} OpenMP threads; "
+                     "see .measured / .extrapolated for the rest of the plan")
+    return out
 
 
 def run_reference(args):
@@ -158,24 +189,369 @@ def run_reference(args):
     import oracle
     threads = oracle.max_threads()
     n = args.ref_n
-    p = gen.CONFIGS[args.workload].get("p", 2147483647)
+    wl = "c3" if args.workload == "all" else args.workload
+    p = gen.CONFIGS[wl].get("p", 2147483647)
     for _ in range(args.warmup):
-        oracle_sample_gmulmod(min(n, 512), p, threads)
-    times = []
-    for _ in range(args.steps):
-        _, dt = oracle_sample_gmulmod(n, p, threads)
-        times.append(dt)
+        oracle_time_fp(min(n, 512), p, threads)
+    times = [oracle_time_fp(n, p, threads) for _ in range(args.steps)]
     t = float(np.mean(times))
     val = (2 * n ** 3 / 3) / t / 1e9
-    sample = f"{n}x{n} dense uniform F_p sample of workload {args.workload}, CPU oracle Gauss-Jordan"
+    sample = f"{n}x{n} dense uniform F_p sample of workload {wl}, CPU oracle Gauss-Jordan"
     print(json.dumps({
         "impl": "reference", "metric": "rref_gmulmod_per_s", "value": val, "unit": "Gmulmod/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
-        "config": {"workload": args.workload, "sample": sample},
+        "config": {"workload": wl, "sample": sample},
         "cpu_baseline": {"value": val, "unit": "Gmulmod/s", "cores": threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": "Gmulmod/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
+
+
+# ------------------------------------------------------------------------------------------------ GPU legs
+class Bench:
+    def __init__(self, torch, L, dev, local, world, rank, opts):
+        self.torch, self.L, self.dev, self.local, self.world, self.rank, self.opts = torch, L, dev, local, world, rank, opts
+        self.peaks_file = load_peaks()
+        self._peak_cache = {}
+
+    def barrier(self):
+        self.torch.cuda.synchronize(self.dev)
+        if self.world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+            self.torch.cuda.synchronize(self.dev)
+
+    def peak(self, what, ms):
+        key = (what, ms)
+        if key not in self._peak_cache:
+            self._peak_cache[key] = self.L.measure_peak(what, ms)
+        return self._peak_cache[key]
+
+    def tensor_peak(self, clocks):
+        """The int8 tensor peak for a run with these clocks: the 2 ms burst figure if the run sat near the maximum clock
+        with no power cap, else the 400 ms power-capped one (both measured live, random operand bytes)."""
+        burst, mhz_b = self.peak("tc_i8_n256", 2.0)
+        sust, mhz_s = self.peak("tc_i8_n256", 400.0)
+        capped = "sw_power_cap" in (clocks.get("reasons") or []) or (
+            clocks.get("sm_mhz") and clocks.get("sm_max_mhz") and clocks["sm_mhz"] < 0.93 * clocks["sm_max_mhz"])
+        use, mhz, kind = (sust, mhz_s, "sustained (400 ms)") if capped else (burst, mhz_b, "burst (2 ms)")
+        return {"peak": use, "peak_kind": kind, "peak_sm_mhz": mhz,
+                "peak_source": "measured live by linac_measure_peak('tc_i8_n256'): tcgen05.mma kind::i8 128x256x32 from "
+                               "on-chip pseudo-random operands",
+                "peak_burst": burst, "peak_burst_sm_mhz": mhz_b, "peak_sustained": sust, "peak_sustained_sm_mhz": mhz_s,
+                "peak_2x_bf16_for_comparison": {"burst": 2 * self.peaks_file["bf16_burst"],
+                                                "sustained": 2 * self.peaks_file["bf16_sustained"],
+                                                "source": self.peaks_file["source"] + " x nominal int8:bf16 ratio 2"}}
+
+    def fp_leg(self, name, steps, warmup, with_e2e=False, nullspace=False):
+        """One F_p config through linac_rref_u32 (or linac_nullspace_u32): device-resident timing, clocks, production-
+        schedule class split and the update roofline."""
+        torch, L, dev = self.torch, self.L, self.dev
+        from paper_2605_25863_b200 import replicas
+        cfg = dict(gen.CONFIGS[name])
+        on_device = cfg["kind"] == "sparse_dep"
+        if on_device:
+            from linac_inputs import gen_torch
+            cfg["seed"] += 1000 * self.rank
+            p, rows, cols = cfg["p"], cfg["rows"], cfg["cols"]
+            d_work = torch.empty((rows, cols), dtype=torch.int32, device=dev)
+            nbytes = rows * cols * 4
+            pinned = d_in = out_host = None
+            restore = lambda: gen_torch.fill_c5(d_work, cfg)            # noqa: E731  (NOT part of the step)
+        else:
+            a_host, p, cfg = make_workload(name, rank_seed=self.rank)
+            rows, cols = a_host.shape
+            nbytes = a_host.nbytes
+            pinned = torch.from_numpy(a_host.view(np.int32)).pin_memory()
+            d_in = pinned.to(dev, non_blocking=False)
+            d_work = torch.empty_like(d_in)
+            out_host = torch.empty_like(pinned).pin_memory() if with_e2e else None
+            restore = lambda: d_work.copy_(d_in)                        # noqa: E731  (NOT part of the step)
+        nominal = 2.0 * rows * cols * min(rows, cols) / 3.0
+        stream = torch.cuda.current_stream(dev)
+
+        def call(buf):
+            if nullspace:
+                rk, _, _ = L.nullspace_u32(buf, p)
+                return rk
+            return L.rref_u32(buf, p)[0]
+
+        def step_resident():
+            restore()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            rk = call(d_work)
+            e1.record(stream)
+            e1.synchronize()
+            return e0.elapsed_time(e1), rk
+
+        L.set_option("timing", 0)
+        for _ in range(warmup):
+            step_resident()
+        sampler = ClockSampler(self.local).start()
+        self.barrier()
+        times, ranks = [], []
+        for _ in range(steps):
+            ms, rk = step_resident()
+            times.append(ms)
+            ranks.append(rk)
+        self.barrier()
+        clocks = sampler.stop()
+        stats = L.last_stats()
+        total_ms = replicas.max_over_ranks(float(sum(times)), dev)
+        ms_per_step = total_ms / steps
+        value = replicas.aggregate_throughput(nominal, ms_per_step * 1e-3, self.world) / 1e9
+        leg = {"workload": f"{name}: {rows}x{cols} uint32 {WORKLOAD_KIND[cfg['kind']]}, p={p}" +
+                           (" + null space" if nullspace else ""),
+               "ms_per_step": ms_per_step, "ms_min": float(min(times)), "value": value, "unit": "Gmulmod/s", "steps": steps,
+               "warmup": warmup, "rank": int(ranks[-1]), "clocks": clocks, "gpu_launches_per_step": int(stats["kernel_launches"]),
+               "us_per_pivot": ms_per_step * 1e3 / max(1, int(ranks[-1])),
+               "l2": "input (%d MB) larger than L2" % (nbytes // 2 ** 20) if nbytes > 126 * 2 ** 20 else
+                     "input fits L2; restored by a device copy before each step, outside the timed region",
+               "stats": {k: stats[k] for k in ("kernel_launches", "host_syncs", "panels", "row_swaps", "update_macs")}}
+
+        # production-schedule class split (timing = 2: event pairs, no host syncs) and the update roofline
+        L.set_option("timing", 2)
+        step_resident()
+        ms_t, _ = step_resident()
+        st_t = L.last_stats()
+        L.set_option("timing", 0)
+        macs, ms_upd = st_t["update_macs"], st_t["ms_update"]
+        roof = {"bound": "tensor", "unit": "TOP/s (int8, 2 ops per u8 multiply-accumulate, 16 per field multiply-accumulate)",
+                "kernel": "Schur-update GEMMs on tcgen05 kind::i8 (gemm_tc_panel_kernel for K <= 256, gemm_tc_kernel above; "
+                          "the CUDA-core kernel only for shapes below 128)"}
+        roof.update(self.tensor_peak(clocks))
+        if st_t.get("tc_launches", 0) and ms_upd > 0:
+            ach = macs * 32.0 / (ms_upd * 1e-3) / 1e12
+            roof.update({"achieved": ach, "frac": ach / roof["peak"]})
+        else:
+            roof.update({"achieved": None, "frac": None})
+        whole = nominal / 2.0 * 32.0 / (ms_per_step * 1e-3) / 1e12          # 2N^3/3 counts multiply AND add: N^3/3 field MACs
+        roof["whole_step_achieved"] = whole
+        roof["whole_step_frac"] = whole / roof["peak"]
+        roof["update_share_of_step"] = ms_upd / st_t["ms_total"] if st_t["ms_total"] else None
+        roof["timed_split_ms"] = {"update": ms_upd, "strip": st_t.get("ms_strip"), "trsm": st_t.get("ms_trsm"),
+                                  "call_with_event_marks": ms_t, "schedule": "production (fused), event pairs, no host syncs"}
+        roof["note"] = ("achieved = executed update field-MACs x 32 / summed CUDA-event time of the update launches of the "
+                        "production schedule, on the call's stream; frac = achieved / peak; whole_step_* = (N^3/3 field MACs x "
+                        "32) / ms_per_step against the same peak")
+        tm_, tn_, tk_ = st_t.get("top_m", 0), st_t.get("top_n", 0), st_t.get("top_k", 0)
+        if st_t.get("ms_update_top", 0) > 0:
+            kp_ = -(-tk_ // 128) * 128
+            top = {"M": tm_, "N": tn_, "K": tk_, "ms": st_t["ms_update_top"],
+                   "achieved": 32.0 * tm_ * tn_ * tk_ / (st_t["ms_update_top"] * 1e-3) / 1e12,
+                   "algorithmic_bytes": 8 * tm_ * tn_ + 4 * kp_ * (tm_ + tn_),
+                   "algorithmic_bytes_note": "C read + C written (8 B per element) + both u8 limb-plane operands read once"}
+            top["frac"] = top["achieved"] / roof["peak"]
+            top["hbm_gbs_at_algorithmic_bytes"] = top["algorithmic_bytes"] / (top["ms"] * 1e-3) / 1e9
+            roof["top_launch"] = top
+        roof["traffic"] = None
+        if os.path.exists(TRAFFIC_FILE):
+            tr = json.load(open(TRAFFIC_FILE)).get(name)
+            if tr:
+                roof["traffic"] = tr["dram_bytes"]
+                roof["traffic_source"] = tr["source"]
+        leg["roofline"] = roof
+
+        if with_e2e and not on_device:
+            def step_e2e():
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                d_work.copy_(pinned, non_blocking=True)
+                rk = call(d_work)
+                out_host.copy_(d_work, non_blocking=True)
+                e1.record(stream)
+                e1.synchronize()
+                return e0.elapsed_time(e1), rk
+
+            def run_pipelined(k_steps):
+                """K end-to-end steps, double buffered: while the call of step k runs, the pinned H2D of step k+1 and the
+                D2H of step k-1 are in flight on their own streams; every step's copies are inside the timed region."""
+                s_c, s_in, s_out = torch.cuda.Stream(dev), torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+                bufs = [d_work, torch.empty_like(d_work)]
+                outs = [out_host, torch.empty_like(out_host).pin_memory()]
+                ev_in = [torch.cuda.Event(), torch.cuda.Event()]
+                ev_done = [torch.cuda.Event(), torch.cuda.Event()]
+                ev_out = [torch.cuda.Event(), torch.cuda.Event()]
+                t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize(dev)
+                t0.record(s_in)
+                with torch.cuda.stream(s_in):
+                    bufs[0].copy_(pinned, non_blocking=True)
+                    ev_in[0].record(s_in)
+                rk = None
+                for k in range(k_steps):
+                    b = k % 2
+                    if k + 1 < k_steps:
+                        nb = (k + 1) % 2
+                        if k >= 1:
+                            s_in.wait_event(ev_out[nb])
+                        with torch.cuda.stream(s_in):
+                            bufs[nb].copy_(pinned, non_blocking=True)
+                            ev_in[nb].record(s_in)
+                    s_c.wait_event(ev_in[b])
+                    with torch.cuda.stream(s_c):
+                        rk = call(bufs[b])
+                        ev_done[b].record(s_c)
+                    s_out.wait_event(ev_done[b])
+                    with torch.cuda.stream(s_out):
+                        outs[b].copy_(bufs[b], non_blocking=True)
+                        ev_out[b].record(s_out)
+                t1.record(s_out)
+                t1.synchronize()
+                torch.cuda.synchronize(dev)
+                return t0.elapsed_time(t1) / k_steps, rk
+
+            step_e2e()
+            self.barrier()
+            serial = [step_e2e()[0] for _ in range(max(2, min(steps, 3)))]
+            self.barrier()
+            serial_ms = replicas.max_over_ranks(float(np.mean(serial)), dev)
+            run_pipelined(2)
+            self.barrier()
+            e2e_ms, rk_p = run_pipelined(max(12, steps))
+            assert rk_p == ranks[-1]
+            self.barrier()
+            e2e_ms = replicas.max_over_ranks(float(e2e_ms), dev)
+            leg["e2e"] = {"value": replicas.aggregate_throughput(nominal, e2e_ms * 1e-3, self.world) / 1e9, "unit": "Gmulmod/s",
+                          "ms_per_step": e2e_ms, "h2d_bytes_per_step": int(nbytes), "d2h_bytes_per_step": int(nbytes),
+                          "mode": "double-buffered: the pinned H2D of step k+1 and the D2H of step k-1 overlap the call of "
+                                  "step k; every step's copies are inside the timed region",
+                          "serial_ms_per_step": serial_ms,
+                          "serial_value": replicas.aggregate_throughput(nominal, serial_ms * 1e-3, self.world) / 1e9}
+        else:
+            leg["e2e"] = {"value": None, "unit": "Gmulmod/s", "ms_per_step": None, "h2d_bytes_per_step": 0,
+                          "d2h_bytes_per_step": 0,
+                          "note": "not measured: generated on the device (40 GB)" if on_device else "not measured for this leg"}
+        del d_work
+        torch.cuda.empty_cache()
+        return leg
+
+    def f64_solve_leg(self, n=16384, nrhs=64, reps=3):
+        """Config c4 through linac_solve_f64: A = G + 4 sqrt(N) I, G i.i.d. N(0,1), 64 N(0,1) right-hand sides, drawn on the
+        device from a seeded torch generator (same distribution as linac_inputs' c4 recipe, whose numpy generator takes
+        half a minute on the host).  Backward error in the infinity norm on the ORIGINAL data with torch fp64 products
+        (cuBLAS; a bench-side check only -- the parity tests use the oracle's long-double residual)."""
+        torch, L, dev = self.torch, self.L, self.dev
+        g = torch.Generator(device=dev)
+        g.manual_seed(5)
+        a0 = torch.randn((n, n), dtype=torch.float64, device=dev, generator=g)
+        a0.diagonal().add_(4.0 * n ** 0.5)
+        b0 = torch.randn((n, nrhs), dtype=torch.float64, device=dev, generator=g)
+        a, b = torch.empty_like(a0), torch.empty_like(b0)
+        stream = torch.cuda.current_stream(dev)
+        times = []
+        sampler = None
+        for i in range(reps + 1):
+            a.copy_(a0)
+            b.copy_(b0)
+            if i == 1:
+                sampler = ClockSampler(self.local).start()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            L.solve_f64(a, b)
+            e1.record(stream)
+            e1.synchronize()
+            if i:
+                times.append(e0.elapsed_time(e1))
+        clocks = sampler.stop()
+        launches = L.last_stats()["kernel_launches"]
+        resid = (a0 @ b - b0).abs().amax(dim=0)
+        eta = float((resid / (a0.abs().sum(dim=1).max() * b.abs().amax(dim=0) + b0.abs().amax(dim=0))).max())
+        ms = float(np.mean(times))
+        flop = 2.0 * n ** 3 / 3.0 + 2.0 * n * n * nrhs
+        peak, mhz = self.peak("dmma", 20.0)
+        del a0, b0, a, b
+        torch.cuda.empty_cache()
+        return {"workload": f"c4: {n}x{n} float64 N(0,1) + 4 sqrt(N) I, {nrhs} right-hand sides (torch generator on the device, "
+                            "seed 5; eta checked with torch fp64 products)",
+                "ms_per_solve": ms, "gflops": flop / ms / 1e6, "backward_error": eta, "backward_error_bound": 1e-11,
+                "clocks": clocks, "gpu_launches_per_solve": int(launches),
+                "roofline": {"bound": "tensor", "achieved": flop / ms / 1e9, "peak": peak, "unit": "TFLOP/s (fp64 DMMA)",
+                             "frac": flop / ms / 1e9 / peak, "peak_sm_mhz": mhz,
+                             "peak_source": "measured live by linac_measure_peak('dmma'): mma.sync m8n8k4 f64 from registers",
+                             "note": "whole solve (panel chain, exchanges and substitutions included) against the FP64 tensor pipe"},
+                "note": "flop = 2N^3/3 + 2N^2 nrhs"}
+
+    def rref_f64_leg(self, rows=8192, cols=8192, r=6144, reps=2):
+        """SURVEY.md 8(f)#3: linac_rref_f64 on a rank-deficient product (rows x r).(r x cols) of N(0,1) factors with rows
+        rescaled over several decades; flop count of the blocked Gauss-Jordan that runs: 2 rows cols rank / ... stated."""
+        torch, L, dev = self.torch, self.L, self.dev
+        g = torch.Generator(device=dev)
+        g.manual_seed(9)
+        a0 = torch.randn((rows, r), dtype=torch.float64, device=dev, generator=g) @ \
+            torch.randn((r, cols), dtype=torch.float64, device=dev, generator=g)
+        a0 *= 10.0 ** (2.0 * torch.randn((rows, 1), dtype=torch.float64, device=dev, generator=g))
+        a = torch.empty_like(a0)
+        stream = torch.cuda.current_stream(dev)
+        times, rk = [], None
+        for i in range(reps + 1):
+            a.copy_(a0)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            rk, piv = L.rref_f64(a, 1e-9)
+            e1.record(stream)
+            e1.synchronize()
+            if i:
+                times.append(e0.elapsed_time(e1))
+        launches = L.last_stats()["kernel_launches"]
+        pv = piv.to(dev).long()
+        recon = a0[:, pv] @ a[:rk]
+        err = float(((recon - a0).abs().amax(dim=1) / a0.abs().amax(dim=1)).max())
+        ms = float(np.mean(times))
+        # executed: every panel updates all rows on the columns from the panel on: sum_j 2 rows (cols - j) 32 ~ rows cols^2
+        flop = float(sum(2.0 * rows * (cols - j0) * 32 for j0 in range(0, cols, 32) if j0 < rk + 32))
+        peak, mhz = self.peak("dmma", 20.0)
+        del a0, a
+        torch.cuda.empty_cache()
+        return {"workload": f"rref_f64: {rows}x{cols} float64, rank {r} product of N(0,1) factors, rows rescaled by 10^(2 N(0,1)), "
+                            "tol 1e-9", "ms_per_call": ms, "rank": int(rk), "gflops_executed": flop / ms / 1e6,
+                "row_space_residual": err, "gpu_launches_per_call": int(launches),
+                "roofline": {"bound": "tensor", "achieved": flop / ms / 1e9, "peak": peak, "unit": "TFLOP/s (fp64 DMMA)",
+                             "frac": flop / ms / 1e9 / peak, "peak_sm_mhz": mhz,
+                             "note": "executed flops of the K = 32 DMMA updates (2 rows (cols - j0) 32 per panel) / whole call"}}
+
+    def wide_leg(self, which, n=4096, reps=2):
+        """SURVEY.md 8(f)#4: dense uniform n x n over F_p with p = 2^32 - 5 (uint32 storage) or 2^61 - 1 (uint64)."""
+        torch, L, dev = self.torch, self.L, self.dev
+        if which == "u32":
+            p = 4294967291
+            a0 = torch.from_numpy(gen.uniform_matrix(n, n, p, seed=4).view(np.int32)).to(dev)
+            fn = L.rref_u32
+        else:
+            p = (1 << 61) - 1
+            a0 = torch.from_numpy(gen.uniform_matrix_u64(n, n, p, seed=4).view(np.int64)).to(dev)
+            fn = L.rref_u64
+        a = torch.empty_like(a0)
+        stream = torch.cuda.current_stream(dev)
+        times, rk = [], None
+        for i in range(reps + 1):
+            a.copy_(a0)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            rk, _ = fn(a, p)
+            e1.record(stream)
+            e1.synchronize()
+            if i:
+                times.append(e0.elapsed_time(e1))
+        st = L.last_stats()
+        ms = float(np.mean(times))
+        imad, mhz = self.peak("imad_wide", 20.0)
+        macs = float(st["update_macs"])
+        # instruction budget per field multiply-accumulate of the Montgomery update (cuobjdump of wide_update_kernel):
+        # u32: 2 IMAD.WIDE + 1 IMAD + ~5 ALU; u64: 4 x (mul.lo + mul.hi pairs = ~16 IMAD) + carries
+        per_mac = 3.0 if which == "u32" else 16.0
+        del a0, a
+        torch.cuda.empty_cache()
+        return {"workload": f"wide_{which}: {n}x{n} dense uniform, p={p}", "ms_per_call": ms, "rank": int(rk),
+                "value": (2.0 * n ** 3 / 3.0) / (ms * 1e-3) / 1e9, "unit": "Gmulmod/s (2N^3/3)",
+                "executed_tmacs_per_s": macs / (ms * 1e-3) / 1e12, "gpu_launches_per_call": int(st["kernel_launches"]),
+                "roofline": {"bound": "alu", "achieved": macs * per_mac / (ms * 1e-3) / 1e12, "peak": imad,
+                             "unit": "T integer multiply-add instructions/s (thread level)", "peak_sm_mhz": mhz,
+                             "frac": macs * per_mac / (ms * 1e-3) / 1e12 / imad,
+                             "peak_source": "measured live by linac_measure_peak('imad_wide')",
+                             "note": f"achieved = executed field MACs (rows x cols-from-panel x 32 per panel, Gauss-Jordan over all "
+                                     f"rows) x {per_mac:g} IMAD-class instructions per Montgomery multiply-accumulate / whole call"}}
 
 
 def main():
@@ -184,12 +560,18 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c5"])
-    ap.add_argument("--ref-n", type=int, default=1280, help="sample size for the oracle legs")
+    ap.add_argument("--workload", default="all", choices=["all", "c1", "c2", "c3", "c5"],
+                    help="all (default): headline c3 + one leg per other config; or a single F_p config as the headline")
+    ap.add_argument("--legs", default="c1,c2,c5,fp64_solve,rref_f64,wide_u32,wide_u64",
+                    help="comma list of the extra legs of the default run")
+    ap.add_argument("--ref-n", type=int, default=1280, help="sample size for --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-f64", action="store_true", help="skip the fp64 leg (config c4) of the default run")
-    ap.add_argument("--fp64-only", action="store_true",
-                    help="run only the fp64 leg (config c4) and print {\"fp64\": ...}; the command of the fp64 launch list")
+    ap.add_argument("--cpu-baseline", default="bounded", choices=["bounded", "full"])
+    ap.add_argument("--no-f64", action="store_true", help="skip the fp64 legs")
+    ap.add_argument("--fp64-only", action="store_true", help="run only legs.fp64_solve and print {\"fp64\": ...}")
+    ap.add_argument("--gemm", default=None, metavar="M,N,K[,path]",
+                    help="time the S5 primitive linac_gemm_sub_u32 alone (C -= A.B mod 2^31-1, path 2 = tensor cores by default) "
+                         "and print {\"gemm\": ...}; the command of the GEMM ncu captures under profiles/")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
                     help="library tunable for A/B runs (linac_set_option), e.g. --opt strip_width=256")
     args = ap.parse_args()
@@ -209,218 +591,85 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
+    for kv in args.opt:
+        name, _, val = kv.partition("=")
+        L.set_option(name, int(val))
+    B = Bench(torch, L, dev, local, world, rank, args.opt)
+    if args.gemm:
+        parts = [int(x) for x in args.gemm.split(",")]
+        m, n, k = parts[:3]
+        path = parts[3] if len(parts) > 3 else 2
+        p = 2147483647
+        from linac_inputs import gen_torch
+        a = gen_torch.uniform_rows(0, m, k, p, 1, dev)
+        b = gen_torch.uniform_rows(0, k, n, p, 2, dev)
+        c = gen_torch.uniform_rows(0, m, n, p, 3, dev)
+        times = []
+        for i in range(args.warmup + min(args.steps, 5)):
+            L.gemm_sub_u32(c, a, b, p, path)
+            if i >= args.warmup:
+                times.append(L.last_stats()["ms_total"])
+        ms = float(np.mean(times))
+        clk = {"sm_mhz": None, "reasons": []}
+        peak = B.tensor_peak(clk)
+        ach = 32.0 * m * n * k / (ms * 1e-3) / 1e12
+        print(json.dumps({"gemm": {"M": m, "N": n, "K": k, "path": path, "ms": ms, "achieved_tops": ach,
+                                   "field_tmacs_per_s": ach / 32.0, "frac_of_burst_peak": ach / peak["peak_burst"],
+                                   "peak_burst": peak["peak_burst"], "peak_sustained": peak["peak_sustained"],
+                                   "note": "event time of the whole call incl. the limb-split pre-passes"}}))
+        return
     if args.fp64_only:
-        for kv in args.opt:
-            name, _, val = kv.partition("=")
-            L.set_option(name, int(val))
         if rank == 0:
-            print(json.dumps({"fp64": f64_leg(torch, L, dev, reps=max(1, min(args.steps, 5)))}))
+            print(json.dumps({"fp64": B.f64_solve_leg(reps=max(1, min(args.steps, 5)))}))
         return
 
-    from paper_2605_25863_b200 import replicas
-    on_device = gen.CONFIGS[args.workload]["kind"] == "sparse_dep"     # c5: 40 GB, generated straight into HBM
-    if on_device:
-        from linac_inputs import gen_torch
-        cfg = dict(gen.CONFIGS[args.workload])
-        cfg["seed"] += 1000 * rank
-        p, rows, cols = cfg["p"], cfg["rows"], cfg["cols"]
-        a_host = pinned = out_host = d_in = None
-        d_work = torch.empty((rows, cols), dtype=torch.int32, device=dev)
-        nbytes = rows * cols * 4
+    headline = "c3" if args.workload == "all" else args.workload
+    if headline == "c5":
+        h = B.fp_leg("c5", steps=min(args.steps, 2), warmup=min(args.warmup, 1))
+        args.steps, args.warmup = h["steps"], h["warmup"]
     else:
-        a_host, p, cfg = make_workload(args.workload, rank_seed=rank)      # replicas: one matrix per rank
-        rows, cols = a_host.shape
-        nbytes = a_host.nbytes
-        pinned = torch.from_numpy(a_host.view(np.int32)).pin_memory()
-        d_in = pinned.to(dev, non_blocking=False)
-        d_work = torch.empty_like(d_in)
-        out_host = torch.empty_like(pinned).pin_memory()
-    n_nominal = 2.0 * rows * cols * min(rows, cols) / 3.0              # 2N^3/3 for square N
-    stream = torch.cuda.current_stream(dev)
-
-    def barrier():
-        torch.cuda.synchronize(dev)
-        if world > 1:
-            dist.barrier()
-            torch.cuda.synchronize(dev)
-
-    def step_resident():
-        if on_device:
-            gen_torch.fill_c5(d_work, cfg)        # regenerate the input: NOT part of the step
-        else:
-            d_work.copy_(d_in)                    # restore the input: NOT part of the step
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        rank_, _ = L.rref_u32(d_work, p)
-        e1.record(stream)
-        e1.synchronize()
-        return e0.elapsed_time(e1), rank_
-
-    def step_e2e():
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        d_work.copy_(pinned, non_blocking=True)   # H2D of this step's input
-        rank_, piv = L.rref_u32(d_work, p)
-        out_host.copy_(d_work, non_blocking=True)  # D2H of the RREF
-        e1.record(stream)
-        e1.synchronize()
-        return e0.elapsed_time(e1), rank_
-
-    def run_e2e_pipelined(k_steps):
-        """K end-to-end steps, double buffered: while the call of step k runs, the pinned H2D of step k+1 and the
-        D2H of step k-1 are in flight on their own streams.  Every step still copies its input from pinned host
-        memory and reads its RREF back; all of it inside the timed region (events across the three streams)."""
-        s_c, s_in, s_out = torch.cuda.Stream(dev), torch.cuda.Stream(dev), torch.cuda.Stream(dev)
-        bufs = [d_work, torch.empty_like(d_work)]
-        outs = [out_host, torch.empty_like(out_host).pin_memory()]
-        ev_in = [torch.cuda.Event(), torch.cuda.Event()]
-        ev_done = [torch.cuda.Event(), torch.cuda.Event()]
-        ev_out = [torch.cuda.Event(), torch.cuda.Event()]
-        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize(dev)
-        t0.record(s_in)
-        with torch.cuda.stream(s_in):
-            bufs[0].copy_(pinned, non_blocking=True)
-            ev_in[0].record(s_in)
-        rk = None
-        for k in range(k_steps):
-            b = k % 2
-            if k + 1 < k_steps:
-                nb = (k + 1) % 2
-                if k >= 1:
-                    s_in.wait_event(ev_out[nb])          # buffer nb is free once step k-1's result has left it
-                with torch.cuda.stream(s_in):
-                    bufs[nb].copy_(pinned, non_blocking=True)
-                    ev_in[nb].record(s_in)
-            s_c.wait_event(ev_in[b])
-            with torch.cuda.stream(s_c):
-                rk, _ = L.rref_u32(bufs[b], p)           # returns when the RREF is complete on s_c
-                ev_done[b].record(s_c)
-            s_out.wait_event(ev_done[b])
-            with torch.cuda.stream(s_out):
-                outs[b].copy_(bufs[b], non_blocking=True)
-                ev_out[b].record(s_out)
-        t1.record(s_out)
-        t1.synchronize()
-        torch.cuda.synchronize(dev)
-        return t0.elapsed_time(t1) / k_steps, rk
-
-    L.set_option("timing", 0)
-    for kv in args.opt:
-        name, val = kv.split("=")
-        L.set_option(name, int(val))
-    for _ in range(args.warmup):
-        step_resident()
-    sampler = ClockSampler(local)
-    barrier()
-    sampler.start()
-    times, ranks = [], []
-    for _ in range(args.steps):
-        ms, rk = step_resident()
-        times.append(ms)
-        ranks.append(rk)
-    barrier()
-    clocks = sampler.stop()
-    stats = L.last_stats()
-    total_ms = float(sum(times))
-    total_ms = replicas.max_over_ranks(total_ms, dev)
-    ms_per_step = total_ms / args.steps
-    value = replicas.aggregate_throughput(n_nominal, ms_per_step * 1e-3, world) / 1e9
-
-    # end-to-end leg (host buffers; not run for the device-generated 40 GB config)
-    e2e_ms = e2e_value = None
-    if not on_device:
-        step_e2e()
-        barrier()
-        e2e_times = [step_e2e()[0] for _ in range(max(2, min(args.steps, 3)))]
-        barrier()
-        e2e_serial_ms = replicas.max_over_ranks(float(np.mean(e2e_times)), dev)
-        run_e2e_pipelined(2)
-        barrier()
-        e2e_ms, rk_p = run_e2e_pipelined(max(12, args.steps))
-        assert rk_p == ranks[-1]
-        barrier()
-        e2e_ms = replicas.max_over_ranks(float(e2e_ms), dev)
-        e2e_value = replicas.aggregate_throughput(n_nominal, e2e_ms * 1e-3, world) / 1e9
-
-    # roofline of the dominant kernel family (Schur update), event-timed launch by launch
-    L.set_option("timing", 1)
-    step_resident()
-    step_resident()
-    st_t = L.last_stats()
-    L.set_option("timing", 0)
-    peaks = load_peaks()
-    macs, ms_upd = st_t["update_macs"], st_t["ms_update"]
-    path = st_t.get("gemm_path_used", None)
-    achieved_tmacs = macs / (ms_upd * 1e-3) / 1e12 if ms_upd > 0 else None
-    tensor_used = bool(st_t.get("tc_launches", 0))
-    if tensor_used:
-        # 16 u8xu8 MACs per field MAC on the int8 tensor pipe; int8 dense peak = 2 x measured bf16 (nominal ratio)
-        peak = peaks["bf16_sustained"] * 2.0
-        ach = achieved_tmacs * 16 * 2 if achieved_tmacs else None
-        roof = {"bound": "tensor", "achieved": ach, "peak": peak, "unit": "TOP/s (int8, 2 ops per MAC)",
-                "frac": ach / peak if ach else None, "traffic": None,
-                "kernel": "Schur-update GEMMs on tcgen05 kind::i8 (gemm_tc_panel_kernel for K <= 256, gemm_tc_kernel above), "
-                          "limb-split pre-passes included in the time",
-                "note": f"achieved = executed update field-MACs x 16 u8 MACs x 2 ops / summed CUDA-event time of those "
-                        f"launches on the call's stream; peak = 2 x {peaks['source']} sustained bf16 (guide's nominal "
-                        f"int8:bf16 ratio); traffic: see profiles/ (ncu --set full capture of the top launch)"}
-    else:
-        # CUDA-core path: one IMAD.WIDE.U32 per field MAC; nominal issue peak 148 SM x 64 lanes x f_max
-        peak = 148 * 64 * peaks["sm_max_mhz"] * 1e6 / 1e12
-        roof = {"bound": "alu", "achieved": achieved_tmacs, "peak": peak, "unit": "T field-MAC/s",
-                "frac": achieved_tmacs / peak if achieved_tmacs else None, "traffic": None,
-                "note": "peak = 148 SM x 64 IMAD lanes x max SM clock (DESIGN.md); "
-                        "achieved = executed update MACs / summed event time of the update kernels"}
-    # the largest single launch, per launch: algorithmic bytes (C read + C written + both limb-plane sets read) and,
-    # for the default workload, the DRAM traffic ncu measured for the same launch (profiles/r01_v9_launches_c3.md)
-    tm_, tn_, tk_ = st_t.get("top_m", 0), st_t.get("top_n", 0), st_t.get("top_k", 0)
-    if tensor_used and st_t.get("ms_update_top", 0) > 0:
-        kp_ = -(-tk_ // 128) * 128
-        roof["top_launch"] = {
-            "M": tm_, "N": tn_, "K": tk_, "ms": st_t["ms_update_top"],
-            "achieved": 32.0 * tm_ * tn_ * tk_ / (st_t["ms_update_top"] * 1e-3) / 1e12,
-            "algorithmic_bytes": 8 * tm_ * tn_ + 4 * kp_ * (tm_ + tn_),
-            "note": "event-timed, limb split included"}
-        if args.workload == "c3" and not args.opt:
-            roof["traffic"] = NCU_TOP_LAUNCH_DRAM_BYTES_C3
-            roof["top_launch"]["traffic_note"] = ("roofline.traffic = dram__bytes_read.sum + dram__bytes_write.sum of the "
-                                                  "M = N = 9744, K = 128 launch in the ncu --set full capture")
-    roof["update_share_of_step"] = ms_upd / st_t["ms_total"] if st_t["ms_total"] else None
-    roof["timed_split_ms"] = {"update": ms_upd, "strip": st_t.get("ms_strip"), "trsm": st_t.get("ms_trsm"),
-                              "total_with_timing_syncs": st_t["ms_total"]}
-
+        h = B.fp_leg(headline, steps=args.steps, warmup=args.warmup, with_e2e=True, nullspace=(headline == "c2"))
     out = {
-        "metric": "rref_gmulmod_per_s", "value": value, "unit": "Gmulmod/s", "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": (value / world / PAPER_A100_GMULMOD[args.workload]) if args.workload in PAPER_A100_GMULMOD else None,
-        "dtype": "u32", "data": "synthetic",
-        "config": {"workload": f"{args.workload}: {rows}x{cols} uint32 {WORKLOAD_KIND[cfg['kind']]}, p={p}", "rank": int(ranks[-1]),
-                   "parallelism": "replicas" if world > 1 else "single", "l2": "input (%d MB) larger than L2" %
-                   (nbytes // 2 ** 20) if nbytes > 126 * 2 ** 20 else "input fits L2; restored by a device copy each step",
-                   "options": args.opt},
-        "e2e": {"value": e2e_value, "unit": "Gmulmod/s", "ms_per_step": e2e_ms,
-                "h2d_bytes_per_step": 0 if on_device else int(nbytes), "d2h_bytes_per_step": 0 if on_device else int(nbytes),
-                **({"note": "not measured: this config is generated on the device (40 GB)"} if on_device else
-                   {"mode": "double-buffered: the pinned H2D of step k+1 and the D2H of step k-1 overlap the call of step k; "
-                            "every step's copies are inside the timed region",
-                    "serial_ms_per_step": e2e_serial_ms,
-                    "serial_value": replicas.aggregate_throughput(n_nominal, e2e_serial_ms * 1e-3, world) / 1e9})},
-        "gpu_launches": int(stats["kernel_launches"]) * args.steps,
-        "clocks": clocks, "roofline": roof,
-        "stats": {k: stats[k] for k in ("kernel_launches", "host_syncs", "panels", "row_swaps", "update_macs")},
-        "baseline_context": "paper, A100: 3.6 s at N=1e4 (PAPER.md:59) = 185 Gmulmod/s, 45 min at N=1e5 (PAPER.md:61) = 247 "
-                            "Gmulmod/s; another machine, context only",
+        "metric": "rref_gmulmod_per_s", "value": h["value"], "unit": "Gmulmod/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": h["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": {"workload": h["workload"], "rank": h["rank"], "parallelism": "replicas" if world > 1 else "single",
+                   "l2": h["l2"], "options": args.opt},
+        "e2e": h["e2e"], "gpu_launches": h["gpu_launches_per_step"] * args.steps, "clocks": h["clocks"],
+        "roofline": h["roofline"], "stats": h["stats"], "us_per_pivot": h["us_per_pivot"],
+        "baseline_context": BASELINE_CONTEXT,
     }
-    if rank == 0 and world == 1 and args.workload == "c3" and not args.no_f64:
-        out["fp64"] = f64_leg(torch, L, dev)
+    if rank == 0 and world == 1 and args.workload == "all":
+        legs = {}
+        want = [x for x in args.legs.split(",") if x]
+        for name in want:
+            try:
+                if name == "c1":
+                    legs[name] = B.fp_leg("c1", steps=20, warmup=3, with_e2e=True)
+                elif name == "c2":
+                    legs[name] = B.fp_leg("c2", steps=10, warmup=3, with_e2e=True, nullspace=True)
+                elif name == "c5":
+                    free_b, _ = torch.cuda.mem_get_info()
+                    if free_b < 60e9:
+                        legs[name] = {"skipped": "needs about 60 GB of free device memory"}
+                    else:
+                        legs[name] = B.fp_leg("c5", steps=2, warmup=1)
+                elif name == "fp64_solve" and not args.no_f64:
+                    legs[name] = B.f64_solve_leg()
+                elif name == "rref_f64" and not args.no_f64:
+                    legs[name] = B.rref_f64_leg()
+                elif name == "wide_u32":
+                    legs[name] = B.wide_leg("u32")
+                elif name == "wide_u64":
+                    legs[name] = B.wide_leg("u64")
+            except Exception as e:                       # a failed leg must not lose the headline line
+                legs[name] = {"error": f"{type(e).__name__}: {e}"}
+        out["legs"] = legs
+        if "fp64_solve" in legs:
+            out["fp64"] = legs["fp64_solve"]
+        out["measured_peaks_live"] = {f"{k[0]}@{k[1]:g}ms": {"value": v[0], "sm_mhz": v[1]} for k, v in B._peak_cache.items()}
     if rank == 0 and not args.no_cpu_baseline:
-        import oracle
-        threads = oracle.max_threads()
-        v, dt = oracle_sample_gmulmod(args.ref_n, p, threads)
-        out["cpu_baseline"] = {"value": v, "unit": "Gmulmod/s", "cores": threads, "kind": "oracle", "seconds": dt,
-                               "sample": f"{args.ref_n}x{args.ref_n} dense uniform F_p (same recipe as the workload), "
-                                         f"oracle Gauss-Jordan, {threads} OpenMP threads"}
+        out["cpu_baseline"] = cpu_baseline_plan(gen.CONFIGS[headline]["p"], full=(args.cpu_baseline == "full"))
     if rank == 0:
         print(json.dumps(out))
     if world > 1:

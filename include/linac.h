@@ -22,9 +22,16 @@
  *     cols..ld-1 are never read as data and never written (the paper pads rows the same way,
  *     PAPER.md:227).
  *   - Workspace: if linac_set_workspace() gave the library a buffer at least as large as the
- *     *_workspace() query, it is used; otherwise the library allocates (and caches) its own with
- *     cudaMalloc and linac_release() frees it.  One call at a time per process (the workspace
- *     and the internal state are global); calls are serialised by an internal mutex.
+ *     *_workspace() query, it is used and the call allocates NO device memory; otherwise the library
+ *     allocates (and caches) its own with cudaMalloc and linac_release() frees it.
+ *   - Re-entrancy: everything a call mutates -- the workspace binding, the statistics, the error text, the
+ *     host mailbox the strip kernels write to, the constant-memory slot that holds the field -- belongs to
+ *     the calling HOST THREAD.  Calls issued from different host threads on different streams (each thread
+ *     with its own workspace) run independently, with different matrices and different moduli; calls from
+ *     one thread are sequential by construction (every call synchronises its stream before returning).
+ *     linac_set_workspace / linac_release / linac_get_last_stats / linac_last_cuda_error act on the calling
+ *     thread's state.  linac_set_option is process-wide: set options while no call is in flight.  At most
+ *     64 host threads may be inside the library at once (LINAC_ERR_INTERNAL beyond that).
  */
 #ifndef LINAC_H_
 #define LINAC_H_
@@ -241,6 +248,22 @@ int linac_get_last_stats(linac_stats *out);
  * "f64_rhs_inv" (fp64 substitution on the right-hand sides: 1 = blocked, with inverted 128 x 128 diagonal blocks, 0 = recursive leaf solves)}.
  * Returns LINAC_ERR_INVALID_ARG for unknown names / out-of-range values. */
 int linac_set_option(const char *name, int64_t value);
+
+/* ---- measured peaks of the pipes the rooflines are quoted against ("Measure, do not assume") ---- */
+/*
+ * linac_measure_peak -- runs a microbenchmark that issues nothing but one instruction class from on-chip operands:
+ *   "tc_i8_n256", "tc_i8_n128"  tcgen05.mma.cta_group::1.kind::i8, M = 128, N = 256 / 128, K = 32 -> *value in TOP/s
+ *                               (2 ops per u8 multiply-accumulate)
+ *   "dmma"                      mma.sync.m8n8k4.f64 (DMMA.8x8x4)                                  -> TFLOP/s
+ *   "imad_wide"                 mad.wide.u32 with 64-bit accumulate (IMAD.WIDE.U32)               -> T instructions/s (thread-level)
+ *   "hbm_copy", "hbm_read"      16-byte grid-stride copy / read over `scratch` (DEVICE, >= 32 MiB; use >= 1 GiB) -> GB/s
+ *                               (copy counts read + written bytes)
+ * ms_target: approximate duration of the timed launch (<= 0: 2 ms; a few hundred ms shows the power-capped rate).
+ * sm_mhz (HOST out, may be NULL): the SM clock the timed launch actually ran at (%clock64 against %globaltimer).
+ * Synchronises `stream`.  scratch may be NULL for the compute kinds.
+ */
+int linac_measure_peak(const char *what, double ms_target, void *scratch, size_t scratch_bytes, void *stream,
+                       double *value, double *sm_mhz);
 
 #ifdef __cplusplus
 }

@@ -22,9 +22,6 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std
          "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "--expt-relaxed-constexpr"]
 
 
-if os.environ.get("LINAC_TRACE"):      # debug build: phase stamps in the strip kernel (fp_strip.cuh)
-    FLAGS.append("-DLINAC_TRACE")
-
 
 def _sources():
     return sorted(glob.glob(os.path.join(CSRC, "*.cu")))

@@ -23,7 +23,6 @@
 namespace cg = cooperative_groups;
 
 namespace linac {
-extern std::mutex g_call_mutex;
 namespace {
 
 constexpr int FW = 32;              // panel width
@@ -1069,7 +1068,6 @@ int linac_solve_f64_workspace(int64_t n, int64_t nrhs, size_t* bytes) {
 
 int linac_solve_f64(double* dA, int64_t n, int64_t lda, double* dB, int64_t nrhs, int64_t ldb, double tol, void* stream,
                     int64_t* info_out) {
-    std::lock_guard<std::mutex> lock(g_call_mutex);
     linac_stats& st = stats();
     st = linac_stats{};
     if (n < 0 || nrhs < 0 || !info_out) return LINAC_ERR_INVALID_ARG;
@@ -1137,9 +1135,10 @@ int linac_solve_f64(double* dA, int64_t n, int64_t lda, double* dB, int64_t nrhs
     LINAC_CUDA(cudaMemsetAsync(c.cand, 0, 2 * 1024 * sizeof(Cand), s));        // tags of an earlier solve must not match
     LINAC_CUDA(cudaMemsetAsync(c.target, 0, 2 * FW * sizeof(double2), s));
 
-    cudaEvent_t e0, e1;
-    LINAC_CUDA(cudaEventCreate(&e0));
-    LINAC_CUDA(cudaEventCreate(&e1));
+    CallEvents evs;
+    rc = evs.create();
+    if (rc) return rc;
+    cudaEvent_t e0 = evs.ev0, e1 = evs.ev1;
     cudaEventRecord(e0, s);
     row_scale_kernel<<<(unsigned)n, 256, 0, s>>>(dA, n, lda, dB, nrhs, ldb, c.info);          // F1
     LINAC_CUDA(cudaGetLastError());
@@ -1164,8 +1163,6 @@ int linac_solve_f64(double* dA, int64_t n, int64_t lda, double* dB, int64_t nrhs
     float ms = 0;
     if (rc == LINAC_OK) cudaEventElapsedTime(&ms, e0, e1);
     st.ms_total = ms;
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
     if (rc) return rc;
     if (h_info != INT_MAX) {
         *info_out = h_info;
@@ -1182,7 +1179,6 @@ int linac_rref_f64_workspace(int64_t rows, int64_t cols, size_t* bytes) {
 
 int linac_rref_f64(double* dA, int64_t rows, int64_t cols, int64_t ld, double tol, void* stream, int64_t* rank_out,
                    int32_t* pivot_cols_out) {
-    std::lock_guard<std::mutex> lock(g_call_mutex);
     linac_stats& st = stats();
     st = linac_stats{};
     if (rows < 0 || cols < 0 || rows >= (1ll << 31) || cols >= (1ll << 31) || !rank_out) return LINAC_ERR_INVALID_ARG;

@@ -19,7 +19,6 @@
 #include "fp_strip.cuh"
 
 namespace linac {
-extern std::mutex g_call_mutex;
 
 namespace {
 
@@ -32,6 +31,7 @@ struct Fp {
     int64_t bps;              // base panels per strip
     int64_t ns;               // number of strips
     int coop_grid;            // CTAs of the cooperative strip kernel
+    int slot;                 // this thread's entry of the constant field table
     // device metadata
     int32_t* d_pivcols;
     int32_t* d_pstart;        // [nb+1]
@@ -43,8 +43,26 @@ struct Fp {
     unsigned long long* h_mail;      // mapped pinned, MAXBP * MAIL_WORDS tagged words written by the strip kernel itself
     std::vector<int64_t> pstart;     // [nb+1] pivots found left of base panel b
     std::vector<int32_t> pivcols;
-    cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev_strip = nullptr;
-    cudaStream_t copy_s = nullptr;   // second stream: device->host reads of the pivot counts
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    // timing == 2: the PRODUCTION schedule with an event pair around every launch and no host synchronisation; the
+    // pairs are read after the call's final sync (class 0 = Schur update, 1 = strip kernel, 2 = triangular solve)
+    std::vector<cudaEvent_t>* pool = nullptr;
+    struct Mark { int cls; int ev; int64_t m, n, k; };
+    std::vector<Mark> marks;
+    int pool_used = 0;
+    int mark_begin(int cls, int64_t m = 0, int64_t n = 0, int64_t k = 0) {
+        if (options().timing != 2 || !pool) return -1;
+        if (pool_used + 2 > (int)pool->size()) {
+            const size_t old = pool->size();
+            pool->resize(old + 512, nullptr);
+            for (size_t i = old; i < pool->size(); ++i) cudaEventCreate(&(*pool)[i]);
+        }
+        marks.push_back({cls, pool_used, m, n, k});
+        cudaEventRecord((*pool)[pool_used], s);
+        pool_used += 2;
+        return (int)marks.size() - 1;
+    }
+    void mark_end(int h) { if (h >= 0) cudaEventRecord((*pool)[marks[h].ev + 1], s); }
 
     int64_t sb0(int64_t s) const { return std::min(nb, s * bps); }          // first base panel of strip s
     int64_t sp(int64_t s) const { return pstart[sb0(s)]; }                  // pivots found left of strip s
@@ -56,8 +74,9 @@ int64_t panel_col0(int64_t b) { return b * PW; }
 
 int run_gemm(Fp& c, const GemmArgs& g) {
     Options& o = options();
-    const bool timing = o.timing != 0;
+    const bool timing = o.timing == 1;
     if (timing) cudaEventRecord(c.ev0, c.s);
+    const int mk = c.mark_begin(0, g.M, g.N, g.K);
     int rc = -1;
     if (o.gemm_path != 1 && g.K >= o.tc_min_k && g.M >= o.tc_min_mn && g.N >= o.tc_min_mn) {
         const size_t mark = c.arena->off;
@@ -65,6 +84,7 @@ int run_gemm(Fp& c, const GemmArgs& g) {
         c.arena->off = mark;
     }
     if (rc < 0) rc = gemm_modp_simt(g, c.f, c.s);
+    c.mark_end(mk);
     if (timing && rc == LINAC_OK) {
         cudaEventRecord(c.ev1, c.s);
         cudaEventSynchronize(c.ev1);
@@ -81,9 +101,12 @@ int run_gemm(Fp& c, const GemmArgs& g) {
 
 // Brackets one kernel class with events when the "timing" option is on (costs a host sync per launch).
 struct Timed {
-    Fp& c; double& acc; bool on;
-    Timed(Fp& c_, double& acc_) : c(c_), acc(acc_), on(options().timing != 0) { if (on) cudaEventRecord(c.ev0, c.s); }
+    Fp& c; double& acc; bool on; int mk;
+    Timed(Fp& c_, double& acc_, int cls) : c(c_), acc(acc_), on(options().timing == 1), mk(c_.mark_begin(cls)) {
+        if (on) cudaEventRecord(c.ev0, c.s);
+    }
     ~Timed() {
+        c.mark_end(mk);
         if (!on) return;
         cudaEventRecord(c.ev1, c.s);
         cudaEventSynchronize(c.ev1);
@@ -99,7 +122,7 @@ int trsm_leaf(Fp& c, int64_t s, uint32_t* X, int64_t ldx, int64_t ncols) {
     const int64_t K = c.sp(s + 1) - c.sp(s);
     if (K <= 0 || ncols <= 0) return LINAC_OK;
     if (!LOWER && c.sb0(s + 1) - c.sb0(s) <= 1) return LINAC_OK;     // U is the identity inside one base panel
-    Timed tm(c, stats().ms_trsm);
+    Timed tm(c, stats().ms_trsm, 2);
     trsm_strip_kernel<LOWER><<<(unsigned)((ncols + PW - 1) / PW), TNT, trsm_smem_bytes(K), c.s>>>(
         c.A, c.ld, X, ldx, ncols, c.d_pstart, (int)c.sb0(s), (int)c.sb0(s + 1), c.d_T, c.d_pivcols, c.f, nullptr, 0, nullptr, 0, nullptr);
     LINAC_CUDA(cudaGetLastError());
@@ -137,20 +160,21 @@ int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r, int64_t early_c0 = 0,
     StripArgs a;
     a.A = c.A; a.ld = c.ld; a.rows = c.rows; a.cols = c.cols; a.i0 = i0; a.j0 = j0; a.ws = (int)(j1 - j0);
     a.rec = c.d_rec; a.T = c.d_T; a.E = c.d_E; a.pivcols = c.d_pivcols; a.pstart = c.d_pstart;
-    static unsigned long long seq_counter = 0;
     a.Aq = tail_Aq; a.kp = early_kp;
-    a.seq = (++seq_counter) & 0xFFFFFFFFull;
-    if (a.seq == 0) a.seq = ++seq_counter & 0xFFFFFFFFull;      // 0 is the mailbox's initial content
-    const bool early = early_ncols > 0 && options().timing == 0;
+    a.slot = c.slot;
+    a.seq = (++ctx().seq) & 0xFFFFFFFFull;
+    if (a.seq == 0) a.seq = ++ctx().seq & 0xFFFFFFFFull;        // 0 is the mailbox's initial content
+    const bool early = early_ncols > 0 && options().timing != 1;
     a.host_mail = early ? nullptr : c.h_mail;                    // with an early solve, the solve kernel mails
     void* args[] = {&a};
     {
-        Timed tm(c, stats().ms_strip);
+        Timed tm(c, stats().ms_strip, 1);
         LINAC_CUDA(cudaLaunchCooperativeKernel((void*)strip_factor_kernel, dim3((unsigned)c.coop_grid), dim3(SNT), args,
                                                sizeof(StripSmem), c.s));
     }
     linac_stats& st = stats();
     if (early) {
+        Timed tm(c, stats().ms_trsm, 2);
         trsm_strip_kernel<true><<<(unsigned)((early_ncols + PW - 1) / PW), TNT, trsm_smem_bytes(j1 - j0), c.s>>>(
             c.A, c.ld, c.A + i0 * c.ld + early_c0, c.ld, early_ncols, c.d_pstart, (int)b0, (int)b1, c.d_T, c.d_pivcols, c.f,
             early_Bq, early_kp, c.h_mail, a.seq, c.d_rec);
@@ -179,17 +203,6 @@ int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r, int64_t early_c0 = 0,
     }
     st.kernel_launches++;
     st.host_syncs++;
-#ifdef LINAC_TRACE
-    if (s == 0 || s == c.ns / 2) {
-        unsigned long long h[64];
-        cudaMemcpyFromSymbol(h, g_strip_trace, sizeof h);
-        for (int ct = 0; ct < 2; ++ct) {
-            printf("strip %ld cta %d panel 1 (ns since phase A start):", (long)s, ct);
-            for (int k = 1; k < 14; ++k) printf(" [%d]%lld", k, h[ct * 32 + k] ? (long long)(h[ct * 32 + k] - h[ct * 32]) : -1ll);
-            printf("\n");
-        }
-    }
-#endif
     int64_t cur = i0;
     for (int64_t b = b0; b < b1; ++b) {
         const unsigned long long* m = c.h_mail + (b - b0) * MAIL_WORDS;
@@ -311,19 +324,18 @@ int trsm_upper(Fp& c, uint32_t* F, int64_t ldf, int64_t nf, int64_t s0, int64_t 
 
 // Grid of the cooperative strip kernel: every CTA must be resident (one per SM with 1024 threads).
 int strip_grid(int* grid) {
-    static int cached = 0;
-    if (!cached) {
+    static PerDeviceOnce once;
+    const int rc = once.run([]() -> int {
         LINAC_CUDA(cudaFuncSetAttribute(strip_factor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(StripSmem)));
-        int dev = 0, sms = 0, per_sm = 0;
-        LINAC_CUDA(cudaGetDevice(&dev));
-        LINAC_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        int per_sm = 0;
         LINAC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, strip_factor_kernel, SNT, sizeof(StripSmem)));
         LINAC_CUDA(cudaFuncSetAttribute(trsm_strip_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)trsm_smem_bytes(SW_MAX)));
         LINAC_CUDA(cudaFuncSetAttribute(trsm_strip_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)trsm_smem_bytes(SW_MAX)));
-        if (per_sm < 1 || sms < 1) return LINAC_ERR_INTERNAL;
-        cached = sms;                                 // one CTA per SM: more would only lengthen the grid barrier
-    }
-    *grid = cached;
+        if (per_sm < 1 || sm_count() < 1) return LINAC_ERR_INTERNAL;
+        return LINAC_OK;
+    });
+    if (rc) return rc;
+    *grid = sm_count();                               // one CTA per SM: more would only lengthen the grid barrier
     return LINAC_OK;
 }
 
@@ -332,7 +344,9 @@ int64_t num_panels(int64_t cols) { return (cols + PW - 1) / PW; }
 size_t meta_bytes(int64_t rows, int64_t cols) {
     const int64_t mn = std::max<int64_t>(1, std::min(rows, cols));
     const int64_t nb = num_panels(cols);
-    return 8192 + (size_t)nb * (sizeof(PanelRec) + 256 + 2 * PW * PW * 4 + 4) + (size_t)mn * 4 + (size_t)cols * 4 + 10 * 256;
+    // + the index arrays of the consumers that run behind the reduction (null space: 2 cols; solve: cols + nrhs; C.R: rank)
+    return 8192 + (size_t)nb * (sizeof(PanelRec) + 256 + 2 * PW * PW * 4 + 4) + (size_t)mn * 4 + (size_t)cols * 4 + 10 * 256 +
+           (size_t)cols * 12 + (size_t)mn * 4 + 4096;
 }
 
 // Free-column slab width for the back-elimination workspace.
@@ -348,11 +362,6 @@ size_t workspace_bytes(int64_t rows, int64_t cols) {
     b += gemm_modp_tc_scratch_bytes(rows, cols, std::min<int64_t>(mn, 4096)) + 256;
     return b;
 }
-
-struct PinnedRec {
-    unsigned long long* p = nullptr;
-    ~PinnedRec() { if (p) cudaFreeHost(p); }
-};
 
 int validate(const uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p) {
     if (rows < 0 || cols < 0 || cols >= (1ll << 31) || rows >= (1ll << 31)) return LINAC_ERR_INVALID_ARG;
@@ -373,17 +382,19 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     if (rows == 0 || cols == 0) return LINAC_OK;
     // 2^31 <= p < 2^32: the CUDA-core Montgomery path of fp_wide.cu; the limb-plane tensor path and the
     // 64-bit accumulators of the strip kernels are built for p < 2^31
-    if (p >= (1u << 31)) return rref_u32_wide(dA, rows, cols, ld, p, s, rank, pivot_cols_out);
     rc = check_device();
     if (rc) return rc;
-    rc = acquire_workspace(workspace_bytes(rows, cols), arena);
+    rc = acquire_workspace(std::max(workspace_bytes(rows, cols), wide_workspace_u32(rows, cols)), arena);
     if (rc) return rc;
+    if (p >= (1u << 31)) return rref_u32_wide(dA, rows, cols, ld, p, s, rank, pivot_cols_out, arena);
 
-    static PinnedRec pinned;
-    if (!pinned.p) {
-        LINAC_CUDA(cudaHostAlloc(&pinned.p, MAXBP * MAIL_WORDS * sizeof(unsigned long long), cudaHostAllocMapped));
-        memset(pinned.p, 0, MAXBP * MAIL_WORDS * sizeof(unsigned long long));
+    Context& cx = ctx();
+    if (!cx.mail) {
+        LINAC_CUDA(cudaHostAlloc(&cx.mail, MAXBP * MAIL_WORDS * sizeof(unsigned long long), cudaHostAllocMapped | cudaHostAllocPortable));
+        memset(cx.mail, 0, MAXBP * MAIL_WORDS * sizeof(unsigned long long));
     }
+    const int slot = acquire_field_slot();
+    if (slot < 0) return LINAC_ERR_INTERNAL;          // more than FIELD_SLOTS host threads inside the library at once
 
     Fp c;
     c.A = dA; c.rows = rows; c.cols = cols; c.ld = ld; c.f = make_modp(p); c.s = s; c.arena = arena;
@@ -401,21 +412,20 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     c.d_pstart = (int32_t*)arena->take((size_t)(c.nb + 1) * 4);
     if (!c.d_rec || !c.d_T || !c.d_E || !c.d_pivcols || !d_colinfo || !c.d_pstart) return LINAC_ERR_WORKSPACE;
     LINAC_CUDA(cudaMemsetAsync(c.d_pstart, 0, (size_t)(c.nb + 1) * 4, s));
-    c.h_mail = pinned.p;
+    c.h_mail = cx.mail;
+    c.slot = slot;
     c.pivcols.assign(mn, -1);
     c.pstart.assign(c.nb + 1, 0);
-    LINAC_CUDA(cudaEventCreate(&c.ev0));
-    LINAC_CUDA(cudaEventCreate(&c.ev1));
-    LINAC_CUDA(cudaEventCreateWithFlags(&c.ev_strip, cudaEventDisableTiming));
-    static cudaStream_t copy_stream = nullptr;
-    if (!copy_stream) LINAC_CUDA(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
-    c.copy_s = copy_stream;
-    cudaEvent_t t0, t1;
-    LINAC_CUDA(cudaEventCreate(&t0));
-    LINAC_CUDA(cudaEventCreate(&t1));
+    CallEvents evs;
+    rc = evs.create();
+    if (rc) return rc;
+    c.ev0 = evs.ev0; c.ev1 = evs.ev1;
+    std::vector<cudaEvent_t>& event_pool = cx.events;
+    c.pool = &event_pool;
+    cudaEvent_t t0 = evs.t0, t1 = evs.t1;
     LINAC_CUDA(cudaEventRecord(t0, s));
 
-    LINAC_CUDA(cudaMemcpyToSymbolAsync(c_f, &c.f, sizeof(ModP), 0, cudaMemcpyHostToDevice, s));
+    LINAC_CUDA(cudaMemcpyToSymbolAsync(c_f, &c.f, sizeof(ModP), (size_t)slot * sizeof(ModP), cudaMemcpyHostToDevice, s));
     // S0 ingest
     {
         const bool vec = ((((uintptr_t)dA) | ((uintptr_t)ld * 4)) & 15) == 0 && cols >= 4;
@@ -487,16 +497,29 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     float ms = 0;
     if (e == cudaSuccess) cudaEventElapsedTime(&ms, t0, t1);
     st.ms_total = ms;
-    cudaEventDestroy(t0); cudaEventDestroy(t1);
-    cudaEventDestroy(c.ev0); cudaEventDestroy(c.ev1); cudaEventDestroy(c.ev_strip);
+    if (e == cudaSuccess && options().timing == 2) {           // per-class device time of the production schedule
+        for (const Fp::Mark& mk : c.marks) {
+            float t = 0;
+            if (cudaEventElapsedTime(&t, event_pool[mk.ev], event_pool[mk.ev + 1]) != cudaSuccess) continue;
+            if (mk.cls == 0) {
+                st.ms_update += t;
+                if ((double)mk.m * mk.n * mk.k > (double)st.top_m * st.top_n * st.top_k) {
+                    st.top_m = mk.m; st.top_n = mk.n; st.top_k = mk.k;
+                    st.ms_update_top = t;
+                }
+            } else if (mk.cls == 1) st.ms_strip += t;
+            else st.ms_trsm += t;
+        }
+    }
     if (rc) return rc;
     *rank = r;
     if (pivot_cols_out) std::copy(c.pivcols.begin(), c.pivcols.begin() + r, pivot_cols_out);
     return LINAC_OK;
 }
 
+// `arena`: workspace to take the two index arrays from (the reduction's arena when called behind it).
 int nullspace_from_rref_impl(const uint32_t* dR, int64_t rows, int64_t cols, int64_t ld, uint32_t p, int64_t rank,
-                             const int32_t* pivot_cols, uint32_t* dK, int64_t ldk, cudaStream_t s) {
+                             const int32_t* pivot_cols, uint32_t* dK, int64_t ldk, cudaStream_t s, Arena* arena) {
     (void)rows;
     const int64_t d = cols - rank;
     if (d <= 0) return LINAC_OK;
@@ -510,8 +533,8 @@ int nullspace_from_rref_impl(const uint32_t* dR, int64_t rows, int64_t cols, int
     }
     for (int64_t cc = 0; cc < cols; ++cc)
         if (!is_piv[cc]) { colmap[cc] = -(int32_t)freec.size() - 1; freec.push_back((int32_t)cc); }
-    int32_t* dm = nullptr;
-    LINAC_CUDA(cudaMalloc(&dm, (size_t)(cols + d) * 4));
+    int32_t* dm = (int32_t*)arena->take((size_t)(cols + d) * 4);
+    if (!dm) return LINAC_ERR_WORKSPACE;
     cudaError_t e = cudaMemcpyAsync(dm, colmap.data(), (size_t)cols * 4, cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) e = cudaMemcpyAsync(dm + cols, freec.data(), (size_t)d * 4, cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) {
@@ -521,7 +544,6 @@ int nullspace_from_rref_impl(const uint32_t* dR, int64_t rows, int64_t cols, int
         stats().kernel_launches++;
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-    cudaFree(dm);
     if (e != cudaSuccess) { set_cuda_error(e, "nullspace", __FILE__, __LINE__); return LINAC_ERR_CUDA; }
     return LINAC_OK;
 }
@@ -541,14 +563,12 @@ int linac_rref_u32_workspace(int64_t rows, int64_t cols, size_t* bytes) {
 
 int linac_rref_u32(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, void* stream, int64_t* rank,
                    int32_t* pivot_cols_out) {
-    std::lock_guard<std::mutex> lock(g_call_mutex);
     Arena arena;
     return rref_impl(dA, rows, cols, ld, p, (cudaStream_t)stream, rank, pivot_cols_out, &arena);
 }
 
 int linac_nullspace_u32(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, void* stream, int64_t* rank,
                         int32_t* pivot_cols_out, uint32_t* dK, int64_t ldk, int64_t k_capacity_cols, int64_t* nullity) {
-    std::lock_guard<std::mutex> lock(g_call_mutex);
     if (!nullity || k_capacity_cols < 0 || (k_capacity_cols > 0 && (!dK || ldk < k_capacity_cols)))
         return LINAC_ERR_INVALID_ARG;
     Arena arena;
@@ -562,14 +582,13 @@ int linac_nullspace_u32(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, ui
     if (cols - r > k_capacity_cols) return LINAC_ERR_BUFFER_TOO_SMALL;
     if (cols == 0) return LINAC_OK;
     const linac_stats keep = stats();
-    rc = nullspace_from_rref_impl(dA, rows, cols, ld, p, r, piv.data(), dK, ldk, (cudaStream_t)stream);
+    rc = nullspace_from_rref_impl(dA, rows, cols, ld, p, r, piv.data(), dK, ldk, (cudaStream_t)stream, &arena);
     stats().kernel_launches = keep.kernel_launches + 1;
     return rc;
 }
 
 int linac_solve_u32(uint32_t* dM, int64_t rows, int64_t cols, int64_t nrhs, int64_t ld, uint32_t p, void* stream,
                     int64_t* rank_a, int32_t* pivot_cols_out, uint8_t* consistent, uint32_t* dX, int64_t ldx) {
-    std::lock_guard<std::mutex> lock(g_call_mutex);
     if (cols < 0 || nrhs < 0 || !rank_a || (nrhs > 0 && !consistent)) return LINAC_ERR_INVALID_ARG;
     if (cols > 0 && nrhs > 0 && (!dX || ldx < nrhs)) return LINAC_ERR_INVALID_ARG;
     const int64_t wide = cols + nrhs;
@@ -592,10 +611,9 @@ int linac_solve_u32(uint32_t* dM, int64_t rows, int64_t cols, int64_t nrhs, int6
     cudaStream_t s = (cudaStream_t)stream;
     std::vector<int32_t> colrow((size_t)std::max<int64_t>(1, cols), -1);
     for (int64_t k = 0; k < ra; ++k) colrow[piv[k]] = (int32_t)k;
-    int32_t* d_colrow = nullptr;
-    uint8_t* d_cons = nullptr;
-    LINAC_CUDA(cudaMalloc(&d_colrow, colrow.size() * 4 + (size_t)nrhs + 16));
-    d_cons = reinterpret_cast<uint8_t*>(d_colrow + colrow.size());
+    int32_t* d_colrow = (int32_t*)arena.take(colrow.size() * 4 + (size_t)nrhs + 16);
+    if (!d_colrow) return LINAC_ERR_WORKSPACE;
+    uint8_t* d_cons = reinterpret_cast<uint8_t*>(d_colrow + colrow.size());
     cudaError_t e = cudaMemcpyAsync(d_colrow, colrow.data(), colrow.size() * 4, cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) {
         dim3 grid((unsigned)((nrhs + 127) / 128), (unsigned)std::max<int64_t>(1, std::min<int64_t>(cols, 2048)));
@@ -605,14 +623,12 @@ int linac_solve_u32(uint32_t* dM, int64_t rows, int64_t cols, int64_t nrhs, int6
     }
     if (e == cudaSuccess) e = cudaMemcpyAsync(consistent, d_cons, (size_t)nrhs, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-    cudaFree(d_colrow);
     if (e != cudaSuccess) { set_cuda_error(e, "linac_solve_u32", __FILE__, __LINE__); return LINAC_ERR_CUDA; }
     return LINAC_OK;
 }
 
 int linac_rank_factor_u32(const uint32_t* dA, int64_t rows, int64_t cols, int64_t lda, uint32_t p, void* stream,
                           uint32_t* dR, int64_t ldr, uint32_t* dC, int64_t ldc, int64_t* rank, int32_t* pivot_cols_out) {
-    std::lock_guard<std::mutex> lock(g_call_mutex);
     if (rows < 0 || cols < 0 || !rank) return LINAC_ERR_INVALID_ARG;
     const int64_t cap = std::min(rows, cols);
     if (rows > 0 && cols > 0 && (!dA || !dR || !dC || lda < cols || ldr < cols || ldc < cap)) return LINAC_ERR_INVALID_ARG;
@@ -631,8 +647,8 @@ int linac_rank_factor_u32(const uint32_t* dA, int64_t rows, int64_t cols, int64_
     *rank = r;
     if (pivot_cols_out) std::copy(piv.begin(), piv.begin() + r, pivot_cols_out);
     if (r == 0) return LINAC_OK;
-    int32_t* d_piv = nullptr;
-    LINAC_CUDA(cudaMalloc(&d_piv, (size_t)r * 4));
+    int32_t* d_piv = (int32_t*)arena.take((size_t)r * 4);
+    if (!d_piv) return LINAC_ERR_WORKSPACE;
     cudaError_t e = cudaMemcpyAsync(d_piv, piv.data(), (size_t)r * 4, cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) {
         dim3 grid((unsigned)((r + 255) / 256), (unsigned)std::min<int64_t>(rows, 148 * 8));
@@ -641,14 +657,12 @@ int linac_rank_factor_u32(const uint32_t* dA, int64_t rows, int64_t cols, int64_
         stats().kernel_launches++;
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-    cudaFree(d_piv);
     if (e != cudaSuccess) { set_cuda_error(e, "linac_rank_factor_u32", __FILE__, __LINE__); return LINAC_ERR_CUDA; }
     return LINAC_OK;
 }
 
 int linac_load_matrix_u32(uint32_t* dA, int64_t n_rows, int64_t n_cols, int64_t ld, const uint32_t* dBases, int64_t n_basis,
                           int64_t ldb, const int32_t* dLindices, int64_t d, uint32_t p, void* stream) {
-    std::lock_guard<std::mutex> lock(g_call_mutex);
     if (n_rows < 0 || n_cols < 0 || n_basis < 0 || d < 0 || d > 4096) return LINAC_ERR_INVALID_ARG;
     if (p < 2 || p >= (1u << 31) || !is_prime_u32(p)) return LINAC_ERR_BAD_MODULUS;
     if (n_rows == 0 || n_cols == 0) return LINAC_OK;
@@ -681,7 +695,6 @@ int linac_load_matrix_u32(uint32_t* dA, int64_t n_rows, int64_t n_cols, int64_t 
 
 int linac_nullspace_from_rref_u32(const uint32_t* dR, int64_t rows, int64_t cols, int64_t ld, uint32_t p, int64_t rank,
                                   const int32_t* pivot_cols, uint32_t* dK, int64_t ldk, void* stream) {
-    std::lock_guard<std::mutex> lock(g_call_mutex);
     if (rows < 0 || cols < 0 || rank < 0 || rank > std::min(rows, cols) || (rank > 0 && !pivot_cols))
         return LINAC_ERR_INVALID_ARG;
     if (cols - rank > 0 && (!dK || ldk < cols - rank)) return LINAC_ERR_INVALID_ARG;
@@ -689,12 +702,14 @@ int linac_nullspace_from_rref_u32(const uint32_t* dR, int64_t rows, int64_t cols
     if (p < 2 || !is_prime_u64(p)) return LINAC_ERR_BAD_MODULUS;
     int rc = check_device();
     if (rc) return rc;
-    return nullspace_from_rref_impl(dR, rows, cols, ld, p, rank, pivot_cols, dK, ldk, (cudaStream_t)stream);
+    Arena arena;
+    rc = acquire_workspace((size_t)(2 * cols + 64) * 4, &arena);
+    if (rc) return rc;
+    return nullspace_from_rref_impl(dR, rows, cols, ld, p, rank, pivot_cols, dK, ldk, (cudaStream_t)stream, &arena);
 }
 
 int linac_gemm_sub_u32(uint32_t* dC, int64_t ldc, const uint32_t* dA, int64_t lda, const uint32_t* dB, int64_t ldb, int64_t M,
                        int64_t N, int64_t K, uint32_t p, int path, void* stream) {
-    std::lock_guard<std::mutex> lock(g_call_mutex);
     if (M < 0 || N < 0 || K < 0 || path < 0 || path > 2) return LINAC_ERR_INVALID_ARG;
     if (p < 2 || p >= (1u << 31) || !is_prime_u32(p)) return LINAC_ERR_BAD_MODULUS;
     if (M == 0 || N == 0 || K == 0) return LINAC_OK;
@@ -705,9 +720,10 @@ int linac_gemm_sub_u32(uint32_t* dC, int64_t ldc, const uint32_t* dA, int64_t ld
     const ModP f = make_modp(p);
     cudaStream_t s = (cudaStream_t)stream;
     GemmArgs g{dC, ldc, dA, lda, nullptr, dB, ldb, M, N, K};
-    cudaEvent_t e0, e1;
-    LINAC_CUDA(cudaEventCreate(&e0));
-    LINAC_CUDA(cudaEventCreate(&e1));
+    CallEvents evs;
+    rc = evs.create();
+    if (rc) return rc;
+    cudaEvent_t e0 = evs.ev0, e1 = evs.ev1;
     rc = -1;
     cudaEventRecord(e0, s);
     if (path == 2 || (path == 0 && K >= options().tc_min_k && M >= options().tc_min_mn && N >= options().tc_min_mn)) {
@@ -725,8 +741,6 @@ int linac_gemm_sub_u32(uint32_t* dC, int64_t ldc, const uint32_t* dA, int64_t ld
     if (e == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
     stats().ms_update = ms;
     stats().ms_total = ms;
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
     return rc;
 }
 

@@ -25,20 +25,10 @@
 namespace linac {
 namespace cg = cooperative_groups;
 
-// Debug build only (-DLINAC_TRACE, see build.py): %globaltimer stamps of CTA 0 / CTA 1 for the first
-// panel of a strip, printed by the host after the launch.
-#ifdef LINAC_TRACE
-__device__ unsigned long long g_strip_trace[64];
-#define STRIP_STAMP(slot) do { if (threadIdx.x == 0 && blockIdx.x < 2 && g_trace_on) { unsigned long long t_; \
-    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_)); g_strip_trace[blockIdx.x * 32 + (slot)] = t_; } } while (0)
-__device__ int g_trace_on = 0;
-#else
-#define STRIP_STAMP(slot) do { } while (0)
-#endif
-
-// The field of the running call (set once per call by the host, cudaMemcpyToSymbolAsync on the call's
-// stream): read through the constant bank, so no device function carries it in registers or on the stack.
-__constant__ ModP c_f;
+// The fields of the running calls: one slot per host thread inside the library (Context::slot), written once per
+// call by the host (cudaMemcpyToSymbolAsync on the call's stream) and read through the constant bank, so no device
+// function carries the descriptor in registers or on the stack.  The strip kernel keeps its slot in shared memory.
+__constant__ ModP c_f[FIELD_SLOTS];
 
 constexpr int SW_MAX = 256;                 // widest strip (columns)
 constexpr int SNT = 1024;                   // threads per CTA of the strip kernel (32 warps)
@@ -57,6 +47,7 @@ struct UPending {
 };
 
 struct StripSmem {
+    int slot;                        // this launch's entry of c_f
     // ---- P1
     uint32_t W[2][PW][PW + 1];       // fast path: double-buffered block; general path: W[0] = chunk X, W[1] = Ep
     uint32_t G[PW][2 * PW + 1];      // general path phase 2: [D | I]
@@ -106,7 +97,7 @@ struct StripSmem {
 #define FAST_IF8(...)
 #endif
 __device__ __forceinline__ bool panel_fast(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t i0, int64_t j0) {
-    const ModP& f = c_f;
+    const ModP& f = c_f[sm.slot];
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
     constexpr int FW = PW / FAST_RPW, RPW = FAST_RPW;          // working warps, block rows per warp (registers)
     uint32_t x0 = 0, x1 = 0, x2 = 0, x3 = 0, x4 = 0, x5 = 0, x6 = 0, x7 = 0;
@@ -121,7 +112,6 @@ __device__ __forceinline__ bool panel_fast(StripSmem& sm, const uint32_t* A, int
 #undef FAST_PUT
     }
     __syncthreads();
-    STRIP_STAMP(1);
     if (wq < FW) {
         unsigned used = 0;
         uint32_t dtot = 1u;                       // product of the pivots so far (the scale of every unused row)
@@ -155,7 +145,6 @@ __device__ __forceinline__ bool panel_fast(StripSmem& sm, const uint32_t* A, int
         if (tid == 0) { sm.fast_ok = ok ? 1 : 0; sm.gs[1][0] = dtot; }
     }
     __syncthreads();
-    STRIP_STAMP(2);
     return sm.fast_ok != 0;     // on success the final block is in W[0] (32 steps); gs[1][0] = product of all pivots
 }
 
@@ -167,7 +156,7 @@ __device__ __forceinline__ bool panel_fast(StripSmem& sm, const uint32_t* A, int
 // column-to-column dependency chain.  The scan stops once w pivots are known; otherwise it has looked
 // at every row, which is what proves the remaining columns are free columns.  Returns r.
 __device__ __noinline__ int panel_scan(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t rows, int64_t i0, int64_t j0, int w) {
-    const ModP& f = c_f;
+    const ModP& f = c_f[sm.slot];
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
     uint32_t (*X)[PW + 1] = sm.W[0];
     uint32_t (*Ep)[PW + 1] = sm.W[1];          // pivot rows as selected (unnormalised), discovery order
@@ -222,7 +211,7 @@ __device__ __noinline__ int panel_scan(StripSmem& sm, const uint32_t* A, int64_t
 // transform in G.  Also E = T.A[P, panel] when r < w.
 __device__ __noinline__ void panel_invert_general(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t j0, int w, int r,
                                                   uint32_t* Tout, uint32_t* Eout) {
-    const ModP& f = c_f;
+    const ModP& f = c_f[sm.slot];
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
     for (int e = tid; e < PW * 2 * PW; e += SNT) {
         const int a = e / (2 * PW), b = e % (2 * PW);
@@ -303,7 +292,7 @@ __device__ void panel_exchange_list(StripSmem& sm, int64_t i0, int r, PanelRec* 
 __device__ bool panel_factor(StripSmem& sm, const uint32_t* A, int64_t ld, int64_t rows, int64_t i0, int64_t j0, int w,
                              PanelRec* rec, uint32_t* Tout, uint32_t* Eout, int32_t* pivcols_global,
                              bool allow_general = true) {
-    const ModP& f = c_f;
+    const ModP& f = c_f[sm.slot];
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
     int r = 0;
     bool fast = false;
@@ -317,7 +306,6 @@ __device__ bool panel_factor(StripSmem& sm, const uint32_t* A, int64_t ld, int64
         if (wq == 0) sm.ginv[lane] = mulredc(sm.gs[0][lane], invmod_fermat(sm.gs[1][0], f), f);
         __syncthreads();
         if (wq == 0) panel_exchange_list(sm, i0, r, rec);
-        STRIP_STAMP(3);
         const int qa = (int)(sm.esrc[wq] - i0);
         Tout[wq * PW + lane] = mulmod(sm.ginv[wq], sm.W[0][qa][lane], f);
     } else {
@@ -344,7 +332,6 @@ __device__ bool panel_factor(StripSmem& sm, const uint32_t* A, int64_t ld, int64
         sm.last_r = r;
         sm.last_nsw = sm.nsw;
     }
-    STRIP_STAMP(4);
     return true;
 }
 
@@ -381,6 +368,7 @@ struct StripArgs {
     int kp;                  //   Aq[limb][m][kp], k-major, zero padded to kp (what the Schur update's TMA loads expect)
     unsigned long long* host_mail;  // mapped pinned host memory: MAXBP * MAIL_WORDS tagged words, written by CTA 0
     unsigned long long seq;         // tag of this launch (32 significant bits)
+    int slot;                       // entry of c_f that holds this call's field
 };
 
 // Deferred write-back of a U12 slice: the raw entries it replaces are read by every row worker of
@@ -404,7 +392,7 @@ template <int RPT>
 __device__ __noinline__ void strip_update_t(StripSmem& sm, int slot, uint32_t* A, int64_t ld, const uint32_t* Tb,
                                             unsigned pcm, int64_t jp, int64_t pr0, int r, int64_t cc0, int nc,
                                             int64_t my0, int64_t my1, bool owner) {
-    const ModP& f = c_f;
+    const ModP& f = c_f[sm.slot];
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
     constexpr int TR = 32 * RPT;
     // pivot index of panel column `lane` (pcm = mask of the panel's pivot columns, ascending), or -1
@@ -427,14 +415,12 @@ __device__ __noinline__ void strip_update_t(StripSmem& sm, int slot, uint32_t* A
             for (int t = 0; t < RPT; ++t) sm.Lk[kcol][wq + 32 * t] = lreg[t];
         }
     };
-    if (slot == 0) STRIP_STAMP(10);
     const uint32_t tval = Tb[wq * PW + lane];
     const uint32_t aval = (wq < r && lane < nc) ? A[(pr0 + wq) * ld + cc0 + lane] : 0u;
     if (my0 < my1) load_tile(my0);
     sm.Ts[wq][lane] = tval;
     sm.Ar[wq][lane] = aval;
     __syncthreads();
-    if (slot == 0) STRIP_STAMP(11);
     {
         uint64_t acc = 0;
 #pragma unroll 8
@@ -452,7 +438,6 @@ __device__ __noinline__ void strip_update_t(StripSmem& sm, int slot, uint32_t* A
             load_tile(m0);
         }
         __syncthreads();
-        if (slot == 0) STRIP_STAMP(12);
         if (m0 + wq * RPT < my1) {
             uint64_t acc[RPT];
 #pragma unroll
@@ -495,7 +480,6 @@ __device__ __noinline__ void strip_update_t(StripSmem& sm, int slot, uint32_t* A
         }
     }
     __syncthreads();                     // Ts / Ar / Lk may be reused by the caller's next phase
-    if (slot == 0) STRIP_STAMP(13);
 }
 
 // CTA 0 running ahead of the others: U = T . A[pr0 : pr0+r, cc0 : cc0+32] (kept in Us[0], written back after the
@@ -504,7 +488,7 @@ __device__ __noinline__ void strip_update_t(StripSmem& sm, int slot, uint32_t* A
 // sits between two panel factorisations on the pivot-to-pivot chain.
 __device__ __noinline__ void strip_ahead_update(StripSmem& sm, uint32_t* A, int64_t ld, const uint32_t* Tb, unsigned pcm,
                                                 int64_t jp, int64_t pr0, int r, int64_t cc0, int64_t c0row) {
-    const ModP& f = c_f;
+    const ModP& f = c_f[sm.slot];
     const int tid = threadIdx.x, lane = tid & 31, a = tid >> 5;
     const int kcol = ((pcm >> lane) & 1u) ? __popc(pcm & ((1u << lane) - 1u)) : -1;
     const uint32_t t = Tb[a * PW + lane];
@@ -611,7 +595,7 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
         if (tid == 0) { sm.pend[0].row0 = -1; sm.pend[1].row0 = -1; }
     };
 
-    if (tid == 0) { sm.pend[0].row0 = -1; sm.pend[1].row0 = -1; }
+    if (tid == 0) { sm.pend[0].row0 = -1; sm.pend[1].row0 = -1; sm.slot = a.slot; }
     __syncthreads();
     factor_full(b0, a.j0, (int)min((int64_t)PW, cu1 - a.j0), cur);
     grid.sync();
@@ -621,10 +605,6 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
         const int w = (int)min((int64_t)PW, cu1 - jp);
         const int64_t cu0 = jp + w;                // first strip column right of panel i
         const int wn = (int)min((int64_t)PW, cu1 - cu0);      // width of panel i+1 (<= 0: panel i is the last)
-#ifdef LINAC_TRACE
-        if (threadIdx.x == 0 && blockIdx.x < 2) g_trace_on = (i == 1);
-#endif
-        STRIP_STAMP(0);
         flush_all();
         // everything the updates need from the panel record, in ONE round trip to L2
         const PanelRec* rec = a.rec + b;
@@ -667,8 +647,7 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
         const int ncb = (ncu + PW - 1) / PW;
         const uint32_t* Tb = a.T + b * PW * PW;
         // CTA 0 runs ahead on the next panel if its 32 candidate rows exist and the fast path can take them
-        const bool ahead = G >= 2 && G - 1 >= ncb && wn == PW && cur + r + PW <= a.rows && c_f.ninv != 0;
-        STRIP_STAMP(5);
+        const bool ahead = G >= 2 && G - 1 >= ncb && wn == PW && cur + r + PW <= a.rows && c_f[a.slot].ninv != 0;
         if (G == 1 || G - 1 < ncb) {
             // degenerate grids: the column blocks in turn (sole reader and writer: the slice goes back at once)
             for (int cb = (G == 1 ? 0 : cta - 1); cb >= 0 && cb < ncb; cb += (G == 1 ? 1 : G - 1)) {
@@ -683,7 +662,6 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
         } else if (cta == 0) {
             if (ahead) {
                 strip_ahead_update(sm, A, ld, Tb, pcm, jp, cur, r, cu0, cur + r);
-                STRIP_STAMP(1);
                 const bool got = panel_factor(sm, A, ld, a.rows, cur + r, cu0, wn, a.rec + b + 1, a.T + (b + 1) * PW * PW,
                                               a.E + (b + 1) * PW * PW, a.pivcols, false);
                 if (tid == 0) {
@@ -703,9 +681,7 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
                              shared0 ? PW : 0, rw == 0 && !shared0);
             }
         }
-        STRIP_STAMP(6);
         grid.sync();
-        STRIP_STAMP(7);
         cur += r;
         // rec.pad is written ONLY between the barriers above (by CTA 0), never by the factorisation that may follow,
         // so every CTA reads the same value however late it gets here

@@ -31,7 +31,6 @@
 #include "linac_internal.h"
 
 namespace linac {
-extern std::mutex g_call_mutex;
 namespace {
 
 constexpr int WP = 32;           // panel width
@@ -363,13 +362,13 @@ F64M make_f64m(uint64_t p) {
 
 template <class T> size_t wide_workspace(int64_t rows, int64_t cols) {
     const int64_t ldu = (cols + 63) / 64 * 64;
-    return 4096 + (size_t)WP * ldu * sizeof(T) + (size_t)rows * WP * sizeof(T) + WP * WP * sizeof(T) + sizeof(WideRec) + 256 +
+    return 8192 + (size_t)cols * 12 + (size_t)WP * ldu * sizeof(T) + (size_t)rows * WP * sizeof(T) + WP * WP * sizeof(T) + sizeof(WideRec) + 256 +
            (size_t)std::max<int64_t>(1, std::min(rows, cols)) * 4 + 1024;
 }
 
 template <class F>
 int rref_wide(typename F::T* dA, int64_t rows, int64_t cols, int64_t ld, const F& f, cudaStream_t s, int64_t* rank,
-              int32_t* pivot_cols_out) {
+              int32_t* pivot_cols_out, Arena* ext_arena) {
     using T = typename F::T;
     linac_stats& st = stats();
     st = linac_stats{};
@@ -377,9 +376,12 @@ int rref_wide(typename F::T* dA, int64_t rows, int64_t cols, int64_t ld, const F
     if (rows == 0 || cols == 0) return LINAC_OK;
     int rc = check_device();
     if (rc) return rc;
-    Arena arena;
-    rc = acquire_workspace(wide_workspace<T>(rows, cols), &arena);
-    if (rc) return rc;
+    Arena own;
+    if (!ext_arena) {
+        rc = acquire_workspace(wide_workspace<T>(rows, cols), &own);
+        if (rc) return rc;
+    }
+    Arena& arena = ext_arena ? *ext_arena : own;
     const int64_t mn = std::min(rows, cols), ldu = (cols + 63) / 64 * 64;
     T* U = (T*)arena.take((size_t)WP * ldu * sizeof(T));
     T* L = (T*)arena.take((size_t)rows * WP * sizeof(T));
@@ -431,10 +433,10 @@ int rref_wide(typename F::T* dA, int64_t rows, int64_t cols, int64_t ld, const F
 
 size_t wide_workspace_u32(int64_t rows, int64_t cols) { return wide_workspace<uint32_t>(rows, cols); }
 
-// linac_rref_u32 with 2^31 <= p < 2^32 (called with the library mutex held)
+// linac_rref_u32 with 2^31 <= p < 2^32; `arena` is the caller's workspace (the consumers behind it take more from it)
 int rref_u32_wide(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, cudaStream_t s, int64_t* rank,
-                  int32_t* pivot_cols_out) {
-    return rref_wide<F32W>(dA, rows, cols, ld, make_f32w(p), s, rank, pivot_cols_out);
+                  int32_t* pivot_cols_out, Arena* arena) {
+    return rref_wide<F32W>(dA, rows, cols, ld, make_f32w(p), s, rank, pivot_cols_out, arena);
 }
 
 }  // namespace linac
@@ -451,12 +453,11 @@ int linac_rref_u64_workspace(int64_t rows, int64_t cols, size_t* bytes) {
 
 int linac_rref_u64(uint64_t* dA, int64_t rows, int64_t cols, int64_t ld, uint64_t p, void* stream, int64_t* rank,
                    int32_t* pivot_cols_out) {
-    std::lock_guard<std::mutex> lock(g_call_mutex);
     if (rows < 0 || cols < 0 || cols >= (1ll << 31) || rows >= (1ll << 31) || !rank) return LINAC_ERR_INVALID_ARG;
     if (rows > 0 && cols > 0 && (dA == nullptr || ld < cols)) return LINAC_ERR_INVALID_ARG;
     if (p < 3 || p >= (1ull << 63) || !is_prime_u64(p)) return LINAC_ERR_BAD_MODULUS;
     return rref_wide<F64M>(reinterpret_cast<unsigned long long*>(dA), rows, cols, ld, make_f64m(p), (cudaStream_t)stream, rank,
-                           pivot_cols_out);
+                           pivot_cols_out, nullptr);
 }
 
 }  // extern "C"

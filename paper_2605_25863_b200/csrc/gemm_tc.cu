@@ -23,6 +23,7 @@
 
 #include <algorithm>
 #include <mutex>
+#include <vector>
 
 #include "linac_internal.h"
 #include "tc_ptx.cuh"
@@ -45,7 +46,8 @@ constexpr int64_t KC_MAX = 4096;
 // ----------------------------------------------------------------------------- the GEMM kernel
 __global__ void __launch_bounds__(NTHREADS, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, uint32_t* __restrict__ C,
-               int64_t ldc, int64_t M, int64_t N, int kp /* padded K of this launch, multiple of KB */, ModP f) {
+               int64_t ldc, int64_t M, int64_t N, int kp /* padded K of this launch, multiple of KB */, ModP f,
+               int mtiles, int ntiles, int gm /* row tiles per band */) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     uint8_t* sA = smem;                                  // [STAGES][4][TM][KB]
@@ -57,7 +59,18 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     uint32_t* tmem_holder = (uint32_t*)(bars + 2 * STAGES + 1);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int m_tile = blockIdx.y, n_tile = blockIdx.x;
+    // Tile order: bands of `gm` row tiles, row tiles fastest inside a band.  The CTAs in flight together (one wave) then
+    // share gm A panels -- which stay in L2 while the band sweeps over the column tiles -- and a handful of B panels.
+    // In row-major tile order a wave touched 148 different B panels (more than L2 holds at K = 4096), so every row of
+    // tiles re-read all of B from DRAM: 35.7 GB of DRAM reads for a 16384^2 x 4096 product whose operands are 0.5 GB.
+    int m_tile, n_tile;
+    {
+        const int lin = blockIdx.x, per_band = gm * ntiles;
+        const int band = lin / per_band, within = lin - band * per_band;
+        const int first = band * gm, gmm = min(gm, mtiles - first);
+        n_tile = within / gmm;
+        m_tile = first + within - n_tile * gmm;
+    }
     const int nk = kp / KB;
 
     if (warp == 0 && lane == 0) {
@@ -523,16 +536,6 @@ bool make_c_map(CUtensorMap* tm, uint32_t* C, int64_t ldc, int64_t M, int64_t N)
     return r == CUDA_SUCCESS;
 }
 
-int sm_count() {
-    static int sms = 0;
-    if (!sms) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    }
-    return sms;
-}
-
 // Work items of the panel kernel: (128-row tile, run of 32-column tiles); run length chosen so that the
 // items fill a whole number of waves over the persistent grid with runs of about 24 tiles.
 PanelSched make_sched(int64_t M, int64_t N, int grid) {
@@ -566,25 +569,19 @@ size_t gemm_modp_tc_scratch_bytes(int64_t M, int64_t N, int64_t K) {
 int gemm_modp_tc(const GemmArgs& g, const ModP& f, cudaStream_t s, Arena* scratch) {
     if (g.M <= 0 || g.N <= 0 || g.K <= 0) return LINAC_OK;
     if (g.M >= (1ll << 31) || g.N >= (1ll << 31)) return -1;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(gemm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES) != cudaSuccess) {
-            cudaGetLastError();
-            return -1;
-        }
-        attr_set = true;
-    }
-    const bool panel_ok = g.K <= 2 * KB && options().tc_panel != 0 && ((((uintptr_t)g.C) | ((uintptr_t)g.ldc * 4)) & 15) == 0;
-    if (panel_ok) {
-        static bool pattr = false;
-        if (!pattr) {
-            if (cudaFuncSetAttribute(gemm_tc_panel_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM) != cudaSuccess ||
+    static PerDeviceOnce attr_once;
+    if (attr_once.run([]() -> int {
+            if (cudaFuncSetAttribute(gemm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES) != cudaSuccess ||
+                cudaFuncSetAttribute(gemm_tc_panel_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM) != cudaSuccess ||
                 cudaFuncSetAttribute(gemm_tc_panel_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM) != cudaSuccess) {
                 cudaGetLastError();
-                return -1;
+                return LINAC_ERR_CUDA;
             }
-            pattr = true;
-        }
+            return LINAC_OK;
+        }) != LINAC_OK)
+        return -1;
+    const bool panel_ok = g.K <= 2 * KB && options().tc_panel != 0 && ((((uintptr_t)g.C) | ((uintptr_t)g.ldc * 4)) & 15) == 0;
+    if (panel_ok) {
         const bool b_ready = g.Bq_ready != nullptr && g.kp_ready >= g.K && g.kp_ready <= 2 * KB && g.kp_ready % KB == 0;
         const int64_t kp = b_ready ? g.kp_ready : (g.K + KB - 1) / KB * KB;
         const bool a_ready = b_ready && g.Aq_ready != nullptr;
@@ -622,7 +619,18 @@ int gemm_modp_tc(const GemmArgs& g, const ModP& f, cudaStream_t s, Arena* scratc
     uint8_t* Aq = (uint8_t*)scratch->take((size_t)4 * g.M * kc, 1024);
     uint8_t* Bq = (uint8_t*)scratch->take((size_t)4 * g.N * kc, 1024);
     if (!Aq || !Bq) return -1;
+    // every chunk's tensor maps are encoded BEFORE the first launch: once a chunk has updated C there is no falling
+    // back to the CUDA-core kernel over the full K (it would subtract that chunk's product twice)
+    std::vector<CUtensorMap> maps;
     for (int64_t k0 = 0; k0 < g.K; k0 += kc) {
+        const int64_t kp = (std::min(kc, g.K - k0) + KB - 1) / KB * KB;
+        CUtensorMap tmA, tmB;
+        if (!make_limb_map(&tmA, Aq, g.M, kp, TM) || !make_limb_map(&tmB, Bq, g.N, kp, TN)) return -1;
+        maps.push_back(tmA);
+        maps.push_back(tmB);
+    }
+    size_t chunk = 0;
+    for (int64_t k0 = 0; k0 < g.K; k0 += kc, ++chunk) {
         const int64_t kv = std::min(kc, g.K - k0);
         const int64_t kp = (kv + KB - 1) / KB * KB;
         {
@@ -635,10 +643,14 @@ int gemm_modp_tc(const GemmArgs& g, const ModP& f, cudaStream_t s, Arena* scratc
             split_b_kernel<<<grid, 256, 0, s>>>(g.B + k0 * g.ldb, g.ldb, kv, g.N, kp, Bq);
             LINAC_CUDA(cudaGetLastError());
         }
-        CUtensorMap tmA, tmB;
-        if (!make_limb_map(&tmA, Aq, g.M, kp, TM) || !make_limb_map(&tmB, Bq, g.N, kp, TN)) return -1;
-        dim3 grid((unsigned)((g.N + TN - 1) / TN), (unsigned)((g.M + TM - 1) / TM));
-        gemm_tc_kernel<<<grid, NTHREADS, SMEM_BYTES, s>>>(tmA, tmB, g.C, g.ldc, g.M, g.N, (int)kp, f);
+        const CUtensorMap& tmA = maps[2 * chunk];
+        const CUtensorMap& tmB = maps[2 * chunk + 1];
+        const int64_t mtiles = (g.M + TM - 1) / TM, ntiles = (g.N + TN - 1) / TN;
+        if (mtiles * ntiles >= (1ll << 31)) return LINAC_ERR_INVALID_ARG;
+        // a band's A panels (gm x 128 rows x kp x 4 planes) should take about a quarter of the 126 MB L2
+        const int gm = (int)std::max<int64_t>(4, std::min<int64_t>(32, (32ll << 20) / (4 * TM * kp)));
+        gemm_tc_kernel<<<(unsigned)(mtiles * ntiles), NTHREADS, SMEM_BYTES, s>>>(tmA, tmB, g.C, g.ldc, g.M, g.N, (int)kp, f, (int)mtiles,
+                                                                                (int)ntiles, gm);
         LINAC_CUDA(cudaGetLastError());
         stats().kernel_launches += 3;
         stats().tc_launches++;

@@ -1,51 +1,90 @@
 // linac_common.cu -- library state, error plumbing, workspace, host number theory.
 #include <cstring>
 #include <mutex>
-#include <string>
 
 #include "linac_internal.h"
 
 namespace linac {
 
-static std::string g_cuda_error = "";
 static Options g_options;
-static linac_stats g_stats;
-static void* g_user_ws = nullptr;
-static size_t g_user_ws_bytes = 0;
-static void* g_own_ws = nullptr;
-static size_t g_own_ws_bytes = 0;
-std::mutex g_call_mutex;
+std::mutex g_init_mutex;                       // one-time initialisations, slot table, option writes
+static bool g_slot_used[FIELD_SLOTS] = {};
+
+Context& ctx() {
+    thread_local Context c;
+    return c;
+}
+
+Context::~Context() {
+    // the thread is leaving: give back what it owns (errors are ignored: the CUDA context may already be gone)
+    if (own_ws) cudaFree(own_ws);
+    if (mail) cudaFreeHost(mail);
+    for (cudaEvent_t e : events) if (e) cudaEventDestroy(e);
+    if (slot >= 0) {
+        std::lock_guard<std::mutex> lock(g_init_mutex);
+        g_slot_used[slot] = false;
+    }
+    cudaGetLastError();
+}
+
+int acquire_field_slot() {
+    Context& c = ctx();
+    if (c.slot >= 0) return c.slot;
+    std::lock_guard<std::mutex> lock(g_init_mutex);
+    for (int i = 0; i < FIELD_SLOTS; ++i)
+        if (!g_slot_used[i]) { g_slot_used[i] = true; c.slot = i; return i; }
+    return -1;                                 // more than FIELD_SLOTS threads inside the library at once
+}
+
+int current_device() {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -1;
+    return dev;
+}
+
+int sm_count() {
+    static int sms[64] = {};
+    const int dev = current_device();
+    if (dev < 0 || dev >= 64) return 0;
+    if (!sms[dev]) {
+        int v = 0;
+        cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
+        sms[dev] = v;                          // benign race: every thread writes the same value
+    }
+    return sms[dev];
+}
 
 void set_cuda_error(cudaError_t e, const char* what, const char* file, int line) {
-    char buf[1024];
-    snprintf(buf, sizeof buf, "%s (%s) at %s:%d: %s", cudaGetErrorName(e), cudaGetErrorString(e), file, line, what);
-    g_cuda_error = buf;
+    snprintf(ctx().cuda_error, sizeof ctx().cuda_error, "%s (%s) at %s:%d: %s", cudaGetErrorName(e), cudaGetErrorString(e),
+             file, line, what);
     cudaGetLastError();   // clear the sticky-less error so the next call starts clean
 }
 
 Options& options() { return g_options; }
-linac_stats& stats() { return g_stats; }
 
 int acquire_workspace(size_t bytes, Arena* arena) {
-    if (g_user_ws && g_user_ws_bytes >= bytes) {
-        arena->base = (char*)g_user_ws;
-        arena->size = g_user_ws_bytes;
+    Context& c = ctx();
+    if (c.user_ws && c.user_ws_bytes >= bytes) {
+        arena->base = (char*)c.user_ws;
+        arena->size = c.user_ws_bytes;
         arena->off = 0;
         return LINAC_OK;
     }
-    if (g_own_ws_bytes < bytes) {
-        if (g_own_ws) cudaFree(g_own_ws);
-        g_own_ws = nullptr;
-        g_own_ws_bytes = 0;
-        cudaError_t e = cudaMalloc(&g_own_ws, bytes);
+    const int dev = current_device();
+    if (c.own_ws_bytes < bytes || c.own_ws_dev != dev) {
+        if (c.own_ws) cudaFree(c.own_ws);
+        c.own_ws = nullptr;
+        c.own_ws_bytes = 0;
+        cudaError_t e = cudaMalloc(&c.own_ws, bytes);
         if (e != cudaSuccess) {
             set_cuda_error(e, "cudaMalloc(workspace)", __FILE__, __LINE__);
             return LINAC_ERR_WORKSPACE;
         }
-        g_own_ws_bytes = bytes;
+        c.own_ws_bytes = bytes;
+        c.own_ws_dev = dev;
     }
-    arena->base = (char*)g_own_ws;
-    arena->size = g_own_ws_bytes;
+    arena->base = (char*)c.own_ws;
+    arena->size = c.own_ws_bytes;
     arena->off = 0;
     return LINAC_OK;
 }
@@ -155,40 +194,40 @@ const char* linac_status_string(int status) {
     }
 }
 
-const char* linac_last_cuda_error(void) { return g_cuda_error.c_str(); }
+const char* linac_last_cuda_error(void) { return ctx().cuda_error; }
 
 int linac_version(void) { return 100; }   // 0.1.0
 
 int linac_set_workspace(void* dev_ptr, size_t bytes) {
-    std::lock_guard<std::mutex> lock(g_call_mutex);
     if ((dev_ptr == nullptr) != (bytes == 0)) return LINAC_ERR_INVALID_ARG;
-    g_user_ws = dev_ptr;
-    g_user_ws_bytes = bytes;
+    ctx().user_ws = dev_ptr;
+    ctx().user_ws_bytes = bytes;
     return LINAC_OK;
 }
 
 int linac_release(void) {
-    std::lock_guard<std::mutex> lock(g_call_mutex);
-    if (g_own_ws) cudaFree(g_own_ws);
-    g_own_ws = nullptr;
-    g_own_ws_bytes = 0;
+    Context& c = ctx();
+    if (c.own_ws) cudaFree(c.own_ws);
+    c.own_ws = nullptr;
+    c.own_ws_bytes = 0;
+    c.own_ws_dev = -1;
     return LINAC_OK;
 }
 
 int linac_get_last_stats(linac_stats* out) {
     if (!out) return LINAC_ERR_INVALID_ARG;
-    *out = g_stats;
+    *out = ctx().stats;
     return LINAC_OK;
 }
 
 int linac_set_option(const char* name, int64_t value) {
     if (!name) return LINAC_ERR_INVALID_ARG;
-    std::lock_guard<std::mutex> lock(g_call_mutex);
+    std::lock_guard<std::mutex> lock(g_init_mutex);
     if (!strcmp(name, "gemm_path")) {
         if (value < 0 || value > 2) return LINAC_ERR_INVALID_ARG;
         g_options.gemm_path = value;
     } else if (!strcmp(name, "timing")) {
-        if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
+        if (value < 0 || value > 2) return LINAC_ERR_INVALID_ARG;
         g_options.timing = value;
     } else if (!strcmp(name, "tc_min_k")) {
         if (value < 32) return LINAC_ERR_INVALID_ARG;

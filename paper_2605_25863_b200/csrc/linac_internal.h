@@ -4,6 +4,8 @@
 
 #include <cstdint>
 #include <cstdio>
+#include <mutex>
+#include <vector>
 
 #include "../../include/linac.h"
 #include "modp.cuh"
@@ -34,11 +36,13 @@ void set_cuda_error(cudaError_t e, const char* what, const char* file, int line)
         }                                                                    \
     } while (0)
 
-// Global, mutex-protected library state (workspace, options, stats).
+// Process-wide tunables (linac_set_option; set them while no call is in flight).
 struct Options {
     int64_t gemm_path = 0;    // 0 = auto, 1 = CUDA-core (SIMT) only, 2 = tensor (tcgen05) where legal
-    int64_t timing = 0;       // 1 = bracket update kernels with events (costs syncs; for profiling runs)
-    int64_t tc_min_k = 128;   // smallest K the tensor path is used for
+    int64_t timing = 0;       // 1 = event + host sync around every launch of the UN-fused schedule (A/B of kernel classes);
+                              // 2 = event pairs around every launch of the production schedule, no syncs, read at the end
+    int64_t tc_min_k = 48;    // smallest K the tensor path is used for (K is zero padded to 128: a strip that found fewer than 128
+                              // pivots -- free columns inside it -- must not fall to the CUDA-core kernel)
     int64_t tc_min_mn = 128;  // smallest M and N the tensor path is used for
     int64_t f64_mma = 1;      // fp64 trailing update: 1 = DMMA (FP64 tensor pipe), 0 = DFMA register tile
     int64_t f64_strip = 512;   // fp64 factorisation: flat sweep over strips of this many columns (0 = pure recursion)
@@ -53,7 +57,35 @@ struct Options {
     int64_t strip_width = 128; // columns factored by one cooperative strip kernel (multiple of 32, <= 256)
 };
 Options& options();
-linac_stats& stats();
+
+// Per-HOST-THREAD call state: the workspace handed over with linac_set_workspace, the library-owned fallback
+// workspace, the statistics of the thread's last call, its mapped mailbox, its timing events and its slot in the
+// constant-memory table of field descriptors.  Nothing a call mutates is shared between threads, so calls issued from
+// different host threads on different streams are independent ("re-entrant across streams when each
+// call has its own workspace").
+struct Context {
+    linac_stats stats{};
+    void* user_ws = nullptr; size_t user_ws_bytes = 0;
+    void* own_ws = nullptr;  size_t own_ws_bytes = 0; int own_ws_dev = -1;
+    unsigned long long* mail = nullptr;       // mapped pinned host memory (strip records), allocated on first use
+    unsigned long long seq = 0;               // tag of the last strip launch
+    std::vector<cudaEvent_t> events;          // pool for the timing modes
+    int slot = -1;                            // index into the __constant__ ModP table of fp_strip.cuh
+    char cuda_error[1024] = {0};
+    ~Context();
+};
+Context& ctx();
+inline linac_stats& stats() { return ctx().stats; }
+int acquire_field_slot();                      // a free slot of the constant table for this thread (kept until thread exit)
+constexpr int FIELD_SLOTS = 64;
+
+// One-time initialisation per (call site, device): function attributes are per device.
+struct PerDeviceOnce {
+    bool done[64] = {};
+    template <class Fn> int run(Fn&& fn);
+};
+int current_device();
+int sm_count();                                // multiprocessors of the current device (cached per device)
 
 // Workspace arena: bump allocation inside either the caller's buffer or a library-owned one.
 struct Arena {
@@ -68,13 +100,38 @@ struct Arena {
 };
 int acquire_workspace(size_t bytes, Arena* arena);   // returns linac_status
 
+extern std::mutex g_init_mutex;
+template <class Fn> int PerDeviceOnce::run(Fn&& fn) {
+    const int dev = current_device();
+    if (dev < 0 || dev >= 64) return LINAC_ERR_UNSUPPORTED_DEVICE;
+    std::lock_guard<std::mutex> lock(g_init_mutex);
+    if (!done[dev]) {
+        const int rc = fn();
+        if (rc) return rc;
+        done[dev] = true;
+    }
+    return LINAC_OK;
+}
+
+// Events of one call, destroyed on every exit path.
+struct CallEvents {
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr, t0 = nullptr, t1 = nullptr;
+    int create() {
+        LINAC_CUDA(cudaEventCreate(&ev0));
+        LINAC_CUDA(cudaEventCreate(&ev1));
+        LINAC_CUDA(cudaEventCreate(&t0));
+        LINAC_CUDA(cudaEventCreate(&t1));
+        return LINAC_OK;
+    }
+    ~CallEvents() {
+        for (cudaEvent_t e : {ev0, ev1, t0, t1}) if (e) cudaEventDestroy(e);
+    }
+};
+
 ModP make_modp(uint32_t p);
 bool is_prime_u32(uint32_t p);
 bool is_prime_u64(uint64_t p);                         // deterministic Miller-Rabin for every p < 2^64
-size_t wide_workspace_u32(int64_t rows, int64_t cols);
-// linac_rref_u32 for 2^31 <= p < 2^32 (fp_wide.cu); the caller holds the library mutex
-int rref_u32_wide(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, cudaStream_t s, int64_t* rank,
-                  int32_t* pivot_cols_out);
+
 int check_device();                                    // LINAC_OK or UNSUPPORTED_DEVICE / CUDA
 
 // ---- F_p GEMM  C -= Aop . B  (mod p) ------------------------------------------------------------
@@ -97,5 +154,10 @@ int gemm_modp_simt(const GemmArgs& g, const ModP& f, cudaStream_t s);
 // shape/alignment is not supported (caller falls back to the SIMT kernel).
 int gemm_modp_tc(const GemmArgs& g, const ModP& f, cudaStream_t s, Arena* scratch);
 size_t gemm_modp_tc_scratch_bytes(int64_t M, int64_t N, int64_t K);
+
+size_t wide_workspace_u32(int64_t rows, int64_t cols);
+// linac_rref_u32 for 2^31 <= p < 2^32 (fp_wide.cu); the caller holds the library mutex
+int rref_u32_wide(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, cudaStream_t s, int64_t* rank,
+                  int32_t* pivot_cols_out, Arena* arena);
 
 }  // namespace linac

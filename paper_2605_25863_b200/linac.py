@@ -24,7 +24,7 @@ SYMBOLS = [
     "linac_rref_u64_workspace", "linac_rref_u64",
     "linac_rref_u32", "linac_nullspace_u32", "linac_nullspace_from_rref_u32", "linac_solve_u32", "linac_rank_factor_u32", "linac_load_matrix_u32", "linac_gemm_sub_u32",
     "linac_solve_f64", "linac_rref_f64_workspace", "linac_rref_f64",
-    "linac_get_last_stats", "linac_set_option",
+    "linac_get_last_stats", "linac_set_option", "linac_measure_peak",
 ]
 
 
@@ -78,6 +78,7 @@ def _lib() -> C.CDLL:
         L.linac_solve_f64.argtypes = [vp, i64, i64, vp, i64, i64, C.c_double, vp, C.POINTER(i64)]
         L.linac_rref_f64_workspace.argtypes = [i64, i64, C.POINTER(sz)]
         L.linac_rref_f64.argtypes = [vp, i64, i64, i64, C.c_double, vp, C.POINTER(i64), vp]
+        L.linac_measure_peak.argtypes = [C.c_char_p, C.c_double, vp, sz, vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.linac_get_last_stats.argtypes = [C.POINTER(Stats)]
         L.linac_set_option.argtypes = [C.c_char_p, i64]
         _LIB = L
@@ -100,28 +101,29 @@ def last_stats() -> dict:
     return s.as_dict()
 
 
-_ws_tensor = None
+import threading
+
+_tls = threading.local()      # the library keeps its workspace binding per host thread; so does this binding
 
 
 def _ensure_workspace(nbytes: int, device) -> None:
-    """Workspace is a torch allocation handed to the library (the caller owns device memory)."""
-    global _ws_tensor
+    """Workspace is a torch allocation handed to the library (the caller owns device memory); one per Python thread."""
     if nbytes == 0:
         return
-    if _ws_tensor is None or _ws_tensor.numel() < nbytes or _ws_tensor.device != device:
+    ws = getattr(_tls, "ws", None)
+    if ws is None or ws.numel() < nbytes or ws.device != device:
         _lib().linac_set_workspace(None, 0)
-        _ws_tensor = None
-        _ws_tensor = torch.empty(nbytes, dtype=torch.uint8, device=device)
-        rc = _lib().linac_set_workspace(_ws_tensor.data_ptr(), _ws_tensor.numel())
+        _tls.ws = None
+        _tls.ws = torch.empty(nbytes, dtype=torch.uint8, device=device)
+        rc = _lib().linac_set_workspace(_tls.ws.data_ptr(), _tls.ws.numel())
         if rc:
             raise LinacError(rc, "linac_set_workspace")
 
 
 def release_workspace() -> None:
-    global _ws_tensor
     _lib().linac_set_workspace(None, 0)
     _lib().linac_release()
-    _ws_tensor = None
+    _tls.ws = None
 
 
 def _check_matrix(t: torch.Tensor, dtypes, what: str):
@@ -349,3 +351,16 @@ def rref_f64(a: torch.Tensor, tol: float = -1.0):
     if rc:
         raise LinacError(rc, "linac_rref_f64")
     return int(rank.value), piv[: rank.value].clone()
+
+
+def measure_peak(what: str, ms_target: float = 2.0, scratch: torch.Tensor | None = None):
+    """Microbenchmark of one pipe (mirrors linac_measure_peak).  Returns (value, sm_mhz)."""
+    dev = scratch.device if scratch is not None else torch.device("cuda", torch.cuda.current_device())
+    with torch.cuda.device(dev):
+        val, mhz = C.c_double(0), C.c_double(0)
+        rc = _lib().linac_measure_peak(what.encode(), float(ms_target), scratch.data_ptr() if scratch is not None else None,
+                                       scratch.numel() * scratch.element_size() if scratch is not None else 0,
+                                       _stream_ptr(dev), C.byref(val), C.byref(mhz))
+    if rc:
+        raise LinacError(rc, f"linac_measure_peak({what})")
+    return float(val.value), float(mhz.value)
