@@ -566,12 +566,15 @@ def main():
                     help="comma list of the extra legs of the default run")
     ap.add_argument("--ref-n", type=int, default=1280, help="sample size for --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--cpu-baseline", default="bounded", choices=["bounded", "full"])
     ap.add_argument("--no-f64", action="store_true", help="skip the fp64 legs")
     ap.add_argument("--fp64-only", action="store_true", help="run only legs.fp64_solve and print {\"fp64\": ...}")
     ap.add_argument("--gemm", default=None, metavar="M,N,K[,path]",
                     help="time the S5 primitive linac_gemm_sub_u32 alone (C -= A.B mod 2^31-1, path 2 = tensor cores by default) "
                          "and print {\"gemm\": ...}; the command of the GEMM ncu captures under profiles/")
+    ap.add_argument("--load-matrix", default=None, metavar="ROWS,COLS,D",
+                    help="time linac_load_matrix_u32 alone (SURVEY.md 8(f)#2) and print {\"load_matrix\": ...}")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
                     help="library tunable for A/B runs (linac_set_option), e.g. --opt strip_width=256")
     args = ap.parse_args()
@@ -618,6 +621,32 @@ def main():
                                    "peak_burst": peak["peak_burst"], "peak_sustained": peak["peak_sustained"],
                                    "note": "event time of the whole call incl. the limb-split pre-passes"}}))
         return
+    if args.load_matrix:
+        rows, cols, d = (int(x) for x in args.load_matrix.split(","))
+        p, nb = 2147483647, 64
+        from linac_inputs import gen_torch
+        bases = gen_torch.uniform_rows(0, rows, nb, p, 11, dev)
+        lind = (gen_torch.uniform_rows(0, cols, d, nb, 12, dev)).to(torch.int32).contiguous()
+        out_t = torch.empty((rows, cols), dtype=torch.int32, device=dev)
+        stream = torch.cuda.current_stream(dev)
+        times = []
+        for i in range(args.warmup + min(args.steps, 5)):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            L.load_matrix_u32(bases, lind, p, out=out_t)
+            e1.record(stream)
+            e1.synchronize()
+            if i >= args.warmup:
+                times.append(e0.elapsed_time(e1))
+        ms = float(np.mean(times))
+        imad, mhz = B.peak("imad_wide", 20.0)
+        print(json.dumps({"load_matrix": {"rows": rows, "cols": cols, "d": d, "n_basis": nb, "ms": ms,
+                                          "gb_per_s_written": rows * cols * 4 / (ms * 1e-3) / 1e9,
+                                          "field_products_per_s_T": rows * cols * d / (ms * 1e-3) / 1e12,
+                                          "imad_wide_peak_T": imad, "hbm_peak_gbs": B.peaks_file["hbm_gbs"],
+                                          "note": "d Montgomery products (IMAD.WIDE + IMAD + IMAD.WIDE each) per 4-byte element: "
+                                                  "ALU-bound, not HBM-bound, for d >= 2"}}))
+        return
     if args.fp64_only:
         if rank == 0:
             print(json.dumps({"fp64": B.f64_solve_leg(reps=max(1, min(args.steps, 5)))}))
@@ -628,7 +657,7 @@ def main():
         h = B.fp_leg("c5", steps=min(args.steps, 2), warmup=min(args.warmup, 1))
         args.steps, args.warmup = h["steps"], h["warmup"]
     else:
-        h = B.fp_leg(headline, steps=args.steps, warmup=args.warmup, with_e2e=True, nullspace=(headline == "c2"))
+        h = B.fp_leg(headline, steps=args.steps, warmup=args.warmup, with_e2e=not args.no_e2e, nullspace=(headline == "c2"))
     out = {
         "metric": "rref_gmulmod_per_s", "value": h["value"], "unit": "Gmulmod/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": h["ms_per_step"], "higher_is_better": True, "scaling": "weak",

@@ -734,11 +734,24 @@ constexpr int TLR = SW_MAX - PW;                       // most rows an L block c
 constexpr int TNL = (TLR * PW + TNT - 1) / TNT;        // prefetch registers per thread for one L block
 
 __host__ __device__ inline size_t trsm_smem_bytes(int64_t K) {
-    return (size_t)K * PW * 4 + (size_t)PW * (PW + 1) * 4 + (size_t)TLR * TLS * 4;
+    return (size_t)K * PW * 4 + (size_t)PW * TLS * 4 + (size_t)TLR * TLS * 4;
+}
+
+// sum_k row[k] * x[k] over a full 32-pivot panel: the row (16-byte aligned in shared memory) by LDS.128, the column of
+// X from registers, one fold per two products (fold64 keeps the accumulator below 2^63 + 2^32).
+__device__ __forceinline__ uint64_t dot32_pair(const uint32_t* __restrict__ row, const uint32_t (&x)[PW], const ModP& f) {
+    uint64_t acc = 0;
+#pragma unroll
+    for (int k = 0; k < PW; k += 4) {
+        const uint4 v = *reinterpret_cast<const uint4*>(row + k);
+        acc = fold64(acc + (uint64_t)v.x * x[k] + (uint64_t)v.y * x[k + 1], f);
+        acc = fold64(acc + (uint64_t)v.z * x[k + 2] + (uint64_t)v.w * x[k + 3], f);
+    }
+    return acc;
 }
 
 template <bool LOWER>
-__global__ void __launch_bounds__(TNT) trsm_strip_kernel(const uint32_t* __restrict__ A, int64_t ld,
+__global__ void __launch_bounds__(TNT, 2) trsm_strip_kernel(const uint32_t* __restrict__ A, int64_t ld,
                                                          uint32_t* __restrict__ X, int64_t ldx, int64_t ncols,
                                                          const int32_t* __restrict__ pstart, int bs0, int bs1,
                                                          const uint32_t* __restrict__ T,
@@ -750,8 +763,8 @@ __global__ void __launch_bounds__(TNT) trsm_strip_kernel(const uint32_t* __restr
     if (host_mail != nullptr && blockIdx.x == 0) mail_records(host_mail, seq, rec + bs0, bs1 - bs0);
     const int t0 = pstart[bs0], K = pstart[bs1] - t0;
     uint32_t (*Xs)[PW] = reinterpret_cast<uint32_t (*)[PW]>(trsm_smem_raw);                                 // [K][32]
-    uint32_t (*Ts)[PW + 1] = reinterpret_cast<uint32_t (*)[PW + 1]>(trsm_smem_raw + (size_t)K * PW * 4);     // [32][33]
-    uint32_t (*Lp)[TLS] = reinterpret_cast<uint32_t (*)[TLS]>(trsm_smem_raw + (size_t)K * PW * 4 + PW * (PW + 1) * 4);
+    uint32_t (*Ts)[TLS] = reinterpret_cast<uint32_t (*)[TLS]>(trsm_smem_raw + (size_t)K * PW * 4);           // [32][36]
+    uint32_t (*Lp)[TLS] = reinterpret_cast<uint32_t (*)[TLS]>(trsm_smem_raw + (size_t)K * PW * 4 + PW * TLS * 4);
     const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
     constexpr int NW = TNT / 32;
     const int64_t c = (int64_t)blockIdx.x * PW + lane;
@@ -801,6 +814,35 @@ __global__ void __launch_bounds__(TNT) trsm_strip_kernel(const uint32_t* __restr
         __syncthreads();
         nxt = ii + 1;
         prefetch();
+        if (r == PW) {
+            // Full panel (the common case): the 32 entries of this thread's column of X_b live in registers for the whole
+            // panel, rows of T / L come in by LDS.128, everything is unrolled -- about 2.5 instructions per multiply-
+            // accumulate against 10 in the general loops below (run-time r, scalar shared-memory operands).
+            uint32_t x[PW];
+            if (LOWER) {
+#pragma unroll
+                for (int k = 0; k < PW; ++k) x[k] = Xs[s + k][lane];
+                const uint32_t y0 = reduce64(dot32_pair(Ts[wq], x, f), f);
+                const uint32_t y1 = reduce64(dot32_pair(Ts[wq + NW], x, f), f);
+                __syncthreads();
+                Xs[s + wq][lane] = y0;
+                Xs[s + wq + NW][lane] = y1;
+                __syncthreads();
+            }
+            if (nrow > 0) {
+#pragma unroll
+                for (int k = 0; k < PW; ++k) x[k] = Xs[s + k][lane];
+                for (int row = wq; row < nrow; row += 2 * NW) {
+                    const bool two = row + NW < nrow;
+                    const uint64_t a0 = dot32_pair(Lp[row], x, f);
+                    const uint64_t a1 = dot32_pair(Lp[two ? row + NW : row], x, f);
+                    Xs[lo + row][lane] = submod(Xs[lo + row][lane], reduce64(a0, f), f);
+                    if (two) Xs[lo + row + NW][lane] = submod(Xs[lo + row + NW][lane], reduce64(a1, f), f);
+                }
+            }
+            __syncthreads();
+            continue;
+        }
         if (LOWER) {
             // two outputs per thread (rows wq and wq + 16 of T) share the X loads
             static_assert(PW / NW == 2, "the T product below is written for two rows per warp");

@@ -168,7 +168,7 @@ def test_schedule_options_do_not_change_the_result(oracle, opts):
     is unique, so the bytes must not move.  One rank-deficient and one full-rank wide matrix."""
     import paper_2605_25863_b200 as L
     defaults = {"strip_width": 128, "flat_group": 1, "flat_cols": 16384, "tc_panel": 1, "gemm_path": 0,
-                "tc_min_k": 128, "tc_min_mn": 128}
+                "tc_min_k": 48, "tc_min_mn": 128}
     a1, _, _ = gen.lowrank_factors(700, 333, 900, P29, seed_b=21, seed_c=22)
     a2 = gen.uniform_matrix(600, 1100, P31, seed=23)
     try:
