@@ -359,7 +359,7 @@ size_t workspace_bytes(int64_t rows, int64_t cols) {
     const int64_t mn = std::max<int64_t>(1, std::min(rows, cols));
     size_t b = meta_bytes(rows, cols);
     b += (size_t)mn * (size_t)backelim_slab(rows, cols) * 4 + 2 * (size_t)backelim_slab(rows, cols) * 4 + 1024;   // gathered free columns
-    b += gemm_modp_tc_scratch_bytes(rows, cols, std::min<int64_t>(mn, 4096)) + 256;
+    b += gemm_modp_tc_scratch_bytes(rows, cols, std::min<int64_t>(mn, 8192)) + 256;
     return b;
 }
 

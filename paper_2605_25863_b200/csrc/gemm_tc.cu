@@ -41,7 +41,7 @@ constexpr int B_STAGE = 4 * TN * KB;      // 32768
 constexpr int SMEM_BYTES = STAGES * (A_STAGE + B_STAGE) + 1024 /*align*/ + 256 /*barriers*/;
 constexpr int TMEM_COLS = 512;
 constexpr int NTHREADS = 192;    // warp 0: TMA, warp 1: MMA + TMEM alloc, warps 2..5: epilogue
-constexpr int64_t KC_MAX = 4096;
+constexpr int64_t KC_MAX = 8192;     // K per launch (multiple of 128; the s32 accumulators hold K <= 8256, see the header)
 
 // ----------------------------------------------------------------------------- the GEMM kernel
 __global__ void __launch_bounds__(NTHREADS, 1)

@@ -34,6 +34,7 @@ def expected(oracle, c, a, b, p):
 SHAPES = [(1, 1, 1), (5, 7, 3), (128, 64, 16), (129, 65, 17), (200, 300, 100), (257, 130, 33)]
 TC_SHAPES = [(128, 64, 128), (128, 64, 32), (256, 128, 256), (300, 200, 150), (512, 512, 512), (1000, 900, 700),
              (640, 576, 4224), (130, 70, 1),
+             (256, 192, 9000),      # K > 8192: two chunks per call (the s32 accumulators hold K <= 8256)
              # K <= 256: the persistent A-stationary panel kernel (several items per CTA, ragged M and N tiles)
              (1000, 2100, 256), (3000, 1500, 128), (5000, 40, 200), (20000, 100, 256)]
 
@@ -53,8 +54,8 @@ def test_simt_kernel(oracle, m, n, k, p):
 @pytest.mark.parametrize("m,n,k", TC_SHAPES)
 @pytest.mark.parametrize("p", [P31, P29, 7])
 def test_tensor_core_kernel(oracle, m, n, k, p):
-    if (m, n, k) == (640, 576, 4224) and p != P31:
-        pytest.skip("one modulus is enough at the largest shape")
+    if (m, n, k) in ((640, 576, 4224), (256, 192, 9000)) and p != P31:
+        pytest.skip("one modulus is enough at the largest shapes")
     a = gen.uniform_matrix(m, k, p, seed=1)
     b = gen.uniform_matrix(k, n, p, seed=2)
     c = gen.uniform_matrix(m, n, p, seed=3)
@@ -64,8 +65,8 @@ def test_tensor_core_kernel(oracle, m, n, k, p):
 
 
 def test_tensor_core_worst_case_operands(oracle):
-    """All entries p-1: every limb product at its maximum, K = 4096 in one launch (s32 accumulator headroom)."""
-    m, n, k = 128, 64, 4096
+    """All entries p-1: every limb product at its maximum, K = 8192 in one launch (s32 accumulator headroom)."""
+    m, n, k = 128, 64, 8192
     a = np.full((m, k), P31 - 1, dtype=np.uint32)
     b = np.full((k, n), P31 - 1, dtype=np.uint32)
     c = np.zeros((m, n), dtype=np.uint32)
