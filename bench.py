@@ -227,14 +227,22 @@ class Bench:
             self._peak_cache[key] = self.L.measure_peak(what, ms)
         return self._peak_cache[key]
 
-    def tensor_peak(self, clocks):
+    def tensor_peak(self, clocks, hot=False):
         """The int8 tensor peak for a run with these clocks: the 2 ms burst figure if the run sat near the maximum clock
-        with no power cap, else the 400 ms power-capped one (both measured live, random operand bytes)."""
+        with no power cap, else a power-capped one (both measured live, random operand bytes).  hot=True: the leg has just
+        run under the power cap, so the sustained figure is taken NOW, in the same thermal / power state, over one second
+        (the pipe itself delivers 3.2-3.4 PTOP/s right after a long dense run against 3.8-3.9 from an idle board)."""
         burst, mhz_b = self.peak("tc_i8_n256", 2.0)
-        sust, mhz_s = self.peak("tc_i8_n256", 400.0)
         capped = "sw_power_cap" in (clocks.get("reasons") or []) or (
             clocks.get("sm_mhz") and clocks.get("sm_max_mhz") and clocks["sm_mhz"] < 0.93 * clocks["sm_max_mhz"])
-        use, mhz, kind = (sust, mhz_s, "sustained (400 ms)") if capped else (burst, mhz_b, "burst (2 ms)")
+        if capped and hot:
+            sust, mhz_s = self.L.measure_peak("tc_i8_n256", 1000.0)
+            self._peak_cache[("tc_i8_n256 (hot, right after the leg)", 1000.0)] = (sust, mhz_s)
+            skind = "sustained (1 s, measured right after the leg in the same power state)"
+        else:
+            sust, mhz_s = self.peak("tc_i8_n256", 400.0)
+            skind = "sustained (400 ms)"
+        use, mhz, kind = (sust, mhz_s, skind) if capped else (burst, mhz_b, "burst (2 ms)")
         return {"peak": use, "peak_kind": kind, "peak_sm_mhz": mhz,
                 "peak_source": "measured live by linac_measure_peak('tc_i8_n256'): tcgen05.mma kind::i8 128x256x32 from "
                                "on-chip pseudo-random operands",
@@ -298,6 +306,7 @@ class Bench:
         self.barrier()
         clocks = sampler.stop()
         stats = L.last_stats()
+        peak_info = self.tensor_peak(clocks, hot=True)          # right after the timed steps (same power state)
         total_ms = replicas.max_over_ranks(float(sum(times)), dev)
         ms_per_step = total_ms / steps
         value = replicas.aggregate_throughput(nominal, ms_per_step * 1e-3, self.world) / 1e9
@@ -320,7 +329,7 @@ class Bench:
         roof = {"bound": "tensor", "unit": "TOP/s (int8, 2 ops per u8 multiply-accumulate, 16 per field multiply-accumulate)",
                 "kernel": "Schur-update GEMMs on tcgen05 kind::i8 (gemm_tc_panel_kernel for K <= 256, gemm_tc_kernel above; "
                           "the CUDA-core kernel only for shapes below 128)"}
-        roof.update(self.tensor_peak(clocks))
+        roof.update(peak_info)
         if st_t.get("tc_launches", 0) and ms_upd > 0:
             ach = macs * 32.0 / (ms_upd * 1e-3) / 1e12
             roof.update({"achieved": ach, "frac": ach / roof["peak"]})

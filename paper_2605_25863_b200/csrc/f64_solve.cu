@@ -29,25 +29,68 @@ constexpr int FW = 32;              // panel width
 
 // ---------------------------------------------------------------- F1
 // One block per row: s = max_c |A[r,c]| over A's columns (reading Q11), then A[r,:] /= s, B[r,:] /= s.
-__global__ void __launch_bounds__(256) row_scale_kernel(double* __restrict__ A, int64_t n, int64_t lda,
-                                                        double* __restrict__ B, int64_t nrhs, int64_t ldb,
-                                                        int* __restrict__ info) {
-    __shared__ double red[8];
+// The row is kept in shared memory between the two passes when it fits (n <= 24576 doubles), so the matrix is read
+// once and written once: 16 B per element, the algorithmic minimum (the first version read it twice: 24 B).
+constexpr int RS_THREADS = 512;
+__global__ void __launch_bounds__(RS_THREADS) row_scale_kernel(double* __restrict__ A, int64_t n, int64_t lda,
+                                                               double* __restrict__ B, int64_t nrhs, int64_t ldb,
+                                                               int* __restrict__ info, int cache_n) {
+    extern __shared__ __align__(16) double rs_row[];
+    __shared__ double red[RS_THREADS / 32];
     const int64_t r = blockIdx.x;
     double* row = A + r * lda;
+    const bool vec = ((reinterpret_cast<uintptr_t>(row) & 15) == 0) && (n % 2 == 0);
     double m = 0.0;
-    for (int64_t c = threadIdx.x; c < n; c += blockDim.x) m = fmax(m, fabs(row[c]));
+    if (vec) {
+        const double2* row2 = reinterpret_cast<const double2*>(row);
+        for (int64_t c = threadIdx.x; c < n / 2; c += blockDim.x) {
+            const double2 v = row2[c];
+            if (2 * c + 1 < cache_n) reinterpret_cast<double2*>(rs_row)[c] = v;
+            m = fmax(m, fmax(fabs(v.x), fabs(v.y)));
+        }
+    } else {
+        for (int64_t c = threadIdx.x; c < n; c += blockDim.x) {
+            const double v = row[c];
+            if (c < cache_n) rs_row[c] = v;
+            m = fmax(m, fabs(v));
+        }
+    }
     for (int o = 16; o; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
     if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
     __syncthreads();
     m = red[0];
-    for (int w = 1; w < 8; ++w) m = fmax(m, red[w]);
+    for (int w = 1; w < RS_THREADS / 32; ++w) m = fmax(m, red[w]);
     if (m == 0.0) {
         if (threadIdx.x == 0) atomicMin(info, 1);      // a zero row: singular at the very first column
         return;
     }
-    for (int64_t c = threadIdx.x; c < n; c += blockDim.x) row[c] = row[c] / m;
+    if (vec) {
+        double2* row2 = reinterpret_cast<double2*>(row);
+        for (int64_t c = threadIdx.x; c < n / 2; c += blockDim.x) {
+            double2 v = 2 * c + 1 < cache_n ? reinterpret_cast<const double2*>(rs_row)[c] : row2[c];
+            v.x = v.x / m;
+            v.y = v.y / m;
+            row2[c] = v;
+        }
+    } else {
+        for (int64_t c = threadIdx.x; c < n; c += blockDim.x) row[c] = (c < cache_n ? rs_row[c] : row[c]) / m;
+    }
     for (int64_t c = threadIdx.x; c < nrhs; c += blockDim.x) B[r * ldb + c] = B[r * ldb + c] / m;
+}
+
+// Launch helper: the row cache takes what is left of one SM's shared memory for two resident CTAs.
+int launch_row_scale(double* A, int64_t rows, int64_t n, int64_t lda, double* B, int64_t nrhs, int64_t ldb, int* info,
+                     cudaStream_t s) {
+    static PerDeviceOnce once;
+    const int rc = once.run([]() -> int {
+        LINAC_CUDA(cudaFuncSetAttribute(row_scale_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+        return LINAC_OK;
+    });
+    if (rc) return rc;
+    const int cache_n = (int)std::min<int64_t>(n / 2 * 2, 100 * 1024 / 8);
+    row_scale_kernel<<<(unsigned)rows, RS_THREADS, (size_t)cache_n * 8, s>>>(A, n, lda, B, nrhs, ldb, info, cache_n);
+    LINAC_CUDA(cudaGetLastError());
+    return LINAC_OK;
 }
 
 // ---------------------------------------------------------------- F2 panel
@@ -1140,8 +1183,8 @@ int linac_solve_f64(double* dA, int64_t n, int64_t lda, double* dB, int64_t nrhs
     if (rc) return rc;
     cudaEvent_t e0 = evs.ev0, e1 = evs.ev1;
     cudaEventRecord(e0, s);
-    row_scale_kernel<<<(unsigned)n, 256, 0, s>>>(dA, n, lda, dB, nrhs, ldb, c.info);          // F1
-    LINAC_CUDA(cudaGetLastError());
+    rc = launch_row_scale(dA, n, n, lda, dB, nrhs, ldb, c.info, s);                            // F1
+    if (rc) return rc;
     st.kernel_launches++;
     // F2 with B as trailing columns: factor A in outer blocks so B's forward substitution is blocked too
     rc = factor_flat_f64(c);
@@ -1221,8 +1264,8 @@ int linac_rref_f64(double* dA, int64_t rows, int64_t cols, int64_t ld, double to
     LINAC_CUDA(cudaMemsetAsync(state, 0, 256, s));
     LINAC_CUDA(cudaMemsetAsync(cand, 0, 2 * 1024 * sizeof(Cand), s));
     LINAC_CUDA(cudaMemsetAsync(target, 0, 2 * FW * sizeof(double2), s));
-    row_scale_kernel<<<(unsigned)rows, 256, 0, s>>>(dA, cols, ld, nullptr, 0, 0, dummy_info);        // K1/K2; zero rows stay zero
-    LINAC_CUDA(cudaGetLastError());
+    rc = launch_row_scale(dA, rows, cols, ld, nullptr, 0, 0, dummy_info, s);                         // K1/K2; zero rows stay zero
+    if (rc) return rc;
     st.kernel_launches++;
     const size_t smem = (size_t)rows_per_cta * (FW + 2) * sizeof(double);
     double tolv = c.tol;
