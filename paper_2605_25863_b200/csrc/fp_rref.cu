@@ -47,22 +47,23 @@ struct Fp {
     // timing == 2: the PRODUCTION schedule with an event pair around every launch and no host synchronisation; the
     // pairs are read after the call's final sync (class 0 = Schur update, 1 = strip kernel, 2 = triangular solve)
     std::vector<cudaEvent_t>* pool = nullptr;
-    struct Mark { int cls; int ev; int64_t m, n, k; };
+    struct Mark { int cls; int ev; int64_t m, n, k; cudaStream_t on; };
     std::vector<Mark> marks;
     int pool_used = 0;
-    int mark_begin(int cls, int64_t m = 0, int64_t n = 0, int64_t k = 0) {
+    int mark_begin(int cls, int64_t m = 0, int64_t n = 0, int64_t k = 0, cudaStream_t on = nullptr) {
         if (options().timing != 2 || !pool) return -1;
+        if (!on) on = s;
         if (pool_used + 2 > (int)pool->size()) {
             const size_t old = pool->size();
             pool->resize(old + 512, nullptr);
             for (size_t i = old; i < pool->size(); ++i) cudaEventCreate(&(*pool)[i]);
         }
-        marks.push_back({cls, pool_used, m, n, k});
-        cudaEventRecord((*pool)[pool_used], s);
+        marks.push_back({cls, pool_used, m, n, k, on});
+        cudaEventRecord((*pool)[pool_used], on);
         pool_used += 2;
         return (int)marks.size() - 1;
     }
-    void mark_end(int h) { if (h >= 0) cudaEventRecord((*pool)[marks[h].ev + 1], s); }
+    void mark_end(int h) { if (h >= 0) cudaEventRecord((*pool)[marks[h].ev + 1], marks[h].on); }
 
     int64_t sb0(int64_t s) const { return std::min(nb, s * bps); }          // first base panel of strip s
     int64_t sp(int64_t s) const { return pstart[sb0(s)]; }                  // pivots found left of strip s
@@ -102,7 +103,8 @@ int run_gemm(Fp& c, const GemmArgs& g) {
 // Brackets one kernel class with events when the "timing" option is on (costs a host sync per launch).
 struct Timed {
     Fp& c; double& acc; bool on; int mk;
-    Timed(Fp& c_, double& acc_, int cls) : c(c_), acc(acc_), on(options().timing == 1), mk(c_.mark_begin(cls)) {
+    Timed(Fp& c_, double& acc_, int cls, cudaStream_t stream = nullptr)
+        : c(c_), acc(acc_), on(options().timing == 1), mk(c_.mark_begin(cls, 0, 0, 0, stream)) {
         if (on) cudaEventRecord(c.ev0, c.s);
     }
     ~Timed() {
@@ -124,7 +126,8 @@ int trsm_leaf(Fp& c, int64_t s, uint32_t* X, int64_t ldx, int64_t ncols) {
     if (!LOWER && c.sb0(s + 1) - c.sb0(s) <= 1) return LINAC_OK;     // U is the identity inside one base panel
     Timed tm(c, stats().ms_trsm, 2);
     trsm_strip_kernel<LOWER><<<(unsigned)((ncols + PW - 1) / PW), TNT, trsm_smem_bytes(K), c.s>>>(
-        c.A, c.ld, X, ldx, ncols, c.d_pstart, (int)c.sb0(s), (int)c.sb0(s + 1), c.d_T, c.d_pivcols, c.f, nullptr, 0, nullptr, 0, nullptr);
+        c.A, c.ld, X, ldx, ncols, c.d_pstart, (int)c.sb0(s), (int)c.sb0(s + 1), c.d_T, c.d_pivcols, c.f, nullptr, 0, nullptr, 0, nullptr,
+        0, 0);
     LINAC_CUDA(cudaGetLastError());
     stats().kernel_launches++;
     stats().update_macs += K * K / 2 * ncols;
@@ -149,63 +152,68 @@ int trsm_lower(Fp& c, int64_t s0, int64_t s1, int64_t c0, int64_t c1) {
     return trsm_lower(c, sh, s1, c0, c1);
 }
 
-// One strip s with active rows >= i0 (one cooperative launch).  Returns the number of pivots through *r.
-// If early_ncols > 0 the strip's row-block solve on columns [early_c0, early_c0 + early_ncols) is enqueued right
-// behind the strip kernel (it takes the pivot counts from device memory), and the host reads the pivot counts
-// through a second stream meanwhile: the round trip then hides under the solve instead of idling the GPU.
-int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r, int64_t early_c0 = 0, int64_t early_ncols = 0,
-                 uint8_t* early_Bq = nullptr, int early_kp = 0, uint8_t* tail_Aq = nullptr) {
+int factor(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t* r_out, bool allow_flat);
+
+// A strip kernel in flight: what collect_strip needs to read its mail.
+struct StripLaunch {
+    unsigned long long seq = 0;
+    int64_t b0 = 0, b1 = 0, j0 = 0, j1 = 0;
+    cudaStream_t stream = nullptr;
+};
+
+// Launches the cooperative strip kernel for strip s (active rows >= i0) on `stream` with `grid` CTAs.
+//   self_mail  the kernel posts its records to the host mailbox itself (otherwise the solve kernel behind it does)
+//   la         look-ahead launch: row exchanges are applied to the strip's own columns only (deferred_swaps_kernel
+//              applies the rest once the previous strip's bulk update has finished with those rows)
+int launch_strip(Fp& c, int64_t s, int64_t i0, cudaStream_t stream, int grid, bool la, bool self_mail, uint8_t* tail_Aq,
+                 int kp, StripLaunch* out) {
     const int64_t b0 = c.sb0(s), b1 = c.sb0(s + 1);
     const int64_t j0 = panel_col0(b0), j1 = std::min(c.cols, panel_col0(b1));
     StripArgs a;
     a.A = c.A; a.ld = c.ld; a.rows = c.rows; a.cols = c.cols; a.i0 = i0; a.j0 = j0; a.ws = (int)(j1 - j0);
     a.rec = c.d_rec; a.T = c.d_T; a.E = c.d_E; a.pivcols = c.d_pivcols; a.pstart = c.d_pstart;
-    a.Aq = tail_Aq; a.kp = early_kp;
+    a.Aq = tail_Aq; a.kp = kp;
     a.slot = c.slot;
+    a.swap_c0 = la ? j0 : 0;
+    a.swap_c1 = la ? j1 : c.cols;
     a.seq = (++ctx().seq) & 0xFFFFFFFFull;
     if (a.seq == 0) a.seq = ++ctx().seq & 0xFFFFFFFFull;        // 0 is the mailbox's initial content
-    const bool early = early_ncols > 0 && options().timing != 1;
-    a.host_mail = early ? nullptr : c.h_mail;                    // with an early solve, the solve kernel mails
+    a.host_mail = self_mail ? c.h_mail : nullptr;
     void* args[] = {&a};
     {
-        Timed tm(c, stats().ms_strip, 1);
-        LINAC_CUDA(cudaLaunchCooperativeKernel((void*)strip_factor_kernel, dim3((unsigned)c.coop_grid), dim3(SNT), args,
-                                               sizeof(StripSmem), c.s));
+        Timed tm(c, stats().ms_strip, 1, stream);
+        LINAC_CUDA(cudaLaunchCooperativeKernel((void*)strip_factor_kernel, dim3((unsigned)grid), dim3(SNT), args, sizeof(StripSmem),
+                                               stream));
     }
+    stats().kernel_launches++;
+    out->seq = a.seq; out->b0 = b0; out->b1 = b1; out->j0 = j0; out->j1 = j1; out->stream = stream;
+    return LINAC_OK;
+}
+
+// Waits for the mail of a launched strip (it may arrive before the kernel has ended) and records its pivots.
+int collect_strip(Fp& c, const StripLaunch& L, int64_t i0, int64_t* r) {
     linac_stats& st = stats();
-    if (early) {
-        Timed tm(c, stats().ms_trsm, 2);
-        trsm_strip_kernel<true><<<(unsigned)((early_ncols + PW - 1) / PW), TNT, trsm_smem_bytes(j1 - j0), c.s>>>(
-            c.A, c.ld, c.A + i0 * c.ld + early_c0, c.ld, early_ncols, c.d_pstart, (int)b0, (int)b1, c.d_T, c.d_pivcols, c.f,
-            early_Bq, early_kp, c.h_mail, a.seq, c.d_rec);
-        LINAC_CUDA(cudaGetLastError());
-        st.kernel_launches++;
-    } else {
-        early_ncols = 0;
-    }
-    // Wait for the strip kernel's mail (it may arrive before the kernel, let alone the solve behind it, has ended).
     {
         volatile unsigned long long* mailbox = c.h_mail;
-        const int nw = (int)(b1 - b0) * MAIL_WORDS;
+        const int nw = (int)(L.b1 - L.b0) * MAIL_WORDS;
         int seen = 0;                                     // words [0, seen) already carry this launch's tag
         for (uint64_t spins = 0; seen < nw; ++spins) {
-            while (seen < nw && (mailbox[seen] >> 32) == a.seq) ++seen;
+            while (seen < nw && (mailbox[seen] >> 32) == L.seq) ++seen;
             if (seen < nw && (spins & 0x3FFF) == 0x3FFF) {
-                const cudaError_t q = cudaStreamQuery(c.s);
+                const cudaError_t q = cudaStreamQuery(L.stream);
                 if (q != cudaSuccess && q != cudaErrorNotReady) { set_cuda_error(q, "strip kernel", __FILE__, __LINE__); return LINAC_ERR_CUDA; }
                 if (q == cudaSuccess) {                   // stream drained: the mail must be complete by now
-                    while (seen < nw && (mailbox[seen] >> 32) == a.seq) ++seen;
+                    while (seen < nw && (mailbox[seen] >> 32) == L.seq) ++seen;
                     if (seen < nw) return LINAC_ERR_INTERNAL;
                 }
             }
         }
         std::atomic_thread_fence(std::memory_order_acquire);
     }
-    st.kernel_launches++;
     st.host_syncs++;
     int64_t cur = i0;
-    for (int64_t b = b0; b < b1; ++b) {
-        const unsigned long long* m = c.h_mail + (b - b0) * MAIL_WORDS;
+    for (int64_t b = L.b0; b < L.b1; ++b) {
+        const unsigned long long* m = c.h_mail + (b - L.b0) * MAIL_WORDS;
         const int32_t hr = (int32_t)(uint32_t)m[0], hns = (int32_t)(uint32_t)m[1];
         if (hr < 0 || hr > PW || cur + hr > c.rows) return LINAC_ERR_INTERNAL;
         st.panels++;
@@ -215,12 +223,198 @@ int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r, int64_t early_c0 = 0,
         c.pstart[b + 1] = cur;
     }
     *r = cur - i0;
-    if (early_ncols > 0) st.update_macs += (*r) * (*r) / 2 * early_ncols;
-    return early_ncols > 0 ? LINAC_EARLY_SOLVE_DONE : LINAC_OK;
+    return LINAC_OK;
+}
+
+// The strip's row-block solve on columns [c0, c0 + ncols) of its pivot rows (S4), optionally writing the u8 limb planes
+// of the result (Bq) and posting the strip's records to the host (mail != nullptr).
+// bq_col0 / bq_total: position of column c0 inside the planes and the planes' total column count (0 = this launch only).
+int launch_strip_solve(Fp& c, const StripLaunch& L, int64_t i0, int64_t c0, int64_t ncols, uint8_t* Bq, int kp, bool mail,
+                       int64_t bq_col0 = 0, int64_t bq_total = 0) {
+    if (ncols <= 0) return LINAC_OK;
+    Timed tm(c, stats().ms_trsm, 2);
+    trsm_strip_kernel<true><<<(unsigned)((ncols + PW - 1) / PW), TNT, trsm_smem_bytes(L.j1 - L.j0), c.s>>>(
+        c.A, c.ld, c.A + i0 * c.ld + c0, c.ld, ncols, c.d_pstart, (int)L.b0, (int)L.b1, c.d_T, c.d_pivcols, c.f, Bq, kp,
+        mail ? c.h_mail : nullptr, L.seq, c.d_rec, bq_col0, bq_total > 0 ? bq_total : ncols);
+    LINAC_CUDA(cudaGetLastError());
+    stats().kernel_launches++;
+    return LINAC_OK;
+}
+
+// One strip s with active rows >= i0 (one cooperative launch).  Returns the number of pivots through *r.
+// If early_ncols > 0 the strip's row-block solve on columns [early_c0, early_c0 + early_ncols) is enqueued right
+// behind the strip kernel (it takes the pivot counts from device memory and posts the records to the host): the
+// round trip then hides under the solve instead of idling the GPU.
+int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r, int64_t early_c0 = 0, int64_t early_ncols = 0,
+                 uint8_t* early_Bq = nullptr, int early_kp = 0, uint8_t* tail_Aq = nullptr) {
+    const bool early = early_ncols > 0 && options().timing != 1;
+    StripLaunch L;
+    int rc = launch_strip(c, s, i0, c.s, c.coop_grid, false, !early, tail_Aq, early_kp, &L);
+    if (rc) return rc;
+    if (early) {
+        rc = launch_strip_solve(c, L, i0, early_c0, early_ncols, early_Bq, early_kp, true);
+        if (rc) return rc;
+    }
+    rc = collect_strip(c, L, i0, r);
+    if (rc) return rc;
+    if (early) stats().update_macs += (*r) * (*r) / 2 * early_ncols;
+    return early ? LINAC_EARLY_SOLVE_DONE : LINAC_OK;
+}
+
+// Flat sweep with LOOK-AHEAD over strips [s0, s1) (columns up to jend): once strip s is factored and its row-block solve
+// has run, the Schur update is split in two: the next strip's columns first (a narrow product), then -- concurrently --
+// the strip kernel of s+1 on `la_ctas` SMs (second stream) and the bulk of the update on the remaining SMs.  The strip
+// kernel is a latency chain that leaves most issue slots of the GPU unused; the bulk update fills them.
+//   stream c.s:   ... | solve_s | update_s[next strip] | update_s[rest] ----------| swaps_{s+1} solve_{s+1} | ...
+//   second stream:                                      | strip kernel s+1 -------|
+// Row exchanges of a look-ahead strip touch only its own columns while the bulk update owns the rest of those rows;
+// deferred_swaps_kernel applies them to the other columns afterwards.  The L21 limb planes are double buffered (the
+// bulk update of strip s still reads its planes while strip s+1 writes the next ones).
+int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jend, int64_t* r_out) {
+    const Options& o = options();
+    Context& cx = ctx();
+    if (!cx.la_stream) {                                       // highest priority: its CTAs are placed before the bulk's
+        int lo = 0, hi = 0;
+        LINAC_CUDA(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+        LINAC_CUDA(cudaStreamCreateWithPriority(&cx.la_stream, cudaStreamNonBlocking, hi));
+    }
+    for (cudaEvent_t& e : cx.la_ev)
+        if (!e) LINAC_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    cudaStream_t sB = cx.la_stream;
+    cudaEvent_t ev_narrow = cx.la_ev[1], ev_strip = cx.la_ev[2];
+    // How many SMs the look-ahead strip kernel gets, per strip.  Cost model in microseconds, fitted to sweeps of the
+    // fixed-partition schedule on a B200 at config c3 (`profiles/r02_lookahead.md`): a 128-column strip kernel on G CTAs
+    // takes 63.5 + 4300 (m / 1e4) / G (the chain of CTA 0 plus the in-strip updates and the L21 limb split, which spread
+    // over G CTAs); the K = 128 bulk update takes 207 (m / 1e4)(n / 1e4) on the whole GPU and 1.05 + 0.62 G / (148 - G)
+    // times that beside a strip kernel on G SMs (it is partly HBM-bound, so it slows less than in proportion).  The
+    // partition that minimises the longer of the two is taken; option la_ctas > 0 forces a value.
+    auto pick_grid = [&](int64_t m, int64_t n, double* t_la, double* t_seq) {
+        const double mm = (double)m / 1e4, nn = (double)n / 1e4;
+        auto t_strip = [&](int G) { return 63.5 + 4300.0 * mm / G; };
+        auto t_bulk = [&](int G) { return 207.0 * mm * nn * (1.05 + 0.62 * G / (148.0 - G)); };
+        int best = 32;
+        double bt = 1e30;
+        for (int G : {16, 24, 32, 40, 48, 56, 64, 72, 80, 96, 112}) {
+            if (o.la_ctas > 0 && G != (int)o.la_ctas) continue;
+            if (G >= c.coop_grid) continue;
+            const double t = std::max(t_strip(G), t_bulk(G));
+            if (t < bt) { bt = t; best = G; }
+        }
+        if (bt > 1e29) { best = (int)std::min<int64_t>(std::max<int64_t>(o.la_ctas, 4), c.coop_grid - 1); bt = std::max(t_strip(best), t_bulk(best)); }
+        *t_la = bt + 14.0;                                      // + the narrow update that precedes the fork
+        *t_seq = t_strip(c.coop_grid) + 207.0 * mm * nn;
+        return best;
+    };
+    const int64_t j_first = panel_col0(c.sb0(s0));
+    const int kp = (int)((c.bps * PW + 127) / 128 * 128);
+    const size_t mark = c.arena->off;
+    uint8_t* Bq = (uint8_t*)c.arena->take((size_t)4 * (jend - j_first) * kp, 1024);
+    uint8_t* Aq[2] = {nullptr, nullptr};
+    if (Bq) Aq[0] = (uint8_t*)c.arena->take((size_t)4 * (c.rows - i0) * kp, 1024);
+    if (Aq[0]) Aq[1] = (uint8_t*)c.arena->take((size_t)4 * (c.rows - i0) * kp, 1024);
+    if (!Aq[1]) { c.arena->off = mark; return -1; }           // not enough workspace: the caller runs the sequential sweep
+    int64_t cur = i0;
+    *r_out = 0;
+    // strip s0 alone, on the whole GPU
+    StripLaunch L;
+    bool la_launched = false;                                  // was the strip in L launched as a look-ahead strip?
+    int rc = launch_strip(c, s0, cur, c.s, c.coop_grid, false, true, Aq[s0 & 1], kp, &L);
+    if (rc) return rc;
+    int64_t r = 0;
+    rc = collect_strip(c, L, cur, &r);
+    if (rc) return rc;
+    for (int64_t s = s0; s < s1; ++s) {
+        // here: strip s is launched and collected (r pivots from row cur), on c.s or on sB (la_launched)
+        const int64_t jc = L.j1;
+        if (la_launched) {
+            LINAC_CUDA(cudaStreamWaitEvent(c.s, ev_strip, 0));
+            const int64_t ncol_out = c.cols - (L.j1 - L.j0);
+            if (ncol_out > 0) {
+                deferred_swaps_kernel<<<(unsigned)((ncol_out + 255) / 256), 256, 0, c.s>>>(c.A, c.ld, c.cols, L.j0, L.j1, c.d_rec,
+                                                                                         c.d_pstart, (int)L.b0, (int)(L.b1 - L.b0));
+                LINAC_CUDA(cudaGetLastError());
+                stats().kernel_launches++;
+            }
+        }
+        const bool last = s + 1 >= s1;
+        const int64_t m2 = c.rows - (cur + r);
+        const int64_t jn = last ? jc : std::min(jend, panel_col0(c.sb0(s + 2)));       // end of the next strip's columns
+        bool next_launched = false;
+        StripLaunch Ln;
+        if (r > 0 && jend > jc) {
+            const bool planes = r <= kp && (jend - jc) >= o.tc_min_mn && r >= o.tc_min_k && m2 >= o.tc_min_mn && o.gemm_path != 1 && o.tc_panel != 0;
+            auto update = [&](int64_t c0, int64_t c1, int grid_limit) -> int {
+                GemmArgs g{c.A + (cur + r) * c.ld + c0, c.ld, c.A + (cur + r) * c.ld, c.ld, c.d_pivcols + cur,
+                           c.A + cur * c.ld + c0,       c.ld, m2,                      c1 - c0, r};
+                if (planes) {
+                    g.Bq_ready = Bq; g.kp_ready = kp; g.Aq_ready = Aq[s & 1];
+                    g.bq_row0 = c0 - jc; g.bq_rows_total = jend - jc;
+                }
+                g.grid_limit = grid_limit;
+                return run_gemm(c, g);
+            };
+            // look ahead only when there is bulk to hide the next strip kernel behind
+            // (and only for row blocks no taller than three times their width: the cost model below was fitted on square
+            // trailing blocks; on the tall flat nodes of the N = 1e5 recursion the fork measured 0.8 % slower than none)
+            bool la = !last && m2 > 0 && planes && jn - jc >= o.tc_min_mn && jend - jn >= 4 * o.tc_min_mn && m2 >= 8 * o.tc_min_mn &&
+                      cur + r < c.rows && m2 <= 3 * (jend - jn);
+            int la_grid = 32;
+            if (la) {
+                double t_la = 0, t_seq = 0;
+                la_grid = pick_grid(m2, jend - jn, &t_la, &t_seq);
+                la = t_la < t_seq;                                                 // not worth forking for this strip
+            }
+            stats().update_macs += r * r / 2 * (jend - jc);
+            if (la) {
+                // the whole row-block solve first (measured: solving only the next strip's columns before the fork and the
+                // rest beside the strip kernel is SLOWER, 13.5 -> 15.3 ms at c3: the solve is not a persistent kernel, its
+                // 300 CTAs spread over every SM and get in the way of the strip kernel's chain), then the next strip's
+                // columns of the update, the fork, and the bulk of the update beside the strip kernel
+                rc = launch_strip_solve(c, L, cur, jc, jend - jc, Bq, kp, false);
+                if (rc) return rc;
+                rc = update(jc, jn, 0);
+                if (rc) return rc;
+                LINAC_CUDA(cudaEventRecord(ev_narrow, c.s));
+                LINAC_CUDA(cudaStreamWaitEvent(sB, ev_narrow, 0));
+                rc = launch_strip(c, s + 1, cur + r, sB, la_grid, true, true, Aq[(s + 1) & 1], kp, &Ln);
+                if (rc) return rc;
+                LINAC_CUDA(cudaEventRecord(ev_strip, sB));
+                next_launched = true;
+                rc = update(jn, jend, c.coop_grid - la_grid);
+                if (rc) return rc;
+            } else {
+                rc = launch_strip_solve(c, L, cur, jc, jend - jc, planes ? Bq : nullptr, kp, false);
+                if (rc) return rc;
+                if (m2 > 0) {
+                    rc = update(jc, jend, 0);
+                    if (rc) return rc;
+                }
+            }
+        }
+        cur += r;
+        *r_out = cur - i0;
+        if (last) break;
+        if (cur >= c.rows) {                                   // no rows left: every remaining column of the node is free
+            int64_t r_rest = 0;
+            rc = factor(c, s + 1, s1, cur, &r_rest, false);
+            if (rc) return rc;
+            break;
+        }
+        if (!next_launched) {
+            rc = launch_strip(c, s + 1, cur, c.s, c.coop_grid, false, true, Aq[(s + 1) & 1], kp, &Ln);
+            if (rc) return rc;
+        }
+        rc = collect_strip(c, Ln, cur, &r);
+        if (rc) return rc;
+        L = Ln;
+        la_launched = next_launched;
+    }
+    c.arena->off = mark;
+    return LINAC_OK;
 }
 
 // Recursive factorisation of strips [s0, s1) with active rows [i0, rows).  Fills pstart for their panels.
-int factor(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t* r_out, bool allow_flat = true) {
+int factor(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t* r_out, bool allow_flat) {
     *r_out = 0;
     if (s1 <= s0) return LINAC_OK;
     if (i0 >= c.rows) {                              // no rows left: every remaining column is free
@@ -238,6 +432,11 @@ int factor(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t* r_out, bool allow
         // half as many read-modify-write passes over the trailing matrix as a per-strip update).
         const int64_t jend = std::min(c.cols, panel_col0(c.sb0(s1)));
         const int64_t grp = std::max<int64_t>(1, options().flat_group);
+        if (options().lookahead != 0 && grp == 1 && options().timing != 1 && s1 - s0 >= 3 && c.bps * PW <= 256 &&
+            options().gemm_path != 1 && options().tc_panel != 0 && jend - panel_col0(c.sb0(s0)) >= 1536 && c.rows - i0 >= 1536) {
+            const int rc_la = factor_flat_lookahead(c, s0, s1, i0, jend, r_out);
+            if (rc_la >= 0) return rc_la;                  // < 0: not enough workspace for its planes, sweep sequentially
+        }
         int64_t cur = i0;
         for (int64_t s = s0; s < s1; s += grp) {
             const int64_t se = std::min(s1, s + grp);
@@ -446,7 +645,7 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     }
     // forward elimination
     int64_t r = 0;
-    rc = factor(c, 0, c.ns, 0, &r);
+    rc = factor(c, 0, c.ns, 0, &r, true);
     // column classification: pivot index, or the threshold row of a free column
     std::vector<int32_t> colinfo(cols);
     std::vector<int32_t> freec, freeth;

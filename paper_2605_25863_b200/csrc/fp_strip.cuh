@@ -369,6 +369,9 @@ struct StripArgs {
     unsigned long long* host_mail;  // mapped pinned host memory: MAXBP * MAIL_WORDS tagged words, written by CTA 0
     unsigned long long seq;         // tag of this launch (32 significant bits)
     int slot;                       // entry of c_f that holds this call's field
+    int64_t swap_c0, swap_c1;       // columns on which row exchanges are applied at once ([0, cols) normally; the strip's own
+                                    // columns under look-ahead, where the previous strip's bulk update is still writing the
+                                    // other columns of the same rows: deferred_swaps_kernel applies the rest afterwards)
 };
 
 // Deferred write-back of a U12 slice: the raw entries it replaces are read by every row worker of
@@ -627,7 +630,7 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
         // ---- row exchanges on complete rows, one thread per column (so the sequence of exchanges
         // needs no inter-thread ordering)
         if (nsw > 0) {
-            for (int64_t c = (int64_t)cta * SNT + tid; c < a.cols; c += (int64_t)G * SNT) {
+            for (int64_t c = a.swap_c0 + (int64_t)cta * SNT + tid; c < a.swap_c1; c += (int64_t)G * SNT) {
                 for (int t = 0; t < r; ++t) {
                     const int64_t s = rec->swp[t];
                     if (s != cur + t) {
@@ -719,6 +722,31 @@ __global__ void __launch_bounds__(SNT, 1) strip_factor_kernel(const StripArgs a)
     }
 }
 
+// Row exchanges of a whole strip on the columns a look-ahead strip kernel left out ([0, skip0) and [skip1, cols)), in
+// the order the strip performed them; one thread per column.  Exits at once when the strip exchanged nothing.
+__global__ void deferred_swaps_kernel(uint32_t* __restrict__ A, int64_t ld, int64_t cols, int64_t skip0, int64_t skip1,
+                                      const PanelRec* __restrict__ rec, const int32_t* __restrict__ pstart, int b0, int nbp) {
+    bool any = false;
+    for (int b = b0; b < b0 + nbp; ++b) any = any || (rec[b].r > 0 && rec[b].nswaps > 0);
+    if (!any) return;
+    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= skip0) c += skip1 - skip0;
+    if (c >= cols) return;
+    for (int b = b0; b < b0 + nbp; ++b) {
+        const int r = rec[b].r;
+        if (r == 0 || rec[b].nswaps == 0) continue;
+        const int64_t cur = pstart[b];
+        for (int t = 0; t < r; ++t) {
+            const int64_t s = rec[b].swp[t];
+            if (s != cur + t) {
+                const uint32_t x = A[(cur + t) * ld + c], y = A[s * ld + c];
+                A[(cur + t) * ld + c] = y;
+                A[s * ld + c] = x;
+            }
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // S4 / S6 leaf: triangular solve against ONE strip's pivots, column-parallel (a CTA owns 32 columns
 // of X and keeps them in shared memory, so the sequential dependence between base panels never
@@ -758,7 +786,7 @@ __global__ void __launch_bounds__(TNT, 2) trsm_strip_kernel(const uint32_t* __re
                                                          const int32_t* __restrict__ pivcols, ModP f,
                                                          uint8_t* __restrict__ Bq, int kp,
                                                          unsigned long long* host_mail, unsigned long long seq,
-                                                         const PanelRec* rec) {
+                                                         const PanelRec* rec, int64_t bq_col0, int64_t bq_total) {
     extern __shared__ __align__(16) unsigned char trsm_smem_raw[];
     if (host_mail != nullptr && blockIdx.x == 0) mail_records(host_mail, seq, rec + bs0, bs1 - bs0);
     const int t0 = pstart[bs0], K = pstart[bs1] - t0;
@@ -900,8 +928,10 @@ __global__ void __launch_bounds__(TNT, 2) trsm_strip_kernel(const uint32_t* __re
         for (int t = wq; t < K; t += NW) X[(int64_t)t * ldx + c] = Xs[t][lane];
     // Optionally hand the result to the Schur update already split into its four u8 limb planes
     // (Bq[limb][column][kp], k-major, zero padded to kp): saves the update its own pass over U12.
+    // The planes may belong to a wider row block than this launch solves (look-ahead splits the solve into the next
+    // strip's columns and the rest): bq_total columns per plane, this launch starts at column bq_col0.
     if (Bq != nullptr && cok) {
-        const int64_t plane = ncols * (int64_t)kp;
+        const int64_t plane = bq_total * (int64_t)kp;
         for (int job = wq; job < 4 * (kp / 16); job += NW) {          // (limb, 16 consecutive k) per warp, lane = column
             const int l = job / (kp / 16), k0 = (job % (kp / 16)) * 16;
             uint32_t w[4];
@@ -916,7 +946,7 @@ __global__ void __launch_bounds__(TNT, 2) trsm_strip_kernel(const uint32_t* __re
                 }
                 w[q] = packed;
             }
-            *reinterpret_cast<uint4*>(Bq + (int64_t)l * plane + c * kp + k0) = make_uint4(w[0], w[1], w[2], w[3]);
+            *reinterpret_cast<uint4*>(Bq + (int64_t)l * plane + (bq_col0 + c) * kp + k0) = make_uint4(w[0], w[1], w[2], w[3]);
         }
     }
 }

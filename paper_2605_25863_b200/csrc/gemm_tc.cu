@@ -511,11 +511,12 @@ EncodeTiledFn get_encode_fn() {
 }
 
 // 3-D map over limb planes: (k bytes, rows, 4 planes); box = (128, box_rows, 4); 128-byte swizzle.
-bool make_limb_map(CUtensorMap* tm, uint8_t* base, int64_t rows, int64_t kp, int box_rows) {
+bool make_limb_map(CUtensorMap* tm, uint8_t* base, int64_t rows, int64_t kp, int box_rows, int64_t plane_rows = 0) {
     EncodeTiledFn enc = get_encode_fn();
     if (!enc) return false;
+    if (plane_rows <= 0) plane_rows = rows;               // rows between two limb planes (>= rows when `base` is a sub-range)
     cuuint64_t dims[3] = {(cuuint64_t)kp, (cuuint64_t)rows, 4};
-    cuuint64_t strides[2] = {(cuuint64_t)kp, (cuuint64_t)rows * (cuuint64_t)kp};
+    cuuint64_t strides[2] = {(cuuint64_t)kp, (cuuint64_t)plane_rows * (cuuint64_t)kp};
     cuuint32_t box[3] = {(cuuint32_t)KB, (cuuint32_t)box_rows, 4};
     cuuint32_t estr[3] = {1, 1, 1};
     CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -601,9 +602,12 @@ int gemm_modp_tc(const GemmArgs& g, const ModP& f, cudaStream_t s, Arena* scratc
             stats().kernel_launches++;
         }
         CUtensorMap tmA, tmB, tmC;
-        if (!make_limb_map(&tmA, Aq, g.M, kp, TM) || !make_limb_map(&tmB, Bq, g.N, kp, PN) || !make_c_map(&tmC, g.C, g.ldc, g.M, g.N))
+        const int64_t b_total = b_ready && g.bq_rows_total > 0 ? g.bq_rows_total : g.N;
+        const int64_t b_row0 = b_ready ? g.bq_row0 : 0;
+        if (!make_limb_map(&tmA, Aq, g.M, kp, TM) || !make_limb_map(&tmB, Bq + b_row0 * kp, g.N, kp, PN, b_total) ||
+            !make_c_map(&tmC, g.C, g.ldc, g.M, g.N))
             return -1;
-        const int grid = sm_count();
+        const int grid = g.grid_limit > 0 ? std::min(g.grid_limit, sm_count()) : sm_count();
         const PanelSched sc = make_sched(g.M, g.N, grid);
         if (f.ninv)
             gemm_tc_panel_kernel<true><<<(unsigned)std::min(grid, sc.nitems), P_THREADS, P_SMEM, s>>>(tmA, tmB, tmC, (int)(kp / KB), sc, f);

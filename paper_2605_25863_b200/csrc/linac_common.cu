@@ -20,6 +20,8 @@ Context::~Context() {
     if (own_ws) cudaFree(own_ws);
     if (mail) cudaFreeHost(mail);
     for (cudaEvent_t e : events) if (e) cudaEventDestroy(e);
+    for (cudaEvent_t e : la_ev) if (e) cudaEventDestroy(e);
+    if (la_stream) cudaStreamDestroy(la_stream);
     if (slot >= 0) {
         std::lock_guard<std::mutex> lock(g_init_mutex);
         g_slot_used[slot] = false;
@@ -268,6 +270,12 @@ int linac_set_option(const char* name, int64_t value) {
     } else if (!strcmp(name, "flat_cols")) {
         if (value < 0) return LINAC_ERR_INVALID_ARG;
         g_options.flat_cols = value;
+    } else if (!strcmp(name, "lookahead")) {
+        if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
+        g_options.lookahead = value;
+    } else if (!strcmp(name, "la_ctas")) {
+        if (value != 0 && (value < 4 || value > 128)) return LINAC_ERR_INVALID_ARG;
+        g_options.la_ctas = value;
     } else if (!strcmp(name, "strip_width")) {
         if (value < 32 || value > 256 || value % 32) return LINAC_ERR_INVALID_ARG;
         g_options.strip_width = value;

@@ -55,6 +55,9 @@ struct Options {
     int64_t flat_cols = 16384; // nodes of at most this many columns are swept flat (right-looking), wider ones recurse
     int64_t flat_group = 1;   // strips per Schur update of the flat sweep (K = flat_group * strip_width)
     int64_t strip_width = 128; // columns factored by one cooperative strip kernel (multiple of 32, <= 256)
+    int64_t lookahead = 1;    // flat sweep: 1 = factor strip s+1 on `la_ctas` SMs (second stream) while the bulk of strip s's
+                              // Schur update runs on the other SMs; 0 = strictly sequential
+    int64_t la_ctas = 0;      // CTAs (= SMs) of the look-ahead strip kernel; 0 = chosen per strip from a cost model
 };
 Options& options();
 
@@ -71,6 +74,8 @@ struct Context {
     unsigned long long seq = 0;               // tag of the last strip launch
     std::vector<cudaEvent_t> events;          // pool for the timing modes
     int slot = -1;                            // index into the __constant__ ModP table of fp_strip.cuh
+    cudaStream_t la_stream = nullptr;         // second stream of the look-ahead schedule (created on first use)
+    cudaEvent_t la_ev[4] = {nullptr, nullptr, nullptr, nullptr};
     char cuda_error[1024] = {0};
     ~Context();
 };
@@ -148,6 +153,10 @@ struct GemmArgs {
     uint8_t* Bq_ready = nullptr;
     int64_t kp_ready = 0;
     uint8_t* Aq_ready = nullptr;      // same for A: Aq[limb][m][kp_ready], written by the strip kernel's tail
+    // Bq_ready may describe MORE columns than this update touches (look-ahead splits one update into the next strip's
+    // columns and the rest): the planes hold bq_rows_total columns (0 = N) and this update starts at column bq_row0
+    int64_t bq_row0 = 0, bq_rows_total = 0;
+    int grid_limit = 0;               // persistent kernels: use at most this many CTAs (0 = one per SM)
 };
 int gemm_modp_simt(const GemmArgs& g, const ModP& f, cudaStream_t s);
 // Tensor-core (tcgen05 int8 limb) path; returns LINAC_OK if it ran, or a negative value if the
