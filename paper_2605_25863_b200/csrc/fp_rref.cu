@@ -73,18 +73,19 @@ constexpr int LINAC_EARLY_SOLVE_DONE = -1000;      // internal: factor_strip alr
 
 int64_t panel_col0(int64_t b) { return b * PW; }
 
-int run_gemm(Fp& c, const GemmArgs& g) {
+int run_gemm(Fp& c, const GemmArgs& g, cudaStream_t stream = nullptr) {
     Options& o = options();
+    if (!stream) stream = c.s;
     const bool timing = o.timing == 1;
     if (timing) cudaEventRecord(c.ev0, c.s);
-    const int mk = c.mark_begin(0, g.M, g.N, g.K);
+    const int mk = c.mark_begin(0, g.M, g.N, g.K, stream);
     int rc = -1;
     if (o.gemm_path != 1 && g.K >= o.tc_min_k && g.M >= o.tc_min_mn && g.N >= o.tc_min_mn) {
         const size_t mark = c.arena->off;
-        rc = gemm_modp_tc(g, c.f, c.s, c.arena);
+        rc = gemm_modp_tc(g, c.f, stream, c.arena);
         c.arena->off = mark;
     }
-    if (rc < 0) rc = gemm_modp_simt(g, c.f, c.s);
+    if (rc < 0) rc = gemm_modp_simt(g, c.f, stream);
     c.mark_end(mk);
     if (timing && rc == LINAC_OK) {
         cudaEventRecord(c.ev1, c.s);
@@ -230,10 +231,11 @@ int collect_strip(Fp& c, const StripLaunch& L, int64_t i0, int64_t* r) {
 // of the result (Bq) and posting the strip's records to the host (mail != nullptr).
 // bq_col0 / bq_total: position of column c0 inside the planes and the planes' total column count (0 = this launch only).
 int launch_strip_solve(Fp& c, const StripLaunch& L, int64_t i0, int64_t c0, int64_t ncols, uint8_t* Bq, int kp, bool mail,
-                       int64_t bq_col0 = 0, int64_t bq_total = 0) {
+                       int64_t bq_col0 = 0, int64_t bq_total = 0, cudaStream_t stream = nullptr) {
     if (ncols <= 0) return LINAC_OK;
-    Timed tm(c, stats().ms_trsm, 2);
-    trsm_strip_kernel<true><<<(unsigned)((ncols + PW - 1) / PW), TNT, trsm_smem_bytes(L.j1 - L.j0), c.s>>>(
+    if (!stream) stream = c.s;
+    Timed tm(c, stats().ms_trsm, 2, stream);
+    trsm_strip_kernel<true><<<(unsigned)((ncols + PW - 1) / PW), TNT, trsm_smem_bytes(L.j1 - L.j0), stream>>>(
         c.A, c.ld, c.A + i0 * c.ld + c0, c.ld, ncols, c.d_pstart, (int)L.b0, (int)L.b1, c.d_T, c.d_pivcols, c.f, Bq, kp,
         mail ? c.h_mail : nullptr, L.seq, c.d_rec, bq_col0, bq_total > 0 ? bq_total : ncols);
     LINAC_CUDA(cudaGetLastError());
@@ -265,18 +267,18 @@ int factor_strip(Fp& c, int64_t s, int64_t i0, int64_t* r, int64_t early_c0 = 0,
 // has run, the Schur update is split in two: the next strip's columns first (a narrow product), then -- concurrently --
 // the strip kernel of s+1 on `la_ctas` SMs (second stream) and the bulk of the update on the remaining SMs.  The strip
 // kernel is a latency chain that leaves most issue slots of the GPU unused; the bulk update fills them.
-//   stream c.s:   ... | solve_s | update_s[next strip] | update_s[rest] ----------| swaps_{s+1} solve_{s+1} | ...
-//   second stream:                                      | strip kernel s+1 -------|
+//   stream c.s:   ... | solve_s | update_s[next strip] | strip kernel s+1 -------| swaps_{s+1} solve_{s+1} | ...
+//   second stream:                                      | update_s[rest] ---------|
 // Row exchanges of a look-ahead strip touch only its own columns while the bulk update owns the rest of those rows;
 // deferred_swaps_kernel applies them to the other columns afterwards.  The L21 limb planes are double buffered (the
 // bulk update of strip s still reads its planes while strip s+1 writes the next ones).
 int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jend, int64_t* r_out) {
     const Options& o = options();
     Context& cx = ctx();
-    if (!cx.la_stream) {                                       // highest priority: its CTAs are placed before the bulk's
+    if (!cx.la_stream) {                                       // lowest priority: the bulk must never be placed before the chain
         int lo = 0, hi = 0;
         LINAC_CUDA(cudaDeviceGetStreamPriorityRange(&lo, &hi));
-        LINAC_CUDA(cudaStreamCreateWithPriority(&cx.la_stream, cudaStreamNonBlocking, hi));
+        LINAC_CUDA(cudaStreamCreateWithPriority(&cx.la_stream, cudaStreamNonBlocking, lo));
     }
     for (cudaEvent_t& e : cx.la_ev)
         if (!e) LINAC_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
@@ -343,7 +345,7 @@ int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jen
         StripLaunch Ln;
         if (r > 0 && jend > jc) {
             const bool planes = r <= kp && (jend - jc) >= o.tc_min_mn && r >= o.tc_min_k && m2 >= o.tc_min_mn && o.gemm_path != 1 && o.tc_panel != 0;
-            auto update = [&](int64_t c0, int64_t c1, int grid_limit) -> int {
+            auto update = [&](int64_t c0, int64_t c1, int grid_limit, cudaStream_t stream) -> int {
                 GemmArgs g{c.A + (cur + r) * c.ld + c0, c.ld, c.A + (cur + r) * c.ld, c.ld, c.d_pivcols + cur,
                            c.A + cur * c.ld + c0,       c.ld, m2,                      c1 - c0, r};
                 if (planes) {
@@ -351,7 +353,7 @@ int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jen
                     g.bq_row0 = c0 - jc; g.bq_rows_total = jend - jc;
                 }
                 g.grid_limit = grid_limit;
-                return run_gemm(c, g);
+                return run_gemm(c, g, stream);
             };
             // look ahead only when there is bulk to hide the next strip kernel behind
             // (and only for row blocks no taller than three times their width: the cost model below was fitted on square
@@ -366,27 +368,30 @@ int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jen
             }
             stats().update_macs += r * r / 2 * (jend - jc);
             if (la) {
-                // the whole row-block solve first (measured: solving only the next strip's columns before the fork and the
-                // rest beside the strip kernel is SLOWER, 13.5 -> 15.3 ms at c3: the solve is not a persistent kernel, its
-                // 300 CTAs spread over every SM and get in the way of the strip kernel's chain), then the next strip's
-                // columns of the update, the fork, and the bulk of the update beside the strip kernel
+                // the whole row-block solve first (measured twice: solving only the next strip's columns before the fork and
+                // the rest beside the strip kernel is SLOWER, 13.5 -> 15.3 / 16.0 ms at c3: squeezed onto the bulk's SMs the
+                // solve needs two rounds of CTAs and pushes the bulk update, which then bounds the step), then the next
+                // strip's columns of the update, the fork, and the bulk of the update beside the strip kernel
                 rc = launch_strip_solve(c, L, cur, jc, jend - jc, Bq, kp, false);
                 if (rc) return rc;
-                rc = update(jc, jn, 0);
+                rc = update(jc, jn, 0, c.s);
                 if (rc) return rc;
+                // the chain stays on the call's stream (the strip kernel starts the moment the narrow update ends and takes
+                // its SMs first); the bulk goes to the second stream, where the cross-stream event latency does no harm
                 LINAC_CUDA(cudaEventRecord(ev_narrow, c.s));
-                LINAC_CUDA(cudaStreamWaitEvent(sB, ev_narrow, 0));
-                rc = launch_strip(c, s + 1, cur + r, sB, la_grid, true, true, Aq[(s + 1) & 1], kp, &Ln);
+                rc = launch_strip(c, s + 1, cur + r, c.s, la_grid, true, true, Aq[(s + 1) & 1], kp, &Ln);
                 if (rc) return rc;
-                LINAC_CUDA(cudaEventRecord(ev_strip, sB));
                 next_launched = true;
-                rc = update(jn, jend, c.coop_grid - la_grid);
+                stats().lookahead_strips++;
+                LINAC_CUDA(cudaStreamWaitEvent(sB, ev_narrow, 0));
+                rc = update(jn, jend, c.coop_grid - la_grid, sB);
                 if (rc) return rc;
+                LINAC_CUDA(cudaEventRecord(ev_strip, sB));                          // = "bulk of strip s done"
             } else {
                 rc = launch_strip_solve(c, L, cur, jc, jend - jc, planes ? Bq : nullptr, kp, false);
                 if (rc) return rc;
                 if (m2 > 0) {
-                    rc = update(jc, jend, 0);
+                    rc = update(jc, jend, 0, c.s);
                     if (rc) return rc;
                 }
             }
@@ -697,9 +702,13 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     if (e == cudaSuccess) cudaEventElapsedTime(&ms, t0, t1);
     st.ms_total = ms;
     if (e == cudaSuccess && options().timing == 2) {           // per-class device time of the production schedule
+        std::vector<std::pair<float, float>> iv_strip, iv_update;      // intervals relative to the call's start
         for (const Fp::Mark& mk : c.marks) {
-            float t = 0;
+            float t = 0, b0 = 0, b1 = 0;
             if (cudaEventElapsedTime(&t, event_pool[mk.ev], event_pool[mk.ev + 1]) != cudaSuccess) continue;
+            if (mk.cls != 2 && cudaEventElapsedTime(&b0, t0, event_pool[mk.ev]) == cudaSuccess &&
+                cudaEventElapsedTime(&b1, t0, event_pool[mk.ev + 1]) == cudaSuccess)
+                (mk.cls == 1 ? iv_strip : iv_update).push_back(std::make_pair(b0, b1));
             if (mk.cls == 0) {
                 st.ms_update += t;
                 if ((double)mk.m * mk.n * mk.k > (double)st.top_m * st.top_n * st.top_k) {
@@ -709,6 +718,10 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
             } else if (mk.cls == 1) st.ms_strip += t;
             else st.ms_trsm += t;
         }
+        double ov = 0;                                         // a strip kernel and an update kernel in flight together
+        for (const auto& a : iv_strip)
+            for (const auto& b : iv_update) ov += std::max(0.f, std::min(a.second, b.second) - std::max(a.first, b.first));
+        st.ms_overlap = ov;
     }
     if (rc) return rc;
     *rank = r;
