@@ -358,13 +358,14 @@ int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jen
             // look ahead only when there is bulk to hide the next strip kernel behind
             // (and only for row blocks no taller than three times their width: the cost model below was fitted on square
             // trailing blocks; on the tall flat nodes of the N = 1e5 recursion the fork measured 0.8 % slower than none)
-            bool la = !last && m2 > 0 && planes && jn - jc >= o.tc_min_mn && jend - jn >= 4 * o.tc_min_mn && m2 >= 8 * o.tc_min_mn &&
+            bool la = !last && m2 > 0 && planes && jn - jc >= o.tc_min_mn && jend - jn >= 2 * o.tc_min_mn && m2 >= 4 * o.tc_min_mn &&
                       cur + r < c.rows && m2 <= 3 * (jend - jn);
             int la_grid = 32;
             if (la) {
                 double t_la = 0, t_seq = 0;
                 la_grid = pick_grid(m2, jend - jn, &t_la, &t_seq);
-                la = t_la < t_seq;                                                 // not worth forking for this strip
+                la = t_la < t_seq || o.la_ctas > 0;                                // not worth forking for this strip (a forced
+                                                                                   // partition, option la_ctas, forks regardless)
             }
             stats().update_macs += r * r / 2 * (jend - jc);
             if (la) {

@@ -121,3 +121,30 @@ def test_c3_scale_rank_deficient_wide_certificates(oracle):
     got = oracle.matmul_modp(np.ascontiguousarray(a[rows_s][:, :rank]), np.ascontiguousarray(r_cols), p,
                              nthreads=oracle.max_threads())
     assert np.array_equal(got, a[rows_s][:, cols_s])
+
+
+@pytest.mark.parametrize("lookahead", [1, 0])
+def test_lookahead_with_row_exchanges_in_every_strip(oracle, lookahead):
+    """The look-ahead schedule defers a strip's row exchanges on all columns but its own while the previous strip's bulk
+    update still owns those rows.  Here every strip must fetch pivots from far below its candidate rows (the block
+    under the diagonal is zero), some rows are dependent, and a band of columns is free: exchanges, the general panel
+    path and free columns occur in every strip, with look-ahead on and off; both must give the oracle's bytes."""
+    import paper_2605_25863_b200 as L
+    p, n, m = P31, 3072, 2816
+    a = gen.uniform_matrix(n, m, p, seed=41)
+    for s in range(0, m, 128):
+        a[s:s + 96, s:s + 128] = 0                      # the candidate rows of every strip are zero in its columns
+    a[500:520] = ((a[100:120].astype(np.uint64) * 3 + a[900:920].astype(np.uint64)) % p).astype(np.uint32)   # dependent rows
+    a[:, 1500:1530] = 0                                 # free columns
+    r_ref, rank_ref, piv_ref = oracle.rref_modp(a, p, nthreads=oracle.max_threads())
+    try:
+        L.set_option("lookahead", lookahead)
+        L.set_option("la_ctas", 40)                     # force the fork (the cost model would not fork at this size)
+        out, rank, piv, st = gpu_rref(a, p)
+    finally:
+        L.set_option("lookahead", 1)
+        L.set_option("la_ctas", 0)
+    assert rank == rank_ref and np.array_equal(piv, piv_ref)
+    assert np.array_equal(out, r_ref)
+    assert st["row_swaps"] > 1000
+    assert (st["lookahead_strips"] > 5) == (lookahead == 1)
