@@ -546,7 +546,7 @@ class Bench:
                 "row_space_residual": err, "gpu_launches_per_call": int(launches),
                 "roofline": {"bound": "tensor", "achieved": flop / ms / 1e9, "peak": peak, "unit": "TFLOP/s (fp64 DMMA)",
                              "frac": flop / ms / 1e9 / peak, "peak_sm_mhz": mhz,
-                             "note": "executed flops of the K = 32 DMMA updates (2 rows (cols - j0) 32 per panel) / whole call"}}
+                             "note": "executed flops of the DMMA updates (2 rows (cols - j0) 32 per panel: K = 32 inside the panel's 128-column strip, K = 128 right of it) / whole call"}}
 
     def wide_leg(self, which, n=4096, reps=2):
         """SURVEY.md 8(f)#4: dense uniform n x n over F_p with p = 2^32 - 5 (uint32 storage) or 2^61 - 1 (uint64)."""

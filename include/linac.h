@@ -250,6 +250,8 @@ int linac_get_last_stats(linac_stats *out);
  * "f64_panel_threads" (256/512/1024) and "f64_panel_grid" (0 = one CTA per SM) of the fp64 panel kernel, "f64_panel_tags" (1 = tagged
  * candidate records instead of a grid barrier per column), "f64_panel_cluster" (CTAs of the cluster + DSMEM panel variant, 0 = off) with
  * "f64_cluster_rows" (rows per CTA up to which it is used),
+ * "f64_rref_strip" (linac_rref_f64: columns per strip, 32..128 in steps of 32; the columns right of a strip are updated once per strip
+ * with K = that width, 32 = once per panel),
  * "f64_rhs_inv" (fp64 substitution on the right-hand sides: 1 = blocked, with inverted 128 x 128 diagonal blocks, 0 = recursive leaf solves)}.
  * Returns LINAC_ERR_INVALID_ARG for unknown names / out-of-range values. */
 int linac_set_option(const char *name, int64_t value);

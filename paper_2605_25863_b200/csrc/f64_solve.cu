@@ -572,14 +572,29 @@ __device__ __forceinline__ void dmma_8x8x4(double& c0, double& c1, double a, dou
 // TN = 128 (8 warps as 2 x 4, 64 x 32 warp tiles) or 64 (64 x 16 warp tiles: the skinny right-hand-side updates).
 // ASSIGN: C = A.B instead of C -= A.B; a CTA reads every B element of its column range before its epilogue, so
 // C may alias B when one CTA covers all M rows (the diagonal-block step of the blocked substitution).
+// Shape taken from device memory (linac_rref_f64, which never syncs with the host inside its loop): K and M are clipped
+// to *kact / *mact and the rows of C and A start at *row0.  All null for the ordinary call.
+struct DevShape {
+    const int* kact;
+    const int* mact;
+    const long long* row0;
+};
 template <int TN, bool ASSIGN, int NW>
 __global__ void __launch_bounds__(NW * 32, TN == 64 ? 2 : 1) dgemm_sub_mma_kernel(double* C, int64_t ldc,
                                                             const double* __restrict__ A, int64_t lda,
                                                             const double* B, int64_t ldb, int64_t M,
-                                                            int64_t N, int64_t K, const int* __restrict__ kact) {
-    if (kact != nullptr) {                                 // K read from device memory (linac_rref_f64: the panel's pivot count)
-        K = min(K, (int64_t)*kact);
+                                                            int64_t N, int64_t K, DevShape ds) {
+    if (ds.kact != nullptr) {                              // the panel's pivot count
+        K = min(K, (int64_t)*ds.kact);
         if (K <= 0) return;
+    }
+    if (ds.mact != nullptr) {
+        M = min(M, (int64_t)*ds.mact);
+        if (M <= 0) return;
+    }
+    if (ds.row0 != nullptr) {
+        C += *ds.row0 * ldc;
+        A += *ds.row0 * lda;
     }
     constexpr int NJ = TN / 32;                            // MMA tiles per warp along n
     constexpr int NT = NW * 32;                            // threads: 8 warps as 2 x 4 (16 as 4 x 4 measured no faster)
@@ -606,6 +621,7 @@ __global__ void __launch_bounds__(NW * 32, TN == 64 ? 2 : 1) dgemm_sub_mma_kerne
         tx = band * RB + within - ty * bw;
     }
     const int64_t m0 = (int64_t)ty * DM, n0 = (int64_t)tx * TN;
+    if (m0 >= M) return;                                   // only when *mact clipped M below the grid
     double acc[MI][NJ][2];
 #pragma unroll
     for (int i = 0; i < MI; ++i)
@@ -788,21 +804,23 @@ struct F64 {
 };
 
 int dgemm_sub(F64& c, double* C, int64_t ldc, const double* A, int64_t lda, const double* B, int64_t ldb, int64_t M,
-              int64_t N, int64_t K, bool assign = false, const int* kact = nullptr) {
+              int64_t N, int64_t K, bool assign = false, const int* kact = nullptr, const int* mact = nullptr,
+              const long long* row0 = nullptr) {
     if (M <= 0 || N <= 0 || K <= 0) return LINAC_OK;
+    const DevShape ds{kact, mact, row0};
     // 128 x 64 tiles with two CTAs per SM (16 warps in flight) beat one 128 x 128 CTA per SM on every shape measured
     // (c4: 225 -> 217 ms); option f64_mma = 2 keeps the 128 x 128 tile for A/B runs
     const bool skinny = N <= 64 || assign || options().f64_mma != 2;
     const int tn = skinny ? 64 : DN;
     dim3 grid((unsigned)((N + tn - 1) / tn), (unsigned)((M + DM - 1) / DM));
     if (assign)
-        dgemm_sub_mma_kernel<64, true, 8><<<grid, 256, dmma_smem_bytes(64), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K, kact);
+        dgemm_sub_mma_kernel<64, true, 8><<<grid, 256, dmma_smem_bytes(64), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K, ds);
     else if (options().f64_mma == 0 && kact == nullptr)
         dgemm_sub_kernel<<<grid, DTHREADS, 0, c.s>>>(C, ldc, A, lda, B, ldb, M, N, K);
     else if (skinny)
-        dgemm_sub_mma_kernel<64, false, 8><<<grid, 256, dmma_smem_bytes(64), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K, kact);
+        dgemm_sub_mma_kernel<64, false, 8><<<grid, 256, dmma_smem_bytes(64), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K, ds);
     else
-        dgemm_sub_mma_kernel<128, false, 8><<<grid, 256, dmma_smem_bytes(128), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K, kact);
+        dgemm_sub_mma_kernel<128, false, 8><<<grid, 256, dmma_smem_bytes(128), c.s>>>(C, ldc, A, lda, B, ldb, M, N, K, ds);
     LINAC_CUDA(cudaGetLastError());
     stats().kernel_launches++;
     stats().update_macs += M * N * K;
@@ -969,24 +987,69 @@ int factor_flat_f64(F64& c) {
 //   f64_rref_pivot_rows_kernel U = D^-1 . A[pivot rows, j0:], D = the panel's pivot block (Gauss-Jordan without
 //                              further pivoting: the rows are in the order partial pivoting chose them), exactly the
 //                              identity on the pivot columns
+//   f64_rref_tinv_kernel       T = D^-1
 //   f64_rref_lcopy_kernel      L[k][t] = A[k][pivot column t], zero for the pivot rows themselves
-//   dgemm_sub_mma_kernel       A[:, j0:] -= L . U for ALL rows (above too, as in the paper's RowReduce), on DMMA
+//   dgemm_sub_mma_kernel       A -= L . U for ALL rows (above too, as in the paper's RowReduce), on DMMA: at once on the
+//                              columns of the panel's 128-column strip, once per strip (K = 128) right of it
 // so the matrix ends as the RREF without a back-elimination pass.
-__global__ void f64_rref_swap_kernel(double* __restrict__ M, int64_t ld, int64_t c0, int64_t cols,
-                                     const F64Rec* __restrict__ rec, const long long* __restrict__ ipiv) {
+// The panel's exchanges (ipiv[i0 + a] <-> i0 + a, a = 0 .. r-1, in that order) touch at most 2 r rows: thread 0 composes
+// them into one permutation of those rows, then a CTA moves 32 columns of them through shared memory -- two memory round
+// trips instead of r dependent ones.
+__global__ void __launch_bounds__(256) f64_rref_swap_kernel(double* __restrict__ M, int64_t ld, int64_t c0, int64_t cols,
+                                                           const F64Rec* __restrict__ rec, const long long* __restrict__ ipiv) {
+    __shared__ long long s_row[2 * FW];                     // the touched rows: the panel's pivot rows, then their partners
+    __shared__ long long s_piv[FW];
+    __shared__ int s_cur[2 * FW];                           // s_cur[k] = the slot whose ORIGINAL content ends in slot k
+    __shared__ int s_n;
+    __shared__ double tile[2 * FW][33];
     const int r = rec->r;
     if (r == 0) return;
-    const int64_t c = c0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= cols) return;
     const int64_t i0 = rec->i0;
-    for (int a = 0; a < r; ++a) {
-        const int64_t s = ipiv[i0 + a];
-        if (s != i0 + a) {
-            const double x = M[(i0 + a) * ld + c], y = M[s * ld + c];
-            M[(i0 + a) * ld + c] = y;
-            M[s * ld + c] = x;
+    const int tid = threadIdx.x;
+    if (tid < r) s_piv[tid] = ipiv[i0 + tid];
+    __syncthreads();
+    if (tid < 32) {                                         // warp 0: lane k keeps partner slot r + k
+        long long ext = -1;
+        int n = r;
+        bool any = false;
+        if (tid < r) { s_row[tid] = i0 + tid; s_cur[tid] = tid; }
+        __syncwarp();
+        for (int a = 0; a < r; ++a) {
+            const long long sr = s_piv[a];
+            if (sr == i0 + a) continue;
+            any = true;
+            int k;
+            if (sr < i0 + r) k = (int)(sr - i0);
+            else {
+                const unsigned m = __ballot_sync(0xffffffffu, ext == sr);
+                if (m) k = r + __ffs(m) - 1;
+                else {
+                    k = n;
+                    if (tid == n - r) { ext = sr; s_row[n] = sr; s_cur[n] = n; }
+                    ++n;
+                    __syncwarp();
+                }
+            }
+            if (tid == 0) {
+                const int t = s_cur[a];
+                s_cur[a] = s_cur[k];
+                s_cur[k] = t;
+            }
+            __syncwarp();
         }
+        if (tid == 0) s_n = any ? n : 0;
     }
+    __syncthreads();
+    const int n = s_n;
+    if (n == 0) return;
+    const int cx = tid & 31, g = tid >> 5;
+    const int64_t c = c0 + (int64_t)blockIdx.x * 32 + cx;
+    if (c < cols)
+        for (int k = g; k < n; k += 8) tile[k][cx] = M[s_row[k] * ld + c];
+    __syncthreads();
+    if (c < cols)
+        for (int k = g; k < n; k += 8)
+            if (s_cur[k] != k) M[s_row[k] * ld + c] = tile[s_cur[k]][cx];
 }
 
 // T = D^-1, D = A[i0 : i0+r, pivot columns] after the exchanges (one CTA; its own launch, so that the kernel below can
@@ -1012,12 +1075,14 @@ __global__ void __launch_bounds__(128) f64_rref_tinv_kernel(const double* __rest
     }
     __syncthreads();
     // Gauss-Jordan on [D | I]: thread = (row a, 16 columns); two phases per step so nobody reads a half-updated row t
-    const int a = tid >> 2, cg0 = (tid & 3) * 16;
+    const int a = tid & 31, cg0 = (tid >> 5) * 16;          // a warp = 32 rows x the same 16 columns: conflict-free
     for (int t = 0; t < r; ++t) {
-        const double d = G[t][t], h = G[a][t];
+        // one reciprocal per step: a division per entry took the slow path of the double-precision division on every
+        // zero of [D | I] (116 us per panel)
+        const double rd = 1.0 / G[t][t], h = G[a][t];
         double pt[16];
 #pragma unroll
-        for (int q = 0; q < 16; ++q) pt[q] = G[t][cg0 + q] / d;
+        for (int q = 0; q < 16; ++q) pt[q] = G[t][cg0 + q] * rd;
         __syncthreads();
         if (a < r) {
 #pragma unroll
@@ -1061,8 +1126,11 @@ __global__ void __launch_bounds__(128) f64_rref_pivot_rows_kernel(double* __rest
     }
 }
 
+// L[k][col_off + t] = A[k][pivot column t] (the raw entries ARE the multipliers once the pivot rows hold T . rows);
+// for the panel's own pivot rows the whole row of L up to col_off + 32 is zeroed: this panel's multipliers, and those
+// of the strip's earlier panels, which the catch-up product has just applied to these rows.
 __global__ void f64_rref_lcopy_kernel(const double* __restrict__ A, int64_t ld, int64_t rows, int64_t j0,
-                                      const F64Rec* __restrict__ rec, double* __restrict__ L) {
+                                      const F64Rec* __restrict__ rec, double* __restrict__ L, int ldl, int col_off) {
     const int r = rec->r;
     if (r == 0) return;
     const int t = threadIdx.x & 31;
@@ -1070,7 +1138,11 @@ __global__ void f64_rref_lcopy_kernel(const double* __restrict__ A, int64_t ld, 
     const int pc = rec->pc[t];
     for (int64_t k = (int64_t)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); k < rows; k += (int64_t)gridDim.x * (blockDim.x / 32)) {
         const bool pivot_row = k >= i0 && k < i0 + r;
-        L[k * FW + t] = (pc >= 0 && !pivot_row) ? A[k * ld + j0 + pc] : 0.0;
+        if (pivot_row) {
+            for (int q = t; q < col_off + FW; q += 32) L[k * ldl + q] = 0.0;
+        } else {
+            L[k * ldl + col_off + t] = pc >= 0 ? A[k * ld + j0 + pc] : 0.0;
+        }
     }
 }
 
@@ -1084,10 +1156,11 @@ __global__ void f64_rref_finalize_kernel(double* __restrict__ A, int64_t ld, int
     for (int64_t c = threadIdx.x; c < end; c += blockDim.x) A[k * ld + c] = 0.0;
 }
 
+constexpr int RW = 128;                   // strip width of linac_rref_f64: the wide update's K
 size_t f64_rref_workspace_bytes(int64_t rows, int64_t cols) {
     const int64_t ldu = (cols + 63) / 64 * 64;
     return 16384 + 2 * 1024 * sizeof(Cand) + 2 * FW * sizeof(double2) + (size_t)std::max<int64_t>(rows, 1) * 8 +
-           (size_t)FW * ldu * 8 + (size_t)rows * FW * 8 + (size_t)std::max<int64_t>(1, std::min(rows, cols)) * 4;
+           (size_t)RW * ldu * 8 + (size_t)rows * RW * 8 + (size_t)std::max<int64_t>(1, std::min(rows, cols)) * 4;
 }
 
 size_t f64_workspace_bytes(int64_t n) {
@@ -1256,8 +1329,8 @@ int linac_rref_f64(double* dA, int64_t rows, int64_t cols, int64_t ld, double to
     long long* state = (long long*)arena.take(256);
     int* dummy_info = (int*)(state + 8);
     F64Rec* rec = (F64Rec*)arena.take(sizeof(F64Rec));
-    double* U = (double*)arena.take((size_t)FW * ldu * 8);
-    double* L = (double*)arena.take((size_t)rows * FW * 8);
+    double* U = (double*)arena.take((size_t)RW * ldu * 8);
+    double* L = (double*)arena.take((size_t)rows * RW * 8);
     int32_t* d_piv = (int32_t*)arena.take((size_t)mn * 4);
     double* Tb = (double*)arena.take(FW * FW * 8);
     if (!cand || !target || !ipiv || !state || !rec || !U || !L || !d_piv || !Tb) return LINAC_ERR_WORKSPACE;
@@ -1270,22 +1343,51 @@ int linac_rref_f64(double* dA, int64_t rows, int64_t cols, int64_t ld, double to
     const size_t smem = (size_t)rows_per_cta * (FW + 2) * sizeof(double);
     double tolv = c.tol;
     int* info = dummy_info;
-    for (int64_t j0 = 0; j0 < cols; j0 += FW) {
-        int w = (int)std::min<int64_t>(FW, cols - j0);
-        int64_t j0v = j0, nv = rows, ldv = ld;
-        const int64_t nc = cols - j0;
-        unsigned tag0 = options().f64_panel_tags != 0 ? (unsigned)(j0 + 1) : 0u;
-        void* args[] = {&dA, &nv, &ldv, &j0v, &w, &rows_per_cta, &tolv, &cand, &target, &ipiv, &info, &tag0, &state, &rec, &d_piv};
-        LINAC_CUDA(cudaLaunchCooperativeKernel((void*)f64_panel_kernel<512, false, true>, dim3(c.grid), dim3(512), args, smem, s));
-        f64_rref_swap_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, s>>>(dA, ld, j0, cols, rec, ipiv);
-        f64_rref_tinv_kernel<<<1, 128, 0, s>>>(dA, ld, j0, rec, Tb);
-        f64_rref_pivot_rows_kernel<<<(unsigned)((nc + 127) / 128), 128, 0, s>>>(dA, ld, j0, cols, rec, Tb, U, ldu);
-        f64_rref_lcopy_kernel<<<(unsigned)std::min<int64_t>((rows + 7) / 8, 148 * 8), 256, 0, s>>>(dA, ld, rows, j0, rec, L);
-        LINAC_CUDA(cudaGetLastError());
-        st.kernel_launches += 5;
-        st.panels++;
-        rc = dgemm_sub(c, dA + j0, ld, L, FW, U + j0, ldu, rows, nc, FW, false, &rec->r);
-        if (rc) return rc;
+    // Strips of RW columns, panels of FW inside.  A panel's multipliers L_p (all rows) and normalised pivot rows U_p go
+    // to column block p of L and row block p of U; the panel updates the strip's own columns at once (K = 32) and the
+    // columns right of the strip once per strip (K = RW): A[:, right] -= L . U.  Before a panel's pivot rows are
+    // normalised their right part is brought up to date with the strip's earlier panels (the catch-up product, row
+    // offset and count read from the panel record on the device), and their rows of L are zeroed so the strip-wide
+    // product does not apply those panels twice.  Row exchanges move the rows of L with the rows of A.
+    const int rw = (int)std::max<int64_t>(FW, std::min<int64_t>(RW, options().f64_rref_strip / FW * FW));
+    for (int64_t s0 = 0; s0 < cols; s0 += rw) {
+        const int64_t s1 = std::min<int64_t>(cols, s0 + rw), nright = cols - s1;
+        if (nright > 0 && rw > FW) {
+            LINAC_CUDA(cudaMemsetAsync(L, 0, (size_t)rows * RW * 8, s));
+            LINAC_CUDA(cudaMemsetAsync(U, 0, (size_t)RW * ldu * 8, s));
+        }
+        const bool deferred = nright > 0 && rw > FW;       // else every panel updates all the columns right of it at once
+        for (int64_t j0 = s0; j0 < s1; j0 += FW) {
+            int w = (int)std::min<int64_t>(FW, cols - j0);
+            const int poff = (int)(j0 - s0);
+            int64_t j0v = j0, nv = rows, ldv = ld;
+            const int64_t nc = (deferred ? s1 : cols) - j0;
+            unsigned tag0 = options().f64_panel_tags != 0 ? (unsigned)(j0 + 1) : 0u;
+            void* args[] = {&dA, &nv, &ldv, &j0v, &w, &rows_per_cta, &tolv, &cand, &target, &ipiv, &info, &tag0, &state, &rec, &d_piv};
+            LINAC_CUDA(cudaLaunchCooperativeKernel((void*)f64_panel_kernel<512, false, true>, dim3(c.grid), dim3(512), args, smem, s));
+            f64_rref_swap_kernel<<<(unsigned)((cols - j0 + 31) / 32), 256, 0, s>>>(dA, ld, j0, cols, rec, ipiv);
+            st.kernel_launches += 2;
+            double* Up = deferred ? U + (size_t)poff * ldu : U;
+            if (deferred && poff > 0) {
+                f64_rref_swap_kernel<<<(unsigned)((poff + 31) / 32), 256, 0, s>>>(L, RW, 0, poff, rec, ipiv);
+                st.kernel_launches++;
+                rc = dgemm_sub(c, dA + s1, ld, L, RW, U + s1, ldu, FW, nright, poff, false, nullptr, &rec->r, &rec->i0);
+                if (rc) return rc;
+            }
+            f64_rref_tinv_kernel<<<1, 128, 0, s>>>(dA, ld, j0, rec, Tb);
+            f64_rref_pivot_rows_kernel<<<(unsigned)((cols - j0 + 127) / 128), 128, 0, s>>>(dA, ld, j0, cols, rec, Tb, Up, ldu);
+            f64_rref_lcopy_kernel<<<(unsigned)std::min<int64_t>((rows + 7) / 8, 148 * 8), 256, 0, s>>>(dA, ld, rows, j0, rec,
+                                                                                                      L, deferred ? RW : FW, deferred ? poff : 0);
+            LINAC_CUDA(cudaGetLastError());
+            st.kernel_launches += 3;
+            st.panels++;
+            rc = dgemm_sub(c, dA + j0, ld, deferred ? L + poff : L, deferred ? RW : FW, Up + j0, ldu, rows, nc, FW, false, &rec->r);
+            if (rc) return rc;
+        }
+        if (deferred) {
+            rc = dgemm_sub(c, dA + s1, ld, L, RW, U + s1, ldu, rows, nright, s1 - s0);
+            if (rc) return rc;
+        }
     }
     f64_rref_finalize_kernel<<<(unsigned)rows, 256, 0, s>>>(dA, ld, rows, cols, state, d_piv);
     LINAC_CUDA(cudaGetLastError());

@@ -594,6 +594,7 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     if (p >= (1u << 31)) return rref_u32_wide(dA, rows, cols, ld, p, s, rank, pivot_cols_out, arena);
 
     Context& cx = ctx();
+    cx.bind_device(current_device());
     if (!cx.mail) {
         LINAC_CUDA(cudaHostAlloc(&cx.mail, MAXBP * MAIL_WORDS * sizeof(unsigned long long), cudaHostAllocMapped | cudaHostAllocPortable));
         memset(cx.mail, 0, MAXBP * MAIL_WORDS * sizeof(unsigned long long));

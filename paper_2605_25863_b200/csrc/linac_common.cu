@@ -29,6 +29,21 @@ Context::~Context() {
     cudaGetLastError();
 }
 
+void Context::bind_device(int dev) {
+    if (res_dev == dev) return;
+    if (res_dev >= 0) {                       // events and streams belong to the device they were created on
+        int cur = -1;
+        cudaGetDevice(&cur);
+        cudaSetDevice(res_dev);
+        for (cudaEvent_t& e : events) { if (e) cudaEventDestroy(e); e = nullptr; }
+        events.clear();
+        for (cudaEvent_t& e : la_ev) { if (e) cudaEventDestroy(e); e = nullptr; }
+        if (la_stream) { cudaStreamDestroy(la_stream); la_stream = nullptr; }
+        if (cur >= 0) cudaSetDevice(cur);
+    }
+    res_dev = dev;
+}
+
 int acquire_field_slot() {
     Context& c = ctx();
     if (c.slot >= 0) return c.slot;
@@ -258,6 +273,9 @@ int linac_set_option(const char* name, int64_t value) {
     } else if (!strcmp(name, "f64_panel_tags")) {
         if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
         g_options.f64_panel_tags = value;
+    } else if (!strcmp(name, "f64_rref_strip")) {
+        if (value < 32 || value > 128 || value % 32) return LINAC_ERR_INVALID_ARG;
+        g_options.f64_rref_strip = value;
     } else if (!strcmp(name, "f64_rhs_inv")) {
         if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
         g_options.f64_rhs_inv = value;

@@ -49,6 +49,7 @@ struct Options {
     int64_t f64_panel_threads = 512, f64_panel_grid = 0;   // fp64 panel kernel: block size (256/512/1024), grid (0 = one CTA per SM)
     int64_t f64_panel_cluster = 0;    // fp64 panel: CTAs of the thread-block cluster that factors strips which fit its shared memory (0 = off)
     int64_t f64_cluster_rows = 128;   // ... up to this many rows per CTA (beyond it the per-column shared-memory traffic of one SM costs more than the grid barrier)
+    int64_t f64_rref_strip = 128;     // linac_rref_f64: columns per strip (the K of the update right of the strip); 32 = every panel updates everything
     int64_t f64_panel_tags = 1;       // fp64 panel: 1 = tagged candidate records replace the per-column grid barrier, 0 = grid.sync
     int64_t f64_rhs_inv = 1;  // fp64 substitution on B: 1 = blocked with inverted diagonal blocks, 0 = recursive leaf solves
     int64_t tc_panel = 1;     // 1 = K <= 256 updates use the persistent A-stationary tensor kernel
@@ -76,6 +77,8 @@ struct Context {
     int slot = -1;                            // index into the __constant__ ModP table of fp_strip.cuh
     cudaStream_t la_stream = nullptr;         // second stream of the look-ahead schedule (created on first use)
     cudaEvent_t la_ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    int res_dev = -1;                         // device the events / second stream above belong to
+    void bind_device(int dev);                // drops them when the thread has moved to another device
     char cuda_error[1024] = {0};
     ~Context();
 };

@@ -135,3 +135,25 @@ def test_large_rank_deficient(oracle):
     a = gen.normal_matrix(2100, 700, 21) @ gen.normal_matrix(700, 2500, 22)
     _, rank, _ = check(oracle, a, recon_tol=1e-9)
     assert rank == 700
+
+
+@pytest.mark.parametrize("strip", [32, 64, 96, 128])
+def test_strip_widths_against_the_oracle(oracle, strip):
+    """Strips of 32 (every panel updates everything), 64, 96 and 128 columns: the deferred K = strip update right of the
+    strip, the catch-up product on the pivot rows and the exchanged rows of the L stack, on shapes with ragged last
+    strips, free columns inside strips (rank-deficient products) and row exchanges in every panel."""
+    import paper_2605_25863_b200 as L
+    cases = [gen.normal_matrix(520, 130, 31) @ gen.normal_matrix(130, 777, 32),       # free columns from column ~130 on
+             gen.normal_matrix(300, 300, 33),                                         # full rank: the RREF is the identity
+             gen.normal_matrix(450, 449, 34) @ gen.normal_matrix(449, 600, 35)]       # nearly every column a pivot
+    # free columns in the middle of strips: duplicate / zero some columns of a full-rank matrix
+    b = gen.normal_matrix(400, 400, 36)
+    b[:, 5::7] = 0.0
+    b[:, 130:170] = b[:, 10:50] * 3.0
+    cases.append(b)
+    try:
+        L.set_option("f64_rref_strip", strip)
+        for a in cases:
+            check(oracle, a, recon_tol=1e-9)
+    finally:
+        L.set_option("f64_rref_strip", 128)
