@@ -575,9 +575,9 @@ class Bench:
         ms = float(np.mean(times))
         imad, mhz = self.peak("imad_wide", 20.0)
         macs = float(st["update_macs"])
-        # instruction budget per field multiply-accumulate of the Montgomery update (cuobjdump of wide_update_kernel):
-        # u32: 2 IMAD.WIDE + 1 IMAD + ~5 ALU; u64: 4 x (mul.lo + mul.hi pairs = ~16 IMAD) + carries
-        per_mac = 3.0 if which == "u32" else 16.0
+        # instruction budget per field multiply-accumulate of the lazily reduced update (cuobjdump of wide_update_kernel's
+        # inner loop): u32: IMAD.WIDE with carry-out + IMAD.X; u64: the 128-bit product (5 IMAD.WIDE + 2 IMAD) + 2 IMAD.X/IADD
+        per_mac = 2.0 if which == "u32" else 9.0
         del a0, a
         torch.cuda.empty_cache()
         return {"workload": f"wide_{which}: {n}x{n} dense uniform, p={p}", "ms_per_call": ms, "rank": int(rk),
@@ -588,7 +588,8 @@ class Bench:
                              "frac": macs * per_mac / (ms * 1e-3) / 1e12 / imad,
                              "peak_source": "measured live by linac_measure_peak('imad_wide')",
                              "note": f"achieved = executed field MACs (rows x cols-from-panel x 32 per panel, Gauss-Jordan over all "
-                                     f"rows) x {per_mac:g} IMAD-class instructions per Montgomery multiply-accumulate / whole call"}}
+                                     f"rows) x {per_mac:g} IMAD-class instructions per multiply-accumulate (raw products summed in a 96 / 192-bit "
+                                     f"accumulator, one Montgomery reduction per output and panel) / whole call"}}
 
 
 def main():

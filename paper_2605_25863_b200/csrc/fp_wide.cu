@@ -49,6 +49,22 @@ struct F32W {                    // uint32 storage, odd p < 2^32, R = 2^32
     __device__ __forceinline__ T add(T a, T b) const { const uint64_t s = (uint64_t)a + b; return (T)(s >= p ? s - p : s); }
     __device__ __forceinline__ T sub(T a, T b) const { return a >= b ? a - b : a + (p - b); }   // a + (p - b) < p
     __device__ __forceinline__ T canon(T a) const { return a >= p ? a % p : a; }
+    // Lazy dot product: the raw 64-bit products are summed in a 96-bit accumulator (two instructions per term: an
+    // IMAD.WIDE with carry-out and the carry into the top word -- what the compiler makes of the 128-bit sum, whose
+    // top 32 bits are never read) and reduced once -- sum_t mul(l_t, u_t) without a reduction per term.
+    struct Acc { unsigned __int128 v; };
+    __device__ __forceinline__ void acc_zero(Acc& c) const { c.v = 0; }
+    __device__ __forceinline__ void acc_mac(Acc& c, T a, T b) const { c.v += (uint64_t)a * b; }
+    // (a2 2^64 + a1 2^32 + a0) R^-1 mod p, R = 2^32: one Montgomery step on (a1 : a0) leaves u < 2^33, and
+    // u mod p = mul(mul(u_lo, R^2), 1), 2^32 k mod p = mul(k, R^2) for the small k = a2 + (u >> 32)
+    __device__ __forceinline__ T acc_reduce(const Acc& c) const {
+        const uint32_t a0 = (uint32_t)c.v, a1 = (uint32_t)(c.v >> 32), a2 = (uint32_t)(c.v >> 64);
+        const uint32_t m = a0 * ninv;
+        const uint64_t u = (uint64_t)a1 + (((uint64_t)m * p) >> 32) + (a0 != 0u ? 1u : 0u);
+        const T x = mul(mul((T)u, r2), 1u);
+        const T w = mul((T)(a2 + (uint32_t)(u >> 32)), r2);
+        return add(x, w);
+    }
 };
 struct F64M {                    // uint64 storage, odd p < 2^63, R = 2^64
     using T = unsigned long long;
@@ -62,6 +78,23 @@ struct F64M {                    // uint64 storage, odd p < 2^63, R = 2^64
     __device__ __forceinline__ T add(T a, T b) const { const T s = a + b; return s >= p ? s - p : s; }   // p < 2^63
     __device__ __forceinline__ T sub(T a, T b) const { return a >= b ? a - b : a + (p - b); }
     __device__ __forceinline__ T canon(T a) const { return a >= p ? a % p : a; }
+    // Lazy dot product in a 192-bit accumulator (see F32W), R = 2^64.
+    struct Acc { unsigned long long a0, a1, a2; };
+    __device__ __forceinline__ void acc_zero(Acc& c) const { c.a0 = c.a1 = c.a2 = 0ull; }
+    __device__ __forceinline__ void acc_mac(Acc& c, T a, T b) const {
+        const T lo = a * b, hi = __umul64hi(a, b);
+        asm("add.cc.u64 %0, %0, %3;\n\taddc.cc.u64 %1, %1, %4;\n\taddc.u64 %2, %2, 0;"
+            : "+l"(c.a0), "+l"(c.a1), "+l"(c.a2) : "l"(lo), "l"(hi));
+    }
+    __device__ __forceinline__ T acc_reduce(const Acc& c) const {
+        const T m = c.a0 * ninv;
+        T u = c.a1 + __umul64hi(m, p);                     // (a1 : a0 + m p) / 2^64, up to 65 bits
+        unsigned long long ov = u < c.a1 ? 1ull : 0ull;
+        if (c.a0 != 0ull) { u += 1ull; ov += u == 0ull ? 1ull : 0ull; }
+        const T x = mul(mul(u, r2), 1ull);                 // u mod p (mul takes any 64-bit first factor)
+        const T w = mul(c.a2 + ov, r2);                    // 2^64 k mod p
+        return add(x, w);
+    }
 };
 template <class F> __device__ __forceinline__ typename F::T to_mont(const F& f, typename F::T a) { return f.mul(f.canon(a), f.r2); }
 template <class F> __device__ __forceinline__ typename F::T from_mont(const F& f, typename F::T a) { return f.mul(a, 1); }
@@ -263,8 +296,11 @@ __global__ void __launch_bounds__(128) wide_pivot_rows_kernel(typename F::T* __r
     for (int a = 0; a < WP; ++a) {
         T acc = 0;
         if (a < r) {
+            typename F::Acc s;
+            f.acc_zero(s);
 #pragma unroll
-            for (int b = 0; b < WP; ++b) acc = f.add(acc, f.mul(Ts[a][b], x[b]));
+            for (int b = 0; b < WP; ++b) f.acc_mac(s, Ts[a][b], x[b]);
+            acc = f.acc_reduce(s);
             A[(i0 + a) * ld + c] = acc;
         }
         U[(int64_t)a * ldu + c] = acc;
@@ -307,16 +343,17 @@ __global__ void __launch_bounds__(256) wide_update_kernel(typename F::T* __restr
         Us[t][nn] = (t < r && n0 + nn < cols) ? U[(int64_t)t * ldu + n0 + nn] : (T)0;
     }
     __syncthreads();
-    T acc[4][4];
+    typename F::Acc acc[4][4];
 #pragma unroll
     for (int i = 0; i < 4; ++i)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j] = 0;
+        for (int j = 0; j < 4; ++j) f.acc_zero(acc[i][j]);
     bool any = false;
 #pragma unroll
     for (int i = 0; i < 4; ++i)
         for (int t = 0; t < r; ++t) any = any || Ls[ty * 4 + i][t] != 0;
     if (!any) return;                                   // conditional skipping: rows with zero heads
+#pragma unroll 2
     for (int t = 0; t < r; ++t) {
         T l[4], u[4];
 #pragma unroll
@@ -326,7 +363,7 @@ __global__ void __launch_bounds__(256) wide_update_kernel(typename F::T* __restr
 #pragma unroll
         for (int i = 0; i < 4; ++i)
 #pragma unroll
-            for (int j = 0; j < 4; ++j) acc[i][j] = f.add(acc[i][j], f.mul(l[i], u[j]));
+            for (int j = 0; j < 4; ++j) f.acc_mac(acc[i][j], l[i], u[j]);
     }
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
@@ -335,7 +372,7 @@ __global__ void __launch_bounds__(256) wide_update_kernel(typename F::T* __restr
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const int64_t c = n0 + tx + 16 * j;
-            if (c < cols) A[m * ld + c] = f.sub(A[m * ld + c], acc[i][j]);
+            if (c < cols) A[m * ld + c] = f.sub(A[m * ld + c], f.acc_reduce(acc[i][j]));
         }
     }
 }
