@@ -402,14 +402,17 @@ class Bench:
                 return e0.elapsed_time(e1), rk
 
             def run_pipelined(k_steps):
-                """K end-to-end steps, double buffered: while the call of step k runs, the pinned H2D of step k+1 and the
+                """K end-to-end steps, pipelined: while the call of step k runs, the pinned H2D of step k+1 and the
                 D2H of step k-1 are in flight on their own streams; every step's copies are inside the timed region."""
                 s_c, s_in, s_out = torch.cuda.Stream(dev), torch.cuda.Stream(dev), torch.cuda.Stream(dev)
-                bufs = [d_work, torch.empty_like(d_work)]
+                # three device buffers: with two, the D2H of step k-1 and the H2D of step k+1 use the same buffer one after
+                # the other and their sum (14 ms at c3), not the call (13.5 ms), sets the period
+                NB = 3
+                bufs = [d_work] + [torch.empty_like(d_work) for _ in range(NB - 1)]
                 outs = [out_host, torch.empty_like(out_host).pin_memory()]
-                ev_in = [torch.cuda.Event(), torch.cuda.Event()]
-                ev_done = [torch.cuda.Event(), torch.cuda.Event()]
-                ev_out = [torch.cuda.Event(), torch.cuda.Event()]
+                ev_in = [torch.cuda.Event() for _ in range(NB)]
+                ev_done = [torch.cuda.Event() for _ in range(NB)]
+                ev_out = [torch.cuda.Event() for _ in range(NB)]
                 t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 torch.cuda.synchronize(dev)
                 t0.record(s_in)
@@ -418,11 +421,11 @@ class Bench:
                     ev_in[0].record(s_in)
                 rk = None
                 for k in range(k_steps):
-                    b = k % 2
+                    b = k % NB
                     if k + 1 < k_steps:
-                        nb = (k + 1) % 2
-                        if k >= 1:
-                            s_in.wait_event(ev_out[nb])
+                        nb = (k + 1) % NB
+                        if k + 1 >= NB:
+                            s_in.wait_event(ev_out[nb])                 # the D2H of step k + 1 - NB has left this buffer
                         with torch.cuda.stream(s_in):
                             bufs[nb].copy_(pinned, non_blocking=True)
                             ev_in[nb].record(s_in)
@@ -432,7 +435,7 @@ class Bench:
                         ev_done[b].record(s_c)
                     s_out.wait_event(ev_done[b])
                     with torch.cuda.stream(s_out):
-                        outs[b].copy_(bufs[b], non_blocking=True)
+                        outs[k % 2].copy_(bufs[b], non_blocking=True)
                         ev_out[b].record(s_out)
                 t1.record(s_out)
                 t1.synchronize()
@@ -452,8 +455,8 @@ class Bench:
             e2e_ms = replicas.max_over_ranks(float(e2e_ms), dev)
             leg["e2e"] = {"value": replicas.aggregate_throughput(nominal, e2e_ms * 1e-3, self.world) / 1e9, "unit": "Gmulmod/s",
                           "ms_per_step": e2e_ms, "h2d_bytes_per_step": int(nbytes), "d2h_bytes_per_step": int(nbytes),
-                          "mode": "double-buffered: the pinned H2D of step k+1 and the D2H of step k-1 overlap the call of "
-                                  "step k; every step's copies are inside the timed region",
+                          "mode": "pipelined over three device buffers: the pinned H2D of step k+1 and the D2H of step k-1 overlap "
+                                  "the call of step k; every step's copies are inside the timed region",
                           "serial_ms_per_step": serial_ms,
                           "serial_value": replicas.aggregate_throughput(nominal, serial_ms * 1e-3, self.world) / 1e9}
         else:
@@ -608,6 +611,8 @@ def main():
     ap.add_argument("--cpu-baseline", default="bounded", choices=["bounded", "full"])
     ap.add_argument("--no-f64", action="store_true", help="skip the fp64 legs")
     ap.add_argument("--fp64-only", action="store_true", help="run only legs.fp64_solve and print {\"fp64\": ...}")
+    ap.add_argument("--only-leg", default="", choices=["", "rref_f64", "wide_u32", "wide_u64"],
+                    help="run only this leg of the widened rows (SURVEY.md 8(f)) and print {name: ...}; for profiles")
     ap.add_argument("--gemm", default=None, metavar="M,N,K[,path]",
                     help="time the S5 primitive linac_gemm_sub_u32 alone (C -= A.B mod 2^31-1, path 2 = tensor cores by default) "
                          "and print {\"gemm\": ...}; the command of the GEMM ncu captures under profiles/")
@@ -688,6 +693,13 @@ def main():
     if args.fp64_only:
         if rank == 0:
             print(json.dumps({"fp64": B.f64_solve_leg(reps=max(1, min(args.steps, 5)))}))
+        return
+    if args.only_leg:
+        if rank == 0:
+            reps = max(1, min(args.steps, 3))
+            leg = {"rref_f64": lambda: B.rref_f64_leg(reps=reps), "wide_u32": lambda: B.wide_leg("u32", reps=reps),
+                   "wide_u64": lambda: B.wide_leg("u64", reps=reps)}[args.only_leg]()
+            print(json.dumps({args.only_leg: leg}))
         return
 
     headline = "c3" if args.workload == "all" else args.workload
