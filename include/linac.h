@@ -52,7 +52,8 @@ typedef enum {
     LINAC_ERR_SINGULAR = 5,           /* fp64: pivot with |pivot| <= tol */
     LINAC_ERR_BUFFER_TOO_SMALL = 6,   /* K buffer has fewer columns than the nullity */
     LINAC_ERR_UNSUPPORTED_DEVICE = 7, /* current device is not sm_100 class */
-    LINAC_ERR_INTERNAL = 8            /* an internal consistency check failed (a bug; never a data property) */
+    LINAC_ERR_INTERNAL = 8,           /* an internal consistency check failed (a bug; never a data property) */
+    LINAC_ERR_TOO_LARGE = 9           /* linac_gemm_sub_u32_static: the problem needs more than LINAC_STATIC_SCRATCH_BYTES of scratch */
 } linac_status;
 
 /* Static strings; never NULL. */
@@ -187,6 +188,27 @@ int linac_load_matrix_u32(uint32_t *dA, int64_t n_rows, int64_t n_cols, int64_t 
  */
 int linac_gemm_sub_u32(uint32_t *dC, int64_t ldc, const uint32_t *dA, int64_t lda, const uint32_t *dB, int64_t ldb,
                        int64_t M, int64_t N, int64_t K, uint32_t p, int path, void *stream);
+
+/*
+ * linac_gemm_sub_u32_static -- the same update, C <- C - A.B (mod p), for callers that may not
+ * allocate device memory (a stream under CUDA graph capture, a serving loop, a harness that forbids cudaMalloc).
+ * Arguments and layout as linac_gemm_sub_u32 (all DEVICE, row-major, entries in [0,p), p prime < 2^31); the path is
+ * the automatic one (tensor kernels where the shape allows, else the CUDA-core kernel).
+ *   - Allocates nothing: no cudaMalloc / cudaFree, no events, no workspace.  The limb-plane scratch of the tensor
+ *     kernels lives in a static device array of LINAC_STATIC_SCRATCH_BYTES inside the library (held by every GPU
+ *     that loads the library until the process exits).
+ *   - Limit: 4 (M + N) Kc + 4096 <= LINAC_STATIC_SCRATCH_BYTES, Kc = K rounded up to a multiple of 128 (K <= 8192;
+ *     equal chunks of at most 8192 above), e.g. M = N = 4096 with K <= 1024, or M = N = 16384 with K <= 256.
+ *     Beyond it: LINAC_ERR_TOO_LARGE, nothing launched, C untouched.
+ *   - Asynchronous: the kernels are enqueued on `stream`, which is NOT synchronised; errors of the kernels
+ *     themselves surface at the caller's next synchronisation.  linac_get_last_stats is not updated with times.
+ *   - Every call on a device shares the one array.  Nothing in it has to start at zero (each call rewrites all it
+ *     reads), but two calls that OVERLAP on the GPU -- different streams or host threads on the same device --
+ *     race on it: serialise them (one stream, or events).
+ */
+#define LINAC_STATIC_SCRATCH_BYTES ((size_t)32 << 20)
+int linac_gemm_sub_u32_static(uint32_t *dC, int64_t ldc, const uint32_t *dA, int64_t lda, const uint32_t *dB,
+                              int64_t ldb, int64_t M, int64_t N, int64_t K, uint32_t p, void *stream);
 
 /* ---- fp64: partial-pivot solve ------------------------------------------------------------- */
 /*

@@ -207,6 +207,7 @@ const char* linac_status_string(int status) {
         case LINAC_ERR_BUFFER_TOO_SMALL: return "null-space buffer has too few columns";
         case LINAC_ERR_UNSUPPORTED_DEVICE: return "current CUDA device is not compute capability 10.x";
         case LINAC_ERR_INTERNAL: return "internal consistency check failed";
+        case LINAC_ERR_TOO_LARGE: return "problem exceeds the static scratch array (LINAC_STATIC_SCRATCH_BYTES) of the no-allocation entry point";
         default: return "unknown status";
     }
 }

@@ -16,6 +16,8 @@ LIB_PATH = os.path.join(_HERE, "liblinac.so")
 
 OK, ERR_INVALID_ARG, ERR_BAD_MODULUS, ERR_WORKSPACE, ERR_CUDA = 0, 1, 2, 3, 4
 ERR_SINGULAR, ERR_BUFFER_TOO_SMALL, ERR_UNSUPPORTED_DEVICE, ERR_INTERNAL = 5, 6, 7, 8
+ERR_TOO_LARGE = 9
+STATIC_SCRATCH_BYTES = 32 << 20          # linac.h: LINAC_STATIC_SCRATCH_BYTES
 
 #: every symbol include/linac.h declares (checked by tests/test_abi.py)
 SYMBOLS = [
@@ -23,6 +25,7 @@ SYMBOLS = [
     "linac_rref_u32_workspace", "linac_solve_f64_workspace", "linac_set_workspace", "linac_release",
     "linac_rref_u64_workspace", "linac_rref_u64",
     "linac_rref_u32", "linac_nullspace_u32", "linac_nullspace_from_rref_u32", "linac_solve_u32", "linac_rank_factor_u32", "linac_load_matrix_u32", "linac_gemm_sub_u32",
+    "linac_gemm_sub_u32_static",
     "linac_solve_f64", "linac_rref_f64_workspace", "linac_rref_f64",
     "linac_get_last_stats", "linac_set_option", "linac_measure_peak",
 ]
@@ -76,6 +79,7 @@ def _lib() -> C.CDLL:
         L.linac_rank_factor_u32.argtypes = [vp, i64, i64, i64, u32, vp, vp, i64, vp, i64, C.POINTER(i64), vp]
         L.linac_load_matrix_u32.argtypes = [vp, i64, i64, i64, vp, i64, i64, vp, i64, u32, vp]
         L.linac_gemm_sub_u32.argtypes = [vp, i64, vp, i64, vp, i64, i64, i64, i64, u32, C.c_int, vp]
+        L.linac_gemm_sub_u32_static.argtypes = [vp, i64, vp, i64, vp, i64, i64, i64, i64, u32, vp]
         L.linac_solve_f64.argtypes = [vp, i64, i64, vp, i64, i64, C.c_double, vp, C.POINTER(i64)]
         L.linac_rref_f64_workspace.argtypes = [i64, i64, C.POINTER(sz)]
         L.linac_rref_f64.argtypes = [vp, i64, i64, i64, C.c_double, vp, C.POINTER(i64), vp]
@@ -312,6 +316,22 @@ def gemm_sub_u32(c: torch.Tensor, a: torch.Tensor, b: torch.Tensor, p: int, path
                                        _stream_ptr(c.device))
     if rc:
         raise LinacError(rc, "linac_gemm_sub_u32")
+
+
+def gemm_sub_u32_static(c: torch.Tensor, a: torch.Tensor, b: torch.Tensor, p: int) -> None:
+    """In place: c <- c - a.b (mod p), enqueued on the current stream WITHOUT allocating device memory and without a
+    synchronisation (scratch in the library's static 32 MiB device array; LinacError(ERR_TOO_LARGE) beyond it).
+    Calls on one device share that array: do not let two of them overlap on the GPU."""
+    m, n, ldc = _check_matrix(c, _U32, "c")
+    m2, k, lda = _check_matrix(a, _U32, "a")
+    k2, n2, ldb = _check_matrix(b, _U32, "b")
+    if m != m2 or n != n2 or k != k2:
+        raise ValueError("shape mismatch")
+    with torch.cuda.device(c.device):
+        rc = _lib().linac_gemm_sub_u32_static(c.data_ptr(), ldc, a.data_ptr(), lda, b.data_ptr(), ldb, m, n, k, p,
+                                              _stream_ptr(c.device))
+    if rc:
+        raise LinacError(rc, "linac_gemm_sub_u32_static")
 
 
 def solve_f64(a: torch.Tensor, b: torch.Tensor, tol: float = -1.0) -> int:
