@@ -17,6 +17,8 @@
 
 #include "fp_kernels.cuh"
 #include "fp_strip.cuh"
+#include "tc_ptx.cuh"
+#include "fp_trsm_inv.cuh"
 
 namespace linac {
 
@@ -38,6 +40,7 @@ struct Fp {
     PanelRec* d_rec;          // [nb]
     uint32_t* d_T;            // [nb][PW*PW]
     uint32_t* d_E;            // [nb][PW*PW]
+    uint8_t* d_W = nullptr;   // [4][WK][WK] limb planes of the current regular strip's solve operator (fp_trsm_inv.cuh)
     Arena* arena;
     // host
     unsigned long long* h_mail;      // mapped pinned, MAXBP * MAIL_WORDS tagged words written by the strip kernel itself
@@ -160,6 +163,10 @@ struct StripLaunch {
     unsigned long long seq = 0;
     int64_t b0 = 0, b1 = 0, j0 = 0, j1 = 0;
     cudaStream_t stream = nullptr;
+    bool winv = false;        // strip_winv_kernel was enqueued behind the strip kernel (it writes W only for a regular strip)
+    // filled by collect_strip
+    int64_t nswaps = 0;       // row exchanges of the strip's panels that found pivots
+    bool regular = false;     // four base panels with 32 pivots each
 };
 
 // Launches the cooperative strip kernel for strip s (active rows >= i0) on `stream` with `grid` CTAs.
@@ -192,7 +199,7 @@ int launch_strip(Fp& c, int64_t s, int64_t i0, cudaStream_t stream, int grid, bo
 }
 
 // Waits for the mail of a launched strip (it may arrive before the kernel has ended) and records its pivots.
-int collect_strip(Fp& c, const StripLaunch& L, int64_t i0, int64_t* r) {
+int collect_strip(Fp& c, StripLaunch& L, int64_t i0, int64_t* r) {
     linac_stats& st = stats();
     {
         volatile unsigned long long* mailbox = c.h_mail;
@@ -213,17 +220,32 @@ int collect_strip(Fp& c, const StripLaunch& L, int64_t i0, int64_t* r) {
     }
     st.host_syncs++;
     int64_t cur = i0;
+    L.nswaps = 0;
+    L.regular = L.b1 - L.b0 == WK / PW;
     for (int64_t b = L.b0; b < L.b1; ++b) {
         const unsigned long long* m = c.h_mail + (b - L.b0) * MAIL_WORDS;
         const int32_t hr = (int32_t)(uint32_t)m[0], hns = (int32_t)(uint32_t)m[1];
         if (hr < 0 || hr > PW || cur + hr > c.rows) return LINAC_ERR_INTERNAL;
         st.panels++;
         st.row_swaps += hr > 0 ? hns : 0;
+        L.nswaps += hr > 0 ? hns : 0;
+        L.regular = L.regular && hr == PW;
         for (int q = 0; q < hr; ++q) c.pivcols[cur + q] = (int32_t)(panel_col0(b) + (int32_t)(uint32_t)m[2 + q]);
         cur += hr;
         c.pstart[b + 1] = cur;
     }
     *r = cur - i0;
+    return LINAC_OK;
+}
+
+// Enqueues strip_winv_kernel behind a strip kernel: W = the strip's solve operator, if the strip turns out regular.
+int launch_winv(Fp& c, StripLaunch& L, cudaStream_t stream) {
+    if (options().trsm_winv == 0 || c.d_W == nullptr || L.b1 - L.b0 != WK / PW || L.j1 - L.j0 != WK) return LINAC_OK;
+    Timed tm(c, stats().ms_trsm, 2, stream);
+    strip_winv_kernel<<<WINV_CTAS, WINV_NT, sizeof(WinvSmem), stream>>>(c.A, c.ld, c.d_pstart, (int)L.b0, c.d_T, c.d_pivcols, c.f, c.d_W);
+    LINAC_CUDA(cudaGetLastError());
+    stats().kernel_launches++;
+    L.winv = true;
     return LINAC_OK;
 }
 
@@ -235,6 +257,15 @@ int launch_strip_solve(Fp& c, const StripLaunch& L, int64_t i0, int64_t c0, int6
     if (ncols <= 0) return LINAC_OK;
     if (!stream) stream = c.s;
     Timed tm(c, stats().ms_trsm, 2, stream);
+    if (L.winv && L.regular && !mail && (Bq == nullptr || kp == WK)) {          // one dense product with the strip's W
+        const int64_t ntiles = (ncols + WTN - 1) / WTN;
+        trsm_winv_kernel<<<(unsigned)std::min<int64_t>(ntiles, 2 * sm_count()), WNT, WTRSM_SMEM, stream>>>(
+            c.d_W, c.A + i0 * c.ld + c0, c.ld, ncols, c.f, Bq, kp, bq_col0, bq_total > 0 ? bq_total : ncols);
+        LINAC_CUDA(cudaGetLastError());
+        stats().kernel_launches++;
+        stats().winv_solves++;
+        return LINAC_OK;
+    }
     trsm_strip_kernel<true><<<(unsigned)((ncols + PW - 1) / PW), TNT, trsm_smem_bytes(L.j1 - L.j0), stream>>>(
         c.A, c.ld, c.A + i0 * c.ld + c0, c.ld, ncols, c.d_pstart, (int)L.b0, (int)L.b1, c.d_T, c.d_pivcols, c.f, Bq, kp,
         mail ? c.h_mail : nullptr, L.seq, c.d_rec, bq_col0, bq_total > 0 ? bq_total : ncols);
@@ -322,6 +353,8 @@ int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jen
     bool la_launched = false;                                  // was the strip in L launched as a look-ahead strip?
     int rc = launch_strip(c, s0, cur, c.s, c.coop_grid, false, true, Aq[s0 & 1], kp, &L);
     if (rc) return rc;
+    rc = launch_winv(c, L, c.s);
+    if (rc) return rc;
     int64_t r = 0;
     rc = collect_strip(c, L, cur, &r);
     if (rc) return rc;
@@ -331,7 +364,7 @@ int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jen
         if (la_launched) {
             LINAC_CUDA(cudaStreamWaitEvent(c.s, ev_strip, 0));
             const int64_t ncol_out = c.cols - (L.j1 - L.j0);
-            if (ncol_out > 0) {
+            if (ncol_out > 0 && L.nswaps > 0) {                // the host has the strip's records: no exchanges, no launch
                 deferred_swaps_kernel<<<(unsigned)((ncol_out + 255) / 256), 256, 0, c.s>>>(c.A, c.ld, c.cols, L.j0, L.j1, c.d_rec,
                                                                                          c.d_pstart, (int)L.b0, (int)(L.b1 - L.b0));
                 LINAC_CUDA(cudaGetLastError());
@@ -382,6 +415,8 @@ int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jen
                 LINAC_CUDA(cudaEventRecord(ev_narrow, c.s));
                 rc = launch_strip(c, s + 1, cur + r, c.s, la_grid, true, true, Aq[(s + 1) & 1], kp, &Ln);
                 if (rc) return rc;
+                rc = launch_winv(c, Ln, c.s);                                       // needs the strip's own columns only
+                if (rc) return rc;
                 next_launched = true;
                 stats().lookahead_strips++;
                 LINAC_CUDA(cudaStreamWaitEvent(sB, ev_narrow, 0));
@@ -408,6 +443,8 @@ int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jen
         }
         if (!next_launched) {
             rc = launch_strip(c, s + 1, cur, c.s, c.coop_grid, false, true, Aq[(s + 1) & 1], kp, &Ln);
+            if (rc) return rc;
+            rc = launch_winv(c, Ln, c.s);
             if (rc) return rc;
         }
         rc = collect_strip(c, Ln, cur, &r);
@@ -536,6 +573,8 @@ int strip_grid(int* grid) {
         LINAC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, strip_factor_kernel, SNT, sizeof(StripSmem)));
         LINAC_CUDA(cudaFuncSetAttribute(trsm_strip_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)trsm_smem_bytes(SW_MAX)));
         LINAC_CUDA(cudaFuncSetAttribute(trsm_strip_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)trsm_smem_bytes(SW_MAX)));
+        LINAC_CUDA(cudaFuncSetAttribute(strip_winv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WinvSmem)));
+        LINAC_CUDA(cudaFuncSetAttribute(trsm_winv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WTRSM_SMEM));
         if (per_sm < 1 || sm_count() < 1) return LINAC_ERR_INTERNAL;
         return LINAC_OK;
     });
@@ -550,7 +589,7 @@ size_t meta_bytes(int64_t rows, int64_t cols) {
     const int64_t mn = std::max<int64_t>(1, std::min(rows, cols));
     const int64_t nb = num_panels(cols);
     // + the index arrays of the consumers that run behind the reduction (null space: 2 cols; solve: cols + nrhs; C.R: rank)
-    return 8192 + (size_t)nb * (sizeof(PanelRec) + 256 + 2 * PW * PW * 4 + 4) + (size_t)mn * 4 + (size_t)cols * 4 + 10 * 256 +
+    return 8192 + (size_t)WK * WK * 4 + 1024 + (size_t)nb * (sizeof(PanelRec) + 256 + 2 * PW * PW * 4 + 4) + (size_t)mn * 4 + (size_t)cols * 4 + 10 * 256 +
            (size_t)cols * 12 + (size_t)mn * 4 + 4096;
 }
 
@@ -616,7 +655,8 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     c.d_pivcols = (int32_t*)arena->take((size_t)mn * 4);
     int32_t* d_colinfo = (int32_t*)arena->take((size_t)cols * 4);
     c.d_pstart = (int32_t*)arena->take((size_t)(c.nb + 1) * 4);
-    if (!c.d_rec || !c.d_T || !c.d_E || !c.d_pivcols || !d_colinfo || !c.d_pstart) return LINAC_ERR_WORKSPACE;
+    c.d_W = (uint8_t*)arena->take((size_t)WK * WK * 4, 1024);
+    if (!c.d_rec || !c.d_T || !c.d_E || !c.d_pivcols || !d_colinfo || !c.d_pstart || !c.d_W) return LINAC_ERR_WORKSPACE;
     LINAC_CUDA(cudaMemsetAsync(c.d_pstart, 0, (size_t)(c.nb + 1) * 4, s));
     c.h_mail = cx.mail;
     c.slot = slot;

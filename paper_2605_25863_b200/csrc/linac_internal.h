@@ -59,6 +59,8 @@ struct Options {
     int64_t lookahead = 1;    // flat sweep: 1 = factor strip s+1 on `la_ctas` SMs (second stream) while the bulk of strip s's
                               // Schur update runs on the other SMs; 0 = strictly sequential
     int64_t la_ctas = 0;      // CTAs (= SMs) of the look-ahead strip kernel; 0 = chosen per strip from a cost model
+    int64_t trsm_winv = 1;    // look-ahead sweep: row-block solve of a regular strip (4 x 32 pivots) as ONE product with the strip's
+                              // explicit 128 x 128 operator W (fp_trsm_inv.cuh); 0 = the panel-by-panel chain kernel everywhere
 };
 Options& options();
 

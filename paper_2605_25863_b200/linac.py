@@ -46,7 +46,7 @@ class Stats(C.Structure):
                 ("ms_update", C.c_double), ("ms_total", C.c_double),
                 ("ms_strip", C.c_double), ("ms_trsm", C.c_double), ("ms_update_top", C.c_double),
                 ("top_m", C.c_int64), ("top_n", C.c_int64), ("top_k", C.c_int64),
-                ("ms_overlap", C.c_double), ("lookahead_strips", C.c_int64)]
+                ("ms_overlap", C.c_double), ("lookahead_strips", C.c_int64), ("winv_solves", C.c_int64)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
