@@ -43,6 +43,67 @@ __device__ __forceinline__ void winv_dot(uint64_t& a0, uint64_t& a1, const uint3
     }
 }
 
+// One CTA's share of W: column block C (compile-time, so that every loop below unrolls and the loads of a thread --
+// up to 40 -- are all in flight together instead of one load-then-store after the other), columns j0..j0+7 of it.
+template <int C>
+__device__ __forceinline__ void winv_body(WinvSmem& sm, const uint32_t* __restrict__ A, int64_t ld, int t0, int b0, int j0,
+                                          const uint32_t* __restrict__ T, const int32_t* __restrict__ pivcols,
+                                          const ModP& f, uint8_t* __restrict__ Wq) {
+    const int tid = threadIdx.x;
+    constexpr int NQ = PW * PW / WINV_NT;                        // elements of a 32 x 32 block per thread
+    const int kk = tid % PW, i0 = tid / PW;                      // element q of the thread: (row i0 + 8 q, column kk)
+    int32_t pc[4];
+#pragma unroll
+    for (int d = C; d < 3; ++d) pc[d] = pivcols[t0 + PW * d + kk];
+    uint32_t tv[4][NQ], lv[6][NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) {
+        const int ii = i0 + (WINV_NT / PW) * q;
+#pragma unroll
+        for (int b = C; b < 4; ++b) {
+            tv[b][q] = T[(int64_t)(b0 + b) * PW * PW + ii * PW + kk];
+#pragma unroll
+            for (int d = C; d < b; ++d) lv[b * (b - 1) / 2 + d][q] = A[(int64_t)(t0 + PW * b + ii) * ld + pc[d]];
+        }
+    }
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) {
+        const int ii = i0 + (WINV_NT / PW) * q;
+#pragma unroll
+        for (int b = C; b < 4; ++b) {
+            sm.Ts[b][ii][kk] = tv[b][q];
+#pragma unroll
+            for (int d = C; d < b; ++d) sm.Ls[b * (b - 1) / 2 + d][ii][kk] = lv[b * (b - 1) / 2 + d][q];
+        }
+    }
+    __syncthreads();
+    const int i = tid / 8, jj = tid % 8;
+    sm.Wc[C][i][jj] = sm.Ts[C][i][j0 + jj];
+    __syncthreads();
+#pragma unroll
+    for (int b = C + 1; b < 4; ++b) {
+        uint64_t a0 = 0, a1 = 0;
+#pragma unroll
+        for (int d = C; d < b; ++d) winv_dot(a0, a1, sm.Ls[b * (b - 1) / 2 + d][i], sm.Wc[d], jj, f);
+        sm.Ys[i][jj] = reduce64(fold64(a0, f) + fold64(a1, f), f);
+        __syncthreads();
+        a0 = a1 = 0;
+        winv_dot(a0, a1, sm.Ts[b][i], sm.Ys, jj, f);
+        const uint32_t v = reduce64(fold64(a0, f) + fold64(a1, f), f);
+        sm.Wc[b][i][jj] = v ? f.p - v : 0u;
+        __syncthreads();
+    }
+    const int k = PW * C + j0 + jj;
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+        const int m = PW * b + i;
+        const uint32_t v = b >= C ? sm.Wc[b][i][jj] : 0u;
+        const int off = m * WK + (((k >> 4) ^ (m & 7)) << 4) + (k & 15);
+#pragma unroll
+        for (int l = 0; l < 4; ++l) Wq[l * WK * WK + off] = (uint8_t)(v >> (8 * l));
+    }
+}
+
 // W for the strip whose first base panel is b0 and whose pivots start at row / pivot index pstart[b0], as the
 // shared-memory image of a K-major tcgen05 operand: Wq[limb][m][128 bytes of k], the 16-byte pieces of a row XOR-ed
 // with m % 8 (SWIZZLE_128B).  The blocks above the diagonal are written as zeros.  Exits without writing when the strip
@@ -55,47 +116,18 @@ __global__ void __launch_bounds__(WINV_NT) strip_winv_kernel(const uint32_t* __r
     extern __shared__ __align__(16) unsigned char winv_smem_raw[];
     WinvSmem& sm = *reinterpret_cast<WinvSmem*>(winv_smem_raw);
     const int t0 = pstart[b0];
-#pragma unroll
-    for (int b = 0; b < 4; ++b)
-        if (pstart[b0 + b + 1] - pstart[b0 + b] != PW) return;
-    const int tid = threadIdx.x;
-    const int c = blockIdx.x / 4;                                // column block of W
+    const int t4 = pstart[b0 + 4], t1 = pstart[b0 + 1], t2 = pstart[b0 + 2], t3 = pstart[b0 + 3];
+    if (t1 - t0 != PW || t2 - t1 != PW || t3 - t2 != PW || t4 - t3 != PW) return;
     const int j0 = 8 * (blockIdx.x % 4);                         // first of this CTA's columns inside the block
-    // everything this CTA needs, in one round of independent loads
-    for (int e = tid; e < PW * PW; e += WINV_NT) {
-        const int ii = e / PW, kk = e % PW;
-        for (int b = c; b < 4; ++b) {
-            sm.Ts[b][ii][kk] = T[(int64_t)(b0 + b) * PW * PW + e];
-            for (int d = c; d < b; ++d)
-                sm.Ls[b * (b - 1) / 2 + d][ii][kk] = A[(int64_t)(t0 + PW * b + ii) * ld + pivcols[t0 + PW * d + kk]];
-        }
-    }
-    __syncthreads();
-    const int i = tid / 8, jj = tid % 8;
-    sm.Wc[c][i][jj] = sm.Ts[c][i][j0 + jj];
-    __syncthreads();
-    for (int b = c + 1; b < 4; ++b) {
-        uint64_t a0 = 0, a1 = 0;
-        for (int d = c; d < b; ++d) winv_dot(a0, a1, sm.Ls[b * (b - 1) / 2 + d][i], sm.Wc[d], jj, f);
-        sm.Ys[i][jj] = reduce64(fold64(a0, f) + fold64(a1, f), f);
-        __syncthreads();
-        a0 = a1 = 0;
-        winv_dot(a0, a1, sm.Ts[b][i], sm.Ys, jj, f);
-        const uint32_t v = reduce64(fold64(a0, f) + fold64(a1, f), f);
-        sm.Wc[b][i][jj] = v ? f.p - v : 0u;
-        __syncthreads();
-    }
-    const int k = PW * c + j0 + jj;
-    for (int b = 0; b < 4; ++b) {
-        const int m = PW * b + i;
-        const uint32_t v = b >= c ? sm.Wc[b][i][jj] : 0u;
-        const int off = m * WK + (((k >> 4) ^ (m & 7)) << 4) + (k & 15);
-#pragma unroll
-        for (int l = 0; l < 4; ++l) Wq[l * WK * WK + off] = (uint8_t)(v >> (8 * l));
+    switch (blockIdx.x / 4) {                                    // column block of W
+        case 0: winv_body<0>(sm, A, ld, t0, b0, j0, T, pivcols, f, Wq); break;
+        case 1: winv_body<1>(sm, A, ld, t0, b0, j0, T, pivcols, f, Wq); break;
+        case 2: winv_body<2>(sm, A, ld, t0, b0, j0, T, pivcols, f, Wq); break;
+        default: winv_body<3>(sm, A, ld, t0, b0, j0, T, pivcols, f, Wq); break;
     }
 }
 
-constexpr int WNT = 128;             // threads of trsm_winv_kernel: four warps = the four TMEM lane quarters
+constexpr int WNT = 256;             // threads of trsm_winv_kernel: eight warps = four TMEM lane quarters x two column halves
 constexpr int WTN = 32;              // columns of X per tile
 constexpr int W_A_BYTES = 4 * WK * WK;           // W limb planes
 constexpr int W_B_BYTES = 4 * WTN * WK;          // limb planes of one X tile, stacked along N
@@ -149,12 +181,13 @@ __global__ void __launch_bounds__(WNT, 2) trsm_winv_kernel(const uint8_t* __rest
             const bool cok = c < ncols;
             const uint32_t* src = X + c;
             const int sw = lane & 7;
-            uint32_t v[32];
+            constexpr int KW = WK / (WNT / 32);                                                    // k per warp
+            uint32_t v[KW];
 #pragma unroll
-            for (int q = 0; q < 32; ++q) v[q] = cok ? src[(int64_t)(32 * warp + q) * ldx] : 0u;     // k = 32 warp + q
+            for (int q = 0; q < KW; ++q) v[q] = cok ? src[(int64_t)(KW * warp + q) * ldx] : 0u;     // k = KW warp + q
 #pragma unroll
-            for (int g = 0; g < 8; ++g) {
-                const int k = 32 * warp + 4 * g;
+            for (int g = 0; g < KW / 4; ++g) {
+                const int k = KW * warp + 4 * g;
                 const int off = lane * WK + (((k >> 4) ^ sw) << 4) + (k & 15);
 #pragma unroll
                 for (int l = 0; l < 4; ++l) {
@@ -189,15 +222,17 @@ __global__ void __launch_bounds__(WNT, 2) trsm_winv_kernel(const uint8_t* __rest
         mbar_wait(bar_m, phase);
         phase ^= 1;
         tc_fence_after();
-        // ---- epilogue: thread = row m of U; recombine the seven limb accumulators, write U and its limb planes
+        // ---- epilogue: thread = row m of U and one half of the tile's columns (a warp reaches the TMEM lanes of its
+        // quarter warp % 4 only); recombine the seven limb accumulators, write U and its limb planes
         {
-            const int m = 32 * warp + lane;
+            const int quarter = warp & 3, half = warp >> 2;
+            const int m = 32 * quarter + lane;
             uint32_t* urow = X + (int64_t)m * ldx + n0;
 #pragma unroll 1
-            for (int c8 = 0; c8 < WTN / 8; ++c8) {
+            for (int c8 = half * (WTN / 16); c8 < (half + 1) * (WTN / 16); ++c8) {
                 uint32_t S[7][8];
 #pragma unroll
-                for (int w = 0; w < 7; ++w) tmem_ld8(tmem_base + ((uint32_t)(32 * warp) << 16) + (uint32_t)(w * WTN + c8 * 8), S[w]);
+                for (int w = 0; w < 7; ++w) tmem_ld8(tmem_base + ((uint32_t)(32 * quarter) << 16) + (uint32_t)(w * WTN + c8 * 8), S[w]);
                 tmem_ld_wait();
                 uint32_t u[8];
 #pragma unroll
