@@ -578,20 +578,21 @@ class Bench:
         ms = float(np.mean(times))
         imad, mhz = self.peak("imad_wide", 20.0)
         macs = float(st["update_macs"])
-        # instruction budget per field multiply-accumulate of the lazily reduced update (cuobjdump of wide_update_kernel's
-        # inner loop): u32: IMAD.WIDE with carry-out + IMAD.X; u64: the 128-bit product (5 IMAD.WIDE + 2 IMAD) + 2 IMAD.X/IADD
-        per_mac = 2.0 if which == "u32" else 9.0
+        # 32 x 32 -> 64-bit multiplies per field multiply-accumulate of the lazily reduced update (cuobjdump of
+        # wide_update_kernel's inner loop): u32: one IMAD.WIDE (+ the carry additions the peak kernel also pays);
+        # u64: the 128-bit product = 5 IMAD.WIDE + 2 IMAD (counted as half a wide multiply each)
+        per_mac = 1.0 if which == "u32" else 6.0
         del a0, a
         torch.cuda.empty_cache()
         return {"workload": f"wide_{which}: {n}x{n} dense uniform, p={p}", "ms_per_call": ms, "rank": int(rk),
                 "value": (2.0 * n ** 3 / 3.0) / (ms * 1e-3) / 1e9, "unit": "Gmulmod/s (2N^3/3)",
                 "executed_tmacs_per_s": macs / (ms * 1e-3) / 1e12, "gpu_launches_per_call": int(st["kernel_launches"]),
                 "roofline": {"bound": "alu", "achieved": macs * per_mac / (ms * 1e-3) / 1e12, "peak": imad,
-                             "unit": "T integer multiply-add instructions/s (thread level)", "peak_sm_mhz": mhz,
+                             "unit": "T 32x32->64-bit multiply-adds/s (thread level)", "peak_sm_mhz": mhz,
                              "frac": macs * per_mac / (ms * 1e-3) / 1e12 / imad,
                              "peak_source": "measured live by linac_measure_peak('imad_wide')",
                              "note": f"achieved = executed field MACs (rows x cols-from-panel x 32 per panel, Gauss-Jordan over all "
-                                     f"rows) x {per_mac:g} IMAD-class instructions per multiply-accumulate (raw products summed in a 96 / 192-bit "
+                                     f"rows) x {per_mac:g} wide multiplies per multiply-accumulate (raw products summed in a 96 / 192-bit "
                                      f"accumulator, one Montgomery reduction per output and panel) / whole call"}}
 
 

@@ -285,7 +285,7 @@ int linac_set_option(const char *name, int64_t value);
  *   "tc_i8_n256", "tc_i8_n128"  tcgen05.mma.cta_group::1.kind::i8, M = 128, N = 256 / 128, K = 32 -> *value in TOP/s
  *                               (2 ops per u8 multiply-accumulate)
  *   "dmma"                      mma.sync.m8n8k4.f64 (DMMA.8x8x4)                                  -> TFLOP/s
- *   "imad_wide"                 mad.wide.u32 with 64-bit accumulate (IMAD.WIDE.U32)               -> T instructions/s (thread-level)
+ *   "imad_wide"                 32 x 32 -> 64-bit multiply + 64-bit accumulate, new operands every time -> T multiply-adds/s (thread-level)
  *   "hbm_copy", "hbm_read"      16-byte grid-stride copy / read over `scratch` (DEVICE, >= 32 MiB; use >= 1 GiB) -> GB/s
  *                               (copy counts read + written bytes)
  * ms_target: approximate duration of the timed launch (<= 0: 2 ms; a few hundred ms shows the power-capped rate).
