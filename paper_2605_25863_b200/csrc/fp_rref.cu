@@ -129,6 +129,23 @@ int trsm_leaf(Fp& c, int64_t s, uint32_t* X, int64_t ldx, int64_t ncols) {
     if (K <= 0 || ncols <= 0) return LINAC_OK;
     if (!LOWER && c.sb0(s + 1) - c.sb0(s) <= 1) return LINAC_OK;     // U is the identity inside one base panel
     Timed tm(c, stats().ms_trsm, 2);
+    if (LOWER && options().trsm_winv != 0 && c.d_W != nullptr && K == WK && c.sb0(s + 1) - c.sb0(s) == WK / PW && ncols >= 4 * WTN) {
+        bool regular = true;                                   // four base panels with 32 pivots each: one product with W
+        for (int64_t b = c.sb0(s); b < c.sb0(s + 1); ++b) regular = regular && c.pstart[b + 1] - c.pstart[b] == PW;
+        if (regular) {
+            strip_winv_kernel<<<WINV_CTAS, WINV_NT, sizeof(WinvSmem), c.s>>>(c.A, c.ld, c.d_pstart, (int)c.sb0(s), c.d_T, c.d_pivcols,
+                                                                             c.f, c.d_W);
+            LINAC_CUDA(cudaGetLastError());
+            const int64_t ntiles = (ncols + WTN - 1) / WTN;
+            trsm_winv_kernel<<<(unsigned)std::min<int64_t>(ntiles, 2 * sm_count()), WNT, WTRSM_SMEM, c.s>>>(
+                c.d_W, X, ldx, ncols, c.f, nullptr, 0, 0, ncols);
+            LINAC_CUDA(cudaGetLastError());
+            stats().kernel_launches += 2;
+            stats().winv_solves++;
+            stats().update_macs += K * K / 2 * ncols;
+            return LINAC_OK;
+        }
+    }
     trsm_strip_kernel<LOWER><<<(unsigned)((ncols + PW - 1) / PW), TNT, trsm_smem_bytes(K), c.s>>>(
         c.A, c.ld, X, ldx, ncols, c.d_pstart, (int)c.sb0(s), (int)c.sb0(s + 1), c.d_T, c.d_pivcols, c.f, nullptr, 0, nullptr, 0, nullptr,
         0, 0);
