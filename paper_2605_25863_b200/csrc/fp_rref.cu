@@ -40,7 +40,9 @@ struct Fp {
     PanelRec* d_rec;          // [nb]
     uint32_t* d_T;            // [nb][PW*PW]
     uint32_t* d_E;            // [nb][PW*PW]
-    uint8_t* d_W = nullptr;   // [4][WK][WK] limb planes of the current regular strip's solve operator (fp_trsm_inv.cuh)
+    uint8_t* d_W = nullptr;   // 2 x [4][WK][WK] limb planes of a regular strip's solve operator (fp_trsm_inv.cuh); strip s uses
+                              // buffer s & 1: the tail of strip s's solve (second stream) may still read W while W of s+1 is written
+    int64_t winv_count = 0;
     Arena* arena;
     // host
     unsigned long long* h_mail;      // mapped pinned, MAXBP * MAIL_WORDS tagged words written by the strip kernel itself
@@ -133,12 +135,13 @@ int trsm_leaf(Fp& c, int64_t s, uint32_t* X, int64_t ldx, int64_t ncols) {
         bool regular = true;                                   // four base panels with 32 pivots each: one product with W
         for (int64_t b = c.sb0(s); b < c.sb0(s + 1); ++b) regular = regular && c.pstart[b + 1] - c.pstart[b] == PW;
         if (regular) {
+            uint8_t* W = c.d_W + (size_t)((c.winv_count++) & 1) * W_A_BYTES;
             strip_winv_kernel<<<WINV_CTAS, WINV_NT, sizeof(WinvSmem), c.s>>>(c.A, c.ld, c.d_pstart, (int)c.sb0(s), c.d_T, c.d_pivcols,
-                                                                             c.f, c.d_W);
+                                                                             c.f, W);
             LINAC_CUDA(cudaGetLastError());
             const int64_t ntiles = (ncols + WTN - 1) / WTN;
             trsm_winv_kernel<<<(unsigned)std::min<int64_t>(ntiles, 2 * sm_count()), WNT, WTRSM_SMEM, c.s>>>(
-                c.d_W, X, ldx, ncols, c.f, nullptr, 0, 0, ncols);
+                W, X, ldx, ncols, c.f, nullptr, 0, 0, ncols);
             LINAC_CUDA(cudaGetLastError());
             stats().kernel_launches += 2;
             stats().winv_solves++;
@@ -181,6 +184,7 @@ struct StripLaunch {
     int64_t b0 = 0, b1 = 0, j0 = 0, j1 = 0;
     cudaStream_t stream = nullptr;
     bool winv = false;        // strip_winv_kernel was enqueued behind the strip kernel (it writes W only for a regular strip)
+    uint8_t* W = nullptr;     // ... into this buffer
     // filled by collect_strip
     int64_t nswaps = 0;       // row exchanges of the strip's panels that found pivots
     bool regular = false;     // four base panels with 32 pivots each
@@ -259,7 +263,8 @@ int collect_strip(Fp& c, StripLaunch& L, int64_t i0, int64_t* r) {
 int launch_winv(Fp& c, StripLaunch& L, cudaStream_t stream) {
     if (options().trsm_winv == 0 || c.d_W == nullptr || L.b1 - L.b0 != WK / PW || L.j1 - L.j0 != WK) return LINAC_OK;
     Timed tm(c, stats().ms_trsm, 2, stream);
-    strip_winv_kernel<<<WINV_CTAS, WINV_NT, sizeof(WinvSmem), stream>>>(c.A, c.ld, c.d_pstart, (int)L.b0, c.d_T, c.d_pivcols, c.f, c.d_W);
+    L.W = c.d_W + (size_t)((c.winv_count++) & 1) * W_A_BYTES;
+    strip_winv_kernel<<<WINV_CTAS, WINV_NT, sizeof(WinvSmem), stream>>>(c.A, c.ld, c.d_pstart, (int)L.b0, c.d_T, c.d_pivcols, c.f, L.W);
     LINAC_CUDA(cudaGetLastError());
     stats().kernel_launches++;
     L.winv = true;
@@ -277,7 +282,7 @@ int launch_strip_solve(Fp& c, const StripLaunch& L, int64_t i0, int64_t c0, int6
     if (L.winv && L.regular && !mail && (Bq == nullptr || kp == WK)) {          // one dense product with the strip's W
         const int64_t ntiles = (ncols + WTN - 1) / WTN;
         trsm_winv_kernel<<<(unsigned)std::min<int64_t>(ntiles, 2 * sm_count()), WNT, WTRSM_SMEM, stream>>>(
-            c.d_W, c.A + i0 * c.ld + c0, c.ld, ncols, c.f, Bq, kp, bq_col0, bq_total > 0 ? bq_total : ncols);
+            L.W, c.A + i0 * c.ld + c0, c.ld, ncols, c.f, Bq, kp, bq_col0, bq_total > 0 ? bq_total : ncols);
         LINAC_CUDA(cudaGetLastError());
         stats().kernel_launches++;
         stats().winv_solves++;
@@ -331,7 +336,7 @@ int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jen
     for (cudaEvent_t& e : cx.la_ev)
         if (!e) LINAC_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     cudaStream_t sB = cx.la_stream;
-    cudaEvent_t ev_narrow = cx.la_ev[1], ev_strip = cx.la_ev[2];
+    cudaEvent_t ev_pre = cx.la_ev[0], ev_narrow = cx.la_ev[1], ev_strip = cx.la_ev[2];
     // How many SMs the look-ahead strip kernel gets, per strip.  Cost model in microseconds, fitted to sweeps of the
     // fixed-partition schedule on a B200 at config c3 (`profiles/r02_lookahead.md`): a 128-column strip kernel on G CTAs
     // takes 63.5 + 4300 (m / 1e4) / G (the chain of CTA 0 plus the in-strip updates and the L21 limb split, which spread
@@ -423,7 +428,18 @@ int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jen
                 // the rest beside the strip kernel is SLOWER, 13.5 -> 15.3 / 16.0 ms at c3: squeezed onto the bulk's SMs the
                 // solve needs two rounds of CTAs and pushes the bulk update, which then bounds the step), then the next
                 // strip's columns of the update, the fork, and the bulk of the update beside the strip kernel
-                rc = launch_strip_solve(c, L, cur, jc, jend - jc, Bq, kp, false);
+                if (L.winv && L.regular && o.trsm_split != 0) {
+                    // regular strip: the product with W is cheap and has no chain, so only the next strip's columns are
+                    // solved in front of the narrow update; the rest goes to the second stream, in front of the bulk it
+                    // feeds, and runs beside the narrow update instead of before it
+                    LINAC_CUDA(cudaEventRecord(ev_pre, c.s));                      // exchanges of strip s applied, W written
+                    rc = launch_strip_solve(c, L, cur, jc, jn - jc, Bq, kp, false, 0, jend - jc);
+                    if (rc) return rc;
+                    LINAC_CUDA(cudaStreamWaitEvent(sB, ev_pre, 0));
+                    rc = launch_strip_solve(c, L, cur, jn, jend - jn, Bq, kp, false, jn - jc, jend - jc, sB);
+                } else {
+                    rc = launch_strip_solve(c, L, cur, jc, jend - jc, Bq, kp, false);
+                }
                 if (rc) return rc;
                 rc = update(jc, jn, 0, c.s);
                 if (rc) return rc;
@@ -606,7 +622,7 @@ size_t meta_bytes(int64_t rows, int64_t cols) {
     const int64_t mn = std::max<int64_t>(1, std::min(rows, cols));
     const int64_t nb = num_panels(cols);
     // + the index arrays of the consumers that run behind the reduction (null space: 2 cols; solve: cols + nrhs; C.R: rank)
-    return 8192 + (size_t)WK * WK * 4 + 1024 + (size_t)nb * (sizeof(PanelRec) + 256 + 2 * PW * PW * 4 + 4) + (size_t)mn * 4 + (size_t)cols * 4 + 10 * 256 +
+    return 8192 + (size_t)2 * W_A_BYTES + 1024 + (size_t)nb * (sizeof(PanelRec) + 256 + 2 * PW * PW * 4 + 4) + (size_t)mn * 4 + (size_t)cols * 4 + 10 * 256 +
            (size_t)cols * 12 + (size_t)mn * 4 + 4096;
 }
 
@@ -672,7 +688,7 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
     c.d_pivcols = (int32_t*)arena->take((size_t)mn * 4);
     int32_t* d_colinfo = (int32_t*)arena->take((size_t)cols * 4);
     c.d_pstart = (int32_t*)arena->take((size_t)(c.nb + 1) * 4);
-    c.d_W = (uint8_t*)arena->take((size_t)WK * WK * 4, 1024);
+    c.d_W = (uint8_t*)arena->take((size_t)2 * W_A_BYTES, 1024);
     if (!c.d_rec || !c.d_T || !c.d_E || !c.d_pivcols || !d_colinfo || !c.d_pstart || !c.d_W) return LINAC_ERR_WORKSPACE;
     LINAC_CUDA(cudaMemsetAsync(c.d_pstart, 0, (size_t)(c.nb + 1) * 4, s));
     c.h_mail = cx.mail;

@@ -61,6 +61,8 @@ struct Options {
     int64_t la_ctas = 0;      // CTAs (= SMs) of the look-ahead strip kernel; 0 = chosen per strip from a cost model
     int64_t trsm_winv = 1;    // look-ahead sweep: row-block solve of a regular strip (4 x 32 pivots) as ONE product with the strip's
                               // explicit 128 x 128 operator W (fp_trsm_inv.cuh); 0 = the panel-by-panel chain kernel everywhere
+    int64_t trsm_split = 1;   // ... and, when the update forks, only on the next strip's columns before the narrow update; the
+                              // rest of the solve runs on the second stream in front of the bulk update (0 = whole solve first)
 };
 Options& options();
 
