@@ -356,7 +356,7 @@ class Bench:
         roof["whole_step_frac"] = whole / roof["peak"]
         roof["update_share_of_step"] = ms_upd / st_alone["ms_total"] if st_alone["ms_total"] else None
         if st_alone is not st_t:
-            roof["kernels_timed_alone"] = {"schedule": "look-ahead off (option lookahead = 0): every kernel has the whole GPU",
+            roof["kernels_timed_alone"] = {"schedule": "look-ahead off (option lookahead = 0): every kernel has the whole GPU; trsm here is the chain kernel (the sequential sweep enqueues the solve before the host has the strip's records, so it cannot pick the tensor-core W product)",
                                            "update": st_alone["ms_update"], "strip": st_alone.get("ms_strip"),
                                            "trsm": st_alone.get("ms_trsm"), "call_with_event_marks": st_alone["ms_total"]}
             la_ach = st_t["update_macs"] * 32.0 / (st_t["ms_update"] * 1e-3) / 1e12 if st_t["ms_update"] > 0 else None
