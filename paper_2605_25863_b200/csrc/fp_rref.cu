@@ -400,12 +400,13 @@ int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jen
         StripLaunch Ln;
         if (r > 0 && jend > jc) {
             const bool planes = r <= kp && (jend - jc) >= o.tc_min_mn && r >= o.tc_min_k && m2 >= o.tc_min_mn && o.gemm_path != 1 && o.tc_panel != 0;
-            auto update = [&](int64_t c0, int64_t c1, int grid_limit, cudaStream_t stream) -> int {
+            auto update = [&](int64_t c0, int64_t c1, int grid_limit, cudaStream_t stream, bool pdl = false) -> int {
                 GemmArgs g{c.A + (cur + r) * c.ld + c0, c.ld, c.A + (cur + r) * c.ld, c.ld, c.d_pivcols + cur,
                            c.A + cur * c.ld + c0,       c.ld, m2,                      c1 - c0, r};
                 if (planes) {
                     g.Bq_ready = Bq; g.kp_ready = kp; g.Aq_ready = Aq[s & 1];
                     g.bq_row0 = c0 - jc; g.bq_rows_total = jend - jc;
+                    g.pdl = pdl;
                 }
                 g.grid_limit = grid_limit;
                 return run_gemm(c, g, stream);
@@ -428,7 +429,8 @@ int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jen
                 // the rest beside the strip kernel is SLOWER, 13.5 -> 15.3 / 16.0 ms at c3: squeezed onto the bulk's SMs the
                 // solve needs two rounds of CTAs and pushes the bulk update, which then bounds the step), then the next
                 // strip's columns of the update, the fork, and the bulk of the update beside the strip kernel
-                if (L.winv && L.regular && o.trsm_split != 0) {
+                const bool wsplit = L.winv && L.regular && o.trsm_split != 0;
+                if (wsplit) {
                     // regular strip: the product with W is cheap and has no chain, so only the next strip's columns are
                     // solved in front of the narrow update; the rest goes to the second stream, in front of the bulk it
                     // feeds, and runs beside the narrow update instead of before it
@@ -441,7 +443,9 @@ int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jen
                     rc = launch_strip_solve(c, L, cur, jc, jend - jc, Bq, kp, false);
                 }
                 if (rc) return rc;
-                rc = update(jc, jn, 0, c.s);
+                // behind the W product the update is a programmatic dependent: its prologue, its A stages and its first C
+                // tiles overlap the product, only its B loads wait for it
+                rc = update(jc, jn, 0, c.s, wsplit && o.pdl != 0);
                 if (rc) return rc;
                 // the chain stays on the call's stream (the strip kernel starts the moment the narrow update ends and takes
                 // its SMs first); the bulk goes to the second stream, where the cross-stream event latency does no harm
@@ -453,7 +457,7 @@ int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jen
                 next_launched = true;
                 stats().lookahead_strips++;
                 LINAC_CUDA(cudaStreamWaitEvent(sB, ev_narrow, 0));
-                rc = update(jn, jend, c.coop_grid - la_grid, sB);
+                rc = update(jn, jend, c.coop_grid - la_grid, sB, wsplit && o.pdl != 0);
                 if (rc) return rc;
                 LINAC_CUDA(cudaEventRecord(ev_strip, sB));                          // = "bulk of strip s done"
             } else {

@@ -142,6 +142,7 @@ __global__ void __launch_bounds__(WNT, 2) trsm_winv_kernel(const uint8_t* __rest
                                                           int64_t ldx, int64_t ncols, ModP f, uint8_t* __restrict__ Bq,
                                                           int kp, int64_t bq_col0, int64_t bq_total) {
     using namespace tc;
+    grid_dep_launch();                                    // an update launched as a programmatic dependent may start its prologue now
     extern __shared__ uint8_t wtrsm_smem_raw[];
     uint8_t* smem = (uint8_t*)(((uintptr_t)wtrsm_smem_raw + 1023) & ~(uintptr_t)1023);
     uint8_t* sA = smem;                                   // [4][WK][128]

@@ -277,6 +277,7 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
     if (warp == 0) {
         if (lane == 0) {
             uint32_t a_cnt = 0, b_cnt = 0;
+            bool dep_waited = false;
             TileIter it;
             it.init(sc);
             while (it.valid) {
@@ -287,6 +288,10 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                     tma_load_3d(sA + s * P_A_STAGE, &tmA, &a_full[s], ks * KB, it.mt * TM, 0);
                 }
                 const int item = it.item;
+                // B is the only operand the kernel right before this one in the stream may have produced (the row-block
+                // solve writes U12's limb planes): under a programmatic dependent launch everything above -- barriers,
+                // TMEM, the A stages, the first C tiles -- has run beside that kernel, and only this waits for it
+                if (!dep_waited) { grid_dep_wait(); dep_waited = true; }
                 while (it.valid && it.item == item) {
                     for (int ks = 0; ks < nks; ++ks, ++b_cnt) {
                         const int s = b_cnt % P_NBS;
@@ -609,7 +614,23 @@ int gemm_modp_tc(const GemmArgs& g, const ModP& f, cudaStream_t s, Arena* scratc
             return -1;
         const int grid = g.grid_limit > 0 ? std::min(g.grid_limit, sm_count()) : sm_count();
         const PanelSched sc = make_sched(g.M, g.N, grid);
-        if (f.ninv)
+        if (g.pdl) {
+            // programmatic dependent launch behind the kernel that produced B (the caller vouches that this kernel wrote
+            // neither A nor C): the prologue and the A / C loads overlap that kernel's tail
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3((unsigned)std::min(grid, sc.nitems));
+            cfg.blockDim = dim3(P_THREADS);
+            cfg.dynamicSmemBytes = P_SMEM;
+            cfg.stream = s;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            at[0].val.programmaticStreamSerializationAllowed = 1;
+            cfg.attrs = at;
+            cfg.numAttrs = 1;
+            const int nks = (int)(kp / KB);
+            if (f.ninv) LINAC_CUDA(cudaLaunchKernelEx(&cfg, gemm_tc_panel_kernel<true>, tmA, tmB, tmC, nks, sc, f));
+            else LINAC_CUDA(cudaLaunchKernelEx(&cfg, gemm_tc_panel_kernel<false>, tmA, tmB, tmC, nks, sc, f));
+        } else if (f.ninv)
             gemm_tc_panel_kernel<true><<<(unsigned)std::min(grid, sc.nitems), P_THREADS, P_SMEM, s>>>(tmA, tmB, tmC, (int)(kp / KB), sc, f);
         else
             gemm_tc_panel_kernel<false><<<(unsigned)std::min(grid, sc.nitems), P_THREADS, P_SMEM, s>>>(tmA, tmB, tmC, (int)(kp / KB), sc, f);

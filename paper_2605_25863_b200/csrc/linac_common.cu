@@ -298,6 +298,9 @@ int linac_set_option(const char* name, int64_t value) {
     } else if (!strcmp(name, "trsm_winv")) {
         if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
         g_options.trsm_winv = value;
+    } else if (!strcmp(name, "pdl")) {
+        if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
+        g_options.pdl = value;
     } else if (!strcmp(name, "trsm_split")) {
         if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
         g_options.trsm_split = value;

@@ -61,6 +61,7 @@ struct Options {
     int64_t la_ctas = 0;      // CTAs (= SMs) of the look-ahead strip kernel; 0 = chosen per strip from a cost model
     int64_t trsm_winv = 1;    // look-ahead sweep: row-block solve of a regular strip (4 x 32 pivots) as ONE product with the strip's
                               // explicit 128 x 128 operator W (fp_trsm_inv.cuh); 0 = the panel-by-panel chain kernel everywhere
+    int64_t pdl = 1;          // look-ahead sweep: the updates right behind a W solve start beside it (programmatic dependent launch)
     int64_t trsm_split = 1;   // ... and, when the update forks, only on the next strip's columns before the narrow update; the
                               // rest of the solve runs on the second stream in front of the bulk update (0 = whole solve first)
 };
@@ -164,6 +165,8 @@ struct GemmArgs {
     // columns and the rest): the planes hold bq_rows_total columns (0 = N) and this update starts at column bq_row0
     int64_t bq_row0 = 0, bq_rows_total = 0;
     int grid_limit = 0;               // persistent kernels: use at most this many CTAs (0 = one per SM)
+    bool pdl = false;                 // K <= 256 panel kernel with ready planes: programmatic dependent launch behind the kernel that
+                                      // wrote the B planes (which must have written neither C nor the A planes)
 };
 int gemm_modp_simt(const GemmArgs& g, const ModP& f, cudaStream_t s);
 // Tensor-core (tcgen05 int8 limb) path; returns LINAC_OK if it ran, or a negative value if the
