@@ -59,6 +59,8 @@ def lib() -> C.CDLL:
                                            C.c_int64, C.c_uint64, C.c_int]
         L.oracle_rref_f64.restype = C.c_int
         L.oracle_rref_f64.argtypes = [f64p, C.c_int64, C.c_int64, C.c_int64, C.c_double, C.c_int, i64p, i32p]
+        L.oracle_rref_c128.restype = C.c_int
+        L.oracle_rref_c128.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_double, C.c_int, i64p, i32p]
         L.oracle_backward_error.restype = C.c_double
         L.oracle_backward_error.argtypes = [f64p, C.c_int64, C.c_int64, f64p, C.c_int64, f64p, C.c_int64, C.c_int64,
                                             C.c_int]
@@ -278,4 +280,21 @@ def rref_f64(a: np.ndarray, tol: float = -1.0, nthreads: int = 1):
                                piv.ctypes.data_as(C.POINTER(C.c_int32)))
     if rc != 0:
         raise ValueError(f"oracle_rref_f64 failed: {rc}")
+    return r, int(rank.value), piv[: rank.value].copy()
+
+
+def rref_c128(a: np.ndarray, tol: float = -1.0, nthreads: int = 1):
+    """The same reduction on a complex128 matrix (rows rescaled by their largest real or imaginary part,
+    reading Q21; pivot = largest modulus).  Returns (R, rank, pivot_cols); the input is untouched.
+    Pinned in tests/test_oracle_c128.py: exact RREF over Q(i) (sympy) of Gaussian-integer matrices, agreement with
+    rref_f64 on real input and through the real 2 x 2 block embedding, numpy SVD rank, invariance under row phases."""
+    a = np.ascontiguousarray(a, dtype=np.complex128)
+    rows, cols = a.shape
+    r = a.copy()
+    rank = C.c_int64(0)
+    piv = np.zeros(max(1, min(rows, cols)), dtype=np.int32)
+    rc = lib().oracle_rref_c128(r.ctypes.data_as(C.c_void_p), rows, cols, max(cols, 1), tol, nthreads, C.byref(rank),
+                                piv.ctypes.data_as(C.POINTER(C.c_int32)))
+    if rc != 0:
+        raise ValueError(f"oracle_rref_c128 failed: {rc}")
     return r, int(rank.value), piv[: rank.value].copy()

@@ -469,3 +469,65 @@ int oracle_rref_f64(double *A, int64_t rows, int64_t cols, int64_t ld, double to
             for (int64_t c = 0; c < pivot_cols[r]; ++c) A[r * ld + c] = 0.0;
     return 0;
 }
+
+/* =====================================================================================================
+ * SURVEY.md 8(f) rank 3, complex128 ("complex128" is one of the data types the reduction is
+ * instantiated for): the same loop as oracle_rref_f64 on double _Complex entries (row-major, ld in elements).
+ *   1. row scale: s_r = max_c max(|Re A[r,c]|, |Im A[r,c]|)  -- reading Q21: the
+ *      paper does not say which absolute value a complex row is rescaled by; the largest real or imaginary part
+ *      keeps the scale a real number that depends on the row only, within sqrt(2) of the largest modulus;
+ *   2. pivot = arg max_{r >= i} |A[r,j]| (modulus), lowest index on ties; |head| <= tol => free column;
+ *      row i /= head; every other row r: row_r -= head_r * row_i on the columns from j on, head of row r set to 0;
+ *   3. what the thresholds declared zero is written as zero (reading Q19).
+ * tol < 0 selects max(rows, cols) * 2^-52.  Returns 0, or -1 on bad arguments.
+ * ===================================================================================================== */
+#include <complex.h>
+int oracle_rref_c128(double _Complex *A, int64_t rows, int64_t cols, int64_t ld, double tol, int nthreads, int64_t *rank,
+                     int32_t *pivot_cols) {
+    if (rows < 0 || cols < 0 || ld < cols || (rows > 0 && cols > 0 && !A)) return -1;
+    if (tol < 0) tol = (double)(rows > cols ? rows : cols) * ldexp(1.0, -52);
+    (void)nthreads;
+    for (int64_t r = 0; r < rows; ++r) {
+        double s = 0.0;
+        for (int64_t c = 0; c < cols; ++c) {
+            const double re = fabs(creal(A[r * ld + c])), im = fabs(cimag(A[r * ld + c]));
+            if (re > s) s = re;
+            if (im > s) s = im;
+        }
+        if (s == 0.0) continue;
+        for (int64_t c = 0; c < cols; ++c) A[r * ld + c] /= s;
+    }
+    int64_t i = 0;
+    for (int64_t j = 0; j < cols && i < rows; ++j) {
+        int64_t k = i;
+        double best = cabs(A[i * ld + j]);
+        for (int64_t r = i + 1; r < rows; ++r) { double v = cabs(A[r * ld + j]); if (v > best) { best = v; k = r; } }
+        if (k != i)
+            for (int64_t c = 0; c < cols; ++c) { double _Complex t = A[i * ld + c]; A[i * ld + c] = A[k * ld + c]; A[k * ld + c] = t; }
+        const double _Complex head = A[i * ld + j];
+        if (!(cabs(head) > tol)) continue;
+        double _Complex *pi = A + i * ld;
+        for (int64_t c = j; c < cols; ++c) pi[c] /= head;
+        pi[j] = 1.0;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) num_threads(nthreads) if (nthreads > 1)
+#endif
+        for (int64_t r = 0; r < rows; ++r) {
+            if (r == i) continue;
+            double _Complex *pr = A + r * ld;
+            const double _Complex h = pr[j];
+            if (h == 0.0) continue;
+            for (int64_t c = j + 1; c < cols; ++c) pr[c] -= h * pi[c];
+            pr[j] = 0.0;
+        }
+        if (pivot_cols) pivot_cols[i] = (int32_t)j;
+        ++i;
+    }
+    if (rank) *rank = i;
+    for (int64_t r = i; r < rows; ++r)
+        for (int64_t c = 0; c < cols; ++c) A[r * ld + c] = 0.0;
+    if (pivot_cols)
+        for (int64_t r = 0; r < i; ++r)
+            for (int64_t c = 0; c < pivot_cols[r]; ++c) A[r * ld + c] = 0.0;
+    return 0;
+}
