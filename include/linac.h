@@ -243,6 +243,22 @@ int linac_rref_f64_workspace(int64_t rows, int64_t cols, size_t *bytes);
 int linac_rref_f64(double *dA, int64_t rows, int64_t cols, int64_t ld, double tol, void *stream, int64_t *rank,
                    int32_t *pivot_cols_out);
 
+/* ---- complex128 (the reduction is instantiated for complex128 as well) ---------------------------
+ * linac_rref_c128: the same reduction with a threshold on a rows x cols matrix of complex doubles (interleaved re, im:
+ * C's double _Complex / numpy complex128 / torch.complex128; dA 16-byte aligned, ld in complex elements), in place;
+ * rank, pivot columns, tol and the written-as-zero convention as linac_rref_f64.  Rows are rescaled by their largest
+ * real or imaginary part (reading Q21).
+ * Computed as the real reduction of the 2 x 2 block embedding  x + iy -> [[x, -y], [y, x]]  (a ring homomorphism, and the
+ * reduced echelon form of a row space is unique, so RREF_real(E(A)) = E(RREF_complex(A))): the fp64 tensor-pipe
+ * kernels serve unchanged, at twice the flops and memory of a native complex elimination.  The workspace holds the
+ * 2 rows x 2 cols real matrix (32 bytes per complex entry) plus linac_rref_f64's own for that shape.
+ * LINAC_ERR_SINGULAR if the threshold fell between the two real columns of one complex column (a pivot within a factor
+ * sqrt(2) of tol: choose another tol); dA is then unchanged.
+ */
+int linac_rref_c128_workspace(int64_t rows, int64_t cols, size_t *bytes);
+int linac_rref_c128(void *dA, int64_t rows, int64_t cols, int64_t ld, double tol, void *stream, int64_t *rank,
+                    int32_t *pivot_cols_out);
+
 /* ---- instrumentation (host-side counters of the LAST F_p call; for tests and bench.py) ------ */
 typedef struct {
     int64_t kernel_launches;     /* kernels this library launched                                 */

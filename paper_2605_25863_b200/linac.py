@@ -26,7 +26,7 @@ SYMBOLS = [
     "linac_rref_u64_workspace", "linac_rref_u64",
     "linac_rref_u32", "linac_nullspace_u32", "linac_nullspace_from_rref_u32", "linac_solve_u32", "linac_rank_factor_u32", "linac_load_matrix_u32", "linac_gemm_sub_u32",
     "linac_gemm_sub_u32_static",
-    "linac_solve_f64", "linac_rref_f64_workspace", "linac_rref_f64",
+    "linac_solve_f64", "linac_rref_f64_workspace", "linac_rref_f64", "linac_rref_c128_workspace", "linac_rref_c128",
     "linac_get_last_stats", "linac_set_option", "linac_measure_peak",
 ]
 
@@ -83,6 +83,8 @@ def _lib() -> C.CDLL:
         L.linac_solve_f64.argtypes = [vp, i64, i64, vp, i64, i64, C.c_double, vp, C.POINTER(i64)]
         L.linac_rref_f64_workspace.argtypes = [i64, i64, C.POINTER(sz)]
         L.linac_rref_f64.argtypes = [vp, i64, i64, i64, C.c_double, vp, C.POINTER(i64), vp]
+        L.linac_rref_c128_workspace.argtypes = [i64, i64, C.POINTER(sz)]
+        L.linac_rref_c128.argtypes = [vp, i64, i64, i64, C.c_double, vp, C.POINTER(i64), vp]
         L.linac_measure_peak.argtypes = [C.c_char_p, C.c_double, vp, sz, vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.linac_get_last_stats.argtypes = [C.POINTER(Stats)]
         L.linac_set_option.argtypes = [C.c_char_p, i64]
@@ -371,6 +373,23 @@ def rref_f64(a: torch.Tensor, tol: float = -1.0):
                                    piv.data_ptr())
     if rc:
         raise LinacError(rc, "linac_rref_f64")
+    return int(rank.value), piv[: rank.value].clone()
+
+
+def rref_c128(a: torch.Tensor, tol: float = -1.0):
+    """In place: `a` (CUDA complex128, rows x cols) -> its reduced row-echelon form with the threshold `tol` on the
+    row-scaled matrix.  Returns (rank, pivot_cols).  Mirrors linac_rref_c128."""
+    rows, cols, ld = _check_matrix(a, (torch.complex128,), "a")
+    with torch.cuda.device(a.device):
+        need = C.c_size_t(0)
+        _lib().linac_rref_c128_workspace(rows, cols, C.byref(need))
+        _ensure_workspace(need.value, a.device)
+        rank = C.c_int64(0)
+        piv = torch.empty(max(1, min(rows, cols)), dtype=torch.int32)
+        rc = _lib().linac_rref_c128(a.data_ptr(), rows, cols, ld, float(tol), _stream_ptr(a.device), C.byref(rank),
+                                    piv.data_ptr())
+    if rc:
+        raise LinacError(rc, "linac_rref_c128")
     return int(rank.value), piv[: rank.value].clone()
 
 
