@@ -10,6 +10,7 @@ carries one leg per remaining config and per widened row, each with its own timi
   legs.c5            N = 10^5 (40 GB, generated on the device): 1 warm-up + 2 timed calls
   legs.fp64_solve    config c4 through linac_solve_f64: ms per solve, GFLOP/s, backward error
   legs.rref_f64      SURVEY.md 8(f)#3: linac_rref_f64 on a rank-deficient float64 matrix
+  legs.rref_c128     the same for complex128 (linac_rref_c128: the fp64 reduction of the 2 x 2 real block embedding)
   legs.wide_u32/u64  SURVEY.md 8(f)#4: linac_rref_u32 with p = 2^32 - 5 and linac_rref_u64 with p = 2^61 - 1
 
   value      : whole-job Gmulmod/s = (2 N^3 / 3) / t, matrix already resident in HBM, t = CUDA-event time of the C-ABI
@@ -551,6 +552,50 @@ class Bench:
                              "frac": flop / ms / 1e9 / peak, "peak_sm_mhz": mhz,
                              "note": "executed flops of the DMMA updates (2 rows (cols - j0) 32 per panel: K = 32 inside the panel's 128-column strip, K = 128 right of it) / whole call"}}
 
+    def rref_c128_leg(self, rows=4096, cols=4096, r=3072, reps=2):
+        """SURVEY.md 8(f)#3, complex128: linac_rref_c128 on a rank-deficient complex product with rows rescaled over several
+        decades and rotated by arbitrary phases.  The GPU reduces the 2 rows x 2 cols real embedding, so the flops that run
+        are those of linac_rref_f64 at that shape: twice what a native complex elimination needs (stated in the note)."""
+        torch, L, dev = self.torch, self.L, self.dev
+        g = torch.Generator(device=dev)
+        g.manual_seed(10)
+        def cn(m, n):
+            return torch.complex(torch.randn((m, n), dtype=torch.float64, device=dev, generator=g),
+                                 torch.randn((m, n), dtype=torch.float64, device=dev, generator=g))
+        a0 = cn(rows, r) @ cn(r, cols)
+        a0 *= 10.0 ** (2.0 * torch.randn((rows, 1), dtype=torch.float64, device=dev, generator=g))
+        a0 *= torch.exp(2j * np.pi * torch.rand((rows, 1), dtype=torch.float64, device=dev, generator=g))
+        a = torch.empty_like(a0)
+        stream = torch.cuda.current_stream(dev)
+        times, rk = [], None
+        for i in range(reps + 1):
+            a.copy_(a0)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            rk, piv = L.rref_c128(a, 1e-9)
+            e1.record(stream)
+            e1.synchronize()
+            if i:
+                times.append(e0.elapsed_time(e1))
+        launches = L.last_stats()["kernel_launches"]
+        pv = piv.to(dev).long()
+        recon = a0[:, pv] @ a[:rk]
+        err = float(((recon - a0).abs().amax(dim=1) / a0.abs().amax(dim=1)).max())
+        ms = float(np.mean(times))
+        R, Cc, rk2 = 2 * rows, 2 * cols, 2 * rk
+        flop = float(sum(2.0 * R * (Cc - j0) * 32 for j0 in range(0, Cc, 32) if j0 < rk2 + 32))
+        peak, mhz = self.peak("dmma", 20.0)
+        del a0, a
+        torch.cuda.empty_cache()
+        return {"workload": f"rref_c128: {rows}x{cols} complex128, rank {r} product of complex N(0,1) factors, rows rescaled by "
+                            "10^(2 N(0,1)) and rotated by random phases, tol 1e-9", "ms_per_call": ms, "rank": int(rk),
+                "gflops_executed": flop / ms / 1e6, "row_space_residual": err, "gpu_launches_per_call": int(launches),
+                "roofline": {"bound": "tensor", "achieved": flop / ms / 1e9, "peak": peak, "unit": "TFLOP/s (fp64 DMMA)",
+                             "frac": flop / ms / 1e9 / peak, "peak_sm_mhz": mhz,
+                             "note": "executed real flops of the DMMA updates on the 2 rows x 2 cols embedding (2x the real "
+                                     "flops of a native complex elimination, which needs 4 real multiply-adds per complex one "
+                                     "where the embedding spends 8) / whole call incl. the expand and contract kernels"}}
+
     def wide_leg(self, which, n=4096, reps=2):
         """SURVEY.md 8(f)#4: dense uniform n x n over F_p with p = 2^32 - 5 (uint32 storage) or 2^61 - 1 (uint64)."""
         torch, L, dev = self.torch, self.L, self.dev
@@ -604,7 +649,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="all", choices=["all", "c1", "c2", "c3", "c5"],
                     help="all (default): headline c3 + one leg per other config; or a single F_p config as the headline")
-    ap.add_argument("--legs", default="c1,c2,c5,fp64_solve,rref_f64,wide_u32,wide_u64",
+    ap.add_argument("--legs", default="c1,c2,c5,fp64_solve,rref_f64,rref_c128,wide_u32,wide_u64",
                     help="comma list of the extra legs of the default run")
     ap.add_argument("--ref-n", type=int, default=1280, help="sample size for --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -612,7 +657,7 @@ def main():
     ap.add_argument("--cpu-baseline", default="bounded", choices=["bounded", "full"])
     ap.add_argument("--no-f64", action="store_true", help="skip the fp64 legs")
     ap.add_argument("--fp64-only", action="store_true", help="run only legs.fp64_solve and print {\"fp64\": ...}")
-    ap.add_argument("--only-leg", default="", choices=["", "rref_f64", "wide_u32", "wide_u64"],
+    ap.add_argument("--only-leg", default="", choices=["", "rref_f64", "rref_c128", "wide_u32", "wide_u64"],
                     help="run only this leg of the widened rows (SURVEY.md 8(f)) and print {name: ...}; for profiles")
     ap.add_argument("--gemm", default=None, metavar="M,N,K[,path]",
                     help="time the S5 primitive linac_gemm_sub_u32 alone (C -= A.B mod 2^31-1, path 2 = tensor cores by default) "
@@ -698,7 +743,7 @@ def main():
     if args.only_leg:
         if rank == 0:
             reps = max(1, min(args.steps, 3))
-            leg = {"rref_f64": lambda: B.rref_f64_leg(reps=reps), "wide_u32": lambda: B.wide_leg("u32", reps=reps),
+            leg = {"rref_f64": lambda: B.rref_f64_leg(reps=reps), "rref_c128": lambda: B.rref_c128_leg(reps=reps), "wide_u32": lambda: B.wide_leg("u32", reps=reps),
                    "wide_u64": lambda: B.wide_leg("u64", reps=reps)}[args.only_leg]()
             print(json.dumps({args.only_leg: leg}))
         return
@@ -738,6 +783,8 @@ def main():
                     legs[name] = B.f64_solve_leg()
                 elif name == "rref_f64" and not args.no_f64:
                     legs[name] = B.rref_f64_leg()
+                elif name == "rref_c128" and not args.no_f64:
+                    legs[name] = B.rref_c128_leg()
                 elif name == "wide_u32":
                     legs[name] = B.wide_leg("u32")
                 elif name == "wide_u64":
