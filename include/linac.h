@@ -285,7 +285,7 @@ int linac_get_last_stats(linac_stats *out);
  * of strip s's Schur update), "trsm_winv" (0/1: row-block solve of a strip with 128 pivots as one tensor-core product with its explicit operator W),
  * "trsm_split" (0/1: under look-ahead that product runs on the next strip's columns first and on the rest beside the narrow update), "la_ctas" (SMs of the look-ahead strip kernel, 0 = cost model), "tc_min_k", "tc_min_mn",
  * "strip_width" (columns per cooperative strip kernel: 32..256, multiple of 32), "flat_cols" (nodes up to this many
- * columns are swept flat, wider ones recurse), "flat_group" (strips per Schur update of the flat sweep), "tc_panel" (0/1), "f64_mma" (fp64 trailing update: 1 = DMMA tensor pipe with 128 x 64 tiles, 2 = DMMA with 128 x 128 tiles, 0 = DFMA),
+ * columns are swept flat, wider ones recurse), "flat_group" (strips per Schur update of the flat sweep), "tc_panel" (0/1), "tc_panel_deep" (0/1: K <= 128 updates with one A stage and seven C-tile buffers), "f64_mma" (fp64 trailing update: 1 = DMMA tensor pipe with 128 x 64 tiles, 2 = DMMA with 128 x 128 tiles, 0 = DFMA),
  * "f64_strip" (fp64 factorisation: columns per strip of the flat top-level sweep, multiple of 32, 0 = pure recursion),
  * "f64_panel_threads" (256/512/1024) and "f64_panel_grid" (0 = one CTA per SM) of the fp64 panel kernel, "f64_panel_tags" (1 = tagged
  * candidate records instead of a grid barrier per column), "f64_panel_cluster" (CTAs of the cluster + DSMEM panel variant, 0 = off) with

@@ -204,6 +204,7 @@ constexpr int P_B_STAGE = 4 * PN * KB;       // 16384
 constexpr int P_C_TILE = TM * PN * 4;        // 16384
 constexpr int P_NAS = 2, P_NBS = 3, P_NCS = 3;
 constexpr int P_SMEM = P_NAS * P_A_STAGE + P_NBS * P_B_STAGE + P_NCS * P_C_TILE + 1024 + 256;
+static_assert(1 * P_A_STAGE + P_NBS * P_B_STAGE + 7 * P_C_TILE + 1024 + 256 == P_SMEM, "both stage configurations fill the same shared memory");
 constexpr int P_EPI_WARPS = 16;              // epilogue warps: 4 TMEM lane quarters x 4 groups of 8 columns
 constexpr int P_THREADS = 96 + 32 * P_EPI_WARPS;
 constexpr int P_PF = 6;                      // L2 prefetch distance for C tiles
@@ -237,25 +238,29 @@ __device__ __forceinline__ TileIter sc_init(const PanelSched& sc) {
     return it;
 }
 
-template <bool MONT>
+// NAS A stages and NCS C-tile buffers: (2, 3) serves any K <= 256; (1, 7) is the K <= 128 configuration -- one A stage is all a
+// single k-stage needs, and the shared memory it frees holds four more C tiles, so the C mover keeps six tile loads in flight
+// instead of two (the K = 128 update is bound by data movement: profiles/r02_experiments.md).
+template <bool MONT, int NAS, int NCS>
 __global__ void __launch_bounds__(P_THREADS, 1)
 gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                      const __grid_constant__ CUtensorMap tmC, int nks /* k-stages: kp / 128 */, PanelSched sc, ModP f) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     uint8_t* sA = smem;
-    uint8_t* sB = sA + P_NAS * P_A_STAGE;
+    uint8_t* sB = sA + NAS * P_A_STAGE;
     uint8_t* sC = sB + P_NBS * P_B_STAGE;
-    uint64_t* bars = (uint64_t*)(sC + P_NCS * P_C_TILE);
+    uint64_t* bars = (uint64_t*)(sC + NCS * P_C_TILE);
     uint64_t* a_full = bars;                 // [2]
     uint64_t* a_empty = bars + 2;            // [2]
     uint64_t* b_full = bars + 4;             // [4]
     uint64_t* b_empty = bars + 8;            // [4]
     uint64_t* acc_full = bars + 12;          // [2]
     uint64_t* acc_empty = bars + 14;         // [2]
-    uint64_t* c_full = bars + 16;            // [3]
-    uint64_t* c_done = bars + 19;            // [3]
-    uint32_t* tmem_holder = (uint32_t*)(bars + 22);
+    uint64_t* c_full = bars + 16;            // [NCS]
+    uint64_t* c_done = bars + 16 + NCS;      // [NCS]
+    uint32_t* tmem_holder = (uint32_t*)(bars + 16 + 2 * NCS);
+    static_assert((16 + 2 * NCS) * 8 + 4 <= 256, "the barrier block is 256 bytes");
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (warp == 0 && lane == 0) {
@@ -264,7 +269,7 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
         prefetch_tmap(&tmC);
         for (int i = 0; i < 2; ++i) { mbar_init(&a_full[i], 1); mbar_init(&a_empty[i], 1); mbar_init(&acc_full[i], 1);
                                       mbar_init(&acc_empty[i], P_EPI_WARPS); }
-        for (int i = 0; i < P_NCS; ++i) { mbar_init(&c_full[i], 1); mbar_init(&c_done[i], P_EPI_WARPS); }
+        for (int i = 0; i < NCS; ++i) { mbar_init(&c_full[i], 1); mbar_init(&c_done[i], P_EPI_WARPS); }
         for (int i = 0; i < P_NBS; ++i) { mbar_init(&b_full[i], 1); mbar_init(&b_empty[i], 1); }
         fence_barrier_init();
     }
@@ -282,8 +287,8 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             it.init(sc);
             while (it.valid) {
                 for (int ks = 0; ks < nks; ++ks, ++a_cnt) {
-                    const int s = a_cnt % P_NAS;
-                    mbar_wait(&a_empty[s], ((a_cnt / P_NAS) & 1) ^ 1);
+                    const int s = a_cnt % NAS;
+                    mbar_wait(&a_empty[s], ((a_cnt / NAS) & 1) ^ 1);
                     mbar_expect_tx(&a_full[s], P_A_STAGE);
                     tma_load_3d(sA + s * P_A_STAGE, &tmA, &a_full[s], ks * KB, it.mt * TM, 0);
                 }
@@ -309,9 +314,9 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
         constexpr uint32_t id128 = make_idesc_i8(4 * PN), id96 = make_idesc_i8(3 * PN), id32 = make_idesc_i8(PN);
         constexpr uint64_t LIMB = (uint64_t)((TM * KB) >> 4);          // descriptor step between A limb planes
         constexpr uint64_t KSTEP = 32 >> 4;                            // descriptor step of one 32-byte k slice
-        uint64_t adesc[P_NAS], bdesc[P_NBS];
+        uint64_t adesc[2], bdesc[P_NBS];
 #pragma unroll
-        for (int i = 0; i < P_NAS; ++i) adesc[i] = make_desc_sw128(smem_u32(sA + i * P_A_STAGE));
+        for (int i = 0; i < 2; ++i) adesc[i] = make_desc_sw128(smem_u32(sA + (i % NAS) * P_A_STAGE));
 #pragma unroll
         for (int i = 0; i < P_NBS; ++i) bdesc[i] = make_desc_sw128(smem_u32(sB + i * P_B_STAGE));
         uint32_t a_cnt = 0, b_cnt = 0, t_cnt = 0;
@@ -327,8 +332,8 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                 const bool last = it.last_of_item();
                 for (int ks = 0; ks < nks; ++ks, ++b_cnt) {
                     const uint32_t ac = a_cnt + ks;
-                    const int sa = ac % P_NAS;
-                    if (first_tile) mbar_wait(&a_full[sa], (ac / P_NAS) & 1);
+                    const int sa = ac % NAS;
+                    if (first_tile) mbar_wait(&a_full[sa], (ac / NAS) & 1);
                     const int sb = b_cnt % P_NBS;
                     mbar_wait(&b_full[sb], (b_cnt / P_NBS) & 1);
                     tc_fence_after();
@@ -360,29 +365,29 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             a_cnt += nks;
         }
     } else if (warp == 2) {
-        // C mover: TMA loads of the C tiles two tiles ahead (three buffers), L2 prefetch P_PF tiles ahead
+        // C mover: TMA loads of the C tiles NCS - 1 tiles ahead, L2 prefetch further ahead
         // (the trailing matrix is far larger than L2), TMA stores once the epilogue warps are done with a tile.
         if (lane == 0) {
             TileIter ld = sc_init(sc), pf = ld, st = ld;
             uint32_t l_cnt = 0, t_cnt = 0;
-            for (int i = 0; i < P_PF && pf.valid; ++i) pf.next(sc);
-            for (int i = 0; i < 2 && ld.valid; ++i, ++l_cnt) {
-                mbar_expect_tx(&c_full[l_cnt % P_NCS], P_C_TILE);
-                tma_load_2d(sC + (l_cnt % P_NCS) * P_C_TILE, &tmC, &c_full[l_cnt % P_NCS], ld.nt * PN, ld.mt * TM);
+            for (int i = 0; i < P_PF + NCS - 3 && pf.valid; ++i) pf.next(sc);
+            for (int i = 0; i < NCS - 1 && ld.valid; ++i, ++l_cnt) {
+                mbar_expect_tx(&c_full[l_cnt % NCS], P_C_TILE);
+                tma_load_2d(sC + (l_cnt % NCS) * P_C_TILE, &tmC, &c_full[l_cnt % NCS], ld.nt * PN, ld.mt * TM);
                 ld.next(sc);
             }
             while (st.valid) {
-                const uint32_t cb = t_cnt % P_NCS;
+                const uint32_t cb = t_cnt % NCS;
                 if (pf.valid) { tma_prefetch_l2_2d(&tmC, pf.nt * PN, pf.mt * TM); pf.next(sc); }
-                mbar_wait(&c_done[cb], (t_cnt / P_NCS) & 1);
+                mbar_wait(&c_done[cb], (t_cnt / NCS) & 1);
                 tma_store_2d(&tmC, sC + cb * P_C_TILE, st.nt * PN, st.mt * TM);
                 tma_store_commit();
                 st.next(sc);
                 ++t_cnt;
                 if (ld.valid) {
-                    // buffer of tile t+2 == buffer of tile t-1, whose store was committed one iteration ago
+                    // buffer of tile t + NCS - 1 == buffer of tile t - 1, whose store was committed one iteration ago
                     tma_store_wait_read1();
-                    const uint32_t lb = l_cnt % P_NCS;
+                    const uint32_t lb = l_cnt % NCS;
                     mbar_expect_tx(&c_full[lb], P_C_TILE);
                     tma_load_2d(sC + lb * P_C_TILE, &tmC, &c_full[lb], ld.nt * PN, ld.mt * TM);
                     ld.next(sc);
@@ -398,7 +403,7 @@ gemm_tc_panel_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
         TileIter it = sc_init(sc);
         while (it.valid) {
             const uint32_t buf = t_cnt & 1, ph = (t_cnt >> 1) & 1;
-            const uint32_t cb = t_cnt % P_NCS, cph = (t_cnt / P_NCS) & 1;
+            const uint32_t cb = t_cnt % NCS, cph = (t_cnt / NCS) & 1;
             it.next(sc);
             mbar_wait(&acc_full[buf], ph);
             tc_fence_after();
@@ -578,8 +583,10 @@ int gemm_modp_tc(const GemmArgs& g, const ModP& f, cudaStream_t s, Arena* scratc
     static PerDeviceOnce attr_once;
     if (attr_once.run([]() -> int {
             if (cudaFuncSetAttribute(gemm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES) != cudaSuccess ||
-                cudaFuncSetAttribute(gemm_tc_panel_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM) != cudaSuccess ||
-                cudaFuncSetAttribute(gemm_tc_panel_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM) != cudaSuccess) {
+                cudaFuncSetAttribute(gemm_tc_panel_kernel<true, 2, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM) != cudaSuccess ||
+                cudaFuncSetAttribute(gemm_tc_panel_kernel<false, 2, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM) != cudaSuccess ||
+                cudaFuncSetAttribute(gemm_tc_panel_kernel<true, 1, 7>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM) != cudaSuccess ||
+                cudaFuncSetAttribute(gemm_tc_panel_kernel<false, 1, 7>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM) != cudaSuccess) {
                 cudaGetLastError();
                 return LINAC_ERR_CUDA;
             }
@@ -614,26 +621,24 @@ int gemm_modp_tc(const GemmArgs& g, const ModP& f, cudaStream_t s, Arena* scratc
             return -1;
         const int grid = g.grid_limit > 0 ? std::min(g.grid_limit, sm_count()) : sm_count();
         const PanelSched sc = make_sched(g.M, g.N, grid);
-        if (g.pdl) {
-            // programmatic dependent launch behind the kernel that produced B (the caller vouches that this kernel wrote
-            // neither A nor C): the prologue and the A / C loads overlap that kernel's tail
-            cudaLaunchConfig_t cfg = {};
-            cfg.gridDim = dim3((unsigned)std::min(grid, sc.nitems));
-            cfg.blockDim = dim3(P_THREADS);
-            cfg.dynamicSmemBytes = P_SMEM;
-            cfg.stream = s;
-            cudaLaunchAttribute at[1];
-            at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-            at[0].val.programmaticStreamSerializationAllowed = 1;
-            cfg.attrs = at;
-            cfg.numAttrs = 1;
-            const int nks = (int)(kp / KB);
-            if (f.ninv) LINAC_CUDA(cudaLaunchKernelEx(&cfg, gemm_tc_panel_kernel<true>, tmA, tmB, tmC, nks, sc, f));
-            else LINAC_CUDA(cudaLaunchKernelEx(&cfg, gemm_tc_panel_kernel<false>, tmA, tmB, tmC, nks, sc, f));
-        } else if (f.ninv)
-            gemm_tc_panel_kernel<true><<<(unsigned)std::min(grid, sc.nitems), P_THREADS, P_SMEM, s>>>(tmA, tmB, tmC, (int)(kp / KB), sc, f);
-        else
-            gemm_tc_panel_kernel<false><<<(unsigned)std::min(grid, sc.nitems), P_THREADS, P_SMEM, s>>>(tmA, tmB, tmC, (int)(kp / KB), sc, f);
+        const int nks = (int)(kp / KB);
+        const bool deep = nks == 1 && options().tc_panel_deep != 0;     // K <= 128: one A stage, seven C buffers
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)std::min(grid, sc.nitems));
+        cfg.blockDim = dim3(P_THREADS);
+        cfg.dynamicSmemBytes = P_SMEM;
+        cfg.stream = s;
+        // programmatic dependent launch behind the kernel that produced B (the caller vouches that this kernel wrote
+        // neither A nor C): the prologue and the A / C loads overlap that kernel's tail
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = g.pdl ? 1 : 0;
+        if (f.ninv && deep) LINAC_CUDA(cudaLaunchKernelEx(&cfg, gemm_tc_panel_kernel<true, 1, 7>, tmA, tmB, tmC, nks, sc, f));
+        else if (f.ninv) LINAC_CUDA(cudaLaunchKernelEx(&cfg, gemm_tc_panel_kernel<true, 2, 3>, tmA, tmB, tmC, nks, sc, f));
+        else if (deep) LINAC_CUDA(cudaLaunchKernelEx(&cfg, gemm_tc_panel_kernel<false, 1, 7>, tmA, tmB, tmC, nks, sc, f));
+        else LINAC_CUDA(cudaLaunchKernelEx(&cfg, gemm_tc_panel_kernel<false, 2, 3>, tmA, tmB, tmC, nks, sc, f));
         LINAC_CUDA(cudaGetLastError());
         stats().kernel_launches += 1;
         stats().tc_launches++;

@@ -280,6 +280,9 @@ int linac_set_option(const char* name, int64_t value) {
     } else if (!strcmp(name, "f64_rhs_inv")) {
         if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
         g_options.f64_rhs_inv = value;
+    } else if (!strcmp(name, "tc_panel_deep")) {
+        if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
+        g_options.tc_panel_deep = value;
     } else if (!strcmp(name, "tc_panel")) {
         if (value < 0 || value > 1) return LINAC_ERR_INVALID_ARG;
         g_options.tc_panel = value;

@@ -52,6 +52,7 @@ struct Options {
     int64_t f64_rref_strip = 128;     // linac_rref_f64: columns per strip (the K of the update right of the strip); 32 = every panel updates everything
     int64_t f64_panel_tags = 1;       // fp64 panel: 1 = tagged candidate records replace the per-column grid barrier, 0 = grid.sync
     int64_t f64_rhs_inv = 1;  // fp64 substitution on B: 1 = blocked with inverted diagonal blocks, 0 = recursive leaf solves
+    int64_t tc_panel_deep = 1; // K <= 128 updates: one A stage and seven C-tile buffers (six tile loads in flight) instead of two and three
     int64_t tc_panel = 1;     // 1 = K <= 256 updates use the persistent A-stationary tensor kernel
     int64_t flat_cols = 16384; // nodes of at most this many columns are swept flat (right-looking), wider ones recurse
     int64_t flat_group = 1;   // strips per Schur update of the flat sweep (K = flat_group * strip_width)
