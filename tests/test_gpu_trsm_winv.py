@@ -35,7 +35,7 @@ def _run(a, p, ld=None, **opts):
         return gpu_rref(a, p, ld)
     finally:
         for k in opts:
-            L.set_option(k, {"trsm_winv": 1, "la_ctas": 0, "lookahead": 1}[k])
+            L.set_option(k, {"trsm_winv": 1, "la_ctas": 0, "lookahead": 1, "trsm_split": 1, "pdl": 1, "tc_panel_deep": 1}[k])
 
 
 @pytest.mark.parametrize("p", [P31, P29, 3, 2])
@@ -81,3 +81,22 @@ def test_regular_strips_that_exchange_rows(oracle, p, la_ctas):
     assert st["row_swaps"] > 100
     assert st["winv_solves"] >= 10
     assert (st["lookahead_strips"] > 5) == (la_ctas == 40)
+
+
+@pytest.fixture(scope="module")
+def forked_case(oracle):
+    """2304 x 2500 dense over F_{2^31-1}, its oracle RREF computed once for the option sweep below."""
+    a = gen.uniform_matrix(2304, 2500, P31, seed=91)
+    return a, oracle.rref_modp(a, P31, nthreads=oracle.max_threads())
+
+
+@pytest.mark.parametrize("opts", [{"trsm_split": 0}, {"pdl": 0}, {"tc_panel_deep": 0}, {"trsm_split": 0, "pdl": 0, "tc_panel_deep": 0},
+                                  {"lookahead": 0}])
+def test_schedule_options_of_the_forked_sweep_keep_the_bytes(forked_case, opts):
+    """The split of the W product over two streams, the programmatic dependent launch of the updates behind it and the
+    deep C-tile ring of the K = 128 update only change the schedule; with a forced partition every strip is forked."""
+    a, (r_ref, rank_ref, piv_ref) = forked_case
+    out, rank, piv, st = _run(a, P31, la_ctas=40, **opts)
+    assert rank == rank_ref and np.array_equal(piv, piv_ref)
+    assert np.array_equal(out, r_ref)
+    assert (st["lookahead_strips"] > 5) == (opts.get("lookahead", 1) == 1)
