@@ -1,6 +1,8 @@
 """linac_gemm_sub_u32_static: the entry point that allocates no device memory (scratch in the library's static
 32 MiB device array) against the existing linac_gemm_sub_u32, bit for bit -- integer work, so the tolerance is
 equality, as in tests/test_gpu_gemm.py -- on calls in a row that share the array.  This file sorts last on purpose."""
+import gc
+
 import numpy as np
 import pytest
 import torch
@@ -42,13 +44,15 @@ def test_two_calls_in_a_row_match_the_existing_path_without_allocating():
     tiny = torch.zeros((8, 8), dtype=torch.int32, device="cuda")
     L.gemm_sub_u32_static(tiny, tiny.clone(), tiny.clone(), P31)      # set-up: the module with the array is loaded here
     torch.cuda.synchronize()
+    gc.collect()                                                       # tensors of earlier tests still waiting in reference cycles go now,
+    torch.cuda.synchronize()                                           # not in the middle of the measurement below
     before = torch.cuda.memory_allocated()
     free_before, _ = torch.cuda.mem_get_info()
     for t in dev:                                                      # back to back on one stream, no sync between
         L.gemm_sub_u32_static(*t)
     torch.cuda.synchronize()
     free_after, _ = torch.cuda.mem_get_info()
-    assert torch.cuda.memory_allocated() == before
+    assert torch.cuda.memory_allocated() <= before                     # the binding made no tensor (a collection may still free one)
     assert free_after >= free_before, "device memory was allocated inside the no-allocation entry point"
     for t, want in zip(dev, ref):
         assert np.array_equal(from_device(t[0]), want)
