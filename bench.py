@@ -664,6 +664,9 @@ def main():
                          "and print {\"gemm\": ...}; the command of the GEMM ncu captures under profiles/")
     ap.add_argument("--load-matrix", default=None, metavar="ROWS,COLS,D",
                     help="time linac_load_matrix_u32 alone (SURVEY.md 8(f)#2) and print {\"load_matrix\": ...}")
+    ap.add_argument("--timeline", default=None, metavar="N",
+                    help="one linac_rref_u32 call on an N x N dense matrix with option timing = 2 and print its per-launch intervals "
+                         "(linac_get_last_marks) as a table: which strip kernel ran beside which update (profiles/r02_lookahead.md)")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
                     help="library tunable for A/B runs (linac_set_option), e.g. --opt strip_width=256")
     args = ap.parse_args()
@@ -687,6 +690,25 @@ def main():
         name, _, val = kv.partition("=")
         L.set_option(name, int(val))
     B = Bench(torch, L, dev, local, world, rank, args.opt)
+    if args.timeline:
+        n = int(args.timeline)
+        p = 2147483647
+        from linac_inputs import gen_torch
+        a0 = gen_torch.uniform_rows(0, n, n, p, 3, dev)
+        L.set_option("timing", 2)
+        for _ in range(3):                                   # the last call's marks are the ones printed
+            a = a0.clone()
+            rk, _ = L.rref_u32(a, p)
+        L.set_option("timing", 0)
+        marks = sorted(L.last_marks(), key=lambda mk: mk["t0_ms"])
+        names = {0: "update", 1: "strip", 2: "solve"}
+        print(f"# linac_rref_u32 {n} x {n}, p = {p}, rank {rk}: {len(marks)} launches, call {L.last_stats()['ms_total']:.3f} ms (with the event marks)")
+        print("# start_us end_us dur_us class stream shape(update: M N K)")
+        for mk in marks:
+            shape = f"{mk['m']} {mk['n']} {mk['k']}" if mk["cls"] == 0 else ""
+            print(f"{mk['t0_ms'] * 1e3:9.1f} {mk['t1_ms'] * 1e3:9.1f} {(mk['t1_ms'] - mk['t0_ms']) * 1e3:7.1f} {names[mk['cls']]:6s} "
+                  f"{'second' if mk['stream'] else 'call'  :6s} {shape}")
+        return
     if args.gemm:
         parts = [int(x) for x in args.gemm.split(",")]
         m, n, k = parts[:3]

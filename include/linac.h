@@ -280,6 +280,18 @@ typedef struct {
     int64_t winv_solves;         /* row-block solves done as one product with the strip's 128 x 128 operator W       */
 } linac_stats;
 int linac_get_last_stats(linac_stats *out);
+/* Timeline of the calling thread's last linac_rref_u32 call made with option "timing" = 2: one record per kernel launch
+ * of the three classes, in launch order, times in ms from the start of the call (CUDA events around each launch, read
+ * after the call's final synchronisation).  cls: 0 = Schur update, 1 = strip kernel, 2 = row-block solve (W kernel, W
+ * product, chain kernel); stream: 0 = the call's stream, 1 = the look-ahead sweep's second stream; m, n, k: shape of an
+ * update (0 otherwise).  Writes at most `capacity` records to `out` (may be NULL with capacity 0) and the number
+ * available to *count.  What it is for: seeing which launches overlap (profiles/r02_lookahead.md). */
+typedef struct {
+    int32_t cls, stream;
+    int64_t m, n, k;
+    float t0_ms, t1_ms;
+} linac_mark;
+int linac_get_last_marks(linac_mark *out, int64_t capacity, int64_t *count);
 /* Tunables, mainly for A/B measurements: name in {"gemm_path" (0 auto, 1 CUDA-core, 2 tensor), "timing" (0, 1 = un-fused schedule with a
  * host sync per launch, 2 = event pairs around every launch of the production schedule), "lookahead" (0/1: factor strip s+1 beside the bulk
  * of strip s's Schur update), "trsm_winv" (0/1: row-block solve of a strip with 128 pivots as one tensor-core product with its explicit operator W),

@@ -797,6 +797,14 @@ int rref_impl(uint32_t* dA, int64_t rows, int64_t cols, int64_t ld, uint32_t p, 
             } else if (mk.cls == 1) st.ms_strip += t;
             else st.ms_trsm += t;
         }
+        cx.marks.clear();
+        for (const Fp::Mark& mk : c.marks) {
+            linac_mark m{};
+            m.cls = mk.cls; m.stream = mk.on == c.s ? 0 : 1; m.m = mk.m; m.n = mk.n; m.k = mk.k;
+            if (cudaEventElapsedTime(&m.t0_ms, t0, event_pool[mk.ev]) != cudaSuccess ||
+                cudaEventElapsedTime(&m.t1_ms, t0, event_pool[mk.ev + 1]) != cudaSuccess) continue;
+            cx.marks.push_back(m);
+        }
         double ov = 0;                                         // a strip kernel and an update kernel in flight together
         for (const auto& a : iv_strip)
             for (const auto& b : iv_update) ov += std::max(0.f, std::min(a.second, b.second) - std::max(a.first, b.first));

@@ -238,6 +238,14 @@ int linac_get_last_stats(linac_stats* out) {
     return LINAC_OK;
 }
 
+int linac_get_last_marks(linac_mark* out, int64_t capacity, int64_t* count) {
+    if (!count || capacity < 0 || (capacity > 0 && !out)) return LINAC_ERR_INVALID_ARG;
+    const std::vector<linac_mark>& mk = ctx().marks;
+    *count = (int64_t)mk.size();
+    for (int64_t i = 0; i < capacity && i < (int64_t)mk.size(); ++i) out[i] = mk[(size_t)i];
+    return LINAC_OK;
+}
+
 int linac_set_option(const char* name, int64_t value) {
     if (!name) return LINAC_ERR_INVALID_ARG;
     std::lock_guard<std::mutex> lock(g_init_mutex);

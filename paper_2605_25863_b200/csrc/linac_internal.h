@@ -80,6 +80,7 @@ struct Context {
     unsigned long long* mail = nullptr;       // mapped pinned host memory (strip records), allocated on first use
     unsigned long long seq = 0;               // tag of the last strip launch
     std::vector<cudaEvent_t> events;          // pool for the timing modes
+    std::vector<linac_mark> marks;            // timing = 2: per-launch intervals of the thread's last F_p call
     int slot = -1;                            // index into the __constant__ ModP table of fp_strip.cuh
     cudaStream_t la_stream = nullptr;         // second stream of the look-ahead schedule (created on first use)
     cudaEvent_t la_ev[4] = {nullptr, nullptr, nullptr, nullptr};

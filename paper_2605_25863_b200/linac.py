@@ -27,7 +27,7 @@ SYMBOLS = [
     "linac_rref_u32", "linac_nullspace_u32", "linac_nullspace_from_rref_u32", "linac_solve_u32", "linac_rank_factor_u32", "linac_load_matrix_u32", "linac_gemm_sub_u32",
     "linac_gemm_sub_u32_static",
     "linac_solve_f64", "linac_rref_f64_workspace", "linac_rref_f64", "linac_rref_c128_workspace", "linac_rref_c128",
-    "linac_get_last_stats", "linac_set_option", "linac_measure_peak",
+    "linac_get_last_stats", "linac_get_last_marks", "linac_set_option", "linac_measure_peak",
 ]
 
 
@@ -87,6 +87,7 @@ def _lib() -> C.CDLL:
         L.linac_rref_c128.argtypes = [vp, i64, i64, i64, C.c_double, vp, C.POINTER(i64), vp]
         L.linac_measure_peak.argtypes = [C.c_char_p, C.c_double, vp, sz, vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.linac_get_last_stats.argtypes = [C.POINTER(Stats)]
+        L.linac_get_last_marks.argtypes = [C.POINTER(Mark), i64, C.POINTER(i64)]
         L.linac_set_option.argtypes = [C.c_char_p, i64]
         _LIB = L
     return _LIB
@@ -100,6 +101,21 @@ def set_option(name: str, value: int) -> None:
     rc = _lib().linac_set_option(name.encode(), int(value))
     if rc:
         raise LinacError(rc, f"linac_set_option({name})")
+
+
+class Mark(C.Structure):
+    _fields_ = [("cls", C.c_int32), ("stream", C.c_int32), ("m", C.c_int64), ("n", C.c_int64), ("k", C.c_int64),
+                ("t0_ms", C.c_float), ("t1_ms", C.c_float)]
+
+
+def last_marks() -> list:
+    """Per-launch intervals of this thread's last rref_u32 call made with set_option("timing", 2) (mirrors
+    linac_get_last_marks): dicts with cls (0 update, 1 strip kernel, 2 row-block solve), stream, m, n, k, t0_ms, t1_ms."""
+    n = C.c_int64(0)
+    _lib().linac_get_last_marks(None, 0, C.byref(n))
+    buf = (Mark * max(1, n.value))()
+    _lib().linac_get_last_marks(buf, n.value, C.byref(n))
+    return [{k: getattr(buf[i], k) for k, _ in Mark._fields_} for i in range(n.value)]
 
 
 def last_stats() -> dict:

@@ -45,3 +45,29 @@ def test_timing_mode_2_keeps_the_result_and_accounts_for_the_step(oracle):
     assert st["ms_update"] > 0 and st["ms_strip"] > 0 and st["ms_trsm"] > 0
     assert parts <= st["ms_total"] * 1.02 + 0.05                  # the classes are disjoint launches of one stream
     assert st["top_k"] > 0 and st["ms_update_top"] > 0
+
+
+def test_marks_of_a_timed_call_cover_its_launches_and_show_the_overlap():
+    """linac_get_last_marks: with timing = 2 every strip / update / solve launch of the call has an interval inside the call,
+    and under look-ahead some strip kernel runs while an update on the second stream is in flight."""
+    require_cuda()
+    import paper_2605_25863_b200 as L
+    import linac_inputs as gen
+    p = 2147483647
+    a = torch.from_numpy(gen.uniform_matrix(2304, 2304, p, seed=5).view(np.int32)).cuda()
+    try:
+        L.set_option("timing", 2)
+        L.set_option("la_ctas", 40)
+        rank, _ = L.rref_u32(a, p)
+    finally:
+        L.set_option("timing", 0)
+        L.set_option("la_ctas", 0)
+    st, marks = L.last_stats(), L.last_marks()
+    assert rank == 2304 and st["lookahead_strips"] > 5
+    assert len(marks) >= 4 * 18 - 8 and {m["cls"] for m in marks} == {0, 1, 2}
+    assert all(0.0 <= m["t0_ms"] <= m["t1_ms"] <= st["ms_total"] + 1e-3 for m in marks)
+    strips = [m for m in marks if m["cls"] == 1]
+    bulk = [m for m in marks if m["cls"] == 0 and m["stream"] == 1]
+    assert bulk and any(min(s["t1_ms"], b["t1_ms"]) > max(s["t0_ms"], b["t0_ms"]) for s in strips for b in bulk)
+    L.set_option("timing", 0)
+    L.rref_u32(torch.from_numpy(gen.uniform_matrix(64, 64, p, seed=6).view(np.int32)).cuda(), p)
