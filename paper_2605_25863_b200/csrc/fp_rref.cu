@@ -136,8 +136,8 @@ int trsm_leaf(Fp& c, int64_t s, uint32_t* X, int64_t ldx, int64_t ncols) {
         for (int64_t b = c.sb0(s); b < c.sb0(s + 1); ++b) regular = regular && c.pstart[b + 1] - c.pstart[b] == PW;
         if (regular) {
             uint8_t* W = c.d_W + (size_t)((c.winv_count++) & 1) * W_A_BYTES;
-            strip_winv_kernel<<<WINV_CTAS, WINV_NT, sizeof(WinvSmem), c.s>>>(c.A, c.ld, c.d_pstart, (int)c.sb0(s), c.d_T, c.d_pivcols,
-                                                                             c.f, W);
+            strip_winv_kernel<<<WINV_CTAS, WINV_NT, sizeof(WinvSmem), c.s>>>(c.A, c.ld, c.d_pstart, (int)c.sb0(s), c.d_T,
+                                                                             (int)c.sp(s), c.f, W);
             LINAC_CUDA(cudaGetLastError());
             const int64_t ntiles = (ncols + WTN - 1) / WTN;
             trsm_winv_kernel<<<(unsigned)std::min<int64_t>(ntiles, 2 * sm_count()), WNT, WTRSM_SMEM, c.s>>>(
@@ -260,11 +260,11 @@ int collect_strip(Fp& c, StripLaunch& L, int64_t i0, int64_t* r) {
 }
 
 // Enqueues strip_winv_kernel behind a strip kernel: W = the strip's solve operator, if the strip turns out regular.
-int launch_winv(Fp& c, StripLaunch& L, cudaStream_t stream) {
-    if (options().trsm_winv == 0 || c.d_W == nullptr || L.b1 - L.b0 != WK / PW || L.j1 - L.j0 != WK) return LINAC_OK;
+int launch_winv(Fp& c, StripLaunch& L, cudaStream_t stream, int64_t i0) {
+    if (options().trsm_winv == 0 || c.d_W == nullptr || L.b1 - L.b0 != WK / PW || L.j1 - L.j0 != WK || i0 + WK > c.rows) return LINAC_OK;
     Timed tm(c, stats().ms_trsm, 2, stream);
     L.W = c.d_W + (size_t)((c.winv_count++) & 1) * W_A_BYTES;
-    strip_winv_kernel<<<WINV_CTAS, WINV_NT, sizeof(WinvSmem), stream>>>(c.A, c.ld, c.d_pstart, (int)L.b0, c.d_T, c.d_pivcols, c.f, L.W);
+    strip_winv_kernel<<<WINV_CTAS, WINV_NT, sizeof(WinvSmem), stream>>>(c.A, c.ld, c.d_pstart, (int)L.b0, c.d_T, (int)i0, c.f, L.W);
     LINAC_CUDA(cudaGetLastError());
     stats().kernel_launches++;
     L.winv = true;
@@ -375,7 +375,7 @@ int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jen
     bool la_launched = false;                                  // was the strip in L launched as a look-ahead strip?
     int rc = launch_strip(c, s0, cur, c.s, c.coop_grid, false, true, Aq[s0 & 1], kp, &L);
     if (rc) return rc;
-    rc = launch_winv(c, L, c.s);
+    rc = launch_winv(c, L, c.s, cur);
     if (rc) return rc;
     int64_t r = 0;
     rc = collect_strip(c, L, cur, &r);
@@ -452,7 +452,7 @@ int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jen
                 LINAC_CUDA(cudaEventRecord(ev_narrow, c.s));
                 rc = launch_strip(c, s + 1, cur + r, c.s, la_grid, true, true, Aq[(s + 1) & 1], kp, &Ln);
                 if (rc) return rc;
-                rc = launch_winv(c, Ln, c.s);                                       // needs the strip's own columns only
+                rc = launch_winv(c, Ln, c.s, cur + r);                              // needs the strip's own columns only
                 if (rc) return rc;
                 next_launched = true;
                 stats().lookahead_strips++;
@@ -481,7 +481,7 @@ int factor_flat_lookahead(Fp& c, int64_t s0, int64_t s1, int64_t i0, int64_t jen
         if (!next_launched) {
             rc = launch_strip(c, s + 1, cur, c.s, c.coop_grid, false, true, Aq[(s + 1) & 1], kp, &Ln);
             if (rc) return rc;
-            rc = launch_winv(c, Ln, c.s);
+            rc = launch_winv(c, Ln, c.s, cur);
             if (rc) return rc;
         }
         rc = collect_strip(c, Ln, cur, &r);

@@ -47,14 +47,17 @@ __device__ __forceinline__ void winv_dot(uint64_t& a0, uint64_t& a1, const uint3
 // up to 40 -- are all in flight together instead of one load-then-store after the other), columns j0..j0+7 of it.
 template <int C>
 __device__ __forceinline__ void winv_body(WinvSmem& sm, const uint32_t* __restrict__ A, int64_t ld, int t0, int b0, int j0,
-                                          const uint32_t* __restrict__ T, const int32_t* __restrict__ pivcols,
+                                          const uint32_t* __restrict__ T, int64_t jstrip, const int32_t* __restrict__ pstart,
                                           const ModP& f, uint8_t* __restrict__ Wq) {
     const int tid = threadIdx.x;
     constexpr int NQ = PW * PW / WINV_NT;                        // elements of a 32 x 32 block per thread
     const int kk = tid % PW, i0 = tid / PW;                      // element q of the thread: (row i0 + 8 q, column kk)
-    int32_t pc[4];
+    // a base panel that found 32 pivots in its 32 columns has every column as a pivot column, in order: pivot 32 d + k of
+    // a regular strip sits in column jstrip + 32 d + k, so no load here waits for another (the pivot-column list and the
+    // pivot counts are only needed to CONFIRM that the strip is regular, below, beside these loads)
+    int64_t pc[4];
 #pragma unroll
-    for (int d = C; d < 3; ++d) pc[d] = pivcols[t0 + PW * d + kk];
+    for (int d = C; d < 3; ++d) pc[d] = jstrip + PW * d + kk;
     uint32_t tv[4][NQ], lv[6][NQ];
 #pragma unroll
     for (int q = 0; q < NQ; ++q) {
@@ -75,6 +78,10 @@ __device__ __forceinline__ void winv_body(WinvSmem& sm, const uint32_t* __restri
 #pragma unroll
             for (int d = C; d < b; ++d) sm.Ls[b * (b - 1) / 2 + d][ii][kk] = lv[b * (b - 1) / 2 + d][q];
         }
+    }
+    {
+        const int p0 = pstart[b0], p1 = pstart[b0 + 1], p2 = pstart[b0 + 2], p3 = pstart[b0 + 3], p4 = pstart[b0 + 4];
+        if (p0 != t0 || p1 - p0 != PW || p2 - p1 != PW || p3 - p2 != PW || p4 - p3 != PW) return;    // uniform over the CTA
     }
     __syncthreads();
     const int i = tid / 8, jj = tid % 8;
@@ -104,26 +111,25 @@ __device__ __forceinline__ void winv_body(WinvSmem& sm, const uint32_t* __restri
     }
 }
 
-// W for the strip whose first base panel is b0 and whose pivots start at row / pivot index pstart[b0], as the
+// W for the strip whose first base panel is b0 and whose pivots start at row / pivot index t0 (= pstart[b0]), as the
 // shared-memory image of a K-major tcgen05 operand: Wq[limb][m][128 bytes of k], the 16-byte pieces of a row XOR-ed
 // with m % 8 (SWIZZLE_128B).  The blocks above the diagonal are written as zeros.  Exits without writing when the strip
 // is not regular (the host takes the chain kernel then).
 __global__ void __launch_bounds__(WINV_NT) strip_winv_kernel(const uint32_t* __restrict__ A, int64_t ld,
                                                             const int32_t* __restrict__ pstart, int b0,
-                                                            const uint32_t* __restrict__ T,
-                                                            const int32_t* __restrict__ pivcols, ModP f,
+                                                            const uint32_t* __restrict__ T, int t0, ModP f,
                                                             uint8_t* __restrict__ Wq) {
     extern __shared__ __align__(16) unsigned char winv_smem_raw[];
     WinvSmem& sm = *reinterpret_cast<WinvSmem*>(winv_smem_raw);
-    const int t0 = pstart[b0];
-    const int t4 = pstart[b0 + 4], t1 = pstart[b0 + 1], t2 = pstart[b0 + 2], t3 = pstart[b0 + 3];
-    if (t1 - t0 != PW || t2 - t1 != PW || t3 - t2 != PW || t4 - t3 != PW) return;
+    // t0 = first pivot row of the strip, from the host (it launched the strip kernel with it); the rows t0 .. t0 + 127
+    // exist (the host checks).  Whether the strip IS regular is confirmed inside winv_body, beside the loads.
     const int j0 = 8 * (blockIdx.x % 4);                         // first of this CTA's columns inside the block
+    const int64_t jstrip = (int64_t)b0 * PW;
     switch (blockIdx.x / 4) {                                    // column block of W
-        case 0: winv_body<0>(sm, A, ld, t0, b0, j0, T, pivcols, f, Wq); break;
-        case 1: winv_body<1>(sm, A, ld, t0, b0, j0, T, pivcols, f, Wq); break;
-        case 2: winv_body<2>(sm, A, ld, t0, b0, j0, T, pivcols, f, Wq); break;
-        default: winv_body<3>(sm, A, ld, t0, b0, j0, T, pivcols, f, Wq); break;
+        case 0: winv_body<0>(sm, A, ld, t0, b0, j0, T, jstrip, pstart, f, Wq); break;
+        case 1: winv_body<1>(sm, A, ld, t0, b0, j0, T, jstrip, pstart, f, Wq); break;
+        case 2: winv_body<2>(sm, A, ld, t0, b0, j0, T, jstrip, pstart, f, Wq); break;
+        default: winv_body<3>(sm, A, ld, t0, b0, j0, T, jstrip, pstart, f, Wq); break;
     }
 }
 
